@@ -1,0 +1,148 @@
+/*
+ * scatman.h -- C ABI of libscatman: B200-native (sm_100a) MSFT forward simulation.
+ *
+ * The method: "The Scatman", arXiv 2202.03411 (reference text: PAPER.md), Multi-Slice Fourier
+ * Transform.  For every detector pixel p with Ewald-sphere momentum transfer q(p) (Eq. 3,
+ * PAPER.md:80-83) the library evaluates directly
+ *
+ *     A(p) = sum_j e^{i qz z_j} sum_{x,y} rho~_j(x,y) e^{i (qx x + qy y)}        (Eq. 2/4)
+ *     rho~_j = f(dn_j) exp(i k dz sum_{l<j} dn_l) dV,  dn = delta + i beta         (Eq. 6-9)
+ *     I(p) = |A(p)|^2                                                             (Block 11)
+ *
+ * in the sign convention of BASELINE.json's north_star (the complex conjugate of the paper's;
+ * same intensity, reading R3).
+ *
+ * Conventions common to every entry point
+ *   - Pointers named d_* are DEVICE pointers (16-byte aligned), h_* are HOST pointers.
+ *   - The caller owns every device buffer, including the workspace; the library allocates no
+ *     device memory in the d_* entry points.  Inputs are never modified.
+ *   - All device work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  No host synchronisation happens unless stated.
+ *   - Every function returns a scatman_status.  No exceptions, no abort, NO CPU FALLBACK: without a
+ *     compute-capability 10.x device scatman_create fails with SCATMAN_UNSUPPORTED_DEVICE.
+ *   - Device data are not validated (no NaN / range checks).
+ *   - Lengths (voxel size, lambda) share one arbitrary unit; k = 2 pi / lambda.
+ *   - Grid layout: dn[b][iz][iy][ix][2] = (delta, beta) FP32 in the paper's sense (n = 1 - delta + i beta,
+ *     Eq. 7), ix fastest, z = beam axis, slice iz = 0 is hit first.  Voxel centres at
+ *     x_i = (i - (nx-1)/2) dx etc. (R6).  One slice per z-layer, slice thickness dz (R8).
+ *   - Output: I[b][iy][ix] FP32 (ix fastest), units length^6 (dV^2 scale, R1).
+ */
+#ifndef SCATMAN_H_
+#define SCATMAN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct scatman_ctx scatman_ctx; /* opaque; one per device; not thread-safe */
+
+typedef enum {
+    SCATMAN_OK = 0,
+    SCATMAN_INVALID_ARGUMENT = 1,   /* null pointer, non-positive dims, lambda <= 0, theta_max outside (0,90),
+                                       batch < 1, |quat| not 1 within 1e-6, unknown enum value */
+    SCATMAN_UNSUPPORTED_DEVICE = 2, /* no CUDA device, or compute capability != 10.x */
+    SCATMAN_WORKSPACE_TOO_SMALL = 3,
+    SCATMAN_CUDA_ERROR = 4,         /* message via scatman_last_error */
+    SCATMAN_NOT_IMPLEMENTED = 5
+} scatman_status;
+
+/* Voxel grid: z = beam axis, x fastest. */
+typedef struct {
+    int32_t nx, ny, nz;
+    double dx, dy, dz;
+} scatman_grid;
+
+/* Flat detector perpendicular to the beam at unit distance, npx x npy square pixels; the mid-points of
+ * its outer edges in x sit at scattering angle theta_max (R9).  (cx, cy) shifts the detector centre off
+ * the axis, in pixels.  Pixel (ix, iy) has u = (ix + 1/2 - npx/2 + cx) pitch, v likewise with npy, cy;
+ * pitch = 2 tan(theta_max) / npx. */
+typedef struct {
+    int32_t npx, npy;
+    double theta_max_deg;
+    double cx, cy;
+} scatman_detector;
+
+enum { SCATMAN_RHO_LINEAR = 0, /* f(c) = c        : north_star's contrast dn = delta + i beta   */
+       SCATMAN_RHO_N2M1 = 1 }; /* f(c) = c (2 - c): the paper's n^2 - 1 (Eq. 5/9), conjugated */
+
+enum { SCATMAN_METHOD_AUTO = 0,        /* = TENSOR */
+       SCATMAN_METHOD_TENSOR = 1,      /* tcgen05 split-precision contraction + fused epilogue */
+       SCATMAN_METHOD_SIMT_SINCOS = 2, /* CUDA-core variant: one sincos of the full phase per term */
+       SCATMAN_METHOD_SIMT_TABLE = 3 };/* CUDA-core variant: FP32 FMA against 1-D phase tables */
+
+enum { SCATMAN_PRECISION_AUTO = 0,     /* = FP16X3 */
+       SCATMAN_PRECISION_FP16X3 = 1 }; /* A = Ah + Al, B = Bh + Bl in FP16; AhBh + AlBh + AhBl, FP32 accumulate */
+
+typedef struct {
+    int32_t rho_mode;
+    int32_t method;
+    int32_t precision;
+    uint32_t flags; /* reserved, must be 0 */
+} scatman_options;
+
+/* Create / destroy a context on CUDA device `device`.  Fails with SCATMAN_UNSUPPORTED_DEVICE unless the
+ * device is compute capability 10.x.  scatman_destroy(NULL) is SCATMAN_OK. */
+int scatman_create(scatman_ctx **out, int device);
+int scatman_destroy(scatman_ctx *ctx);
+
+/* Bytes of workspace scatman_simulate / scatman_simulate_q need for this problem (any orientation).
+ * npix = npx*npy for scatman_simulate.  opts may be NULL (all AUTO). */
+int scatman_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int64_t npix, int32_t batch,
+                            const scatman_options *opts, size_t *bytes);
+
+/* Step a1, q-map (Eq. 3; north_star (1)): detector pixels -> Ewald-sphere
+ * q = k (s_pixel - z^), FP64, d_q[p][3] with p = iy*npx + ix; qz = -k (u^2+v^2) / (r (r+1)) (R10). */
+int scatman_qmap(scatman_ctx *ctx, const scatman_detector *det, double lambda, double *d_q, void *cuda_stream);
+
+/* Step a0, orientation (Block 5; Fig. 6; R11): beam-frame grid = trilinear
+ * resample (FP64 coordinates, zero outside) of the body-frame grid at r_body = R^T r_beam, same dims.
+ * h_quat[b][4] = (w,x,y,z) unit quaternion, body -> beam; read on the host before return.
+ * d_dn_out must not alias d_dn_in. */
+int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *grid, const double *h_quat,
+                   int32_t batch, float *d_dn_out, void *cuda_stream);
+
+/* Step a2, column prefix (Eq. 6/8/9; north_star (2)): effective scattering strength
+ * d_rho[b][iz][iy][ix][2] = f(dn_j) exp(i k dz sum_{l<j} dn_l) as FP32 (Re, Im), WITHOUT the dV factor.
+ * The prefix runs in FP64. */
+int scatman_effective_strength(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                               int32_t rho_mode, int32_t batch, float *d_rho, void *cuda_stream);
+
+/* The whole hot path a0-a6 (north_star (1)-(5)): `batch` grids of identical dims -> `batch` intensity
+ * patterns on the flat detector.  h_quat may be NULL (identity for every item: a0 skipped).
+ * d_I[b][npy][npx] FP32.  d_ws/ws_bytes: workspace of at least scatman_workspace_bytes(). */
+int scatman_simulate(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                     const scatman_detector *det, const double *h_quat, int32_t batch,
+                     const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
+
+/* Same path minus a1, at an explicit list of momentum transfers d_q[npix][3] (FP64, device):
+ * for tests (q = 0, FFT-grid q's) and non-flat detectors.  d_I[b][npix]. */
+int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                       const double *d_q, int64_t npix, const double *h_quat, int32_t batch,
+                       const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies h_dn to the device, runs
+ * scatman_simulate on the context's own stream, copies I back into h_I and synchronises.  This entry
+ * point alone owns device memory: a grow-only arena kept in the context until scatman_destroy.
+ * h_dn and h_I should be pinned for full copy bandwidth (pageable memory works). */
+int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
+                          const scatman_detector *det, const double *h_quat, int32_t batch,
+                          const scatman_options *opts, float *h_I);
+
+/* Number of kernels the last scatman_simulate* call on this context launched (for bench accounting). */
+int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count);
+
+/* Device time of the contraction kernel (step a4+a5) of the last scatman_simulate* call, measured with
+ * CUDA events on the call's stream.  Synchronises on the end event.  -1 if none was recorded. */
+int scatman_last_contraction_ms(scatman_ctx *ctx, float *ms);
+
+const char *scatman_status_string(int status);
+const char *scatman_last_error(scatman_ctx *ctx); /* never NULL; "" if none */
+int scatman_version(void);                        /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCATMAN_H_ */

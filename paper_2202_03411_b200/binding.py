@@ -1,0 +1,251 @@
+"""Thin ctypes binding of libscatman (include/scatman.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels.  PyTorch is used for device
+memory and streams; tensors are passed as raw pointers.  There is NO fallback: if the shared
+library is missing or the device is not a B200-class (cc 10.x) GPU, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libscatman.so")
+
+OK, INVALID_ARGUMENT, UNSUPPORTED_DEVICE, WORKSPACE_TOO_SMALL, CUDA_ERROR, NOT_IMPLEMENTED = range(6)
+RHO_LINEAR, RHO_N2M1 = 0, 1
+METHOD_AUTO, METHOD_TENSOR, METHOD_SIMT_SINCOS, METHOD_SIMT_TABLE = 0, 1, 2, 3
+PRECISION_AUTO, PRECISION_FP16X3 = 0, 1
+
+EXPORTS = [
+    "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
+    "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
+    "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_status_string", "scatman_last_error",
+    "scatman_version",
+]
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double)]
+
+
+class Detector(C.Structure):
+    _fields_ = [("npx", C.c_int32), ("npy", C.c_int32), ("theta_max_deg", C.c_double),
+                ("cx", C.c_double), ("cy", C.c_double)]
+
+
+class Options(C.Structure):
+    _fields_ = [("rho_mode", C.c_int32), ("method", C.c_int32), ("precision", C.c_int32), ("flags", C.c_uint32)]
+
+
+class ScatmanError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"scatman status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libscatman.so (built in-tree by paper_2202_03411_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(f"{LIB_PATH} is missing: run `python -m paper_2202_03411_b200.build` "
+                                "(or __graft_entry__.build()).  There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.scatman_create.argtypes = [C.POINTER(vp), C.c_int]
+    L.scatman_destroy.argtypes = [vp]
+    L.scatman_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i64, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
+    L.scatman_qmap.argtypes = [vp, C.POINTER(Detector), dbl, vp, vp]
+    L.scatman_orient.argtypes = [vp, vp, C.POINTER(Grid), C.POINTER(dbl), i32, vp, vp]
+    L.scatman_effective_strength.argtypes = [vp, vp, C.POINTER(Grid), dbl, i32, i32, vp, vp]
+    L.scatman_simulate.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
+                                   C.POINTER(Options), vp, C.c_size_t, vp, vp]
+    L.scatman_simulate_q.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i64, C.POINTER(dbl), i32,
+                                     C.POINTER(Options), vp, C.c_size_t, vp, vp]
+    L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
+                                        C.POINTER(Options), vp]
+    L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
+    L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.scatman_status_string.argtypes = [C.c_int]
+    L.scatman_status_string.restype = C.c_char_p
+    L.scatman_last_error.argtypes = [vp]
+    L.scatman_last_error.restype = C.c_char_p
+    L.scatman_version.restype = C.c_int
+    for name in EXPORTS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+def _quat_arg(quat, batch: int):
+    if quat is None:
+        return None, None
+    flat = [float(v) for row in quat for v in row]
+    if len(flat) != 4 * batch:
+        raise ValueError("quat must be [batch][4]")
+    arr = (C.c_double * len(flat))(*flat)
+    return arr, C.cast(arr, C.POINTER(C.c_double))
+
+
+class Scatman:
+    """One context per device.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, device: int = 0):
+        self.lib = load_library()
+        self._ctx = C.c_void_p()
+        rc = self.lib.scatman_create(C.byref(self._ctx), int(device))
+        if rc != OK:
+            raise ScatmanError(rc, self.lib.scatman_status_string(rc).decode())
+        self.device = int(device)
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.scatman_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != OK:
+            msg = self.lib.scatman_last_error(self._ctx).decode() or self.lib.scatman_status_string(rc).decode()
+            raise ScatmanError(rc, msg)
+
+    # -- marshalling helpers -------------------------------------------------------------------
+    @staticmethod
+    def _stream(stream) -> C.c_void_p:
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream()
+        return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+    @staticmethod
+    def _grid_of(dn, voxel) -> Grid:
+        if dn.dim() == 4:
+            nz, ny, nx, two = dn.shape
+        else:
+            _, nz, ny, nx, two = dn.shape
+        assert two == 2
+        return Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+
+    @staticmethod
+    def _batch_of(dn) -> int:
+        return 1 if dn.dim() == 4 else int(dn.shape[0])
+
+    @staticmethod
+    def _check_dn(dn):
+        import torch
+        if not (dn.is_cuda and dn.dtype == torch.float32 and dn.is_contiguous()):
+            raise ValueError("grid must be a contiguous CUDA float32 tensor [B][nz][ny][nx][2]")
+
+    # -- entry points --------------------------------------------------------------------------
+    def workspace_bytes(self, grid: Grid, npix: int, batch: int, opts: Optional[Options] = None) -> int:
+        out = C.c_size_t(0)
+        self._check(self.lib.scatman_workspace_bytes(self._ctx, C.byref(grid), int(npix), int(batch),
+                                                     C.byref(opts) if opts else None, C.byref(out)))
+        return int(out.value)
+
+    def qmap(self, npx: int, npy: int, theta_max_deg: float, lam: float, cx: float = 0.0, cy: float = 0.0, stream=None):
+        import torch
+        q = torch.empty((npx * npy, 3), dtype=torch.float64, device=f"cuda:{self.device}")
+        det = Detector(npx, npy, float(theta_max_deg), float(cx), float(cy))
+        self._check(self.lib.scatman_qmap(self._ctx, C.byref(det), float(lam), C.c_void_p(q.data_ptr()), self._stream(stream)))
+        return q
+
+    def orient(self, dn, voxel, quat, stream=None):
+        import torch
+        self._check_dn(dn)
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        out = torch.empty_like(dn)
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_orient(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), qp, batch,
+                                            C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out
+
+    def effective_strength(self, dn, voxel, lam: float, rho_mode: int = RHO_LINEAR, stream=None):
+        import torch
+        self._check_dn(dn)
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        out = torch.empty_like(dn)
+        self._check(self.lib.scatman_effective_strength(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
+                                                        int(rho_mode), batch, C.c_void_p(out.data_ptr()),
+                                                        self._stream(stream)))
+        return out
+
+    def simulate(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
+                 rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, cx: float = 0.0, cy: float = 0.0,
+                 workspace=None, out=None, stream=None):
+        """I float32 [B][npy][npx] on the device ([npy][npx] for a 4-D grid).  Asynchronous."""
+        import torch
+        self._check_dn(dn)
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        need = self.workspace_bytes(grid, npx * npy, batch, opts)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
+                                              C.byref(det), qp, batch, C.byref(opts), C.c_void_p(workspace.data_ptr()),
+                                              workspace.numel(), C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out if dn.dim() == 5 else out[0]
+
+    def simulate_q(self, dn, voxel, lam: float, q, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,
+                   workspace=None, out=None, stream=None):
+        """I float32 [B][npix] at the explicit device q list [npix][3] (float64)."""
+        import torch
+        self._check_dn(dn)
+        if not (q.is_cuda and q.dtype == torch.float64 and q.is_contiguous() and q.shape[-1] == 3):
+            raise ValueError("q must be a contiguous CUDA float64 tensor [npix][3]")
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        npix = int(q.shape[0])
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        need = self.workspace_bytes(grid, npix, batch, opts)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
+        if out is None:
+            out = torch.empty((batch, npix), dtype=torch.float32, device=dn.device)
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_q(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
+                                                C.c_void_p(q.data_ptr()), npix, qp, batch, C.byref(opts),
+                                                C.c_void_p(workspace.data_ptr()), workspace.numel(),
+                                                C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out if dn.dim() == 5 else out[0]
+
+    def simulate_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
+                      rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None):
+        """Host-buffer end-to-end call: h_dn / h_out are CPU float32 tensors (pinned for speed). Synchronous."""
+        import torch
+        if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
+            raise ValueError("h_dn must be a contiguous CPU float32 tensor")
+        grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        if h_out is None:
+            h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_host(self._ctx, C.c_void_p(h_dn.data_ptr()), C.byref(grid), float(lam),
+                                                   C.byref(det), qp, batch, C.byref(opts), C.c_void_p(h_out.data_ptr())))
+        return h_out
+
+    def last_launch_count(self) -> int:
+        n = C.c_int32(0)
+        self._check(self.lib.scatman_last_launch_count(self._ctx, C.byref(n)))
+        return int(n.value)
+
+    def last_contraction_ms(self) -> float:
+        ms = C.c_float(0)
+        self._check(self.lib.scatman_last_contraction_ms(self._ctx, C.byref(ms)))
+        return float(ms.value)

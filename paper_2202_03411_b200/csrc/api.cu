@@ -1,0 +1,417 @@
+// api.cu -- the C ABI of libscatman (include/scatman.h): argument validation, workspace planning and the
+// enqueue order of the hot path.  Host logic only; every step of the path runs in the kernels.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "internal.h"
+
+using namespace scatman;
+
+struct scatman_ctx {
+    int device = 0;
+    int num_sms = 0;
+    std::string last_error;
+    int last_launches = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    // arena of scatman_simulate_host (grow-only)
+    cudaStream_t host_stream = nullptr;
+    void *arena = nullptr;
+    size_t arena_bytes = 0;
+};
+
+namespace scatman {
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Batch chunks x z splits of the tensor kernel: minimise waves * per-item length (in slices), where an
+// item costs its slices plus ~2 slice-equivalents of fill (A load, pipeline ramp).
+void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs) {
+    double best = 1e300;
+    int bc = 1, bz = 1;
+    const int max_z = p.nz < 16 ? p.nz : 16;
+    const int max_c = p.batch < 64 ? p.batch : 64;
+    for (int c = 1; c <= max_c; ++c) {
+        const int bpc = (p.batch + c - 1) / c;
+        const int cc = (p.batch + bpc - 1) / bpc;
+        for (int z = 1; z <= max_z; ++z) {
+            const long long items = (long long)cc * z * p.ngroups * p.ntiles;
+            const long long waves = (items + num_sms - 1) / num_sms;
+            const double len = (double)bpc * (double)((p.nz + z - 1) / z) + 2.0;
+            const double cost = (double)waves * len;
+            if (cost < best * (1.0 - 1e-9)) { best = cost; bc = cc; bz = z; }
+        }
+    }
+    *nchunks = bc;
+    *nzs = bz;
+}
+
+static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int batch, const scatman_options &o,
+                      int num_sms) {
+    Plan p;
+    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
+    p.npix = npix; p.batch = batch; p.rho_mode = o.rho_mode;
+    p.method = o.method == SCATMAN_METHOD_AUTO ? SCATMAN_METHOD_TENSOR : o.method;
+    p.nvox = (int64_t)g.nx * g.ny * g.nz;
+    p.nx_pad = (int)align_up(g.nx, kTileX);
+    p.ny_pad = (int)align_up(g.ny, kBlockY);
+    p.nyb = p.ny_pad / kBlockY;
+    p.ngroups = (p.nyb + kGroupYB - 1) / kGroupYB;
+    p.nxt = p.nx_pad / kTileX;
+    p.nxa = p.nx_pad / kFine;
+    p.ntiles = (int)((npix + kTileP - 1) / kTileP);
+    p.npix_pad = (int64_t)p.ntiles * kTileP;
+    if (p.method == SCATMAN_METHOD_TENSOR) {
+        tensor_schedule(p, num_sms, &p.t_nchunks, &p.t_nzs);
+        p.nsplit = p.ngroups * p.t_nzs;
+    } else {
+        p.nsplit = simt_zsplit(p, num_sms);
+    }
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o2 = off; off = align_up(off + bytes, 1024); return o2; };
+    p.off_q = take(sizeof(double) * 3 * (size_t)npix);
+    p.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
+    p.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    p.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    p.off_max = take(sizeof(unsigned) * (size_t)batch);
+    p.off_ampscale = take(sizeof(float) * (size_t)batch);
+    p.off_partial = take(sizeof(float2) * (size_t)batch * p.nsplit * (size_t)p.npix_pad);
+    if (p.method == SCATMAN_METHOD_TENSOR) {
+        p.off_B = take(sizeof(__half) * 4 * (size_t)p.nx_pad * p.ny_pad * (size_t)p.nz * batch);
+        p.off_A = take(sizeof(__half) * 4 * (size_t)p.npix_pad * p.ny_pad);
+        p.off_anchor = take(sizeof(float2) * (size_t)p.ntiles * p.nxa * kTileP);
+        p.off_fine = take(sizeof(float2) * (size_t)p.ntiles * kFine * kTileP);
+        p.off_mz = take(sizeof(float2) * (size_t)p.ntiles * p.nz * kTileP);
+    }
+    p.total = off;
+    return p;
+}
+
+}  // namespace scatman
+
+static int fail(scatman_ctx *ctx, int status, const std::string &msg) {
+    if (ctx) ctx->last_error = msg;
+    return status;
+}
+static int cuda_fail(scatman_ctx *ctx, cudaError_t e, const char *where) {
+    return fail(ctx, SCATMAN_CUDA_ERROR, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+static bool valid_grid(const scatman_grid *g) {
+    return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->dx > 0 && g->dy > 0 && g->dz > 0 && std::isfinite(g->dx) &&
+           std::isfinite(g->dy) && std::isfinite(g->dz) && g->nx <= 8192 && g->ny <= 8192 && g->nz <= 65535;
+}
+static bool valid_detector(const scatman_detector *d) {
+    return d && d->npx > 0 && d->npy > 0 && d->theta_max_deg > 0.0 && d->theta_max_deg < 90.0 && std::isfinite(d->cx) &&
+           std::isfinite(d->cy);
+}
+static bool valid_options(const scatman_options &o) {
+    return (o.rho_mode == SCATMAN_RHO_LINEAR || o.rho_mode == SCATMAN_RHO_N2M1) && o.method >= 0 && o.method <= 3 &&
+           o.precision >= 0 && o.precision <= 1 && o.flags == 0;
+}
+static bool valid_quats(const double *q, int batch) {
+    for (int b = 0; b < batch; ++b) {
+        double n2 = 0;
+        for (int i = 0; i < 4; ++i) n2 += q[4 * b + i] * q[4 * b + i];
+        if (!(std::fabs(n2 - 1.0) <= 2e-6)) return false;
+    }
+    return true;
+}
+static bool all_identity(const double *q, int batch) {
+    for (int b = 0; b < batch; ++b)
+        if (std::fabs(q[4 * b]) != 1.0 || q[4 * b + 1] != 0.0 || q[4 * b + 2] != 0.0 || q[4 * b + 3] != 0.0) return false;
+    return true;
+}
+static void quat_to_rotmat(const double *q, double *R) {
+    const double w = q[0], a = q[1], b = q[2], c = q[3];
+    R[0] = 1 - 2 * (b * b + c * c); R[1] = 2 * (a * b - w * c);     R[2] = 2 * (a * c + w * b);
+    R[3] = 2 * (a * b + w * c);     R[4] = 1 - 2 * (a * a + c * c); R[5] = 2 * (b * c - w * a);
+    R[6] = 2 * (a * c - w * b);     R[7] = 2 * (b * c + w * a);     R[8] = 1 - 2 * (a * a + b * b);
+}
+
+// Rotation matrices reach the device as kernel arguments (no host buffer outlives the call).
+struct RotChunk {
+    double r[32 * 9];
+};
+__global__ void store_rotmat_kernel(RotChunk c, int n, double *__restrict__ dst) {
+    const int i = threadIdx.x;
+    if (i < n * 9) dst[i] = c.r[i];
+}
+static cudaError_t upload_rotmats(const double *h_quat, int batch, double *d_rotmat, cudaStream_t st, int *nlaunch) {
+    for (int b0 = 0; b0 < batch; b0 += 32) {
+        RotChunk c;
+        const int n = batch - b0 < 32 ? batch - b0 : 32;
+        for (int i = 0; i < n; ++i) quat_to_rotmat(h_quat + 4 * (b0 + i), c.r + 9 * i);
+        store_rotmat_kernel<<<1, 288, 0, st>>>(c, n, d_rotmat + 9 * b0);
+        if (nlaunch) ++*nlaunch;
+    }
+    return cudaGetLastError();
+}
+
+extern "C" {
+
+int scatman_version(void) { return 100; }
+
+const char *scatman_status_string(int status) {
+    switch (status) {
+        case SCATMAN_OK: return "ok";
+        case SCATMAN_INVALID_ARGUMENT: return "invalid argument";
+        case SCATMAN_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.x)";
+        case SCATMAN_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case SCATMAN_CUDA_ERROR: return "CUDA error";
+        case SCATMAN_NOT_IMPLEMENTED: return "not implemented";
+        default: return "unknown status";
+    }
+}
+
+const char *scatman_last_error(scatman_ctx *ctx) { return ctx ? ctx->last_error.c_str() : ""; }
+
+int scatman_create(scatman_ctx **out, int device) {
+    if (!out) return SCATMAN_INVALID_ARGUMENT;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count <= 0) {
+        cudaGetLastError();
+        return SCATMAN_UNSUPPORTED_DEVICE;
+    }
+    if (device < 0 || device >= count) return SCATMAN_INVALID_ARGUMENT;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SCATMAN_CUDA_ERROR;
+    if (prop.major != 10) return SCATMAN_UNSUPPORTED_DEVICE;
+    if (cudaSetDevice(device) != cudaSuccess) return SCATMAN_CUDA_ERROR;
+    scatman_ctx *ctx = new scatman_ctx();
+    ctx->device = device;
+    ctx->num_sms = prop.multiProcessorCount;
+    if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
+        delete ctx;
+        return SCATMAN_CUDA_ERROR;
+    }
+    *out = ctx;
+    return SCATMAN_OK;
+}
+
+int scatman_destroy(scatman_ctx *ctx) {
+    if (!ctx) return SCATMAN_OK;
+    cudaSetDevice(ctx->device);
+    if (ctx->arena) cudaFree(ctx->arena);
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    delete ctx;
+    return SCATMAN_OK;
+}
+
+int scatman_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int64_t npix, int32_t batch,
+                            const scatman_options *opts, size_t *bytes) {
+    if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!valid_grid(grid) || npix < 1 || batch < 1 || !valid_options(o)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = make_plan(*grid, 1.0, npix, batch, o, ctx->num_sms).total;
+    return SCATMAN_OK;
+}
+
+int scatman_qmap(scatman_ctx *ctx, const scatman_detector *det, double lambda, double *d_q, void *cuda_stream) {
+    if (!ctx || !d_q || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    cudaError_t e = launch_qmap(*det, lambda, d_q, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "qmap");
+}
+
+int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *grid, const double *h_quat,
+                   int32_t batch, float *d_dn_out, void *cuda_stream) {
+    if (!ctx || !d_dn_in || !d_dn_out || d_dn_in == d_dn_out || !valid_grid(grid) || !h_quat || batch < 1 ||
+        !valid_quats(h_quat, batch))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the rotation matrices travel in a small stream-ordered allocation
+    double *d_rot = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&d_rot, sizeof(double) * 9 * batch, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "orient: cudaMallocAsync");
+    Plan p;
+    p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.dx = grid->dx; p.dy = grid->dy; p.dz = grid->dz;
+    e = upload_rotmats(h_quat, batch, d_rot, st, nullptr);
+    if (e == cudaSuccess) e = launch_orient(d_dn_in, p, d_rot, batch, d_dn_out, st);
+    cudaFreeAsync(d_rot, st);
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "orient");
+}
+
+int scatman_effective_strength(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                               int32_t rho_mode, int32_t batch, float *d_rho, void *cuda_stream) {
+    if (!ctx || !d_dn || !d_rho || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) || batch < 1 ||
+        (rho_mode != SCATMAN_RHO_LINEAR && rho_mode != SCATMAN_RHO_N2M1))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned *d_max = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&d_max, sizeof(unsigned) * batch, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "effective_strength: cudaMallocAsync");
+    Plan p;
+    p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.dx = grid->dx; p.dy = grid->dy; p.dz = grid->dz;
+    p.lambda = lambda; p.rho_mode = rho_mode;
+    e = launch_strength(d_dn, p, batch, d_rho, d_max, st);
+    cudaFreeAsync(d_max, st);
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "effective_strength");
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ hot path
+// Enqueue order: [a1 q-map] -> [a0 orient] -> a2 prefix -> operand pack + a3 tables
+// -> a4/a5 contraction -> |A|^2.  Nothing here waits for the device.
+static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                    const scatman_detector *det, const double *d_q_in, int64_t npix, const double *h_quat, int batch,
+                    const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, cudaStream_t st) {
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_dn || !d_I || !d_ws || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) || batch < 1 ||
+        npix < 1 || batch > 65535 || !valid_options(o) || (!det && !d_q_in) || (det && !valid_detector(det)))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    if (h_quat && !valid_quats(h_quat, batch)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "quaternion is not unit");
+    if (((uintptr_t)d_dn | (uintptr_t)d_ws | (uintptr_t)d_I) & 15)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
+    cudaSetDevice(ctx->device);
+    const Plan p = make_plan(*grid, lambda, npix, batch, o, ctx->num_sms);
+    if (p.method == SCATMAN_METHOD_SIMT_TABLE) return fail(ctx, SCATMAN_NOT_IMPLEMENTED, "SIMT_TABLE is not built yet");
+    if (ws_bytes < p.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    uint8_t *ws = (uint8_t *)d_ws;
+    int nl = 0;
+    cudaError_t e = cudaSuccess;
+    ctx->ev_valid = false;
+
+    const double *d_q = d_q_in;
+    if (!d_q) {
+        double *q = (double *)(ws + p.off_q);
+        e = launch_qmap(*det, lambda, q, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+        d_q = q;
+    }
+    const float *src = d_dn;
+    if (h_quat && !all_identity(h_quat, batch)) {
+        double *rm = (double *)(ws + p.off_rotmat);
+        e = upload_rotmats(h_quat, batch, rm, st, &nl);
+        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + p.off_rot), st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
+        src = (const float *)(ws + p.off_rot);
+    }
+    float *rho = (float *)(ws + p.off_rho);
+    unsigned *maxbits = (unsigned *)(ws + p.off_max);
+    e = launch_strength(src, p, batch, rho, maxbits, st);
+    ++nl;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    float2 *partial = (float2 *)(ws + p.off_partial);
+    const double dV = p.dx * p.dy * p.dz;
+
+    if (p.method == SCATMAN_METHOD_TENSOR) {
+        float *ampscale = (float *)(ws + p.off_ampscale);
+        e = launch_pack_b(rho, p, maxbits, ampscale, (__half *)(ws + p.off_B), st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "pack_b");
+        e = launch_tables(d_q, p, (__half *)(ws + p.off_A), (float2 *)(ws + p.off_anchor), (float2 *)(ws + p.off_fine),
+                          (float2 *)(ws + p.off_mz), st, &nl);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "tables");
+        TensorLaunch t;
+        t.d_A = ws + p.off_A; t.d_B = ws + p.off_B;
+        t.d_anchor = (const float2 *)(ws + p.off_anchor); t.d_fine = (const float2 *)(ws + p.off_fine);
+        t.d_mz = (const float2 *)(ws + p.off_mz); t.d_partial = partial; t.num_sms = ctx->num_sms;
+        std::string err;
+        cudaEventRecord(ctx->ev0, st);
+        e = launch_tensor(p, t, st, &err);
+        cudaEventRecord(ctx->ev1, st);
+        ++nl;
+        if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "contract") : fail(ctx, SCATMAN_CUDA_ERROR, err);
+        ctx->ev_valid = true;
+        e = launch_finalize(partial, p, ampscale, dV, d_I, st);
+    } else {
+        cudaEventRecord(ctx->ev0, st);
+        e = launch_simt_sincos(rho, d_q, p, partial, st);
+        cudaEventRecord(ctx->ev1, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "simt_sincos");
+        ctx->ev_valid = true;
+        e = launch_finalize(partial, p, nullptr, dV, d_I, st);
+    }
+    ++nl;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "finalize");
+    ctx->last_launches = nl;
+    return SCATMAN_OK;
+}
+
+extern "C" {
+
+int scatman_simulate(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                     const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                     void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+    if (!det) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "detector is null");
+    if (!valid_detector(det)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad detector");
+    return run_path(ctx, d_dn, grid, lambda, det, nullptr, (int64_t)det->npx * det->npy, h_quat, batch, opts, d_ws,
+                    ws_bytes, d_I, (cudaStream_t)cuda_stream);
+}
+
+int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_q,
+                       int64_t npix, const double *h_quat, int32_t batch, const scatman_options *opts, void *d_ws,
+                       size_t ws_bytes, float *d_I, void *cuda_stream) {
+    if (!d_q) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "d_q is null");
+    return run_path(ctx, d_dn, grid, lambda, nullptr, d_q, npix, h_quat, batch, opts, d_ws, ws_bytes, d_I,
+                    (cudaStream_t)cuda_stream);
+}
+
+int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
+                          const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                          float *h_I) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!h_dn || !h_I || !valid_grid(grid) || !valid_detector(det) || batch < 1 || !valid_options(o) || !(lambda > 0.0))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    cudaError_t e;
+    if (!ctx->host_stream && (e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
+        return cuda_fail(ctx, e, "stream create");
+    const int64_t npix = (int64_t)det->npx * det->npy;
+    const Plan p = make_plan(*grid, lambda, npix, batch, o, ctx->num_sms);
+    const size_t dn_bytes = (sizeof(float) * 2 * (size_t)p.nvox * batch + 1023) / 1024 * 1024;
+    const size_t I_bytes = (sizeof(float) * (size_t)npix * batch + 1023) / 1024 * 1024;
+    const size_t need = dn_bytes + I_bytes + p.total;
+    if (need > ctx->arena_bytes) {
+        if (ctx->arena) cudaFree(ctx->arena);
+        ctx->arena = nullptr;
+        ctx->arena_bytes = 0;
+        if ((e = cudaMalloc(&ctx->arena, need)) != cudaSuccess) return cuda_fail(ctx, e, "arena cudaMalloc");
+        ctx->arena_bytes = need;
+    }
+    uint8_t *a = (uint8_t *)ctx->arena;
+    float *d_dn = (float *)a;
+    float *d_I = (float *)(a + dn_bytes);
+    void *d_ws = a + dn_bytes + I_bytes;
+    cudaStream_t st = ctx->host_stream;
+    if ((e = cudaMemcpyAsync(d_dn, h_dn, sizeof(float) * 2 * (size_t)p.nvox * batch, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(ctx, e, "H2D");
+    int rc = run_path(ctx, d_dn, grid, lambda, det, nullptr, npix, h_quat, batch, &o, d_ws, p.total, d_I, st);
+    if (rc != SCATMAN_OK) return rc;
+    if ((e = cudaMemcpyAsync(h_I, d_I, sizeof(float) * (size_t)npix * batch, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(ctx, e, "D2H");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "synchronize");
+    return SCATMAN_OK;
+}
+
+int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count) {
+    if (!ctx || !count) return SCATMAN_INVALID_ARGUMENT;
+    *count = ctx->last_launches;
+    return SCATMAN_OK;
+}
+
+int scatman_last_contraction_ms(scatman_ctx *ctx, float *ms) {
+    if (!ctx || !ms) return SCATMAN_INVALID_ARGUMENT;
+    *ms = -1.f;
+    if (!ctx->ev_valid) return SCATMAN_OK;
+    cudaError_t e = cudaEventSynchronize(ctx->ev1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1);
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "event");
+}
+
+}  // extern "C"

@@ -1,0 +1,77 @@
+// internal.h -- shared declarations of libscatman's translation units (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cstddef>
+#include <cstdint>
+#include <string>
+
+#include "../../include/scatman.h"
+
+namespace scatman {
+
+// ---- tile geometry of the tensor-core contraction (tensor_kernel.cu) ---------------------------
+constexpr int kTileP = 128;     // pixels per CTA tile          = UMMA M
+constexpr int kTileX = 128;     // x columns per accumulator    = UMMA N
+constexpr int kBlockY = 64;     // y per smem K-block (64 fp16 = one 128-byte swizzle row)
+constexpr int kGroupYB = 2;     // K-blocks of the A operand resident in smem per work item
+constexpr int kFine = 16;       // x per anchor block in the epilogue row-dot
+constexpr float kScaleA = 1024.0f;  // M_y tables are stored as 2^10 * e^{i qy y} (keeps the FP16 low part normal)
+constexpr int kScaleBExp = 13;  // rho~ is scaled so that max |component| lies in [2^12, 2^13)
+
+// Problem plan: every derived size and every workspace offset, computed on the host.
+struct Plan {
+    int nx = 0, ny = 0, nz = 0;
+    double dx = 0, dy = 0, dz = 0, lambda = 0;
+    int64_t npix = 0;
+    int batch = 0;
+    int rho_mode = 0, method = 0;
+    int64_t nvox = 0;
+    // padded sizes of the tensor path
+    int nx_pad = 0, ny_pad = 0;   // multiples of kTileX / kBlockY
+    int nyb = 0;                  // ny_pad / kBlockY
+    int ngroups = 0;              // y-groups (work items per pixel tile and batch chunk)
+    int nxt = 0;                  // x tiles
+    int nxa = 0;                  // anchor blocks per row = nx_pad / kFine
+    int ntiles = 0;               // pixel tiles
+    int64_t npix_pad = 0;
+    int nsplit = 0;               // partial sums per pixel (tensor: ngroups * t_nzs; simt: z splits)
+    int t_nchunks = 1, t_nzs = 1; // tensor schedule: batch chunks and z splits per (tile, y-group)
+    // workspace offsets (bytes)
+    size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
+           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, total = 0;
+};
+
+int simt_zsplit(const Plan &p, int num_sms);
+void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs);
+
+// ---- kernels launchers (all asynchronous on `st`; return cudaGetLastError()) -------------------
+cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);
+cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out,
+                          cudaStream_t st);
+cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
+                            cudaStream_t st);
+cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_maxbits, float *d_ampscale,
+                          __half *d_B, cudaStream_t st);
+cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
+                          float2 *d_mz, cudaStream_t st, int *nlaunch);
+cudaError_t launch_finalize(const float2 *d_partial, const Plan &p, const float *d_ampscale, double dV,
+                            float *d_I, cudaStream_t st);
+cudaError_t launch_simt_sincos(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
+                               cudaStream_t st);
+cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
+                              cudaStream_t st);
+
+// tensor path: tensor maps are encoded on the host through the driver entry point
+struct TensorMaps;  // opaque here
+struct TensorLaunch {
+    const void *d_A;      // fp16 [4][npix_pad][ny_pad]
+    const void *d_B;      // fp16 [batch][nz][4][nx_pad][ny_pad]
+    const float2 *d_anchor, *d_fine, *d_mz;
+    float2 *d_partial;
+    int num_sms;
+};
+cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st, std::string *err);
+size_t tensor_smem_bytes();
+
+}  // namespace scatman

@@ -1,0 +1,278 @@
+// prep_kernels.cu -- the HBM-bound steps around the contraction: a1 q-map, a0 orient, a2 column prefix,
+// operand packing, a3 phase tables, and the |A|^2 finalize.  All FP64 where a phase is formed.
+#include "internal.h"
+
+namespace scatman {
+
+__device__ __forceinline__ double centre(int i, int n, double d) { return ((double)i - 0.5 * (double)(n - 1)) * d; }
+
+// ------------------------------------------------------------------------------------------------ a1
+// Eq. 3 in north_star's form q = k (s_pixel - z^): flat detector at unit distance.
+__global__ void qmap_kernel(int npx, int npy, double pitch, double cx, double cy, double k, double *__restrict__ q) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= (int64_t)npx * npy) return;
+    const int ix = (int)(p % npx), iy = (int)(p / npx);
+    const double u = ((double)ix + 0.5 - 0.5 * (double)npx + cx) * pitch;
+    const double v = ((double)iy + 0.5 - 0.5 * (double)npy + cy) * pitch;
+    const double s2 = u * u + v * v;
+    const double r = sqrt(s2 + 1.0);
+    q[3 * p + 0] = k * u / r;
+    q[3 * p + 1] = k * v / r;
+    q[3 * p + 2] = -k * s2 / (r * (r + 1.0));  // = k (1/r - 1) without the cancellation (R10)
+}
+
+cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st) {
+    const int64_t npix = (int64_t)det.npx * det.npy;
+    const double pitch = 2.0 * tan(det.theta_max_deg * 3.14159265358979323846 / 180.0) / (double)det.npx;
+    const double k = 2.0 * 3.14159265358979323846 / lambda;
+    qmap_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(det.npx, det.npy, pitch, det.cx, det.cy, k, d_q);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a0
+// Block 5 / Fig. 6: beam-frame voxel <- trilinear sample of the body-frame grid at
+// r_body = R^T r_beam.  rotmat[b][9] row-major R (body -> beam).  One thread per beam-frame voxel.
+__global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz,
+                              const double *__restrict__ rotmat, float2 *__restrict__ out) {
+    const int iy = blockIdx.x % ny;
+    const int iz = (blockIdx.x / ny) % nz, b = blockIdx.x / (ny * nz);
+    const double *R = rotmat + 9 * b;
+    for (int ix = threadIdx.x; ix < nx; ix += blockDim.x) {
+    const double xb = centre(ix, nx, dx), yb = centre(iy, ny, dy), zb = centre(iz, nz, dz);
+    const double xo = R[0] * xb + R[3] * yb + R[6] * zb;
+    const double yo = R[1] * xb + R[4] * yb + R[7] * zb;
+    const double zo = R[2] * xb + R[5] * yb + R[8] * zb;
+    const double fx = xo / dx + 0.5 * (double)(nx - 1);
+    const double fy = yo / dy + 0.5 * (double)(ny - 1);
+    const double fz = zo / dz + 0.5 * (double)(nz - 1);
+    const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
+    const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
+    const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
+    const float2 *src = in + (size_t)b * nx * ny * nz;
+    double are = 0.0, aim = 0.0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const int xi = x0 + (c & 1), yi = y0 + ((c >> 1) & 1), zi = z0 + (c >> 2);
+        if (xi < 0 || xi >= nx || yi < 0 || yi >= ny || zi < 0 || zi >= nz) continue;
+        const double w = ((c & 1) ? tx : 1.0 - tx) * ((c & 2) ? ty : 1.0 - ty) * ((c & 4) ? tz : 1.0 - tz);
+        const float2 s = __ldg(src + ((size_t)zi * ny + yi) * nx + xi);
+        are += w * (double)s.x;
+        aim += w * (double)s.y;
+    }
+    out[(size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx + ix] = make_float2((float)are, (float)aim);
+    }
+}
+
+cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out,
+                          cudaStream_t st) {
+    const unsigned grid = (unsigned)((size_t)p.ny * p.nz * batch);
+    orient_kernel<<<grid, p.nx >= 128 ? 128 : 64, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, d_rotmat,
+                                        (float2 *)d_out);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a2
+// Eq. 6/8/9: exclusive z-prefix C_j of dn = delta + i beta per (x,y) column in FP64,
+// T_j = exp(i k dz C_j), rho~_j = f(dn_j) T_j (dV applied at the end).  One thread per column; x is the
+// fast thread index so every slice access is coalesced.  Also reduces max |component| per batch item
+// for the FP16 operand scale.
+__global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz, double kdz, int rho_mode,
+                                float2 *__restrict__ rho, unsigned *__restrict__ maxbits) {
+    const int ix = blockIdx.x * blockDim.x + threadIdx.x;
+    const int iy = blockIdx.y, b = blockIdx.z;
+    float vmax = 0.f;
+    if (ix < nx) {
+        const size_t plane = (size_t)nx * ny;
+        const size_t base = (size_t)b * plane * nz + (size_t)iy * nx + ix;
+        double Cre = 0.0, Cim = 0.0;
+        double Tre = 1.0, Tim = 0.0;
+        bool stale = false;  // T must be recomputed from C before its next use
+        for (int iz = 0; iz < nz; ++iz) {
+            const float2 c = __ldg(dn + base + iz * plane);
+            float2 o = make_float2(0.f, 0.f);
+            if (c.x != 0.f || c.y != 0.f) {
+                if (stale) {
+                    double s, co;
+                    sincos(kdz * Cre, &s, &co);
+                    const double mag = exp(-kdz * Cim);
+                    Tre = mag * co;
+                    Tim = mag * s;
+                    stale = false;
+                }
+                const double d = (double)c.x, be = (double)c.y;
+                double fre = d, fim = be;
+                if (rho_mode == SCATMAN_RHO_N2M1) {  // c (2 - c)
+                    fre = d * (2.0 - d) + be * be;
+                    fim = 2.0 * be * (1.0 - d);
+                }
+                o.x = (float)(fre * Tre - fim * Tim);
+                o.y = (float)(fre * Tim + fim * Tre);
+                vmax = fmaxf(vmax, fmaxf(fabsf(o.x), fabsf(o.y)));
+                Cre += d;
+                Cim += be;
+                stale = true;
+            }
+            rho[base + iz * plane] = o;
+        }
+    }
+    // block max -> one atomic per block (non-negative floats order like their bit patterns)
+    for (int off = 16; off > 0; off >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, off));
+    __shared__ float wmax[8];
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = vmax;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float m = 0.f;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmaxf(m, wmax[w]);
+        if (m > 0.f) atomicMax(maxbits + b, __float_as_uint(m));
+    }
+}
+
+cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
+                            cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(d_maxbits, 0, sizeof(unsigned) * batch, st);
+    if (e != cudaSuccess) return e;
+    const int threads = p.nx >= 128 ? 128 : 64;
+    dim3 grid((p.nx + threads - 1) / threads, p.ny, batch);
+    const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
+    strength_kernel<<<grid, threads, 0, st>>>((const float2 *)d_dn, p.nx, p.ny, p.nz, kdz, p.rho_mode,
+                                              (float2 *)d_rho, d_maxbits);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ operand B
+// rho~ FP32 [b][z][y][x] -> FP16 split planes [b][z][4][x_pad][y_pad] (y fastest = K-major for UMMA),
+// planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo, scaled by sB[b] = 2^(13 - e), max in [2^(e-1), 2^e).
+// 32x32 (x,y) tiles transposed through shared memory; padding written as zeros.
+__device__ __forceinline__ float scale_from_maxbits(unsigned bits) {
+    const float m = __uint_as_float(bits);
+    if (!(m > 0.f)) return 1.f;
+    int e;
+    frexpf(m, &e);
+    return ldexpf(1.f, kScaleBExp - e);
+}
+
+__global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nx_pad, int ny_pad,
+                              const unsigned *__restrict__ maxbits, float *__restrict__ ampscale, float dV,
+                              __half *__restrict__ B) {
+    __shared__ float2 tile[32][33];
+    const int bz = blockIdx.x;  // b*nz + z
+    const int b = bz / nz;
+    const float s = scale_from_maxbits(maxbits[b]);
+    const int x0 = blockIdx.y * 32, y0 = blockIdx.z * 32;
+    const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+    const float2 *src = rho + (size_t)bz * nx * ny;
+    for (int r = ty; r < 32; r += 8) {
+        const int y = y0 + r, x = x0 + tx;
+        tile[r][tx] = (y < ny && x < nx) ? src[(size_t)y * nx + x] : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    const size_t plane = (size_t)nx_pad * ny_pad;
+    __half *dst = B + (size_t)bz * 4 * plane;
+    for (int r = ty; r < 32; r += 8) {
+        const int x = x0 + r, y = y0 + tx;  // x < nx_pad, y < ny_pad by grid construction
+        const float2 v = tile[tx][r];
+        const float re = v.x * s, im = v.y * s;
+        const __half reh = __float2half_rn(re), imh = __float2half_rn(im);
+        const __half rel = __float2half_rn(re - __half2float(reh)), iml = __float2half_rn(im - __half2float(imh));
+        const size_t o = (size_t)x * ny_pad + y;
+        dst[o] = reh;
+        dst[plane + o] = rel;
+        dst[2 * plane + o] = imh;
+        dst[3 * plane + o] = iml;
+    }
+    if (blockIdx.y == 0 && blockIdx.z == 0 && tx == 0 && ty == 0 && (bz % nz) == 0) ampscale[b] = dV / (kScaleA * s);
+}
+
+cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_maxbits, float *d_ampscale,
+                          __half *d_B, cudaStream_t st) {
+    dim3 grid((unsigned)(p.batch * p.nz), p.nx_pad / 32, p.ny_pad / 32);
+    pack_b_kernel<<<grid, dim3(32, 8), 0, st>>>((const float2 *)d_rho, p.nx, p.ny, p.nz, p.nx_pad, p.ny_pad,
+                                                d_maxbits, d_ampscale, (float)(p.dx * p.dy * p.dz), d_B);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a3
+// Phase tables (Eq. 2's split), phases formed and evaluated in FP64 (R-precision):
+//   A planes  fp16 [4][npix_pad][ny_pad]  = split(2^10 e^{i qy(p) y_i})   (the UMMA A operand)
+//   anchor    float2 [tile][nxa][128]     = e^{i qx(p) x_{16 a}}
+//   fine      float2 [tile][16][128]      = e^{i qx(p) b dx}
+//   mz        float2 [tile][nz][128]      = e^{i qz(p) z_j}
+__global__ void table_a_kernel(const double *__restrict__ q, int64_t npix, int64_t npix_pad, int ny, int ny_pad,
+                               double dy, __half *__restrict__ A) {
+    const int y = blockIdx.y * blockDim.x + threadIdx.x;
+    const int64_t p = blockIdx.x;
+    if (y >= ny_pad) return;
+    float re = 0.f, im = 0.f;
+    if (p < npix && y < ny) {
+        double s, c;
+        sincos(q[3 * p + 1] * centre(y, ny, dy), &s, &c);
+        re = (float)(c * (double)kScaleA);
+        im = (float)(s * (double)kScaleA);
+    }
+    const __half reh = __float2half_rn(re), imh = __float2half_rn(im);
+    const __half rel = __float2half_rn(re - __half2float(reh)), iml = __float2half_rn(im - __half2float(imh));
+    const size_t plane = (size_t)npix_pad * ny_pad, o = (size_t)p * ny_pad + y;
+    A[o] = reh;
+    A[plane + o] = rel;
+    A[2 * plane + o] = imh;
+    A[3 * plane + o] = iml;
+}
+
+// which: 0 anchor (count nxa, coord = centre(16 a)), 1 fine (count 16, coord = b dx), 2 mz (count nz)
+__global__ void table_small_kernel(const double *__restrict__ q, int64_t npix, int which, int count, int n, double d,
+                                   float2 *__restrict__ out) {
+    const int lane = threadIdx.x;  // 128
+    const int idx = blockIdx.y, tile = blockIdx.x;
+    const int64_t p = (int64_t)tile * kTileP + lane;
+    float2 v = make_float2(1.f, 0.f);
+    if (p < npix) {
+        double coord, qq;
+        if (which == 0) { coord = centre(idx * kFine, n, d); qq = q[3 * p + 0]; }
+        else if (which == 1) { coord = (double)idx * d; qq = q[3 * p + 0]; }
+        else { coord = centre(idx, n, d); qq = q[3 * p + 2]; }
+        double s, c;
+        sincos(qq * coord, &s, &c);
+        v = make_float2((float)c, (float)s);
+    }
+    out[((size_t)tile * count + idx) * kTileP + lane] = v;
+}
+
+cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
+                          float2 *d_mz, cudaStream_t st, int *nlaunch) {
+    dim3 ga((unsigned)p.npix_pad, (p.ny_pad + 63) / 64);
+    table_a_kernel<<<ga, 64, 0, st>>>(d_q, p.npix, p.npix_pad, p.ny, p.ny_pad, p.dy, d_A);
+    table_small_kernel<<<dim3(p.ntiles, p.nxa), kTileP, 0, st>>>(d_q, p.npix, 0, p.nxa, p.nx, p.dx, d_anchor);
+    table_small_kernel<<<dim3(p.ntiles, kFine), kTileP, 0, st>>>(d_q, p.npix, 1, kFine, p.nx, p.dx, d_fine);
+    table_small_kernel<<<dim3(p.ntiles, p.nz), kTileP, 0, st>>>(d_q, p.npix, 2, p.nz, p.nz, p.dz, d_mz);
+    if (nlaunch) *nlaunch += 4;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ |A|^2
+// Block 11: I = |sum of the partial amplitudes|^2 with the amplitude scale undone.
+// partial float2 [b][nsplit][npix_pad]; ampscale[b] (device) or NULL -> dV.
+__global__ void finalize_kernel(const float2 *__restrict__ partial, int64_t npix, int64_t npix_pad, int nsplit,
+                                const float *__restrict__ ampscale, float dV, float *__restrict__ I) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (p >= npix) return;
+    float re = 0.f, im = 0.f;
+    for (int g = 0; g < nsplit; ++g) {
+        const float2 v = partial[((size_t)b * nsplit + g) * npix_pad + p];
+        re += v.x;
+        im += v.y;
+    }
+    const float s = ampscale ? ampscale[b] : dV;
+    re *= s;
+    im *= s;
+    I[(size_t)b * npix + p] = re * re + im * im;
+}
+
+cudaError_t launch_finalize(const float2 *d_partial, const Plan &p, const float *d_ampscale, double dV, float *d_I,
+                            cudaStream_t st) {
+    dim3 grid((unsigned)((p.npix + 255) / 256), p.batch);
+    finalize_kernel<<<grid, 256, 0, st>>>(d_partial, p.npix, p.npix_pad, p.nsplit, d_ampscale, (float)dV, d_I);
+    return cudaGetLastError();
+}
+
+}  // namespace scatman

@@ -1,0 +1,322 @@
+// tensor_kernel.cu -- steps a4 + a5 + a6: the per-slice contraction on tcgen05 tensor cores with the fused
+// slice-phase / accumulate epilogue (north_star (3), (4), (5); Eq. 2/9; Blocks 6-8,
+// PAPER.md:154-160).
+//
+// Per work item a CTA owns 128 pixels (UMMA M) and one y-group (<= 128 y).  For every slice j and x-tile
+// (128 x = UMMA N) it forms, in TMEM (FP32),
+//     G_re[p,x] = sum_y  My_re[p,y] Rre_j[y,x] - My_im[p,y] Rim_j[y,x]
+//     G_im[p,x] = sum_y  My_re[p,y] Rim_j[y,x] + My_im[p,y] Rre_j[y,x]
+// where every FP32 factor is split into FP16 hi + lo and the product is AhBh + AlBh + AhBl (FP16x3;
+// the minus sign is the instruction descriptor's negate-A bit).  The epilogue warps then read the
+// accumulators (tcgen05.ld) and reduce them over x against e^{i qx x} = anchor[x/16] * fine[x%16],
+// multiply by e^{i qz z_j} and accumulate over slices in FP32 registers (the fused epilogue).
+//
+// Roles: warp 0 lane 0 = TMA producer, warp 1 lane 0 = MMA issuer, warp 2 = TMEM allocator,
+// warps 4-7 = epilogue (TMEM lane group = warp % 4).  Pipelines: A-resident (a_full/a_empty),
+// B ring of kStagesB 16-KB slots (b_full/b_empty), two TMEM accumulator buffers (t_full/t_empty).
+#include <cuda.h>
+
+#include "internal.h"
+#include "ptx_sm100.h"
+
+namespace scatman {
+
+constexpr int kStagesB = 6;
+constexpr int kSlotBytes = kTileP * kBlockY * 2;            // 16384: 128 rows x 128 bytes
+constexpr int kSmemA = 4 * kGroupYB * kSlotBytes;           // 131072
+constexpr int kSmemB = kStagesB * kSlotBytes;               // 98304
+constexpr int kSmemBar = 256;
+constexpr int kSmemTotal = 1024 + kSmemA + kSmemB + kSmemBar;  // + alignment slack
+constexpr int kThreads = 256;
+constexpr uint32_t kTmemCols = 512;
+
+size_t tensor_smem_bytes() { return kSmemTotal; }
+
+struct TensorParams {
+    int nz, nxt, nyb, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
+    int64_t npix_pad;
+    const float2 *anchor, *fine, *mz;
+    float2 *partial;
+};
+
+struct Item {
+    int c, s, g, t;
+};
+__device__ __forceinline__ Item decode_item(int item, const TensorParams &P) {
+    Item it;
+    it.t = item % P.ntiles;
+    item /= P.ntiles;
+    it.g = item % P.ngroups;
+    item /= P.ngroups;
+    it.s = item % P.nzs;
+    it.c = item / P.nzs;
+    return it;
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                     const TensorParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sA = smem;
+    uint8_t *sB = smem + kSmemA;
+    uint64_t *bars = (uint64_t *)(smem + kSmemA + kSmemB);
+    uint64_t *a_full = bars + 0, *a_empty = bars + 1;
+    uint64_t *b_full = bars + 2, *b_empty = bars + 2 + kStagesB;
+    uint64_t *t_full = bars + 2 + 2 * kStagesB, *t_empty = t_full + 2;
+    uint32_t *tmem_ptr = (uint32_t *)(t_empty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nitems = P.nchunks * P.nzs * P.ngroups * P.ntiles;
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(a_full, 1);
+        ptx::mbar_init(a_empty, 1);
+        for (int i = 0; i < kStagesB; ++i) {
+            ptx::mbar_init(b_full + i, 1);
+            ptx::mbar_init(b_empty + i, 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_empty + i, 4);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemCols);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            // ===================================================================== TMA producer
+            int slot = 0;
+            uint32_t phase = 0;
+            int it_local = 0;
+            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+                const Item it = decode_item(item, P);
+                const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
+                ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
+                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(4 * nybg * kSlotBytes));
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int yb = 0; yb < nybg; ++yb)
+                        ptx::tma_load_3d(sA + (pl * kGroupYB + yb) * kSlotBytes, &tmA, a_full,
+                                         (it.g * kGroupYB + yb) * kBlockY, it.t * kTileP, pl);
+                const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
+                const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+                for (int b = b0; b < b1; ++b)
+                    for (int j = z0; j < z1; ++j)
+                        for (int xt = 0; xt < P.nxt; ++xt)
+                            for (int yb = 0; yb < nybg; ++yb)
+                                for (int pl = 0; pl < 4; ++pl) {
+                                    ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                                    ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
+                                    ptx::tma_load_3d(sB + slot * kSlotBytes, &tmB, b_full + slot,
+                                                     (it.g * kGroupYB + yb) * kBlockY, xt * kTileX,
+                                                     (b * P.nz + j) * 4 + pl);
+                                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        if (lane == 0) {
+            // ===================================================================== MMA issuer
+            constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP, kTileX, false);
+            constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP, kTileX, true);
+            const uint32_t sA_u32 = ptx::smem_u32(sA), sB_u32 = ptx::smem_u32(sB);
+            int slot = 0;
+            uint32_t phase = 0;
+            uint32_t u = 0;
+            int it_local = 0;
+            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+                const Item it = decode_item(item, P);
+                const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
+                const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
+                const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+                const int nunits = (b1 - b0) * (z1 - z0) * P.nxt;
+                ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+                ptx::tc_fence_after();
+                for (int unit = 0; unit < nunits; ++unit, ++u) {
+                    const uint32_t buf = u & 1;
+                    ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1);
+                    ptx::tc_fence_after();
+                    const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                    for (int yb = 0; yb < nybg; ++yb) {
+                        // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
+                        const uint64_t a_reh = ptx::umma_smem_desc_sw128(sA_u32 + (0 * kGroupYB + yb) * kSlotBytes);
+                        const uint64_t a_rel = ptx::umma_smem_desc_sw128(sA_u32 + (1 * kGroupYB + yb) * kSlotBytes);
+                        const uint64_t a_imh = ptx::umma_smem_desc_sw128(sA_u32 + (2 * kGroupYB + yb) * kSlotBytes);
+                        const uint64_t a_iml = ptx::umma_smem_desc_sw128(sA_u32 + (3 * kGroupYB + yb) * kSlotBytes);
+                        for (int pl = 0; pl < 4; ++pl) {
+                            ptx::mbar_wait(b_full + slot, phase);
+                            ptx::tc_fence_after();
+                            const uint64_t bd = ptx::umma_smem_desc_sw128(sB_u32 + slot * kSlotBytes);
+#pragma unroll
+                            for (int k = 0; k < kBlockY / 16; ++k) {
+                                const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
+                                const uint32_t acc0 = (yb | k) != 0 ? 1u : 0u;
+                                if (pl == 0) {         // B = Re_hi
+                                    ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
+                                    ptx::umma_f16(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
+                                    ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
+                                    ptx::umma_f16(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
+                                } else if (pl == 1) {  // B = Re_lo
+                                    ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
+                                    ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
+                                } else if (pl == 2) {  // B = Im_hi
+                                    ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                                    ptx::umma_f16(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
+                                    ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                                    ptx::umma_f16(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
+                                } else {               // B = Im_lo
+                                    ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                                    ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                                }
+                            }
+                            ptx::umma_commit(b_empty + slot);
+                            if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                        }
+                    }
+                    ptx::umma_commit(t_full + buf);
+                }
+                ptx::umma_commit(a_empty);
+            }
+        }
+        __syncwarp();
+    } else if (warp >= 4) {
+        // ========================================================================= epilogue
+        const int ew = warp & 3;
+        const int el = ew * 32 + lane;  // pixel within the tile = TMEM lane
+        const uint32_t lane_base = tmem_base + ((uint32_t)(ew * 32) << 16);
+        uint32_t u = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            const Item it = decode_item(item, P);
+            const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
+            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+            float2 fine[kFine];
+#pragma unroll
+            for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)it.t * kFine + i) * kTileP + el);
+            const float2 *anchor_t = P.anchor + (size_t)it.t * P.nxa * kTileP + el;
+            const float2 *mz_t = P.mz + (size_t)it.t * P.nz * kTileP + el;
+            for (int b = b0; b < b1; ++b) {
+                float acc_re = 0.f, acc_im = 0.f;
+                for (int j = z0; j < z1; ++j) {
+                    const float2 mz = __ldg(mz_t + (size_t)j * kTileP);
+                    float f_re = 0.f, f_im = 0.f;
+                    for (int xt = 0; xt < P.nxt; ++xt, ++u) {
+                        const uint32_t buf = u & 1;
+                        float2 anc[kTileX / kFine];
+#pragma unroll
+                        for (int a = 0; a < kTileX / kFine; ++a)
+                            anc[a] = __ldg(anchor_t + (size_t)(xt * (kTileX / kFine) + a) * kTileP);
+                        ptx::mbar_wait(t_full + buf, (u >> 1) & 1);
+                        ptx::tc_fence_after();
+                        const uint32_t t_re = lane_base + buf * 256, t_im = t_re + 128;
+#pragma unroll
+                        for (int a = 0; a < kTileX / kFine; ++a) {
+                            uint32_t gre[16], gim[16];
+                            ptx::tmem_ld16(t_re + a * kFine, gre);
+                            ptx::tmem_ld16(t_im + a * kFine, gim);
+                            ptx::tmem_ld_wait();
+                            float s_re = 0.f, s_im = 0.f;
+#pragma unroll
+                            for (int i = 0; i < kFine; ++i) {
+                                const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
+                                s_re = fmaf(fine[i].x, gr, s_re);
+                                s_re = fmaf(-fine[i].y, gi, s_re);
+                                s_im = fmaf(fine[i].x, gi, s_im);
+                                s_im = fmaf(fine[i].y, gr, s_im);
+                            }
+                            f_re = fmaf(anc[a].x, s_re, f_re);
+                            f_re = fmaf(-anc[a].y, s_im, f_re);
+                            f_im = fmaf(anc[a].x, s_im, f_im);
+                            f_im = fmaf(anc[a].y, s_re, f_im);
+                        }
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                    }
+                    acc_re = fmaf(mz.x, f_re, acc_re);
+                    acc_re = fmaf(-mz.y, f_im, acc_re);
+                    acc_im = fmaf(mz.x, f_im, acc_im);
+                    acc_im = fmaf(mz.y, f_re, acc_im);
+                }
+                P.partial[((size_t)b * (P.ngroups * P.nzs) + (it.g * P.nzs + it.s)) * P.npix_pad +
+                          (size_t)it.t * kTileP + el] = make_float2(acc_re, acc_im);
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kTmemCols);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+static bool encode_planes(CUtensorMap *tm, const void *base, uint64_t inner, uint64_t rows, uint64_t planes,
+                          uint32_t box_rows) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {inner, rows, planes};
+    cuuint64_t strides[2] = {inner * 2, inner * rows * 2};
+    cuuint32_t box[3] = {(cuuint32_t)kBlockY, box_rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void *>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st, std::string *err) {
+    CUtensorMap tmA, tmB;
+    if (!encode_planes(&tmA, t.d_A, (uint64_t)p.ny_pad, (uint64_t)p.npix_pad, 4, kTileP) ||
+        !encode_planes(&tmB, t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4, kTileX)) {
+        if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
+        return cudaErrorUnknown;
+    }
+    TensorParams P;
+    P.nz = p.nz; P.nxt = p.nxt; P.nyb = p.nyb; P.ngroups = p.ngroups; P.ntiles = p.ntiles; P.batch = p.batch;
+    P.nzs = p.t_nzs;
+    P.bpc = (p.batch + p.t_nchunks - 1) / p.t_nchunks;
+    P.nchunks = (p.batch + P.bpc - 1) / P.bpc;
+    P.nxa = p.nxa;
+    P.npix_pad = p.npix_pad;
+    P.anchor = t.d_anchor; P.fine = t.d_fine; P.mz = t.d_mz; P.partial = t.d_partial;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(msft_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             kSmemTotal);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int nitems = P.nchunks * P.nzs * P.ngroups * P.ntiles;
+    const int grid = nitems < t.num_sms ? nitems : t.num_sms;
+    msft_contract_kernel<<<grid, kThreads, kSmemTotal, st>>>(tmA, tmB, P);
+    return cudaGetLastError();
+}
+
+}  // namespace scatman
