@@ -1,0 +1,273 @@
+#!/usr/bin/env python
+"""bench.py -- MSFT patterns/s on B200 (BASELINE.json metric), one JSON line.
+
+A "step" is one pass of the whole hot path (a0-a6: q-map, [orient], column prefix, operand pack, phase
+tables, tcgen05 contraction with fused epilogue, |A|^2) over one batch of synthetic input through the
+C ABI (scatman_simulate).  Default workload = BASELINE.json configs[2], the 256^3 / 512x512 droplet on
+which north_star quotes its target.  `--impl reference` times the FP64 CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SPLITS = 3           # FP16x3: AhBh + AlBh + AhBl
+FLOP_PER_TERM = 8    # one complex MAC
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return {"burst": float(p["bf16_tflops"]), "sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                "source": "measured"}
+    except Exception:
+        return {"burst": 1590.0, "sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        load = [v for v in sm if mx and v > 0.3 * mx] or sm
+        med = load[len(load) // 2] if load else None
+        return {"sm_mhz": med, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def workload_for(args):
+    from paper_2202_03411_b200 import workloads as W
+    w = W.config(args.config)
+    items = list(range(w.batch if args.batch <= 0 else min(args.batch, w.batch)))
+    return w, items
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores, on a bounded pixel sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    from oracle import oracle as O
+    from paper_2202_03411_b200 import workloads as W
+    w, items = workload_for(args)
+    g = w.grid(0)
+    quat = None if w.quat is None else w.quat[0]
+    vox = (w.dx, w.dy, w.dz)
+    npix_s = max(8, int(args.ref_pixels))
+    pix = W.sample_pixels(w.seed, w.npix, npix_s)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        O.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, pixels=pix)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+    total = sum(times)
+    frac = len(pix) / w.npix                      # of one pattern per step
+    value = frac * len(times) / total             # patterns/s, exact extrapolation (work is linear in pixels)
+    cores = O.num_threads()
+    sample = f"{len(pix)} seeded pixels of one {w.name} pattern per step ({frac:.3e} of a pattern)"
+    line = {"impl": "reference", "metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": 1},
+            "terms_per_s": value * w.nvox * w.npix,
+            "cpu_baseline": {"value": value, "unit": "patterns/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "patterns/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: 256^3 / 512x512)")
+    ap.add_argument("--batch", type=int, default=0, help="limit the batch of config 3 (0 = all)")
+    ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos")
+    ap.add_argument("--ref-pixels", type=int, default=384, help="pixels per step of the CPU oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import numpy as np
+    import torch
+    from paper_2202_03411_b200 import binding as B, build as lib_build
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    if rank == 0:
+        lib_build.build()
+    if dist:
+        dist.barrier()
+    sm = B.Scatman(local)
+
+    w, items = workload_for(args)
+    vox = (w.dx, w.dy, w.dz)
+    # weak scaling: every rank simulates its own replica of the batch (shapes shard with no collective)
+    g = w.grids(items)
+    quat = None if w.quat is None else w.quat[items]
+    batch = len(items)
+    d_dn = torch.from_numpy(g).cuda()
+    grid = B.Grid(w.nx, w.ny, w.nz, *vox)
+    opts = B.Options(0, args.method, 0, 0)
+    ws = torch.empty(sm.workspace_bytes(grid, w.npix, batch, opts), dtype=torch.uint8, device="cuda")
+    out = torch.empty((batch, w.npy, w.npx), dtype=torch.float32, device="cuda")
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
+                    workspace=ws, out=out, stream=stream)
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kernel_ms, launches = [], 0
+    torch.cuda.synchronize()
+    for i in range(args.steps):
+        flush.zero_()                      # L2 flush, outside the timed events
+        ev[i][0].record(stream)
+        step()
+        ev[i][1].record(stream)
+        launches += sm.last_launch_count()
+        kernel_ms.append(sm.last_contraction_ms())   # events on the launch stream; waits for this step
+    torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if dist:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+
+    # end to end through the host-buffer C entry point: pinned host grid in, pinned host intensity out
+    h_dn = torch.from_numpy(g).pin_memory()
+    h_I = torch.empty((batch, w.npy, w.npx), dtype=torch.float32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+    e2e_s = time.perf_counter() - t0
+    if dist:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    if rank != 0:
+        return
+
+    patterns = batch * args.steps * world
+    value = patterns / (total_ms * 1e-3)
+    terms_per_pattern = w.nvox * w.npix
+    peaks = load_peaks()
+    k_ms = sum(kernel_ms) / len(kernel_ms)
+    issued = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch          # tensor flop per contraction launch
+    achieved = issued / (k_ms * 1e-3) / 1e12
+    if args.method == 1:
+        roofline = {"bound": "tensor", "kernel": "msft_contract_kernel", "achieved": achieved, "peak": peaks["sustained"],
+                    "unit": "TFLOP/s", "frac": achieved / peaks["sustained"], "traffic": None,
+                    "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
+                    "useful_tflops": achieved / SPLITS, "kernel_ms": k_ms, "kernel_share_of_step": k_ms * args.steps / total_ms * world / world}
+    else:
+        # direct sincos: 2 MUFU per term; SFU peak = 148 SMs x 16 MUFU/clk x max clock
+        peak = 148 * 16 * 1.965e9 / 2 / 1e12
+        ach = terms_per_pattern * batch / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "simt_sincos_kernel", "achieved": ach, "peak": peak, "unit": "Tterm/s",
+                    "frac": ach / peak, "traffic": None, "kernel_ms": k_ms}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        from paper_2202_03411_b200 import workloads as W
+        pix = W.sample_pixels(w.seed, w.npix, args.ref_pixels)
+        t0 = time.perf_counter()
+        ref = O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=pix)
+        dt = time.perf_counter() - t0
+        got = out[0].flatten()[torch.from_numpy(pix).cuda()].cpu().numpy().astype(np.float64)
+        rel = float(np.sqrt(np.sum((got - ref) ** 2) / np.sum(ref ** 2)))
+        m = ref > 1e-6 * ref.max()
+        pixerr = float(np.max(np.abs(got[m] - ref[m]) / ref[m]))
+        cpu = {"value": (len(pix) / w.npix) / dt, "unit": "patterns/s", "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"{len(pix)} seeded pixels of item 0 of {w.name} ({dt:.1f} s)",
+               "terms_per_s": w.nvox * len(pix) / dt, "parity_rel_l2": rel, "parity_max_pixel_rel": pixerr}
+
+    line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "fp16x3 split (fp32 accumulate)" if args.method == 1 else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "method": {1: "tensor", 2: "simt_sincos"}[args.method],
+                       "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
+            "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
+            "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
+                    "h2d_bytes_per_step": int(h_dn.numel() * 4), "d2h_bytes_per_step": int(h_I.numel() * 4)},
+            "gpu_launches": launches, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()
