@@ -91,105 +91,149 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tmem_base = *tmem_ptr;
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);  // provably warp-uniform
 
     if (warp == 0) {
-        if (lane == 0) {
-            // ===================================================================== TMA producer
-            int slot = 0;
-            uint32_t phase = 0;
-            int it_local = 0;
-            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-                const Item it = decode_item(item, P);
-                const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
-                ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
+        // ===================================================================== TMA producer
+        // The whole warp walks the loop (warp-uniform control flow); one elected lane issues.
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const Item it = decode_item(item, P);
+            const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
+            ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
                 ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(4 * nybg * kSlotBytes));
                 for (int pl = 0; pl < 4; ++pl)
                     for (int yb = 0; yb < nybg; ++yb)
                         ptx::tma_load_3d(sA + (pl * kGroupYB + yb) * kSlotBytes, &tmA, a_full,
                                          (it.g * kGroupYB + yb) * kBlockY, it.t * kTileP, pl);
-                const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
-                const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
-                for (int b = b0; b < b1; ++b)
-                    for (int j = z0; j < z1; ++j)
-                        for (int xt = 0; xt < P.nxt; ++xt)
-                            for (int yb = 0; yb < nybg; ++yb)
-                                for (int pl = 0; pl < 4; ++pl) {
-                                    ptx::mbar_wait(b_empty + slot, phase ^ 1);
+            }
+            __syncwarp();
+            const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
+            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+            for (int b = b0; b < b1; ++b)
+                for (int j = z0; j < z1; ++j)
+                    for (int xt = 0; xt < P.nxt; ++xt)
+                        for (int yb = 0; yb < nybg; ++yb)
+                            for (int pl = 0; pl < 4; ++pl) {
+                                ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                                if (ptx::elect_one()) {
                                     ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
                                     ptx::tma_load_3d(sB + slot * kSlotBytes, &tmB, b_full + slot,
                                                      (it.g * kGroupYB + yb) * kBlockY, xt * kTileX,
                                                      (b * P.nz + j) * 4 + pl);
-                                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                                 }
-            }
-        }
-        __syncwarp();
-    } else if (warp == 1) {
-        if (lane == 0) {
-            // ===================================================================== MMA issuer
-            constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP, kTileX, false);
-            constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP, kTileX, true);
-            const uint32_t sA_u32 = ptx::smem_u32(sA), sB_u32 = ptx::smem_u32(sB);
-            int slot = 0;
-            uint32_t phase = 0;
-            uint32_t u = 0;
-            int it_local = 0;
-            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-                const Item it = decode_item(item, P);
-                const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
-                const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
-                const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
-                const int nunits = (b1 - b0) * (z1 - z0) * P.nxt;
-                ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
-                ptx::tc_fence_after();
-                for (int unit = 0; unit < nunits; ++unit, ++u) {
-                    const uint32_t buf = u & 1;
-                    ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1);
-                    ptx::tc_fence_after();
-                    const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                    for (int yb = 0; yb < nybg; ++yb) {
-                        // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
-                        const uint64_t a_reh = ptx::umma_smem_desc_sw128(sA_u32 + (0 * kGroupYB + yb) * kSlotBytes);
-                        const uint64_t a_rel = ptx::umma_smem_desc_sw128(sA_u32 + (1 * kGroupYB + yb) * kSlotBytes);
-                        const uint64_t a_imh = ptx::umma_smem_desc_sw128(sA_u32 + (2 * kGroupYB + yb) * kSlotBytes);
-                        const uint64_t a_iml = ptx::umma_smem_desc_sw128(sA_u32 + (3 * kGroupYB + yb) * kSlotBytes);
-                        for (int pl = 0; pl < 4; ++pl) {
-                            ptx::mbar_wait(b_full + slot, phase);
-                            ptx::tc_fence_after();
-                            const uint64_t bd = ptx::umma_smem_desc_sw128(sB_u32 + slot * kSlotBytes);
-#pragma unroll
-                            for (int k = 0; k < kBlockY / 16; ++k) {
-                                const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
-                                const uint32_t acc0 = (yb | k) != 0 ? 1u : 0u;
-                                if (pl == 0) {         // B = Re_hi
-                                    ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
-                                    ptx::umma_f16(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
-                                    ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
-                                    ptx::umma_f16(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
-                                } else if (pl == 1) {  // B = Re_lo
-                                    ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
-                                    ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
-                                } else if (pl == 2) {  // B = Im_hi
-                                    ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                                    ptx::umma_f16(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
-                                    ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                                    ptx::umma_f16(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
-                                } else {               // B = Im_lo
-                                    ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                                    ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                                }
+                                __syncwarp();
+                                if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                             }
-                            ptx::umma_commit(b_empty + slot);
-                            if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                        }
-                    }
-                    ptx::umma_commit(t_full + buf);
-                }
-                ptx::umma_commit(a_empty);
-            }
         }
-        __syncwarp();
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer
+        // Warp-uniform loop; descriptors are uniform-register arithmetic; one elected lane issues the
+        // tcgen05.mma / tcgen05.commit instructions.
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP, kTileX, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP, kTileX, true);
+        const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
+        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
+        constexpr uint64_t kSlotDesc = kSlotBytes >> 4;
+        int slot = 0;
+        uint32_t phase = 0;
+        uint32_t u = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const Item it = decode_item(item, P);
+            const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
+            const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
+            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+            const int nunits = (b1 - b0) * (z1 - z0) * P.nxt;
+            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+            ptx::tc_fence_after();
+            for (int unit = 0; unit < nunits; ++unit, ++u) {
+                const uint32_t buf = u & 1;
+                ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                for (int yb = 0; yb < nybg; ++yb) {
+                    // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
+                    const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDesc;
+                    const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDesc;
+                    const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDesc;
+                    const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDesc;
+                    const uint32_t first = yb != 0 ? 1u : 0u;
+                    // ---- B = Re_hi
+                    ptx::mbar_wait(b_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+#pragma unroll
+                        for (int k = 0; k < kBlockY / 16; ++k) {
+                            const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
+                            const uint32_t acc0 = k != 0 ? 1u : first;
+                            ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
+                            ptx::umma_f16(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
+                            ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
+                            ptx::umma_f16(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
+                        }
+                        ptx::umma_commit(b_empty + slot);
+                    }
+                    __syncwarp();
+                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                    // ---- B = Re_lo
+                    ptx::mbar_wait(b_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+#pragma unroll
+                        for (int k = 0; k < kBlockY / 16; ++k) {
+                            const uint64_t ko = (uint64_t)(k * 2);
+                            ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
+                        }
+                        ptx::umma_commit(b_empty + slot);
+                    }
+                    __syncwarp();
+                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                    // ---- B = Im_hi
+                    ptx::mbar_wait(b_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+#pragma unroll
+                        for (int k = 0; k < kBlockY / 16; ++k) {
+                            const uint64_t ko = (uint64_t)(k * 2);
+                            ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                            ptx::umma_f16(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
+                            ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            ptx::umma_f16(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
+                        }
+                        ptx::umma_commit(b_empty + slot);
+                    }
+                    __syncwarp();
+                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                    // ---- B = Im_lo
+                    ptx::mbar_wait(b_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+#pragma unroll
+                        for (int k = 0; k < kBlockY / 16; ++k) {
+                            const uint64_t ko = (uint64_t)(k * 2);
+                            ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                            ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                        }
+                        ptx::umma_commit(b_empty + slot);
+                    }
+                    __syncwarp();
+                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                }
+                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                __syncwarp();
+            }
+            if (ptx::elect_one()) ptx::umma_commit(a_empty);
+            __syncwarp();
+        }
     } else if (warp >= 4) {
         // ========================================================================= epilogue
         const int ew = warp & 3;
