@@ -99,7 +99,13 @@ def run_reference(args):
     g = w.grid(0)
     quat = None if w.quat is None else w.quat[0]
     vox = (w.dx, w.dy, w.dz)
-    npix_s = max(8, int(args.ref_pixels))
+    if args.ref_pixels > 0:
+        npix_s = max(8, int(args.ref_pixels))
+    else:   # ~10 s per step from a short probe
+        probe = W.sample_pixels(w.seed + 99, w.npix, 32)
+        t0 = time.perf_counter()
+        O.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, pixels=probe)
+        npix_s = int(min(8192, max(128, 10.0 / ((time.perf_counter() - t0) / len(probe)))))
     pix = W.sample_pixels(w.seed, w.npix, npix_s)
     times = []
     for i in range(args.warmup + args.steps):
@@ -133,7 +139,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: 256^3 / 512x512)")
     ap.add_argument("--batch", type=int, default=0, help="limit the batch of config 3 (0 = all)")
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos")
-    ap.add_argument("--ref-pixels", type=int, default=384, help="pixels per step of the CPU oracle sample")
+    ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -160,7 +166,11 @@ def main():
 
     w, items = workload_for(args)
     vox = (w.dx, w.dy, w.dz)
-    # weak scaling: every rank simulates its own replica of the batch (shapes shard with no collective)
+    # weak scaling: the global job is `world` copies of the batch; shapes shard across ranks with no collective
+    from paper_2202_03411_b200.sharding import shard_range
+    global_items = [i for _ in range(world) for i in items]
+    lo, hi = shard_range(len(global_items), rank, world)
+    items = global_items[lo:hi]
     g = w.grids(items)
     quat = None if w.quat is None else w.quat[items]
     batch = len(items)
@@ -244,7 +254,13 @@ def main():
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         from paper_2202_03411_b200 import workloads as W
-        pix = W.sample_pixels(w.seed, w.npix, args.ref_pixels)
+        # size the sample for ~15 s of host-core work from a short probe
+        probe = W.sample_pixels(w.seed + 99, w.npix, 32)
+        t0 = time.perf_counter()
+        O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=probe)
+        per_pixel = (time.perf_counter() - t0) / len(probe)
+        npix_s = args.ref_pixels if args.ref_pixels > 0 else int(min(8192, max(256, 15.0 / per_pixel)))
+        pix = W.sample_pixels(w.seed, w.npix, npix_s)
         t0 = time.perf_counter()
         ref = O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=pix)
         dt = time.perf_counter() - t0
