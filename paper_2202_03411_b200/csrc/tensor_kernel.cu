@@ -32,6 +32,16 @@ constexpr uint32_t kTmemCols = 512;
 
 size_t tensor_smem_bytes() { return kSmemTotal; }
 
+#ifdef SCATMAN_TIMING
+// debug-only cycle accounting (built by _work scripts with -DSCATMAN_TIMING; never in the product build)
+__device__ long long g_timing[148 * 8];
+#define TIMING_DECL(name) long long name = 0
+#define TIMED_WAIT(acc, stmt) do { long long _t0 = clock64(); stmt; acc += clock64() - _t0; } while (0)
+#else
+#define TIMING_DECL(name)
+#define TIMED_WAIT(acc, stmt) stmt
+#endif
+
 struct TensorParams {
     int nz, nxt, nyb, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
     int64_t npix_pad;
@@ -142,17 +152,21 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         uint32_t phase = 0;
         uint32_t u = 0;
         int it_local = 0;
+        TIMING_DECL(w_tempty); TIMING_DECL(w_bfull); TIMING_DECL(w_afull);
+#ifdef SCATMAN_TIMING
+        const long long t_begin = clock64();
+#endif
         for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
             const Item it = decode_item(item, P);
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
             const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
             const int nunits = (b1 - b0) * (z1 - z0) * P.nxt;
-            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+            TIMED_WAIT(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
             ptx::tc_fence_after();
             for (int unit = 0; unit < nunits; ++unit, ++u) {
                 const uint32_t buf = u & 1;
-                ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1);
+                TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1));
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                 for (int yb = 0; yb < nybg; ++yb) {
@@ -163,7 +177,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDesc;
                     const uint32_t first = yb != 0 ? 1u : 0u;
                     // ---- B = Re_hi
-                    ptx::mbar_wait(b_full + slot, phase);
+                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
                         const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
@@ -181,7 +195,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     // ---- B = Re_lo
-                    ptx::mbar_wait(b_full + slot, phase);
+                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
                         const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
@@ -196,7 +210,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     // ---- B = Im_hi
-                    ptx::mbar_wait(b_full + slot, phase);
+                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
                         const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
@@ -213,7 +227,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     // ---- B = Im_lo
-                    ptx::mbar_wait(b_full + slot, phase);
+                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
                         const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
@@ -234,12 +248,24 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             if (ptx::elect_one()) ptx::umma_commit(a_empty);
             __syncwarp();
         }
+#ifdef SCATMAN_TIMING
+        if (lane == 0) {
+            g_timing[blockIdx.x * 8 + 0] = clock64() - t_begin;
+            g_timing[blockIdx.x * 8 + 1] = w_tempty;
+            g_timing[blockIdx.x * 8 + 2] = w_bfull;
+            g_timing[blockIdx.x * 8 + 3] = w_afull;
+        }
+#endif
     } else if (warp >= 4) {
         // ========================================================================= epilogue
         const int ew = warp & 3;
         const int el = ew * 32 + lane;  // pixel within the tile = TMEM lane
         const uint32_t lane_base = tmem_base + ((uint32_t)(ew * 32) << 16);
         uint32_t u = 0;
+        TIMING_DECL(w_tfull);
+#ifdef SCATMAN_TIMING
+        const long long e_begin = clock64();
+#endif
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             const Item it = decode_item(item, P);
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
@@ -260,7 +286,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #pragma unroll
                         for (int a = 0; a < kTileX / kFine; ++a)
                             anc[a] = __ldg(anchor_t + (size_t)(xt * (kTileX / kFine) + a) * kTileP);
-                        ptx::mbar_wait(t_full + buf, (u >> 1) & 1);
+                        TIMED_WAIT(w_tfull, ptx::mbar_wait(t_full + buf, (u >> 1) & 1));
                         ptx::tc_fence_after();
                         const uint32_t t_re = lane_base + buf * 256, t_im = t_re + 128;
 #pragma unroll
@@ -296,6 +322,13 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                           (size_t)it.t * kTileP + el] = make_float2(acc_re, acc_im);
             }
         }
+#ifdef SCATMAN_TIMING
+        if (warp == 4 && lane == 0) {
+            g_timing[blockIdx.x * 8 + 4] = clock64() - e_begin;
+            g_timing[blockIdx.x * 8 + 5] = w_tfull;
+            g_timing[blockIdx.x * 8 + 6] = u;
+        }
+#endif
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -362,5 +395,12 @@ cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st,
     msft_contract_kernel<<<grid, kThreads, kSmemTotal, st>>>(tmA, tmB, P);
     return cudaGetLastError();
 }
+
+
+#ifdef SCATMAN_TIMING
+extern "C" int scatman_debug_timing(long long *h_out) {
+    return (int)cudaMemcpyFromSymbol(h_out, g_timing, sizeof(long long) * 148 * 8);
+}
+#endif
 
 }  // namespace scatman
