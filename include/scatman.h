@@ -80,8 +80,13 @@ typedef struct {
     int32_t rho_mode;
     int32_t method;
     int32_t precision;
-    uint32_t flags; /* reserved, must be 0 */
+    uint32_t flags; /* SCATMAN_FLAG_* bits; unknown bits are an error */
 } scatman_options;
+
+/* Tensor path only: run the contraction with one CTA per work item (tcgen05 cta_group::1, UMMA 128x128) instead of
+ * the default CTA pairs (cta_group::2, UMMA 256x128, each CTA holding half of every B tile).  Same results up to
+ * summation order; kept for comparison and as the smaller-cluster variant. */
+#define SCATMAN_FLAG_SINGLE_CTA 1u
 
 /* Create / destroy a context on CUDA device `device`.  Fails with SCATMAN_UNSUPPORTED_DEVICE unless the
  * device is compute capability 10.x.  scatman_destroy(NULL) is SCATMAN_OK. */

@@ -17,6 +17,7 @@ OK, INVALID_ARGUMENT, UNSUPPORTED_DEVICE, WORKSPACE_TOO_SMALL, CUDA_ERROR, NOT_I
 RHO_LINEAR, RHO_N2M1 = 0, 1
 METHOD_AUTO, METHOD_TENSOR, METHOD_SIMT_SINCOS, METHOD_SIMT_TABLE = 0, 1, 2, 3
 PRECISION_AUTO, PRECISION_FP16X3 = 0, 1
+FLAG_SINGLE_CTA = 1
 
 EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
@@ -184,13 +185,13 @@ class Scatman:
 
     def simulate(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
                  rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, cx: float = 0.0, cy: float = 0.0,
-                 workspace=None, out=None, stream=None):
+                 workspace=None, out=None, stream=None, flags: int = 0):
         """I float32 [B][npy][npx] on the device ([npy][npx] for a 4-D grid).  Asynchronous."""
         import torch
         self._check_dn(dn)
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
-        opts = Options(int(rho_mode), int(method), 0, 0)
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
         need = self.workspace_bytes(grid, npx * npy, batch, opts)
         if workspace is None:
             workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
@@ -203,7 +204,7 @@ class Scatman:
         return out if dn.dim() == 5 else out[0]
 
     def simulate_q(self, dn, voxel, lam: float, q, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,
-                   workspace=None, out=None, stream=None):
+                   workspace=None, out=None, stream=None, flags: int = 0):
         """I float32 [B][npix] at the explicit device q list [npix][3] (float64)."""
         import torch
         self._check_dn(dn)
@@ -211,7 +212,7 @@ class Scatman:
             raise ValueError("q must be a contiguous CUDA float64 tensor [npix][3]")
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         npix = int(q.shape[0])
-        opts = Options(int(rho_mode), int(method), 0, 0)
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
         need = self.workspace_bytes(grid, npix, batch, opts)
         if workspace is None:
             workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
@@ -225,14 +226,14 @@ class Scatman:
         return out if dn.dim() == 5 else out[0]
 
     def simulate_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
-                      rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None):
+                      rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None, flags: int = 0):
         """Host-buffer end-to-end call: h_dn / h_out are CPU float32 tensors (pinned for speed). Synchronous."""
         import torch
         if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
             raise ValueError("h_dn must be a contiguous CPU float32 tensor")
         grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
         det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
-        opts = Options(int(rho_mode), int(method), 0, 0)
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
         if h_out is None:
             h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
         keep, qp = _quat_arg(quat, batch)

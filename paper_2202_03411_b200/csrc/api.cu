@@ -28,7 +28,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Batch chunks x z splits of the tensor kernel: minimise waves * per-item length (in slices), where an
 // item costs its slices plus ~2 slice-equivalents of fill (A load, pipeline ramp).
-void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs) {
+void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs) {  // num_sms = concurrent workers (CTAs or CTA pairs)
     double best = 1e300;
     int bc = 1, bz = 1;
     const int max_z = p.nz < 16 ? p.nz : 16;
@@ -37,7 +37,7 @@ void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs) {
         const int bpc = (p.batch + c - 1) / c;
         const int cc = (p.batch + bpc - 1) / bpc;
         for (int z = 1; z <= max_z; ++z) {
-            const long long items = (long long)cc * z * p.ngroups * p.ntiles;
+            const long long items = (long long)cc * z * p.ngroups * (p.ntiles / p.t_ncta);
             const long long waves = (items + num_sms - 1) / num_sms;
             const double len = (double)bpc * (double)((p.nz + z - 1) / z) + 2.0;
             const double cost = (double)waves * len;
@@ -62,9 +62,11 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
     p.nxt = p.nx_pad / kTileX;
     p.nxa = p.nx_pad / kFine;
     p.ntiles = (int)((npix + kTileP - 1) / kTileP);
+    p.t_ncta = (o.flags & SCATMAN_FLAG_SINGLE_CTA) ? 1 : 2;
+    if (p.method == SCATMAN_METHOD_TENSOR && p.t_ncta == 2) p.ntiles = (p.ntiles + 1) / 2 * 2;  // whole CTA pairs
     p.npix_pad = (int64_t)p.ntiles * kTileP;
     if (p.method == SCATMAN_METHOD_TENSOR) {
-        tensor_schedule(p, num_sms, &p.t_nchunks, &p.t_nzs);
+        tensor_schedule(p, num_sms / p.t_ncta, &p.t_nchunks, &p.t_nzs);
         p.nsplit = p.ngroups * p.t_nzs;
     } else {
         p.nsplit = simt_zsplit(p, num_sms);
@@ -109,7 +111,7 @@ static bool valid_detector(const scatman_detector *d) {
 }
 static bool valid_options(const scatman_options &o) {
     return (o.rho_mode == SCATMAN_RHO_LINEAR || o.rho_mode == SCATMAN_RHO_N2M1) && o.method >= 0 && o.method <= 3 &&
-           o.precision >= 0 && o.precision <= 1 && o.flags == 0;
+           o.precision >= 0 && o.precision <= 1 && (o.flags & ~(uint32_t)SCATMAN_FLAG_SINGLE_CTA) == 0;
 }
 static bool valid_quats(const double *q, int batch) {
     for (int b = 0; b < batch; ++b) {

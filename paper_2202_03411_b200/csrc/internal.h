@@ -37,13 +37,14 @@ struct Plan {
     int64_t npix_pad = 0;
     int nsplit = 0;               // partial sums per pixel (tensor: ngroups * t_nzs; simt: z splits)
     int t_nchunks = 1, t_nzs = 1; // tensor schedule: batch chunks and z splits per (tile, y-group)
+    int t_ncta = 2;               // CTAs per work item: 2 = cta_group::2 pairs (default), 1 = single CTA
     // workspace offsets (bytes)
     size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
            off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, total = 0;
 };
 
 int simt_zsplit(const Plan &p, int num_sms);
-void tensor_schedule(const Plan &p, int num_sms, int *nchunks, int *nzs);
+void tensor_schedule(const Plan &p, int num_workers, int *nchunks, int *nzs);
 
 // ---- kernels launchers (all asynchronous on `st`; return cudaGetLastError()) -------------------
 cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);

@@ -21,14 +21,14 @@
 
 namespace scatman {
 
-constexpr int kStagesB = 6;
-constexpr int kSlotBytes = kTileP * kBlockY * 2;            // 16384: 128 rows x 128 bytes
-constexpr int kSmemA = 4 * kGroupYB * kSlotBytes;           // 131072
-constexpr int kSmemB = kStagesB * kSlotBytes;               // 98304
-constexpr int kSmemBar = 256;
+constexpr int kSlotBytes = kTileP * kBlockY * 2;            // 16384: 128 rows x 128 bytes (one A K-block; one B tile)
+constexpr int kSmemA = 4 * kGroupYB * kSlotBytes;           // 131072: resident A planes of one pixel tile
+constexpr int kSmemB = 6 * kSlotBytes;                      // 98304: B ring (6 slots of 16 KB, or 12 of 8 KB per CTA of a pair)
+constexpr int kSmemBar = 512;
 constexpr int kSmemTotal = 1024 + kSmemA + kSmemB + kSmemBar;  // + alignment slack
 constexpr int kThreads = 256;
 constexpr uint32_t kTmemCols = 512;
+constexpr int kMaxStagesB = 12;
 
 size_t tensor_smem_bytes() { return kSmemTotal; }
 
@@ -50,12 +50,13 @@ struct TensorParams {
 };
 
 struct Item {
-    int c, s, g, t;
+    int c, s, g, tp;
 };
-__device__ __forceinline__ Item decode_item(int item, const TensorParams &P) {
+// item -> (batch chunk, z split, y group, tile pair); tile pair fastest so concurrent CTAs stream the same B
+__device__ __forceinline__ Item decode_item(int item, const TensorParams &P, int ntp) {
     Item it;
-    it.t = item % P.ntiles;
-    item /= P.ntiles;
+    it.tp = item % ntp;
+    item /= ntp;
     it.g = item % P.ngroups;
     item /= P.ngroups;
     it.s = item % P.nzs;
@@ -63,21 +64,33 @@ __device__ __forceinline__ Item decode_item(int item, const TensorParams &P) {
     return it;
 }
 
+// NCTA = 1: one CTA per work item (cta_group::1, UMMA 128 x 128).
+// NCTA = 2: a CTA pair per work item (cta_group::2, UMMA 256 x 128): each CTA owns its own 128-pixel tile (A resident in
+//           its smem, D in its TMEM, its own epilogue) and HALF of every B tile (64 of the 128 x rows), so the B bytes
+//           fetched and read from shared memory per CTA halve and the ring is twice as deep.  The leader (rank 0)
+//           issues every MMA; full barriers live in the leader, empty barriers are signalled in both CTAs.
+template <int NCTA>
 __global__ void __launch_bounds__(kThreads, 1)
 msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                      const TensorParams P) {
+    constexpr int kStagesB = 6 * NCTA;
+    constexpr int kSlotB = kSlotBytes / NCTA;     // bytes of a B slot in one CTA
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *sA = smem;
     uint8_t *sB = smem + kSmemA;
     uint64_t *bars = (uint64_t *)(smem + kSmemA + kSmemB);
     uint64_t *a_full = bars + 0, *a_empty = bars + 1;
-    uint64_t *b_full = bars + 2, *b_empty = bars + 2 + kStagesB;
-    uint64_t *t_full = bars + 2 + 2 * kStagesB, *t_empty = t_full + 2;
+    uint64_t *b_full = bars + 2, *b_empty = bars + 2 + kMaxStagesB;
+    uint64_t *t_full = bars + 2 + 2 * kMaxStagesB, *t_empty = t_full + 2;
     uint32_t *tmem_ptr = (uint32_t *)(t_empty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nitems = P.nchunks * P.nzs * P.ngroups * P.ntiles;
+    const uint32_t rank = NCTA == 2 ? ptx::cluster_ctarank() : 0u;
+    const int cluster_id = blockIdx.x / NCTA, nclusters = gridDim.x / NCTA;
+    const int ntp = P.ntiles / NCTA;
+    const int nitems = P.nchunks * P.nzs * P.ngroups * ntp;
+    const bool leader = rank == 0;
 
     if (warp == 0 && lane == 0) {
         ptx::tma_prefetch_desc(&tmA);
@@ -92,33 +105,41 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         }
         for (int i = 0; i < 2; ++i) {
             ptx::mbar_init(t_full + i, 1);
-            ptx::mbar_init(t_empty + i, 4);
+            ptx::mbar_init(t_empty + i, 4 * NCTA);
         }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
-    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemCols);
+    if (warp == 2) {
+        if (NCTA == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemCols);
+        else ptx::tmem_alloc(tmem_ptr, kTmemCols);
+    }
     ptx::tc_fence_before();
     __syncthreads();
+    if (NCTA == 2) ptx::cluster_sync_all();   // peer barriers are initialised before anyone signals them
     ptx::tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);  // provably warp-uniform
 
     if (warp == 0) {
-        // ===================================================================== TMA producer
+        // ===================================================================== TMA producer (both CTAs of a pair)
         // The whole warp walks the loop (warp-uniform control flow); one elected lane issues.
         int slot = 0;
         uint32_t phase = 0;
         int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const Item it = decode_item(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const Item it = decode_item(item, P, ntp);
+            const int tile = it.tp * NCTA + (int)rank;
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
             ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
             if (ptx::elect_one()) {
-                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(4 * nybg * kSlotBytes));
+                if (leader) ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(NCTA * 4 * nybg * kSlotBytes));
                 for (int pl = 0; pl < 4; ++pl)
-                    for (int yb = 0; yb < nybg; ++yb)
-                        ptx::tma_load_3d(sA + (pl * kGroupYB + yb) * kSlotBytes, &tmA, a_full,
-                                         (it.g * kGroupYB + yb) * kBlockY, it.t * kTileP, pl);
+                    for (int yb = 0; yb < nybg; ++yb) {
+                        void *dst = sA + (pl * kGroupYB + yb) * kSlotBytes;
+                        const int cy = (it.g * kGroupYB + yb) * kBlockY;
+                        if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmA, a_full, cy, tile * kTileP, pl);
+                        else ptx::tma_load_3d(dst, &tmA, a_full, cy, tile * kTileP, pl);
+                    }
             }
             __syncwarp();
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
@@ -130,24 +151,37 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                             for (int pl = 0; pl < 4; ++pl) {
                                 ptx::mbar_wait(b_empty + slot, phase ^ 1);
                                 if (ptx::elect_one()) {
-                                    ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
-                                    ptx::tma_load_3d(sB + slot * kSlotBytes, &tmB, b_full + slot,
-                                                     (it.g * kGroupYB + yb) * kBlockY, xt * kTileX,
-                                                     (b * P.nz + j) * 4 + pl);
+                                    if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
+                                    void *dst = sB + slot * kSlotB;
+                                    const int cy = (it.g * kGroupYB + yb) * kBlockY;
+                                    const int cx = xt * kTileX + (int)rank * (kTileX / NCTA);
+                                    const int cp = (b * P.nz + j) * 4 + pl;
+                                    if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, cy, cx, cp);
+                                    else ptx::tma_load_3d(dst, &tmB, b_full + slot, cy, cx, cp);
                                 }
                                 __syncwarp();
                                 if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                             }
         }
     } else if (warp == 1) {
-        // ===================================================================== MMA issuer
+      if (leader) {
+        // ===================================================================== MMA issuer (leader CTA only)
         // Warp-uniform loop; descriptors are uniform-register arithmetic; one elected lane issues the
         // tcgen05.mma / tcgen05.commit instructions.
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP, kTileX, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP, kTileX, true);
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP * NCTA, kTileX, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP * NCTA, kTileX, true);
         const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
         const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
-        constexpr uint64_t kSlotDesc = kSlotBytes >> 4;
+        constexpr uint64_t kSlotDescA = kSlotBytes >> 4;
+        constexpr uint64_t kSlotDescB = kSlotB >> 4;
+        auto mma = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
+            if (NCTA == 2) ptx::umma_f16_2sm(d, a, b, idesc, acc);
+            else ptx::umma_f16(d, a, b, idesc, acc);
+        };
+        auto commit = [](uint64_t *bar) {
+            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x3);
+            else ptx::umma_commit(bar);
+        };
         int slot = 0;
         uint32_t phase = 0;
         uint32_t u = 0;
@@ -156,8 +190,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #ifdef SCATMAN_TIMING
         const long long t_begin = clock64();
 #endif
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const Item it = decode_item(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const Item it = decode_item(item, P, ntp);
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
             const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
@@ -171,26 +205,26 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                 for (int yb = 0; yb < nybg; ++yb) {
                     // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
-                    const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDesc;
-                    const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDesc;
-                    const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDesc;
-                    const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDesc;
+                    const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDescA;
+                    const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDescA;
+                    const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDescA;
+                    const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDescA;
                     const uint32_t first = yb != 0 ? 1u : 0u;
                     // ---- B = Re_hi
                     TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
                         for (int k = 0; k < kBlockY / 16; ++k) {
                             const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
                             const uint32_t acc0 = k != 0 ? 1u : first;
-                            ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
-                            ptx::umma_f16(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
-                            ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
-                            ptx::umma_f16(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
+                            mma(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
+                            mma(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
                         }
-                        ptx::umma_commit(b_empty + slot);
+                        commit(b_empty + slot);
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
@@ -198,14 +232,14 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
                         for (int k = 0; k < kBlockY / 16; ++k) {
                             const uint64_t ko = (uint64_t)(k * 2);
-                            ptx::umma_f16(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
-                            ptx::umma_f16(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
                         }
-                        ptx::umma_commit(b_empty + slot);
+                        commit(b_empty + slot);
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
@@ -213,16 +247,16 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
                         for (int k = 0; k < kBlockY / 16; ++k) {
                             const uint64_t ko = (uint64_t)(k * 2);
-                            ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                            ptx::umma_f16(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
-                            ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                            ptx::umma_f16(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                            mma(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
+                            mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
                         }
-                        ptx::umma_commit(b_empty + slot);
+                        commit(b_empty + slot);
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
@@ -230,22 +264,22 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDesc;
+                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
                         for (int k = 0; k < kBlockY / 16; ++k) {
                             const uint64_t ko = (uint64_t)(k * 2);
-                            ptx::umma_f16(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                            ptx::umma_f16(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                            mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
                         }
-                        ptx::umma_commit(b_empty + slot);
+                        commit(b_empty + slot);
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                 }
-                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                if (ptx::elect_one()) commit(t_full + buf);
                 __syncwarp();
             }
-            if (ptx::elect_one()) ptx::umma_commit(a_empty);
+            if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
         }
 #ifdef SCATMAN_TIMING
@@ -256,6 +290,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             g_timing[blockIdx.x * 8 + 3] = w_afull;
         }
 #endif
+      }
     } else if (warp >= 4) {
         // ========================================================================= epilogue
         const int ew = warp & 3;
@@ -266,15 +301,16 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #ifdef SCATMAN_TIMING
         const long long e_begin = clock64();
 #endif
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-            const Item it = decode_item(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            const Item it = decode_item(item, P, ntp);
+            const int tile = it.tp * NCTA + (int)rank;
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
             const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
             float2 fine[kFine];
 #pragma unroll
-            for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)it.t * kFine + i) * kTileP + el);
-            const float2 *anchor_t = P.anchor + (size_t)it.t * P.nxa * kTileP + el;
-            const float2 *mz_t = P.mz + (size_t)it.t * P.nz * kTileP + el;
+            for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)tile * kFine + i) * kTileP + el);
+            const float2 *anchor_t = P.anchor + (size_t)tile * P.nxa * kTileP + el;
+            const float2 *mz_t = P.mz + (size_t)tile * P.nz * kTileP + el;
             for (int b = b0; b < b1; ++b) {
                 float acc_re = 0.f, acc_im = 0.f;
                 for (int j = z0; j < z1; ++j) {
@@ -311,7 +347,10 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         }
                         ptx::tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                        if (lane == 0) {
+                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                            else ptx::mbar_arrive(t_empty + buf);
+                        }
                     }
                     acc_re = fmaf(mz.x, f_re, acc_re);
                     acc_re = fmaf(-mz.y, f_im, acc_re);
@@ -319,7 +358,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     acc_im = fmaf(mz.y, f_re, acc_im);
                 }
                 P.partial[((size_t)b * (P.ngroups * P.nzs) + (it.g * P.nzs + it.s)) * P.npix_pad +
-                          (size_t)it.t * kTileP + el] = make_float2(acc_re, acc_im);
+                          (size_t)tile * kTileP + el] = make_float2(acc_re, acc_im);
             }
         }
 #ifdef SCATMAN_TIMING
@@ -332,9 +371,11 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     }
     ptx::tc_fence_before();
     __syncthreads();
+    if (NCTA == 2) ptx::cluster_sync_all();   // nobody leaves while the peer may still signal its barriers
     if (warp == 2) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemCols);
+        if (NCTA == 2) ptx::tmem_dealloc_2sm(tmem_base, kTmemCols);
+        else ptx::tmem_dealloc(tmem_base, kTmemCols);
     }
 }
 
@@ -368,10 +409,40 @@ static bool encode_planes(CUtensorMap *tm, const void *base, uint64_t inner, uin
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+template <int NCTA>
+static cudaError_t launch_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const TensorParams &P, int num_sms,
+                                  cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(msft_contract_kernel<NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             kSmemTotal);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int nitems = P.nchunks * P.nzs * P.ngroups * (P.ntiles / NCTA);
+    const int max_clusters = num_sms / NCTA;
+    const int nclusters = nitems < max_clusters ? nitems : max_clusters;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(nclusters * NCTA));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kSmemTotal;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = NCTA;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, msft_contract_kernel<NCTA>, tmA, tmB, P);
+}
+
 cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st, std::string *err) {
+    const int ncta = p.t_ncta;
     CUtensorMap tmA, tmB;
     if (!encode_planes(&tmA, t.d_A, (uint64_t)p.ny_pad, (uint64_t)p.npix_pad, 4, kTileP) ||
-        !encode_planes(&tmB, t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4, kTileX)) {
+        !encode_planes(&tmB, t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4,
+                       kTileX / ncta)) {
         if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
         return cudaErrorUnknown;
     }
@@ -383,19 +454,8 @@ cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st,
     P.nxa = p.nxa;
     P.npix_pad = p.npix_pad;
     P.anchor = t.d_anchor; P.fine = t.d_fine; P.mz = t.d_mz; P.partial = t.d_partial;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(msft_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             kSmemTotal);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    const int nitems = P.nchunks * P.nzs * P.ngroups * P.ntiles;
-    const int grid = nitems < t.num_sms ? nitems : t.num_sms;
-    msft_contract_kernel<<<grid, kThreads, kSmemTotal, st>>>(tmA, tmB, P);
-    return cudaGetLastError();
+    return ncta == 2 ? launch_variant<2>(tmA, tmB, P, t.num_sms, st) : launch_variant<1>(tmA, tmB, P, t.num_sms, st);
 }
-
 
 #ifdef SCATMAN_TIMING
 extern "C" int scatman_debug_timing(long long *h_out) {

@@ -25,7 +25,8 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-METHODS = {"tensor": 1, "simt_sincos": 2}
+# name -> (method, flags): CTA-pair tensor kernel (default), single-CTA tensor kernel, CUDA-core sincos variant
+METHODS = {"tensor": (1, 0), "tensor_1cta": (1, 1), "simt_sincos": (2, 0)}
 
 
 # ------------------------------------------------------------------------------------------ stage kernels
@@ -63,7 +64,7 @@ def test_effective_strength_matches_oracle(sm):
 def test_cfg1_sphere_full_pattern(sm, method):
     w = W.config(0)
     g = w.grid(0)
-    I = sm.simulate(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, method=METHODS[method]).cpu().numpy()
+    I = sm.simulate(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, method=METHODS[method][0], flags=METHODS[method][1]).cpu().numpy()
     ref = O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg)
     assert_parity(I, ref, what=f"cfg1 {method}")
 
@@ -79,7 +80,7 @@ def test_ragged_random_batch_with_orientations(sm, method, mode):
     quat[1] = [1, 0, 0, 0]
     voxel, lam = (2.0, 2.5, 3.0), 14.0
     npx, npy, th = 23, 19, 35.0
-    I = sm.simulate(dev(g), voxel, lam, npx, npy, th, quat=quat, rho_mode=mode, method=METHODS[method]).cpu().numpy()
+    I = sm.simulate(dev(g), voxel, lam, npx, npy, th, quat=quat, rho_mode=mode, method=METHODS[method][0], flags=METHODS[method][1]).cpu().numpy()
     for b in range(B):
         ref = O.simulate(g[b], voxel, lam, npx, npy, th, quat=quat[b], rho_mode=mode)
         assert_parity(I[b], ref, what=f"ragged b={b} {method} mode={mode}")
@@ -89,7 +90,7 @@ def test_ragged_random_batch_with_orientations(sm, method, mode):
 def test_cfg2_ellipsoid_half_scale_oriented(sm, method):
     w = W.config(1, scale=0.5)
     g = w.grid(0)
-    I = sm.simulate(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat, method=METHODS[method]).cpu().numpy()
+    I = sm.simulate(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat, method=METHODS[method][0], flags=METHODS[method][1]).cpu().numpy()
     ref = O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat[0])
     assert_parity(I, ref, what=f"cfg2 half {method}")
 
@@ -131,8 +132,8 @@ def test_forward_pixel_and_explicit_q(sm):
     th = rng.uniform(0, 0.8, 200); ph = rng.uniform(-np.pi, np.pi, 200)
     q = np.stack([k * np.sin(th) * np.cos(ph), k * np.sin(th) * np.sin(ph), k * (np.cos(th) - 1)], axis=1)
     q[0] = 0.0
-    for m in METHODS.values():
-        I = sm.simulate_q(dev(g), voxel, lam, torch.from_numpy(q).cuda(), method=m).cpu().numpy()
+    for m, fl in METHODS.values():
+        I = sm.simulate_q(dev(g), voxel, lam, torch.from_numpy(q).cuda(), method=m, flags=fl).cpu().numpy()
         ref = O.simulate_q(g, voxel, lam, q)
         assert_parity(I, ref, what="explicit q")
         assert abs(I[0] - ref[0]) <= 2e-6 * ref[0]
@@ -141,12 +142,12 @@ def test_forward_pixel_and_explicit_q(sm):
 def test_empty_and_single_voxel(sm):
     voxel, lam = (3.0, 3.0, 3.0), 12.0
     z = np.zeros((8, 8, 8, 2), np.float32)
-    for m in METHODS.values():
-        I = sm.simulate(dev(z), voxel, lam, 16, 16, 30.0, method=m).cpu().numpy()
+    for m, fl in METHODS.values():
+        I = sm.simulate(dev(z), voxel, lam, 16, 16, 30.0, method=m, flags=fl).cpu().numpy()
         assert np.all(I == 0)
         one = z.copy()
         one[2, 5, 1] = (0.03, 0.004)
-        I = sm.simulate(dev(one), voxel, lam, 16, 16, 30.0, method=m).cpu().numpy()
+        I = sm.simulate(dev(one), voxel, lam, 16, 16, 30.0, method=m, flags=fl).cpu().numpy()
         exact = abs((float(np.float32(0.03)) + 1j * float(np.float32(0.004))) * 27.0) ** 2
         assert np.allclose(I, exact, rtol=2e-5)
 
