@@ -325,31 +325,45 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         TIMED_WAIT(w_tfull, ptx::mbar_wait(t_full + buf, (u >> 1) & 1));
                         ptx::tc_fence_after();
                         const uint32_t t_re = lane_base + buf * 256, t_im = t_re + 128;
+                        // software-pipelined: the loads of block a+1 are in flight while block a is reduced; the
+                        // accumulator buffer is handed back to the MMA warp as soon as its last column has landed
+                        uint32_t gre[2][16], gim[2][16];
+                        ptx::tmem_ld16(t_re, gre[0]);
+                        ptx::tmem_ld16(t_im, gim[0]);
+                        ptx::tmem_ld_wait_dep(gre[0]);
+                        ptx::tmem_ld_wait_dep(gim[0]);
 #pragma unroll
                         for (int a = 0; a < kTileX / kFine; ++a) {
-                            uint32_t gre[16], gim[16];
-                            ptx::tmem_ld16(t_re + a * kFine, gre);
-                            ptx::tmem_ld16(t_im + a * kFine, gim);
-                            ptx::tmem_ld_wait();
-                            float s_re = 0.f, s_im = 0.f;
+                            const int cur = a & 1, nxt = cur ^ 1;
+                            if (a + 1 < kTileX / kFine) {
+                                ptx::tmem_ld16(t_re + (a + 1) * kFine, gre[nxt]);
+                                ptx::tmem_ld16(t_im + (a + 1) * kFine, gim[nxt]);
+                            } else {
+                                ptx::tc_fence_before();
+                                __syncwarp();
+                                if (lane == 0) {
+                                    if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                                    else ptx::mbar_arrive(t_empty + buf);
+                                }
+                            }
+                            float sra = 0.f, srb = 0.f, sia = 0.f, sib = 0.f;   // four independent FMA chains
 #pragma unroll
                             for (int i = 0; i < kFine; ++i) {
-                                const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
-                                s_re = fmaf(fine[i].x, gr, s_re);
-                                s_re = fmaf(-fine[i].y, gi, s_re);
-                                s_im = fmaf(fine[i].x, gi, s_im);
-                                s_im = fmaf(fine[i].y, gr, s_im);
+                                const float gr = __uint_as_float(gre[cur][i]), gi = __uint_as_float(gim[cur][i]);
+                                sra = fmaf(fine[i].x, gr, sra);
+                                srb = fmaf(fine[i].y, gi, srb);
+                                sia = fmaf(fine[i].x, gi, sia);
+                                sib = fmaf(fine[i].y, gr, sib);
                             }
+                            const float s_re = sra - srb, s_im = sia + sib;
                             f_re = fmaf(anc[a].x, s_re, f_re);
                             f_re = fmaf(-anc[a].y, s_im, f_re);
                             f_im = fmaf(anc[a].x, s_im, f_im);
                             f_im = fmaf(anc[a].y, s_re, f_im);
-                        }
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) {
-                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                            else ptx::mbar_arrive(t_empty + buf);
+                            if (a + 1 < kTileX / kFine) {
+                                ptx::tmem_ld_wait_dep(gre[nxt]);
+                                ptx::tmem_ld_wait_dep(gim[nxt]);
+                            }
                         }
                     }
                     acc_re = fmaf(mz.x, f_re, acc_re);
