@@ -86,6 +86,7 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
         p.off_anchor = take(sizeof(float2) * (size_t)p.ntiles * p.nxa * kTileP);
         p.off_fine = take(sizeof(float2) * (size_t)p.ntiles * kFine * kTileP);
         p.off_mz = take(sizeof(float2) * (size_t)p.ntiles * p.nz * kTileP);
+        p.off_mask = take(sizeof(unsigned long long) * (size_t)batch * p.nz * p.nxt * p.ngroups);
     }
     p.total = off;
     return p;
@@ -311,7 +312,7 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
 
     if (p.method == SCATMAN_METHOD_TENSOR) {
         float *ampscale = (float *)(ws + p.off_ampscale);
-        e = launch_pack_b(rho, p, maxbits, ampscale, (__half *)(ws + p.off_B), st);
+        e = launch_pack_b(rho, p, maxbits, ampscale, (__half *)(ws + p.off_B), (unsigned long long *)(ws + p.off_mask), st);
         ++nl;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "pack_b");
         e = launch_tables(d_q, p, (__half *)(ws + p.off_A), (float2 *)(ws + p.off_anchor), (float2 *)(ws + p.off_fine),
@@ -320,7 +321,8 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
         TensorLaunch t;
         t.d_A = ws + p.off_A; t.d_B = ws + p.off_B;
         t.d_anchor = (const float2 *)(ws + p.off_anchor); t.d_fine = (const float2 *)(ws + p.off_fine);
-        t.d_mz = (const float2 *)(ws + p.off_mz); t.d_partial = partial; t.num_sms = ctx->num_sms;
+        t.d_mz = (const float2 *)(ws + p.off_mz); t.d_partial = partial;
+        t.d_mask = (const unsigned long long *)(ws + p.off_mask); t.num_sms = ctx->num_sms;
         std::string err;
         cudaEventRecord(ctx->ev0, st);
         e = launch_tensor(p, t, st, &err);

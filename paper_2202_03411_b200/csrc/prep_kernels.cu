@@ -153,7 +153,7 @@ __device__ __forceinline__ float scale_from_maxbits(unsigned bits) {
 
 __global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nx_pad, int ny_pad,
                               const unsigned *__restrict__ maxbits, float *__restrict__ ampscale, float dV,
-                              __half *__restrict__ B) {
+                              __half *__restrict__ B, unsigned long long *__restrict__ mask, int nxt, int ngroups) {
     __shared__ float2 tile[32][33];
     const int bz = blockIdx.x;  // b*nz + z
     const int b = bz / nz;
@@ -168,6 +168,7 @@ __global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, in
     __syncthreads();
     const size_t plane = (size_t)nx_pad * ny_pad;
     __half *dst = B + (size_t)bz * 4 * plane;
+    unsigned long long occ = 0;  // occupancy bits of this warp's 16 x 16 blocks (the contraction skips empty ones)
     for (int r = ty; r < 32; r += 8) {
         const int x = x0 + r, y = y0 + tx;  // x < nx_pad, y < ny_pad by grid construction
         const float2 v = tile[tx][r];
@@ -179,15 +180,25 @@ __global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, in
         dst[plane + o] = rel;
         dst[2 * plane + o] = imh;
         dst[3 * plane + o] = iml;
+        const bool nz16 = ((__half_as_ushort(reh) | __half_as_ushort(rel) | __half_as_ushort(imh) | __half_as_ushort(iml)) & 0x7fffu) != 0;
+        const unsigned bal = __ballot_sync(0xffffffffu, nz16);
+        const int xi = (x % kTileX) / 16, yi = ((y0 % (kGroupYB * kBlockY)) / 16);
+        if (bal & 0x0000ffffu) occ |= 1ull << (8 * yi + xi);
+        if (bal & 0xffff0000u) occ |= 1ull << (8 * (yi + 1) + xi);
     }
+    if (tx == 0 && occ)
+        atomicOr(mask + ((size_t)bz * nxt + x0 / kTileX) * ngroups + y0 / (kGroupYB * kBlockY), occ);
     if (blockIdx.y == 0 && blockIdx.z == 0 && tx == 0 && ty == 0 && (bz % nz) == 0) ampscale[b] = dV / (kScaleA * s);
 }
 
 cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_maxbits, float *d_ampscale,
-                          __half *d_B, cudaStream_t st) {
+                          __half *d_B, unsigned long long *d_mask, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(d_mask, 0, sizeof(unsigned long long) * (size_t)p.batch * p.nz * p.nxt * p.ngroups, st);
+    if (e != cudaSuccess) return e;
     dim3 grid((unsigned)(p.batch * p.nz), p.nx_pad / 32, p.ny_pad / 32);
     pack_b_kernel<<<grid, dim3(32, 8), 0, st>>>((const float2 *)d_rho, p.nx, p.ny, p.nz, p.nx_pad, p.ny_pad,
-                                                d_maxbits, d_ampscale, (float)(p.dx * p.dy * p.dz), d_B);
+                                                d_maxbits, d_ampscale, (float)(p.dx * p.dy * p.dz), d_B, d_mask, p.nxt,
+                                                p.ngroups);
     return cudaGetLastError();
 }
 

@@ -46,6 +46,7 @@ struct TensorParams {
     int nz, nxt, nyb, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
     int64_t npix_pad;
     const float2 *anchor, *fine, *mz;
+    const unsigned long long *mask;   // [batch][nz][nxt][ngroups]: bit 8*yi + xi = 16-y x 16-x block of rho~ is non-zero
     float2 *partial;
 };
 
@@ -62,6 +63,33 @@ __device__ __forceinline__ Item decode_item(int item, const TensorParams &P, int
     it.s = item % P.nzs;
     it.c = item / P.nzs;
     return it;
+}
+
+// Units (batch item b, slice j, x tile xt) of a work item in issue order, with the occupancy word of each.
+// Every role walks the same sequence and skips what the mask says is empty, so their pipelines stay in step.
+struct Walk {
+    int b, j, xt, b1, z0, z1, nxt;
+    __device__ __forceinline__ bool valid() const { return b < b1; }
+    __device__ __forceinline__ void next() {
+        if (++xt == nxt) {
+            xt = 0;
+            if (++j == z1) { j = z0; ++b; }
+        }
+    }
+};
+__device__ __forceinline__ Walk walk_begin(const Item &it, const TensorParams &P) {
+    Walk w;
+    w.b = it.c * P.bpc;
+    w.b1 = min(P.batch, w.b + P.bpc);
+    w.z0 = (int)(((long long)P.nz * it.s) / P.nzs);
+    w.z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
+    w.j = w.z0;
+    w.xt = 0;
+    w.nxt = P.nxt;
+    return w;
+}
+__device__ __forceinline__ unsigned long long walk_mask(const Walk &w, const TensorParams &P, int g) {
+    return w.valid() ? __ldg(P.mask + (((size_t)w.b * P.nz + w.j) * P.nxt + w.xt) * P.ngroups + g) : 0ull;
 }
 
 // NCTA = 1: one CTA per work item (cta_group::1, UMMA 128 x 128).
@@ -142,26 +170,32 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     }
             }
             __syncwarp();
-            const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
-            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
-            for (int b = b0; b < b1; ++b)
-                for (int j = z0; j < z1; ++j)
-                    for (int xt = 0; xt < P.nxt; ++xt)
-                        for (int yb = 0; yb < nybg; ++yb)
-                            for (int pl = 0; pl < 4; ++pl) {
-                                ptx::mbar_wait(b_empty + slot, phase ^ 1);
-                                if (ptx::elect_one()) {
-                                    if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
-                                    void *dst = sB + slot * kSlotB;
-                                    const int cy = (it.g * kGroupYB + yb) * kBlockY;
-                                    const int cx = xt * kTileX + (int)rank * (kTileX / NCTA);
-                                    const int cp = (b * P.nz + j) * 4 + pl;
-                                    if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, cy, cx, cp);
-                                    else ptx::tma_load_3d(dst, &tmB, b_full + slot, cy, cx, cp);
-                                }
-                                __syncwarp();
-                                if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                            }
+            Walk w = walk_begin(it, P);
+            unsigned long long m = walk_mask(w, P, it.g);
+            while (w.valid()) {
+                Walk wn = w;
+                wn.next();
+                const unsigned long long mn = walk_mask(wn, P, it.g);   // in flight while this unit is issued
+                for (int yb = 0; yb < nybg; ++yb) {
+                    if ((uint32_t)(m >> (32 * yb)) == 0u) continue;     // this 64-y block of the slice tile is empty
+                    for (int pl = 0; pl < 4; ++pl) {
+                        ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                        if (ptx::elect_one()) {
+                            if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
+                            void *dst = sB + slot * kSlotB;
+                            const int cy = (it.g * kGroupYB + yb) * kBlockY;
+                            const int cx = w.xt * kTileX + (int)rank * (kTileX / NCTA);
+                            const int cp = (w.b * P.nz + w.j) * 4 + pl;
+                            if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, cy, cx, cp);
+                            else ptx::tma_load_3d(dst, &tmB, b_full + slot, cy, cx, cp);
+                        }
+                        __syncwarp();
+                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                    }
+                }
+                w = wn;
+                m = mn;
+            }
         }
     } else if (warp == 1) {
       if (leader) {
@@ -193,91 +227,106 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
             const Item it = decode_item(item, P, ntp);
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
-            const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
-            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
-            const int nunits = (b1 - b0) * (z1 - z0) * P.nxt;
             TIMED_WAIT(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
             ptx::tc_fence_after();
-            for (int unit = 0; unit < nunits; ++unit, ++u) {
-                const uint32_t buf = u & 1;
-                TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1));
-                ptx::tc_fence_after();
-                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                for (int yb = 0; yb < nybg; ++yb) {
-                    // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
-                    const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDescA;
-                    const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDescA;
-                    const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDescA;
-                    const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDescA;
-                    const uint32_t first = yb != 0 ? 1u : 0u;
-                    // ---- B = Re_hi
-                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+            Walk w = walk_begin(it, P);
+            unsigned long long m = walk_mask(w, P, it.g);
+            while (w.valid()) {
+                Walk wn = w;
+                wn.next();
+                const unsigned long long mn = walk_mask(wn, P, it.g);
+                if (m != 0ull) {   // an all-zero unit adds nothing: no MMA, no accumulator hand-over
+                    const uint32_t buf = u & 1;
+                    TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1));
                     ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
+                    const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                    uint32_t started = 0u;   // 0 until the first k-step of this unit has initialised D_re and D_im
+                    for (int yb = 0; yb < nybg; ++yb) {
+                        const uint32_t occ = (uint32_t)(m >> (32 * yb));   // byte k = x-occupancy of 16-y step k
+                        if (occ == 0u) continue;
+                        // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
+                        const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDescA;
+                        const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDescA;
+                        const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDescA;
+                        const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDescA;
+                        // ---- B = Re_hi
+                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
+                            uint32_t acc0 = started;
 #pragma unroll
-                        for (int k = 0; k < kBlockY / 16; ++k) {
-                            const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
-                            const uint32_t acc0 = k != 0 ? 1u : first;
-                            mma(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
-                            mma(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
-                            mma(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
-                            mma(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
+                            for (int k = 0; k < kBlockY / 16; ++k) {
+                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;   // empty 16-y step
+                                const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
+                                mma(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
+                                mma(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
+                                mma(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
+                                mma(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
+                                acc0 = 1u;
+                            }
+                            commit(b_empty + slot);
                         }
-                        commit(b_empty + slot);
-                    }
-                    __syncwarp();
-                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                    // ---- B = Re_lo
-                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                    ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
+                        __syncwarp();
+                        started = 1u;
+                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                        // ---- B = Re_lo
+                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
-                        for (int k = 0; k < kBlockY / 16; ++k) {
-                            const uint64_t ko = (uint64_t)(k * 2);
-                            mma(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
-                            mma(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
+                            for (int k = 0; k < kBlockY / 16; ++k) {
+                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
+                                const uint64_t ko = (uint64_t)(k * 2);
+                                mma(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
+                                mma(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
+                            }
+                            commit(b_empty + slot);
                         }
-                        commit(b_empty + slot);
-                    }
-                    __syncwarp();
-                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                    // ---- B = Im_hi
-                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                    ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
+                        __syncwarp();
+                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                        // ---- B = Im_hi
+                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
-                        for (int k = 0; k < kBlockY / 16; ++k) {
-                            const uint64_t ko = (uint64_t)(k * 2);
-                            mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                            mma(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
-                            mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                            mma(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
+                            for (int k = 0; k < kBlockY / 16; ++k) {
+                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
+                                const uint64_t ko = (uint64_t)(k * 2);
+                                mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                                mma(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
+                                mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                                mma(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
+                            }
+                            commit(b_empty + slot);
                         }
-                        commit(b_empty + slot);
-                    }
-                    __syncwarp();
-                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                    // ---- B = Im_lo
-                    TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                    ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-                        const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
+                        __syncwarp();
+                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                        // ---- B = Im_lo
+                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
 #pragma unroll
-                        for (int k = 0; k < kBlockY / 16; ++k) {
-                            const uint64_t ko = (uint64_t)(k * 2);
-                            mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                            mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            for (int k = 0; k < kBlockY / 16; ++k) {
+                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
+                                const uint64_t ko = (uint64_t)(k * 2);
+                                mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
+                                mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
+                            }
+                            commit(b_empty + slot);
                         }
-                        commit(b_empty + slot);
+                        __syncwarp();
+                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     }
+                    if (ptx::elect_one()) commit(t_full + buf);
                     __syncwarp();
-                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                    ++u;
                 }
-                if (ptx::elect_one()) commit(t_full + buf);
-                __syncwarp();
+                w = wn;
+                m = mn;
             }
             if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
@@ -311,12 +360,18 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)tile * kFine + i) * kTileP + el);
             const float2 *anchor_t = P.anchor + (size_t)tile * P.nxa * kTileP + el;
             const float2 *mz_t = P.mz + (size_t)tile * P.nz * kTileP + el;
+            Walk w = walk_begin(it, P);
+            unsigned long long m_next = walk_mask(w, P, it.g);
             for (int b = b0; b < b1; ++b) {
                 float acc_re = 0.f, acc_im = 0.f;
                 for (int j = z0; j < z1; ++j) {
                     const float2 mz = __ldg(mz_t + (size_t)j * kTileP);
                     float f_re = 0.f, f_im = 0.f;
-                    for (int xt = 0; xt < P.nxt; ++xt, ++u) {
+                    for (int xt = 0; xt < P.nxt; ++xt) {
+                        const unsigned long long m = m_next;
+                        w.next();
+                        m_next = walk_mask(w, P, it.g);
+                        if (m == 0ull) continue;   // empty unit: G = 0, nothing was issued for it
                         const uint32_t buf = u & 1;
                         float2 anc[kTileX / kFine];
 #pragma unroll
@@ -365,6 +420,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                                 ptx::tmem_ld_wait_dep(gim[nxt]);
                             }
                         }
+                        ++u;
                     }
                     acc_re = fmaf(mz.x, f_re, acc_re);
                     acc_re = fmaf(-mz.y, f_im, acc_re);
@@ -467,7 +523,7 @@ cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st,
     P.nchunks = (p.batch + P.bpc - 1) / P.bpc;
     P.nxa = p.nxa;
     P.npix_pad = p.npix_pad;
-    P.anchor = t.d_anchor; P.fine = t.d_fine; P.mz = t.d_mz; P.partial = t.d_partial;
+    P.anchor = t.d_anchor; P.fine = t.d_fine; P.mz = t.d_mz; P.partial = t.d_partial; P.mask = t.d_mask;
     return ncta == 2 ? launch_variant<2>(tmA, tmB, P, t.num_sms, st) : launch_variant<1>(tmA, tmB, P, t.num_sms, st);
 }
 
