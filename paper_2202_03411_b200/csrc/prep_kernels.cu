@@ -175,7 +175,10 @@ __global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, in
         const float re = v.x * s, im = v.y * s;
         const __half reh = __float2half_rn(re), imh = __float2half_rn(im);
         const __half rel = __float2half_rn(re - __half2float(reh)), iml = __float2half_rn(im - __half2float(imh));
-        const size_t o = (size_t)x * ny_pad + y;
+        // row order inside a 128-x tile: x = 16 blk + t -> row 64 (t / 8) + 8 blk + t % 8, so that each CTA of a pair
+        // (rows 0-63 / 64-127) holds half of every 16-x block and a row prefix of both halves is a contiguous x range
+        const int xrow = (x & ~(kTileX - 1)) | (((x >> 3) & 1) << 6) | (((x >> 4) & 7) << 3) | (x & 7);
+        const size_t o = (size_t)xrow * ny_pad + y;
         dst[o] = reh;
         dst[plane + o] = rel;
         dst[2 * plane + o] = imh;

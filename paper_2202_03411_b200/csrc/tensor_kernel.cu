@@ -65,32 +65,74 @@ __device__ __forceinline__ Item decode_item(int item, const TensorParams &P, int
     return it;
 }
 
-// Units (batch item b, slice j, x tile xt) of a work item in issue order, with the occupancy word of each.
-// Every role walks the same sequence and skips what the mask says is empty, so their pipelines stay in step.
-struct Walk {
-    int b, j, xt, b1, z0, z1, nxt;
-    __device__ __forceinline__ bool valid() const { return b < b1; }
-    __device__ __forceinline__ void next() {
-        if (++xt == nxt) {
-            xt = 0;
-            if (++j == z1) { j = z0; ++b; }
+// The NON-EMPTY units (batch item b, slice j, x tile xt) of a work item in issue order, with the occupancy word of
+// each.  Every role walks the same sequence, so their pipelines stay in step.  Warp-cooperative: each lane holds the
+// occupancy word of one of 32 consecutive units (the next 32 are already in flight), a ballot finds the next
+// non-empty one, a shuffle broadcasts it: one L2 round trip per 32 units instead of one per unit.
+struct Units {
+    int b0, z0, nzr, nxt, total, g, base, lane;
+    unsigned long long cur, ahead;
+    uint32_t live;
+    const TensorParams *P;
+    __device__ __forceinline__ void decode(int n, int &b, int &j, int &xt) const {
+        xt = n % nxt;
+        const int r = n / nxt;
+        j = z0 + r % nzr;
+        b = b0 + r / nzr;
+    }
+    __device__ __forceinline__ unsigned long long load(int n) const {
+        if (n >= total) return 0ull;
+        int b, j, xt;
+        decode(n, b, j, xt);
+        return __ldg(P->mask + (((size_t)b * P->nz + j) * P->nxt + xt) * P->ngroups + g);
+    }
+    __device__ __forceinline__ void begin(const Item &it, const TensorParams &Pr, int lane_) {
+        P = &Pr;
+        lane = lane_;
+        g = it.g;
+        b0 = it.c * Pr.bpc;
+        const int b1 = min(Pr.batch, b0 + Pr.bpc);
+        z0 = (int)(((long long)Pr.nz * it.s) / Pr.nzs);
+        nzr = (int)(((long long)Pr.nz * (it.s + 1)) / Pr.nzs) - z0;
+        nxt = Pr.nxt;
+        total = (b1 - b0) * nzr * nxt;
+        base = 0;
+        cur = load(lane);
+        ahead = load(32 + lane);
+        live = __ballot_sync(0xffffffffu, cur != 0ull);
+    }
+    // next non-empty unit; false when the item is exhausted (warp-uniform result)
+    __device__ __forceinline__ bool next(int &b, int &j, int &xt, unsigned long long &m) {
+        while (live == 0u) {
+            base += 32;
+            if (base >= total) return false;
+            cur = ahead;
+            ahead = load(base + 32 + lane);
+            live = __ballot_sync(0xffffffffu, cur != 0ull);
         }
+        const int pos = __ffs((int)live) - 1;
+        live &= live - 1;
+        m = __shfl_sync(0xffffffffu, cur, pos);
+        decode(base + pos, b, j, xt);
+        return true;
     }
 };
-__device__ __forceinline__ Walk walk_begin(const Item &it, const TensorParams &P) {
-    Walk w;
-    w.b = it.c * P.bpc;
-    w.b1 = min(P.batch, w.b + P.bpc);
-    w.z0 = (int)(((long long)P.nz * it.s) / P.nzs);
-    w.z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
-    w.j = w.z0;
-    w.xt = 0;
-    w.nxt = P.nxt;
-    return w;
+
+// x extent of a unit in 16-x blocks: [a, a + m) = bounding range of the non-empty blocks over the whole y group.
+// CTA pairs run the unit's MMAs at N = 16 m (the B tile rows are stored so that a prefix of each CTA's half is a
+// contiguous x range, see pack_b_kernel); a single CTA always runs the full tile.
+template <int NCTA>
+__device__ __forceinline__ void unit_range(unsigned long long m64, int &a, int &m) {
+    if (NCTA == 1) { a = 0; m = kTileX / 16; return; }
+    uint32_t v = (uint32_t)m64 | (uint32_t)(m64 >> 32);
+    v |= v >> 16;
+    v = (v | (v >> 8)) & 0xffu;
+    a = __ffs((int)v) - 1;
+    m = (32 - __clz((int)v)) - a;
 }
-__device__ __forceinline__ unsigned long long walk_mask(const Walk &w, const TensorParams &P, int g) {
-    return w.valid() ? __ldg(P.mask + (((size_t)w.b * P.nz + w.j) * P.nxt + w.xt) * P.ngroups + g) : 0ull;
-}
+struct TmapsB {
+    CUtensorMap m[kTileX / 16];   // box heights 8, 16, ... rows per CTA of a pair (entry 7 = the full half / full tile)
+};
 
 // NCTA = 1: one CTA per work item (cta_group::1, UMMA 128 x 128).
 // NCTA = 2: a CTA pair per work item (cta_group::2, UMMA 256 x 128): each CTA owns its own 128-pixel tile (A resident in
@@ -99,7 +141,7 @@ __device__ __forceinline__ unsigned long long walk_mask(const Walk &w, const Ten
 //           issues every MMA; full barriers live in the leader, empty barriers are signalled in both CTAs.
 template <int NCTA>
 __global__ void __launch_bounds__(kThreads, 1)
-msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ TmapsB tmB,
                      const TensorParams P) {
     constexpr int kStagesB = 6 * NCTA;
     constexpr int kSlotB = kSlotBytes / NCTA;     // bytes of a B slot in one CTA
@@ -122,7 +164,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 
     if (warp == 0 && lane == 0) {
         ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
+        for (int i = 0; i < kTileX / 16; ++i) ptx::tma_prefetch_desc(&tmB.m[i]);
     }
     if (warp == 1 && lane == 0) {
         ptx::mbar_init(a_full, 1);
@@ -168,33 +210,41 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmA, a_full, cy, tile * kTileP, pl);
                         else ptx::tma_load_3d(dst, &tmA, a_full, cy, tile * kTileP, pl);
                     }
+                // the A tile of this cluster's next work item comes from HBM: start it towards L2 now
+                if (item + nclusters < nitems) {
+                    const Item nx = decode_item(item + nclusters, P, ntp);
+                    const int ntile = nx.tp * NCTA + (int)rank;
+                    const int nyn = min(kGroupYB, P.nyb - nx.g * kGroupYB);
+                    for (int pl = 0; pl < 4; ++pl)
+                        for (int yb = 0; yb < nyn; ++yb)
+                            ptx::tma_prefetch_l2_3d(&tmA, (nx.g * kGroupYB + yb) * kBlockY, ntile * kTileP, pl);
+                }
             }
             __syncwarp();
-            Walk w = walk_begin(it, P);
-            unsigned long long m = walk_mask(w, P, it.g);
-            while (w.valid()) {
-                Walk wn = w;
-                wn.next();
-                const unsigned long long mn = walk_mask(wn, P, it.g);   // in flight while this unit is issued
-                for (int yb = 0; yb < nybg; ++yb) {
-                    if ((uint32_t)(m >> (32 * yb)) == 0u) continue;     // this 64-y block of the slice tile is empty
-                    for (int pl = 0; pl < 4; ++pl) {
-                        ptx::mbar_wait(b_empty + slot, phase ^ 1);
-                        if (ptx::elect_one()) {
-                            if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, kSlotBytes);
-                            void *dst = sB + slot * kSlotB;
-                            const int cy = (it.g * kGroupYB + yb) * kBlockY;
-                            const int cx = w.xt * kTileX + (int)rank * (kTileX / NCTA);
-                            const int cp = (w.b * P.nz + w.j) * 4 + pl;
-                            if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, cy, cx, cp);
-                            else ptx::tma_load_3d(dst, &tmB, b_full + slot, cy, cx, cp);
-                        }
-                        __syncwarp();
-                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+            Units un;
+            un.begin(it, P, lane);
+            int ub, uj, uxt;
+            unsigned long long m;
+            while (un.next(ub, uj, uxt, m)) {
+                int xa, xm;
+                unit_range<NCTA>(m, xa, xm);
+                const CUtensorMap *tmb = &tmB.m[xm - 1];                // box {16 y, 8 xm rows per CTA (128 for one CTA), 4 planes}
+                const uint32_t tx_bytes = NCTA == 2 ? (uint32_t)(2 * 4 * 8 * xm * 32) : (uint32_t)(4 * kTileX * 32);
+                for (int yi = 0; yi < 4 * nybg; ++yi) {
+                    if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // this 16-y step of the slice tile is empty
+                    ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                    if (ptx::elect_one()) {
+                        if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, tx_bytes);
+                        void *dst = sB + slot * kSlotB;
+                        const int cy = it.g * (kGroupYB * kBlockY) + 16 * yi;
+                        const int cx = uxt * kTileX + (int)rank * (kTileX / NCTA) + 8 * xa;
+                        const int cp = (ub * P.nz + uj) * 4;
+                        if (NCTA == 2) ptx::tma_load_3d_2sm(dst, tmb, b_full + slot, cy, cx, cp);
+                        else ptx::tma_load_3d(dst, tmb, b_full + slot, cy, cx, cp);
                     }
+                    __syncwarp();
+                    if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                 }
-                w = wn;
-                m = mn;
             }
         }
     } else if (warp == 1) {
@@ -202,10 +252,10 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         // ===================================================================== MMA issuer (leader CTA only)
         // Warp-uniform loop; descriptors are uniform-register arithmetic; one elected lane issues the
         // tcgen05.mma / tcgen05.commit instructions.
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kTileP * NCTA, kTileX, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kTileP * NCTA, kTileX, true);
+        constexpr uint32_t idesc_pos0 = ptx::umma_idesc_f16(kTileP * NCTA, 0, false);   // N is set per unit
+        constexpr uint32_t idesc_neg0 = ptx::umma_idesc_f16(kTileP * NCTA, 0, true);
         const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
-        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
+        const uint64_t descB0 = ptx::umma_smem_desc_sw32(ptx::smem_u32(sB));
         constexpr uint64_t kSlotDescA = kSlotBytes >> 4;
         constexpr uint64_t kSlotDescB = kSlotB >> 4;
         auto mma = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
@@ -229,104 +279,56 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
             TIMED_WAIT(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
             ptx::tc_fence_after();
-            Walk w = walk_begin(it, P);
-            unsigned long long m = walk_mask(w, P, it.g);
-            while (w.valid()) {
-                Walk wn = w;
-                wn.next();
-                const unsigned long long mn = walk_mask(wn, P, it.g);
-                if (m != 0ull) {   // an all-zero unit adds nothing: no MMA, no accumulator hand-over
+            Units un;
+            un.begin(it, P, lane);
+            int ub, uj, uxt;
+            unsigned long long m;
+            while (un.next(ub, uj, uxt, m)) {   // all-zero units never appear: no MMA, no accumulator hand-over
+                {
                     const uint32_t buf = u & 1;
                     TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1));
                     ptx::tc_fence_after();
                     const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                    int xa, xm;
+                    unit_range<NCTA>(m, xa, xm);
+                    const uint32_t idesc_pos = idesc_pos0 | ((uint32_t)(2 * xm) << 17);   // N = 16 xm
+                    const uint32_t idesc_neg = idesc_neg0 | ((uint32_t)(2 * xm) << 17);
+                    const uint64_t pstride = (uint64_t)((NCTA == 2 ? 8 * xm : kTileX) * 32) >> 4;   // B plane stride in a slot
                     uint32_t started = 0u;   // 0 until the first k-step of this unit has initialised D_re and D_im
-                    for (int yb = 0; yb < nybg; ++yb) {
-                        const uint32_t occ = (uint32_t)(m >> (32 * yb));   // byte k = x-occupancy of 16-y step k
-                        if (occ == 0u) continue;
-                        // A-plane descriptors of this y-block: 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo
-                        const uint64_t a_reh = descA0 + (uint64_t)(0 * kGroupYB + yb) * kSlotDescA;
-                        const uint64_t a_rel = descA0 + (uint64_t)(1 * kGroupYB + yb) * kSlotDescA;
-                        const uint64_t a_imh = descA0 + (uint64_t)(2 * kGroupYB + yb) * kSlotDescA;
-                        const uint64_t a_iml = descA0 + (uint64_t)(3 * kGroupYB + yb) * kSlotDescA;
-                        // ---- B = Re_hi
+                    for (int yi = 0; yi < 4 * nybg; ++yi) {
+                        if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // empty 16-y step: never loaded
                         TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
-                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
-                            uint32_t acc0 = started;
-#pragma unroll
-                            for (int k = 0; k < kBlockY / 16; ++k) {
-                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;   // empty 16-y step
-                                const uint64_t ko = (uint64_t)(k * 2);  // 16 fp16 = 32 bytes = 2 descriptor units
-                                mma(d_re, a_reh + ko, bd + ko, idesc_pos, acc0);
-                                mma(d_re, a_rel + ko, bd + ko, idesc_pos, 1u);
-                                mma(d_im, a_imh + ko, bd + ko, idesc_pos, acc0);
-                                mma(d_im, a_iml + ko, bd + ko, idesc_pos, 1u);
-                                acc0 = 1u;
-                            }
+                            // A planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo of this k-step (32 bytes = 2 descriptor units per step)
+                            const uint64_t a_reh = descA0 + (uint64_t)(yi >> 2) * kSlotDescA + (uint64_t)((yi & 3) * 2);
+                            const uint64_t a_rel = a_reh + (uint64_t)(1 * kGroupYB) * kSlotDescA;
+                            const uint64_t a_imh = a_reh + (uint64_t)(2 * kGroupYB) * kSlotDescA;
+                            const uint64_t a_iml = a_reh + (uint64_t)(3 * kGroupYB) * kSlotDescA;
+                            const uint64_t b_reh = descB0 + (uint64_t)slot * kSlotDescB;
+                            const uint64_t b_rel = b_reh + pstride, b_imh = b_rel + pstride, b_iml = b_imh + pstride;
+                            mma(d_re, a_reh, b_reh, idesc_pos, started);
+                            mma(d_im, a_imh, b_reh, idesc_pos, started);
+                            mma(d_re, a_rel, b_reh, idesc_pos, 1u);
+                            mma(d_im, a_iml, b_reh, idesc_pos, 1u);
+                            mma(d_re, a_reh, b_rel, idesc_pos, 1u);
+                            mma(d_im, a_imh, b_rel, idesc_pos, 1u);
+                            mma(d_re, a_imh, b_imh, idesc_neg, 1u);
+                            mma(d_im, a_reh, b_imh, idesc_pos, 1u);
+                            mma(d_re, a_iml, b_imh, idesc_neg, 1u);
+                            mma(d_im, a_rel, b_imh, idesc_pos, 1u);
+                            mma(d_re, a_imh, b_iml, idesc_neg, 1u);
+                            mma(d_im, a_reh, b_iml, idesc_pos, 1u);
                             commit(b_empty + slot);
                         }
                         __syncwarp();
                         started = 1u;
-                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                        // ---- B = Re_lo
-                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
-#pragma unroll
-                            for (int k = 0; k < kBlockY / 16; ++k) {
-                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
-                                const uint64_t ko = (uint64_t)(k * 2);
-                                mma(d_re, a_reh + ko, bd + ko, idesc_pos, 1u);
-                                mma(d_im, a_imh + ko, bd + ko, idesc_pos, 1u);
-                            }
-                            commit(b_empty + slot);
-                        }
-                        __syncwarp();
-                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                        // ---- B = Im_hi
-                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
-#pragma unroll
-                            for (int k = 0; k < kBlockY / 16; ++k) {
-                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
-                                const uint64_t ko = (uint64_t)(k * 2);
-                                mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                                mma(d_re, a_iml + ko, bd + ko, idesc_neg, 1u);
-                                mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                                mma(d_im, a_rel + ko, bd + ko, idesc_pos, 1u);
-                            }
-                            commit(b_empty + slot);
-                        }
-                        __syncwarp();
-                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
-                        // ---- B = Im_lo
-                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-                            const uint64_t bd = descB0 + (uint64_t)slot * kSlotDescB;
-#pragma unroll
-                            for (int k = 0; k < kBlockY / 16; ++k) {
-                                if (((occ >> (8 * k)) & 0xffu) == 0u) continue;
-                                const uint64_t ko = (uint64_t)(k * 2);
-                                mma(d_re, a_imh + ko, bd + ko, idesc_neg, 1u);
-                                mma(d_im, a_reh + ko, bd + ko, idesc_pos, 1u);
-                            }
-                            commit(b_empty + slot);
-                        }
-                        __syncwarp();
                         if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     }
                     if (ptx::elect_one()) commit(t_full + buf);
                     __syncwarp();
                     ++u;
                 }
-                w = wn;
-                m = mn;
             }
             if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
@@ -354,81 +356,113 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             const Item it = decode_item(item, P, ntp);
             const int tile = it.tp * NCTA + (int)rank;
             const int b0 = it.c * P.bpc, b1 = min(P.batch, b0 + P.bpc);
-            const int z0 = (int)(((long long)P.nz * it.s) / P.nzs), z1 = (int)(((long long)P.nz * (it.s + 1)) / P.nzs);
             float2 fine[kFine];
 #pragma unroll
             for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)tile * kFine + i) * kTileP + el);
             const float2 *anchor_t = P.anchor + (size_t)tile * P.nxa * kTileP + el;
             const float2 *mz_t = P.mz + (size_t)tile * P.nz * kTileP + el;
-            Walk w = walk_begin(it, P);
-            unsigned long long m_next = walk_mask(w, P, it.g);
-            for (int b = b0; b < b1; ++b) {
-                float acc_re = 0.f, acc_im = 0.f;
-                for (int j = z0; j < z1; ++j) {
-                    const float2 mz = __ldg(mz_t + (size_t)j * kTileP);
-                    float f_re = 0.f, f_im = 0.f;
-                    for (int xt = 0; xt < P.nxt; ++xt) {
-                        const unsigned long long m = m_next;
-                        w.next();
-                        m_next = walk_mask(w, P, it.g);
-                        if (m == 0ull) continue;   // empty unit: G = 0, nothing was issued for it
+            float2 *partial_t = P.partial + (size_t)(it.g * P.nzs + it.s) * P.npix_pad + (size_t)tile * kTileP + el;
+            const size_t partial_b = (size_t)(P.ngroups * P.nzs) * P.npix_pad;   // stride between batch items
+            // Flat walk over the non-empty units; f = row-dot of the current slice, acc = amplitude of the current
+            // batch item.  A slice change folds f into acc with e^{i qz z_j}; an item change stores acc.  Items with
+            // no unit at all in this work item still get their (zero) partial written.
+            Units un;
+            un.begin(it, P, lane);
+            int ub, uj, xt;
+            unsigned long long m;
+            int cb = b0, cj = -1;          // current batch item / slice (cj < 0: nothing pending)
+            float2 mz = make_float2(0.f, 0.f);
+            float acc_re = 0.f, acc_im = 0.f, f_re = 0.f, f_im = 0.f;
+            {
+                {
+                    while (un.next(ub, uj, xt, m)) {
+                        if (ub != cb || uj != cj) {
+                            acc_re = fmaf(mz.x, f_re, acc_re);      // fold the finished slice (mz = 0 when none pending)
+                            acc_re = fmaf(-mz.y, f_im, acc_re);
+                            acc_im = fmaf(mz.x, f_im, acc_im);
+                            acc_im = fmaf(mz.y, f_re, acc_im);
+                            f_re = 0.f;
+                            f_im = 0.f;
+                            for (; cb < ub; ++cb) {                 // finished (or empty) batch items
+                                partial_t[(size_t)cb * partial_b] = make_float2(acc_re, acc_im);
+                                acc_re = 0.f;
+                                acc_im = 0.f;
+                            }
+                            cj = uj;
+                            mz = __ldg(mz_t + (size_t)uj * kTileP);
+                        }
                         const uint32_t buf = u & 1;
+                        int xa, xm;
+                        unit_range<NCTA>(m, xa, xm);   // the unit's accumulator holds x blocks [xa, xa + xm)
                         float2 anc[kTileX / kFine];
 #pragma unroll
                         for (int a = 0; a < kTileX / kFine; ++a)
-                            anc[a] = __ldg(anchor_t + (size_t)(xt * (kTileX / kFine) + a) * kTileP);
+                            anc[a] = __ldg(anchor_t + (size_t)(xt * (kTileX / kFine) + min(xa + a, kTileX / kFine - 1)) * kTileP);
                         TIMED_WAIT(w_tfull, ptx::mbar_wait(t_full + buf, (u >> 1) & 1));
                         ptx::tc_fence_after();
                         const uint32_t t_re = lane_base + buf * 256, t_im = t_re + 128;
+                        // Column layout of an accumulator (N = 16 xm): x block a = columns [8a, 8a+8) (its x 0..7) and
+                        // [8 xm + 8a, +8) (its x 8..15): the two halves of B come from the two CTAs of the pair.
+                        const uint32_t half = 8u * (uint32_t)xm;
                         // software-pipelined: the loads of block a+1 are in flight while block a is reduced; the
                         // accumulator buffer is handed back to the MMA warp as soon as its last column has landed
                         uint32_t gre[2][16], gim[2][16];
-                        ptx::tmem_ld16(t_re, gre[0]);
-                        ptx::tmem_ld16(t_im, gim[0]);
+                        ptx::tmem_ld8(t_re, gre[0]);
+                        ptx::tmem_ld8(t_re + half, gre[0] + 8);
+                        ptx::tmem_ld8(t_im, gim[0]);
+                        ptx::tmem_ld8(t_im + half, gim[0] + 8);
                         ptx::tmem_ld_wait_dep(gre[0]);
                         ptx::tmem_ld_wait_dep(gim[0]);
 #pragma unroll
                         for (int a = 0; a < kTileX / kFine; ++a) {
-                            const int cur = a & 1, nxt = cur ^ 1;
-                            if (a + 1 < kTileX / kFine) {
-                                ptx::tmem_ld16(t_re + (a + 1) * kFine, gre[nxt]);
-                                ptx::tmem_ld16(t_im + (a + 1) * kFine, gim[nxt]);
-                            } else {
-                                ptx::tc_fence_before();
-                                __syncwarp();
-                                if (lane == 0) {
-                                    if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                                    else ptx::mbar_arrive(t_empty + buf);
+                            if (a < xm) {   // warp-uniform
+                                const int cur = a & 1, nxt = cur ^ 1;
+                                const bool more = a + 1 < kTileX / kFine && a + 1 < xm;
+                                if (more) {
+                                    ptx::tmem_ld8(t_re + (a + 1) * 8, gre[nxt]);
+                                    ptx::tmem_ld8(t_re + half + (a + 1) * 8, gre[nxt] + 8);
+                                    ptx::tmem_ld8(t_im + (a + 1) * 8, gim[nxt]);
+                                    ptx::tmem_ld8(t_im + half + (a + 1) * 8, gim[nxt] + 8);
+                                } else {
+                                    ptx::tc_fence_before();
+                                    __syncwarp();
+                                    if (lane == 0) {
+                                        if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                                        else ptx::mbar_arrive(t_empty + buf);
+                                    }
                                 }
-                            }
-                            float sra = 0.f, srb = 0.f, sia = 0.f, sib = 0.f;   // four independent FMA chains
+                                float sra = 0.f, srb = 0.f, sia = 0.f, sib = 0.f;   // four independent FMA chains
 #pragma unroll
-                            for (int i = 0; i < kFine; ++i) {
-                                const float gr = __uint_as_float(gre[cur][i]), gi = __uint_as_float(gim[cur][i]);
-                                sra = fmaf(fine[i].x, gr, sra);
-                                srb = fmaf(fine[i].y, gi, srb);
-                                sia = fmaf(fine[i].x, gi, sia);
-                                sib = fmaf(fine[i].y, gr, sib);
-                            }
-                            const float s_re = sra - srb, s_im = sia + sib;
-                            f_re = fmaf(anc[a].x, s_re, f_re);
-                            f_re = fmaf(-anc[a].y, s_im, f_re);
-                            f_im = fmaf(anc[a].x, s_im, f_im);
-                            f_im = fmaf(anc[a].y, s_re, f_im);
-                            if (a + 1 < kTileX / kFine) {
-                                ptx::tmem_ld_wait_dep(gre[nxt]);
-                                ptx::tmem_ld_wait_dep(gim[nxt]);
+                                for (int i = 0; i < kFine; ++i) {
+                                    const float gr = __uint_as_float(gre[cur][i]), gi = __uint_as_float(gim[cur][i]);
+                                    sra = fmaf(fine[i].x, gr, sra);
+                                    srb = fmaf(fine[i].y, gi, srb);
+                                    sia = fmaf(fine[i].x, gi, sia);
+                                    sib = fmaf(fine[i].y, gr, sib);
+                                }
+                                const float s_re = sra - srb, s_im = sia + sib;
+                                f_re = fmaf(anc[a].x, s_re, f_re);
+                                f_re = fmaf(-anc[a].y, s_im, f_re);
+                                f_im = fmaf(anc[a].x, s_im, f_im);
+                                f_im = fmaf(anc[a].y, s_re, f_im);
+                                if (more) {
+                                    ptx::tmem_ld_wait_dep(gre[nxt]);
+                                    ptx::tmem_ld_wait_dep(gim[nxt]);
+                                }
                             }
                         }
                         ++u;
                     }
-                    acc_re = fmaf(mz.x, f_re, acc_re);
-                    acc_re = fmaf(-mz.y, f_im, acc_re);
-                    acc_im = fmaf(mz.x, f_im, acc_im);
-                    acc_im = fmaf(mz.y, f_re, acc_im);
                 }
-                P.partial[((size_t)b * (P.ngroups * P.nzs) + (it.g * P.nzs + it.s)) * P.npix_pad +
-                          (size_t)tile * kTileP + el] = make_float2(acc_re, acc_im);
+            }
+            acc_re = fmaf(mz.x, f_re, acc_re);
+            acc_re = fmaf(-mz.y, f_im, acc_re);
+            acc_im = fmaf(mz.x, f_im, acc_im);
+            acc_im = fmaf(mz.y, f_re, acc_im);
+            for (; cb < b1; ++cb) {
+                partial_t[(size_t)cb * partial_b] = make_float2(acc_re, acc_im);
+                acc_re = 0.f;
+                acc_im = 0.f;
             }
         }
 #ifdef SCATMAN_TIMING
@@ -467,20 +501,20 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 static bool encode_planes(CUtensorMap *tm, const void *base, uint64_t inner, uint64_t rows, uint64_t planes,
-                          uint32_t box_rows) {
+                          uint32_t box_inner, uint32_t box_rows, uint32_t box_planes, CUtensorMapSwizzle swizzle) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return false;
     cuuint64_t dims[3] = {inner, rows, planes};
     cuuint64_t strides[2] = {inner * 2, inner * rows * 2};
-    cuuint32_t box[3] = {(cuuint32_t)kBlockY, box_rows, 1};
+    cuuint32_t box[3] = {box_inner, box_rows, box_planes};
     cuuint32_t estr[3] = {1, 1, 1};
     return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void *>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <int NCTA>
-static cudaError_t launch_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const TensorParams &P, int num_sms,
+static cudaError_t launch_variant(const CUtensorMap &tmA, const TmapsB &tmB, const TensorParams &P, int num_sms,
                                   cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
@@ -509,10 +543,16 @@ static cudaError_t launch_variant(const CUtensorMap &tmA, const CUtensorMap &tmB
 
 cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st, std::string *err) {
     const int ncta = p.t_ncta;
-    CUtensorMap tmA, tmB;
-    if (!encode_planes(&tmA, t.d_A, (uint64_t)p.ny_pad, (uint64_t)p.npix_pad, 4, kTileP) ||
-        !encode_planes(&tmB, t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4,
-                       kTileX / ncta)) {
+    CUtensorMap tmA;
+    TmapsB tmB;
+    bool ok = encode_planes(&tmA, t.d_A, (uint64_t)p.ny_pad, (uint64_t)p.npix_pad, 4, kBlockY, kTileP, 1,
+                            CU_TENSOR_MAP_SWIZZLE_128B);
+    // B: one box = one 16-y k-step of all four planes; CTA pairs fetch only the rows of a unit's x range (one box
+    // height per range length)
+    for (int i = 0; ok && i < kTileX / 16; ++i)
+        ok = encode_planes(&tmB.m[i], t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4, 16,
+                           ncta == 2 ? 8 * (i + 1) : kTileX, 4, CU_TENSOR_MAP_SWIZZLE_32B);
+    if (!ok) {
         if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
         return cudaErrorUnknown;
     }

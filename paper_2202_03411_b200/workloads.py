@@ -273,6 +273,19 @@ def random_grid(seed: int, nx: int, ny: int, nz: int, fill: float = 0.6,
     return out
 
 
+def sparse_blobs_grid(seed: int, nx: int, ny: int, nz: int, nblobs: int = 6, max_extent: int = 24) -> np.ndarray:
+    """A few small random boxes of material per slice range in an otherwise empty grid: most 16 x 16 (x, y) blocks of
+    most slices are exactly zero, and the occupied x / y ranges differ from slice to slice and tile to tile."""
+    rng = np.random.default_rng(seed)
+    out = np.zeros((nz, ny, nx, 2), dtype=np.float32)
+    for _ in range(nblobs):
+        ex, ey, ez = (int(rng.integers(1, max(2, min(max_extent, n)))) for n in (nx, ny, nz))
+        x0, y0, z0 = int(rng.integers(0, nx - ex + 1)), int(rng.integers(0, ny - ey + 1)), int(rng.integers(0, nz - ez + 1))
+        out[z0:z0 + ez, y0:y0 + ey, x0:x0 + ex, 0] = rng.uniform(-0.02, 0.05)
+        out[z0:z0 + ez, y0:y0 + ey, x0:x0 + ex, 1] = rng.uniform(0.0, 0.02)
+    return out
+
+
 def sample_pixels(seed: int, npix: int, count: int, always: List[int] = ()) -> np.ndarray:
     """Seeded pixel subset (sorted, unique) for sampled parity at full sizes."""
     rng = np.random.default_rng(seed)

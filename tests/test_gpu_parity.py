@@ -86,6 +86,21 @@ def test_ragged_random_batch_with_orientations(sm, method, mode):
         assert_parity(I[b], ref, what=f"ragged b={b} {method} mode={mode}")
 
 
+@pytest.mark.parametrize("method", ["tensor", "tensor_1cta"])
+@pytest.mark.parametrize("seed", [71, 72, 73])
+def test_sparse_blobs_exercise_block_skipping(sm, method, seed):
+    """Mostly empty grids whose occupied 16 x 16 blocks differ per slice, x tile and y group: the contraction skips
+    empty y steps and narrows each unit to its occupied x range; the result must not change."""
+    nx, ny, nz, B = 300, 200, 10, 2
+    g = np.stack([W.sparse_blobs_grid(seed + 10 * i, nx, ny, nz, nblobs=5 + 3 * i, max_extent=20 + 60 * i) for i in range(B)])
+    voxel, lam = (2.0, 2.0, 2.5), 11.0
+    npx, npy, th = 20, 17, 25.0
+    I = sm.simulate(dev(g), voxel, lam, npx, npy, th, method=METHODS[method][0], flags=METHODS[method][1]).cpu().numpy()
+    for b in range(B):
+        ref = O.simulate(g[b], voxel, lam, npx, npy, th)
+        assert_parity(I[b], ref, what=f"sparse blobs seed={seed} b={b} {method}")
+
+
 @pytest.mark.parametrize("method", list(METHODS))
 def test_cfg2_ellipsoid_half_scale_oriented(sm, method):
     w = W.config(1, scale=0.5)
