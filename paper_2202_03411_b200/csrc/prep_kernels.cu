@@ -140,9 +140,13 @@ cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *
 }
 
 // ------------------------------------------------------------------------------------------------ operand B
-// rho~ FP32 [b][z][y][x] -> FP16 split planes [b][z][4][x_pad][y_pad] (y fastest = K-major for UMMA),
-// planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo, scaled by sB[b] = 2^(13 - e), max in [2^(e-1), 2^e).
-// 32x32 (x,y) tiles transposed through shared memory; padding written as zeros.
+// rho~ FP32 [b][z][y][x] -> FP16 split planes, scaled by sB[b] = 2^(13 - e) (max in [2^(e-1), 2^e)), laid out as
+// the UMMA B operand wants to find it in shared memory, so that one TMA box of 256-byte rows is one k-step:
+//   B[b][z][y16][xt][hg][plane][atom]      atom = 8 x-rows x 16 y of FP16 = 256 bytes, SWIZZLE_32B pattern applied
+//   planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo;  x = 128 xt + 16 blk + 8 half + r  ->  hg = 8 half + blk, row r
+// (each CTA of a pair owns one `half` of every 16-x block; a run of hg is then a contiguous x range in both).
+// Inside an atom, row r is 32 bytes (y fastest = K-major) and its two 16-byte chunks are swapped when r >= 4.
+// Also emits the occupancy word of every (slice, x tile, y group): bit 8*yi + xi = the 16-y x 16-x block is non-zero.
 __device__ __forceinline__ float scale_from_maxbits(unsigned bits) {
     const float m = __uint_as_float(bits);
     if (!(m > 0.f)) return 1.f;
@@ -151,9 +155,9 @@ __device__ __forceinline__ float scale_from_maxbits(unsigned bits) {
     return ldexpf(1.f, kScaleBExp - e);
 }
 
-__global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nx_pad, int ny_pad,
+__global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nxt, int ny16, int ngroups,
                               const unsigned *__restrict__ maxbits, float *__restrict__ ampscale, float dV,
-                              __half *__restrict__ B, unsigned long long *__restrict__ mask, int nxt, int ngroups) {
+                              __half *__restrict__ B, unsigned long long *__restrict__ mask) {
     __shared__ float2 tile[32][33];
     const int bz = blockIdx.x;  // b*nz + z
     const int b = bz / nz;
@@ -166,31 +170,42 @@ __global__ void pack_b_kernel(const float2 *__restrict__ rho, int nx, int ny, in
         tile[r][tx] = (y < ny && x < nx) ? src[(size_t)y * nx + x] : make_float2(0.f, 0.f);
     }
     __syncthreads();
-    const size_t plane = (size_t)nx_pad * ny_pad;
-    __half *dst = B + (size_t)bz * 4 * plane;
-    unsigned long long occ = 0;  // occupancy bits of this warp's 16 x 16 blocks (the contraction skips empty ones)
-    for (int r = ty; r < 32; r += 8) {
-        const int x = x0 + r, y = y0 + tx;  // x < nx_pad, y < ny_pad by grid construction
-        const float2 v = tile[tx][r];
+    // one warp per atom: ty -> (x8 group ax = ty & 3, y16 block ay = ty >> 2); lane -> row r = tx / 4, 4 y from 4 (tx % 4)
+    const int ax = ty & 3, ay = ty >> 2;
+    const int r = tx >> 2, yq = (tx & 3) * 4;
+    const int xl = ax * 8 + r, yl = ay * 16 + yq;
+    __half h[4][4];   // [plane][y]
+    bool any = false;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float2 v = tile[yl + i][xl];
         const float re = v.x * s, im = v.y * s;
-        const __half reh = __float2half_rn(re), imh = __float2half_rn(im);
-        const __half rel = __float2half_rn(re - __half2float(reh)), iml = __float2half_rn(im - __half2float(imh));
-        // row order inside a 128-x tile: x = 16 blk + t -> row 64 (t / 8) + 8 blk + t % 8, so that each CTA of a pair
-        // (rows 0-63 / 64-127) holds half of every 16-x block and a row prefix of both halves is a contiguous x range
-        const int xrow = (x & ~(kTileX - 1)) | (((x >> 3) & 1) << 6) | (((x >> 4) & 7) << 3) | (x & 7);
-        const size_t o = (size_t)xrow * ny_pad + y;
-        dst[o] = reh;
-        dst[plane + o] = rel;
-        dst[2 * plane + o] = imh;
-        dst[3 * plane + o] = iml;
-        const bool nz16 = ((__half_as_ushort(reh) | __half_as_ushort(rel) | __half_as_ushort(imh) | __half_as_ushort(iml)) & 0x7fffu) != 0;
-        const unsigned bal = __ballot_sync(0xffffffffu, nz16);
-        const int xi = (x % kTileX) / 16, yi = ((y0 % (kGroupYB * kBlockY)) / 16);
-        if (bal & 0x0000ffffu) occ |= 1ull << (8 * yi + xi);
-        if (bal & 0xffff0000u) occ |= 1ull << (8 * (yi + 1) + xi);
+        h[0][i] = __float2half_rn(re);
+        h[1][i] = __float2half_rn(re - __half2float(h[0][i]));
+        h[2][i] = __float2half_rn(im);
+        h[3][i] = __float2half_rn(im - __half2float(h[2][i]));
+        any |= ((__half_as_ushort(h[0][i]) | __half_as_ushort(h[1][i]) | __half_as_ushort(h[2][i]) |
+                 __half_as_ushort(h[3][i])) & 0x7fffu) != 0;
     }
-    if (tx == 0 && occ)
-        atomicOr(mask + ((size_t)bz * nxt + x0 / kTileX) * ngroups + y0 / (kGroupYB * kBlockY), occ);
+    const int x = x0 + ax * 8, y = y0 + ay * 16;          // first x / y of the atom
+    const int xt = x / kTileX, blk = (x % kTileX) / 16, half = (x >> 3) & 1;
+    const int y16 = y >> 4;
+    if (y16 < ny16) {
+        const size_t atom = ((((size_t)bz * ny16 + y16) * nxt + xt) * 16 + half * 8 + blk) * 4;   // x 256 bytes, + plane
+        const int chunk = (yq >> 3) ^ (r >> 2);                                                 // SWIZZLE_32B
+        const int off = r * 16 + chunk * 8 + (yq & 7);                                          // in FP16 elements
+#pragma unroll
+        for (int pl = 0; pl < 4; ++pl) {
+            uint2 w;
+            w.x = (uint32_t)__half_as_ushort(h[pl][0]) | ((uint32_t)__half_as_ushort(h[pl][1]) << 16);
+            w.y = (uint32_t)__half_as_ushort(h[pl][2]) | ((uint32_t)__half_as_ushort(h[pl][3]) << 16);
+            *(uint2 *)(B + (atom + pl) * 128 + off) = w;
+        }
+        if (__any_sync(0xffffffffu, any) && tx == 0) {
+            const int yi = (y % (kGroupYB * kBlockY)) / 16;
+            atomicOr(mask + ((size_t)bz * nxt + xt) * ngroups + y / (kGroupYB * kBlockY), 1ull << (8 * yi + blk));
+        }
+    }
     if (blockIdx.y == 0 && blockIdx.z == 0 && tx == 0 && ty == 0 && (bz % nz) == 0) ampscale[b] = dV / (kScaleA * s);
 }
 
@@ -199,9 +214,8 @@ cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_m
     cudaError_t e = cudaMemsetAsync(d_mask, 0, sizeof(unsigned long long) * (size_t)p.batch * p.nz * p.nxt * p.ngroups, st);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)(p.batch * p.nz), p.nx_pad / 32, p.ny_pad / 32);
-    pack_b_kernel<<<grid, dim3(32, 8), 0, st>>>((const float2 *)d_rho, p.nx, p.ny, p.nz, p.nx_pad, p.ny_pad,
-                                                d_maxbits, d_ampscale, (float)(p.dx * p.dy * p.dz), d_B, d_mask, p.nxt,
-                                                p.ngroups);
+    pack_b_kernel<<<grid, dim3(32, 8), 0, st>>>((const float2 *)d_rho, p.nx, p.ny, p.nz, p.nxt, p.ny_pad / 16, p.ngroups,
+                                                d_maxbits, d_ampscale, (float)(p.dx * p.dy * p.dz), d_B, d_mask);
     return cudaGetLastError();
 }
 

@@ -62,6 +62,13 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const void *tmap, uint64_
         : "memory");
 }
 
+// 4-D variants (the B operand: {atom, plane, x group, y step})
+__device__ __forceinline__ void tma_load_4d(void *dst, const void *tmap, uint64_t *bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
 // bring a tile into L2 only (no shared-memory destination, no completion to wait for)
 __device__ __forceinline__ void tma_prefetch_l2_3d(const void *tmap, int c0, int c1, int c2) {
     asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
@@ -142,6 +149,12 @@ __device__ __forceinline__ void tma_load_3d_2sm(void *dst, const void *tmap, uin
         ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar) & kPeerBitMask), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
 }
+__device__ __forceinline__ void tma_load_4d_2sm(void *dst, const void *tmap, uint64_t *bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar) & kPeerBitMask), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
 // arrive on the barrier at the same offset in CTA `cta` of the cluster
 __device__ __forceinline__ void mbar_arrive_cluster(uint64_t *bar, uint32_t cta) {
     asm volatile(
@@ -189,13 +202,13 @@ __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr) {
     d |= (uint64_t)2 << 61;                        // SWIZZLE_128B, bits [61,64)
     return d;
 }
-// Same for a K-major tile of 32-byte rows with the 32-byte swizzle (TMA box {16 x 16-bit, rows} with SWIZZLE_32B):
-// one row = one K step of 16 FP16, 8-row groups are 256 bytes apart, layout type 6.
-__device__ __forceinline__ uint64_t umma_smem_desc_sw32(uint32_t smem_addr) {
+// K-major tile of 32-byte rows (one row = one K step of 16 FP16) in the SWIZZLE_32B pattern, 8-row groups
+// `group_stride` bytes apart, layout type 6.
+__device__ __forceinline__ uint64_t umma_smem_desc_sw32(uint32_t smem_addr, uint32_t group_stride) {
     uint64_t d = 0;
     d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
     d |= (uint64_t)1 << 16;
-    d |= (uint64_t)(256 >> 4) << 32;
+    d |= (uint64_t)(group_stride >> 4) << 32;
     d |= (uint64_t)1 << 46;
     d |= (uint64_t)6 << 61;
     return d;

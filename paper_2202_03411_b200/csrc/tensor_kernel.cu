@@ -35,15 +35,15 @@ size_t tensor_smem_bytes() { return kSmemTotal; }
 #ifdef SCATMAN_TIMING
 // debug-only cycle accounting (built by _work scripts with -DSCATMAN_TIMING; never in the product build)
 __device__ long long g_timing[148 * 8];
-#define TIMING_DECL(name) long long name = 0
-#define TIMED_WAIT(acc, stmt) do { long long _t0 = clock64(); stmt; acc += clock64() - _t0; } while (0)
+#define TIMING_DECL(name) long long name = 0, name##_long = 0, name##_n = 0
+#define TIMED_WAIT(acc, stmt) do { long long _t0 = clock64(); stmt; long long _d = clock64() - _t0; acc += _d; if (_d > 400) { acc##_long += _d; ++acc##_n; } } while (0)
 #else
 #define TIMING_DECL(name)
 #define TIMED_WAIT(acc, stmt) stmt
 #endif
 
 struct TensorParams {
-    int nz, nxt, nyb, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
+    int nz, nxt, nyb, ny16, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
     int64_t npix_pad;
     const float2 *anchor, *fine, *mz;
     const unsigned long long *mask;   // [batch][nz][nxt][ngroups]: bit 8*yi + xi = 16-y x 16-x block of rho~ is non-zero
@@ -101,6 +101,20 @@ struct Units {
         ahead = load(32 + lane);
         live = __ballot_sync(0xffffffffu, cur != 0ull);
     }
+    // occupancy word of the next non-empty unit only (the MMA issuer needs nothing else)
+    __device__ __forceinline__ bool next_mask(unsigned long long &m) {
+        while (live == 0u) {
+            base += 32;
+            if (base >= total) return false;
+            cur = ahead;
+            ahead = load(base + 32 + lane);
+            live = __ballot_sync(0xffffffffu, cur != 0ull);
+        }
+        const int pos = __ffs((int)live) - 1;
+        live &= live - 1;
+        m = __shfl_sync(0xffffffffu, cur, pos);
+        return true;
+    }
     // next non-empty unit; false when the item is exhausted (warp-uniform result)
     __device__ __forceinline__ bool next(int &b, int &j, int &xt, unsigned long long &m) {
         while (live == 0u) {
@@ -152,8 +166,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     uint64_t *bars = (uint64_t *)(smem + kSmemA + kSmemB);
     uint64_t *a_full = bars + 0, *a_empty = bars + 1;
     uint64_t *b_full = bars + 2, *b_empty = bars + 2 + kMaxStagesB;
-    uint64_t *t_full = bars + 2 + 2 * kMaxStagesB, *t_empty = t_full + 2;
-    uint32_t *tmem_ptr = (uint32_t *)(t_empty + 2);
+    uint64_t *t_full = bars + 2 + 2 * kMaxStagesB, *t_empty = t_full + 2, *first_done = t_empty + 2;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = NCTA == 2 ? ptx::cluster_ctarank() : 0u;
@@ -168,13 +182,14 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     }
     if (warp == 1 && lane == 0) {
         ptx::mbar_init(a_full, 1);
-        ptx::mbar_init(a_empty, 1);
+        ptx::mbar_init(a_empty, 2);      // both MMA issuers
         for (int i = 0; i < kStagesB; ++i) {
             ptx::mbar_init(b_full + i, 1);
             ptx::mbar_init(b_empty + i, 1);
         }
         for (int i = 0; i < 2; ++i) {
-            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_full + i, 2);   // both MMA issuers
+            ptx::mbar_init(first_done + i, 1);
             ptx::mbar_init(t_empty + i, 4 * NCTA);
         }
         ptx::fence_barrier_init();
@@ -228,26 +243,34 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             while (un.next(ub, uj, uxt, m)) {
                 int xa, xm;
                 unit_range<NCTA>(m, xa, xm);
-                const CUtensorMap *tmb = &tmB.m[xm - 1];                // box {16 y, 8 xm rows per CTA (128 for one CTA), 4 planes}
-                const uint32_t tx_bytes = NCTA == 2 ? (uint32_t)(2 * 4 * 8 * xm * 32) : (uint32_t)(4 * kTileX * 32);
+                // one box = one 16-y step: {256-byte atom, 4 planes, xm x-groups of this CTA's half (16 for one CTA)}
+                const CUtensorMap *tmb = &tmB.m[xm - 1];
+                const uint32_t tx_bytes = NCTA == 2 ? (uint32_t)(2 * xm * 1024) : (uint32_t)kSlotBytes;
                 for (int yi = 0; yi < 4 * nybg; ++yi) {
                     if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // this 16-y step of the slice tile is empty
                     ptx::mbar_wait(b_empty + slot, phase ^ 1);
                     if (ptx::elect_one()) {
+#ifdef SCATMAN_ABL_NOLOAD
+                        if (leader) ptx::mbar_arrive(b_full + slot);
+#else
                         if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, tx_bytes);
+#endif
                         void *dst = sB + slot * kSlotB;
-                        const int cy = it.g * (kGroupYB * kBlockY) + 16 * yi;
-                        const int cx = uxt * kTileX + (int)rank * (kTileX / NCTA) + 8 * xa;
-                        const int cp = (ub * P.nz + uj) * 4;
-                        if (NCTA == 2) ptx::tma_load_3d_2sm(dst, tmb, b_full + slot, cy, cx, cp);
-                        else ptx::tma_load_3d(dst, tmb, b_full + slot, cy, cx, cp);
+                        const int cg = uxt * 16 + (NCTA == 2 ? (int)rank * 8 + xa : 0);
+                        const int cs = (ub * P.nz + uj) * P.ny16 + it.g * (kGroupYB * kBlockY / 16) + yi;
+#ifndef SCATMAN_ABL_NOLOAD
+                        if (NCTA == 2) ptx::tma_load_4d_2sm(dst, tmb, b_full + slot, 0, 0, cg, cs);
+                        else ptx::tma_load_4d(dst, tmb, b_full + slot, 0, 0, cg, cs);
+#else
+                        (void)dst; (void)cg; (void)cs; (void)tmb;
+#endif
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                 }
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == 1 || warp == 3) {
       if (leader) {
         // ===================================================================== MMA issuer (leader CTA only)
         // Warp-uniform loop; descriptors are uniform-register arithmetic; one elected lane issues the
@@ -255,7 +278,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         constexpr uint32_t idesc_pos0 = ptx::umma_idesc_f16(kTileP * NCTA, 0, false);   // N is set per unit
         constexpr uint32_t idesc_neg0 = ptx::umma_idesc_f16(kTileP * NCTA, 0, true);
         const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
-        const uint64_t descB0 = ptx::umma_smem_desc_sw32(ptx::smem_u32(sB));
+        const uint64_t descB0 = ptx::umma_smem_desc_sw32(ptx::smem_u32(sB), 1024);   // x groups 1 KB apart: 4 planes x 256 B
         constexpr uint64_t kSlotDescA = kSlotBytes >> 4;
         constexpr uint64_t kSlotDescB = kSlotB >> 4;
         auto mma = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
@@ -266,6 +289,11 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x3);
             else ptx::umma_commit(bar);
         };
+        auto commit_local = [](uint64_t *bar) {   // this (leader) CTA's barrier only
+            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x1);
+            else ptx::umma_commit(bar);
+        };
+        const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
         int slot = 0;
         uint32_t phase = 0;
         uint32_t u = 0;
@@ -279,50 +307,64 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
             TIMED_WAIT(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
             ptx::tc_fence_after();
+            // All-zero units never appear: no MMA, no accumulator hand-over.
+            // TWO issuers (warps 1 and 3) share every unit: k-step n of a unit belongs to issuer n % 2.  For N < 112 a
+            // tcgen05.mma is bound by its shared-memory operand fetch and, measured, a single issuing thread then
+            // exposes every cycle it spends between two k-steps (barrier poll, fences, descriptor arithmetic); two
+            // threads hide each other's gaps.  The unit's first k-step (accumulate = 0) is issuer 0's; issuer 1 starts on
+            // the unit only after that k-step has completed (first_done).  Both commit the accumulator (t_full counts 2).
             Units un;
             un.begin(it, P, lane);
-            int ub, uj, uxt;
             unsigned long long m;
-            while (un.next(ub, uj, uxt, m)) {   // all-zero units never appear: no MMA, no accumulator hand-over
+            while (un.next_mask(m)) {
                 {
                     const uint32_t buf = u & 1;
-                    TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, ((u >> 1) & 1) ^ 1));
+                    const uint32_t upar = (u >> 1) & 1;
+                    TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
                     ptx::tc_fence_after();
                     const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                     int xa, xm;
                     unit_range<NCTA>(m, xa, xm);
                     const uint32_t idesc_pos = idesc_pos0 | ((uint32_t)(2 * xm) << 17);   // N = 16 xm
                     const uint32_t idesc_neg = idesc_neg0 | ((uint32_t)(2 * xm) << 17);
-                    const uint64_t pstride = (uint64_t)((NCTA == 2 ? 8 * xm : kTileX) * 32) >> 4;   // B plane stride in a slot
-                    uint32_t started = 0u;   // 0 until the first k-step of this unit has initialised D_re and D_im
+                    constexpr uint64_t pstride = 256 >> 4;   // B planes of one x group are 256 bytes apart
+                    int kidx = 0;            // k-step index within the unit
                     for (int yi = 0; yi < 4 * nybg; ++yi) {
                         if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // empty 16-y step: never loaded
-                        TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-                            // A planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo of this k-step (32 bytes = 2 descriptor units per step)
-                            const uint64_t a_reh = descA0 + (uint64_t)(yi >> 2) * kSlotDescA + (uint64_t)((yi & 3) * 2);
-                            const uint64_t a_rel = a_reh + (uint64_t)(1 * kGroupYB) * kSlotDescA;
-                            const uint64_t a_imh = a_reh + (uint64_t)(2 * kGroupYB) * kSlotDescA;
-                            const uint64_t a_iml = a_reh + (uint64_t)(3 * kGroupYB) * kSlotDescA;
-                            const uint64_t b_reh = descB0 + (uint64_t)slot * kSlotDescB;
-                            const uint64_t b_rel = b_reh + pstride, b_imh = b_rel + pstride, b_iml = b_imh + pstride;
-                            mma(d_re, a_reh, b_reh, idesc_pos, started);
-                            mma(d_im, a_imh, b_reh, idesc_pos, started);
-                            mma(d_re, a_rel, b_reh, idesc_pos, 1u);
-                            mma(d_im, a_iml, b_reh, idesc_pos, 1u);
-                            mma(d_re, a_reh, b_rel, idesc_pos, 1u);
-                            mma(d_im, a_imh, b_rel, idesc_pos, 1u);
-                            mma(d_re, a_imh, b_imh, idesc_neg, 1u);
-                            mma(d_im, a_reh, b_imh, idesc_pos, 1u);
-                            mma(d_re, a_iml, b_imh, idesc_neg, 1u);
-                            mma(d_im, a_rel, b_imh, idesc_pos, 1u);
-                            mma(d_re, a_imh, b_iml, idesc_neg, 1u);
-                            mma(d_im, a_reh, b_iml, idesc_pos, 1u);
-                            commit(b_empty + slot);
+                        if ((kidx & 1) == iw) {
+                            if (kidx == 1) {   // issuer 1's first k-step of the unit: D must have been initialised
+                                ptx::mbar_wait(first_done + buf, upar);
+                                ptx::tc_fence_after();
+                            }
+                            TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                            ptx::tc_fence_after();
+                            if (ptx::elect_one()) {
+                                // A planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo of this k-step (32 bytes = 2 descriptor units per step)
+                                const uint64_t a_reh = descA0 + (uint64_t)(yi >> 2) * kSlotDescA + (uint64_t)((yi & 3) * 2);
+                                const uint64_t a_rel = a_reh + (uint64_t)(1 * kGroupYB) * kSlotDescA;
+                                const uint64_t a_imh = a_reh + (uint64_t)(2 * kGroupYB) * kSlotDescA;
+                                const uint64_t a_iml = a_reh + (uint64_t)(3 * kGroupYB) * kSlotDescA;
+                                const uint64_t b_reh = descB0 + (uint64_t)slot * kSlotDescB;
+                                const uint64_t b_rel = b_reh + pstride, b_imh = b_rel + pstride, b_iml = b_imh + pstride;
+                                const uint32_t acc0 = kidx != 0 ? 1u : 0u;
+                                mma(d_re, a_reh, b_reh, idesc_pos, acc0);
+                                mma(d_im, a_imh, b_reh, idesc_pos, acc0);
+                                mma(d_re, a_rel, b_reh, idesc_pos, 1u);
+                                mma(d_im, a_iml, b_reh, idesc_pos, 1u);
+                                mma(d_re, a_reh, b_rel, idesc_pos, 1u);
+                                mma(d_im, a_imh, b_rel, idesc_pos, 1u);
+                                mma(d_re, a_imh, b_imh, idesc_neg, 1u);
+                                mma(d_im, a_reh, b_imh, idesc_pos, 1u);
+                                mma(d_re, a_iml, b_imh, idesc_neg, 1u);
+                                mma(d_im, a_rel, b_imh, idesc_pos, 1u);
+                                mma(d_re, a_imh, b_iml, idesc_neg, 1u);
+                                mma(d_im, a_reh, b_iml, idesc_pos, 1u);
+                                commit(b_empty + slot);
+                                if (kidx == 0) commit_local(first_done + buf);
+                            }
+                            __syncwarp();
                         }
-                        __syncwarp();
-                        started = 1u;
+                        ++kidx;
                         if (++slot == kStagesB) { slot = 0; phase ^= 1; }
                     }
                     if (ptx::elect_one()) commit(t_full + buf);
@@ -334,11 +376,15 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             __syncwarp();
         }
 #ifdef SCATMAN_TIMING
-        if (lane == 0) {
+        if (lane == 0 && iw == 0) {
             g_timing[blockIdx.x * 8 + 0] = clock64() - t_begin;
             g_timing[blockIdx.x * 8 + 1] = w_tempty;
             g_timing[blockIdx.x * 8 + 2] = w_bfull;
             g_timing[blockIdx.x * 8 + 3] = w_afull;
+            g_timing[blockIdx.x * 8 + 7] = w_bfull_long;
+            g_timing[blockIdx.x * 8 + 6] = w_bfull_n;
+            g_timing[blockIdx.x * 8 + 5] = w_tempty_long;
+            g_timing[blockIdx.x * 8 + 4] = w_tempty_n;
         }
 #endif
       }
@@ -406,6 +452,17 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         const uint32_t half = 8u * (uint32_t)xm;
                         // software-pipelined: the loads of block a+1 are in flight while block a is reduced; the
                         // accumulator buffer is handed back to the MMA warp as soon as its last column has landed
+#ifdef SCATMAN_ABL_NOEPI
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);
+                            else ptx::mbar_arrive(t_empty + buf);
+                        }
+                        ++u;
+                        f_re += anc[0].x + (float)half + (float)t_im;
+                        continue;
+#endif
                         uint32_t gre[2][16], gim[2][16];
                         ptx::tmem_ld8(t_re, gre[0]);
                         ptx::tmem_ld8(t_re + half, gre[0] + 8);
@@ -466,7 +523,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             }
         }
 #ifdef SCATMAN_TIMING
-        if (warp == 4 && lane == 0) {
+        if (warp == 4 && lane == 0 && (blockIdx.x & 1)) {
             g_timing[blockIdx.x * 8 + 4] = clock64() - e_begin;
             g_timing[blockIdx.x * 8 + 5] = w_tfull;
             g_timing[blockIdx.x * 8 + 6] = u;
@@ -500,16 +557,13 @@ static EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
-static bool encode_planes(CUtensorMap *tm, const void *base, uint64_t inner, uint64_t rows, uint64_t planes,
-                          uint32_t box_inner, uint32_t box_rows, uint32_t box_planes, CUtensorMapSwizzle swizzle) {
+static bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
+                       const cuuint32_t *box, CUtensorMapSwizzle swizzle) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return false;
-    cuuint64_t dims[3] = {inner, rows, planes};
-    cuuint64_t strides[2] = {inner * 2, inner * rows * 2};
-    cuuint32_t box[3] = {box_inner, box_rows, box_planes};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void *>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, (cuuint32_t)rank, const_cast<void *>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -545,19 +599,28 @@ cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st,
     const int ncta = p.t_ncta;
     CUtensorMap tmA;
     TmapsB tmB;
-    bool ok = encode_planes(&tmA, t.d_A, (uint64_t)p.ny_pad, (uint64_t)p.npix_pad, 4, kBlockY, kTileP, 1,
-                            CU_TENSOR_MAP_SWIZZLE_128B);
-    // B: one box = one 16-y k-step of all four planes; CTA pairs fetch only the rows of a unit's x range (one box
-    // height per range length)
-    for (int i = 0; ok && i < kTileX / 16; ++i)
-        ok = encode_planes(&tmB.m[i], t.d_B, (uint64_t)p.ny_pad, (uint64_t)p.nx_pad, (uint64_t)p.batch * p.nz * 4, 16,
-                           ncta == 2 ? 8 * (i + 1) : kTileX, 4, CU_TENSOR_MAP_SWIZZLE_32B);
+    // A: fp16 [4 planes][npix_pad][ny_pad], box = one 64-y K-block of a 128-pixel tile, 128-byte swizzle
+    bool ok;
+    {
+        cuuint64_t dims[3] = {(cuuint64_t)p.ny_pad, (cuuint64_t)p.npix_pad, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)p.ny_pad * 2, (cuuint64_t)p.ny_pad * (cuuint64_t)p.npix_pad * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kBlockY, (cuuint32_t)kTileP, 1};
+        ok = encode_map(&tmA, t.d_A, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+    // B: fp16 [batch nz ny16][16 nxt x-groups][4 planes][128-element atom] (pack_b_kernel); box = one 16-y step of
+    // i+1 x-groups (CTA pairs fetch only the groups of a unit's x range) or of the whole tile (single CTA)
+    for (int i = 0; ok && i < kTileX / 16; ++i) {
+        cuuint64_t dims[4] = {128, 4, (cuuint64_t)p.nxt * 16, (cuuint64_t)p.batch * p.nz * (p.ny_pad / 16)};
+        cuuint64_t strides[3] = {256, 1024, (cuuint64_t)p.nxt * 16 * 1024};
+        cuuint32_t box[4] = {128, 4, (cuuint32_t)(ncta == 2 ? i + 1 : 16), 1};
+        ok = encode_map(&tmB.m[i], t.d_B, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE);
+    }
     if (!ok) {
         if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
         return cudaErrorUnknown;
     }
     TensorParams P;
-    P.nz = p.nz; P.nxt = p.nxt; P.nyb = p.nyb; P.ngroups = p.ngroups; P.ntiles = p.ntiles; P.batch = p.batch;
+    P.nz = p.nz; P.nxt = p.nxt; P.nyb = p.nyb; P.ny16 = p.ny_pad / 16; P.ngroups = p.ngroups; P.ntiles = p.ntiles; P.batch = p.batch;
     P.nzs = p.t_nzs;
     P.bpc = (p.batch + p.t_nchunks - 1) / p.t_nchunks;
     P.nchunks = (p.batch + P.bpc - 1) / P.bpc;
