@@ -21,6 +21,9 @@ sys.path.insert(0, ROOT)
 
 SPLITS = 3           # FP16x3: AhBh + AlBh + AhBl
 FLOP_PER_TERM = 8    # one complex MAC
+# dram__bytes_read.sum + dram__bytes_write.sum of one contraction launch, from the committed `ncu --set full` capture
+# (profiles/r01_contract_cfg3_full.md); only the workload that was captured has a number
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": None}
 
 
 def load_peaks():
@@ -236,13 +239,24 @@ def main():
     terms_per_pattern = w.nvox * w.npix
     peaks = load_peaks()
     k_ms = sum(kernel_ms) / len(kernel_ms)
-    issued = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch          # tensor flop per contraction launch
-    achieved = issued / (k_ms * 1e-3) / 1e12
+    dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
     if args.method == 1:
+        # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
+        # One extra, untimed call with the counting flag (same inputs, same schedule).
+        sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, workspace=ws, out=out,
+                    stream=stream, flags=B.FLAG_COUNT_ISSUED)
+        blocks = sm.last_issued_blocks()
+        npix_pad = (w.npix + 255) // 256 * 256
+        issued = blocks * 256 * npix_pad * SPLITS * FLOP_PER_TERM         # tensor flop per contraction launch
+        achieved = issued / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "tensor", "kernel": "msft_contract_kernel", "achieved": achieved, "peak": peaks["sustained"],
-                    "unit": "TFLOP/s", "frac": achieved / peaks["sustained"], "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / peaks["sustained"],
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name),
                     "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
-                    "useful_tflops": achieved / SPLITS, "kernel_ms": k_ms, "kernel_share_of_step": k_ms * args.steps / total_ms * world / world}
+                    "achieved_is": "issued tensor flop (24 per issued voxel-pixel term: 8 flop x 3 split products) / kernel time",
+                    "issued_fraction_of_dense": issued / dense, "dense_equivalent_tflops": dense / (k_ms * 1e-3) / 1e12,
+                    "useful_dense_tflops": dense / SPLITS / (k_ms * 1e-3) / 1e12, "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms * args.steps / total_ms}
     else:
         # direct sincos: 2 MUFU per term; SFU peak = 148 SMs x 16 MUFU/clk x max clock
         peak = 148 * 16 * 1.965e9 / 2 / 1e12

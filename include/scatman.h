@@ -87,6 +87,10 @@ typedef struct {
  * the default CTA pairs (cta_group::2, UMMA 256x128, each CTA holding half of every B tile).  Same results up to
  * summation order; kept for comparison and as the smaller-cluster variant. */
 #define SCATMAN_FLAG_SINGLE_CTA 1u
+/* Tensor path only: also count the work the contraction really issues (one extra small kernel), for
+ * scatman_last_issued_blocks.  The contraction skips 16-y steps of a (slice, 128-x tile, 128-y group) unit whose
+ * rho~ values are all zero and narrows every unit to the range of its non-empty 16-x blocks. */
+#define SCATMAN_FLAG_COUNT_ISSUED 2u
 
 /* Create / destroy a context on CUDA device `device`.  Fails with SCATMAN_UNSUPPORTED_DEVICE unless the
  * device is compute capability 10.x.  scatman_destroy(NULL) is SCATMAN_OK. */
@@ -142,6 +146,12 @@ int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count);
 /* Device time of the contraction kernel (step a4+a5) of the last scatman_simulate* call, measured with
  * CUDA events on the call's stream.  Synchronises on the end event.  -1 if none was recorded. */
 int scatman_last_contraction_ms(scatman_ctx *ctx, float *ms);
+
+/* With SCATMAN_FLAG_COUNT_ISSUED: the number of 16-y x 16-x blocks of rho~ (256 voxels each) the contraction of the last
+ * scatman_simulate* call multiplied against EVERY pixel, summed over slices and batch items; the dense count is
+ * batch * nz * ceil(ny/16) * ceil(nx/16) blocks of the padded grid.  Issued tensor flop = blocks * 256 * npix_pad * 24.
+ * Synchronises with the call's stream.  -1 if the last call did not count. */
+int scatman_last_issued_blocks(scatman_ctx *ctx, int64_t *blocks);
 
 const char *scatman_status_string(int status);
 const char *scatman_last_error(scatman_ctx *ctx); /* never NULL; "" if none */

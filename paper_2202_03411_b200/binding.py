@@ -18,11 +18,12 @@ RHO_LINEAR, RHO_N2M1 = 0, 1
 METHOD_AUTO, METHOD_TENSOR, METHOD_SIMT_SINCOS, METHOD_SIMT_TABLE = 0, 1, 2, 3
 PRECISION_AUTO, PRECISION_FP16X3 = 0, 1
 FLAG_SINGLE_CTA = 1
+FLAG_COUNT_ISSUED = 2
 
 EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
-    "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_status_string", "scatman_last_error",
+    "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
 
@@ -74,6 +75,7 @@ def load_library() -> C.CDLL:
                                         C.POINTER(Options), vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.scatman_last_issued_blocks.argtypes = [vp, C.POINTER(i64)]
     L.scatman_status_string.argtypes = [C.c_int]
     L.scatman_status_string.restype = C.c_char_p
     L.scatman_last_error.argtypes = [vp]
@@ -244,6 +246,11 @@ class Scatman:
     def last_launch_count(self) -> int:
         n = C.c_int32(0)
         self._check(self.lib.scatman_last_launch_count(self._ctx, C.byref(n)))
+        return int(n.value)
+
+    def last_issued_blocks(self) -> int:
+        n = C.c_int64(-1)
+        self._check(self.lib.scatman_last_issued_blocks(self._ctx, C.byref(n)))
         return int(n.value)
 
     def last_contraction_ms(self) -> float:

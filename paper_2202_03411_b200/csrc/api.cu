@@ -16,6 +16,8 @@ struct scatman_ctx {
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
+    const unsigned long long *d_count = nullptr;   // issued-block counter of the last call (in its workspace)
+    cudaStream_t count_stream = nullptr;
     // arena of scatman_simulate_host (grow-only)
     cudaStream_t host_stream = nullptr;
     void *arena = nullptr;
@@ -87,6 +89,7 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
         p.off_fine = take(sizeof(float2) * (size_t)p.ntiles * kFine * kTileP);
         p.off_mz = take(sizeof(float2) * (size_t)p.ntiles * p.nz * kTileP);
         p.off_mask = take(sizeof(unsigned long long) * (size_t)batch * p.nz * p.nxt * p.ngroups);
+        p.off_count = take(sizeof(unsigned long long));
     }
     p.total = off;
     return p;
@@ -112,7 +115,7 @@ static bool valid_detector(const scatman_detector *d) {
 }
 static bool valid_options(const scatman_options &o) {
     return (o.rho_mode == SCATMAN_RHO_LINEAR || o.rho_mode == SCATMAN_RHO_N2M1) && o.method >= 0 && o.method <= 3 &&
-           o.precision >= 0 && o.precision <= 1 && (o.flags & ~(uint32_t)SCATMAN_FLAG_SINGLE_CTA) == 0;
+           o.precision >= 0 && o.precision <= 1 && (o.flags & ~(uint32_t)(SCATMAN_FLAG_SINGLE_CTA | SCATMAN_FLAG_COUNT_ISSUED)) == 0;
 }
 static bool valid_quats(const double *q, int batch) {
     for (int b = 0; b < batch; ++b) {
@@ -284,6 +287,7 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
     int nl = 0;
     cudaError_t e = cudaSuccess;
     ctx->ev_valid = false;
+    ctx->d_count = nullptr;
 
     const double *d_q = d_q_in;
     if (!d_q) {
@@ -315,6 +319,13 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
         e = launch_pack_b(rho, p, maxbits, ampscale, (__half *)(ws + p.off_B), (unsigned long long *)(ws + p.off_mask), st);
         ++nl;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "pack_b");
+        if (o.flags & SCATMAN_FLAG_COUNT_ISSUED) {
+            e = launch_count_issued((const unsigned long long *)(ws + p.off_mask), p, (unsigned long long *)(ws + p.off_count), st);
+            ++nl;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "count_issued");
+            ctx->d_count = (const unsigned long long *)(ws + p.off_count);
+            ctx->count_stream = st;
+        }
         e = launch_tables(d_q, p, (__half *)(ws + p.off_A), (float2 *)(ws + p.off_anchor), (float2 *)(ws + p.off_fine),
                           (float2 *)(ws + p.off_mz), st, &nl);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "tables");
@@ -406,6 +417,18 @@ int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_gri
 int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count) {
     if (!ctx || !count) return SCATMAN_INVALID_ARGUMENT;
     *count = ctx->last_launches;
+    return SCATMAN_OK;
+}
+
+int scatman_last_issued_blocks(scatman_ctx *ctx, int64_t *blocks) {
+    if (!ctx || !blocks) return SCATMAN_INVALID_ARGUMENT;
+    *blocks = -1;
+    if (!ctx->d_count) return SCATMAN_OK;
+    unsigned long long v = 0;
+    cudaError_t e = cudaMemcpyAsync(&v, ctx->d_count, sizeof(v), cudaMemcpyDeviceToHost, ctx->count_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->count_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "issued blocks");
+    *blocks = (int64_t)v;
     return SCATMAN_OK;
 }
 

@@ -40,7 +40,7 @@ struct Plan {
     int t_ncta = 2;               // CTAs per work item: 2 = cta_group::2 pairs (default), 1 = single CTA
     // workspace offsets (bytes)
     size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
-           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, total = 0;
+           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, total = 0;
 };
 
 int simt_zsplit(const Plan &p, int num_sms);
@@ -54,6 +54,8 @@ cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *
                             cudaStream_t st);
 cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_maxbits, float *d_ampscale,
                           __half *d_B, unsigned long long *d_mask, cudaStream_t st);
+cudaError_t launch_count_issued(const unsigned long long *d_mask, const Plan &p, unsigned long long *d_count,
+                                cudaStream_t st);
 cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
                           float2 *d_mz, cudaStream_t st, int *nlaunch);
 cudaError_t launch_finalize(const float2 *d_partial, const Plan &p, const float *d_ampscale, double dV,

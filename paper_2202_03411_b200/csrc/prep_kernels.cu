@@ -219,6 +219,39 @@ cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_m
     return cudaGetLastError();
 }
 
+// Work the contraction issues (scatman_last_issued_blocks): per occupancy word, (non-empty 16-y steps) x (length of the
+// bounding range of non-empty 16-x blocks); a single CTA per item always runs the full 8 blocks of x.
+__global__ void count_issued_kernel(const unsigned long long *__restrict__ mask, size_t n, int full_x,
+                                    unsigned long long *__restrict__ count) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned v = 0;
+    if (i < n) {
+        const unsigned long long m = mask[i];
+        if (m) {
+            int ky = 0;
+            unsigned ux = 0;
+            for (int yi = 0; yi < 8; ++yi) {
+                const unsigned b = (unsigned)(m >> (8 * yi)) & 0xffu;
+                ky += b != 0;
+                ux |= b;
+            }
+            const int xm = full_x ? 8 : (32 - __clz((int)ux)) - (__ffs((int)ux) - 1);
+            v = (unsigned)(ky * xm);
+        }
+    }
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(count, (unsigned long long)v);
+}
+
+cudaError_t launch_count_issued(const unsigned long long *d_mask, const Plan &p, unsigned long long *d_count,
+                                cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const size_t n = (size_t)p.batch * p.nz * p.nxt * p.ngroups;
+    count_issued_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_mask, n, p.t_ncta == 1, d_count);
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------------------------------------ a3
 // Phase tables (Eq. 2's split), phases formed and evaluated in FP64 (R-precision):
 //   A planes  fp16 [4][npix_pad][ny_pad]  = split(2^10 e^{i qy(p) y_i})   (the UMMA A operand)

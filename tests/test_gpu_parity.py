@@ -167,6 +167,27 @@ def test_empty_and_single_voxel(sm):
         assert np.allclose(I, exact, rtol=2e-5)
 
 
+def test_issued_block_count(sm):
+    """scatman_last_issued_blocks: what the contraction multiplies after skipping empty 16-y steps and narrowing units
+    to their occupied 16-x blocks, on grids where the count is known by hand."""
+    from paper_2202_03411_b200 import binding as B
+    voxel, lam = (2.0, 2.0, 2.0), 12.0
+    g = np.full((13, 70, 150, 2), 0.01, np.float32)          # every voxel non-zero: nz=13, ny=70, nx=150
+    sm.simulate(dev(g), voxel, lam, 16, 16, 20.0, flags=B.FLAG_COUNT_ISSUED)
+    assert sm.last_issued_blocks() == 13 * (5 * 8 + 5 * 2)    # 5 y steps; x tile 0 full (8 blocks), tile 1 holds 22 x (2 blocks)
+    sm.simulate(dev(g), voxel, lam, 16, 16, 20.0, flags=B.FLAG_COUNT_ISSUED | B.FLAG_SINGLE_CTA)
+    assert sm.last_issued_blocks() == 13 * (5 * 8 + 5 * 8)    # a single CTA runs full tiles
+    z = np.zeros_like(g)
+    z[3, 40, 100] = (0.02, 0.001)                             # one voxel -> one block
+    sm.simulate(dev(z), voxel, lam, 16, 16, 20.0, flags=B.FLAG_COUNT_ISSUED)
+    assert sm.last_issued_blocks() == 1
+    z[3, 40, 30] = (0.02, 0.001)                              # same y step, x blocks 1..6 of tile 0 -> range of 6
+    sm.simulate(dev(z), voxel, lam, 16, 16, 20.0, flags=B.FLAG_COUNT_ISSUED)
+    assert sm.last_issued_blocks() == 6
+    sm.simulate(dev(z), voxel, lam, 16, 16, 20.0)
+    assert sm.last_issued_blocks() == -1
+
+
 def test_deterministic_and_workspace_reuse(sm):
     import torch
     w = W.config(0)
