@@ -23,7 +23,7 @@ SPLITS = 3           # FP16x3: AhBh + AlBh + AhBl
 FLOP_PER_TERM = 8    # one complex MAC
 # dram__bytes_read.sum + dram__bytes_write.sum of one contraction launch, from the committed `ncu --set full` capture
 # (profiles/r01_contract_cfg3_full.md); only the workload that was captured has a number
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": None}
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": 2.295495e9 + 8.534016e6}
 
 
 def load_peaks():
