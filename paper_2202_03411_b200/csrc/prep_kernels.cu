@@ -32,42 +32,72 @@ cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q,
 // ------------------------------------------------------------------------------------------------ a0
 // Block 5 / Fig. 6: beam-frame voxel <- trilinear sample of the body-frame grid at
 // r_body = R^T r_beam.  rotmat[b][9] row-major R (body -> beam).  One thread per beam-frame voxel.
+// Threads are grouped as 16 x 4 x 4 output voxels per block so that the 2x2x2 source cells of a block share cache lines
+// for any rotation (row-shaped blocks gather along a slanted line and read 30x more sectors than they use).
 __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz,
-                              const double *__restrict__ rotmat, float2 *__restrict__ out) {
-    const int iy = blockIdx.x % ny;
-    const int iz = (blockIdx.x / ny) % nz, b = blockIdx.x / (ny * nz);
+                              double3 inv, const double *__restrict__ rotmat, float2 *__restrict__ out) {
+    const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
+    int blk = blockIdx.x;
+    const int bx = blk % nbx; blk /= nbx;
+    const int by = blk % nby; blk /= nby;
+    const int bz = blk % nbz;
+    const int b = blk / nbz;
+    const int ix = bx * 16 + (threadIdx.x & 15), iy = by * 4 + ((threadIdx.x >> 4) & 3), iz = bz * 4 + (threadIdx.x >> 6);
+    if (ix >= nx || iy >= ny || iz >= nz) return;
     const double *R = rotmat + 9 * b;
-    for (int ix = threadIdx.x; ix < nx; ix += blockDim.x) {
-    const double xb = centre(ix, nx, dx), yb = centre(iy, ny, dy), zb = centre(iz, nz, dz);
-    const double xo = R[0] * xb + R[3] * yb + R[6] * zb;
-    const double yo = R[1] * xb + R[4] * yb + R[7] * zb;
-    const double zo = R[2] * xb + R[5] * yb + R[8] * zb;
-    const double fx = xo / dx + 0.5 * (double)(nx - 1);
-    const double fy = yo / dy + 0.5 * (double)(ny - 1);
-    const double fz = zo / dz + 0.5 * (double)(nz - 1);
-    const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
-    const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
-    const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
+    // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = f0 + ix * step (one row of R^T per axis)
+    const double yb = centre(iy, ny, dy), zb = centre(iz, nz, dz), xb0 = centre(0, nx, dx);
+    const double ix_dx = inv.x, iy_dy = inv.y, iz_dz = inv.z;   // reciprocals from the host: an FP64 division costs ~40 instructions
+    const double fx0 = (R[0] * xb0 + R[3] * yb + R[6] * zb) * ix_dx + 0.5 * (double)(nx - 1), sx = R[0] * dx * ix_dx;
+    const double fy0 = (R[1] * xb0 + R[4] * yb + R[7] * zb) * iy_dy + 0.5 * (double)(ny - 1), sy = R[1] * dx * iy_dy;
+    const double fz0 = (R[2] * xb0 + R[5] * yb + R[8] * zb) * iz_dz + 0.5 * (double)(nz - 1), sz = R[2] * dx * iz_dz;
     const float2 *src = in + (size_t)b * nx * ny * nz;
-    double are = 0.0, aim = 0.0;
+    float2 *dst = out + (size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx;
+    {
+        const double fx = fma((double)ix, sx, fx0), fy = fma((double)ix, sy, fy0), fz = fma((double)ix, sz, fz0);
+        float2 o = make_float2(0.f, 0.f);
+        // the 2x2x2 cell touches the grid only if every coordinate lies in (-1, n)
+        if (fx > -1.0 && fx < (double)nx && fy > -1.0 && fy < (double)ny && fz > -1.0 && fz < (double)nz) {
+            const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
+            const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
+            const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
+            const double wx[2] = {1.0 - tx, tx}, wy[2] = {1.0 - ty, ty}, wz[2] = {1.0 - tz, tz};
+            double are = 0.0, aim = 0.0;
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        const int xi = x0 + (c & 1), yi = y0 + ((c >> 1) & 1), zi = z0 + (c >> 2);
-        if (xi < 0 || xi >= nx || yi < 0 || yi >= ny || zi < 0 || zi >= nz) continue;
-        const double w = ((c & 1) ? tx : 1.0 - tx) * ((c & 2) ? ty : 1.0 - ty) * ((c & 4) ? tz : 1.0 - tz);
-        const float2 s = __ldg(src + ((size_t)zi * ny + yi) * nx + xi);
-        are += w * (double)s.x;
-        aim += w * (double)s.y;
-    }
-    out[(size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx + ix] = make_float2((float)are, (float)aim);
+            for (int cz = 0; cz < 2; ++cz) {
+                const int zi = z0 + cz;
+                if (zi < 0 || zi >= nz) continue;
+#pragma unroll
+                for (int cy = 0; cy < 2; ++cy) {
+                    const int yi = y0 + cy;
+                    if (yi < 0 || yi >= ny) continue;
+                    const double wyz = wy[cy] * wz[cz];
+                    const float2 *row = src + ((size_t)zi * ny + yi) * nx;
+#pragma unroll
+                    for (int cx = 0; cx < 2; ++cx) {
+                        const int xi = x0 + cx;
+                        if (xi < 0 || xi >= nx) continue;
+                        const float2 v = __ldg(row + xi);
+                        if (v.x == 0.f && v.y == 0.f) continue;   // most of a grid is vacuum: skip the FP64 conversions
+                        const double w = wx[cx] * wyz;
+                        are = fma(w, (double)v.x, are);
+                        aim = fma(w, (double)v.y, aim);
+                    }
+                }
+            }
+            o = make_float2((float)are, (float)aim);
+        }
+        dst[ix] = o;
     }
 }
 
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out,
                           cudaStream_t st) {
-    const unsigned grid = (unsigned)((size_t)p.ny * p.nz * batch);
-    orient_kernel<<<grid, p.nx >= 128 ? 128 : 64, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, d_rotmat,
-                                        (float2 *)d_out);
+    const size_t blocks = (size_t)((p.nx + 15) / 16) * ((p.ny + 3) / 4) * ((p.nz + 3) / 4) * batch;
+    if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    orient_kernel<<<(unsigned)blocks, 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
+                                                   make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat,
+                                                   (float2 *)d_out);
     return cudaGetLastError();
 }
 
