@@ -117,32 +117,42 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
         double Cre = 0.0, Cim = 0.0;
         double Tre = 1.0, Tim = 0.0;
         bool stale = false;  // T must be recomputed from C before its next use
-        for (int iz = 0; iz < nz; ++iz) {
-            const float2 c = __ldg(dn + base + iz * plane);
-            float2 o = make_float2(0.f, 0.f);
-            if (c.x != 0.f || c.y != 0.f) {
-                if (stale) {
-                    double s, co;
-                    sincos(kdz * Cre, &s, &co);
-                    const double mag = exp(-kdz * Cim);
-                    Tre = mag * co;
-                    Tim = mag * s;
-                    stale = false;
+        // slices in batches of 8: the loads of a batch are independent of the running prefix, so they are all in flight
+        // before the (serial) FP64 chain of the batch starts
+        for (int iz0 = 0; iz0 < nz; iz0 += 8) {
+            float2 cin[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                cin[i] = iz0 + i < nz ? __ldg(dn + base + (size_t)(iz0 + i) * plane) : make_float2(0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (iz0 + i >= nz) break;
+                const float2 c = cin[i];
+                float2 o = make_float2(0.f, 0.f);
+                if (c.x != 0.f || c.y != 0.f) {
+                    if (stale) {
+                        double s, co;
+                        sincos(kdz * Cre, &s, &co);
+                        const double mag = exp(-kdz * Cim);
+                        Tre = mag * co;
+                        Tim = mag * s;
+                        stale = false;
+                    }
+                    const double d = (double)c.x, be = (double)c.y;
+                    double fre = d, fim = be;
+                    if (rho_mode == SCATMAN_RHO_N2M1) {  // c (2 - c)
+                        fre = d * (2.0 - d) + be * be;
+                        fim = 2.0 * be * (1.0 - d);
+                    }
+                    o.x = (float)(fre * Tre - fim * Tim);
+                    o.y = (float)(fre * Tim + fim * Tre);
+                    vmax = fmaxf(vmax, fmaxf(fabsf(o.x), fabsf(o.y)));
+                    Cre += d;
+                    Cim += be;
+                    stale = true;
                 }
-                const double d = (double)c.x, be = (double)c.y;
-                double fre = d, fim = be;
-                if (rho_mode == SCATMAN_RHO_N2M1) {  // c (2 - c)
-                    fre = d * (2.0 - d) + be * be;
-                    fim = 2.0 * be * (1.0 - d);
-                }
-                o.x = (float)(fre * Tre - fim * Tim);
-                o.y = (float)(fre * Tim + fim * Tre);
-                vmax = fmaxf(vmax, fmaxf(fabsf(o.x), fabsf(o.y)));
-                Cre += d;
-                Cim += be;
-                stale = true;
+                rho[base + (size_t)(iz0 + i) * plane] = o;
             }
-            rho[base + iz * plane] = o;
         }
     }
     // block max -> one atomic per block (non-negative floats order like their bit patterns)
@@ -288,53 +298,80 @@ cudaError_t launch_count_issued(const unsigned long long *d_mask, const Plan &p,
 //   anchor    float2 [tile][nxa][128]     = e^{i qx(p) x_{16 a}}
 //   fine      float2 [tile][16][128]      = e^{i qx(p) b dx}
 //   mz        float2 [tile][nz][128]      = e^{i qz(p) z_j}
+// One thread = one pixel x 16 consecutive coordinates: FP64 sincos of the first phase and of the step, then the
+// angle-addition recurrence in FP64 (15 complex products; the rounding it adds is ~1e-15, far below the FP32 / FP16-pair
+// storage) -- an FP64 sincos per entry made these kernels FP64-throughput-bound.
+__device__ __forceinline__ void phase_run16(double q, double x0, double step, double (&re)[16], double (&im)[16]) {
+    double s0, c0, ss, cs;
+    sincos(q * x0, &s0, &c0);
+    sincos(q * step, &ss, &cs);
+    re[0] = c0;
+    im[0] = s0;
+#pragma unroll
+    for (int i = 1; i < 16; ++i) {
+        re[i] = re[i - 1] * cs - im[i - 1] * ss;
+        im[i] = re[i - 1] * ss + im[i - 1] * cs;
+    }
+}
+
 __global__ void table_a_kernel(const double *__restrict__ q, int64_t npix, int64_t npix_pad, int ny, int ny_pad,
                                double dy, __half *__restrict__ A) {
-    const int y = blockIdx.y * blockDim.x + threadIdx.x;
-    const int64_t p = blockIdx.x;
-    if (y >= ny_pad) return;
-    float re = 0.f, im = 0.f;
-    if (p < npix && y < ny) {
-        double s, c;
-        sincos(q[3 * p + 1] * centre(y, ny, dy), &s, &c);
-        re = (float)(c * (double)kScaleA);
-        im = (float)(s * (double)kScaleA);
+    const int nrun = ny_pad / 16;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // run fastest: a warp writes 32 x 32 contiguous bytes
+    if (t >= npix_pad * nrun) return;
+    const int64_t p = t / nrun;
+    const int y0 = (int)(t % nrun) * 16;
+    double re[16], im[16];
+    if (p < npix) phase_run16(q[3 * p + 1], centre(y0, ny, dy), dy, re, im);
+    __align__(16) __half h[4][16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        float fr = 0.f, fi = 0.f;
+        if (p < npix && y0 + i < ny) {
+            fr = (float)(re[i] * (double)kScaleA);
+            fi = (float)(im[i] * (double)kScaleA);
+        }
+        h[0][i] = __float2half_rn(fr);
+        h[1][i] = __float2half_rn(fr - __half2float(h[0][i]));
+        h[2][i] = __float2half_rn(fi);
+        h[3][i] = __float2half_rn(fi - __half2float(h[2][i]));
     }
-    const __half reh = __float2half_rn(re), imh = __float2half_rn(im);
-    const __half rel = __float2half_rn(re - __half2float(reh)), iml = __float2half_rn(im - __half2float(imh));
-    const size_t plane = (size_t)npix_pad * ny_pad, o = (size_t)p * ny_pad + y;
-    A[o] = reh;
-    A[plane + o] = rel;
-    A[2 * plane + o] = imh;
-    A[3 * plane + o] = iml;
+    const size_t plane = (size_t)npix_pad * ny_pad, o = (size_t)p * ny_pad + y0;
+#pragma unroll
+    for (int pl = 0; pl < 4; ++pl) {
+        uint4 *dst = (uint4 *)(A + pl * plane + o);
+        dst[0] = ((const uint4 *)h[pl])[0];
+        dst[1] = ((const uint4 *)h[pl])[1];
+    }
 }
 
 // which: 0 anchor (count nxa, coord = centre(16 a)), 1 fine (count 16, coord = b dx), 2 mz (count nz)
 __global__ void table_small_kernel(const double *__restrict__ q, int64_t npix, int which, int count, int n, double d,
                                    float2 *__restrict__ out) {
     const int lane = threadIdx.x;  // 128
-    const int idx = blockIdx.y, tile = blockIdx.x;
+    const int idx0 = blockIdx.y * 16, tile = blockIdx.x;
     const int64_t p = (int64_t)tile * kTileP + lane;
-    float2 v = make_float2(1.f, 0.f);
+    double re[16], im[16];
     if (p < npix) {
-        double coord, qq;
-        if (which == 0) { coord = centre(idx * kFine, n, d); qq = q[3 * p + 0]; }
-        else if (which == 1) { coord = (double)idx * d; qq = q[3 * p + 0]; }
-        else { coord = centre(idx, n, d); qq = q[3 * p + 2]; }
-        double s, c;
-        sincos(qq * coord, &s, &c);
-        v = make_float2((float)c, (float)s);
+        if (which == 0) phase_run16(q[3 * p + 0], centre(idx0 * kFine, n, d), d * (double)kFine, re, im);
+        else if (which == 1) phase_run16(q[3 * p + 0], (double)idx0 * d, d, re, im);
+        else phase_run16(q[3 * p + 2], centre(idx0, n, d), d, re, im);
     }
-    out[((size_t)tile * count + idx) * kTileP + lane] = v;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        if (idx0 + i >= count) break;
+        const float2 v = p < npix ? make_float2((float)re[i], (float)im[i]) : make_float2(1.f, 0.f);
+        out[((size_t)tile * count + idx0 + i) * kTileP + lane] = v;
+    }
 }
 
 cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
                           float2 *d_mz, cudaStream_t st, int *nlaunch) {
-    dim3 ga((unsigned)p.npix_pad, (p.ny_pad + 63) / 64);
-    table_a_kernel<<<ga, 64, 0, st>>>(d_q, p.npix, p.npix_pad, p.ny, p.ny_pad, p.dy, d_A);
-    table_small_kernel<<<dim3(p.ntiles, p.nxa), kTileP, 0, st>>>(d_q, p.npix, 0, p.nxa, p.nx, p.dx, d_anchor);
-    table_small_kernel<<<dim3(p.ntiles, kFine), kTileP, 0, st>>>(d_q, p.npix, 1, kFine, p.nx, p.dx, d_fine);
-    table_small_kernel<<<dim3(p.ntiles, p.nz), kTileP, 0, st>>>(d_q, p.npix, 2, p.nz, p.nz, p.dz, d_mz);
+    const int64_t nthreads_a = p.npix_pad * (p.ny_pad / 16);
+    table_a_kernel<<<(unsigned)((nthreads_a + 127) / 128), 128, 0, st>>>(d_q, p.npix, p.npix_pad, p.ny, p.ny_pad, p.dy, d_A);
+    table_small_kernel<<<dim3(p.ntiles, (p.nxa + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, 0, p.nxa, p.nx, p.dx, d_anchor);
+    table_small_kernel<<<dim3(p.ntiles, 1), kTileP, 0, st>>>(d_q, p.npix, 1, kFine, p.nx, p.dx, d_fine);
+    table_small_kernel<<<dim3(p.ntiles, (p.nz + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, 2, p.nz, p.nz, p.dz, d_mz);
     if (nlaunch) *nlaunch += 4;
     return cudaGetLastError();
 }
