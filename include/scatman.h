@@ -147,6 +147,47 @@ int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count);
  * CUDA events on the call's stream.  Synchronises on the end event.  -1 if none was recorded. */
 int scatman_last_contraction_ms(scatman_ctx *ctx, float *ms);
 
+/* ---- Shape rendering (Block 5 of Fig. 4, "render the slice at the proper spatial coordinates"; shape
+ * models of PAPER.md:245-259, 405-425; readings R18-R21 of DESIGN.md) ----------------------------------------------
+ * A shape is rendered directly in the beam frame: voxel centre r_beam goes to r_body = R^T r_beam (R from `quat`,
+ * body -> beam, as in scatman_orient) and the voxel becomes (delta, beta) if r_body is inside the shape, else (0, 0):
+ * binary voxelisation at voxel centres, evaluated in FP64.  The rendered grid is already oriented, so it is passed to
+ * scatman_simulate with h_quat = NULL.
+ *   ELLIPSOID            (x/a)^2 + (y/b)^2 + (z/c)^2 <= 1, semi-axes a, b, c along body x, y, z.
+ *   SPHERICAL_HARMONICS  |r| <= R(theta, phi) = sum over the triplets (l, m, c) of c * Y_lm, theta =
+ *                        polar angle from body +z, phi = atan2(y, x); Y_lm = REAL orthonormal harmonics with Eq. 10's
+ *                        normalisation and Condon-Shortley phase: m = 0: Y_l^0; m > 0: sqrt2 Re Y_l^m; m < 0:
+ *                        sqrt2 Im Y_l^|m|.  A sphere of radius r is the single triplet (0, 0, r sqrt(4 pi)).
+ *                        h_coef[ncoef][3] = (l, m, c) as doubles on the HOST, ncoef <= 96, l <= 32.
+ *   RADIAL_MAP           |r| <= R(lat, lon), bilinear in d_radii[nlat][nlon] (FP64, DEVICE): sample (i, j) sits at
+ *                        latitude -pi/2 + i pi/nlat and longitude j 2pi/nlon (the paper's 4 x 4 example),
+ *                        periodic in longitude, latitudes above the last sample hold the last row;
+ *                        lat = asin(z/|r|), lon = atan2(y, x) mod 2pi.
+ *   VOLUME_MAP           d_volume[nvz][nvy][nvx] bytes (DEVICE, non-zero = inside): cubic cells of side vdx centred on
+ *                        the origin; inside if the cell containing r_body is set.
+ * Fields of other kinds are ignored. */
+enum { SCATMAN_SHAPE_ELLIPSOID = 0, SCATMAN_SHAPE_SPHERICAL_HARMONICS = 1, SCATMAN_SHAPE_RADIAL_MAP = 2,
+       SCATMAN_SHAPE_VOLUME_MAP = 3 };
+
+typedef struct {
+    int32_t kind;
+    float delta, beta;       /* n = 1 - delta + i beta inside the shape (Eq. 7) */
+    double quat[4];          /* (w, x, y, z) unit quaternion, body -> beam; {1, 0, 0, 0} = identity */
+    double a, b, c;          /* ELLIPSOID */
+    int32_t ncoef;           /* SPHERICAL_HARMONICS */
+    const double *h_coef;
+    int32_t nlat, nlon;      /* RADIAL_MAP */
+    const double *d_radii;
+    int32_t nvx, nvy, nvz;   /* VOLUME_MAP */
+    const uint8_t *d_volume;
+    double vdx;
+} scatman_shape;
+
+/* Render `batch` shapes (host array of descriptors, read before return) into d_dn[batch][nz][ny][nx][2] (device,
+ * FP32 (delta, beta)), asynchronously on cuda_stream; one kernel launch per shape. */
+int scatman_render(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
+                   float *d_dn, void *cuda_stream);
+
 /* With SCATMAN_FLAG_COUNT_ISSUED: the number of 16-y x 16-x blocks of rho~ (256 voxels each) the contraction of the last
  * scatman_simulate* call multiplied against EVERY pixel, summed over slices and batch items; the dense count is
  * batch * nz * ceil(ny/16) * ceil(nx/16) blocks of the padded grid.  Issued tensor flop = blocks * 256 * npix_pad * 24.

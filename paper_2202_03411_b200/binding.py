@@ -23,7 +23,7 @@ FLAG_COUNT_ISSUED = 2
 EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
-    "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
+    "scatman_render", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
 
@@ -40,6 +40,18 @@ class Detector(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("rho_mode", C.c_int32), ("method", C.c_int32), ("precision", C.c_int32), ("flags", C.c_uint32)]
+
+
+SHAPE_ELLIPSOID, SHAPE_SPHERICAL_HARMONICS, SHAPE_RADIAL_MAP, SHAPE_VOLUME_MAP = range(4)
+
+
+class Shape(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("delta", C.c_float), ("beta", C.c_float), ("quat", C.c_double * 4),
+                ("a", C.c_double), ("b", C.c_double), ("c", C.c_double),
+                ("ncoef", C.c_int32), ("h_coef", C.c_void_p),
+                ("nlat", C.c_int32), ("nlon", C.c_int32), ("d_radii", C.c_void_p),
+                ("nvx", C.c_int32), ("nvy", C.c_int32), ("nvz", C.c_int32), ("d_volume", C.c_void_p),
+                ("vdx", C.c_double)]
 
 
 class ScatmanError(RuntimeError):
@@ -73,6 +85,7 @@ def load_library() -> C.CDLL:
                                      C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                         C.POINTER(Options), vp]
+    L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.scatman_last_issued_blocks.argtypes = [vp, C.POINTER(i64)]
@@ -183,6 +196,48 @@ class Scatman:
         self._check(self.lib.scatman_effective_strength(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                         int(rho_mode), batch, C.c_void_p(out.data_ptr()),
                                                         self._stream(stream)))
+        return out
+
+    def render(self, shapes: Sequence[dict], dims, voxel, out=None, stream=None):
+        """(delta, beta) grids float32 [B][nz][ny][nx][2] of shape descriptors (dicts with the keys of include/scatman.h's
+        scatman_shape: kind, delta, beta, quat, and a/b/c | coeffs [(l, m, c)] | radii (CUDA float64 [nlat][nlon]) |
+        volume (CUDA uint8 [nvz][nvy][nvx]) + dx).  Marshalling only: the shapes are evaluated by render_kernel."""
+        import numpy as np
+        import torch
+        nx, ny, nz = (int(v) for v in dims)
+        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+        batch = len(shapes)
+        if out is None:
+            out = torch.empty((batch, nz, ny, nx, 2), dtype=torch.float32, device=f"cuda:{self.device}")
+        arr = (Shape * batch)()
+        keep = []
+        kinds = {"ellipsoid": SHAPE_ELLIPSOID, "spherical_harmonics": SHAPE_SPHERICAL_HARMONICS,
+                 "radial_map": SHAPE_RADIAL_MAP, "volume_map": SHAPE_VOLUME_MAP}
+        for i, sh in enumerate(shapes):
+            s = arr[i]
+            s.kind = kinds[sh["kind"]]
+            s.delta, s.beta = float(sh["delta"]), float(sh["beta"])
+            q = sh.get("quat")
+            s.quat[:] = [1.0, 0.0, 0.0, 0.0] if q is None else [float(v) for v in q]
+            if s.kind == SHAPE_ELLIPSOID:
+                s.a, s.b, s.c = float(sh["a"]), float(sh["b"]), float(sh["c"])
+            elif s.kind == SHAPE_SPHERICAL_HARMONICS:
+                co = np.ascontiguousarray(np.asarray(sh["coeffs"], dtype=np.float64).reshape(-1, 3))
+                keep.append(co)
+                s.ncoef, s.h_coef = co.shape[0], co.ctypes.data
+            elif s.kind == SHAPE_RADIAL_MAP:
+                r = sh["radii"]
+                if not (r.is_cuda and r.dtype == torch.float64 and r.is_contiguous() and r.dim() == 2):
+                    raise ValueError("radii must be a contiguous CUDA float64 tensor [nlat][nlon]")
+                keep.append(r)
+                s.nlat, s.nlon, s.d_radii = int(r.shape[0]), int(r.shape[1]), r.data_ptr()
+            else:
+                v = sh["volume"]
+                if not (v.is_cuda and v.dtype == torch.uint8 and v.is_contiguous() and v.dim() == 3):
+                    raise ValueError("volume must be a contiguous CUDA uint8 tensor [nvz][nvy][nvx]")
+                keep.append(v)
+                s.nvz, s.nvy, s.nvx, s.d_volume, s.vdx = int(v.shape[0]), int(v.shape[1]), int(v.shape[2]), v.data_ptr(), float(sh["dx"])
+        self._check(self.lib.scatman_render(self._ctx, arr, batch, C.byref(grid), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
     def simulate(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,

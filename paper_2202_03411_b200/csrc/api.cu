@@ -245,6 +245,21 @@ int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *g
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "orient");
 }
 
+int scatman_render(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid, float *d_dn,
+                   void *cuda_stream) {
+    if (!ctx || !h_shapes || !d_dn || !valid_grid(grid) || batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    const size_t per_item = (size_t)grid->nx * grid->ny * grid->nz * 2;
+    for (int b = 0; b < batch; ++b) {
+        cudaError_t e = cudaSuccess;
+        if (launch_render(h_shapes[b], *grid, d_dn + (size_t)b * per_item, (cudaStream_t)cuda_stream, &e))
+            return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad shape descriptor " + std::to_string(b));
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "render");
+    }
+    ctx->last_launches = batch;
+    return SCATMAN_OK;
+}
+
 int scatman_effective_strength(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
                                int32_t rho_mode, int32_t batch, float *d_rho, void *cuda_stream) {
     if (!ctx || !d_dn || !d_rho || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) || batch < 1 ||

@@ -65,6 +65,8 @@ cudaError_t launch_simt_sincos(const float *d_rho, const double *d_q, const Plan
 cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
                               cudaStream_t st);
 
+int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
+
 // tensor path: tensor maps are encoded on the host through the driver entry point
 struct TensorMaps;  // opaque here
 struct TensorLaunch {

@@ -1,0 +1,173 @@
+// render_kernels.cu -- shape rendering on the GPU (Block 5 of Fig. 4; shape models PAPER.md:279-281,
+// 405-425): Ellipsoid, SphericalHarmonics, RadialMap, VolumeMap -> (delta, beta) grid, rendered directly
+// in the beam frame at r_body = R^T r_beam (no resampling step), binary voxelisation at voxel centres, all FP64.
+// Readings R18-R21 of DESIGN.md.  One launch per shape, one thread per voxel, x fastest (coalesced 8-byte stores).
+#include <cmath>
+
+#include "internal.h"
+
+namespace scatman {
+
+constexpr int kMaxCoef = 96;
+
+struct RenderArgs {
+    int kind;
+    float delta, beta;
+    int nx, ny, nz;
+    double dx, dy, dz;
+    double Rt[9];            // row-major R^T: r_body = Rt r_beam
+    double a, b, c;          // ellipsoid
+    int ncoef;               // spherical harmonics: value = sum cn[i] P_{l[i]}^{m[i]}(cos theta) {1, cos m phi, sin m phi}
+    signed char l[kMaxCoef], m[kMaxCoef];   // m as given (sign selects cos / sin)
+    double cn[kMaxCoef];     // c * N_lm * (m != 0 ? sqrt 2 : 1)
+    double r_lo, r_hi;       // every voxel with |r| < r_lo is inside, with |r| > r_hi outside
+    int nlat, nlon;          // radial map
+    const double *radii;
+    int nvx, nvy, nvz;       // volume map
+    const unsigned char *vol;
+    double vdx;
+};
+
+// P_l^m(x), m >= 0, Condon-Shortley phase (Eq. 10), by the standard recurrences
+__device__ double legendre_p(int l, int m, double x) {
+    const double s = sqrt(fmax(0.0, 1.0 - x * x));
+    double pmm = 1.0;
+    for (int k = 1; k <= m; ++k) pmm = -pmm * (double)(2 * k - 1) * s;
+    if (l == m) return pmm;
+    double pm1 = x * (double)(2 * m + 1) * pmm;
+    for (int ll = m + 2; ll <= l; ++ll) {
+        const double p = ((double)(2 * ll - 1) * x * pm1 - (double)(ll + m - 1) * pmm) / (double)(ll - m);
+        pmm = pm1;
+        pm1 = p;
+    }
+    return pm1;
+}
+
+__global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
+    const double kPi = 3.14159265358979323846;
+    const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t nvox = (size_t)A.nx * A.ny * A.nz;
+    if (v >= nvox) return;
+    const int ix = (int)(v % A.nx), iy = (int)((v / A.nx) % A.ny), iz = (int)(v / ((size_t)A.nx * A.ny));
+    const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
+    const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
+    const double z = ((double)iz - 0.5 * (double)(A.nz - 1)) * A.dz;
+    const double xb = A.Rt[0] * x + A.Rt[1] * y + A.Rt[2] * z;
+    const double yb = A.Rt[3] * x + A.Rt[4] * y + A.Rt[5] * z;
+    const double zb = A.Rt[6] * x + A.Rt[7] * y + A.Rt[8] * z;
+    bool inside = false;
+    if (A.kind == SCATMAN_SHAPE_ELLIPSOID) {
+        const double u = xb / A.a, w = yb / A.b, t = zb / A.c;
+        inside = u * u + w * w + t * t <= 1.0;
+    } else if (A.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS) {
+        const double r = sqrt(xb * xb + yb * yb + zb * zb);
+        if (r < A.r_lo) inside = true;
+        else if (r <= A.r_hi) {
+            const double ct = r > 0.0 ? zb / r : 1.0;
+            const double ph = atan2(yb, xb);
+            double R = 0.0;
+            for (int i = 0; i < A.ncoef; ++i) {
+                const int l = A.l[i], m = A.m[i], am = m < 0 ? -m : m;
+                double f = A.cn[i] * legendre_p(l, am, ct);
+                if (m > 0) f *= cos((double)am * ph);
+                else if (m < 0) f *= sin((double)am * ph);
+                R += f;
+            }
+            inside = r <= R;
+        }
+    } else if (A.kind == SCATMAN_SHAPE_RADIAL_MAP) {
+        const double r = sqrt(xb * xb + yb * yb + zb * zb);
+        const double sl = r > 0.0 ? fmin(1.0, fmax(-1.0, zb / r)) : 0.0;
+        const double lat = asin(sl);
+        double lon = atan2(yb, xb);
+        if (lon < 0.0) lon += 2.0 * kPi;
+        const double fi = fmin(fmax((lat + 0.5 * kPi) / (kPi / (double)A.nlat), 0.0), (double)(A.nlat - 1));
+        const double fj = lon / (2.0 * kPi / (double)A.nlon);
+        const int i0 = min((int)floor(fi), A.nlat - 1), i1 = min(i0 + 1, A.nlat - 1);
+        const double ti = fi - (double)i0;
+        const double j0f = floor(fj), tj = fj - j0f;
+        const int j0 = (((int)j0f % A.nlon) + A.nlon) % A.nlon, j1 = (j0 + 1) % A.nlon;
+        const double lo = A.radii[(size_t)i0 * A.nlon + j0] * (1.0 - tj) + A.radii[(size_t)i0 * A.nlon + j1] * tj;
+        const double hi = A.radii[(size_t)i1 * A.nlon + j0] * (1.0 - tj) + A.radii[(size_t)i1 * A.nlon + j1] * tj;
+        inside = r <= lo * (1.0 - ti) + hi * ti;
+    } else {
+        const double fx = xb / A.vdx + 0.5 * (double)A.nvx, fy = yb / A.vdx + 0.5 * (double)A.nvy,
+                     fz = zb / A.vdx + 0.5 * (double)A.nvz;
+        const double cx = floor(fx), cy = floor(fy), cz = floor(fz);
+        if (cx >= 0.0 && cx < (double)A.nvx && cy >= 0.0 && cy < (double)A.nvy && cz >= 0.0 && cz < (double)A.nvz)
+            inside = A.vol[((size_t)cz * A.nvy + (size_t)cy) * A.nvx + (size_t)cx] != 0;
+    }
+    out[v] = inside ? make_float2(A.delta, A.beta) : make_float2(0.f, 0.f);
+}
+
+static double factorial_d(int n) {
+    double f = 1.0;
+    for (int i = 2; i <= n; ++i) f *= (double)i;
+    return f;
+}
+
+// 0 ok, 1 bad argument
+int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err) {
+    const double kPi = 3.14159265358979323846;
+    *err = cudaSuccess;
+    RenderArgs A = {};
+    A.kind = s.kind;
+    A.delta = s.delta;
+    A.beta = s.beta;
+    A.nx = g.nx; A.ny = g.ny; A.nz = g.nz;
+    A.dx = g.dx; A.dy = g.dy; A.dz = g.dz;
+    const double w = s.quat[0], a = s.quat[1], b = s.quat[2], c = s.quat[3];
+    if (!(std::fabs(w * w + a * a + b * b + c * c - 1.0) <= 2e-6)) return 1;
+    const double R[9] = {1 - 2 * (b * b + c * c), 2 * (a * b - w * c),     2 * (a * c + w * b),
+                         2 * (a * b + w * c),     1 - 2 * (a * a + c * c), 2 * (b * c - w * a),
+                         2 * (a * c - w * b),     2 * (b * c + w * a),     1 - 2 * (a * a + b * b)};
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) A.Rt[3 * i + j] = R[3 * j + i];
+    switch (s.kind) {
+        case SCATMAN_SHAPE_ELLIPSOID:
+            if (!(s.a > 0.0 && s.b > 0.0 && s.c > 0.0)) return 1;
+            A.a = s.a; A.b = s.b; A.c = s.c;
+            break;
+        case SCATMAN_SHAPE_SPHERICAL_HARMONICS: {
+            if (s.ncoef < 1 || s.ncoef > kMaxCoef || !s.h_coef) return 1;
+            // |sum_m c_lm Y_lm| <= sqrt(sum_m c_lm^2) sqrt((2l+1)/4pi) (addition theorem): brackets R around its l = 0 part
+            double norm2[33] = {0};
+            double r00 = 0.0;
+            for (int i = 0; i < s.ncoef; ++i) {
+                const int l = (int)s.h_coef[3 * i], m = (int)s.h_coef[3 * i + 1];
+                const double cv = s.h_coef[3 * i + 2];
+                if ((double)l != s.h_coef[3 * i] || (double)m != s.h_coef[3 * i + 1] || l < 0 || l > 32 || m < -l || m > l ||
+                    !std::isfinite(cv))
+                    return 1;
+                const int am = m < 0 ? -m : m;
+                const double n = std::sqrt((2 * l + 1) / (4 * kPi) * factorial_d(l - am) / factorial_d(l + am));
+                A.l[i] = (signed char)l;
+                A.m[i] = (signed char)m;
+                A.cn[i] = cv * n * (m != 0 ? std::sqrt(2.0) : 1.0);
+                if (l == 0) r00 += cv * n;
+                else norm2[l] += cv * cv;
+            }
+            double bound = 0.0;
+            for (int l = 1; l <= 32; ++l) bound += std::sqrt(norm2[l]) * std::sqrt((2 * l + 1) / (4 * kPi));
+            A.ncoef = s.ncoef;
+            A.r_lo = (r00 - bound) * (1.0 - 1e-9) - 1e-300;
+            A.r_hi = (r00 + bound) * (1.0 + 1e-9) + 1e-300;
+            break;
+        }
+        case SCATMAN_SHAPE_RADIAL_MAP:
+            if (s.nlat < 1 || s.nlon < 1 || !s.d_radii) return 1;
+            A.nlat = s.nlat; A.nlon = s.nlon; A.radii = s.d_radii;
+            break;
+        case SCATMAN_SHAPE_VOLUME_MAP:
+            if (s.nvx < 1 || s.nvy < 1 || s.nvz < 1 || !s.d_volume || !(s.vdx > 0.0)) return 1;
+            A.nvx = s.nvx; A.nvy = s.nvy; A.nvz = s.nvz; A.vol = s.d_volume; A.vdx = s.vdx;
+            break;
+        default: return 1;
+    }
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    render_kernel<<<(unsigned)((nvox + 255) / 256), 256, 0, st>>>(A, (float2 *)d_dn);
+    *err = cudaGetLastError();
+    return 0;
+}
+
+}  // namespace scatman

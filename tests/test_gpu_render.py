@@ -1,0 +1,142 @@
+"""GPU parity of shape rendering (scatman_render, render_kernels.cu) against oracle/render.py, voxel by voxel, and of
+the rendered-then-simulated path against the oracle's."""
+from math import pi, sqrt
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from oracle import render as R
+from paper_2202_03411_b200 import workloads as W
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sm():
+    import torch
+    from paper_2202_03411_b200 import binding as B, build
+    build.build()
+    assert torch.cuda.is_available()
+    s = B.Scatman(0)
+    yield s
+    s.close()
+
+
+def _to_device(shape):
+    import torch
+    d = dict(shape)
+    if "radii" in d:
+        d["radii"] = torch.from_numpy(np.ascontiguousarray(d["radii"], dtype=np.float64)).cuda()
+    if "volume" in d:
+        d["volume"] = torch.from_numpy(np.ascontiguousarray(d["volume"]).astype(np.uint8)).cuda()
+    return d
+
+
+def _check(sm, shapes, dims, voxel, tie=1e-9):
+    """Byte-exact (delta, beta) everywhere, except voxels whose centre lies on the surface to within rounding: there the
+    inside test is an FP64 comparison of two nearly equal numbers and either answer is valid."""
+    got = sm.render([_to_device(s) for s in shapes], dims, voxel).cpu().numpy()
+    for b, s in enumerate(shapes):
+        ref, margin = R.render(s, dims, voxel, return_margin=True)
+        diff = np.any(got[b] != ref, axis=-1)
+        if diff.any():
+            scale = 100.0 if s["kind"] in ("spherical_harmonics", "radial_map") else 1.0   # margin is a length there
+            assert np.all(np.abs(margin[diff]) <= tie * scale), (b, s["kind"], int(diff.sum()), float(np.abs(margin[diff]).max()))
+            assert diff.sum() <= 1e-5 * diff.size + 2
+        vals = got[b][np.any(got[b] != 0, axis=-1)]
+        if vals.size:
+            assert np.all(vals[:, 0] == np.float32(s["delta"])) and np.all(vals[:, 1] == np.float32(s["beta"]))
+    return got
+
+
+def _droplet_coeffs(rng, r0, lmax, sigma0=0.05):
+    co = [(0, 0, r0 * sqrt(4 * pi))]
+    for l in range(1, lmax + 1):
+        for m in range(-l, l + 1):
+            co.append((l, m, r0 * rng.normal(0.0, sigma0 / l)))
+    return co
+
+
+def test_ellipsoids_ragged_dims_random_orientations(sm):
+    rng = np.random.default_rng(11)
+    quats = W.random_quaternions(rng, 4)
+    shapes = [{"kind": "ellipsoid", "delta": 0.02 + 0.01 * i, "beta": 0.005 * i, "quat": quats[i],
+               "a": 30.0 - 3 * i, "b": 17.5 + i, "c": 9.25 + 2 * i} for i in range(4)]
+    shapes.append({"kind": "ellipsoid", "delta": -0.01, "beta": 0.0, "a": 500.0, "b": 500.0, "c": 500.0})   # fills the grid
+    shapes.append({"kind": "ellipsoid", "delta": 0.01, "beta": 0.0, "a": 0.1, "b": 0.1, "c": 0.1})          # holds only the centre voxel (odd dims)
+    got = _check(sm, shapes, (45, 37, 29), (1.7, 2.1, 1.3))
+    assert np.all(got[4][..., 0] == np.float32(-0.01))
+    assert int(np.count_nonzero(got[5][..., 0])) == 1 and got[5][14, 18, 22, 0] == np.float32(0.01)
+
+
+def test_spherical_harmonics_droplets(sm):
+    rng = np.random.default_rng(12)
+    quats = W.random_quaternions(rng, 3)
+    shapes = [{"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.01, "coeffs": _droplet_coeffs(rng, 40.0, 6)},
+              {"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.01, "quat": quats[0], "coeffs": _droplet_coeffs(rng, 25.0, 4, 0.15)},
+              {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "quat": quats[1],
+               "coeffs": [(0, 0, 100.0), (8, 5, 30.0), (8, -8, 25.0), (3, -2, 20.0), (5, 0, -15.0)]},
+              {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "quat": quats[2], "coeffs": [(0, 0, 33.0 * sqrt(4 * pi))]}]
+    _check(sm, shapes, (64, 60, 56), (1.6, 1.6, 1.6))
+
+
+def test_radial_maps(sm):
+    rng = np.random.default_rng(13)
+    nlat, nlon = 48, 96
+    lat = (-pi / 2 + np.arange(nlat) * pi / nlat)[:, None]
+    lon = (np.arange(nlon) * 2 * pi / nlon)[None, :]
+    smooth = 30.0 + 6.0 * np.cos(3 * lon) * np.cos(lat) ** 2 + 4.0 * np.sin(2 * lat) + rng.uniform(-0.5, 0.5, (nlat, nlon))
+    quats = W.random_quaternions(rng, 2)
+    shapes = [{"kind": "radial_map", "delta": 0.02, "beta": 0.05, "radii": smooth},
+              {"kind": "radial_map", "delta": 0.02, "beta": 0.05, "quat": quats[0], "radii": smooth},
+              {"kind": "radial_map", "delta": 0.02, "beta": 0.0, "quat": quats[1], "radii": rng.uniform(20.0, 38.0, (4, 4))},
+              {"kind": "radial_map", "delta": 0.02, "beta": 0.0, "radii": np.full((1, 1), 21.0)}]
+    _check(sm, shapes, (50, 50, 50), (1.9, 1.9, 1.9))
+
+
+def test_volume_maps(sm):
+    rng = np.random.default_rng(14)
+    quats = W.random_quaternions(rng, 2)
+    vol = rng.random((11, 17, 23)) < 0.5
+    shapes = [{"kind": "volume_map", "delta": 0.04, "beta": 0.02, "volume": vol, "dx": 3.7},
+              {"kind": "volume_map", "delta": 0.04, "beta": 0.02, "quat": quats[0], "volume": vol, "dx": 3.7},
+              {"kind": "volume_map", "delta": 0.04, "beta": 0.02, "quat": quats[1], "volume": np.ones((10, 10, 10), bool), "dx": 2.0}]
+    got = _check(sm, shapes, (64, 48, 40), (1.0, 1.0, 1.0), tie=1e-9)
+    cube = sm.render([_to_device({"kind": "volume_map", "delta": 1.0, "beta": 0.0, "volume": np.ones((10, 10, 10), bool), "dx": 2.0})],
+                     (32, 32, 32), (1.0, 1.0, 1.0)).cpu().numpy()
+    assert int(cube[0, ..., 0].sum()) == 20 ** 3          # the paper's example
+
+
+def test_rendered_shapes_through_the_whole_path(sm):
+    """render -> simulate on the GPU against oracle render -> oracle simulate (the rendered grid is already oriented)."""
+    rng = np.random.default_rng(15)
+    quats = W.random_quaternions(rng, 3)
+    dims, voxel, lam = (48, 40, 36), (3.0, 3.0, 3.0), 18.0
+    shapes = [{"kind": "ellipsoid", "delta": 0.02, "beta": 0.004, "quat": quats[0], "a": 55.0, "b": 35.0, "c": 25.0},
+              {"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.01, "quat": quats[1], "coeffs": _droplet_coeffs(rng, 40.0, 4, 0.1)},
+              {"kind": "volume_map", "delta": 0.05, "beta": 0.0, "quat": quats[2], "volume": rng.random((6, 7, 8)) < 0.6, "dx": 9.0}]
+    g = sm.render([_to_device(s) for s in shapes], dims, voxel)
+    I = sm.simulate(g, voxel, lam, 24, 20, 30.0).cpu().numpy()
+    gh = g.cpu().numpy()
+    for b, s in enumerate(shapes):
+        ref_grid = R.render(s, dims, voxel)
+        assert np.mean(np.any(gh[b] != ref_grid, axis=-1)) < 1e-4
+        ref = O.simulate(gh[b], voxel, lam, 24, 20, 30.0)
+        assert_parity(I[b], ref, what=f"rendered {s['kind']}")
+
+
+def test_render_error_codes(sm):
+    import torch
+    from paper_2202_03411_b200 import binding as B
+    dims, voxel = (8, 8, 8), (1.0, 1.0, 1.0)
+    bad = [{"kind": "ellipsoid", "delta": 0.01, "beta": 0.0, "a": -1.0, "b": 1.0, "c": 1.0},
+           {"kind": "ellipsoid", "delta": 0.01, "beta": 0.0, "quat": [2.0, 0, 0, 0], "a": 1.0, "b": 1.0, "c": 1.0},
+           {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "coeffs": [(2, 3, 1.0)]},
+           {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "coeffs": [(1.5, 0, 1.0)]},
+           {"kind": "volume_map", "delta": 0.01, "beta": 0.0, "volume": torch.ones((2, 2, 2), dtype=torch.uint8, device="cuda"), "dx": 0.0}]
+    for s in bad:
+        with pytest.raises(B.ScatmanError) as e:
+            sm.render([s], dims, voxel)
+        assert e.value.status == B.INVALID_ARGUMENT
