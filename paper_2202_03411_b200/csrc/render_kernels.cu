@@ -3,6 +3,7 @@
 // in the beam frame at r_body = R^T r_beam (no resampling step), binary voxelisation at voxel centres, all FP64.
 // Readings R18-R21 of DESIGN.md.  One launch per shape, one thread per voxel, x fastest (coalesced 8-byte stores).
 #include <cmath>
+#include <utility>
 
 #include "internal.h"
 
@@ -16,7 +17,7 @@ struct RenderArgs {
     int nx, ny, nz;
     double dx, dy, dz;
     double Rt[9];            // row-major R^T: r_body = Rt r_beam
-    double a, b, c;          // ellipsoid
+    double a, b, c;          // ellipsoid: 1 / semi-axis
     int ncoef;               // spherical harmonics: value = sum cn[i] P_{l[i]}^{m[i]}(cos theta) {1, cos m phi, sin m phi}
     signed char l[kMaxCoef], m[kMaxCoef];   // m as given (sign selects cos / sin)
     double cn[kMaxCoef];     // c * N_lm * (m != 0 ? sqrt 2 : 1)
@@ -28,19 +29,39 @@ struct RenderArgs {
     double vdx;
 };
 
-// P_l^m(x), m >= 0, Condon-Shortley phase (Eq. 10), by the standard recurrences
-__device__ double legendre_p(int l, int m, double x) {
-    const double s = sqrt(fmax(0.0, 1.0 - x * x));
-    double pmm = 1.0;
-    for (int k = 1; k <= m; ++k) pmm = -pmm * (double)(2 * k - 1) * s;
-    if (l == m) return pmm;
-    double pm1 = x * (double)(2 * m + 1) * pmm;
-    for (int ll = m + 2; ll <= l; ++ll) {
-        const double p = ((double)(2 * ll - 1) * x * pm1 - (double)(ll + m - 1) * pmm) / (double)(ll - m);
-        pmm = pm1;
-        pm1 = p;
+// R(theta, phi) = sum_i cn[i] P_{l_i}^{|m_i|}(cos theta) {1 | cos |m| phi | sin |m| phi}, the triplets sorted by (|m|, l):
+// P_m^m and (cos m phi, sin m phi) advance with m, P_l^m by the upward recurrence in l
+//   (l + 1 - m) P_{l+1}^m = (2l + 1) x P_l^m - (l + m) P_{l-1}^m        (Condon-Shortley phase, Eq. 10),
+// so one voxel costs O(l_max^2) FP64 operations and no trigonometric call.
+__device__ double sh_radius(const RenderArgs &A, double ct, double cphi, double sphi) {
+    const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+    double R = 0.0, pmm = 1.0, cm = 1.0, sm = 0.0;
+    int am = 0, i = 0;
+    while (i < A.ncoef) {
+        const int target = A.m[i] < 0 ? -A.m[i] : A.m[i];
+        while (am < target) {
+            ++am;
+            pmm = -pmm * (double)(2 * am - 1) * st;
+            const double t = cm * cphi - sm * sphi;
+            sm = sm * cphi + cm * sphi;
+            cm = t;
+        }
+        double pl = pmm, pl_prev = 0.0;
+        int lcur = am;
+        while (i < A.ncoef && (A.m[i] < 0 ? -A.m[i] : A.m[i]) == am) {
+            const int l = A.l[i];
+            while (lcur < l) {
+                const double pn = ((double)(2 * lcur + 1) * ct * pl - (double)(lcur + am) * pl_prev) / (double)(lcur + 1 - am);
+                pl_prev = pl;
+                pl = pn;
+                ++lcur;
+            }
+            const double ang = A.m[i] > 0 ? cm : (A.m[i] < 0 ? sm : 1.0);
+            R = fma(A.cn[i] * pl, ang, R);
+            ++i;
+        }
     }
-    return pm1;
+    return R;
 }
 
 __global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
@@ -57,22 +78,16 @@ __global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
     const double zb = A.Rt[6] * x + A.Rt[7] * y + A.Rt[8] * z;
     bool inside = false;
     if (A.kind == SCATMAN_SHAPE_ELLIPSOID) {
-        const double u = xb / A.a, w = yb / A.b, t = zb / A.c;
+        const double u = xb * A.a, w = yb * A.b, t = zb * A.c;   // A.a, A.b, A.c hold the reciprocal semi-axes
         inside = u * u + w * w + t * t <= 1.0;
     } else if (A.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS) {
         const double r = sqrt(xb * xb + yb * yb + zb * zb);
         if (r < A.r_lo) inside = true;
         else if (r <= A.r_hi) {
             const double ct = r > 0.0 ? zb / r : 1.0;
-            const double ph = atan2(yb, xb);
-            double R = 0.0;
-            for (int i = 0; i < A.ncoef; ++i) {
-                const int l = A.l[i], m = A.m[i], am = m < 0 ? -m : m;
-                double f = A.cn[i] * legendre_p(l, am, ct);
-                if (m > 0) f *= cos((double)am * ph);
-                else if (m < 0) f *= sin((double)am * ph);
-                R += f;
-            }
+            const double rho = sqrt(xb * xb + yb * yb);
+            const double cphi = rho > 0.0 ? xb / rho : 1.0, sphi = rho > 0.0 ? yb / rho : 0.0;   // phi = atan2(y, x)
+            const double R = sh_radius(A, ct, cphi, sphi);
             inside = r <= R;
         }
     } else if (A.kind == SCATMAN_SHAPE_RADIAL_MAP) {
@@ -91,8 +106,8 @@ __global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
         const double hi = A.radii[(size_t)i1 * A.nlon + j0] * (1.0 - tj) + A.radii[(size_t)i1 * A.nlon + j1] * tj;
         inside = r <= lo * (1.0 - ti) + hi * ti;
     } else {
-        const double fx = xb / A.vdx + 0.5 * (double)A.nvx, fy = yb / A.vdx + 0.5 * (double)A.nvy,
-                     fz = zb / A.vdx + 0.5 * (double)A.nvz;
+        const double fx = xb * A.vdx + 0.5 * (double)A.nvx, fy = yb * A.vdx + 0.5 * (double)A.nvy,
+                     fz = zb * A.vdx + 0.5 * (double)A.nvz;   // A.vdx holds 1 / cell size
         const double cx = floor(fx), cy = floor(fy), cz = floor(fz);
         if (cx >= 0.0 && cx < (double)A.nvx && cy >= 0.0 && cy < (double)A.nvy && cz >= 0.0 && cz < (double)A.nvz)
             inside = A.vol[((size_t)cz * A.nvy + (size_t)cy) * A.nvx + (size_t)cx] != 0;
@@ -126,7 +141,7 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
     switch (s.kind) {
         case SCATMAN_SHAPE_ELLIPSOID:
             if (!(s.a > 0.0 && s.b > 0.0 && s.c > 0.0)) return 1;
-            A.a = s.a; A.b = s.b; A.c = s.c;
+            A.a = 1.0 / s.a; A.b = 1.0 / s.b; A.c = 1.0 / s.c;
             break;
         case SCATMAN_SHAPE_SPHERICAL_HARMONICS: {
             if (s.ncoef < 1 || s.ncoef > kMaxCoef || !s.h_coef) return 1;
@@ -150,6 +165,15 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
             double bound = 0.0;
             for (int l = 1; l <= 32; ++l) bound += std::sqrt(norm2[l]) * std::sqrt((2 * l + 1) / (4 * kPi));
             A.ncoef = s.ncoef;
+            for (int i = 1; i < A.ncoef; ++i)   // insertion sort by (|m|, l): the order sh_radius walks
+                for (int j = i; j > 0; --j) {
+                    const int ka = (A.m[j] < 0 ? -A.m[j] : A.m[j]) * 64 + A.l[j];
+                    const int kb = (A.m[j - 1] < 0 ? -A.m[j - 1] : A.m[j - 1]) * 64 + A.l[j - 1];
+                    if (ka >= kb) break;
+                    std::swap(A.l[j], A.l[j - 1]);
+                    std::swap(A.m[j], A.m[j - 1]);
+                    std::swap(A.cn[j], A.cn[j - 1]);
+                }
             A.r_lo = (r00 - bound) * (1.0 - 1e-9) - 1e-300;
             A.r_hi = (r00 + bound) * (1.0 + 1e-9) + 1e-300;
             break;
@@ -160,7 +184,7 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
             break;
         case SCATMAN_SHAPE_VOLUME_MAP:
             if (s.nvx < 1 || s.nvy < 1 || s.nvz < 1 || !s.d_volume || !(s.vdx > 0.0)) return 1;
-            A.nvx = s.nvx; A.nvy = s.nvy; A.nvz = s.nvz; A.vol = s.d_volume; A.vdx = s.vdx;
+            A.nvx = s.nvx; A.nvy = s.nvy; A.nvz = s.nvz; A.vol = s.d_volume; A.vdx = 1.0 / s.vdx;
             break;
         default: return 1;
     }
