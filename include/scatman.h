@@ -132,6 +132,21 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
                        const double *d_q, int64_t npix, const double *h_quat, int32_t batch,
                        const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
 
+/* The separable route (the paper's own evaluation points: Block 6 of Fig. 4 transforms every slice on a
+ * uniform (qx, qy) grid): the detector is a TENSOR GRID of transverse momentum transfers, pixel (a, b)
+ * at (qx[a], qy[b], qz) with qz = -(k - sqrt(k^2 - qx^2 - qy^2)) on the Ewald sphere (Eq. 3-4, in
+ * north_star's sign), so the slice transform factors into two small complex GEMMs per slice instead of the
+ * (pixel x voxel) contraction -- npx-fold less arithmetic, FP32 CUDA-core GEMMs with FP64 phases.  Same a0 / a2 steps,
+ * same conventions and output scale as scatman_simulate; grid points with qx^2 + qy^2 > k^2 (no scattering direction)
+ * get I = 0.  d_qx[npx], d_qy[npy]: FP64 device arrays (any values, e.g. the DFT grid 2 pi m / (N dx)).
+ * d_I[b][npy][npx].  rho_mode from opts; method / precision / flags of opts are ignored. */
+int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
+                                  size_t *bytes);
+int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                           const double *d_qx, int32_t npx, const double *d_qy, int32_t npy, const double *h_quat,
+                           int32_t batch, const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I,
+                           void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies h_dn to the device, runs
  * scatman_simulate on the context's own stream, copies I back into h_I and synchronises.  This entry
  * point alone owns device memory: a grow-only arena kept in the context until scatman_destroy.

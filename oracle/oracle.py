@@ -116,3 +116,27 @@ def simulate(dn: np.ndarray, voxel, lam: float, npx: int, npy: int, theta_max_de
     if pixels is not None:
         return simulate_q(dn, voxel, lam, q[np.asarray(pixels)], quat, rho_mode, method)
     return simulate_q(dn, voxel, lam, q, quat, rho_mode, method).reshape(npy, npx)
+
+
+def qgrid_q(qx: np.ndarray, qy: np.ndarray, lam: float):
+    """Momentum transfers of a tensor-grid detector: pixel (b, a) has transverse components (qx[a], qy[b]) and lies on the
+    Ewald sphere, |q + k z^| = k (Eq. 3-4; the paper's q = k0 - k has qz = k0 (1 - cos theta) >= 0, north_star's
+    q = k (s^ - z^) has the opposite sign): qz = -(k - sqrt(k^2 - qx^2 - qy^2)).  Returns (q float64 [npy*npx][3], propagating
+    bool [npy*npx]); points with qx^2 + qy^2 > k^2 have no scattering direction (propagating False, qz set to 0)."""
+    qx = np.asarray(qx, dtype=np.float64)
+    qy = np.asarray(qy, dtype=np.float64)
+    k = 2.0 * np.pi / float(lam)
+    QX, QY = np.meshgrid(qx, qy, indexing="xy")          # [npy][npx]
+    kz2 = k * k - QX * QX - QY * QY
+    ok = kz2 >= 0.0
+    qz = np.where(ok, -(k - np.sqrt(np.where(ok, kz2, 0.0))), 0.0)
+    q = np.stack([QX.ravel(), QY.ravel(), qz.ravel()], axis=1)
+    return q, ok.ravel()
+
+
+def simulate_qgrid(dn: np.ndarray, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR) -> np.ndarray:
+    """Whole path on a tensor-grid detector: the same direct triple sum, at qgrid_q's points; I = 0 where nothing propagates.
+    float64 [npy][npx]."""
+    q, ok = qgrid_q(qx, qy, lam)
+    I = simulate_q(dn, voxel, lam, q, quat, rho_mode)
+    return np.where(ok, I, 0.0).reshape(len(np.atleast_1d(qy)), len(np.atleast_1d(qx)))

@@ -26,7 +26,7 @@ struct scatman_ctx {
 
 namespace scatman {
 
-static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Batch chunks x z splits of the tensor kernel: minimise waves * per-item length (in slices), where an
 // item costs its slices plus ~2 slice-equivalents of fill (A load, pipeline ramp).
@@ -389,6 +389,95 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
     if (!d_q) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "d_q is null");
     return run_path(ctx, d_dn, grid, lambda, nullptr, d_q, npix, h_quat, batch, opts, d_ws, ws_bytes, d_I,
                     (cudaStream_t)cuda_stream);
+}
+
+// ---- separable route: workspace layout -------------------------------------------------------------------------
+struct SepPlan {
+    Plan p;
+    int nzs = 1;
+    size_t off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
+           off_partial = 0, total = 0;
+};
+static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int num_sms) {
+    SepPlan sp;
+    Plan &p = sp.p;
+    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
+    p.npix = (int64_t)npx * npy; p.batch = batch; p.rho_mode = rho_mode;
+    p.nvox = (int64_t)g.nx * g.ny * g.nz;
+    sp.nzs = sep_zsplit(p, npx, npy, num_sms);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
+    sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
+    sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    sp.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    sp.off_max = take(sizeof(unsigned) * (size_t)batch);
+    sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
+    sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
+    sp.off_h = take(sizeof(float2) * (size_t)g.nz * g.ny * npx);
+    sp.off_flags = take((size_t)g.nz * ((g.ny + 15) / 16));
+    sp.off_partial = take(sizeof(float2) * (size_t)sp.nzs * npx * npy);
+    sp.total = off;
+    return sp;
+}
+
+int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
+                                  size_t *bytes) {
+    if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
+    if (!valid_grid(grid) || npx < 1 || npy < 1 || batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = make_sep_plan(*grid, 1.0, npx, npy, batch, 0, ctx->num_sms).total;
+    return SCATMAN_OK;
+}
+
+int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_qx,
+                           int32_t npx, const double *d_qy, int32_t npy, const double *h_quat, int32_t batch,
+                           const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_dn || !d_I || !d_ws || !d_qx || !d_qy || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) ||
+        batch < 1 || batch > 65535 || npx < 1 || npy < 1 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    if (h_quat && !valid_quats(h_quat, batch)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "quaternion is not unit");
+    if (((uintptr_t)d_dn | (uintptr_t)d_ws | (uintptr_t)d_I) & 15)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
+    cudaSetDevice(ctx->device);
+    const SepPlan sp = make_sep_plan(*grid, lambda, npx, npy, batch, o.rho_mode, ctx->num_sms);
+    const Plan &p = sp.p;
+    if (ws_bytes < sp.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint8_t *ws = (uint8_t *)d_ws;
+    int nl = 0;
+    cudaError_t e = cudaSuccess;
+    ctx->ev_valid = false;
+    ctx->d_count = nullptr;
+    const float *src = d_dn;
+    if (h_quat && !all_identity(h_quat, batch)) {
+        double *rm = (double *)(ws + sp.off_rotmat);
+        e = upload_rotmats(h_quat, batch, rm, st, &nl);
+        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
+        src = (const float *)(ws + sp.off_rot);
+    }
+    float *rho = (float *)(ws + sp.off_rho);
+    e = launch_strength(src, p, batch, rho, (unsigned *)(ws + sp.off_max), st);
+    ++nl;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    float2 *Ex = (float2 *)(ws + sp.off_ex), *Ey = (float2 *)(ws + sp.off_ey);
+    e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
+    nl += 2;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
+    cudaEventRecord(ctx->ev0, st);
+    for (int b = 0; b < batch; ++b) {
+        e = launch_sep_item((const float2 *)rho + (size_t)b * p.nvox, p, Ex, Ey, d_qx, npx, d_qy, npy, sp.nzs,
+                            (float2 *)(ws + sp.off_h), ws + sp.off_flags, (float2 *)(ws + sp.off_partial),
+                            d_I + (size_t)b * npx * npy, st);
+        nl += 4;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid stages");
+    }
+    cudaEventRecord(ctx->ev1, st);
+    ctx->ev_valid = true;
+    ctx->last_launches = nl;
+    return SCATMAN_OK;
 }
 
 int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,

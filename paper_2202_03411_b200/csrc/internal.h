@@ -65,6 +65,12 @@ cudaError_t launch_simt_sincos(const float *d_rho, const double *d_q, const Plan
 cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
                               cudaStream_t st);
 
+cudaError_t launch_sep_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p, float2 *d_Ex,
+                              float2 *d_Ey, cudaStream_t st);
+int sep_zsplit(const Plan &p, int npx, int npy, int num_sms);
+cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_Ex, const float2 *d_Ey, const double *d_qx,
+                            int npx, const double *d_qy, int npy, int nzs, float2 *d_H, unsigned char *d_flags,
+                            float2 *d_partial, float *d_I, cudaStream_t st);
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
 
 // tensor path: tensor maps are encoded on the host through the driver entry point

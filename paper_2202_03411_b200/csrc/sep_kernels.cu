@@ -1,0 +1,266 @@
+// sep_kernels.cu -- the separable route for detectors that are a tensor grid in (qx, qy): the paper's
+// own evaluation points (Block 6 of Fig. 4 takes the 2-D DFT of every slice on a uniform (qx, qy) grid, PAPER.md:154,
+// 146; cost model PAPER.md:435).  On such a grid the inner transform of Eq. 2/9 factors,
+//     F_j[b, a] = sum_y e^{i qy[b] y} ( sum_x rho~_j[y, x] e^{i qx[a] x} ),
+// into two small complex GEMMs per slice instead of one (pixel x voxel) contraction, N_p times less work:
+//   stage X   H[(j, y), a] = sum_x rho~[(j, y), x] Ex[x, a]               one GEMM over all slices at once
+//   stage YZ  A[b, a]     = sum_j e^{i qz(a, b) z_j} sum_y Ey[b, y] H[(j, y), a]   (Blocks 7-8 fused: the slice phase
+//             is applied to the accumulator tile in registers, slices are summed in registers)
+// with qz = -(k - sqrt(k^2 - qx^2 - qy^2)) on the Ewald sphere (Eq. 3-4, north_star's sign).
+// FP32 CUDA-core GEMMs (64 x 64 x 16 tiles, 4 x 4 complex outputs per thread), FP64 phases.
+#include "internal.h"
+
+namespace scatman {
+
+constexpr int kBM = 64, kBN = 64, kBK = 16;
+
+__device__ __forceinline__ double centre_d(int i, int n, double d) { return ((double)i - 0.5 * (double)(n - 1)) * d; }
+
+// E[i][a] = e^{i q[a] x_i} (transposed = false, a fastest) or E[a][i] (transposed = true, i fastest); FP64 phase
+__global__ void sep_table_kernel(const double *__restrict__ q, int nq, int n, double d, int transposed,
+                                 float2 *__restrict__ E) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)nq * n) return;
+    int a, i;
+    if (transposed) { a = (int)(t / n); i = (int)(t % n); }
+    else { i = (int)(t / nq); a = (int)(t % nq); }
+    double s, c;
+    sincos(q[a] * centre_d(i, n, d), &s, &c);
+    E[t] = make_float2((float)c, (float)s);
+}
+
+// One 64 x 64 complex output tile: acc[4][4] += A[m0.., k] B[k, n0..] over k in [0, K).  A row-major [M][lda] (k fastest),
+// B row-major [K][ldb] (n fastest).  256 threads: thread (ty, tx) = (tid / 16, tid % 16) owns rows ty*4.. and cols tx*4..
+struct TileSmem {
+    float2 As[kBK][kBM + 2];
+    float2 Bs[kBK][kBN + 2];
+};
+
+// kflag (optional): one byte per 16-k chunk, 0 = every B row of the chunk is zero -> the chunk is skipped (uniformly).
+__device__ __forceinline__ int next_chunk(const unsigned char *kflag, int k0, int K) {
+    if (kflag)
+        while (k0 < K && kflag[k0 / kBK] == 0) k0 += kBK;
+    return k0;
+}
+
+__device__ __forceinline__ void tile_gemm(const float2 *__restrict__ A, int lda, int M, int m0, const float2 *__restrict__ B,
+                                          int ldb, int N, int n0, int K, const unsigned char *__restrict__ kflag, TileSmem &sm,
+                                          float2 (&acc)[4][4]) {
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    // loader roles: A tile 64 rows x 16 k: thread -> row tid / 4, k = (tid % 4) * 4 .. +3;  B tile 16 k x 64 n: k = tid / 16, n = (tid % 16) * 4 .. +3
+    const int ar = tid >> 2, ak = (tid & 3) * 4;
+    const int bk = tid >> 4, bn = (tid & 15) * 4;
+    float2 ra[4], rb[4];
+    auto load = [&](int k0) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m = m0 + ar, k = k0 + ak + i;
+            ra[i] = (m < M && k < K) ? __ldg(A + (size_t)m * lda + k) : make_float2(0.f, 0.f);
+            const int kk = k0 + bk, n = n0 + bn + i;
+            rb[i] = (kk < K && n < N) ? __ldg(B + (size_t)kk * ldb + n) : make_float2(0.f, 0.f);
+        }
+    };
+    int k0 = next_chunk(kflag, 0, K);
+    if (k0 < K) load(k0);
+    while (k0 < K) {
+        __syncthreads();   // previous tile fully consumed
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            sm.As[ak + i][ar] = ra[i];
+            sm.Bs[bk][bn + i] = rb[i];
+        }
+        __syncthreads();
+        const int kn = next_chunk(kflag, k0 + kBK, K);
+        if (kn < K) load(kn);   // next tile's global loads overlap this tile's FMAs
+#pragma unroll
+        for (int k = 0; k < kBK; ++k) {
+            float2 a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                a[i] = sm.As[k][ty * 4 + i];
+                b[i] = sm.Bs[k][tx * 4 + i];
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    acc[i][j].x = fmaf(a[i].x, b[j].x, acc[i][j].x);
+                    acc[i][j].x = fmaf(-a[i].y, b[j].y, acc[i][j].x);
+                    acc[i][j].y = fmaf(a[i].x, b[j].y, acc[i][j].y);
+                    acc[i][j].y = fmaf(a[i].y, b[j].x, acc[i][j].y);
+                }
+        }
+        k0 = kn;
+    }
+}
+
+// flags[j][c] = 1 if any rho~ value of slice j, y rows [16c, 16c+16) is non-zero (one warp per chunk)
+__global__ void sep_rowflags_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nyc,
+                                    unsigned char *__restrict__ flags) {
+    const int chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (chunk >= nz * nyc) return;
+    const int j = chunk / nyc, c = chunk % nyc;
+    const int y0 = c * 16, y1 = min(ny, y0 + 16);
+    const float2 *src = rho + ((size_t)j * ny + y0) * nx;
+    const size_t n = (size_t)(y1 - y0) * nx;
+    bool any = false;
+    for (size_t e = lane; e < n; e += 32) {
+        const float2 v = __ldg(src + e);
+        any |= (v.x != 0.f) | (v.y != 0.f);
+    }
+    any = __any_sync(0xffffffffu, any);
+    if (lane == 0) flags[chunk] = any ? 1 : 0;
+}
+
+// stage X: H[M][N] = rho[M][K] Ex[K][N]  (M = nz * ny, K = nx, N = npx).  Row tiles whose rho rows are all zero are not
+// multiplied: H is written as zeros (vacuum rows are most of a grid).
+__global__ void __launch_bounds__(256) sep_stage_x_kernel(const float2 *__restrict__ rho, const float2 *__restrict__ Ex, int M,
+                                                          int K, int N, float2 *__restrict__ H) {
+    __shared__ TileSmem sm;
+    __shared__ int s_any;
+    const int m0 = blockIdx.x * kBM, n0 = blockIdx.y * kBN;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    if (tid == 0) s_any = 0;
+    __syncthreads();
+    bool any = false;
+    for (size_t e = tid; e < (size_t)kBM * K; e += 256) {
+        const int m = m0 + (int)(e / K);
+        if (m < M) {
+            const float2 v = __ldg(rho + (size_t)m * K + (e % K));
+            any |= (v.x != 0.f) | (v.y != 0.f);
+        }
+    }
+    if (any) s_any = 1;
+    __syncthreads();
+    float2 acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_float2(0.f, 0.f);
+    if (s_any) tile_gemm(rho, K, M, m0, Ex, N, N, n0, K, nullptr, sm, acc);
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int m = m0 + ty * 4 + i, n = n0 + tx * 4 + j;
+            if (m < M && n < N) H[(size_t)m * N + n] = acc[i][j];
+        }
+}
+
+// stage YZ: partial[zs][b * npx + a] = sum over this z range of e^{i qz z_j} sum_y Ey[b][y] H[j][y][a].
+// qz in turns per unit length: qzt = qz / 2pi, so the phase of slice j is sincospi(2 frac(qzt z_j)) with the reduction in FP64.
+__global__ void __launch_bounds__(256) sep_stage_yz_kernel(const float2 *__restrict__ Ey, const float2 *__restrict__ H,
+                                                           const double *__restrict__ qx, const double *__restrict__ qy,
+                                                           double k, int npx, int npy, int ny, int nz, double dz, int nzs,
+                                                           const unsigned char *__restrict__ flags, int nyc,
+                                                           float2 *__restrict__ partial) {
+    __shared__ TileSmem sm;
+    const int m0 = blockIdx.y * kBM, n0 = blockIdx.x * kBN, zs = blockIdx.z;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int z0 = (int)(((long long)nz * zs) / nzs), z1 = (int)(((long long)nz * (zs + 1)) / nzs);
+    double qzt[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int b = m0 + ty * 4 + i, a = n0 + tx * 4 + j;
+            double v = 0.0;
+            if (b < npy && a < npx) {
+                const double qxy2 = qx[a] * qx[a] + qy[b] * qy[b];
+                const double kz2 = k * k - qxy2;
+                // qz = -(k - sqrt(k^2 - qxy^2)) = -qxy^2 / (k + sqrt(k^2 - qxy^2)): no cancellation near forward
+                v = kz2 >= 0.0 ? -qxy2 / (k + sqrt(kz2)) : 0.0;
+            }
+            qzt[i][j] = v * (0.5 / 3.14159265358979323846);
+        }
+    float2 tot[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tot[i][j] = make_float2(0.f, 0.f);
+    for (int jz = z0; jz < z1; ++jz) {
+        float2 acc[4][4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j] = make_float2(0.f, 0.f);
+        tile_gemm(Ey, ny, npy, m0, H + (size_t)jz * ny * npx, npx, npx, n0, ny, flags + (size_t)jz * nyc, sm, acc);
+        const double zj = centre_d(jz, nz, dz);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                double t = qzt[i][j] * zj;
+                t -= rint(t);
+                float s, c;
+                sincospif(2.0f * (float)t, &s, &c);
+                tot[i][j].x = fmaf(c, acc[i][j].x, tot[i][j].x);
+                tot[i][j].x = fmaf(-s, acc[i][j].y, tot[i][j].x);
+                tot[i][j].y = fmaf(c, acc[i][j].y, tot[i][j].y);
+                tot[i][j].y = fmaf(s, acc[i][j].x, tot[i][j].y);
+            }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int b = m0 + ty * 4 + i, a = n0 + tx * 4 + j;
+            if (b < npy && a < npx) partial[(size_t)zs * npx * npy + (size_t)b * npx + a] = tot[i][j];
+        }
+}
+
+// I[b][a] = |dV sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
+__global__ void sep_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
+                                    const double *__restrict__ qy, double k, int npx, int npy, int nzs, float dV,
+                                    float *__restrict__ I) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= (int64_t)npx * npy) return;
+    const int a = (int)(p % npx), b = (int)(p / npx);
+    float re = 0.f, im = 0.f;
+    for (int s = 0; s < nzs; ++s) {
+        const float2 v = partial[(size_t)s * npx * npy + p];
+        re += v.x;
+        im += v.y;
+    }
+    re *= dV;
+    im *= dV;
+    const bool real = qx[a] * qx[a] + qy[b] * qy[b] <= k * k;
+    I[p] = real ? re * re + im * im : 0.f;
+}
+
+cudaError_t launch_sep_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p, float2 *d_Ex,
+                              float2 *d_Ey, cudaStream_t st) {
+    const int64_t nxe = (int64_t)npx * p.nx, nye = (int64_t)npy * p.ny;
+    sep_table_kernel<<<(unsigned)((nxe + 255) / 256), 256, 0, st>>>(d_qx, npx, p.nx, p.dx, 0, d_Ex);   // Ex[x][a]
+    sep_table_kernel<<<(unsigned)((nye + 255) / 256), 256, 0, st>>>(d_qy, npy, p.ny, p.dy, 1, d_Ey);   // Ey[b][y]
+    return cudaGetLastError();
+}
+
+int sep_zsplit(const Plan &p, int npx, int npy, int num_sms) {
+    const int tiles = ((npx + kBN - 1) / kBN) * ((npy + kBM - 1) / kBM);
+    int nzs = (2 * num_sms + tiles - 1) / tiles;
+    if (nzs > p.nz) nzs = p.nz;
+    if (nzs > 64) nzs = 64;
+    return nzs < 1 ? 1 : nzs;
+}
+
+// one batch item: rho (FP32 complex [nz][ny][nx], without dV) -> I[npy][npx]
+cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_Ex, const float2 *d_Ey, const double *d_qx,
+                            int npx, const double *d_qy, int npy, int nzs, float2 *d_H, unsigned char *d_flags,
+                            float2 *d_partial, float *d_I, cudaStream_t st) {
+    const int M = p.nz * p.ny;
+    const int nyc = (p.ny + 15) / 16;
+    const double k = 2.0 * 3.14159265358979323846 / p.lambda;
+    sep_rowflags_kernel<<<(unsigned)((p.nz * nyc + 7) / 8), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nyc, d_flags);
+    dim3 gx((M + kBM - 1) / kBM, (npx + kBN - 1) / kBN);
+    sep_stage_x_kernel<<<gx, 256, 0, st>>>(d_rho, d_Ex, M, p.nx, npx, d_H);
+    dim3 gy((npx + kBN - 1) / kBN, (npy + kBM - 1) / kBM, nzs);
+    sep_stage_yz_kernel<<<gy, 256, 0, st>>>(d_Ey, d_H, d_qx, d_qy, k, npx, npy, p.ny, p.nz, p.dz, nzs, d_flags, nyc,
+                                            d_partial);
+    const int64_t npix = (int64_t)npx * npy;
+    sep_finalize_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(d_partial, d_qx, d_qy, k, npx, npy, nzs,
+                                                                        (float)(p.dx * p.dy * p.dz), d_I);
+    return cudaGetLastError();
+}
+
+}  // namespace scatman

@@ -286,3 +286,41 @@ def test_p11_half_voxel_trilinear_weights():
     assert np.allclose(out[:, 3, 3, 0], np.float32(wgt)) and np.allclose(out[:, 3, 3, 1], np.float32(0.5 * wgt))
     # beam voxel (x=+2, y=+2) maps to body (2 sqrt2, 0): outside the grid (x index 4.83 -> neighbour 5 is out, 4 is empty)
     assert np.all(out[:, 4, 4] == 0)
+
+
+# ------------------------------------------------------------------------------------------ tensor-grid detector
+def test_qgrid_points_lie_on_the_ewald_sphere_and_match_the_flat_detector():
+    """qgrid_q: |q + k z^| = k for every propagating point (Eq. 3-4); fed the (qx, qy) of a flat-detector pixel it returns that
+    pixel's qz (the q-map is pinned by geometry above); forward point qz = 0; |q_xy| = k is 90 degrees: qz = -k."""
+    lam = 13.0
+    k = 2 * np.pi / lam
+    qx = np.linspace(-0.9 * k, 1.1 * k, 23)
+    qy = np.linspace(-0.5 * k, 0.7 * k, 17)
+    q, ok = O.qgrid_q(qx, qy, lam)
+    assert q.shape == (17 * 23, 3) and np.array_equal(q[:23, 0], qx) and np.all(q[:23, 1] == qy[0])
+    r = np.sqrt(q[:, 0] ** 2 + q[:, 1] ** 2 + (q[:, 2] + k) ** 2)
+    assert np.allclose(r[ok], k, rtol=1e-13)
+    assert np.array_equal(ok, (q[:, 0] ** 2 + q[:, 1] ** 2) <= k * k) and not ok.all() and np.all(q[~ok, 2] == 0)
+    qm = O.qmap(9, 7, 50.0, lam, 0.3, -0.2)
+    for p in range(0, 63, 5):
+        qq, okp = O.qgrid_q([qm[p, 0]], [qm[p, 1]], lam)
+        assert okp[0] and np.isclose(qq[0, 2], qm[p, 2], rtol=1e-12, atol=1e-15)
+    q0, _ = O.qgrid_q([0.0, k], [0.0], lam)
+    assert q0[0, 2] == 0.0 and np.isclose(q0[1, 2], -k)
+
+
+def test_qgrid_single_slice_on_the_dft_grid_is_numpy_fft2():
+    """One slice, q on the DFT grid: the whole tensor-grid pattern equals |dV fft2(rho)|^2 (library routine), and qz drops out."""
+    rng = np.random.default_rng(21)
+    nx, ny, d = 12, 10, 1.5
+    g = np.zeros((1, ny, nx, 2), np.float32)
+    g[0, ..., 0] = rng.uniform(-0.02, 0.05, (ny, nx))
+    g[0, ..., 1] = rng.uniform(0.0, 0.02, (ny, nx))
+    lam = 2.0                                   # k = 3.14 > max |q_xy| = 2.96 so that every point propagates
+    mx, my = np.arange(nx), np.arange(ny)
+    qx = -2 * np.pi * np.where(mx < nx / 2, mx, mx - nx) / (nx * d)     # e^{i q x} = e^{-2 pi i m n / N}
+    qy = -2 * np.pi * np.where(my < ny / 2, my, my - ny) / (ny * d)
+    I = O.simulate_qgrid(g, (d, d, 2.0), lam, qx, qy)
+    rho = g[0, ..., 0].astype(np.float64) + 1j * g[0, ..., 1].astype(np.float64)
+    ref = np.abs(np.fft.fft2(rho) * d * d * 2.0) ** 2
+    assert np.allclose(I, ref, rtol=1e-11)
