@@ -23,6 +23,7 @@ FLAG_COUNT_ISSUED = 2
 EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
+    "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid",
     "scatman_render", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
@@ -85,6 +86,9 @@ def load_library() -> C.CDLL:
                                      C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                         C.POINTER(Options), vp]
+    L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(C.c_size_t)]
+    L.scatman_simulate_qgrid.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i32, vp, i32, C.POINTER(dbl), i32,
+                                         C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -280,6 +284,31 @@ class Scatman:
                                                 C.c_void_p(q.data_ptr()), npix, qp, batch, C.byref(opts),
                                                 C.c_void_p(workspace.data_ptr()), workspace.numel(),
                                                 C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out if dn.dim() == 5 else out[0]
+
+    def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, workspace=None, out=None,
+                       stream=None):
+        """I float32 [B][npy][npx] on the tensor grid (qx[a], qy[b]) of transverse momentum transfers (CUDA float64 1-D
+        tensors): the separable route (scatman_simulate_qgrid)."""
+        import torch
+        self._check_dn(dn)
+        for q in (qx, qy):
+            if not (q.is_cuda and q.dtype == torch.float64 and q.is_contiguous() and q.dim() == 1):
+                raise ValueError("qx, qy must be contiguous 1-D CUDA float64 tensors")
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        npx, npy = int(qx.numel()), int(qy.numel())
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(need)))
+        if workspace is None:
+            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dn.device)
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+        opts = Options(int(rho_mode), 0, 0, 0)
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_qgrid(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
+                                                    C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy, qp, batch,
+                                                    C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
+                                                    C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out if dn.dim() == 5 else out[0]
 
     def simulate_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,

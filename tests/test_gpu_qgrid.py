@@ -1,0 +1,124 @@
+"""GPU parity of the separable tensor-grid route (scatman_simulate_qgrid, sep_kernels.cu) against the oracle's direct
+triple sum at the same grid points, and against numpy.fft2 where the grid is the DFT grid."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2202_03411_b200 import workloads as W
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sm():
+    import torch
+    from paper_2202_03411_b200 import binding as B, build
+    build.build()
+    assert torch.cuda.is_available()
+    s = B.Scatman(0)
+    yield s
+    s.close()
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _uniform_q(lam, theta_max_deg, n):
+    """n points of a uniform transverse grid reaching sin(theta_max) k (the paper's 'same angular cross section' pixels)."""
+    k = 2 * np.pi / lam
+    return (np.arange(n) + 0.5 - 0.5 * n) * (2 * k * np.sin(np.radians(theta_max_deg)) / n)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_ragged_batch_with_orientations(sm, mode):
+    rng = np.random.default_rng(31)
+    nx, ny, nz, B = 70, 45, 11, 3
+    g = np.stack([W.random_grid(81 + i, nx, ny, nz, fill=0.4) for i in range(B)])
+    quat = W.random_quaternions(rng, B)
+    quat[2] = [1, 0, 0, 0]
+    voxel, lam = (2.0, 2.5, 3.0), 14.0
+    qx, qy = _uniform_q(lam, 35.0, 37), _uniform_q(lam, 25.0, 29)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), quat=quat, rho_mode=mode).cpu().numpy()
+    for b in range(B):
+        ref = O.simulate_qgrid(g[b], voxel, lam, qx, qy, quat=quat[b], rho_mode=mode)
+        assert_parity(I[b], ref, what=f"qgrid ragged b={b} mode={mode}")
+
+
+def test_sparse_blobs_and_evanescent_points(sm):
+    """Mostly empty grid (the kernels skip vacuum rows); a q grid that runs past |q_xy| = k: those points must be exactly 0."""
+    g = W.sparse_blobs_grid(91, 150, 130, 9, nblobs=6, max_extent=40)
+    voxel, lam = (2.0, 2.0, 2.5), 11.0
+    k = 2 * np.pi / lam
+    qx, qy = np.linspace(-1.2 * k, 1.2 * k, 41), np.linspace(-0.8 * k, 0.8 * k, 33)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy)).cpu().numpy()
+    ref = O.simulate_qgrid(g, voxel, lam, qx, qy)
+    _, ok = O.qgrid_q(qx, qy, lam)
+    assert not ok.all() and np.all(I.ravel()[~ok] == 0)
+    assert_parity(I, ref, what="qgrid sparse")
+
+
+def test_cfg1_sphere_on_a_uniform_q_grid(sm):
+    w = W.config(0)
+    g = w.grid(0)
+    vox = (w.dx, w.dy, w.dz)
+    qx = qy = _uniform_q(w.lam, w.theta_max_deg, 64)
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy()
+    ref = O.simulate_qgrid(g, vox, w.lam, qx, qy)
+    assert_parity(I, ref, what="qgrid cfg1")
+    assert np.allclose(I, I[::-1, :], rtol=1e-4) and np.allclose(I, I.T, rtol=1e-4)   # D4 symmetry of the sphere pattern
+
+
+def test_cfg3_quarter_scale_droplet(sm):
+    w = W.config(2, scale=0.25)
+    g = w.grid(0)
+    vox = (w.dx, w.dy, w.dz)
+    qx, qy = _uniform_q(w.lam, w.theta_max_deg, w.npx), _uniform_q(w.lam, w.theta_max_deg, w.npy)
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy()
+    ref = O.simulate_qgrid(g, vox, w.lam, qx, qy)
+    assert_parity(I, ref, what="qgrid cfg3 quarter")
+
+
+def test_single_slice_on_the_dft_grid_is_fft2(sm):
+    rng = np.random.default_rng(33)
+    nx, ny, d = 96, 80, 1.5
+    g = np.zeros((1, ny, nx, 2), np.float32)
+    g[0, ..., 0] = rng.uniform(-0.02, 0.05, (ny, nx))
+    g[0, ..., 1] = rng.uniform(0.0, 0.02, (ny, nx))
+    lam = 2.0
+    mx, my = np.arange(nx), np.arange(ny)
+    qx = -2 * np.pi * np.where(mx < nx / 2, mx, mx - nx) / (nx * d)
+    qy = -2 * np.pi * np.where(my < ny / 2, my, my - ny) / (ny * d)
+    I = sm.simulate_qgrid(dev(g), (d, d, 2.0), lam, dev(qx), dev(qy)).cpu().numpy()
+    rho = g[0, ..., 0].astype(np.float64) + 1j * g[0, ..., 1].astype(np.float64)
+    ref = np.abs(np.fft.fft2(rho) * d * d * 2.0) ** 2
+    assert_parity(I, ref, what="qgrid fft2")
+
+
+def test_full_size_cfg3_sampled_points(sm):
+    """256^3 droplet on a 512 x 512 uniform q grid, checked at seeded grid points (the oracle takes them one by one)."""
+    w = W.config(2)
+    g = w.grid(0)
+    vox = (w.dx, w.dy, w.dz)
+    qx, qy = _uniform_q(w.lam, w.theta_max_deg, w.npx), _uniform_q(w.lam, w.theta_max_deg, w.npy)
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy().ravel()
+    q, ok = O.qgrid_q(qx, qy, w.lam)
+    c = w.npy // 2 * w.npx + w.npx // 2
+    pix = W.sample_pixels(w.seed + 7, w.npix, 160, always=[int(np.argmax(I)), c, c - 1, c - w.npx])
+    ref = O.simulate_q(g, vox, w.lam, q[pix]) * ok[pix]
+    assert_parity(I[pix], ref, what="qgrid cfg3 full sampled")
+
+
+def test_error_codes(sm):
+    import torch
+    from paper_2202_03411_b200 import binding as B
+    g = dev(W.random_grid(5, 8, 8, 4))
+    q = dev(np.linspace(-0.1, 0.1, 8))
+    with pytest.raises(B.ScatmanError) as e:
+        sm.simulate_qgrid(g, (1.0, 1.0, 1.0), 10.0, q, q, workspace=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == B.WORKSPACE_TOO_SMALL
+    with pytest.raises(B.ScatmanError) as e:
+        sm.simulate_qgrid(g, (1.0, 1.0, 1.0), -1.0, q, q)
+    assert e.value.status == B.INVALID_ARGUMENT
