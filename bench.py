@@ -9,6 +9,7 @@ which north_star quotes its target.  `--impl reference` times the FP64 CPU oracl
 from __future__ import annotations
 
 import argparse
+import ctypes as C
 import json
 import os
 import subprocess
@@ -144,6 +145,9 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid"],
+                    help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
+                         "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -185,7 +189,21 @@ def main():
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    if args.route == "qgrid":
+        kk = 2 * np.pi / w.lam
+        qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
+        qy = torch.from_numpy((np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)).cuda()
+        ws = None
+
     def step():
+        if args.route == "qgrid":
+            nonlocal ws
+            if ws is None:
+                need = C.c_size_t(0)
+                sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(need)))
+                ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+            sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, workspace=ws, out=out, stream=stream)
+            return
         sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
                     workspace=ws, out=out, stream=stream)
 
@@ -222,10 +240,20 @@ def main():
     h_dn = torch.from_numpy(g).pin_memory()
     h_I = torch.empty((batch, w.npy, w.npx), dtype=torch.float32).pin_memory()
     e2e_steps = max(1, min(args.steps, 3))
-    sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+
+    def e2e_step():
+        if args.route == "qgrid":   # no host-buffer C entry point for this route: the copies go through torch
+            d_dn.copy_(h_dn, non_blocking=True)
+            step()
+            h_I.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        else:
+            sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+
+    e2e_step()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+        e2e_step()
     e2e_s = time.perf_counter() - t0
     if dist:
         t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
@@ -240,7 +268,16 @@ def main():
     peaks = load_peaks()
     k_ms = sum(kernel_ms) / len(kernel_ms)
     dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
-    if args.method == 1:
+    if args.route == "qgrid":
+        # two FP32 complex GEMMs per slice on CUDA cores: 8 flop per complex MAC, dense count (vacuum rows are skipped)
+        flop = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12      # FP32 FMA: 148 SMs x 128 lanes x 2 flop x max clock
+        ach = flop / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "sep_stage_x_kernel + sep_stage_yz_kernel", "achieved": ach, "peak": peak,
+                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
+                    "achieved_is": "dense FP32 flop of both GEMM stages / their CUDA-event time; all-vacuum rows are skipped, so "
+                                   "this can exceed what the ALUs executed"}
+    elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
         # One extra, untimed call with the counting flag (same inputs, same schedule).
         sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, workspace=ws, out=out,
@@ -278,6 +315,11 @@ def main():
         t0 = time.perf_counter()
         ref = O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=pix)
         dt = time.perf_counter() - t0
+        if args.route == "qgrid":
+            qg, okg = O.qgrid_q(qx.cpu().numpy(), qy.cpu().numpy(), w.lam)
+            t0 = time.perf_counter()
+            ref = O.simulate_q(g[0], vox, w.lam, qg[pix], quat=None if quat is None else quat[0]) * okg[pix]
+            dt = time.perf_counter() - t0
         got = out[0].flatten()[torch.from_numpy(pix).cuda()].cpu().numpy().astype(np.float64)
         rel = float(np.sqrt(np.sum((got - ref) ** 2) / np.sum(ref ** 2)))
         m = ref > 1e-6 * ref.max()
@@ -288,9 +330,9 @@ def main():
 
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "fp16x3 split (fp32 accumulate)" if args.method == 1 else "f32", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32" if args.route == "qgrid" or args.method != 1 else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "method": {1: "tensor", 2: "simt_sincos"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
