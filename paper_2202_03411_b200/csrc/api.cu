@@ -77,6 +77,7 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
     auto take = [&](size_t bytes) { size_t o2 = off; off = align_up(off + bytes, 1024); return o2; };
     p.off_q = take(sizeof(double) * 3 * (size_t)npix);
     p.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
+    p.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     p.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     p.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     p.off_max = take(sizeof(unsigned) * (size_t)batch);
@@ -235,12 +236,12 @@ int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *g
     cudaStream_t st = (cudaStream_t)cuda_stream;
     // the rotation matrices travel in a small stream-ordered allocation
     double *d_rot = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&d_rot, sizeof(double) * 9 * batch, st);
+    cudaError_t e = cudaMallocAsync((void **)&d_rot, (sizeof(double) * 9 + sizeof(int) * 6) * batch, st);   // matrices + boxes
     if (e != cudaSuccess) return cuda_fail(ctx, e, "orient: cudaMallocAsync");
     Plan p;
     p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.dx = grid->dx; p.dy = grid->dy; p.dz = grid->dz;
     e = upload_rotmats(h_quat, batch, d_rot, st, nullptr);
-    if (e == cudaSuccess) e = launch_orient(d_dn_in, p, d_rot, batch, d_dn_out, st);
+    if (e == cudaSuccess) e = launch_orient(d_dn_in, p, d_rot, batch, d_dn_out, (int *)(d_rot + 9 * batch), st);
     cudaFreeAsync(d_rot, st);
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "orient");
 }
@@ -316,8 +317,8 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
     if (h_quat && !all_identity(h_quat, batch)) {
         double *rm = (double *)(ws + p.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
-        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + p.off_rot), st);
-        ++nl;
+        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + p.off_rot), (int *)(ws + p.off_bbox), st);
+        nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + p.off_rot);
     }
@@ -395,7 +396,7 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
 struct SepPlan {
     Plan p;
     int nzs = 1;
-    size_t off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
+    size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
            off_partial = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int num_sms) {
@@ -408,6 +409,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
     sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
+    sp.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
@@ -453,8 +455,8 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     if (h_quat && !all_identity(h_quat, batch)) {
         double *rm = (double *)(ws + sp.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
-        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), st);
-        ++nl;
+        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), (int *)(ws + sp.off_bbox), st);
+        nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + sp.off_rot);
     }

@@ -40,7 +40,7 @@ struct Plan {
     int t_ncta = 2;               // CTAs per work item: 2 = cta_group::2 pairs (default), 1 = single CTA
     // workspace offsets (bytes)
     size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
-           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, total = 0;
+           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, off_bbox = 0, total = 0;
 };
 
 int simt_zsplit(const Plan &p, int num_sms);
@@ -48,7 +48,7 @@ void tensor_schedule(const Plan &p, int num_workers, int *nchunks, int *nzs);
 
 // ---- kernels launchers (all asynchronous on `st`; return cudaGetLastError()) -------------------
 cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);
-cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out,
+cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
                           cudaStream_t st);
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
                             cudaStream_t st);

@@ -32,10 +32,45 @@ cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q,
 // ------------------------------------------------------------------------------------------------ a0
 // Block 5 / Fig. 6: beam-frame voxel <- trilinear sample of the body-frame grid at
 // r_body = R^T r_beam.  rotmat[b][9] row-major R (body -> beam).  One thread per beam-frame voxel.
+// Bounding box (voxel indices, inclusive) of the non-vacuum voxels of every body-frame grid: bbox[b] = {x0, y0, z0, x1, y1, z1},
+// initialised by the launcher to {INT_MAX x3, -1 x3}.  One block per (b, z) slice.  The resampling below gathers 8 corners
+// along a slanted line (its cost is cache wavefronts, not bytes); beam-frame voxels that land outside this box are vacuum
+// without looking.
+__global__ void bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox) {
+    const int iz = blockIdx.x % nz, b = blockIdx.x / nz;
+    const float2 *src = in + ((size_t)b * nz + iz) * (size_t)nx * ny;
+    int x0 = 0x7fffffff, y0 = 0x7fffffff, x1 = -1, y1 = -1;
+    for (int e = threadIdx.x; e < nx * ny; e += blockDim.x) {
+        const float2 v = __ldg(src + e);
+        if (v.x != 0.f || v.y != 0.f) {
+            const int x = e % nx, y = e / nx;
+            x0 = min(x0, x); x1 = max(x1, x);
+            y0 = min(y0, y); y1 = max(y1, y);
+        }
+    }
+    for (int off = 16; off > 0; off >>= 1) {
+        x0 = min(x0, __shfl_xor_sync(0xffffffffu, x0, off));
+        y0 = min(y0, __shfl_xor_sync(0xffffffffu, y0, off));
+        x1 = max(x1, __shfl_xor_sync(0xffffffffu, x1, off));
+        y1 = max(y1, __shfl_xor_sync(0xffffffffu, y1, off));
+    }
+    if ((threadIdx.x & 31) == 0 && x1 >= 0) {
+        int *o = bbox + 6 * b;
+        atomicMin(o + 0, x0); atomicMin(o + 1, y0); atomicMin(o + 2, iz);
+        atomicMax(o + 3, x1); atomicMax(o + 4, y1); atomicMax(o + 5, iz);
+    }
+}
+
+__global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) bbox[i] = (i % 6) < 3 ? 0x7fffffff : -1;
+}
+
 // Threads are grouped as 16 x 4 x 4 output voxels per block so that the 2x2x2 source cells of a block share cache lines
 // for any rotation (row-shaped blocks gather along a slanted line and read 30x more sectors than they use).
 __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz,
-                              double3 inv, const double *__restrict__ rotmat, float2 *__restrict__ out) {
+                              double3 inv, const double *__restrict__ rotmat, const int *__restrict__ bbox,
+                              float2 *__restrict__ out) {
     const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
     int blk = blockIdx.x;
     const int bx = blk % nbx; blk /= nbx;
@@ -56,8 +91,10 @@ __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int
     {
         const double fx = fma((double)ix, sx, fx0), fy = fma((double)ix, sy, fy0), fz = fma((double)ix, sz, fz0);
         float2 o = make_float2(0.f, 0.f);
-        // the 2x2x2 cell touches the grid only if every coordinate lies in (-1, n)
-        if (fx > -1.0 && fx < (double)nx && fy > -1.0 && fy < (double)ny && fz > -1.0 && fz < (double)nz) {
+        // the 2x2x2 cell holds material only if every coordinate lies within one voxel of the box of non-vacuum voxels
+        const int *bb = bbox + 6 * b;
+        if (fx > (double)(bb[0] - 1) && fx < (double)(bb[3] + 1) && fy > (double)(bb[1] - 1) && fy < (double)(bb[4] + 1) &&
+            fz > (double)(bb[2] - 1) && fz < (double)(bb[5] + 1)) {
             const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
             const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
             const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
@@ -91,12 +128,14 @@ __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int
     }
 }
 
-cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out,
+cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
                           cudaStream_t st) {
     const size_t blocks = (size_t)((p.nx + 15) / 16) * ((p.ny + 3) / 4) * ((p.nz + 3) / 4) * batch;
-    if (blocks > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    if (blocks > 0x7fffffffull || (size_t)p.nz * batch > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    bbox_init_kernel<<<(6 * batch + 255) / 256, 256, 0, st>>>(d_bbox, 6 * batch);
+    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox);
     orient_kernel<<<(unsigned)blocks, 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
-                                                   make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat,
+                                                   make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
                                                    (float2 *)d_out);
     return cudaGetLastError();
 }
