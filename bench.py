@@ -145,9 +145,10 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid"],
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
-                         "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid)")
+                         "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
+                         "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -193,15 +194,25 @@ def main():
         kk = 2 * np.pi / w.lam
         qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
         qy = torch.from_numpy((np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)).cuda()
-        ws = None
+        need = C.c_size_t(0)
+        sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(need)))
+        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+
+    shapes = None
+    if args.route == "shapes":
+        shapes = w.shapes(items)
+        if shapes is None:
+            raise SystemExit(f"{w.name} is not one shape per item: --route shapes does not apply")
+        need = C.c_size_t(0)
+        sm._check(sm.lib.scatman_shapes_workspace_bytes(sm._ctx, C.byref(grid), w.npix, batch, C.byref(opts), C.byref(need)))
+        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
 
     def step():
+        if args.route == "shapes":
+            sm.simulate_shapes(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method,
+                               workspace=ws, out=out, stream=stream)
+            return
         if args.route == "qgrid":
-            nonlocal ws
-            if ws is None:
-                need = C.c_size_t(0)
-                sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(need)))
-                ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
             sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, workspace=ws, out=out, stream=stream)
             return
         sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
@@ -242,7 +253,11 @@ def main():
     e2e_steps = max(1, min(args.steps, 3))
 
     def e2e_step():
-        if args.route == "qgrid":   # no host-buffer C entry point for this route: the copies go through torch
+        if args.route == "shapes":  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
+            step()
+            h_I.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        elif args.route == "qgrid":   # no host-buffer C entry point for this route: the copies go through torch
             d_dn.copy_(h_dn, non_blocking=True)
             step()
             h_I.copy_(out, non_blocking=True)
@@ -280,8 +295,12 @@ def main():
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
         # One extra, untimed call with the counting flag (same inputs, same schedule).
-        sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, workspace=ws, out=out,
-                    stream=stream, flags=B.FLAG_COUNT_ISSUED)
+        if args.route == "shapes":
+            sm.simulate_shapes(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method,
+                               workspace=ws, out=out, stream=stream, flags=B.FLAG_COUNT_ISSUED)
+        else:
+            sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, workspace=ws, out=out,
+                        stream=stream, flags=B.FLAG_COUNT_ISSUED)
         blocks = sm.last_issued_blocks()
         npix_pad = (w.npix + 255) // 256 * 256
         issued = blocks * 256 * npix_pad * SPLITS * FLOP_PER_TERM         # tensor flop per contraction launch
@@ -306,19 +325,23 @@ def main():
         from oracle import oracle as O
         from paper_2202_03411_b200 import workloads as W
         # size the sample for ~15 s of host-core work from a short probe
+        g0, q0 = g[0], (None if quat is None else quat[0])
+        if args.route == "shapes":     # the oracle's own rendering of item 0 (already in the beam frame)
+            from oracle import render as OR
+            g0, q0 = OR.render(shapes[0], (w.nx, w.ny, w.nz), vox), None
         probe = W.sample_pixels(w.seed + 99, w.npix, 32)
         t0 = time.perf_counter()
-        O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=probe)
+        O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=probe)
         per_pixel = (time.perf_counter() - t0) / len(probe)
         npix_s = args.ref_pixels if args.ref_pixels > 0 else int(min(8192, max(256, 15.0 / per_pixel)))
         pix = W.sample_pixels(w.seed, w.npix, npix_s)
         t0 = time.perf_counter()
-        ref = O.simulate(g[0], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[0], pixels=pix)
+        ref = O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=pix)
         dt = time.perf_counter() - t0
         if args.route == "qgrid":
             qg, okg = O.qgrid_q(qx.cpu().numpy(), qy.cpu().numpy(), w.lam)
             t0 = time.perf_counter()
-            ref = O.simulate_q(g[0], vox, w.lam, qg[pix], quat=None if quat is None else quat[0]) * okg[pix]
+            ref = O.simulate_q(g0, vox, w.lam, qg[pix], quat=q0) * okg[pix]
             dt = time.perf_counter() - t0
         got = out[0].flatten()[torch.from_numpy(pix).cuda()].cpu().numpy().astype(np.float64)
         rel = float(np.sqrt(np.sum((got - ref) ** 2) / np.sum(ref ** 2)))
@@ -332,11 +355,12 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if args.route == "qgrid" or args.method != 1 else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
-                    "h2d_bytes_per_step": int(h_dn.numel() * 4), "d2h_bytes_per_step": int(h_I.numel() * 4)},
+                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route != "shapes" else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
+                    "d2h_bytes_per_step": int(h_I.numel() * 4)},
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line), flush=True)
 

@@ -203,6 +203,15 @@ typedef struct {
 int scatman_render(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
                    float *d_dn, void *cuda_stream);
 
+/* Shapes in, patterns out (north_star (5), forward fitting: the candidates of an optimiser step are shape parameters, not
+ * voxel grids): scatman_render into the workspace, then the whole path a1-a6 on the rendered (already oriented) grids.
+ * Only the descriptors cross the host-device boundary.  d_I[batch][npy][npx].  Workspace: scatman_shapes_workspace_bytes. */
+int scatman_shapes_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int64_t npix, int32_t batch,
+                                   const scatman_options *opts, size_t *bytes);
+int scatman_simulate_shapes(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
+                            double lambda, const scatman_detector *det, const scatman_options *opts, void *d_ws,
+                            size_t ws_bytes, float *d_I, void *cuda_stream);
+
 /* With SCATMAN_FLAG_COUNT_ISSUED: the number of 16-y x 16-x blocks of rho~ (256 voxels each) the contraction of the last
  * scatman_simulate* call multiplied against EVERY pixel, summed over slices and batch items; the dense count is
  * batch * nz * ceil(ny/16) * ceil(nx/16) blocks of the padded grid.  Issued tensor flop = blocks * 256 * npix_pad * 24.

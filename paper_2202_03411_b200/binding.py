@@ -23,7 +23,7 @@ FLAG_COUNT_ISSUED = 2
 EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
-    "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid",
+    "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
     "scatman_render", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
@@ -89,6 +89,9 @@ def load_library() -> C.CDLL:
     L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(C.c_size_t)]
     L.scatman_simulate_qgrid.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i32, vp, i32, C.POINTER(dbl), i32,
                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
+    L.scatman_shapes_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i64, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
+    L.scatman_simulate_shapes.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), dbl, C.POINTER(Detector),
+                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -202,17 +205,12 @@ class Scatman:
                                                         self._stream(stream)))
         return out
 
-    def render(self, shapes: Sequence[dict], dims, voxel, out=None, stream=None):
-        """(delta, beta) grids float32 [B][nz][ny][nx][2] of shape descriptors (dicts with the keys of include/scatman.h's
-        scatman_shape: kind, delta, beta, quat, and a/b/c | coeffs [(l, m, c)] | radii (CUDA float64 [nlat][nlon]) |
-        volume (CUDA uint8 [nvz][nvy][nvx]) + dx).  Marshalling only: the shapes are evaluated by render_kernel."""
+    @staticmethod
+    def _shape_array(shapes: Sequence[dict]):
+        """ctypes array of scatman_shape from descriptor dicts (+ the objects that must outlive the call)."""
         import numpy as np
         import torch
-        nx, ny, nz = (int(v) for v in dims)
-        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
         batch = len(shapes)
-        if out is None:
-            out = torch.empty((batch, nz, ny, nx, 2), dtype=torch.float32, device=f"cuda:{self.device}")
         arr = (Shape * batch)()
         keep = []
         kinds = {"ellipsoid": SHAPE_ELLIPSOID, "spherical_harmonics": SHAPE_SPHERICAL_HARMONICS,
@@ -241,6 +239,20 @@ class Scatman:
                     raise ValueError("volume must be a contiguous CUDA uint8 tensor [nvz][nvy][nvx]")
                 keep.append(v)
                 s.nvz, s.nvy, s.nvx, s.d_volume, s.vdx = int(v.shape[0]), int(v.shape[1]), int(v.shape[2]), v.data_ptr(), float(sh["dx"])
+        return arr, keep
+
+    def render(self, shapes: Sequence[dict], dims, voxel, out=None, stream=None):
+        """(delta, beta) grids float32 [B][nz][ny][nx][2] of shape descriptors (dicts with the keys of include/scatman.h's
+        scatman_shape: kind, delta, beta, quat, and a/b/c | coeffs [(l, m, c)] | radii (CUDA float64 [nlat][nlon]) |
+        volume (CUDA uint8 [nvz][nvy][nvx]) + dx).  Marshalling only: the shapes are evaluated by render_kernel."""
+        import numpy as np
+        import torch
+        nx, ny, nz = (int(v) for v in dims)
+        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+        batch = len(shapes)
+        if out is None:
+            out = torch.empty((batch, nz, ny, nx, 2), dtype=torch.float32, device=f"cuda:{self.device}")
+        arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_render(self._ctx, arr, batch, C.byref(grid), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
@@ -285,6 +297,29 @@ class Scatman:
                                                 C.c_void_p(workspace.data_ptr()), workspace.numel(),
                                                 C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out if dn.dim() == 5 else out[0]
+
+    def simulate_shapes(self, shapes: Sequence[dict], dims, voxel, lam: float, npx: int, npy: int, theta_max_deg: float,
+                        rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, workspace=None, out=None, stream=None,
+                        flags: int = 0):
+        """Shape descriptors (see render) -> I float32 [B][npy][npx]: rendered and simulated on the device."""
+        import torch
+        nx, ny, nz = (int(v) for v in dims)
+        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+        batch = len(shapes)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_shapes_workspace_bytes(self._ctx, C.byref(grid), npx * npy, batch, C.byref(opts), C.byref(need)))
+        dev = f"cuda:{self.device}"
+        if workspace is None:
+            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dev)
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dev)
+        arr, keep = self._shape_array(shapes)
+        self._check(self.lib.scatman_simulate_shapes(self._ctx, arr, batch, C.byref(grid), float(lam), C.byref(det), C.byref(opts),
+                                                     C.c_void_p(workspace.data_ptr()), workspace.numel(),
+                                                     C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out
 
     def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, workspace=None, out=None,
                        stream=None):

@@ -392,6 +392,33 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
                     (cudaStream_t)cuda_stream);
 }
 
+int scatman_shapes_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int64_t npix, int32_t batch,
+                                   const scatman_options *opts, size_t *bytes) {
+    size_t inner = 0;
+    const int rc = scatman_workspace_bytes(ctx, grid, npix, batch, opts, &inner);
+    if (rc != SCATMAN_OK) return rc;
+    *bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024) + inner;
+    return SCATMAN_OK;
+}
+
+int scatman_simulate_shapes(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
+                            double lambda, const scatman_detector *det, const scatman_options *opts, void *d_ws,
+                            size_t ws_bytes, float *d_I, void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!h_shapes || !d_ws || !valid_grid(grid) || batch < 1 || !det || !valid_detector(det))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    const size_t dn_bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024);
+    if (ws_bytes < dn_bytes) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    float *d_dn = (float *)d_ws;
+    int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
+    if (rc != SCATMAN_OK) return rc;
+    const int rendered = ctx->last_launches;
+    rc = run_path(ctx, d_dn, grid, lambda, det, nullptr, (int64_t)det->npx * det->npy, nullptr, batch, opts,
+                  (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes, d_I, (cudaStream_t)cuda_stream);
+    if (rc == SCATMAN_OK) ctx->last_launches += rendered;
+    return rc;
+}
+
 // ---- separable route: workspace layout -------------------------------------------------------------------------
 struct SepPlan {
     Plan p;

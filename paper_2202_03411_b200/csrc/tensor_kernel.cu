@@ -332,10 +332,12 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     for (int yi = 0; yi < 4 * nybg; ++yi) {
                         if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // empty 16-y step: never loaded
                         if ((kidx & 1) == iw) {
+#ifndef SCATMAN_ABL_NOFIRST
                             if (kidx == 1) {   // issuer 1's first k-step of the unit: D must have been initialised
                                 ptx::mbar_wait(first_done + buf, upar);
                                 ptx::tc_fence_after();
                             }
+#endif
                             TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                             ptx::tc_fence_after();
                             if (ptx::elect_one()) {

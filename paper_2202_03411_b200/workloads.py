@@ -39,6 +39,7 @@ class Workload:
     quat: Optional[np.ndarray]   # [batch][4] (w,x,y,z) float64 or None = identity
     seed: int
     _gen: object = None          # callable(b) -> float32 [nz][ny][nx][2]
+    _shape: object = None        # callable(b) -> shape descriptor dict (scatman_shape fields) or None if not a single shape
 
     @property
     def nvox(self) -> int:
@@ -55,6 +56,20 @@ class Workload:
     def grid(self, b: int = 0) -> np.ndarray:
         """Body-frame (delta, beta) grid of batch item b, float32 [nz][ny][nx][2]."""
         return self._gen(b)
+
+    def shapes(self, items=None):
+        """Shape descriptors (the fields of scatman_shape, orientation included) of the items: the same particles as grid(b),
+        for rendering on the device.  None for workloads that are not one shape per item (cfg5)."""
+        if self._shape is None:
+            return None
+        items = range(self.batch) if items is None else items
+        out = []
+        for b in items:
+            d = dict(self._shape(b))
+            if self.quat is not None:
+                d["quat"] = [float(v) for v in self.quat[b]]
+            out.append(d)
+        return out
 
     def grids(self, items=None) -> np.ndarray:
         items = range(self.batch) if items is None else items
@@ -191,6 +206,11 @@ def _sh_coeffs(rng: np.random.Generator, lmax: int, sigma0: float = 0.05):
     return out
 
 
+def _triplets(r0: float, coeffs):
+    """R0 (1 + sum a_lm Y_lm) as the paper's triplet list (l, m, c) with R = sum c Y_lm: c_00 = R0 sqrt(4 pi), c_lm = R0 a_lm."""
+    return [(0, 0, r0 * float(np.sqrt(4.0 * np.pi)))] + [(l, m, r0 * a) for (l, m, a) in coeffs]
+
+
 def config(index: int, scale: float = 1.0) -> Workload:
     """Workload for BASELINE.json configs[index] (0..4).
 
@@ -207,19 +227,22 @@ def config(index: int, scale: float = 1.0) -> Workload:
         n, npx = sc(32), sc(64)
         d = 4.0 * 32 / n
         gen = lambda b: _fill(ellipsoid_mask(n, n, n, d, d, d, 60.0, 60.0, 60.0), 0.01, 0.001)
-        return Workload("cfg1_sphere_32", 0, n, n, n, d, d, d, 20.0, npx, npx, 30.0, 1, None, seed, gen)
+        shp = lambda b: {"kind": "ellipsoid", "delta": 0.01, "beta": 0.001, "a": 60.0, "b": 60.0, "c": 60.0}
+        return Workload("cfg1_sphere_32", 0, n, n, n, d, d, d, 20.0, npx, npx, 30.0, 1, None, seed, gen, shp)
     if index == 1:
         n, npx = sc(128), sc(256)
         d = 4.0 * 128 / n
         quat = random_quaternions(rng, 1)
         gen = lambda b: _fill(ellipsoid_mask(n, n, n, d, d, d, 200.0, 150.0, 120.0), 0.02, 0.005)
-        return Workload("cfg2_ellipsoid_128", 1, n, n, n, d, d, d, 13.5, npx, npx, 40.0, 1, quat, seed, gen)
+        shp = lambda b: {"kind": "ellipsoid", "delta": 0.02, "beta": 0.005, "a": 200.0, "b": 150.0, "c": 120.0}
+        return Workload("cfg2_ellipsoid_128", 1, n, n, n, d, d, d, 13.5, npx, npx, 40.0, 1, quat, seed, gen, shp)
     if index == 2:
         n, npx = sc(256), sc(512)
         d = 4.0 * 256 / n
         coeffs = _sh_coeffs(rng, 6)
         gen = lambda b: _fill(droplet_mask(n, n, n, d, d, d, 400.0, coeffs), 0.03, 0.01)
-        return Workload("cfg3_droplet_256", 2, n, n, n, d, d, d, 30.0, npx, npx, 45.0, 1, None, seed, gen)
+        shp = lambda b: {"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.01, "coeffs": _triplets(400.0, coeffs)}
+        return Workload("cfg3_droplet_256", 2, n, n, n, d, d, d, 30.0, npx, npx, 45.0, 1, None, seed, gen, shp)
     if index == 3:
         n, npx = sc(128), sc(256)
         d = 6.0 * 128 / n
@@ -238,7 +261,14 @@ def config(index: int, scale: float = 1.0) -> Workload:
                 co = _sh_coeffs(np.random.default_rng(int(sh_seeds[b])), 4)
                 m = droplet_mask(n, n, n, d, d, d, r0[b], co)
             return _fill(m, delta[b], beta[b])
-        return Workload("cfg4_fit_batch_256x128", 3, n, n, n, d, d, d, 20.0, npx, npx, 35.0, batch, quat, seed, gen)
+
+        def shp(b):
+            if b % 2 == 0:
+                return {"kind": "ellipsoid", "delta": float(delta[b]), "beta": float(beta[b]), "a": float(r0[b]),
+                        "b": float(r0[b] * ratios[b, 0]), "c": float(r0[b] * ratios[b, 1])}
+            co = _sh_coeffs(np.random.default_rng(int(sh_seeds[b])), 4)
+            return {"kind": "spherical_harmonics", "delta": float(delta[b]), "beta": float(beta[b]), "coeffs": _triplets(float(r0[b]), co)}
+        return Workload("cfg4_fit_batch_256x128", 3, n, n, n, d, d, d, 20.0, npx, npx, 35.0, batch, quat, seed, gen, shp)
     if index == 4:
         n, npx = sc(512), sc(1024)
         d = 2.0 * 512 / n

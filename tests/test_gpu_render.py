@@ -140,3 +140,32 @@ def test_render_error_codes(sm):
         with pytest.raises(B.ScatmanError) as e:
             sm.render([s], dims, voxel)
         assert e.value.status == B.INVALID_ARGUMENT
+
+
+def test_simulate_shapes_equals_render_then_simulate_and_matches_oracle(sm):
+    """scatman_simulate_shapes = scatman_render + scatman_simulate on the rendered grids (bit for bit), and the result matches
+    the oracle run on the oracle's own rendering (cfg4 shapes at quarter scale: ellipsoids and l <= 4 droplets, oriented)."""
+    import torch
+    w = W.config(3, scale=0.25)
+    items = [0, 1, 2, 3, 4, 5]
+    shapes = w.shapes(items)
+    dims, vox = (w.nx, w.ny, w.nz), (w.dx, w.dy, w.dz)
+    I = sm.simulate_shapes(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+    g = sm.render(shapes, dims, vox)
+    I2 = sm.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+    assert torch.equal(I, I2)
+    I = I.cpu().numpy()
+    for i, s in enumerate(shapes):
+        ref_grid = R.render(s, dims, vox)
+        assert np.mean(np.any(g[i].cpu().numpy() != ref_grid, axis=-1)) < 1e-4
+        ref = O.simulate(g[i].cpu().numpy(), vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+        assert_parity(I[i], ref, what=f"shapes item {items[i]}")
+
+
+def test_workload_shape_descriptors_describe_the_same_particles_as_the_grids(sm):
+    """The descriptors of cfg1 / cfg3 (identity orientation) render to exactly the voxel grids the generators produce."""
+    for idx, scale in ((0, 1.0), (2, 0.25)):
+        w = W.config(idx, scale=scale)
+        got = sm.render(w.shapes([0]), (w.nx, w.ny, w.nz), (w.dx, w.dy, w.dz)).cpu().numpy()[0]
+        ref = w.grid(0)
+        assert np.mean(np.any(got != ref, axis=-1)) < 1e-5, idx
