@@ -35,6 +35,7 @@ def test_version_and_status_strings(lib):
 def test_struct_layout_matches_header():
     from paper_2202_03411_b200 import binding as B
     assert C.sizeof(B.Grid) == 40 and C.sizeof(B.Detector) == 32 and C.sizeof(B.Options) == 16
+    assert C.sizeof(B.Shape) == 136 and B.Shape.quat.offset == 16 and B.Shape.h_coef.offset == 80 and B.Shape.vdx.offset == 128
 
 
 def test_no_device_fails_loudly(lib):
