@@ -167,6 +167,38 @@ def test_empty_and_single_voxel(sm):
         assert np.allclose(I, exact, rtol=2e-5)
 
 
+def test_large_batch_with_vacuum_items_and_many_orientations(sm):
+    """40 small grids in one call (more than one 32-matrix upload chunk), random orientations, some items all vacuum, some
+    identity: every item's pattern is its own (no cross-talk through the batch loop, the per-item scales or the partial sums)."""
+    rng = np.random.default_rng(17)
+    B, n = 40, 24
+    g = np.stack([W.sparse_blobs_grid(300 + i, n + 8, n, n - 4, nblobs=3, max_extent=10) for i in range(B)])
+    g[[3, 17, 39]] = 0.0
+    g[5] *= 1e-3                                  # a much weaker item: its FP16 scale differs by 2^10 from its neighbours'
+    quat = W.random_quaternions(rng, B)
+    quat[[0, 9]] = [1, 0, 0, 0]
+    voxel, lam = (3.0, 3.0, 3.0), 16.0
+    npx, npy, th = 12, 10, 30.0
+    for name in ("tensor", "tensor_1cta"):
+        I = sm.simulate(dev(g), voxel, lam, npx, npy, th, quat=quat, method=METHODS[name][0], flags=METHODS[name][1]).cpu().numpy()
+        assert np.all(I[[3, 17, 39]] == 0)
+        for b in range(B):
+            if b in (3, 17, 39):
+                continue
+            ref = O.simulate(g[b], voxel, lam, npx, npy, th, quat=quat[b])
+            assert_parity(I[b], ref, what=f"batch40 {name} b={b}")
+
+
+def test_n2m1_mode_on_an_absorbing_inhomogeneous_grid(sm):
+    """rho = n^2 - 1 (paper, Eq. 5/9) against the oracle on a grid where it is not proportional to n - 1."""
+    g = W.random_grid(77, 64, 48, 20, fill=0.7, delta=(-0.05, 0.3), beta=(0.0, 0.2))
+    voxel, lam = (2.0, 2.0, 2.0), 9.0
+    I1 = sm.simulate(dev(g), voxel, lam, 24, 24, 40.0, rho_mode=1).cpu().numpy()
+    I0 = sm.simulate(dev(g), voxel, lam, 24, 24, 40.0, rho_mode=0).cpu().numpy()
+    assert_parity(I1, O.simulate(g, voxel, lam, 24, 24, 40.0, rho_mode=1), what="n2m1")
+    assert np.max(np.abs(I1 / I0 - 4.0)) > 0.3          # far from the homogeneous-particle constant |2 - dn|^2 ~ 4
+
+
 def test_issued_block_count(sm):
     """scatman_last_issued_blocks: what the contraction multiplies after skipping empty 16-y steps and narrowing units
     to their occupied 16-x blocks, on grids where the count is known by hand."""
