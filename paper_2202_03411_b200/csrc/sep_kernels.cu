@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(256) sep_stage_x_kernel(const float2 *__restri
 
 // stage YZ: partial[zs][b * npx + a] = sum over this z range of e^{i qz z_j} sum_y Ey[b][y] H[j][y][a].
 // qz in turns per unit length: qzt = qz / 2pi, so the phase of slice j is sincospi(2 frac(qzt z_j)) with the reduction in FP64.
-__global__ void __launch_bounds__(256) sep_stage_yz_kernel(const float2 *__restrict__ Ey, const float2 *__restrict__ H,
+__global__ void __launch_bounds__(256, 2) sep_stage_yz_kernel(const float2 *__restrict__ Ey, const float2 *__restrict__ H,
                                                            const double *__restrict__ qx, const double *__restrict__ qy,
                                                            double k, int npx, int npy, int ny, int nz, double dz, int nzs,
                                                            const unsigned char *__restrict__ flags, int nyc,
@@ -158,7 +158,9 @@ __global__ void __launch_bounds__(256) sep_stage_yz_kernel(const float2 *__restr
     const int m0 = blockIdx.y * kBM, n0 = blockIdx.x * kBN, zs = blockIdx.z;
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int z0 = (int)(((long long)nz * zs) / nzs), z1 = (int)(((long long)nz * (zs + 1)) / nzs);
-    double qzt[4][4];
+    // qz of this thread's 4 x 4 outputs, in turns per unit length, parked in shared memory (32 FP64 registers otherwise)
+    extern __shared__ double s_qzt_raw[];
+    double (*s_qzt)[256] = (double (*)[256])s_qzt_raw;   // [16][256], dynamic: 32 KB
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -171,7 +173,7 @@ __global__ void __launch_bounds__(256) sep_stage_yz_kernel(const float2 *__restr
                 // qz = -(k - sqrt(k^2 - qxy^2)) = -qxy^2 / (k + sqrt(k^2 - qxy^2)): no cancellation near forward
                 v = kz2 >= 0.0 ? -qxy2 / (k + sqrt(kz2)) : 0.0;
             }
-            qzt[i][j] = v * (0.5 / 3.14159265358979323846);
+            s_qzt[i * 4 + j][tid] = v * (0.5 / 3.14159265358979323846);
         }
     float2 tot[4][4];
 #pragma unroll
@@ -190,7 +192,7 @@ __global__ void __launch_bounds__(256) sep_stage_yz_kernel(const float2 *__restr
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                double t = qzt[i][j] * zj;
+                double t = s_qzt[i * 4 + j][tid] * zj;
                 t -= rint(t);
                 float s, c;
                 sincospif(2.0f * (float)t, &s, &c);
@@ -255,7 +257,13 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
     dim3 gx((M + kBM - 1) / kBM, (npx + kBN - 1) / kBN);
     sep_stage_x_kernel<<<gx, 256, 0, st>>>(d_rho, d_Ex, M, p.nx, npx, d_H);
     dim3 gy((npx + kBN - 1) / kBN, (npy + kBM - 1) / kBM, nzs);
-    sep_stage_yz_kernel<<<gy, 256, 0, st>>>(d_Ey, d_H, d_qx, d_qy, k, npx, npy, p.ny, p.nz, p.dz, nzs, d_flags, nyc,
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t ea = cudaFuncSetAttribute(sep_stage_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * 8);
+        if (ea != cudaSuccess) return ea;
+        attr_set = true;
+    }
+    sep_stage_yz_kernel<<<gy, 256, 16 * 256 * 8, st>>>(d_Ey, d_H, d_qx, d_qy, k, npx, npy, p.ny, p.nz, p.dz, nzs, d_flags, nyc,
                                             d_partial);
     const int64_t npix = (int64_t)npx * npy;
     sep_finalize_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(d_partial, d_qx, d_qy, k, npx, npy, nzs,
