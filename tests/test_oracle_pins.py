@@ -324,3 +324,17 @@ def test_qgrid_single_slice_on_the_dft_grid_is_numpy_fft2():
     rho = g[0, ..., 0].astype(np.float64) + 1j * g[0, ..., 1].astype(np.float64)
     ref = np.abs(np.fft.fft2(rho) * d * d * 2.0) ** 2
     assert np.allclose(I, ref, rtol=1e-11)
+
+
+def test_oracle_matches_its_stored_values():
+    """tests/golden/cfg1_oracle_pixels.txt (written by tests/golden/make_golden.py, which calls only oracle/): the oracle as it
+    stands reproduces its stored intensities on config 1; an unintended change of its arithmetic fails here."""
+    import os
+    from paper_2202_03411_b200 import workloads as W
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg1_oracle_pixels.txt")
+    rows = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    pix = np.array([int(r[0]) for r in rows], dtype=np.int64)
+    want = np.array([float(r[1]) for r in rows])
+    w = W.config(0)
+    got = O.simulate(w.grid(0), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, pixels=pix)
+    assert np.allclose(got, want, rtol=1e-12, atol=0)

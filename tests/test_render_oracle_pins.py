@@ -88,12 +88,21 @@ def test_orientation_convention_matches_a0_on_quarter_turns():
     assert np.array_equal(got, swapped)
 
 
+def _golden(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    return [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+
+
 def test_radial_map_paper_example_sample_positions():
-    """a 4 x 4 array gives the radii at theta = -pi/2, -pi/4, 0, pi/4 and phi = 0, pi/2, pi, 3pi/2."""
+    """PAPER.md:419 (tests/golden/radial_map_example.txt): a 4 x 4 array gives the radii at theta = -pi/2, -pi/4, 0, pi/4 and
+    phi = 0, pi/2, pi, 3pi/2."""
     rng = np.random.default_rng(4)
     radii = rng.uniform(5.0, 9.0, (4, 4))
-    lats = np.array([-pi / 2, -pi / 4, 0.0, pi / 4])
-    lons = np.array([0.0, pi / 2, pi, 3 * pi / 2])
+    rows = {r[0]: r for r in _golden("radial_map_example.txt")}
+    assert int(rows["theta"][1]) == 4 and int(rows["phi"][1]) == 4
+    lats = np.array([float(v) for v in rows["theta"][2:]]) * pi
+    lons = np.array([float(v) for v in rows["phi"][2:]]) * pi
     L, M = np.meshgrid(lats, lons, indexing="ij")
     assert np.allclose(R.radial_map_radius(radii, L, M), radii, rtol=0, atol=1e-14)
     # linear in between, periodic in longitude, held above the last latitude sample
@@ -118,9 +127,12 @@ def test_radial_map_constant_is_a_sphere_and_analytic_profile():
 
 
 def test_volume_map_paper_example_cube():
-    """a 10^3 all-True array with dx = 2 is a 20 x 20 x 20 cube; dx = 4 doubles it."""
+    """PAPER.md:423 (tests/golden/volume_map_example.txt): a 10^3 all-True array with dx = 2 is a 20 x 20 x 20 cube; dx = 4 doubles it."""
+    cases = [(int(r[0]), float(r[1]), float(r[2])) for r in _golden("volume_map_example.txt")]
+    assert cases == [(10, 2.0, 20.0), (10, 4.0, 40.0)]
     vol = np.ones((10, 10, 10), dtype=bool)
-    for dx, side, n in ((2.0, 20, 32), (4.0, 40, 48)):
+    for (cells, dx, side_nm), n in zip(cases, (32, 48)):
+        side = int(side_nm)                     # rendered on 1 nm voxels
         g = R.render({"kind": "volume_map", "delta": 1.0, "beta": 0.5, "volume": vol, "dx": dx}, (n, n, n), (1.0, 1.0, 1.0))
         assert int(g[..., 0].sum()) == side ** 3
         idx = np.nonzero(g[..., 0])
