@@ -142,7 +142,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: 256^3 / 512x512)")
     ap.add_argument("--batch", type=int, default=0, help="limit the batch of config 3 (0 = all)")
-    ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos")
+    ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes"],
@@ -313,6 +313,12 @@ def main():
                     "issued_fraction_of_dense": issued / dense, "dense_equivalent_tflops": dense / (k_ms * 1e-3) / 1e12,
                     "useful_dense_tflops": dense / SPLITS / (k_ms * 1e-3) / 1e12, "kernel_ms": k_ms,
                     "kernel_share_of_step": k_ms * args.steps / total_ms}
+    elif args.method == 3:
+        # FP32 FMA against phase tables: 8 flop per term (dense count; vacuum y chunks are skipped); FP32 peak as for qgrid
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        ach = FLOP_PER_TERM * terms_per_pattern * batch / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "simt_table_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ach / peak, "traffic": None, "kernel_ms": k_ms}
     else:
         # direct sincos: 2 MUFU per term; SFU peak = 148 SMs x 16 MUFU/clk x max clock
         peak = 148 * 16 * 1.965e9 / 2 / 1e12
@@ -355,7 +361,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if args.route == "qgrid" or args.method != 1 else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",

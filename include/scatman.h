@@ -71,7 +71,7 @@ enum { SCATMAN_RHO_LINEAR = 0, /* f(c) = c        : north_star's contrast dn = d
 enum { SCATMAN_METHOD_AUTO = 0,        /* = TENSOR */
        SCATMAN_METHOD_TENSOR = 1,      /* tcgen05 split-precision contraction + fused epilogue */
        SCATMAN_METHOD_SIMT_SINCOS = 2, /* CUDA-core variant: one sincos of the full phase per term */
-       SCATMAN_METHOD_SIMT_TABLE = 3 };/* CUDA-core variant: FP32 FMA against 1-D phase tables */
+       SCATMAN_METHOD_SIMT_TABLE = 3 };/* CUDA-core variant: FP32 FMA GEMM per slice against per-pixel phase tables */
 
 enum { SCATMAN_PRECISION_AUTO = 0,     /* = FP16X3 */
        SCATMAN_PRECISION_FP16X3 = 1 }; /* A = Ah + Al, B = Bh + Bl in FP16; AhBh + AlBh + AhBl, FP32 accumulate */

@@ -92,6 +92,12 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
         p.off_mask = take(sizeof(unsigned long long) * (size_t)batch * p.nz * p.nxt * p.ngroups);
         p.off_count = take(sizeof(unsigned long long));
     }
+    if (p.method == SCATMAN_METHOD_SIMT_TABLE) {
+        p.off_tab_y = take(sizeof(float2) * (size_t)npix * g.ny);
+        p.off_tab_x = take(sizeof(float2) * (size_t)npix * g.nx);
+        p.off_tab_z = take(sizeof(float2) * (size_t)npix * g.nz);
+        p.off_flags = take((size_t)batch * g.nz * ((g.ny + 15) / 16));
+    }
     p.total = off;
     return p;
 }
@@ -297,7 +303,6 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
     cudaSetDevice(ctx->device);
     const Plan p = make_plan(*grid, lambda, npix, batch, o, ctx->num_sms);
-    if (p.method == SCATMAN_METHOD_SIMT_TABLE) return fail(ctx, SCATMAN_NOT_IMPLEMENTED, "SIMT_TABLE is not built yet");
     if (ws_bytes < p.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     uint8_t *ws = (uint8_t *)d_ws;
     int nl = 0;
@@ -358,6 +363,14 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
         if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "contract") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         ctx->ev_valid = true;
         e = launch_finalize(partial, p, ampscale, dV, d_I, st);
+    } else if (p.method == SCATMAN_METHOD_SIMT_TABLE) {
+        cudaEventRecord(ctx->ev0, st);
+        e = launch_simt_table(rho, d_q, p, (float2 *)(ws + p.off_tab_y), (float2 *)(ws + p.off_tab_x), (float2 *)(ws + p.off_tab_z),
+                              ws + p.off_flags, partial, st, &nl);
+        cudaEventRecord(ctx->ev1, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "simt_table");
+        ctx->ev_valid = true;
+        e = launch_finalize(partial, p, nullptr, dV, d_I, st);
     } else {
         cudaEventRecord(ctx->ev0, st);
         e = launch_simt_sincos(rho, d_q, p, partial, st);

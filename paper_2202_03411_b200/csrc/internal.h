@@ -40,7 +40,7 @@ struct Plan {
     int t_ncta = 2;               // CTAs per work item: 2 = cta_group::2 pairs (default), 1 = single CTA
     // workspace offsets (bytes)
     size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
-           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, off_bbox = 0, total = 0;
+           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, off_bbox = 0, off_tab_y = 0, off_tab_x = 0, off_tab_z = 0, off_flags = 0, total = 0;
 };
 
 int simt_zsplit(const Plan &p, int num_sms);
@@ -62,8 +62,8 @@ cudaError_t launch_finalize(const float2 *d_partial, const Plan &p, const float 
                             float *d_I, cudaStream_t st);
 cudaError_t launch_simt_sincos(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
                                cudaStream_t st);
-cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
-                              cudaStream_t st);
+cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_My, float2 *d_Mx, float2 *d_Mz,
+                              unsigned char *d_flags, float2 *d_partial, cudaStream_t st, int *nlaunch);
 
 cudaError_t launch_sep_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p, float2 *d_Ex,
                               float2 *d_Ey, cudaStream_t st);

@@ -230,6 +230,112 @@ __global__ void sep_finalize_kernel(const float2 *__restrict__ partial, const do
     I[p] = real ? re * re + im * im : 0.f;
 }
 
+// ------------------------------------------------------------------------------------------------ SIMT_TABLE (a7)
+// The CUDA-core counterpart of the tensor contraction for the flat detector ("FP32 FMA against 1-D phase
+// tables"): per slice the same G_j[p, x] = sum_y My[p, y] rho~_j[y, x] as an FP32 complex GEMM on 64-pixel x 64-x tiles, the
+// row-dot with Mx[p, x], the slice phase Mz[p, j] and the slice sum in registers.  Tables are per-pixel FP32 roundings of
+// FP64 phases.  Vacuum y chunks are skipped like in the separable route.
+__global__ void pixel_table_kernel(const double *__restrict__ q, int comp, int64_t npix, int n, double d,
+                                   float2 *__restrict__ out) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= npix * n) return;
+    const int64_t p = t / n;
+    const int i = (int)(t % n);
+    double s, c;
+    sincos(q[3 * p + comp] * centre_d(i, n, d), &s, &c);
+    out[t] = make_float2((float)c, (float)s);
+}
+
+__global__ void __launch_bounds__(256) simt_table_kernel(const float2 *__restrict__ My, const float2 *__restrict__ Mx,
+                                                         const float2 *__restrict__ Mz, const float2 *__restrict__ rho,
+                                                         const unsigned char *__restrict__ flags, int64_t npix,
+                                                         int64_t npix_pad, int nx, int ny, int nz, int nyc, int nsplit,
+                                                         float2 *__restrict__ partial) {
+    __shared__ TileSmem sm;
+    const int64_t m0 = (int64_t)blockIdx.x * kBM;
+    const int zs = blockIdx.y, b = blockIdx.z;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int z0 = (int)(((long long)nz * zs) / nsplit), z1 = (int)(((long long)nz * (zs + 1)) / nsplit);
+    const float2 *vol = rho + (size_t)b * nx * ny * nz;
+    const unsigned char *fl = flags + (size_t)b * nz * nyc;
+    // tile_gemm addresses rows with int: shift the table pointers to this tile
+    const float2 *My_t = My + (size_t)m0 * ny;
+    const int rows = (int)((npix - m0) < kBM ? (npix - m0) : kBM);
+    float2 tot[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) tot[i] = make_float2(0.f, 0.f);
+    for (int j = z0; j < z1; ++j) {
+        bool has = false;
+        for (int c = 0; c < nyc; ++c) has |= fl[(size_t)j * nyc + c] != 0;
+        if (!has) continue;   // vacuum slice (uniform over the block)
+        float2 f[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) f[i] = make_float2(0.f, 0.f);
+        for (int x0 = 0; x0 < nx; x0 += kBN) {
+            float2 acc[4][4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) acc[i][jj] = make_float2(0.f, 0.f);
+            tile_gemm(My_t, ny, rows, 0, vol + (size_t)j * ny * nx, nx, nx, x0, ny, fl + (size_t)j * nyc, sm, acc);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int r = ty * 4 + i;
+                if (r >= rows) continue;
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const int x = x0 + tx * 4 + jj;
+                    if (x >= nx) continue;
+                    const float2 w = __ldg(Mx + (size_t)(m0 + r) * nx + x);
+                    f[i].x = fmaf(acc[i][jj].x, w.x, f[i].x);
+                    f[i].x = fmaf(-acc[i][jj].y, w.y, f[i].x);
+                    f[i].y = fmaf(acc[i][jj].x, w.y, f[i].y);
+                    f[i].y = fmaf(acc[i][jj].y, w.x, f[i].y);
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+#pragma unroll
+            for (int off = 8; off > 0; off >>= 1) {   // the 16 threads of a row group hold the 64 x of the tile
+                f[i].x += __shfl_xor_sync(0xffffffffu, f[i].x, off, 16);
+                f[i].y += __shfl_xor_sync(0xffffffffu, f[i].y, off, 16);
+            }
+            const int r = ty * 4 + i;
+            if (r < rows) {
+                const float2 w = __ldg(Mz + (size_t)(m0 + r) * nz + j);
+                tot[i].x = fmaf(w.x, f[i].x, tot[i].x);
+                tot[i].x = fmaf(-w.y, f[i].y, tot[i].x);
+                tot[i].y = fmaf(w.x, f[i].y, tot[i].y);
+                tot[i].y = fmaf(w.y, f[i].x, tot[i].y);
+            }
+        }
+    }
+    if (tx == 0)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = ty * 4 + i;
+            if (r < rows) partial[((size_t)b * nsplit + zs) * npix_pad + m0 + r] = tot[i];
+        }
+}
+
+cudaError_t launch_simt_table(const float *d_rho, const double *d_q, const Plan &p, float2 *d_My, float2 *d_Mx, float2 *d_Mz,
+                              unsigned char *d_flags, float2 *d_partial, cudaStream_t st, int *nlaunch) {
+    const int nyc = (p.ny + 15) / 16;
+    const int64_t ey = p.npix * p.ny, ex = p.npix * p.nx, ez = p.npix * p.nz;
+    pixel_table_kernel<<<(unsigned)((ey + 255) / 256), 256, 0, st>>>(d_q, 1, p.npix, p.ny, p.dy, d_My);
+    pixel_table_kernel<<<(unsigned)((ex + 255) / 256), 256, 0, st>>>(d_q, 0, p.npix, p.nx, p.dx, d_Mx);
+    pixel_table_kernel<<<(unsigned)((ez + 255) / 256), 256, 0, st>>>(d_q, 2, p.npix, p.nz, p.dz, d_Mz);
+    for (int b = 0; b < p.batch; ++b)
+        sep_rowflags_kernel<<<(unsigned)((p.nz * nyc + 7) / 8), 256, 0, st>>>((const float2 *)d_rho + (size_t)b * p.nvox, p.nx, p.ny,
+                                                                            p.nz, nyc, d_flags + (size_t)b * p.nz * nyc);
+    dim3 grid((unsigned)((p.npix + kBM - 1) / kBM), p.nsplit, p.batch);
+    simt_table_kernel<<<grid, 256, 0, st>>>(d_My, d_Mx, d_Mz, (const float2 *)d_rho, d_flags, p.npix, p.npix_pad, p.nx, p.ny, p.nz,
+                                            nyc, p.nsplit, d_partial);
+    if (nlaunch) *nlaunch += 4 + p.batch;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_sep_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p, float2 *d_Ex,
                               float2 *d_Ey, cudaStream_t st) {
     const int64_t nxe = (int64_t)npx * p.nx, nye = (int64_t)npy * p.ny;

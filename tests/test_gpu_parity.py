@@ -25,8 +25,8 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-# name -> (method, flags): CTA-pair tensor kernel (default), single-CTA tensor kernel, CUDA-core sincos variant
-METHODS = {"tensor": (1, 0), "tensor_1cta": (1, 1), "simt_sincos": (2, 0)}
+# name -> (method, flags): CTA-pair tensor kernel (default), single-CTA tensor kernel, CUDA-core sincos and table variants
+METHODS = {"tensor": (1, 0), "tensor_1cta": (1, 1), "simt_sincos": (2, 0), "simt_table": (3, 0)}
 
 
 # ------------------------------------------------------------------------------------------ stage kernels
@@ -254,9 +254,6 @@ def test_error_codes(sm):
             sm.simulate(d, vox, bad.get("lam", w.lam), 64, 64, bad.get("theta", 30.0), quat=bad.get("quat"),
                         method=bad.get("method", 0))
         assert e.value.status == B.INVALID_ARGUMENT
-    with pytest.raises(B.ScatmanError) as e:
-        sm.simulate(d, vox, w.lam, 64, 64, 30.0, method=B.METHOD_SIMT_TABLE)
-    assert e.value.status == B.NOT_IMPLEMENTED
 
 
 # ------------------------------------------------------------------------------------------ full sizes, sampled pixels
