@@ -115,7 +115,8 @@ __global__ void sep_rowflags_kernel(const float2 *__restrict__ rho, int nx, int 
 // stage X: H[M][N] = rho[M][K] Ex[K][N]  (M = nz * ny, K = nx, N = npx).  Row tiles whose rho rows are all zero are not
 // multiplied: H is written as zeros (vacuum rows are most of a grid).
 __global__ void __launch_bounds__(256) sep_stage_x_kernel(const float2 *__restrict__ rho, const float2 *__restrict__ Ex, int M,
-                                                          int K, int N, float2 *__restrict__ H) {
+                                                          int K, int N, const unsigned char *__restrict__ rowflags,
+                                                          float2 *__restrict__ H) {
     __shared__ TileSmem sm;
     __shared__ int s_any;
     const int m0 = blockIdx.x * kBM, n0 = blockIdx.y * kBN;
@@ -123,11 +124,16 @@ __global__ void __launch_bounds__(256) sep_stage_x_kernel(const float2 *__restri
     if (tid == 0) s_any = 0;
     __syncthreads();
     bool any = false;
-    for (size_t e = tid; e < (size_t)kBM * K; e += 256) {
-        const int m = m0 + (int)(e / K);
-        if (m < M) {
-            const float2 v = __ldg(rho + (size_t)m * K + (e % K));
-            any |= (v.x != 0.f) | (v.y != 0.f);
+    if (rowflags) {   // ny is a multiple of 16: the 16-row chunks of sep_rowflags_kernel are rows [16 c, 16 c + 16) of rho
+        for (int c = 0; c < kBM / 16; ++c)
+            if (m0 + 16 * c < M) any |= rowflags[m0 / 16 + c] != 0;
+    } else {
+        for (size_t e = tid; e < (size_t)kBM * K; e += 256) {
+            const int m = m0 + (int)(e / K);
+            if (m < M) {
+                const float2 v = __ldg(rho + (size_t)m * K + (e % K));
+                any |= (v.x != 0.f) | (v.y != 0.f);
+            }
         }
     }
     if (any) s_any = 1;
@@ -180,13 +186,35 @@ __global__ void __launch_bounds__(256, 2) sep_stage_yz_kernel(const float2 *__re
     for (int i = 0; i < 4; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) tot[i][j] = make_float2(0.f, 0.f);
-    for (int jz = z0; jz < z1; ++jz) {
-        float2 acc[4][4];
+    // One pipeline over the non-vacuum (slice, 16-y chunk) pairs of the z range, c = (jz - z0) * nyc + chunk: the operand
+    // tiles of the next pair (possibly of the next slice) are in flight while the current one is multiplied; when the slice
+    // changes, the finished slice's tile gets its phase and joins the total.
+    const int ar = tid >> 2, ak = (tid & 3) * 4;     // loader roles as in tile_gemm
+    const int bk = tid >> 4, bn = (tid & 15) * 4;
+    const int nc = (z1 - z0) * nyc;
+    const unsigned char *fl = flags + (size_t)z0 * nyc;
+    auto next_pair = [&](int c) {
+        while (c < nc && fl[c] == 0) ++c;
+        return c;
+    };
+    float2 ra[4], rb[4];
+    auto load = [&](int c) {
+        const int jz = z0 + c / nyc, k0 = (c % nyc) * kBK;
+        const float2 *Hj = H + (size_t)jz * ny * npx;
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 4; ++i) {
+            const int m = m0 + ar, kk = k0 + ak + i;
+            ra[i] = (m < npy && kk < ny) ? __ldg(Ey + (size_t)m * ny + kk) : make_float2(0.f, 0.f);
+            const int kb = k0 + bk, n = n0 + bn + i;
+            rb[i] = (kb < ny && n < npx) ? __ldg(Hj + (size_t)kb * npx + n) : make_float2(0.f, 0.f);
+        }
+    };
+    float2 acc[4][4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[i][j] = make_float2(0.f, 0.f);
-        tile_gemm(Ey, ny, npy, m0, H + (size_t)jz * ny * npx, npx, npx, n0, ny, flags + (size_t)jz * nyc, sm, acc);
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_float2(0.f, 0.f);
+    auto fold = [&](int jz) {   // Blocks 7-8: tot += e^{i qz z_j} acc, acc = 0
         const double zj = centre_d(jz, nz, dz);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
@@ -194,13 +222,47 @@ __global__ void __launch_bounds__(256, 2) sep_stage_yz_kernel(const float2 *__re
             for (int j = 0; j < 4; ++j) {
                 double t = s_qzt[i * 4 + j][tid] * zj;
                 t -= rint(t);
-                float s, c;
-                sincospif(2.0f * (float)t, &s, &c);
-                tot[i][j].x = fmaf(c, acc[i][j].x, tot[i][j].x);
-                tot[i][j].x = fmaf(-s, acc[i][j].y, tot[i][j].x);
-                tot[i][j].y = fmaf(c, acc[i][j].y, tot[i][j].y);
-                tot[i][j].y = fmaf(s, acc[i][j].x, tot[i][j].y);
+                float sn, cs;
+                sincospif(2.0f * (float)t, &sn, &cs);
+                tot[i][j].x = fmaf(cs, acc[i][j].x, tot[i][j].x);
+                tot[i][j].x = fmaf(-sn, acc[i][j].y, tot[i][j].x);
+                tot[i][j].y = fmaf(cs, acc[i][j].y, tot[i][j].y);
+                tot[i][j].y = fmaf(sn, acc[i][j].x, tot[i][j].y);
+                acc[i][j] = make_float2(0.f, 0.f);
             }
+    };
+    int c = next_pair(0);
+    if (c < nc) load(c);
+    while (c < nc) {
+        __syncthreads();   // previous tile fully consumed
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            sm.As[ak + i][ar] = ra[i];
+            sm.Bs[bk][bn + i] = rb[i];
+        }
+        __syncthreads();
+        const int cn = next_pair(c + 1);
+        if (cn < nc) load(cn);
+#pragma unroll
+        for (int kk = 0; kk < kBK; ++kk) {
+            float2 av[4], bv[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                av[i] = sm.As[kk][ty * 4 + i];
+                bv[i] = sm.Bs[kk][tx * 4 + i];
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    acc[i][j].x = fmaf(av[i].x, bv[j].x, acc[i][j].x);
+                    acc[i][j].x = fmaf(-av[i].y, bv[j].y, acc[i][j].x);
+                    acc[i][j].y = fmaf(av[i].x, bv[j].y, acc[i][j].y);
+                    acc[i][j].y = fmaf(av[i].y, bv[j].x, acc[i][j].y);
+                }
+        }
+        if (cn >= nc || cn / nyc != c / nyc) fold(z0 + c / nyc);   // last pair of its slice
+        c = cn;
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i)
@@ -361,7 +423,7 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
     const double k = 2.0 * 3.14159265358979323846 / p.lambda;
     sep_rowflags_kernel<<<(unsigned)((p.nz * nyc + 7) / 8), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nyc, d_flags);
     dim3 gx((M + kBM - 1) / kBM, (npx + kBN - 1) / kBN);
-    sep_stage_x_kernel<<<gx, 256, 0, st>>>(d_rho, d_Ex, M, p.nx, npx, d_H);
+    sep_stage_x_kernel<<<gx, 256, 0, st>>>(d_rho, d_Ex, M, p.nx, npx, p.ny % 16 == 0 ? d_flags : nullptr, d_H);
     dim3 gy((npx + kBN - 1) / kBN, (npy + kBM - 1) / kBM, nzs);
     static bool attr_set = false;
     if (!attr_set) {
