@@ -384,17 +384,22 @@ __global__ void table_a_kernel(const double *__restrict__ q, int64_t npix, int64
     }
 }
 
-// which: 0 anchor (count nxa, coord = centre(16 a)), 1 fine (count 16, coord = b dx), 2 mz (count nz)
-__global__ void table_small_kernel(const double *__restrict__ q, int64_t npix, int which, int count, int n, double d,
-                                   float2 *__restrict__ out) {
-    const int lane = threadIdx.x;  // 128
-    const int idx0 = blockIdx.y * 16, tile = blockIdx.x;
+// anchor, fine and mz in ONE launch: blockIdx.y ranges [0, ya) anchor runs, [ya, ya + 1) fine, the rest mz runs
+__global__ void table_small_all_kernel(const double *__restrict__ q, int64_t npix, int nxa, int nx, double dx, int nz, double dz,
+                                       int ya, float2 *__restrict__ anchor, float2 *__restrict__ fine, float2 *__restrict__ mz) {
+    const int lane = threadIdx.x, tile = blockIdx.x;
     const int64_t p = (int64_t)tile * kTileP + lane;
+    int which, y = blockIdx.y, count;
+    float2 *out;
+    if (y < ya) { which = 0; count = nxa; out = anchor; }
+    else if (y == ya) { which = 1; y = 0; count = kFine; out = fine; }
+    else { which = 2; y -= ya + 1; count = nz; out = mz; }
+    const int idx0 = y * 16;
     double re[16], im[16];
     if (p < npix) {
-        if (which == 0) phase_run16(q[3 * p + 0], centre(idx0 * kFine, n, d), d * (double)kFine, re, im);
-        else if (which == 1) phase_run16(q[3 * p + 0], (double)idx0 * d, d, re, im);
-        else phase_run16(q[3 * p + 2], centre(idx0, n, d), d, re, im);
+        if (which == 0) phase_run16(q[3 * p + 0], centre(idx0 * kFine, nx, dx), dx * (double)kFine, re, im);
+        else if (which == 1) phase_run16(q[3 * p + 0], 0.0, dx, re, im);
+        else phase_run16(q[3 * p + 2], centre(idx0, nz, dz), dz, re, im);
     }
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -408,10 +413,10 @@ cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 
                           float2 *d_mz, cudaStream_t st, int *nlaunch) {
     const int64_t nthreads_a = p.npix_pad * (p.ny_pad / 16);
     table_a_kernel<<<(unsigned)((nthreads_a + 127) / 128), 128, 0, st>>>(d_q, p.npix, p.npix_pad, p.ny, p.ny_pad, p.dy, d_A);
-    table_small_kernel<<<dim3(p.ntiles, (p.nxa + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, 0, p.nxa, p.nx, p.dx, d_anchor);
-    table_small_kernel<<<dim3(p.ntiles, 1), kTileP, 0, st>>>(d_q, p.npix, 1, kFine, p.nx, p.dx, d_fine);
-    table_small_kernel<<<dim3(p.ntiles, (p.nz + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, 2, p.nz, p.nz, p.dz, d_mz);
-    if (nlaunch) *nlaunch += 4;
+    const int ya = (p.nxa + 15) / 16;
+    table_small_all_kernel<<<dim3(p.ntiles, ya + 1 + (p.nz + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, p.nxa, p.nx, p.dx, p.nz, p.dz, ya,
+                                                                                       d_anchor, d_fine, d_mz);
+    if (nlaunch) *nlaunch += 2;
     return cudaGetLastError();
 }
 
