@@ -195,7 +195,9 @@ def main():
         qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
         qy = torch.from_numpy((np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)).cuda()
         need = C.c_size_t(0)
-        sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(need)))
+        qmethod = args.method if args.method in (0, 1, 3) else 0
+        qopts = B.Options(0, qmethod, 0, 0)
+        sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
         ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
 
     shapes = None
@@ -213,7 +215,7 @@ def main():
                                workspace=ws, out=out, stream=stream)
             return
         if args.route == "qgrid":
-            sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, workspace=ws, out=out, stream=stream)
+            sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=stream)
             return
         sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
                     workspace=ws, out=out, stream=stream)

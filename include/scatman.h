@@ -141,7 +141,7 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
  * get I = 0.  d_qx[npx], d_qy[npy]: FP64 device arrays (any values, e.g. the DFT grid 2 pi m / (N dx)).
  * d_I[b][npy][npx].  rho_mode from opts; method / precision / flags of opts are ignored. */
 int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
-                                  size_t *bytes);
+                                  const scatman_options *opts, size_t *bytes);
 int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
                            const double *d_qx, int32_t npx, const double *d_qy, int32_t npy, const double *h_quat,
                            int32_t batch, const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I,

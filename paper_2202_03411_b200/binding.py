@@ -86,7 +86,7 @@ def load_library() -> C.CDLL:
                                      C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                         C.POINTER(Options), vp]
-    L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(C.c_size_t)]
+    L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
     L.scatman_simulate_qgrid.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i32, vp, i32, C.POINTER(dbl), i32,
                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_shapes_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i64, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
@@ -321,10 +321,11 @@ class Scatman:
                                                      C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
-    def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, workspace=None, out=None,
-                       stream=None):
+    def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,
+                       workspace=None, out=None, stream=None):
         """I float32 [B][npy][npx] on the tensor grid (qx[a], qy[b]) of transverse momentum transfers (CUDA float64 1-D
-        tensors): the separable route (scatman_simulate_qgrid)."""
+        tensors): the separable route (scatman_simulate_qgrid).  method: AUTO / TENSOR = both GEMM stages on tcgen05,
+        SIMT_TABLE = FP32 CUDA cores."""
         import torch
         self._check_dn(dn)
         for q in (qx, qy):
@@ -333,12 +334,13 @@ class Scatman:
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         npx, npy = int(qx.numel()), int(qy.numel())
         need = C.c_size_t(0)
-        self._check(self.lib.scatman_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(need)))
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        self._check(self.lib.scatman_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(opts),
+                                                           C.byref(need)))
         if workspace is None:
             workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dn.device)
         if out is None:
             out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
-        opts = Options(int(rho_mode), 0, 0, 0)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate_qgrid(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                     C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy, qp, batch,

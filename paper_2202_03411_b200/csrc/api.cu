@@ -435,17 +435,22 @@ int scatman_simulate_shapes(scatman_ctx *ctx, const scatman_shape *h_shapes, int
 // ---- separable route: workspace layout -------------------------------------------------------------------------
 struct SepPlan {
     Plan p;
+    SepTcPlan tc;
+    bool tensor = true;   // both GEMM stages on tcgen05 (method AUTO / TENSOR) or FP32 CUDA cores (SIMT_TABLE)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_hp = 0, off_scale = 0, total = 0;
 };
-static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int num_sms) {
+static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
+                             int num_sms) {
     SepPlan sp;
     Plan &p = sp.p;
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
     p.npix = (int64_t)npx * npy; p.batch = batch; p.rho_mode = rho_mode;
     p.nvox = (int64_t)g.nx * g.ny * g.nz;
+    sp.tensor = method != SCATMAN_METHOD_SIMT_TABLE;
     sp.nzs = sep_zsplit(p, npx, npy, num_sms);
+    if (sp.tensor) sp.tc = make_sep_tc_plan(p, npx, npy, num_sms);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
     sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
@@ -454,19 +459,34 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
     sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
-    sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
-    sp.off_h = take(sizeof(float2) * (size_t)g.nz * g.ny * npx);
-    sp.off_flags = take((size_t)g.nz * ((g.ny + 15) / 16));
-    sp.off_partial = take(sizeof(float2) * (size_t)sp.nzs * npx * npy);
+    if (sp.tensor) {
+        const SepTcPlan &t = sp.tc;
+        sp.off_eyp = take(sizeof(__half) * 4 * (size_t)t.NPYP * t.NY);
+        sp.off_hp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NPXP * t.NY);
+        sp.off_flags = take((size_t)g.nz * (t.NY / 64));
+        sp.off_scale = take(sizeof(float) * 2);
+        sp.off_partial = take(sizeof(float2) * (size_t)t.nsplit * npx * npy);
+    } else {
+        sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
+        sp.off_h = take(sizeof(float2) * (size_t)g.nz * g.ny * npx);
+        sp.off_flags = take((size_t)g.nz * ((g.ny + 15) / 16));
+        sp.off_partial = take(sizeof(float2) * (size_t)sp.nzs * npx * npy);
+    }
     sp.total = off;
     return sp;
 }
 
+static bool valid_qgrid_method(int m) {
+    return m == SCATMAN_METHOD_AUTO || m == SCATMAN_METHOD_TENSOR || m == SCATMAN_METHOD_SIMT_TABLE;
+}
+
 int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
-                                  size_t *bytes) {
+                                  const scatman_options *opts, size_t *bytes) {
     if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
-    if (!valid_grid(grid) || npx < 1 || npy < 1 || batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
-    *bytes = make_sep_plan(*grid, 1.0, npx, npy, batch, 0, ctx->num_sms).total;
+    const int method = opts ? opts->method : SCATMAN_METHOD_AUTO;
+    if (!valid_grid(grid) || npx < 1 || npy < 1 || batch < 1 || !valid_qgrid_method(method))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = make_sep_plan(*grid, 1.0, npx, npy, batch, 0, method, ctx->num_sms).total;
     return SCATMAN_OK;
 }
 
@@ -476,13 +496,14 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !d_qx || !d_qy || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) ||
-        batch < 1 || batch > 65535 || npx < 1 || npy < 1 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1))
+        batch < 1 || batch > 65535 || npx < 1 || npy < 1 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1) ||
+        !valid_qgrid_method(o.method))
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
     if (h_quat && !valid_quats(h_quat, batch)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "quaternion is not unit");
     if (((uintptr_t)d_dn | (uintptr_t)d_ws | (uintptr_t)d_I) & 15)
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
     cudaSetDevice(ctx->device);
-    const SepPlan sp = make_sep_plan(*grid, lambda, npx, npy, batch, o.rho_mode, ctx->num_sms);
+    const SepPlan sp = make_sep_plan(*grid, lambda, npx, npy, batch, o.rho_mode, o.method, ctx->num_sms);
     const Plan &p = sp.p;
     if (ws_bytes < sp.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -501,20 +522,47 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         src = (const float *)(ws + sp.off_rot);
     }
     float *rho = (float *)(ws + sp.off_rho);
-    e = launch_strength(src, p, batch, rho, (unsigned *)(ws + sp.off_max), st);
+    unsigned *maxbits = (unsigned *)(ws + sp.off_max);
+    e = launch_strength(src, p, batch, rho, maxbits, st);
     ++nl;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
     float2 *Ex = (float2 *)(ws + sp.off_ex), *Ey = (float2 *)(ws + sp.off_ey);
-    e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
-    nl += 2;
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
-    cudaEventRecord(ctx->ev0, st);
-    for (int b = 0; b < batch; ++b) {
-        e = launch_sep_item((const float2 *)rho + (size_t)b * p.nvox, p, Ex, Ey, d_qx, npx, d_qy, npy, sp.nzs,
-                            (float2 *)(ws + sp.off_h), ws + sp.off_flags, (float2 *)(ws + sp.off_partial),
-                            d_I + (size_t)b * npx * npy, st);
-        nl += 4;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid stages");
+    if (sp.tensor) {
+        const SepTcPlan &t = sp.tc;
+        __half *Eyp = (__half *)(ws + sp.off_eyp), *Hp = (__half *)(ws + sp.off_hp);
+        float *scaleH = (float *)(ws + sp.off_scale), *ampscale = scaleH + 1;
+        e = launch_sep_tables(d_qx, npx, nullptr, 0, p, Ex, nullptr, st);
+        if (e == cudaSuccess) e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, nullptr, Eyp, st);
+        nl += 2;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
+        cudaEventRecord(ctx->ev0, st);
+        for (int b = 0; b < batch; ++b) {
+            const float2 *rho_b = (const float2 *)rho + (size_t)b * p.nvox;
+            std::string err;
+            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, ws + sp.off_flags, scaleH, ampscale, st);
+            if (e == cudaSuccess)
+                e = launch_sep_stage_x_planes(rho_b, Ex, p, npx, t.NY, t.NPXP, ws + sp.off_flags, scaleH, Hp, st);
+            if (e == cudaSuccess)
+                e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, d_qx, npx, d_qy, npy, (float2 *)(ws + sp.off_partial),
+                                     ctx->num_sms, st, &err);
+            if (e == cudaSuccess)
+                e = launch_sep_tc_finalize((const float2 *)(ws + sp.off_partial), d_qx, npx, d_qy, npy, p, t, ampscale,
+                                           d_I + (size_t)b * npx * npy, st);
+            nl += 5;
+            if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "qgrid stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
+        }
+    } else {
+        e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
+        nl += 2;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
+        cudaEventRecord(ctx->ev0, st);
+        for (int b = 0; b < batch; ++b) {
+            e = launch_sep_item((const float2 *)rho + (size_t)b * p.nvox, p, Ex, Ey, d_qx, npx, d_qy, npy, sp.nzs,
+                                (float2 *)(ws + sp.off_h), ws + sp.off_flags, (float2 *)(ws + sp.off_partial),
+                                d_I + (size_t)b * npx * npy, st);
+            nl += 4;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid stages");
+        }
     }
     cudaEventRecord(ctx->ev1, st);
     ctx->ev_valid = true;

@@ -71,6 +71,23 @@ int sep_zsplit(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_Ex, const float2 *d_Ey, const double *d_qx,
                             int npx, const double *d_qy, int npy, int nzs, float2 *d_H, unsigned char *d_flags,
                             float2 *d_partial, float *d_I, cudaStream_t st);
+// separable route on tensor cores (sep_tensor_kernels.cu)
+struct SepTcPlan {
+    int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
+    int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
+};
+SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
+cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
+                                 const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
+cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
+                                    unsigned char *d_flags64, float *d_scaleH, float *d_ampscale, cudaStream_t st);
+cudaError_t launch_sep_stage_x_planes(const float2 *d_rho, const float2 *d_Ex, const Plan &p, int npx, int NY, int NPXP,
+                                      const unsigned char *d_flags64, const float *d_scaleH, __half *d_Hp, cudaStream_t st);
+cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
+                             const unsigned char *d_flags64, const double *d_qx, int npx, const double *d_qy, int npy,
+                             float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);
+cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
+                                   const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st);
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
 
 // tensor path: tensor maps are encoded on the host through the driver entry point

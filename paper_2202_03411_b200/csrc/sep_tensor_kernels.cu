@@ -1,0 +1,464 @@
+// sep_tensor_kernels.cu -- the separable tensor-grid route (Block 6 of Fig. 4 transforms every slice on a
+// uniform (qx, qy) grid) with both GEMM stages on tcgen05 tensor cores, FP16x3 split precision:
+//   stage X   H_j[a, y]  = sum_x rho~_j[y, x] e^{i qx[a] x}                  (M = 128 y rows, N = a columns, K = x)
+//   stage YZ  A[b, a]    = sum_j e^{i qz(a,b) z_j} sum_y e^{i qy[b] y} H_j[a, y]   (M = 128 b rows, N = 64 a columns, K = y)
+// Every operand is four FP16 planes (Re_hi, Re_lo, Im_hi, Im_lo) of a scaled FP32 value, K-major, fetched by TMA boxes of
+// 64 K x rows with the 128-byte swizzle; a complex product is the 12 real MMAs AhBh + AlBh + AhBl of tensor_kernel.cu
+// (the minus sign of Re = ArBr - AiBi is the instruction descriptor's negate-A bit).  Accumulators live in TMEM (four
+// buffers of D_re, D_im), FP32.  Stage X's epilogue rescales H and splits it into the FP16 planes stage YZ reads as its
+// B operand; stage YZ's epilogue is Blocks 7-8 of Fig. 4: the slice phase e^{i qz(a,b) z_j} applied to
+// the accumulator tile and the sum over slices, both in registers.  Vacuum is skipped in 64-y blocks (byte flags).
+//
+// Slice phase: qz z_j = 2 pi t (2j - nz + 1) with t = qz dz / (4 pi) turns; frac(t) is kept as a 32-bit fixed-point
+// fraction of a turn, so the product with the integer (2j - nz + 1) wraps modulo one turn for free (error <= 512 * 2^-33
+// turns = 4e-7 rad), and sin / cos come from the SFU on an argument in [-pi, pi) (absolute error ~4e-7).
+#include <cuda.h>
+
+#include "internal.h"
+#include "ptx_sm100.h"
+
+namespace scatman {
+
+bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
+                const cuuint32_t *box, CUtensorMapSwizzle swizzle);   // tensor_kernel.cu
+
+namespace {
+
+constexpr int kM = 128;              // UMMA M: rows of the A operand tile
+constexpr int kKB = 64;              // K per block (one 128-byte swizzle row of FP16)
+constexpr int kSlotA = kM * kKB * 2; // 16384: one plane, one K block of an A tile
+constexpr int kNyz = 64;             // stage YZ: a columns per accumulator
+constexpr int kThreadsTc = 384;      // warp 0 TMA, 1 MMA, 2 TMEM, 3 idle, 4-11 epilogue
+constexpr uint32_t kTmemColsTc = 512;
+constexpr int kNBuf = 4;             // accumulator buffers (128 columns each: D_re 64 + D_im 64)
+
+__device__ __forceinline__ double centre_t(int i, int n, double d) { return ((double)i - 0.5 * (double)(n - 1)) * d; }
+
+__device__ __forceinline__ void split4(float re, float im, __half (&h)[4]) {
+    h[0] = __float2half_rn(re);
+    h[1] = __float2half_rn(re - __half2float(h[0]));
+    h[2] = __float2half_rn(im);
+    h[3] = __float2half_rn(im - __half2float(h[2]));
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ operands
+// E planes fp16 [4][rows_pad][kpad] = split(2^10 e^{i q[r] c_i}), c_i centred coordinates; zero in the padding
+__global__ void sep_tc_table_kernel(const double *__restrict__ q, int nq, int rows_pad, int n, int kpad, double d,
+                                    __half *__restrict__ E) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)rows_pad * kpad) return;
+    const int r = (int)(t / kpad), i = (int)(t % kpad);
+    float re = 0.f, im = 0.f;
+    if (r < nq && i < n) {
+        double s, c;
+        sincos(q[r] * centre_t(i, n, d), &s, &c);
+        re = (float)(c * (double)kScaleA);
+        im = (float)(s * (double)kScaleA);
+    }
+    __half h[4];
+    split4(re, im, h);
+    const size_t plane = (size_t)rows_pad * kpad;
+#pragma unroll
+    for (int pl = 0; pl < 4; ++pl) E[pl * plane + t] = h[pl];
+}
+
+// per item: sH = 2^(14 - e - L) (max |rho~ component| in [2^(e-1), 2^e), 2^L >= nx) is the scale H is stored with;
+// ampscale = dV / (2^10 sH) takes the summed amplitude back to physical units
+__global__ void sep_tc_scale_kernel(const unsigned *__restrict__ maxbits, int L, float dV, float *__restrict__ scaleH,
+                                    float *__restrict__ ampscale) {
+    const float m = __uint_as_float(maxbits[0]);
+    int e = 0;
+    if (m > 0.f) frexpf(m, &e);
+    const float sH = ldexpf(1.f, 14 - e - L);
+    scaleH[0] = sH;
+    ampscale[0] = dV / (kScaleA * sH);
+}
+
+// flags64[j][yb] = 1 if any rho~ of slice j, y in [64 yb, 64 yb + 64) is non-zero (one warp per block)
+__global__ void sep_tc_flags_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nyb,
+                                    unsigned char *__restrict__ flags) {
+    const int blk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (blk >= nz * nyb) return;
+    const int j = blk / nyb, yb = blk % nyb;
+    const int y0 = yb * kKB, y1 = min(ny, y0 + kKB);
+    bool any = false;
+    if (y0 < ny) {
+        const float2 *src = rho + ((size_t)j * ny + y0) * nx;
+        const size_t n = (size_t)(y1 - y0) * nx;
+        for (size_t e = lane; e < n; e += 32) {
+            const float2 v = __ldg(src + e);
+            any |= (v.x != 0.f) | (v.y != 0.f);
+        }
+    }
+    any = __any_sync(0xffffffffu, any);
+    if (lane == 0) flags[blk] = any ? 1 : 0;
+}
+
+// ------------------------------------------------------------------------------------------------ stage YZ
+struct SepYzParams {
+    int nz, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nkb = NY / 64
+    double k, dz;
+    const double *qx, *qy;
+    const unsigned char *flags;   // [nz][nkb]
+    float2 *partial;              // [ng * nzs][npy][npx]
+};
+
+struct YzItem {
+    int tb, ta, g, s;
+};
+__device__ __forceinline__ YzItem yz_decode(int item, const SepYzParams &P) {
+    YzItem it;
+    it.tb = item % P.ntb;   // b tiles fastest: concurrent CTAs stream the same H tiles
+    item /= P.ntb;
+    it.ta = item % P.nta;
+    item /= P.nta;
+    it.g = item % P.ng;
+    it.s = item / P.ng;
+    return it;
+}
+
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
+    constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
+    constexpr int kStageB = 4 * kNyz * kKB * 2;       // 32768: four planes of one 64-y block of an H tile
+    constexpr int kStages = 3;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sA = smem;
+    uint8_t *sB = smem + kSmemA;
+    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kStageB);
+    uint64_t *a_full = bars + 0, *a_empty = bars + 1;
+    uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
+    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNBuf;
+    uint32_t *tmem_ptr = (uint32_t *)(t_empty + kNBuf);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nitems = P.ntb * P.nta * P.ng * P.nzs;
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(a_full, 1);
+        ptx::mbar_init(a_empty, 1);
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(b_full + i, 1);
+            ptx::mbar_init(b_empty + i, 1);
+        }
+        for (int i = 0; i < kNBuf; ++i) {
+            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_empty + i, 8);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    auto zrange = [&](int s, int &z0, int &z1) {
+        z0 = (int)(((long long)P.nz * s) / P.nzs);
+        z1 = (int)(((long long)P.nz * (s + 1)) / P.nzs);
+    };
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const YzItem it = yz_decode(item, P);
+            ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
+                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)kSmemA);
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int kb = 0; kb < 2; ++kb)
+                        ptx::tma_load_3d(sA + (pl * 2 + kb) * kSlotA, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
+            }
+            __syncwarp();
+            int z0, z1;
+            zrange(it.s, z0, z1);
+            for (int j = z0; j < z1; ++j) {
+                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
+                for (int kb = 0; kb < 2; ++kb) {
+                    if (__ldg(fl + kb) == 0) continue;
+                    ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kStageB);
+                        for (int pl = 0; pl < 4; ++pl)
+                            ptx::tma_load_3d(sB + slot * kStageB + pl * (kStageB / 4), &tmB, b_full + slot,
+                                             (it.g * 2 + kb) * kKB, j * P.NPXP + it.ta * kNyz, pl);
+                    }
+                    __syncwarp();
+                    if (++slot == kStages) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, kNyz, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, kNyz, true);
+        const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
+        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
+        constexpr uint64_t kA = kSlotA >> 4, kBst = kStageB >> 4, kBpl = (kStageB / 4) >> 4;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const YzItem it = yz_decode(item, P);
+            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+            ptx::tc_fence_after();
+            int z0, z1;
+            zrange(it.s, z0, z1);
+            for (int j = z0; j < z1; ++j) {
+                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
+                const int f0 = __ldg(fl), f1 = __ldg(fl + 1);
+                if ((f0 | f1) == 0) continue;
+                const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
+                bool first = true;
+                for (int kb = 0; kb < 2; ++kb) {
+                    if ((kb ? f1 : f0) == 0) continue;
+                    ptx::mbar_wait(b_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks) {
+                            const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
+                            const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
+                            const uint64_t b_reh = descB0 + (uint64_t)slot * kBst + (uint64_t)(ks * 2);
+                            const uint64_t b_rel = b_reh + kBpl, b_imh = b_rel + kBpl, b_iml = b_imh + kBpl;
+                            const uint32_t acc0 = (first && ks == 0) ? 0u : 1u;
+                            ptx::umma_f16(d_re, a_reh, b_reh, idesc_pos, acc0);
+                            ptx::umma_f16(d_im, a_imh, b_reh, idesc_pos, acc0);
+                            ptx::umma_f16(d_re, a_rel, b_reh, idesc_pos, 1u);
+                            ptx::umma_f16(d_im, a_iml, b_reh, idesc_pos, 1u);
+                            ptx::umma_f16(d_re, a_reh, b_rel, idesc_pos, 1u);
+                            ptx::umma_f16(d_im, a_imh, b_rel, idesc_pos, 1u);
+                            ptx::umma_f16(d_re, a_imh, b_imh, idesc_neg, 1u);
+                            ptx::umma_f16(d_im, a_reh, b_imh, idesc_pos, 1u);
+                            ptx::umma_f16(d_re, a_iml, b_imh, idesc_neg, 1u);
+                            ptx::umma_f16(d_im, a_rel, b_imh, idesc_pos, 1u);
+                            ptx::umma_f16(d_re, a_imh, b_iml, idesc_neg, 1u);
+                            ptx::umma_f16(d_im, a_reh, b_iml, idesc_pos, 1u);
+                        }
+                        ptx::umma_commit(b_empty + slot);
+                    }
+                    __syncwarp();
+                    first = false;
+                    if (++slot == kStages) { slot = 0; phase ^= 1; }
+                }
+                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                __syncwarp();
+                ++u;
+            }
+            if (ptx::elect_one()) ptx::umma_commit(a_empty);
+            __syncwarp();
+        }
+    } else if (warp >= 4) {
+        // ===================================================================== epilogue: Blocks 7-8
+        const int lg = warp & 3, ch = (warp - 4) >> 2;   // TMEM lane group, column half
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 32);
+        uint32_t u = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            const YzItem it = yz_decode(item, P);
+            const int b = it.tb * kM + lg * 32 + lane;
+            const int a0 = it.ta * kNyz + ch * 32;
+            const double qyb = b < P.npy ? P.qy[b] : 0.0;
+            uint32_t dph[32];
+#pragma unroll
+            for (int c = 0; c < 32; ++c) {
+                const int a = a0 + c;
+                double t = 0.0;
+                if (a < P.npx && b < P.npy) {
+                    const double qxa = P.qx[a];
+                    const double qxy2 = qxa * qxa + qyb * qyb;
+                    const double kz2 = P.k * P.k - qxy2;
+                    // qz = -(k - sqrt(k^2 - qxy^2)) = -qxy^2 / (k + sqrt(k^2 - qxy^2)): no cancellation near forward
+                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
+                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
+                    t -= rint(t);
+                }
+                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
+            }
+            float2 tot[32];
+#pragma unroll
+            for (int c = 0; c < 32; ++c) tot[c] = make_float2(0.f, 0.f);
+            int z0, z1;
+            zrange(it.s, z0, z1);
+            for (int j = z0; j < z1; ++j) {
+                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
+                if ((__ldg(fl) | __ldg(fl + 1)) == 0) continue;
+                const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
+                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
+                ptx::mbar_wait(t_full + buf, upar);
+                ptx::tc_fence_after();
+                const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
+                uint32_t gre[2][8], gim[2][8];
+                ptx::tmem_ld8(t_re, gre[0]);
+                ptx::tmem_ld8(t_im, gim[0]);
+                ptx::tmem_ld_wait();
+#pragma unroll
+                for (int q4 = 0; q4 < 4; ++q4) {
+                    const int cur = q4 & 1, nxt = cur ^ 1;
+                    if (q4 < 3) {
+                        ptx::tmem_ld8(t_re + (q4 + 1) * 8, gre[nxt]);
+                        ptx::tmem_ld8(t_im + (q4 + 1) * 8, gim[nxt]);
+                    } else {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);   // every column of this warp has landed
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int c = q4 * 8 + i;
+                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
+                        float sn, cs;
+                        __sincosf(ang, &sn, &cs);
+                        const float gr = __uint_as_float(gre[cur][i]), gi = __uint_as_float(gim[cur][i]);
+                        tot[c].x = fmaf(cs, gr, tot[c].x);
+                        tot[c].x = fmaf(-sn, gi, tot[c].x);
+                        tot[c].y = fmaf(cs, gi, tot[c].y);
+                        tot[c].y = fmaf(sn, gr, tot[c].y);
+                    }
+                    if (q4 < 3) ptx::tmem_ld_wait();
+                }
+                ++u;
+            }
+            if (b < P.npy) {
+                float2 *dst = P.partial + ((size_t)(it.g * P.nzs + it.s) * P.npy + b) * P.npx;
+#pragma unroll
+                for (int c = 0; c < 32; ++c)
+                    if (a0 + c < P.npx) dst[a0 + c] = tot[c];
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
+    }
+}
+
+// I[b][a] = |ampscale * sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
+__global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
+                                       const double *__restrict__ qy, double k, int npx, int npy, int nsplit,
+                                       const float *__restrict__ ampscale, float *__restrict__ I) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= (int64_t)npx * npy) return;
+    const int a = (int)(p % npx), b = (int)(p / npx);
+    float re = 0.f, im = 0.f;
+    for (int s = 0; s < nsplit; ++s) {
+        const float2 v = partial[(size_t)s * npx * npy + p];
+        re += v.x;
+        im += v.y;
+    }
+    const float sc = ampscale[0];
+    re *= sc;
+    im *= sc;
+    const bool real = qx[a] * qx[a] + qy[b] * qy[b] <= k * k;
+    I[p] = real ? re * re + im * im : 0.f;
+}
+
+// ------------------------------------------------------------------------------------------------ host
+SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
+    SepTcPlan t;
+    t.NY = (p.ny + 127) / 128 * 128;
+    t.NXP = (p.nx + kKB - 1) / kKB * kKB;
+    t.NPXP = (npx + kNyz - 1) / kNyz * kNyz;
+    t.NPYP = (npy + kM - 1) / kM * kM;
+    t.ng = t.NY / 128;
+    int L = 0;
+    while ((1 << L) < p.nx) ++L;
+    t.L = L;
+    // z splits: enough items for >= 3 waves of CTAs, picked for the best last-wave fill
+    const int base = (t.NPYP / kM) * (t.NPXP / kNyz) * t.ng;
+    int best = 1;
+    double best_eff = -1.0;
+    const int max_z = p.nz < 64 ? p.nz : 64;
+    for (int z = 1; z <= max_z; ++z) {
+        const long long items = (long long)base * z;
+        const long long waves = (items + num_sms - 1) / num_sms;
+        double eff = (double)items / (double)(waves * num_sms);
+        if (waves < 3) eff *= 0.5 + 0.15 * (double)waves;   // few waves: vacuum makes items uneven
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = z; }
+    }
+    t.nzs = best;
+    t.nsplit = t.ng * t.nzs;
+    return t;
+}
+
+cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
+                                 const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st) {
+    const int64_t nye = (int64_t)t.NPYP * t.NY;
+    sep_tc_table_kernel<<<(unsigned)((nye + 255) / 256), 256, 0, st>>>(d_qy, npy, t.NPYP, p.ny, t.NY, p.dy, d_Eyp);
+    (void)d_qx; (void)npx; (void)d_Exp;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
+                             const unsigned char *d_flags64, const double *d_qx, int npx, const double *d_qy, int npy,
+                             float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
+    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    CUtensorMap tmA, tmB;
+    bool ok;
+    {
+        cuuint64_t dims[3] = {(cuuint64_t)t.NY, (cuuint64_t)t.NPYP, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * (cuuint64_t)t.NPYP * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
+        ok = encode_map(&tmA, d_Eyp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+    if (ok) {
+        const cuuint64_t rows = (cuuint64_t)p.nz * t.NPXP;
+        cuuint64_t dims[3] = {(cuuint64_t)t.NY, rows, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kNyz, 1};
+        ok = encode_map(&tmB, d_Hp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+    if (!ok) {
+        if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
+        return cudaErrorUnknown;
+    }
+    SepYzParams P;
+    P.nz = p.nz; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
+    P.ntb = t.NPYP / kM; P.nta = t.NPXP / kNyz; P.nkb = t.NY / kKB;
+    P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
+    P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.partial = d_partial;
+    const int nitems = P.ntb * P.nta * P.ng * P.nzs;
+    const int grid = nitems < num_sms ? nitems : num_sms;
+    sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
+                                    unsigned char *d_flags64, float *d_scaleH, float *d_ampscale, cudaStream_t st) {
+    const int nyb = t.NY / kKB;
+    sep_tc_flags_kernel<<<(unsigned)((p.nz * nyb + 7) / 8), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nyb, d_flags64);
+    sep_tc_scale_kernel<<<1, 1, 0, st>>>(d_maxbits, t.L, (float)(p.dx * p.dy * p.dz), d_scaleH, d_ampscale);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
+                                   const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st) {
+    const int64_t npix = (int64_t)npx * npy;
+    const double k = 2.0 * 3.14159265358979323846 / p.lambda;
+    sep_tc_finalize_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(d_partial, d_qx, d_qy, k, npx, npy, t.nsplit,
+                                                                          d_ampscale, d_I);
+    return cudaGetLastError();
+}
+
+}  // namespace scatman

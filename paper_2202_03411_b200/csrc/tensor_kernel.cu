@@ -559,7 +559,7 @@ static EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
-static bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
+bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
                        const cuuint32_t *box, CUtensorMapSwizzle swizzle) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return false;

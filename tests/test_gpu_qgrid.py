@@ -1,5 +1,6 @@
-"""GPU parity of the separable tensor-grid route (scatman_simulate_qgrid, sep_kernels.cu) against the oracle's direct
-triple sum at the same grid points, and against numpy.fft2 where the grid is the DFT grid."""
+"""GPU parity of the separable tensor-grid route (scatman_simulate_qgrid; tcgen05 stages of sep_tensor_kernels.cu and the
+FP32 CUDA-core stages of sep_kernels.cu) against the oracle's direct triple sum at the same grid points, and against
+numpy.fft2 where the grid is the DFT grid."""
 import numpy as np
 import pytest
 
@@ -21,6 +22,10 @@ def sm():
     s.close()
 
 
+METHODS = {"tensor": 1, "simt": 3}
+both_methods = pytest.mark.parametrize("method", list(METHODS))
+
+
 def dev(a):
     import torch
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -32,8 +37,9 @@ def _uniform_q(lam, theta_max_deg, n):
     return (np.arange(n) + 0.5 - 0.5 * n) * (2 * k * np.sin(np.radians(theta_max_deg)) / n)
 
 
+@both_methods
 @pytest.mark.parametrize("mode", [0, 1])
-def test_ragged_batch_with_orientations(sm, mode):
+def test_ragged_batch_with_orientations(sm, mode, method):
     rng = np.random.default_rng(31)
     nx, ny, nz, B = 70, 45, 11, 3
     g = np.stack([W.random_grid(81 + i, nx, ny, nz, fill=0.4) for i in range(B)])
@@ -41,47 +47,51 @@ def test_ragged_batch_with_orientations(sm, mode):
     quat[2] = [1, 0, 0, 0]
     voxel, lam = (2.0, 2.5, 3.0), 14.0
     qx, qy = _uniform_q(lam, 35.0, 37), _uniform_q(lam, 25.0, 29)
-    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), quat=quat, rho_mode=mode).cpu().numpy()
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), quat=quat, rho_mode=mode, method=METHODS[method]).cpu().numpy()
     for b in range(B):
         ref = O.simulate_qgrid(g[b], voxel, lam, qx, qy, quat=quat[b], rho_mode=mode)
-        assert_parity(I[b], ref, what=f"qgrid ragged b={b} mode={mode}")
+        assert_parity(I[b], ref, what=f"qgrid {method} ragged b={b} mode={mode}")
 
 
-def test_sparse_blobs_and_evanescent_points(sm):
+@both_methods
+def test_sparse_blobs_and_evanescent_points(sm, method):
     """Mostly empty grid (the kernels skip vacuum rows); a q grid that runs past |q_xy| = k: those points must be exactly 0."""
     g = W.sparse_blobs_grid(91, 150, 130, 9, nblobs=6, max_extent=40)
     voxel, lam = (2.0, 2.0, 2.5), 11.0
     k = 2 * np.pi / lam
     qx, qy = np.linspace(-1.2 * k, 1.2 * k, 41), np.linspace(-0.8 * k, 0.8 * k, 33)
-    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy)).cpu().numpy()
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
     ref = O.simulate_qgrid(g, voxel, lam, qx, qy)
     _, ok = O.qgrid_q(qx, qy, lam)
     assert not ok.all() and np.all(I.ravel()[~ok] == 0)
-    assert_parity(I, ref, what="qgrid sparse")
+    assert_parity(I, ref, what=f"qgrid sparse {method}")
 
 
-def test_cfg1_sphere_on_a_uniform_q_grid(sm):
+@both_methods
+def test_cfg1_sphere_on_a_uniform_q_grid(sm, method):
     w = W.config(0)
     g = w.grid(0)
     vox = (w.dx, w.dy, w.dz)
     qx = qy = _uniform_q(w.lam, w.theta_max_deg, 64)
-    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy()
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
     ref = O.simulate_qgrid(g, vox, w.lam, qx, qy)
-    assert_parity(I, ref, what="qgrid cfg1")
+    assert_parity(I, ref, what=f"qgrid cfg1 {method}")
     assert np.allclose(I, I[::-1, :], rtol=1e-4) and np.allclose(I, I.T, rtol=1e-4)   # D4 symmetry of the sphere pattern
 
 
-def test_cfg3_quarter_scale_droplet(sm):
+@both_methods
+def test_cfg3_quarter_scale_droplet(sm, method):
     w = W.config(2, scale=0.25)
     g = w.grid(0)
     vox = (w.dx, w.dy, w.dz)
     qx, qy = _uniform_q(w.lam, w.theta_max_deg, w.npx), _uniform_q(w.lam, w.theta_max_deg, w.npy)
-    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy()
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
     ref = O.simulate_qgrid(g, vox, w.lam, qx, qy)
-    assert_parity(I, ref, what="qgrid cfg3 quarter")
+    assert_parity(I, ref, what=f"qgrid cfg3 quarter {method}")
 
 
-def test_single_slice_on_the_dft_grid_is_fft2(sm):
+@both_methods
+def test_single_slice_on_the_dft_grid_is_fft2(sm, method):
     rng = np.random.default_rng(33)
     nx, ny, d = 96, 80, 1.5
     g = np.zeros((1, ny, nx, 2), np.float32)
@@ -91,24 +101,25 @@ def test_single_slice_on_the_dft_grid_is_fft2(sm):
     mx, my = np.arange(nx), np.arange(ny)
     qx = -2 * np.pi * np.where(mx < nx / 2, mx, mx - nx) / (nx * d)
     qy = -2 * np.pi * np.where(my < ny / 2, my, my - ny) / (ny * d)
-    I = sm.simulate_qgrid(dev(g), (d, d, 2.0), lam, dev(qx), dev(qy)).cpu().numpy()
+    I = sm.simulate_qgrid(dev(g), (d, d, 2.0), lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
     rho = g[0, ..., 0].astype(np.float64) + 1j * g[0, ..., 1].astype(np.float64)
     ref = np.abs(np.fft.fft2(rho) * d * d * 2.0) ** 2
-    assert_parity(I, ref, what="qgrid fft2")
+    assert_parity(I, ref, what=f"qgrid fft2 {method}")
 
 
-def test_full_size_cfg3_sampled_points(sm):
+@both_methods
+def test_full_size_cfg3_sampled_points(sm, method):
     """256^3 droplet on a 512 x 512 uniform q grid, checked at seeded grid points (the oracle takes them one by one)."""
     w = W.config(2)
     g = w.grid(0)
     vox = (w.dx, w.dy, w.dz)
     qx, qy = _uniform_q(w.lam, w.theta_max_deg, w.npx), _uniform_q(w.lam, w.theta_max_deg, w.npy)
-    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy)).cpu().numpy().ravel()
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy().ravel()
     q, ok = O.qgrid_q(qx, qy, w.lam)
     c = w.npy // 2 * w.npx + w.npx // 2
     pix = W.sample_pixels(w.seed + 7, w.npix, 160, always=[int(np.argmax(I)), c, c - 1, c - w.npx])
     ref = O.simulate_q(g, vox, w.lam, q[pix]) * ok[pix]
-    assert_parity(I[pix], ref, what="qgrid cfg3 full sampled")
+    assert_parity(I[pix], ref, what=f"qgrid cfg3 full sampled {method}")
 
 
 def test_error_codes(sm):
