@@ -439,7 +439,7 @@ struct SepPlan {
     bool tensor = true;   // both GEMM stages on tcgen05 (method AUTO / TENSOR) or FP32 CUDA cores (SIMT_TABLE)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, off_eyp = 0, off_hp = 0, off_scale = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
                              int num_sms) {
@@ -448,7 +448,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
     p.npix = (int64_t)npx * npy; p.batch = batch; p.rho_mode = rho_mode;
     p.nvox = (int64_t)g.nx * g.ny * g.nz;
-    sp.tensor = method != SCATMAN_METHOD_SIMT_TABLE;
+    sp.tensor = method != SCATMAN_METHOD_SIMT_TABLE && g.nx <= 1024;   // stage X keeps an Ex tile of >= 16 columns resident
     sp.nzs = sep_zsplit(p, npx, npy, num_sms);
     if (sp.tensor) sp.tc = make_sep_tc_plan(p, npx, npy, num_sms);
     size_t off = 0;
@@ -458,15 +458,17 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
-    sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
         sp.off_eyp = take(sizeof(__half) * 4 * (size_t)t.NPYP * t.NY);
+        sp.off_exp = take(sizeof(__half) * 4 * (size_t)t.NPXP * t.NXP);
+        sp.off_rp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NY * t.NXP);
         sp.off_hp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NPXP * t.NY);
         sp.off_flags = take((size_t)g.nz * (t.NY / 64));
         sp.off_scale = take(sizeof(float) * 2);
         sp.off_partial = take(sizeof(float2) * (size_t)t.nsplit * npx * npy);
     } else {
+        sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
         sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
         sp.off_h = take(sizeof(float2) * (size_t)g.nz * g.ny * npx);
         sp.off_flags = take((size_t)g.nz * ((g.ny + 15) / 16));
@@ -526,22 +528,20 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     e = launch_strength(src, p, batch, rho, maxbits, st);
     ++nl;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
-    float2 *Ex = (float2 *)(ws + sp.off_ex), *Ey = (float2 *)(ws + sp.off_ey);
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
-        __half *Eyp = (__half *)(ws + sp.off_eyp), *Hp = (__half *)(ws + sp.off_hp);
+        __half *Eyp = (__half *)(ws + sp.off_eyp), *Exp = (__half *)(ws + sp.off_exp), *Rp = (__half *)(ws + sp.off_rp),
+               *Hp = (__half *)(ws + sp.off_hp);
         float *scaleH = (float *)(ws + sp.off_scale), *ampscale = scaleH + 1;
-        e = launch_sep_tables(d_qx, npx, nullptr, 0, p, Ex, nullptr, st);
-        if (e == cudaSuccess) e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, nullptr, Eyp, st);
+        e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, Exp, Eyp, st);
         nl += 2;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
         cudaEventRecord(ctx->ev0, st);
         for (int b = 0; b < batch; ++b) {
             const float2 *rho_b = (const float2 *)rho + (size_t)b * p.nvox;
             std::string err;
-            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, ws + sp.off_flags, scaleH, ampscale, st);
-            if (e == cudaSuccess)
-                e = launch_sep_stage_x_planes(rho_b, Ex, p, npx, t.NY, t.NPXP, ws + sp.off_flags, scaleH, Hp, st);
+            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, Rp, ws + sp.off_flags, scaleH, ampscale, st);
+            if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, Hp, ctx->num_sms, st, &err);
             if (e == cudaSuccess)
                 e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, d_qx, npx, d_qy, npy, (float2 *)(ws + sp.off_partial),
                                      ctx->num_sms, st, &err);
@@ -552,6 +552,7 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
             if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "qgrid stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         }
     } else {
+        float2 *Ex = (float2 *)(ws + sp.off_ex), *Ey = (float2 *)(ws + sp.off_ey);
         e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
         nl += 2;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");

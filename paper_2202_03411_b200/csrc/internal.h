@@ -75,14 +75,16 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
 struct SepTcPlan {
     int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
     int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
+    int NX = 64, nsx = 1;                      // stage X: a columns per tile, z splits
 };
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
 cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    unsigned char *d_flags64, float *d_scaleH, float *d_ampscale, cudaStream_t st);
-cudaError_t launch_sep_stage_x_planes(const float2 *d_rho, const float2 *d_Ex, const Plan &p, int npx, int NY, int NPXP,
-                                      const unsigned char *d_flags64, const float *d_scaleH, __half *d_Hp, cudaStream_t st);
+                                    __half *d_Rp, unsigned char *d_flags64, float *d_scaleH, float *d_ampscale,
+                                    cudaStream_t st);
+cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
+                            const unsigned char *d_flags64, __half *d_Hp, int num_sms, cudaStream_t st, std::string *err);
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
                              const unsigned char *d_flags64, const double *d_qx, int npx, const double *d_qy, int npy,
                              float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);

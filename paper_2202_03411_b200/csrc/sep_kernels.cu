@@ -153,59 +153,6 @@ __global__ void __launch_bounds__(256) sep_stage_x_kernel(const float2 *__restri
         }
 }
 
-// stage X for the tensor-core stage YZ (sep_tensor_kernels.cu): the same FP32 GEMM per (slice, 64-y block, 64-a tile), but H
-// leaves as the FP16 planes stage YZ's TMA boxes read: Hp[plane][j][a][y] = split(sH * H_j[y, a]), y fastest (K-major).
-// Blocks whose flag is 0 (vacuum) are neither computed nor written: stage YZ never reads them.
-__global__ void __launch_bounds__(256) sep_stage_x_planes_kernel(const float2 *__restrict__ rho, const float2 *__restrict__ Ex,
-                                                                 int nx, int ny, int nz, int npx, int NY, int NPXP,
-                                                                 const unsigned char *__restrict__ flags64,
-                                                                 const float *__restrict__ scaleH, __half *__restrict__ Hp) {
-    __shared__ TileSmem sm;
-    const int nyb = NY / 64;
-    const int j = blockIdx.x / nyb, yb = blockIdx.x % nyb;
-    if (flags64[blockIdx.x] == 0) return;
-    const int n0 = blockIdx.y * kBN;
-    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
-    float2 acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int jj = 0; jj < 4; ++jj) acc[i][jj] = make_float2(0.f, 0.f);
-    tile_gemm(rho + (size_t)j * ny * nx, nx, ny, yb * 64, Ex, npx, npx, n0, nx, nullptr, sm, acc);
-    const float s = scaleH[0];
-    const size_t plane = (size_t)nz * NPXP * NY;
-    const int y0 = yb * 64 + ty * 4;
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) {
-        const int a = n0 + tx * 4 + jj;
-        unsigned short h[4][4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const float re = acc[i][jj].x * s, im = acc[i][jj].y * s;
-            const __half rh = __float2half_rn(re), ih = __float2half_rn(im);
-            h[0][i] = __half_as_ushort(rh);
-            h[1][i] = __half_as_ushort(__float2half_rn(re - __half2float(rh)));
-            h[2][i] = __half_as_ushort(ih);
-            h[3][i] = __half_as_ushort(__float2half_rn(im - __half2float(ih)));
-        }
-        const size_t o = ((size_t)j * NPXP + a) * NY + y0;
-#pragma unroll
-        for (int pl = 0; pl < 4; ++pl) {
-            uint2 w;
-            w.x = (uint32_t)h[pl][0] | ((uint32_t)h[pl][1] << 16);
-            w.y = (uint32_t)h[pl][2] | ((uint32_t)h[pl][3] << 16);
-            *(uint2 *)(Hp + pl * plane + o) = w;
-        }
-    }
-}
-
-cudaError_t launch_sep_stage_x_planes(const float2 *d_rho, const float2 *d_Ex, const Plan &p, int npx, int NY, int NPXP,
-                                      const unsigned char *d_flags64, const float *d_scaleH, __half *d_Hp, cudaStream_t st) {
-    dim3 grid((unsigned)(p.nz * (NY / 64)), (unsigned)(NPXP / kBN));
-    sep_stage_x_planes_kernel<<<grid, 256, 0, st>>>(d_rho, d_Ex, p.nx, p.ny, p.nz, npx, NY, NPXP, d_flags64, d_scaleH, d_Hp);
-    return cudaGetLastError();
-}
-
 // stage YZ: partial[zs][b * npx + a] = sum over this z range of e^{i qz z_j} sum_y Ey[b][y] H[j][y][a].
 // qz in turns per unit length: qzt = qz / 2pi, so the phase of slice j is sincospi(2 frac(qzt z_j)) with the reduction in FP64.
 __global__ void __launch_bounds__(256, 2) sep_stage_yz_kernel(const float2 *__restrict__ Ey, const float2 *__restrict__ H,
@@ -455,7 +402,7 @@ cudaError_t launch_sep_tables(const double *d_qx, int npx, const double *d_qy, i
                               float2 *d_Ey, cudaStream_t st) {
     const int64_t nxe = (int64_t)npx * p.nx, nye = (int64_t)npy * p.ny;
     sep_table_kernel<<<(unsigned)((nxe + 255) / 256), 256, 0, st>>>(d_qx, npx, p.nx, p.dx, 0, d_Ex);   // Ex[x][a]
-    if (d_Ey) sep_table_kernel<<<(unsigned)((nye + 255) / 256), 256, 0, st>>>(d_qy, npy, p.ny, p.dy, 1, d_Ey);   // Ey[b][y]
+    sep_table_kernel<<<(unsigned)((nye + 255) / 256), 256, 0, st>>>(d_qy, npy, p.ny, p.dy, 1, d_Ey);   // Ey[b][y]
     return cudaGetLastError();
 }
 

@@ -76,24 +76,250 @@ __global__ void sep_tc_scale_kernel(const unsigned *__restrict__ maxbits, int L,
     ampscale[0] = dV / (kScaleA * sH);
 }
 
-// flags64[j][yb] = 1 if any rho~ of slice j, y in [64 yb, 64 yb + 64) is non-zero (one warp per block)
-__global__ void sep_tc_flags_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int nyb,
-                                    unsigned char *__restrict__ flags) {
-    const int blk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (blk >= nz * nyb) return;
-    const int j = blk / nyb, yb = blk % nyb;
-    const int y0 = yb * kKB, y1 = min(ny, y0 + kKB);
+// rho~ FP32 [nz][ny][nx] -> planes fp16 [4][nz * NY][NXP] = split(sR rho~), x fastest (K-major for stage X), zero in the
+// padding; sR = 2^(13 - e) as in pack_b_kernel.  Also raises flags64[j][y / 64] for every 64-y block holding a non-zero value
+// (flags are cleared by a memset before).  One thread = 8 consecutive x of one row.
+__global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int NY, int NXP,
+                                       const unsigned *__restrict__ maxbits, __half *__restrict__ R,
+                                       unsigned char *__restrict__ flags) {
+    const int nx8 = NXP / 8;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)nz * NY * nx8) return;
+    const int x0 = (int)(t % nx8) * 8;
+    const int64_t row = t / nx8;
+    const int y = (int)(row % NY), j = (int)(row / NY);
+    const float m = __uint_as_float(maxbits[0]);
+    int e = 0;
+    if (m > 0.f) frexpf(m, &e);
+    const float s = ldexpf(1.f, kScaleBExp - e);
+    __align__(16) __half h[4][8];
     bool any = false;
-    if (y0 < ny) {
-        const float2 *src = rho + ((size_t)j * ny + y0) * nx;
-        const size_t n = (size_t)(y1 - y0) * nx;
-        for (size_t e = lane; e < n; e += 32) {
-            const float2 v = __ldg(src + e);
-            any |= (v.x != 0.f) | (v.y != 0.f);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        float2 v = make_float2(0.f, 0.f);
+        if (y < ny && x0 + i < nx) v = __ldg(rho + ((size_t)j * ny + y) * nx + x0 + i);
+        any |= (v.x != 0.f) | (v.y != 0.f);
+        __half q[4];
+        split4(v.x * s, v.y * s, q);
+#pragma unroll
+        for (int pl = 0; pl < 4; ++pl) h[pl][i] = q[pl];
+    }
+    const size_t plane = (size_t)nz * NY * NXP, o = (size_t)row * NXP + x0;
+#pragma unroll
+    for (int pl = 0; pl < 4; ++pl) *(uint4 *)(R + pl * plane + o) = *(const uint4 *)h[pl];
+    if (any) flags[(size_t)j * (NY / kKB) + y / kKB] = 1;
+}
+
+// ------------------------------------------------------------------------------------------------ stage X
+struct SepXParams {
+    int nz, NY, NPXP, ng, nkx, nta, nsx, nkb;   // nkx = NXP / 64, nta = a tiles of NX columns, nsx = z splits, nkb = NY / 64
+    float hscale;                               // 2^(-9 - L): accumulator (2^10 sR H) -> stored H (sH H)
+    const unsigned char *flags;                 // [nz][nkb]
+    __half *Hp;                                 // [4][nz][NPXP][NY]
+};
+
+// NX = a columns per accumulator = rows of the resident Ex tile (NX * NXP * 8 bytes <= 128 KB)
+template <int NX>
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepXParams P) {
+    constexpr int kSmemE = 131072;                // resident Ex planes: [4][nkx][NX rows x 128 bytes]
+    constexpr int kStages = 6;                    // ring of single-plane 64-x blocks of a rho~ row tile (16 KB each)
+    constexpr int kBlkE = NX * kKB * 2;           // bytes of one plane, one K block of the Ex tile
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sE = smem;
+    uint8_t *sR = smem + kSmemE;
+    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kSlotA);
+    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
+    uint64_t *r_full = bars + 2, *r_empty = r_full + kStages;
+    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNBuf;
+    uint32_t *tmem_ptr = (uint32_t *)(t_empty + kNBuf);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nitems = P.nta * P.nsx;
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(e_full, 1);
+        ptx::mbar_init(e_empty, 1);
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(r_full + i, 1);
+            ptx::mbar_init(r_empty + i, 1);
+        }
+        for (int i = 0; i < kNBuf; ++i) {
+            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_empty + i, 8);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    // units of an item: (slice j of its z range, 128-y group g) with a non-empty 64-y block; u = (j - z0) * ng + g
+    auto zrange = [&](int s, int &z0, int &z1) {
+        z0 = (int)(((long long)P.nz * s) / P.nsx);
+        z1 = (int)(((long long)P.nz * (s + 1)) / P.nsx);
+    };
+    auto live = [&](int j, int g) {
+        const unsigned char *fl = P.flags + (size_t)j * P.nkb + g * 2;
+        return (__ldg(fl) | __ldg(fl + 1)) != 0;
+    };
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const int ta = item % P.nta, s = item / P.nta;   // a tiles fastest: concurrent CTAs stream the same rho~ tiles
+            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
+                ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(4 * P.nkx * kBlkE));
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int kx = 0; kx < P.nkx; ++kx)
+                        ptx::tma_load_3d(sE + (pl * P.nkx + kx) * kBlkE, &tmB, e_full, kx * kKB, ta * NX, pl);
+            }
+            __syncwarp();
+            int z0, z1;
+            zrange(s, z0, z1);
+            for (int j = z0; j < z1; ++j)
+                for (int g = 0; g < P.ng; ++g) {
+                    if (!live(j, g)) continue;
+                    for (int kx = 0; kx < P.nkx; ++kx)
+                        for (int pl = 0; pl < 4; ++pl) {
+                            ptx::mbar_wait(r_empty + slot, phase ^ 1);
+                            if (ptx::elect_one()) {
+                                ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)kSlotA);
+                                ptx::tma_load_3d(sR + slot * kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, pl);
+                            }
+                            __syncwarp();
+                            if (++slot == kStages) { slot = 0; phase ^= 1; }
+                        }
+                }
+        }
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, NX, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, NX, true);
+        const uint64_t descR0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sR));
+        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
+        constexpr uint64_t kR = kSlotA >> 4, kE = kBlkE >> 4;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const int s = item / P.nta;
+            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
+            ptx::tc_fence_after();
+            const uint64_t kEpl = (uint64_t)P.nkx * kE;   // descriptor distance between Ex planes
+            int z0, z1;
+            zrange(s, z0, z1);
+            for (int j = z0; j < z1; ++j)
+                for (int g = 0; g < P.ng; ++g) {
+                    if (!live(j, g)) continue;
+                    const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
+                    ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                    ptx::tc_fence_after();
+                    const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
+                    for (int kx = 0; kx < P.nkx; ++kx)
+                        for (int pl = 0; pl < 4; ++pl) {
+                            ptx::mbar_wait(r_full + slot, phase);
+                            ptx::tc_fence_after();
+                            if (ptx::elect_one()) {
+#pragma unroll
+                                for (int ks = 0; ks < 4; ++ks) {
+                                    const uint64_t a = descR0 + (uint64_t)slot * kR + (uint64_t)(ks * 2);
+                                    const uint64_t e_reh = descE0 + (uint64_t)kx * kE + (uint64_t)(ks * 2);
+                                    const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
+                                    const uint32_t acc0 = (kx == 0 && ks == 0) ? 0u : 1u;
+                                    // (Ar + i Ai)(Er + i Ei), A = rho~ plane of this stage, three split products AhEh + AlEh + AhEl
+                                    if (pl == 0) {          // Re_hi
+                                        ptx::umma_f16(d_re, a, e_reh, idesc_pos, acc0);
+                                        ptx::umma_f16(d_im, a, e_imh, idesc_pos, acc0);
+                                        ptx::umma_f16(d_re, a, e_rel, idesc_pos, 1u);
+                                        ptx::umma_f16(d_im, a, e_iml, idesc_pos, 1u);
+                                    } else if (pl == 1) {   // Re_lo
+                                        ptx::umma_f16(d_re, a, e_reh, idesc_pos, 1u);
+                                        ptx::umma_f16(d_im, a, e_imh, idesc_pos, 1u);
+                                    } else if (pl == 2) {   // Im_hi
+                                        ptx::umma_f16(d_re, a, e_imh, idesc_neg, 1u);
+                                        ptx::umma_f16(d_im, a, e_reh, idesc_pos, 1u);
+                                        ptx::umma_f16(d_re, a, e_iml, idesc_neg, 1u);
+                                        ptx::umma_f16(d_im, a, e_rel, idesc_pos, 1u);
+                                    } else {                // Im_lo
+                                        ptx::umma_f16(d_re, a, e_imh, idesc_neg, 1u);
+                                        ptx::umma_f16(d_im, a, e_reh, idesc_pos, 1u);
+                                    }
+                                }
+                                ptx::umma_commit(r_empty + slot);
+                            }
+                            __syncwarp();
+                            if (++slot == kStages) { slot = 0; phase ^= 1; }
+                        }
+                    if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                    __syncwarp();
+                    ++u;
+                }
+            if (ptx::elect_one()) ptx::umma_commit(e_empty);
+            __syncwarp();
+        }
+    } else if (warp >= 4) {
+        // ===================================================================== epilogue: H -> FP16 planes [j][a][y]
+        constexpr int kCols = NX / 2;                    // columns of this warp's half
+        const int lg = warp & 3, ch = (warp - 4) >> 2;
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * kCols);
+        const size_t plane = (size_t)P.nz * P.NPXP * P.NY;
+        uint32_t u = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            const int ta = item % P.nta, s = item / P.nta;
+            const int a0 = ta * NX + ch * kCols;
+            int z0, z1;
+            zrange(s, z0, z1);
+            for (int j = z0; j < z1; ++j)
+                for (int g = 0; g < P.ng; ++g) {
+                    if (!live(j, g)) continue;
+                    const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
+                    ptx::mbar_wait(t_full + buf, upar);
+                    ptx::tc_fence_after();
+                    const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
+                    __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
+#pragma unroll 1
+                    for (int c0 = 0; c0 < kCols; c0 += 8) {
+                        uint32_t gre[8], gim[8];
+                        ptx::tmem_ld8(t_re + c0, gre);
+                        ptx::tmem_ld8(t_im + c0, gim);
+                        ptx::tmem_ld_wait();
+                        if (c0 + 8 >= kCols) {
+                            ptx::tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            __half h[4];
+                            split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
+                            __half *d = dst + (size_t)(c0 + i) * P.NY;
+#pragma unroll
+                            for (int pl = 0; pl < 4; ++pl) d[pl * plane] = h[pl];
+                        }
+                    }
+                    ++u;
+                }
         }
     }
-    any = __any_sync(0xffffffffu, any);
-    if (lane == 0) flags[blk] = any ? 1 : 0;
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ stage YZ
@@ -393,6 +619,11 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     }
     t.nzs = best;
     t.nsplit = t.ng * t.nzs;
+    // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for ~4 waves of a-tile items
+    t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
+    const int nta = t.NPXP / t.NX;
+    int nsx = (4 * num_sms + nta - 1) / nta;
+    t.nsx = nsx < 1 ? 1 : nsx > p.nz ? p.nz : nsx;
     return t;
 }
 
@@ -400,7 +631,8 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st) {
     const int64_t nye = (int64_t)t.NPYP * t.NY;
     sep_tc_table_kernel<<<(unsigned)((nye + 255) / 256), 256, 0, st>>>(d_qy, npy, t.NPYP, p.ny, t.NY, p.dy, d_Eyp);
-    (void)d_qx; (void)npx; (void)d_Exp;
+    const int64_t nxe = (int64_t)t.NPXP * t.NXP;
+    sep_tc_table_kernel<<<(unsigned)((nxe + 255) / 256), 256, 0, st>>>(d_qx, npx, t.NPXP, p.nx, t.NXP, p.dx, d_Exp);
     return cudaGetLastError();
 }
 
@@ -445,11 +677,64 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 }
 
 cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    unsigned char *d_flags64, float *d_scaleH, float *d_ampscale, cudaStream_t st) {
+                                    __half *d_Rp, unsigned char *d_flags64, float *d_scaleH, float *d_ampscale,
+                                    cudaStream_t st) {
     const int nyb = t.NY / kKB;
-    sep_tc_flags_kernel<<<(unsigned)((p.nz * nyb + 7) / 8), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nyb, d_flags64);
+    cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)p.nz * nyb, st);
+    if (e != cudaSuccess) return e;
+    const int64_t nthreads = (int64_t)p.nz * t.NY * (t.NXP / 8);
+    sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, t.NY, t.NXP, d_maxbits,
+                                                                             d_Rp, d_flags64);
     sep_tc_scale_kernel<<<1, 1, 0, st>>>(d_maxbits, t.L, (float)(p.dx * p.dy * p.dz), d_scaleH, d_ampscale);
     return cudaGetLastError();
+}
+
+template <int NX>
+static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
+                                    cudaStream_t st) {
+    constexpr int kSmem = 1024 + 131072 + 6 * kSlotA + 256;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sep_tc_x_kernel<NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int nitems = P.nta * P.nsx;
+    sep_tc_x_kernel<NX><<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
+                            const unsigned char *d_flags64, __half *d_Hp, int num_sms, cudaStream_t st, std::string *err) {
+    CUtensorMap tmA, tmB;
+    bool ok;
+    {
+        const cuuint64_t rows = (cuuint64_t)p.nz * t.NY;
+        cuuint64_t dims[3] = {(cuuint64_t)t.NXP, rows, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * rows * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
+        ok = encode_map(&tmA, d_Rp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+    if (ok) {
+        cuuint64_t dims[3] = {(cuuint64_t)t.NXP, (cuuint64_t)t.NPXP, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * (cuuint64_t)t.NPXP * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)t.NX, 1};
+        ok = encode_map(&tmB, d_Exp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
+    if (!ok) {
+        if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
+        return cudaErrorUnknown;
+    }
+    SepXParams P;
+    P.nz = p.nz; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / t.NX; P.nsx = t.nsx;
+    P.nkb = t.NY / kKB;
+    P.hscale = ldexpf(1.f, -9 - t.L);
+    P.flags = d_flags64; P.Hp = d_Hp;
+    switch (t.NX) {
+        case 64: return launch_x_variant<64>(tmA, tmB, P, num_sms, st);
+        case 32: return launch_x_variant<32>(tmA, tmB, P, num_sms, st);
+        default: return launch_x_variant<16>(tmA, tmB, P, num_sms, st);
+    }
 }
 
 cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,

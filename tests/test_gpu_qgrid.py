@@ -67,6 +67,17 @@ def test_sparse_blobs_and_evanescent_points(sm, method):
     assert_parity(I, ref, what=f"qgrid sparse {method}")
 
 
+@pytest.mark.parametrize("nx", [300, 530, 1100])
+def test_wide_grids_use_narrower_stage_x_tiles(sm, nx):
+    """nx > 256 / > 512: stage X keeps 32- / 16-column Ex tiles resident; nx > 1024 falls back to the CUDA-core stages."""
+    g = W.random_grid(97, nx, 20, 3, fill=0.5)
+    voxel, lam = (1.5, 2.0, 2.5), 9.0
+    qx, qy = _uniform_q(lam, 20.0, 70), _uniform_q(lam, 30.0, 19)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS["tensor"]).cpu().numpy()
+    ref = O.simulate_qgrid(g, voxel, lam, qx, qy)
+    assert_parity(I, ref, what=f"qgrid tensor nx={nx}")
+
+
 @both_methods
 def test_cfg1_sphere_on_a_uniform_q_grid(sm, method):
     w = W.config(0)
