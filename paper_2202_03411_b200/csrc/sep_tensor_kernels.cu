@@ -28,7 +28,7 @@ constexpr int kM = 128;              // UMMA M: rows of the A operand tile
 constexpr int kKB = 64;              // K per block (one 128-byte swizzle row of FP16)
 constexpr int kSlotA = kM * kKB * 2; // 16384: one plane, one K block of an A tile
 constexpr int kNyz = 64;             // stage YZ: a columns per accumulator
-constexpr int kThreadsTc = 384;      // warp 0 TMA, 1 MMA, 2 TMEM, 3 idle, 4-11 epilogue
+constexpr int kThreadsTc = 384;      // warp 0 TMA, 1 and 3 MMA issuers, 2 TMEM, 4-11 epilogue
 constexpr uint32_t kTmemColsTc = 512;
 constexpr int kNBuf = 4;             // accumulator buffers (128 columns each: D_re 64 + D_im 64)
 
@@ -40,6 +40,44 @@ __device__ __forceinline__ void split4(float re, float im, __half (&h)[4]) {
     h[2] = __float2half_rn(im);
     h[3] = __float2half_rn(im - __half2float(h[2]));
 }
+
+// The live units of a work item in issue order.  Unit n of the item is (slice z0 + n / ngw, 128-y group g0 + n % ngw); its two
+// flag bytes say which of its 64-y blocks hold anything.  Warp-cooperative like tensor_kernel.cu's Units: each lane holds the
+// flags of one of 32 consecutive units (the next 32 are already in flight), a ballot finds the next live one -- one L2 round
+// trip per 32 units instead of one per unit in the critical path of every role.
+struct LiveUnits {
+    const unsigned char *fl;
+    int nkb, z0, ngw, g0, total, base, lane;
+    uint32_t cur, ahead, live;
+    __device__ __forceinline__ uint32_t load(int n) const {
+        if (n >= total) return 0u;
+        const unsigned char *p = fl + (size_t)(z0 + n / ngw) * nkb + 2 * (g0 + n % ngw);
+        return (uint32_t)__ldg(p) | ((uint32_t)__ldg(p + 1) << 1);
+    }
+    __device__ __forceinline__ void begin(const unsigned char *flags, int nkb_, int z0_, int z1, int ngw_, int g0_, int lane_) {
+        fl = flags; nkb = nkb_; z0 = z0_; ngw = ngw_; g0 = g0_; lane = lane_;
+        total = (z1 - z0_) * ngw_;
+        base = 0;
+        cur = load(lane);
+        ahead = load(32 + lane);
+        live = __ballot_sync(0xffffffffu, cur != 0u);
+    }
+    // next live unit: n = its index in the item, f = bit 0 / 1: first / second 64-y block non-empty; false at the end
+    __device__ __forceinline__ bool next(int &n, uint32_t &f) {
+        while (live == 0u) {
+            base += 32;
+            if (base >= total) return false;
+            cur = ahead;
+            ahead = load(base + 32 + lane);
+            live = __ballot_sync(0xffffffffu, cur != 0u);
+        }
+        const int pos = __ffs((int)live) - 1;
+        live &= live - 1;
+        f = __shfl_sync(0xffffffffu, cur, pos);
+        n = base + pos;
+        return true;
+    }
+};
 
 }  // namespace
 
@@ -132,8 +170,8 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kSlotA);
     uint64_t *e_full = bars + 0, *e_empty = bars + 1;
     uint64_t *r_full = bars + 2, *r_empty = r_full + kStages;
-    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNBuf;
-    uint32_t *tmem_ptr = (uint32_t *)(t_empty + kNBuf);
+    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNBuf, *first_done = t_empty + kNBuf;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNBuf);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nitems = P.nta * P.nsx;
@@ -144,14 +182,15 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
     if (warp == 1 && lane == 0) {
         ptx::mbar_init(e_full, 1);
-        ptx::mbar_init(e_empty, 1);
+        ptx::mbar_init(e_empty, 2);          // both MMA issuers
         for (int i = 0; i < kStages; ++i) {
             ptx::mbar_init(r_full + i, 1);
-            ptx::mbar_init(r_empty + i, 1);
+            ptx::mbar_init(r_empty + i, 2);
         }
         for (int i = 0; i < kNBuf; ++i) {
-            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_full + i, 2);
             ptx::mbar_init(t_empty + i, 8);
+            ptx::mbar_init(first_done + i, 1);
         }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
@@ -166,10 +205,6 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     auto zrange = [&](int s, int &z0, int &z1) {
         z0 = (int)(((long long)P.nz * s) / P.nsx);
         z1 = (int)(((long long)P.nz * (s + 1)) / P.nsx);
-    };
-    auto live = [&](int j, int g) {
-        const unsigned char *fl = P.flags + (size_t)j * P.nkb + g * 2;
-        return (__ldg(fl) | __ldg(fl + 1)) != 0;
     };
 
     if (warp == 0) {
@@ -189,28 +224,40 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             __syncwarp();
             int z0, z1;
             zrange(s, z0, z1);
-            for (int j = z0; j < z1; ++j)
-                for (int g = 0; g < P.ng; ++g) {
-                    if (!live(j, g)) continue;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                    const int j = z0 + n / P.ng, g = n % P.ng;
                     for (int kx = 0; kx < P.nkx; ++kx)
                         for (int pl = 0; pl < 4; ++pl) {
                             ptx::mbar_wait(r_empty + slot, phase ^ 1);
                             if (ptx::elect_one()) {
+#ifdef SEPABL_X_NOLOAD   // debug-only ablation (built by _work scripts; never in the product build)
+                                ptx::mbar_arrive(r_full + slot);
+#else
                                 ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)kSlotA);
                                 ptx::tma_load_3d(sR + slot * kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, pl);
+#endif
                             }
                             __syncwarp();
                             if (++slot == kStages) { slot = 0; phase ^= 1; }
                         }
                 }
         }
-    } else if (warp == 1) {
-        // ===================================================================== MMA issuer
+    } else if (warp == 1 || warp == 3) {
+        // ===================================================================== MMA issuers
+        // Two issuer warps share every stage: k-step ks belongs to issuer ks % 2.  At N = 64 a tcgen05.mma is bound by its
+        // shared-memory operand fetch (48 cycles) and a single issuing thread exposes whatever it spends between stages
+        // (measured 72-107 cycles per MMA with one issuer); two threads hide each other's gaps (as in tensor_kernel.cu).
+        // The unit's first k-step (accumulate = 0) is issuer 0's; issuer 1 starts on the unit once it has completed.
         constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, NX, false);
         constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, NX, true);
         const uint64_t descR0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sR));
         const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
         constexpr uint64_t kR = kSlotA >> 4, kE = kBlkE >> 4;
+        const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
@@ -221,20 +268,27 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             const uint64_t kEpl = (uint64_t)P.nkx * kE;   // descriptor distance between Ex planes
             int z0, z1;
             zrange(s, z0, z1);
-            for (int j = z0; j < z1; ++j)
-                for (int g = 0; g < P.ng; ++g) {
-                    if (!live(j, g)) continue;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
                     const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                     ptx::mbar_wait(t_empty + buf, upar ^ 1);
                     ptx::tc_fence_after();
                     const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
                     for (int kx = 0; kx < P.nkx; ++kx)
                         for (int pl = 0; pl < 4; ++pl) {
+                            if (iw == 1 && kx == 0 && pl == 0) {   // D must have been initialised by issuer 0
+                                ptx::mbar_wait(first_done + buf, upar);
+                                ptx::tc_fence_after();
+                            }
                             ptx::mbar_wait(r_full + slot, phase);
                             ptx::tc_fence_after();
                             if (ptx::elect_one()) {
 #pragma unroll
-                                for (int ks = 0; ks < 4; ++ks) {
+                                for (int kk = 0; kk < 2; ++kk) {
+                                    const int ks = 2 * kk + iw;
                                     const uint64_t a = descR0 + (uint64_t)slot * kR + (uint64_t)(ks * 2);
                                     const uint64_t e_reh = descE0 + (uint64_t)kx * kE + (uint64_t)(ks * 2);
                                     const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
@@ -257,6 +311,7 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                                         ptx::umma_f16(d_re, a, e_imh, idesc_neg, 1u);
                                         ptx::umma_f16(d_im, a, e_reh, idesc_pos, 1u);
                                     }
+                                    if (iw == 0 && kk == 0 && kx == 0 && pl == 0) ptx::umma_commit(first_done + buf);
                                 }
                                 ptx::umma_commit(r_empty + slot);
                             }
@@ -282,14 +337,25 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             const int a0 = ta * NX + ch * kCols;
             int z0, z1;
             zrange(s, z0, z1);
-            for (int j = z0; j < z1; ++j)
-                for (int g = 0; g < P.ng; ++g) {
-                    if (!live(j, g)) continue;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                    const int j = z0 + n / P.ng, g = n % P.ng;
                     const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                     ptx::mbar_wait(t_full + buf, upar);
                     ptx::tc_fence_after();
                     const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
                     __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
+#ifdef SEPABL_X_NOEPI
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                    ++u;
+                    if (dst == nullptr) *dst = __float2half(0.f);
+                    continue;
+#endif
 #pragma unroll 1
                     for (int c0 = 0; c0 < kCols; c0 += 8) {
                         uint32_t gre[8], gim[8];
@@ -357,8 +423,8 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kStageB);
     uint64_t *a_full = bars + 0, *a_empty = bars + 1;
     uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
-    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNBuf;
-    uint32_t *tmem_ptr = (uint32_t *)(t_empty + kNBuf);
+    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNBuf, *first_done = t_empty + kNBuf;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNBuf);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nitems = P.ntb * P.nta * P.ng * P.nzs;
@@ -369,14 +435,15 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     }
     if (warp == 1 && lane == 0) {
         ptx::mbar_init(a_full, 1);
-        ptx::mbar_init(a_empty, 1);
+        ptx::mbar_init(a_empty, 2);          // both MMA issuers
         for (int i = 0; i < kStages; ++i) {
             ptx::mbar_init(b_full + i, 1);
-            ptx::mbar_init(b_empty + i, 1);
+            ptx::mbar_init(b_empty + i, 2);
         }
         for (int i = 0; i < kNBuf; ++i) {
-            ptx::mbar_init(t_full + i, 1);
+            ptx::mbar_init(t_full + i, 2);
             ptx::mbar_init(t_empty + i, 8);
+            ptx::mbar_init(first_done + i, 1);
         }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
@@ -409,29 +476,38 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             __syncwarp();
             int z0, z1;
             zrange(it.s, z0, z1);
-            for (int j = z0; j < z1; ++j) {
-                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                const int j = z0 + n;
                 for (int kb = 0; kb < 2; ++kb) {
-                    if (__ldg(fl + kb) == 0) continue;
+                    if (((f >> kb) & 1u) == 0u) continue;
                     ptx::mbar_wait(b_empty + slot, phase ^ 1);
                     if (ptx::elect_one()) {
+#ifdef SEPABL_YZ_NOLOAD
+                        ptx::mbar_arrive(b_full + slot);
+#else
                         ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kStageB);
                         for (int pl = 0; pl < 4; ++pl)
                             ptx::tma_load_3d(sB + slot * kStageB + pl * (kStageB / 4), &tmB, b_full + slot,
                                              (it.g * 2 + kb) * kKB, j * P.NPXP + it.ta * kNyz, pl);
+#endif
                     }
                     __syncwarp();
                     if (++slot == kStages) { slot = 0; phase ^= 1; }
                 }
             }
         }
-    } else if (warp == 1) {
-        // ===================================================================== MMA issuer
+    } else if (warp == 1 || warp == 3) {
+        // ===================================================================== MMA issuers (k-step ks belongs to issuer ks % 2)
         constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, kNyz, false);
         constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, kNyz, true);
         const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
         const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
         constexpr uint64_t kA = kSlotA >> 4, kBst = kStageB >> 4, kBpl = (kStageB / 4) >> 4;
+        const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
@@ -441,22 +517,28 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             ptx::tc_fence_after();
             int z0, z1;
             zrange(it.s, z0, z1);
-            for (int j = z0; j < z1; ++j) {
-                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
-                const int f0 = __ldg(fl), f1 = __ldg(fl + 1);
-                if ((f0 | f1) == 0) continue;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
                 const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                 ptx::mbar_wait(t_empty + buf, upar ^ 1);
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
                 bool first = true;
                 for (int kb = 0; kb < 2; ++kb) {
-                    if ((kb ? f1 : f0) == 0) continue;
+                    if (((f >> kb) & 1u) == 0u) continue;
+                    if (first && iw == 1) {   // D must have been initialised by issuer 0's first k-step
+                        ptx::mbar_wait(first_done + buf, upar);
+                        ptx::tc_fence_after();
+                    }
                     ptx::mbar_wait(b_full + slot, phase);
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
 #pragma unroll
-                        for (int ks = 0; ks < 4; ++ks) {
+                        for (int kk = 0; kk < 2; ++kk) {
+                            const int ks = 2 * kk + iw;
                             const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
                             const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
                             const uint64_t b_reh = descB0 + (uint64_t)slot * kBst + (uint64_t)(ks * 2);
@@ -474,6 +556,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                             ptx::umma_f16(d_im, a_rel, b_imh, idesc_pos, 1u);
                             ptx::umma_f16(d_re, a_imh, b_iml, idesc_neg, 1u);
                             ptx::umma_f16(d_im, a_reh, b_iml, idesc_pos, 1u);
+                            if (first && iw == 0 && kk == 0) ptx::umma_commit(first_done + buf);
                         }
                         ptx::umma_commit(b_empty + slot);
                     }
@@ -519,14 +602,25 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             for (int c = 0; c < 32; ++c) tot[c] = make_float2(0.f, 0.f);
             int z0, z1;
             zrange(it.s, z0, z1);
-            for (int j = z0; j < z1; ++j) {
-                const unsigned char *fl = P.flags + (size_t)j * P.nkb + it.g * 2;
-                if ((__ldg(fl) | __ldg(fl + 1)) == 0) continue;
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                const int j = z0 + n;
                 const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                 const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
+#ifdef SEPABL_YZ_NOEPI
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                ++u;
+                tot[0].x += (float)(mult + t_im);
+                continue;
+#endif
                 uint32_t gre[2][8], gim[2][8];
                 ptx::tmem_ld8(t_re, gre[0]);
                 ptx::tmem_ld8(t_im, gim[0]);
@@ -605,17 +699,16 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     int L = 0;
     while ((1 << L) < p.nx) ++L;
     t.L = L;
-    // z splits: enough items for >= 3 waves of CTAs, picked for the best last-wave fill
+    // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
     const int base = (t.NPYP / kM) * (t.NPXP / kNyz) * t.ng;
     int best = 1;
-    double best_eff = -1.0;
-    const int max_z = p.nz < 64 ? p.nz : 64;
+    double best_cost = 1e300;
+    const int max_z = p.nz < 32 ? p.nz : 32;
     for (int z = 1; z <= max_z; ++z) {
         const long long items = (long long)base * z;
         const long long waves = (items + num_sms - 1) / num_sms;
-        double eff = (double)items / (double)(waves * num_sms);
-        if (waves < 3) eff *= 0.5 + 0.15 * (double)waves;   // few waves: vacuum makes items uneven
-        if (eff > best_eff + 1e-9) { best_eff = eff; best = z; }
+        const double cost = (double)waves * ((double)((p.nz + z - 1) / z) + 3.0);
+        if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = z; }
     }
     t.nzs = best;
     t.nsplit = t.ng * t.nzs;
