@@ -190,6 +190,7 @@ def main():
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    qmethod = args.method if args.method in (0, 1, 3) else 0
     if args.route == "qgrid":
         kk = 2 * np.pi / w.lam
         qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
@@ -286,14 +287,37 @@ def main():
     k_ms = sum(kernel_ms) / len(kernel_ms)
     dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
     if args.route == "qgrid":
-        # two FP32 complex GEMMs per slice on CUDA cores: 8 flop per complex MAC, dense count (vacuum rows are skipped)
-        flop = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)
-        peak = 148 * 128 * 2 * 1.965e9 / 1e12      # FP32 FMA: 148 SMs x 128 lanes x 2 flop x max clock
-        ach = flop / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "sep_stage_x_kernel + sep_stage_yz_kernel", "achieved": ach, "peak": peak,
-                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
-                    "achieved_is": "dense FP32 flop of both GEMM stages / their CUDA-event time; all-vacuum rows are skipped, so "
-                                   "this can exceed what the ALUs executed"}
+        dense_sep = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)   # both stages, 8 flop per complex MAC
+        if qmethod == 3:
+            # two FP32 complex GEMMs per slice on CUDA cores, dense count (vacuum rows are skipped)
+            peak = 148 * 128 * 2 * 1.965e9 / 1e12      # FP32 FMA: 148 SMs x 128 lanes x 2 flop x max clock
+            ach = dense_sep / (k_ms * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": "sep_stage_x_kernel + sep_stage_yz_kernel", "achieved": ach, "peak": peak,
+                        "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
+                        "achieved_is": "dense FP32 flop of both GEMM stages / their CUDA-event time; all-vacuum rows are skipped, so "
+                                       "this can exceed what the ALUs executed"}
+        else:
+            # both stages on tcgen05, FP16x3: 24 tensor flop per complex MAC of the tiles the kernels issue.  The live tiles follow
+            # from the input alone (a 64-y block of a slice is skipped iff it is all vacuum), counted here on the host:
+            # stage X issues 128-y row tiles x all padded x x all padded columns, stage YZ 64-y blocks x padded rows x columns.
+            pad = lambda n, m: (n + m - 1) // m * m
+            NY, NXP, NPXP, NPYP = pad(w.ny, 128), pad(w.nx, 64), pad(w.npx, 64), pad(w.npy, 128)
+            issued = 0.0
+            for gi in g:
+                occ = np.zeros((w.nz, NY), bool)
+                occ[:, :w.ny] = (gi != 0).any(axis=(2, 3))
+                blk = occ.reshape(w.nz, NY // 64, 64).any(axis=2)                 # live 64-y blocks
+                grp = blk.reshape(w.nz, NY // 128, 2).any(axis=2)                 # live 128-y row tiles of stage X
+                issued += 24.0 * (grp.sum() * 128.0 * NXP * NPXP + blk.sum() * 64.0 * NPYP * NPXP)
+            peak = peaks["sustained"]
+            ach = issued / (k_ms * 1e-3) / 1e12
+            roofline = {"bound": "tensor", "kernel": "sep_tc_x_kernel + sep_tc_yz_kernel", "achieved": ach, "peak": peak,
+                        "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
+                        "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
+                        "achieved_is": "issued tensor flop (24 per complex MAC of the live tiles: 8 flop x 3 split products) / "
+                                       "CUDA-event time of the per-item launches (pack, stage X, stage YZ, finalize)",
+                        "issued_fraction_of_dense": issued / (3.0 * dense_sep),
+                        "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12}
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
         # One extra, untimed call with the counting flag (same inputs, same schedule).
@@ -361,9 +385,9 @@ def main():
 
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32" if args.route == "qgrid" or args.method != 1 else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32" if (args.route == "qgrid" and qmethod == 3) or (args.route != "qgrid" and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": "separable_qgrid" if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",

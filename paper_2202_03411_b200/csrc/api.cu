@@ -439,7 +439,7 @@ struct SepPlan {
     bool tensor = true;   // both GEMM stages on tcgen05 (method AUTO / TENSOR) or FP32 CUDA cores (SIMT_TABLE)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
                              int num_sms) {
@@ -466,6 +466,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
         sp.off_hp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NPXP * t.NY);
         sp.off_flags = take((size_t)g.nz * (t.NY / 64));
         sp.off_scale = take(sizeof(float) * 2);
+        sp.off_bounds = take(sizeof(int) * (size_t)((t.nsx + 1) + t.ng * (t.nzs + 1)));
         sp.off_partial = take(sizeof(float2) * (size_t)t.nsplit * npx * npy);
     } else {
         sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
@@ -540,15 +541,16 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         for (int b = 0; b < batch; ++b) {
             const float2 *rho_b = (const float2 *)rho + (size_t)b * p.nvox;
             std::string err;
-            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, Rp, ws + sp.off_flags, scaleH, ampscale, st);
-            if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, Hp, ctx->num_sms, st, &err);
+            int *bounds = (int *)(ws + sp.off_bounds);
+            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, Rp, ws + sp.off_flags, bounds, scaleH, ampscale, st);
+            if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, Hp, ctx->num_sms, st, &err);
             if (e == cudaSuccess)
-                e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, d_qx, npx, d_qy, npy, (float2 *)(ws + sp.off_partial),
+                e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, bounds, d_qx, npx, d_qy, npy, (float2 *)(ws + sp.off_partial),
                                      ctx->num_sms, st, &err);
             if (e == cudaSuccess)
                 e = launch_sep_tc_finalize((const float2 *)(ws + sp.off_partial), d_qx, npx, d_qy, npy, p, t, ampscale,
                                            d_I + (size_t)b * npx * npy, st);
-            nl += 5;
+            nl += 6;
             if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "qgrid stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         }
     } else {

@@ -81,13 +81,14 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
 cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    __half *d_Rp, unsigned char *d_flags64, float *d_scaleH, float *d_ampscale,
-                                    cudaStream_t st);
+                                    __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_scaleH,
+                                    float *d_ampscale, cudaStream_t st);
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
-                            const unsigned char *d_flags64, __half *d_Hp, int num_sms, cudaStream_t st, std::string *err);
+                            const unsigned char *d_flags64, const int *d_bounds, __half *d_Hp, int num_sms, cudaStream_t st,
+                            std::string *err);
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
-                             const unsigned char *d_flags64, const double *d_qx, int npx, const double *d_qy, int npy,
-                             float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);
+                             const unsigned char *d_flags64, const int *d_bounds, const double *d_qx, int npx,
+                             const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);
 cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
                                    const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st);
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);

@@ -148,11 +148,62 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
     if (any) flags[(size_t)j * (NY / kKB) + y / kKB] = 1;
 }
 
+// Balanced z splits.  Sequence 0 (stage X): weight of slice j = its live 128-y row tiles; sequence 1 + g (stage YZ, group g):
+// its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
+// every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam.
+__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz, int nkb, int ng, int nsx, int nzs,
+                                     int *__restrict__ bx, int *__restrict__ by) {
+    extern __shared__ unsigned char s_w[];   // [ng + 1][nz] weights, when they fit (else read from the flags directly)
+    const bool in_smem = (size_t)nz * (ng + 1) <= 32768;
+    auto weight_of = [&](int seq, int j) {
+        const unsigned char *fl = flags + (size_t)j * nkb;
+        int w = 0;
+        if (seq == 0) {
+            for (int g = 0; g < ng; ++g) w += (fl[2 * g] | fl[2 * g + 1]) != 0;
+        } else {
+            w = (fl[2 * (seq - 1)] != 0) + (fl[2 * (seq - 1) + 1] != 0);
+        }
+        return w;
+    };
+    __shared__ unsigned s_total[64];
+    if (threadIdx.x < 64) s_total[threadIdx.x] = 0u;
+    __syncthreads();
+    if (in_smem) {   // weights and their totals, cooperatively
+        for (int i = threadIdx.x; i < nz * (ng + 1); i += blockDim.x) {
+            const int w = weight_of(i / nz, i % nz);
+            s_w[i] = (unsigned char)w;
+            if (w) atomicAdd(&s_total[(i / nz) & 63], (unsigned)w);
+        }
+        __syncthreads();
+    }
+    const int seq = threadIdx.x;
+    if (seq > ng) return;
+    const int ns = seq == 0 ? nsx : nzs;
+    int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
+    auto weight = [&](int j) { return in_smem ? (int)s_w[seq * nz + j] : weight_of(seq, j); };
+    unsigned long long total = 0;
+    if (in_smem && ng + 1 <= 64) total = s_total[seq];
+    else for (int j = 0; j < nz; ++j) total += (unsigned)weight(j);
+    const bool small = total * (unsigned long long)ns < 0xffffffffull;   // 32-bit divisions suffice
+    unsigned long long E = 0, target = 0;   // weight of the slices before j; total * sidx / ns
+    int sidx = 0;
+    for (int j = 0; j < nz; ++j) {
+        while (sidx < ns && target <= E) {
+            out[sidx++] = j;
+            target = small ? (unsigned long long)(((unsigned)total * (unsigned)sidx) / (unsigned)ns) : (total * sidx) / ns;
+        }
+        E += (unsigned)weight(j);
+    }
+    while (sidx < ns) out[sidx++] = nz;
+    out[ns] = nz;
+}
+
 // ------------------------------------------------------------------------------------------------ stage X
 struct SepXParams {
     int nz, NY, NPXP, ng, nkx, nta, nsx, nkb;   // nkx = NXP / 64, nta = a tiles of NX columns, nsx = z splits, nkb = NY / 64
     float hscale;                               // 2^(-9 - L): accumulator (2^10 sR H) -> stored H (sH H)
     const unsigned char *flags;                 // [nz][nkb]
+    const int *zb;                              // [nsx + 1] balanced z split bounds (sep_tc_bounds_kernel)
     __half *Hp;                                 // [4][nz][NPXP][NY]
 };
 
@@ -203,8 +254,8 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
     // units of an item: (slice j of its z range, 128-y group g) with a non-empty 64-y block; u = (j - z0) * ng + g
     auto zrange = [&](int s, int &z0, int &z1) {
-        z0 = (int)(((long long)P.nz * s) / P.nsx);
-        z1 = (int)(((long long)P.nz * (s + 1)) / P.nsx);
+        z0 = __ldg(P.zb + s);
+        z1 = __ldg(P.zb + s + 1);
     };
 
     if (warp == 0) {
@@ -394,6 +445,7 @@ struct SepYzParams {
     double k, dz;
     const double *qx, *qy;
     const unsigned char *flags;   // [nz][nkb]
+    const int *zb;                // [ng][nzs + 1] balanced z split bounds per 128-y group (sep_tc_bounds_kernel)
     float2 *partial;              // [ng * nzs][npy][npx]
 };
 
@@ -454,9 +506,9 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     ptx::tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
 
-    auto zrange = [&](int s, int &z0, int &z1) {
-        z0 = (int)(((long long)P.nz * s) / P.nzs);
-        z1 = (int)(((long long)P.nz * (s + 1)) / P.nzs);
+    auto zrange = [&](int g, int s, int &z0, int &z1) {
+        z0 = __ldg(P.zb + g * (P.nzs + 1) + s);
+        z1 = __ldg(P.zb + g * (P.nzs + 1) + s + 1);
     };
 
     if (warp == 0) {
@@ -475,7 +527,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
             __syncwarp();
             int z0, z1;
-            zrange(it.s, z0, z1);
+            zrange(it.g, it.s, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
@@ -516,7 +568,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             int z0, z1;
-            zrange(it.s, z0, z1);
+            zrange(it.g, it.s, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
@@ -601,7 +653,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll
             for (int c = 0; c < 32; ++c) tot[c] = make_float2(0.f, 0.f);
             int z0, z1;
-            zrange(it.s, z0, z1);
+            zrange(it.g, it.s, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
@@ -715,7 +767,7 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for ~4 waves of a-tile items
     t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
     const int nta = t.NPXP / t.NX;
-    int nsx = (4 * num_sms + nta - 1) / nta;
+    int nsx = (2 * num_sms + nta - 1) / nta;   // two balanced items per CTA
     t.nsx = nsx < 1 ? 1 : nsx > p.nz ? p.nz : nsx;
     return t;
 }
@@ -730,8 +782,8 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 }
 
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
-                             const unsigned char *d_flags64, const double *d_qx, int npx, const double *d_qy, int npy,
-                             float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
+                             const unsigned char *d_flags64, const int *d_bounds, const double *d_qx, int npx,
+                             const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
     constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;
     static bool attr_set = false;
     if (!attr_set) {
@@ -762,7 +814,7 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     P.nz = p.nz; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
     P.ntb = t.NPYP / kM; P.nta = t.NPXP / kNyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
-    P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.partial = d_partial;
+    P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
     const int nitems = P.ntb * P.nta * P.ng * P.nzs;
     const int grid = nitems < num_sms ? nitems : num_sms;
     sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
@@ -770,8 +822,8 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 }
 
 cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    __half *d_Rp, unsigned char *d_flags64, float *d_scaleH, float *d_ampscale,
-                                    cudaStream_t st) {
+                                    __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_scaleH,
+                                    float *d_ampscale, cudaStream_t st) {
     const int nyb = t.NY / kKB;
     cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)p.nz * nyb, st);
     if (e != cudaSuccess) return e;
@@ -779,6 +831,10 @@ cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbi
     sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, t.NY, t.NXP, d_maxbits,
                                                                              d_Rp, d_flags64);
     sep_tc_scale_kernel<<<1, 1, 0, st>>>(d_maxbits, t.L, (float)(p.dx * p.dy * p.dz), d_scaleH, d_ampscale);
+    const size_t wbytes = (size_t)p.nz * (t.ng + 1);
+    const int bthreads = t.ng + 1 > 256 ? 32 * ((t.ng + 1 + 31) / 32) : 256;
+    sep_tc_bounds_kernel<<<1, bthreads, wbytes <= 32768 ? wbytes : 0, st>>>(d_flags64, p.nz, nyb, t.ng, t.nsx, t.nzs, d_bounds,
+                                                                           d_bounds + (t.nsx + 1));
     return cudaGetLastError();
 }
 
@@ -798,7 +854,8 @@ static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &t
 }
 
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
-                            const unsigned char *d_flags64, __half *d_Hp, int num_sms, cudaStream_t st, std::string *err) {
+                            const unsigned char *d_flags64, const int *d_bounds, __half *d_Hp, int num_sms, cudaStream_t st,
+                            std::string *err) {
     CUtensorMap tmA, tmB;
     bool ok;
     {
@@ -822,7 +879,7 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
     P.nz = p.nz; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / t.NX; P.nsx = t.nsx;
     P.nkb = t.NY / kKB;
     P.hscale = ldexpf(1.f, -9 - t.L);
-    P.flags = d_flags64; P.Hp = d_Hp;
+    P.flags = d_flags64; P.zb = d_bounds; P.Hp = d_Hp;
     switch (t.NX) {
         case 64: return launch_x_variant<64>(tmA, tmB, P, num_sms, st);
         case 32: return launch_x_variant<32>(tmA, tmB, P, num_sms, st);
