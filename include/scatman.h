@@ -136,10 +136,12 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
  * uniform (qx, qy) grid): the detector is a TENSOR GRID of transverse momentum transfers, pixel (a, b)
  * at (qx[a], qy[b], qz) with qz = -(k - sqrt(k^2 - qx^2 - qy^2)) on the Ewald sphere (Eq. 3-4, in
  * north_star's sign), so the slice transform factors into two small complex GEMMs per slice instead of the
- * (pixel x voxel) contraction -- npx-fold less arithmetic, FP32 CUDA-core GEMMs with FP64 phases.  Same a0 / a2 steps,
- * same conventions and output scale as scatman_simulate; grid points with qx^2 + qy^2 > k^2 (no scattering direction)
- * get I = 0.  d_qx[npx], d_qy[npy]: FP64 device arrays (any values, e.g. the DFT grid 2 pi m / (N dx)).
- * d_I[b][npy][npx].  rho_mode from opts; method / precision / flags of opts are ignored. */
+ * (pixel x voxel) contraction -- npx-fold less arithmetic.  Same a0 / a2 steps, same conventions and output scale as
+ * scatman_simulate; grid points with qx^2 + qy^2 > k^2 (no scattering direction) get I = 0.
+ * d_qx[npx], d_qy[npy]: FP64 device arrays (any values, e.g. the DFT grid 2 pi m / (N dx)).  d_I[b][npy][npx].
+ * opts: rho_mode; method AUTO / TENSOR = both GEMMs on tcgen05 tensor cores with the FP16x3 split (grids with nx > 1024
+ * use the CUDA-core stages), SIMT_TABLE = FP32 CUDA-core GEMMs; SIMT_SINCOS is INVALID_ARGUMENT here; precision and
+ * flags are ignored.  The workspace size depends on the method: pass the same opts to both calls. */
 int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
                                   const scatman_options *opts, size_t *bytes);
 int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
