@@ -153,11 +153,16 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam.
 __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz, int nkb, int ng, int nsx, int nzs,
                                      int *__restrict__ bx, int *__restrict__ by) {
-    extern __shared__ unsigned char s_w[];   // [ng + 1][nz] weights, when they fit (else read from the flags directly)
-    const bool in_smem = (size_t)nz * (ng + 1) <= 32768;
-    auto weight_of = [&](int seq, int j) {
+    // bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
+    // One warp per sequence, 32 slices per step: warp scan of the weights; the lane of slice j writes the bounds with
+    // E(j - 1) < target(s) <= E(j) (E(-1) = -1; j = nz is a last, weightless slice so that E(nz) = total is covered).
+    const int seq = blockIdx.x, lane = threadIdx.x;
+    const int ns = seq == 0 ? nsx : nzs;
+    int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
+    auto weight = [&](int j) -> unsigned {
+        if (j >= nz) return 0u;
         const unsigned char *fl = flags + (size_t)j * nkb;
-        int w = 0;
+        unsigned w = 0;
         if (seq == 0) {
             for (int g = 0; g < ng; ++g) w += (fl[2 * g] | fl[2 * g + 1]) != 0;
         } else {
@@ -165,37 +170,38 @@ __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, in
         }
         return w;
     };
-    __shared__ unsigned s_total[64];
-    if (threadIdx.x < 64) s_total[threadIdx.x] = 0u;
-    __syncthreads();
-    if (in_smem) {   // weights and their totals, cooperatively
-        for (int i = threadIdx.x; i < nz * (ng + 1); i += blockDim.x) {
-            const int w = weight_of(i / nz, i % nz);
-            s_w[i] = (unsigned char)w;
-            if (w) atomicAdd(&s_total[(i / nz) & 63], (unsigned)w);
-        }
-        __syncthreads();
+    long long total = 0;
+    for (int j0 = 0; j0 < nz; j0 += 32) {
+        unsigned w = weight(j0 + lane);
+        for (int off = 16; off > 0; off >>= 1) w += __shfl_xor_sync(0xffffffffu, w, off);
+        total += w;
     }
-    const int seq = threadIdx.x;
-    if (seq > ng) return;
-    const int ns = seq == 0 ? nsx : nzs;
-    int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
-    auto weight = [&](int j) { return in_smem ? (int)s_w[seq * nz + j] : weight_of(seq, j); };
-    unsigned long long total = 0;
-    if (in_smem && ng + 1 <= 64) total = s_total[seq];
-    else for (int j = 0; j < nz; ++j) total += (unsigned)weight(j);
-    const bool small = total * (unsigned long long)ns < 0xffffffffull;   // 32-bit divisions suffice
-    unsigned long long E = 0, target = 0;   // weight of the slices before j; total * sidx / ns
-    int sidx = 0;
-    for (int j = 0; j < nz; ++j) {
-        while (sidx < ns && target <= E) {
-            out[sidx++] = j;
-            target = small ? (unsigned long long)(((unsigned)total * (unsigned)sidx) / (unsigned)ns) : (total * sidx) / ns;
+    auto target = [&](int sidx) { return (total * sidx) / ns; };
+    long long carry = 0;    // E(j0)
+    unsigned wlast = 0;     // weight of slice j0 - 1
+    for (int j0 = 0; j0 <= nz; j0 += 32) {
+        const int j = j0 + lane;
+        const unsigned w = weight(j);
+        unsigned inc = w;
+        for (int off = 1; off < 32; off <<= 1) {
+            const unsigned v = __shfl_up_sync(0xffffffffu, inc, off);
+            if (lane >= off) inc += v;
         }
-        E += (unsigned)weight(j);
+        unsigned wprev = __shfl_up_sync(0xffffffffu, w, 1);
+        if (lane == 0) wprev = wlast;
+        const long long hi = carry + (long long)(inc - w);             // E(j)
+        const long long lo = j == 0 ? -1 : hi - (long long)wprev;      // E(j - 1)
+        if (j <= nz && lo < hi) {
+            int sidx = total > 0 ? (int)(((lo + 1) * ns) / total) : 0;
+            if (sidx > ns) sidx = ns;
+            while (sidx > 0 && target(sidx - 1) > lo) --sidx;
+            while (sidx < ns && target(sidx) <= lo) ++sidx;
+            for (; sidx < ns && target(sidx) <= hi; ++sidx) out[sidx] = j;
+        }
+        carry += (long long)__shfl_sync(0xffffffffu, inc, 31);
+        wlast = __shfl_sync(0xffffffffu, w, 31);
     }
-    while (sidx < ns) out[sidx++] = nz;
-    out[ns] = nz;
+    if (lane == 0) out[ns] = nz;
 }
 
 // ------------------------------------------------------------------------------------------------ stage X
@@ -831,10 +837,7 @@ cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbi
     sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, t.NY, t.NXP, d_maxbits,
                                                                              d_Rp, d_flags64);
     sep_tc_scale_kernel<<<1, 1, 0, st>>>(d_maxbits, t.L, (float)(p.dx * p.dy * p.dz), d_scaleH, d_ampscale);
-    const size_t wbytes = (size_t)p.nz * (t.ng + 1);
-    const int bthreads = t.ng + 1 > 256 ? 32 * ((t.ng + 1 + 31) / 32) : 256;
-    sep_tc_bounds_kernel<<<1, bthreads, wbytes <= 32768 ? wbytes : 0, st>>>(d_flags64, p.nz, nyb, t.ng, t.nsx, t.nzs, d_bounds,
-                                                                           d_bounds + (t.nsx + 1));
+    sep_tc_bounds_kernel<<<t.ng + 1, 32, 0, st>>>(d_flags64, p.nz, nyb, t.ng, t.nsx, t.nzs, d_bounds, d_bounds + (t.nsx + 1));
     return cudaGetLastError();
 }
 
