@@ -134,6 +134,98 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_fit(args):
+    """--route fit: the forward-fitting pieces on cfg4's shape of work: 256 candidate patterns of 256 x 256
+    pixels against one measured pattern.  A step = scatman_discrepancy (integral-normalised L2, masked) of the whole batch; the
+    Poisson deviance (FP64 log per pixel: FP64-ALU-bound) and the Ideal detector are timed beside it.  Single GPU; HBM-bound: 8 B per pixel and item (two passes over the FP32 patterns; the
+    measured pattern and the mask are shared and stay in L2)."""
+    import numpy as np
+    import torch
+    from oracle import fitting as F
+    from paper_2202_03411_b200 import binding as B, build as lib_build
+    lib_build.build()
+    sm = B.Scatman(0)
+    rng = np.random.default_rng(220203411 + 40)
+    batch, npy, npx = 256, 256, 256
+    npix = npy * npx
+    I = (rng.uniform(0.0, 1.0, (batch, npix)) ** 6 * 1e4).astype(np.float32)       # six decades, like a wide-angle pattern
+    M = rng.poisson(0.5 * I[0]).astype(np.float32)
+    mask = (rng.uniform(size=npix) < 0.9).astype(np.uint8)
+    d_I, d_M, d_mask = (torch.from_numpy(a).cuda() for a in (I, M, mask))
+    out = torch.empty(batch, dtype=torch.float64, device="cuda")
+    counts = torch.empty_like(d_I)
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(args.warmup):
+            flush.zero_()
+            fn()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev) / args.steps
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.25)
+    ms_d = timed(lambda: sm.discrepancy(d_I, d_M, d_mask, metric=B.LOSS_L2_NORMALISED, out=out, stream=stream))
+    launches = sm.last_launch_count() * args.steps
+    ms_p = timed(lambda: sm.discrepancy(d_I, d_M, d_mask, metric=B.LOSS_POISSON_DEVIANCE, out=out, stream=stream))
+    ms_n = timed(lambda: sm.ideal_detector(d_I, 1.0e7, seed=1, out=counts, stream=stream))
+    clocks = sampler.stop()
+    h_I = torch.from_numpy(I).pin_memory()
+    h_out = torch.empty(batch, dtype=torch.float64).pin_memory()
+    t0 = time.perf_counter()
+    for _ in range(3):
+        d_I.copy_(h_I, non_blocking=True)
+        sm.discrepancy(d_I, d_M, d_mask, metric=B.LOSS_L2_NORMALISED, out=out, stream=stream)
+        h_out.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / 3
+    t0 = time.perf_counter()
+    ref = F.discrepancy_l2(I, M, mask)
+    cpu_s = time.perf_counter() - t0
+    parity = float(np.max(np.abs(out.cpu().numpy() - ref) / np.abs(ref)))
+    peaks = load_peaks_hbm()
+    bytes_step = 8.0 * batch * npix
+    ach = bytes_step / (ms_d * 1e-3) / 1e9
+    line = {"metric": "fit_patterns_per_s", "value": batch / (ms_d * 1e-3), "unit": "patterns/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_d, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64 accumulation of f32 patterns", "data": "synthetic",
+            "config": {"workload": "fit_batch_256x256x256", "detector": [npy, npx], "batch": batch, "route": "fit",
+                       "metric": "l2_normalised, 90 % mask", "l2": "flushed between steps (192 MiB write)"},
+            "roofline": {"bound": "hbm", "kernel": "fit_sums_kernel + fit_metric_kernel", "achieved": ach, "peak": peaks[0],
+                         "unit": "GB/s", "frac": ach / peaks[0], "traffic": None, "peak_source": peaks[1],
+                         "achieved_is": "8 B per pixel and item (two passes over the FP32 patterns) / CUDA-event time of the call"},
+            "poisson_deviance": {"ms_per_step": ms_p, "patterns_per_s": batch / (ms_p * 1e-3), "bound": "alu (FP64 log per pixel)"},
+            "ideal_detector": {"ms_per_step": ms_n, "patterns_per_s": batch / (ms_n * 1e-3), "photons_per_pattern": 1.0e7,
+                               "bytes_per_pixel_item": 12, "gbps": 12.0 * batch * npix / (ms_n * 1e-3) / 1e9},
+            "cpu_baseline": {"value": batch / cpu_s, "unit": "patterns/s", "cores": 1, "kind": "oracle",
+                             "sample": f"oracle.fitting.discrepancy_l2 on the same {batch} patterns ({cpu_s:.2f} s)",
+                             "parity_max_rel": parity},
+            "e2e": {"value": batch / e2e_s, "unit": "patterns/s", "h2d_bytes_per_step": int(I.nbytes), "d2h_bytes_per_step": batch * 8},
+            "gpu_launches": launches, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+
+
+def load_peaks_hbm():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        for k in ("hbm_gbs", "hbm_gbps"):
+            if k in p:
+                return float(p[k]), f"MEASURED_PEAKS.json {k} (measured)"
+    except Exception:
+        pass
+    return 6500.0, "fallback of B200_PROFILING.md"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -145,13 +237,17 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes"],
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "fit"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
                          "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.route == "fit":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_fit(args)
         return
 
     import numpy as np

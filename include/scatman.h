@@ -157,6 +157,30 @@ int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_gri
                           const scatman_detector *det, const double *h_quat, int32_t batch,
                           const scatman_options *opts, float *h_I);
 
+/* ---- Forward-fitting pieces (simulate, compare with the measured pattern, improve) -------
+ * scatman_discrepancy: one number per simulated pattern instead of an image.  d_I[batch][npix] FP32 simulated patterns;
+ * d_M measured pattern(s), FP32: m_stride = 0 -> one pattern d_M[npix] for every item, m_stride = npix -> d_M[batch][npix];
+ * d_mask[npix] bytes (0 = pixel ignored: detector gaps, beam stop, angular window) or NULL = all pixels; d_out[batch] FP64.
+ *   SCATMAN_LOSS_L2_NORMALISED     sum_p w (I / S_I - M / S_M)^2, S = sum_p w (.): each pattern divided by its integral over
+ *                                  the masked region, the normalisation of the paper's Fig. 5 (reading R22)
+ *   SCATMAN_LOSS_POISSON_DEVIANCE  2 sum_p w [M log(M / mu) - (M - mu)], mu = (S_M / S_I) I: deviance of measured counts
+ *                                  against the scale-fitted simulation (M log M = 0 at M = 0; +inf where mu = 0 < M) (R24)
+ * FP64 accumulation, deterministic.  d_ws: scatman_fit_workspace_bytes(npix, batch) bytes.  Asynchronous on cuda_stream. */
+enum { SCATMAN_LOSS_L2_NORMALISED = 0, SCATMAN_LOSS_POISSON_DEVIANCE = 1 };
+int scatman_fit_workspace_bytes(scatman_ctx *ctx, int64_t npix, int32_t batch, size_t *bytes);
+int scatman_discrepancy(scatman_ctx *ctx, const float *d_I, const float *d_M, int64_t m_stride, const uint8_t *d_mask,
+                        int64_t npix, int32_t batch, int32_t metric, void *d_ws, size_t ws_bytes, double *d_out,
+                        void *cuda_stream);
+
+/* The Ideal detector ("even a perfect real-life detector is subjected to Poisson statistics of photons";
+ * the paper's photon estimate is in its unavailable supplement, so the caller states it, reading R23): d_counts[b][p] =
+ * Poisson(h_photons[b] * I[b][p] / sum_p I[b][p]) as FP32 integers, h_photons[batch] = expected detected photons per pattern
+ * (host, read before return).  Draws come from Philox-4x32-10 with counter (p low word, p high word, b, draw) and key = seed:
+ * a pixel's count depends only on (its mean, p, b, seed).  Means below 10 use inversion on one uniform, larger ones
+ * Hoermann's transformed rejection (PTRS).  An all-zero pattern gives all-zero counts.  Same workspace as above. */
+int scatman_ideal_detector(scatman_ctx *ctx, const float *d_I, int64_t npix, int32_t batch, const double *h_photons,
+                           uint64_t seed, void *d_ws, size_t ws_bytes, float *d_counts, void *cuda_stream);
+
 /* Number of kernels the last scatman_simulate* call on this context launched (for bench accounting). */
 int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count);
 

@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "libscatman.so")
 OK, INVALID_ARGUMENT, UNSUPPORTED_DEVICE, WORKSPACE_TOO_SMALL, CUDA_ERROR, NOT_IMPLEMENTED = range(6)
 RHO_LINEAR, RHO_N2M1 = 0, 1
 METHOD_AUTO, METHOD_TENSOR, METHOD_SIMT_SINCOS, METHOD_SIMT_TABLE = 0, 1, 2, 3
+LOSS_L2_NORMALISED, LOSS_POISSON_DEVIANCE = 0, 1
 PRECISION_AUTO, PRECISION_FP16X3 = 0, 1
 FLAG_SINGLE_CTA = 1
 FLAG_COUNT_ISSUED = 2
@@ -24,7 +25,7 @@ EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
     "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
-    "scatman_render", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
+    "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
 
@@ -93,6 +94,9 @@ def load_library() -> C.CDLL:
     L.scatman_simulate_shapes.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), dbl, C.POINTER(Detector),
                                           C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
+    L.scatman_fit_workspace_bytes.argtypes = [vp, i64, i32, C.POINTER(C.c_size_t)]
+    L.scatman_discrepancy.argtypes = [vp, vp, vp, i64, vp, i64, i32, i32, vp, C.c_size_t, vp, vp]
+    L.scatman_ideal_detector.argtypes = [vp, vp, i64, i32, C.POINTER(dbl), C.c_uint64, vp, C.c_size_t, vp, vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.scatman_last_issued_blocks.argtypes = [vp, C.POINTER(i64)]
@@ -347,6 +351,51 @@ class Scatman:
                                                     C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
                                                     C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out if dn.dim() == 5 else out[0]
+
+    def _fit_ws(self, npix: int, batch: int, device):
+        import torch
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_fit_workspace_bytes(self._ctx, npix, batch, C.byref(need)))
+        return torch.empty(int(need.value), dtype=torch.uint8, device=device)
+
+    def discrepancy(self, I, M, mask=None, metric: int = LOSS_L2_NORMALISED, out=None, stream=None):
+        """float64 [B]: discrepancy of each simulated pattern I[B][...] (CUDA float32) against the measured pattern M (same
+        pixel shape, or [B][...] for one per item); mask: CUDA uint8 per pixel, 0 = ignored (scatman_discrepancy)."""
+        import torch
+        if not (I.is_cuda and I.dtype == torch.float32 and I.is_contiguous() and I.dim() >= 2):
+            raise ValueError("I must be a contiguous CUDA float32 tensor [B][...pixels]")
+        batch, npix = int(I.shape[0]), int(I[0].numel())
+        if not (M.is_cuda and M.dtype == torch.float32 and M.is_contiguous() and M.numel() in (npix, batch * npix)):
+            raise ValueError("M must be a contiguous CUDA float32 tensor with the pixels of one pattern or of every item")
+        m_stride = 0 if M.numel() == npix else npix
+        if mask is not None and not (mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous() and mask.numel() == npix):
+            raise ValueError("mask must be a contiguous CUDA uint8 tensor with one byte per pixel")
+        ws = self._fit_ws(npix, batch, I.device)
+        if out is None:
+            out = torch.empty(batch, dtype=torch.float64, device=I.device)
+        self._check(self.lib.scatman_discrepancy(self._ctx, C.c_void_p(I.data_ptr()), C.c_void_p(M.data_ptr()), m_stride,
+                                                 C.c_void_p(mask.data_ptr()) if mask is not None else None, npix, batch,
+                                                 int(metric), C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()),
+                                                 self._stream(stream)))
+        return out
+
+    def ideal_detector(self, I, n_photons, seed: int, out=None, stream=None):
+        """float32 counts of I's shape: Poisson(n_photons[b] I[b] / sum I[b]) from the (pixel, item, seed) Philox stream
+        (scatman_ideal_detector).  n_photons: a number or one per item."""
+        import numpy as np
+        import torch
+        if not (I.is_cuda and I.dtype == torch.float32 and I.is_contiguous() and I.dim() >= 2):
+            raise ValueError("I must be a contiguous CUDA float32 tensor [B][...pixels]")
+        batch, npix = int(I.shape[0]), int(I[0].numel())
+        ph = np.ascontiguousarray(np.broadcast_to(np.asarray(n_photons, dtype=np.float64), (batch,)))
+        ws = self._fit_ws(npix, batch, I.device)
+        if out is None:
+            out = torch.empty_like(I)
+        self._check(self.lib.scatman_ideal_detector(self._ctx, C.c_void_p(I.data_ptr()), npix, batch,
+                                                    ph.ctypes.data_as(C.POINTER(C.c_double)), C.c_uint64(int(seed) & (2 ** 64 - 1)),
+                                                    C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()),
+                                                    self._stream(stream)))
+        return out
 
     def simulate_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
                       rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None, flags: int = 0):

@@ -573,6 +573,45 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     return SCATMAN_OK;
 }
 
+// ---- forward-fitting pieces ---------------------------------------------------------------------------------------
+int scatman_fit_workspace_bytes(scatman_ctx *ctx, int64_t npix, int32_t batch, size_t *bytes) {
+    if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
+    if (npix < 1 || batch < 1 || batch > 65535) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = fit_workspace_bytes(npix, batch);
+    return SCATMAN_OK;
+}
+
+int scatman_discrepancy(scatman_ctx *ctx, const float *d_I, const float *d_M, int64_t m_stride, const uint8_t *d_mask,
+                        int64_t npix, int32_t batch, int32_t metric, void *d_ws, size_t ws_bytes, double *d_out,
+                        void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_I || !d_M || !d_ws || !d_out || npix < 1 || batch < 1 || batch > 65535 || (m_stride != 0 && m_stride != npix) ||
+        (metric != SCATMAN_LOSS_L2_NORMALISED && metric != SCATMAN_LOSS_POISSON_DEVIANCE))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    if (((uintptr_t)d_ws | (uintptr_t)d_out) & 7) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "d_ws, d_out must be 8-byte aligned");
+    if (ws_bytes < fit_workspace_bytes(npix, batch)) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    cudaSetDevice(ctx->device);
+    cudaError_t e = launch_discrepancy(d_I, d_M, m_stride, d_mask, npix, batch, metric, (double *)d_ws, d_out,
+                                       (cudaStream_t)cuda_stream);
+    ctx->last_launches = 4;
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "discrepancy");
+}
+
+int scatman_ideal_detector(scatman_ctx *ctx, const float *d_I, int64_t npix, int32_t batch, const double *h_photons,
+                           uint64_t seed, void *d_ws, size_t ws_bytes, float *d_counts, void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_I || !h_photons || !d_ws || !d_counts || npix < 1 || batch < 1 || batch > 65535)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    for (int b = 0; b < batch; ++b)
+        if (!(h_photons[b] >= 0.0) || !std::isfinite(h_photons[b])) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad photon number");
+    if ((uintptr_t)d_ws & 7) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "d_ws must be 8-byte aligned");
+    if (ws_bytes < fit_workspace_bytes(npix, batch)) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    cudaSetDevice(ctx->device);
+    cudaError_t e = launch_ideal_detector(d_I, npix, batch, h_photons, seed, (double *)d_ws, d_counts, (cudaStream_t)cuda_stream);
+    ctx->last_launches = 3;
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "ideal detector");
+}
+
 int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
                           float *h_I) {

@@ -1,0 +1,241 @@
+// fit_kernels.cu -- forward-fitting pieces on the device ("simulating its diffraction pattern,
+// comparing it with the desired experimental data, and then iteratively improving the guess"):
+//   * discrepancy between simulated patterns and a measured one, so that a fit step returns one number per candidate
+//     instead of an image: the integral-normalised squared distance (the normalisation of Fig. 5) and the
+//     scale-fitted Poisson deviance;
+//   * the Ideal detector: Poisson counts with means n_photons * I / sum(I), drawn from Philox-4x32-10 with
+//     the counter (pixel lo, pixel hi, item, draw) and the seed as key -- every pixel's draw is independent of the launch shape.
+// HBM-bound: one or two passes over the patterns (4 B per pixel and item, + 4 B for the measured pattern, + 1 B mask),
+// FP64 accumulation (free at this intensity), deterministic two-level sums (per-block partials, summed in index order).
+#include "internal.h"
+
+namespace scatman {
+
+namespace {
+
+constexpr int kFitThreads = 256;
+constexpr int kFitChunk = 32768;  // pixels per block
+
+__device__ __forceinline__ double block_sum(double v, double *s_red) {
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    __syncthreads();   // s_red may still be read from the previous call
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < kFitThreads / 32; ++w) t += s_red[w];
+    return t;   // valid in thread 0
+}
+
+}  // namespace
+
+// pass 1: partial[b][chunk][5] = sums over the chunk of w I, w M, w I^2, w M^2, w I M
+__global__ void __launch_bounds__(kFitThreads) fit_sums_kernel(const float *__restrict__ I, const float *__restrict__ M,
+                                                               int64_t m_stride, const unsigned char *__restrict__ mask,
+                                                               int64_t npix, int nchunk, double *__restrict__ partial) {
+    __shared__ double s_red[5 * kFitThreads / 32];
+    const int b = blockIdx.y, chunk = blockIdx.x;
+    const float *Ib = I + (size_t)b * npix;
+    const float *Mb = M ? M + (size_t)b * m_stride : nullptr;
+    double a[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    const int64_t p1 = min((int64_t)(chunk + 1) * kFitChunk, npix);
+    for (int64_t p0 = (int64_t)chunk * kFitChunk + threadIdx.x; p0 < p1; p0 += 4 * kFitThreads) {
+        float fi[4], fm[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {   // four independent loads in flight per thread
+            const int64_t p = p0 + k * kFitThreads;
+            const bool in = p < p1;   // the three loads do not wait for one another; the mask is applied afterwards
+            const unsigned char w = in ? (mask ? mask[p] : (unsigned char)1) : (unsigned char)0;
+            const float vi = in ? Ib[p] : 0.f, vm = in && Mb ? Mb[p] : 0.f;
+            fi[k] = w ? vi : 0.f;
+            fm[k] = w ? vm : 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double i = (double)fi[k], m = (double)fm[k];
+            a[0] += i;
+            a[1] += m;
+            a[2] += i * i;
+            a[3] += m * m;
+            a[4] += i * m;
+        }
+    }
+    // the five sums through one shared-memory stage
+#pragma unroll
+    for (int k = 0; k < 5; ++k)
+        for (int off = 16; off > 0; off >>= 1) a[k] += __shfl_xor_sync(0xffffffffu, a[k], off);
+    if ((threadIdx.x & 31) == 0)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) s_red[(threadIdx.x >> 5) * 5 + k] = a[k];
+    __syncthreads();
+    if (threadIdx.x < 5) {
+        double t = 0.0;
+        for (int w = 0; w < kFitThreads / 32; ++w) t += s_red[w * 5 + threadIdx.x];
+        partial[((size_t)b * nchunk + chunk) * 5 + threadIdx.x] = t;
+    }
+}
+
+// sums[b][5] = partials summed in chunk order (one warp per item would do; one thread is enough at these sizes)
+__global__ void fit_reduce_kernel(const double *__restrict__ partial, int nchunk, int nk, int batch, double *__restrict__ sums) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= batch * nk) return;
+    const int b = t / nk, k = t % nk;
+    double s = 0.0;
+    for (int c = 0; c < nchunk; ++c) s += partial[((size_t)b * nchunk + c) * nk + k];
+    sums[t] = s;
+}
+
+// L2: D = sum w (I / S_I - M / S_M)^2 = S_II / S_I^2 - 2 S_IM / (S_I S_M) + S_MM / S_M^2 would cancel catastrophically
+// for close patterns, so the squared differences are summed directly in a second pass (same cost: HBM-bound).
+// metric 0: w (I / S_I - M / S_M)^2; metric 1: 2 w [M log(M / (c I)) - (M - c I)], c = S_M / S_I
+__global__ void __launch_bounds__(kFitThreads) fit_metric_kernel(const float *__restrict__ I, const float *__restrict__ M,
+                                                                 int64_t m_stride, const unsigned char *__restrict__ mask,
+                                                                 int64_t npix, int nchunk, int metric,
+                                                                 const double *__restrict__ sums, double *__restrict__ partial) {
+    __shared__ double s_red[kFitThreads / 32];
+    const int b = blockIdx.y, chunk = blockIdx.x;
+    const float *Ib = I + (size_t)b * npix;
+    const float *Mb = M + (size_t)b * m_stride;
+    const double SI = sums[b * 5 + 0], SM = sums[b * 5 + 1];
+    const double c = SM / SI, rSI = 1.0 / SI, rSM = 1.0 / SM;
+    double acc = 0.0;
+    const int64_t p1 = min((int64_t)(chunk + 1) * kFitChunk, npix);
+    for (int64_t p0 = (int64_t)chunk * kFitChunk + threadIdx.x; p0 < p1; p0 += 4 * kFitThreads) {
+        float fi[4], fm[4];
+        bool on[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int64_t p = p0 + k * kFitThreads;
+            const bool in = p < p1;
+            const unsigned char w = in ? (mask ? mask[p] : (unsigned char)1) : (unsigned char)0;
+            fi[k] = in ? Ib[p] : 0.f;
+            fm[k] = in ? Mb[p] : 0.f;
+            on[k] = w != 0;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (!on[k]) continue;
+            const double i = (double)fi[k], m = (double)fm[k];
+            if (metric == SCATMAN_LOSS_L2_NORMALISED) {
+                const double d = __dmul_rn(i, rSI) - __dmul_rn(m, rSM);   // no FMA contraction: identical patterns give exactly 0
+                acc += d * d;
+            } else {
+                const double mu = c * i;
+                acc += 2.0 * ((m > 0.0 ? m * log(m / mu) : 0.0) - (m - mu));
+            }
+        }
+    }
+    const double t = block_sum(acc, s_red);
+    if (threadIdx.x == 0) partial[(size_t)b * nchunk + chunk] = t;
+}
+
+// ---- Ideal detector -----------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t &o0, uint32_t &o1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    o0 = c0;
+    o1 = c1;
+}
+
+__device__ __forceinline__ void uniforms(uint64_t p, uint32_t b, uint32_t draw, uint64_t seed, double &u, double &v) {
+    uint32_t x0, x1;
+    philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), b, draw, (uint32_t)seed, (uint32_t)(seed >> 32), x0, x1);
+    u = ((double)x0 + 0.5) * 2.3283064365386963e-10;   // 2^-32
+    v = ((double)x1 + 0.5) * 2.3283064365386963e-10;
+}
+
+// Poisson(lam): inversion by sequential search below 10, Hoermann's transformed rejection with squeeze (PTRS) from 10 on
+__device__ double poisson_draw(double lam, uint64_t p, uint32_t b, uint64_t seed) {
+    if (!(lam > 0.0)) return 0.0;
+    double u, v;
+    if (lam < 10.0) {
+        uniforms(p, b, 0u, seed, u, v);
+        int k = 0;
+        double pk = exp(-lam), s = pk;
+        while (u > s && k < 1000) {
+            ++k;
+            pk *= lam / (double)k;
+            s += pk;
+        }
+        return (double)k;
+    }
+    const double slam = sqrt(lam), loglam = log(lam);
+    const double bb = 0.931 + 2.53 * slam, a = -0.059 + 0.02483 * bb;
+    const double invalpha = 1.1239 + 1.1328 / (bb - 3.4), vr = 0.9277 - 3.6224 / (bb - 2.0);
+    for (uint32_t draw = 0;; ++draw) {
+        uniforms(p, b, draw, seed, u, v);
+        u -= 0.5;
+        const double us = 0.5 - fabs(u);
+        const double k = floor((2.0 * a / us + bb) * u + lam + 0.43);
+        if (us >= 0.07 && v <= vr) return k;
+        if (k < 0.0 || (us < 0.013 && v > us)) continue;
+        if (log(v) + log(invalpha) - log(a / (us * us) + bb) <= -lam + k * loglam - lgamma(k + 1.0)) return k;
+    }
+}
+
+__global__ void __launch_bounds__(kFitThreads) ideal_detector_kernel(const float *__restrict__ I, int64_t npix,
+                                                                     const double *__restrict__ sums,
+                                                                     const double *__restrict__ photons, uint64_t seed,
+                                                                     float *__restrict__ counts) {
+    const int b = blockIdx.y;
+    const int64_t p = (int64_t)blockIdx.x * kFitThreads + threadIdx.x;
+    if (p >= npix) return;
+    const double S = sums[b * 5 + 0];
+    double n = 0.0;
+    if (S > 0.0) n = poisson_draw((double)I[(size_t)b * npix + p] * (photons[b] / S), (uint64_t)p, (uint32_t)b, seed);
+    counts[(size_t)b * npix + p] = (float)n;
+}
+
+// ------------------------------------------------------------------------------------------------ host
+int fit_nchunk(int64_t npix) { return (int)((npix + kFitChunk - 1) / kFitChunk); }
+
+size_t fit_workspace_bytes(int64_t npix, int batch) {
+    // partial[b][nchunk][5] + sums[b][5] + partial2[b][nchunk] + photons[b]
+    return sizeof(double) * ((size_t)batch * fit_nchunk(npix) * 6 + (size_t)batch * 6);
+}
+
+cudaError_t launch_fit_sums(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
+                            int batch, double *d_ws, cudaStream_t st) {
+    const int nchunk = fit_nchunk(npix);
+    double *partial = d_ws, *sums = d_ws + (size_t)batch * nchunk * 5;
+    fit_sums_kernel<<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, partial);
+    fit_reduce_kernel<<<(batch * 5 + 127) / 128, 128, 0, st>>>(partial, nchunk, 5, batch, sums);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
+                               int batch, int metric, double *d_ws, double *d_out, cudaStream_t st) {
+    cudaError_t e = launch_fit_sums(d_I, d_M, m_stride, d_mask, npix, batch, d_ws, st);
+    if (e != cudaSuccess) return e;
+    const int nchunk = fit_nchunk(npix);
+    double *sums = d_ws + (size_t)batch * nchunk * 5, *partial2 = sums + (size_t)batch * 5;
+    fit_metric_kernel<<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, metric, sums, partial2);
+    fit_reduce_kernel<<<(batch + 127) / 128, 128, 0, st>>>(partial2, nchunk, 1, batch, d_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, const double *h_photons, uint64_t seed, double *d_ws,
+                                  float *d_counts, cudaStream_t st) {
+    cudaError_t e = launch_fit_sums(d_I, nullptr, 0, nullptr, npix, batch, d_ws, st);
+    if (e != cudaSuccess) return e;
+    const int nchunk = fit_nchunk(npix);
+    double *sums = d_ws + (size_t)batch * nchunk * 5;
+    double *photons = sums + (size_t)batch * 5 + (size_t)batch * nchunk;
+    e = cudaMemcpyAsync(photons, h_photons, sizeof(double) * batch, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    ideal_detector_kernel<<<dim3((unsigned)((npix + kFitThreads - 1) / kFitThreads), batch), kFitThreads, 0, st>>>(
+        d_I, npix, sums, photons, seed, d_counts);
+    return cudaGetLastError();
+}
+
+}  // namespace scatman

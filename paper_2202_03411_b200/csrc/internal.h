@@ -93,6 +93,13 @@ cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, 
                                    const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st);
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
 
+// forward-fitting pieces (fit_kernels.cu)
+size_t fit_workspace_bytes(int64_t npix, int batch);
+cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
+                               int batch, int metric, double *d_ws, double *d_out, cudaStream_t st);
+cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, const double *h_photons, uint64_t seed, double *d_ws,
+                                  float *d_counts, cudaStream_t st);
+
 // tensor path: tensor maps are encoded on the host through the driver entry point
 struct TensorMaps;  // opaque here
 struct TensorLaunch {
