@@ -153,10 +153,14 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
     if (ix < nx) {
         const size_t plane = (size_t)nx * ny;
         const size_t base = (size_t)b * plane * nz + (size_t)iy * nx + ix;
-        double Cre = 0.0, Cim = 0.0;
+        // T_j = exp(i k dz C_j) as a running FP64 product of the per-voxel factors g(dn) = exp(i k dz dn): exp of the
+        // prefix sum, one complex multiplication per non-vacuum voxel.  The factor of the last (delta, beta) seen is kept, so a
+        // homogeneous stretch of material costs no sincos / exp at all (each costs ~10x the product); a product of N factors
+        // rounds N times (N 2^-53 relative), far below the FP32 the result is stored in.
         double Tre = 1.0, Tim = 0.0;
-        bool stale = false;  // T must be recomputed from C before its next use
-        // slices in batches of 8: the loads of a batch are independent of the running prefix, so they are all in flight
+        double gre = 1.0, gim = 0.0;
+        float ld = 0.f, lb = 0.f;          // the (delta, beta) of g; (0, 0) <-> g = 1
+        // slices in batches of 8: the loads of a batch are independent of the running product, so they are all in flight
         // before the (serial) FP64 chain of the batch starts
         for (int iz0 = 0; iz0 < nz; iz0 += 8) {
             float2 cin[8];
@@ -169,14 +173,6 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
                 const float2 c = cin[i];
                 float2 o = make_float2(0.f, 0.f);
                 if (c.x != 0.f || c.y != 0.f) {
-                    if (stale) {
-                        double s, co;
-                        sincos(kdz * Cre, &s, &co);
-                        const double mag = exp(-kdz * Cim);
-                        Tre = mag * co;
-                        Tim = mag * s;
-                        stale = false;
-                    }
                     const double d = (double)c.x, be = (double)c.y;
                     double fre = d, fim = be;
                     if (rho_mode == SCATMAN_RHO_N2M1) {  // c (2 - c)
@@ -186,9 +182,18 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
                     o.x = (float)(fre * Tre - fim * Tim);
                     o.y = (float)(fre * Tim + fim * Tre);
                     vmax = fmaxf(vmax, fmaxf(fabsf(o.x), fabsf(o.y)));
-                    Cre += d;
-                    Cim += be;
-                    stale = true;
+                    if (c.x != ld || c.y != lb) {
+                        double s, co;
+                        sincos(kdz * d, &s, &co);
+                        const double mag = exp(-kdz * be);
+                        gre = mag * co;
+                        gim = mag * s;
+                        ld = c.x;
+                        lb = c.y;
+                    }
+                    const double t = Tre * gre - Tim * gim;
+                    Tim = Tre * gim + Tim * gre;
+                    Tre = t;
                 }
                 rho[base + (size_t)(iz0 + i) * plane] = o;
             }
