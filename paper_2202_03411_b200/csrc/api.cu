@@ -462,12 +462,12 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
         const SepTcPlan &t = sp.tc;
         sp.off_eyp = take(sizeof(__half) * 4 * (size_t)t.NPYP * t.NY);
         sp.off_exp = take(sizeof(__half) * 4 * (size_t)t.NPXP * t.NXP);
-        sp.off_rp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NY * t.NXP);
-        sp.off_hp = take(sizeof(__half) * 4 * (size_t)g.nz * t.NPXP * t.NY);
-        sp.off_flags = take((size_t)g.nz * (t.NY / 64));
-        sp.off_scale = take(sizeof(float) * 2);
-        sp.off_bounds = take(sizeof(int) * (size_t)((t.nsx + 1) + t.ng * (t.nzs + 1)));
-        sp.off_partial = take(sizeof(float2) * (size_t)t.nsplit * npx * npy);
+        sp.off_rp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NY * t.NXP);
+        sp.off_hp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NPXP * t.NY);
+        sp.off_flags = take((size_t)t.nb * g.nz * (t.NY / 64));
+        sp.off_scale = take(sizeof(float) * (size_t)batch);
+        sp.off_bounds = take(sizeof(int) * (size_t)((t.nsx + 1) + (size_t)t.nb * t.ng * (t.nzs + 1)));
+        sp.off_partial = take(sizeof(float2) * (size_t)t.nb * t.nsplit * npx * npy);
     } else {
         sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
         sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
@@ -533,23 +533,24 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         const SepTcPlan &t = sp.tc;
         __half *Eyp = (__half *)(ws + sp.off_eyp), *Exp = (__half *)(ws + sp.off_exp), *Rp = (__half *)(ws + sp.off_rp),
                *Hp = (__half *)(ws + sp.off_hp);
-        float *scaleH = (float *)(ws + sp.off_scale), *ampscale = scaleH + 1;
+        float *ampscale = (float *)(ws + sp.off_scale);
+        int *bounds = (int *)(ws + sp.off_bounds);
         e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, Exp, Eyp, st);
         nl += 2;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
         cudaEventRecord(ctx->ev0, st);
-        for (int b = 0; b < batch; ++b) {
-            const float2 *rho_b = (const float2 *)rho + (size_t)b * p.nvox;
+        for (int b0 = 0; b0 < batch; b0 += t.nb) {   // a chunk of items per set of launches, stacked along z
+            const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
+            const float2 *rho_b = (const float2 *)rho + (size_t)b0 * p.nvox;
             std::string err;
-            int *bounds = (int *)(ws + sp.off_bounds);
-            e = launch_sep_tc_prep_item(rho_b, maxbits + b, p, t, Rp, ws + sp.off_flags, bounds, scaleH, ampscale, st);
-            if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, Hp, ctx->num_sms, st, &err);
+            e = launch_sep_tc_prep(rho_b, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds, ampscale + b0, st);
+            if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
             if (e == cudaSuccess)
-                e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, bounds, d_qx, npx, d_qy, npy, (float2 *)(ws + sp.off_partial),
-                                     ctx->num_sms, st, &err);
+                e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, bounds, nb, d_qx, npx, d_qy, npy,
+                                     (float2 *)(ws + sp.off_partial), ctx->num_sms, st, &err);
             if (e == cudaSuccess)
-                e = launch_sep_tc_finalize((const float2 *)(ws + sp.off_partial), d_qx, npx, d_qy, npy, p, t, ampscale,
-                                           d_I + (size_t)b * npx * npy, st);
+                e = launch_sep_tc_finalize((const float2 *)(ws + sp.off_partial), d_qx, npx, d_qy, npy, p, t, nb, ampscale + b0,
+                                           d_I + (size_t)b0 * npx * npy, st);
             nl += 6;
             if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "qgrid stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         }

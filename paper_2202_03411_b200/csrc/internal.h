@@ -76,21 +76,22 @@ struct SepTcPlan {
     int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
     int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
     int NX = 64, nsx = 1;                      // stage X: a columns per tile, z splits
+    int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
-cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_scaleH,
-                                    float *d_ampscale, cudaStream_t st);
+cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
+                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st);
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
-                            const unsigned char *d_flags64, const int *d_bounds, __half *d_Hp, int num_sms, cudaStream_t st,
-                            std::string *err);
+                            const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
+                            cudaStream_t st, std::string *err);
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
-                             const unsigned char *d_flags64, const int *d_bounds, const double *d_qx, int npx,
+                             const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);
 cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
-                                   const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st);
+                                   const Plan &p, const SepTcPlan &t, int nb, const float *d_ampscale, float *d_I,
+                                   cudaStream_t st);
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
 
 // forward-fitting pieces (fit_kernels.cu)

@@ -104,29 +104,29 @@ __global__ void sep_tc_table_kernel(const double *__restrict__ q, int nq, int ro
 
 // per item: sH = 2^(14 - e - L) (max |rho~ component| in [2^(e-1), 2^e), 2^L >= nx) is the scale H is stored with;
 // ampscale = dV / (2^10 sH) takes the summed amplitude back to physical units
-__global__ void sep_tc_scale_kernel(const unsigned *__restrict__ maxbits, int L, float dV, float *__restrict__ scaleH,
-                                    float *__restrict__ ampscale) {
-    const float m = __uint_as_float(maxbits[0]);
+__global__ void sep_tc_scale_kernel(const unsigned *__restrict__ maxbits, int nb, int L, float dV, float *__restrict__ ampscale) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nb) return;
+    const float m = __uint_as_float(maxbits[b]);
     int e = 0;
     if (m > 0.f) frexpf(m, &e);
-    const float sH = ldexpf(1.f, 14 - e - L);
-    scaleH[0] = sH;
-    ampscale[0] = dV / (kScaleA * sH);
+    ampscale[b] = dV / (kScaleA * ldexpf(1.f, 14 - e - L));
 }
 
-// rho~ FP32 [nz][ny][nx] -> planes fp16 [4][nz * NY][NXP] = split(sR rho~), x fastest (K-major for stage X), zero in the
-// padding; sR = 2^(13 - e) as in pack_b_kernel.  Also raises flags64[j][y / 64] for every 64-y block holding a non-zero value
+// rho~ FP32 [nb][nz][ny][nx] -> planes fp16 [4][nb * nz * NY][NXP] = split(sR[b] rho~), x fastest (K-major for stage X), zero
+// in the padding; sR = 2^(13 - e) per item as in pack_b_kernel.  The items of a chunk are stacked along z: global slice
+// jg = b nz + j.  Also raises flags64[j][y / 64] for every 64-y block holding a non-zero value
 // (flags are cleared by a memset before).  One thread = 8 consecutive x of one row.
-__global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz, int NY, int NXP,
+__global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, int ny, int nz1, int nz, int NY, int NXP,
                                        const unsigned *__restrict__ maxbits, __half *__restrict__ R,
-                                       unsigned char *__restrict__ flags) {
+                                       unsigned char *__restrict__ flags) {   // nz1: slices per item, nz: of the chunk
     const int nx8 = NXP / 8;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (int64_t)nz * NY * nx8) return;
     const int x0 = (int)(t % nx8) * 8;
     const int64_t row = t / nx8;
     const int y = (int)(row % NY), j = (int)(row / NY);
-    const float m = __uint_as_float(maxbits[0]);
+    const float m = __uint_as_float(maxbits[j / nz1]);
     int e = 0;
     if (m > 0.f) frexpf(m, &e);
     const float s = ldexpf(1.f, kScaleBExp - e);
@@ -151,22 +151,31 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // Balanced z splits.  Sequence 0 (stage X): weight of slice j = its live 128-y row tiles; sequence 1 + g (stage YZ, group g):
 // its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
 // every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam.
-__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz, int nkb, int ng, int nsx, int nzs,
+__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int nsx, int nzs,
                                      int *__restrict__ bx, int *__restrict__ by) {
     // bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
     // One warp per sequence, 32 slices per step: warp scan of the weights; the lane of slice j writes the bounds with
     // E(j - 1) < target(s) <= E(j) (E(-1) = -1; j = nz is a last, weightless slice so that E(nz) = total is covered).
+    // sequence 0: stage X over all nzt slices of the chunk; sequence 1 + b ng + g: stage YZ of item b, group g (its nz1 slices).
+    // Bounds are GLOBAL slice indices (jbase + j).
     const int seq = blockIdx.x, lane = threadIdx.x;
     const int ns = seq == 0 ? nsx : nzs;
     int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
+    const int gsel = seq == 0 ? 0 : (seq - 1) % ng;
+    const int jbase = seq == 0 ? 0 : ((seq - 1) / ng) * nz1;
+    const int nz = seq == 0 ? nzt : nz1;
+    if (seq == 0 && nzt > 4096) {   // many stacked items: equal slice counts per range balance well enough, no scan
+        for (int sidx = lane; sidx <= ns; sidx += 32) out[sidx] = (int)(((long long)nzt * sidx) / ns);
+        return;
+    }
     auto weight = [&](int j) -> unsigned {
         if (j >= nz) return 0u;
-        const unsigned char *fl = flags + (size_t)j * nkb;
+        const unsigned char *fl = flags + (size_t)(jbase + j) * nkb;
         unsigned w = 0;
         if (seq == 0) {
             for (int g = 0; g < ng; ++g) w += (fl[2 * g] | fl[2 * g + 1]) != 0;
         } else {
-            w = (fl[2 * (seq - 1)] != 0) + (fl[2 * (seq - 1) + 1] != 0);
+            w = (fl[2 * gsel] != 0) + (fl[2 * gsel + 1] != 0);
         }
         return w;
     };
@@ -196,12 +205,12 @@ __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, in
             if (sidx > ns) sidx = ns;
             while (sidx > 0 && target(sidx - 1) > lo) --sidx;
             while (sidx < ns && target(sidx) <= lo) ++sidx;
-            for (; sidx < ns && target(sidx) <= hi; ++sidx) out[sidx] = j;
+            for (; sidx < ns && target(sidx) <= hi; ++sidx) out[sidx] = jbase + j;
         }
         carry += (long long)__shfl_sync(0xffffffffu, inc, 31);
         wlast = __shfl_sync(0xffffffffu, w, 31);
     }
-    if (lane == 0) out[ns] = nz;
+    if (lane == 0) out[ns] = jbase + nz;
 }
 
 // ------------------------------------------------------------------------------------------------ stage X
@@ -447,16 +456,16 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
 // ------------------------------------------------------------------------------------------------ stage YZ
 struct SepYzParams {
-    int nz, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nkb = NY / 64
+    int nz, nb, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nz: slices per item, nb: items of the chunk, nkb = NY / 64
     double k, dz;
     const double *qx, *qy;
     const unsigned char *flags;   // [nz][nkb]
-    const int *zb;                // [ng][nzs + 1] balanced z split bounds per 128-y group (sep_tc_bounds_kernel)
-    float2 *partial;              // [ng * nzs][npy][npx]
+    const int *zb;                // [nb][ng][nzs + 1] balanced z split bounds (global slice indices) per item and 128-y group
+    float2 *partial;              // [nb][ng * nzs][npy][npx]
 };
 
 struct YzItem {
-    int tb, ta, g, s;
+    int tb, ta, g, s, b;
 };
 __device__ __forceinline__ YzItem yz_decode(int item, const SepYzParams &P) {
     YzItem it;
@@ -465,7 +474,9 @@ __device__ __forceinline__ YzItem yz_decode(int item, const SepYzParams &P) {
     it.ta = item % P.nta;
     item /= P.nta;
     it.g = item % P.ng;
-    it.s = item / P.ng;
+    item /= P.ng;
+    it.s = item % P.nzs;
+    it.b = item / P.nzs;
     return it;
 }
 
@@ -485,7 +496,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     uint32_t *tmem_ptr = (uint32_t *)(first_done + kNBuf);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nitems = P.ntb * P.nta * P.ng * P.nzs;
+    const int nitems = P.ntb * P.nta * P.ng * P.nzs * P.nb;
 
     if (warp == 0 && lane == 0) {
         ptx::tma_prefetch_desc(&tmA);
@@ -512,9 +523,10 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     ptx::tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
 
-    auto zrange = [&](int g, int s, int &z0, int &z1) {
-        z0 = __ldg(P.zb + g * (P.nzs + 1) + s);
-        z1 = __ldg(P.zb + g * (P.nzs + 1) + s + 1);
+    auto zrange = [&](const YzItem &it, int &z0, int &z1) {   // global slice indices
+        const int *zb = P.zb + (size_t)(it.b * P.ng + it.g) * (P.nzs + 1) + it.s;
+        z0 = __ldg(zb);
+        z1 = __ldg(zb + 1);
     };
 
     if (warp == 0) {
@@ -533,7 +545,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
             __syncwarp();
             int z0, z1;
-            zrange(it.g, it.s, z0, z1);
+            zrange(it, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
@@ -574,7 +586,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             int z0, z1;
-            zrange(it.g, it.s, z0, z1);
+            zrange(it, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
@@ -659,13 +671,13 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll
             for (int c = 0; c < 32; ++c) tot[c] = make_float2(0.f, 0.f);
             int z0, z1;
-            zrange(it.g, it.s, z0, z1);
+            zrange(it, z0, z1);
             LiveUnits un;
             un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
             int n;
             uint32_t f;
             while (un.next(n, f)) {
-                const int j = z0 + n;
+                const int j = z0 + n - it.b * P.nz;   // slice within its item
                 const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                 const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
                 ptx::mbar_wait(t_full + buf, upar);
@@ -711,7 +723,7 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 ++u;
             }
             if (b < P.npy) {
-                float2 *dst = P.partial + ((size_t)(it.g * P.nzs + it.s) * P.npy + b) * P.npx;
+                float2 *dst = P.partial + (((size_t)it.b * P.ng * P.nzs + it.g * P.nzs + it.s) * P.npy + b) * P.npx;
 #pragma unroll
                 for (int c = 0; c < 32; ++c)
                     if (a0 + c < P.npx) dst[a0 + c] = tot[c];
@@ -731,19 +743,22 @@ __global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const
                                        const double *__restrict__ qy, double k, int npx, int npy, int nsplit,
                                        const float *__restrict__ ampscale, float *__restrict__ I) {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= (int64_t)npx * npy) return;
+    const int item = blockIdx.y;
+    const size_t npix = (size_t)npx * npy;
+    if (p >= (int64_t)npix) return;
     const int a = (int)(p % npx), b = (int)(p / npx);
+    const float2 *part = partial + (size_t)item * nsplit * npix;
     float re = 0.f, im = 0.f;
     for (int s = 0; s < nsplit; ++s) {
-        const float2 v = partial[(size_t)s * npx * npy + p];
+        const float2 v = part[(size_t)s * npix + p];
         re += v.x;
         im += v.y;
     }
-    const float sc = ampscale[0];
+    const float sc = ampscale[item];
     re *= sc;
     im *= sc;
     const bool real = qx[a] * qx[a] + qy[b] * qy[b] <= k * k;
-    I[p] = real ? re * re + im * im : 0.f;
+    I[(size_t)item * npix + p] = real ? re * re + im * im : 0.f;
 }
 
 // ------------------------------------------------------------------------------------------------ host
@@ -757,8 +772,14 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     int L = 0;
     while ((1 << L) < p.nx) ++L;
     t.L = L;
+    // items per chunk (stacked along z, one set of launches per chunk): as many as keep the H planes of a chunk under 4 GB
+    const size_t h_item = (size_t)8 * p.nz * t.NPXP * t.NY;
+    size_t nb = ((size_t)4 << 30) / (h_item ? h_item : 1);
+    if (nb > (size_t)p.batch) nb = (size_t)p.batch;
+    if (nb * p.nz > 60000) nb = 60000 / (size_t)p.nz;   // global slice index and TMA row coordinates stay small
+    t.nb = nb < 1 ? 1 : (int)nb;
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
-    const int base = (t.NPYP / kM) * (t.NPXP / kNyz) * t.ng;
+    const int base = (t.NPYP / kM) * (t.NPXP / kNyz) * t.ng * t.nb;
     int best = 1;
     double best_cost = 1e300;
     const int max_z = p.nz < 32 ? p.nz : 32;
@@ -774,7 +795,7 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
     const int nta = t.NPXP / t.NX;
     int nsx = (2 * num_sms + nta - 1) / nta;   // two balanced items per CTA
-    t.nsx = nsx < 1 ? 1 : nsx > p.nz ? p.nz : nsx;
+    t.nsx = nsx < 1 ? 1 : nsx > p.nz * t.nb ? p.nz * t.nb : nsx;
     return t;
 }
 
@@ -788,7 +809,7 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 }
 
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
-                             const unsigned char *d_flags64, const int *d_bounds, const double *d_qx, int npx,
+                             const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
     constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;
     static bool attr_set = false;
@@ -806,7 +827,7 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         ok = encode_map(&tmA, d_Eyp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
     if (ok) {
-        const cuuint64_t rows = (cuuint64_t)p.nz * t.NPXP;
+        const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
         cuuint64_t dims[3] = {(cuuint64_t)t.NY, rows, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
         cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kNyz, 1};
@@ -817,27 +838,26 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         return cudaErrorUnknown;
     }
     SepYzParams P;
-    P.nz = p.nz; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
+    P.nz = p.nz; P.nb = nb; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
     P.ntb = t.NPYP / kM; P.nta = t.NPXP / kNyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
     P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
-    const int nitems = P.ntb * P.nta * P.ng * P.nzs;
+    const int nitems = P.ntb * P.nta * P.ng * P.nzs * nb;
     const int grid = nitems < num_sms ? nitems : num_sms;
     sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
     return cudaGetLastError();
 }
 
-cudaError_t launch_sep_tc_prep_item(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t,
-                                    __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_scaleH,
-                                    float *d_ampscale, cudaStream_t st) {
-    const int nyb = t.NY / kKB;
-    cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)p.nz * nyb, st);
+cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
+                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st) {
+    const int nyb = t.NY / kKB, nzt = p.nz * nb;
+    cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
     if (e != cudaSuccess) return e;
-    const int64_t nthreads = (int64_t)p.nz * t.NY * (t.NXP / 8);
-    sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, t.NY, t.NXP, d_maxbits,
+    const int64_t nthreads = (int64_t)nzt * t.NY * (t.NXP / 8);
+    sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nzt, t.NY, t.NXP, d_maxbits,
                                                                              d_Rp, d_flags64);
-    sep_tc_scale_kernel<<<1, 1, 0, st>>>(d_maxbits, t.L, (float)(p.dx * p.dy * p.dz), d_scaleH, d_ampscale);
-    sep_tc_bounds_kernel<<<t.ng + 1, 32, 0, st>>>(d_flags64, p.nz, nyb, t.ng, t.nsx, t.nzs, d_bounds, d_bounds + (t.nsx + 1));
+    sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
+    sep_tc_bounds_kernel<<<1 + nb * t.ng, 32, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, t.nsx, t.nzs, d_bounds, d_bounds + (t.nsx + 1));
     return cudaGetLastError();
 }
 
@@ -857,12 +877,12 @@ static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &t
 }
 
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
-                            const unsigned char *d_flags64, const int *d_bounds, __half *d_Hp, int num_sms, cudaStream_t st,
-                            std::string *err) {
+                            const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
+                            cudaStream_t st, std::string *err) {
     CUtensorMap tmA, tmB;
     bool ok;
     {
-        const cuuint64_t rows = (cuuint64_t)p.nz * t.NY;
+        const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NY;
         cuuint64_t dims[3] = {(cuuint64_t)t.NXP, rows, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * rows * 2};
         cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
@@ -879,7 +899,7 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
         return cudaErrorUnknown;
     }
     SepXParams P;
-    P.nz = p.nz; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / t.NX; P.nsx = t.nsx;
+    P.nz = p.nz * nb; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / t.NX; P.nsx = t.nsx;
     P.nkb = t.NY / kKB;
     P.hscale = ldexpf(1.f, -9 - t.L);
     P.flags = d_flags64; P.zb = d_bounds; P.Hp = d_Hp;
@@ -891,11 +911,12 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
 }
 
 cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
-                                   const Plan &p, const SepTcPlan &t, const float *d_ampscale, float *d_I, cudaStream_t st) {
+                                   const Plan &p, const SepTcPlan &t, int nb, const float *d_ampscale, float *d_I,
+                                   cudaStream_t st) {
     const int64_t npix = (int64_t)npx * npy;
     const double k = 2.0 * 3.14159265358979323846 / p.lambda;
-    sep_tc_finalize_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, st>>>(d_partial, d_qx, d_qy, k, npx, npy, t.nsplit,
-                                                                          d_ampscale, d_I);
+    sep_tc_finalize_kernel<<<dim3((unsigned)((npix + 255) / 256), nb), 256, 0, st>>>(d_partial, d_qx, d_qy, k, npx, npy, t.nsplit,
+                                                                                    d_ampscale, d_I);
     return cudaGetLastError();
 }
 

@@ -67,6 +67,44 @@ def test_sparse_blobs_and_evanescent_points(sm, method):
     assert_parity(I, ref, what=f"qgrid sparse {method}")
 
 
+@both_methods
+def test_batch_with_a_vacuum_item_and_a_single_voxel(sm, method):
+    """Items are stacked along z inside one set of launches: an all-vacuum item must come out exactly 0, a single voxel as
+    |rho dV|^2 at every propagating grid point, and neither may disturb its neighbours."""
+    nx, ny, nz = 40, 70, 9
+    voxel, lam = (2.0, 2.0, 3.0), 12.0
+    g = np.stack([W.random_grid(60 + i, nx, ny, nz, fill=0.3) for i in range(5)])
+    g[1] = 0.0
+    g[3] = 0.0
+    g[3, 4, 33, 17] = (0.02, 0.003)
+    k = 2 * np.pi / lam
+    qx, qy = np.linspace(-0.7 * k, 0.9 * k, 45), np.linspace(-0.5 * k, 0.5 * k, 31)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
+    _, ok = O.qgrid_q(qx, qy, lam)
+    ok = ok.reshape(31, 45)
+    assert np.all(I[1] == 0)
+    one = (0.02 ** 2 + 0.003 ** 2) * (2.0 * 2.0 * 3.0) ** 2
+    assert np.allclose(I[3][ok], one, rtol=2e-5) and np.all(I[3][~ok] == 0)
+    for b in (0, 2, 4):
+        assert_parity(I[b], O.simulate_qgrid(g[b], voxel, lam, qx, qy), what=f"qgrid {method} batch item {b}")
+
+
+def test_batch_larger_than_one_chunk(sm):
+    """The H planes of a chunk are capped at 4 GB: nine items of 512 MB each run as a chunk of eight and a chunk of one.
+    Checked at seeded grid points of three items."""
+    nx, ny, nz, B_ = 16, 900, 64, 9
+    voxel, lam = (3.0, 1.0, 2.0), 9.0
+    g = np.stack([W.sparse_blobs_grid(300 + i, nx, ny, nz, nblobs=5, max_extent=12) for i in range(B_)])
+    k = 2 * np.pi / lam
+    qx, qy = np.linspace(-0.6 * k, 0.6 * k, 1000), np.linspace(-0.3 * k, 0.3 * k, 8)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS["tensor"]).cpu().numpy()
+    q, ok = O.qgrid_q(qx, qy, lam)
+    pix = W.sample_pixels(17, 8000, 60)
+    for b in (0, 7, 8):
+        ref = O.simulate_q(g[b], voxel, lam, q[pix]) * ok[pix]
+        assert_parity(I[b].ravel()[pix], ref, what=f"qgrid chunked batch item {b}")
+
+
 @pytest.mark.parametrize("nx", [300, 530, 1100])
 def test_wide_grids_use_narrower_stage_x_tiles(sm, nx):
     """nx > 256 / > 512: stage X keeps 32- / 16-column Ex tiles resident; nx > 1024 falls back to the CUDA-core stages."""
