@@ -738,6 +738,270 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     }
 }
 
+// ---- stage YZ with 128-column accumulators ------------------------------------------------------------------------
+// Same work as sep_tc_yz_kernel with UMMA 128 x 128 x 16: at N = 128 the instruction's 64 tensor cycles cover its
+// shared-memory operand fetch (8 KB), at N = 64 they do not (48.7 cycles for 32 of work).  H tiles of 128 columns stream
+// plane by plane through a ring of 6 x 16 KB (as the rho~ tiles of stage X); two accumulator buffers of D_re, D_im x 128
+// columns.  An epilogue thread now carries 64 columns: 128 running totals + 64 phase fractions, more than the 168 registers
+// a 384-thread CTA gives each thread, so the register file is re-split with setmaxnreg: the producer / issuer warpgroup
+// drops to 48 registers per thread, the two epilogue warpgroups rise to 224: 128 x 48 + 256 x 224 = 63488 <= the 384 x 168 =
+// 64512 registers the CTA owns (an increase can only take what the CTA's own warps released, or it waits forever).
+__device__ __forceinline__ void setmaxnreg_inc_224() { asm volatile("setmaxnreg.inc.sync.aligned.u32 224;"); }
+__device__ __forceinline__ void setmaxnreg_dec_48() { asm volatile("setmaxnreg.dec.sync.aligned.u32 48;"); }
+
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
+    constexpr int kN = 128;
+    constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
+    constexpr int kStages = 6;                        // single-plane 64-y blocks of an H tile: 128 rows x 128 bytes = 16 KB
+    constexpr int kNB = 2;                            // accumulator buffers (256 columns each)
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sA = smem;
+    uint8_t *sB = smem + kSmemA;
+    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kSlotA);
+    uint64_t *a_full = bars + 0, *a_empty = bars + 1;
+    uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
+    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nitems = P.ntb * P.nta * P.ng * P.nzs * P.nb;
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(a_full, 1);
+        ptx::mbar_init(a_empty, 2);
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(b_full + i, 1);
+            ptx::mbar_init(b_empty + i, 2);
+        }
+        for (int i = 0; i < kNB; ++i) {
+            ptx::mbar_init(t_full + i, 2);
+            ptx::mbar_init(t_empty + i, 8);
+            ptx::mbar_init(first_done + i, 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    auto zrange = [&](const YzItem &it, int &z0, int &z1) {
+        const int *zb = P.zb + (size_t)(it.b * P.ng + it.g) * (P.nzs + 1) + it.s;
+        z0 = __ldg(zb);
+        z1 = __ldg(zb + 1);
+    };
+
+    if (warp < 4) {
+      setmaxnreg_dec_48();
+      if (warp == 0) {
+        // ===================================================================== TMA producer
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const YzItem it = yz_decode(item, P);
+            ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
+                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)kSmemA);
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int kb = 0; kb < 2; ++kb)
+                        ptx::tma_load_3d(sA + (pl * 2 + kb) * kSlotA, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
+            }
+            __syncwarp();
+            int z0, z1;
+            zrange(it, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                const int j = z0 + n;
+                for (int kb = 0; kb < 2; ++kb) {
+                    if (((f >> kb) & 1u) == 0u) continue;
+                    for (int pl = 0; pl < 4; ++pl) {
+                        ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                        if (ptx::elect_one()) {
+                            ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kSlotA);
+                            ptx::tma_load_3d(sB + slot * kSlotA, &tmB, b_full + slot, (it.g * 2 + kb) * kKB,
+                                             j * P.NPXP + it.ta * kN, pl);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+                }
+            }
+        }
+      } else if (warp == 1 || warp == 3) {
+        // ===================================================================== MMA issuers (k-step ks belongs to issuer ks % 2)
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, kN, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, kN, true);
+        const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
+        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
+        constexpr uint64_t kA = kSlotA >> 4;
+        const int iw = warp >> 1;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        int it_local = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
+            const YzItem it = yz_decode(item, P);
+            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+            ptx::tc_fence_after();
+            int z0, z1;
+            zrange(it, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                bool first = true;
+                for (int kb = 0; kb < 2; ++kb) {
+                    if (((f >> kb) & 1u) == 0u) continue;
+                    for (int pl = 0; pl < 4; ++pl) {
+                        if (first && pl == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
+                            ptx::mbar_wait(first_done + buf, upar);
+                            ptx::tc_fence_after();
+                        }
+                        ptx::mbar_wait(b_full + slot, phase);
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+#pragma unroll
+                            for (int kk = 0; kk < 2; ++kk) {
+                                const int ks = 2 * kk + iw;
+                                const uint64_t b = descB0 + (uint64_t)slot * kA + (uint64_t)(ks * 2);
+                                const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
+                                const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
+                                const uint32_t acc0 = (first && pl == 0 && ks == 0) ? 0u : 1u;
+                                // (Ar + i Ai)(Br + i Bi), B = the H plane of this stage, three split products AhBh + AlBh + AhBl
+                                if (pl == 0) {          // B Re_hi
+                                    ptx::umma_f16(d_re, a_reh, b, idesc_pos, acc0);
+                                    ptx::umma_f16(d_im, a_imh, b, idesc_pos, acc0);
+                                    ptx::umma_f16(d_re, a_rel, b, idesc_pos, 1u);
+                                    ptx::umma_f16(d_im, a_iml, b, idesc_pos, 1u);
+                                } else if (pl == 1) {   // B Re_lo
+                                    ptx::umma_f16(d_re, a_reh, b, idesc_pos, 1u);
+                                    ptx::umma_f16(d_im, a_imh, b, idesc_pos, 1u);
+                                } else if (pl == 2) {   // B Im_hi
+                                    ptx::umma_f16(d_re, a_imh, b, idesc_neg, 1u);
+                                    ptx::umma_f16(d_im, a_reh, b, idesc_pos, 1u);
+                                    ptx::umma_f16(d_re, a_iml, b, idesc_neg, 1u);
+                                    ptx::umma_f16(d_im, a_rel, b, idesc_pos, 1u);
+                                } else {                // B Im_lo
+                                    ptx::umma_f16(d_re, a_imh, b, idesc_neg, 1u);
+                                    ptx::umma_f16(d_im, a_reh, b, idesc_pos, 1u);
+                                }
+                                if (first && pl == 0 && iw == 0 && kk == 0) ptx::umma_commit(first_done + buf);
+                            }
+                            ptx::umma_commit(b_empty + slot);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+                    first = false;
+                }
+                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                __syncwarp();
+                ++u;
+            }
+            if (ptx::elect_one()) ptx::umma_commit(a_empty);
+            __syncwarp();
+        }
+      }
+    } else {
+        setmaxnreg_inc_224();
+        // ===================================================================== epilogue: Blocks 7-8, 64 columns per thread
+        const int lg = warp & 3, ch = (warp - 4) >> 2;
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 64);
+        uint32_t u = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            const YzItem it = yz_decode(item, P);
+            const int b = it.tb * kM + lg * 32 + lane;
+            const int a0 = it.ta * kN + ch * 64;
+            const double qyb = b < P.npy ? P.qy[b] : 0.0;
+            uint32_t dph[64];
+#pragma unroll
+            for (int c = 0; c < 64; ++c) {
+                const int a = a0 + c;
+                double t = 0.0;
+                if (a < P.npx && b < P.npy) {
+                    const double qxa = P.qx[a];
+                    const double qxy2 = qxa * qxa + qyb * qyb;
+                    const double kz2 = P.k * P.k - qxy2;
+                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
+                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
+                    t -= rint(t);
+                }
+                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
+            }
+            float2 tot[64];
+#pragma unroll
+            for (int c = 0; c < 64; ++c) tot[c] = make_float2(0.f, 0.f);
+            int z0, z1;
+            zrange(it, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
+            int n;
+            uint32_t f;
+            while (un.next(n, f)) {
+                const int j = z0 + n - it.b * P.nz;
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
+                ptx::mbar_wait(t_full + buf, upar);
+                ptx::tc_fence_after();
+                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+#pragma unroll
+                for (int q8 = 0; q8 < 8; ++q8) {
+                    uint32_t gre[8], gim[8];
+                    ptx::tmem_ld8(t_re + q8 * 8, gre);
+                    ptx::tmem_ld8(t_im + q8 * 8, gim);
+                    ptx::tmem_ld_wait();
+                    if (q8 == 7) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int c = q8 * 8 + i;
+                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
+                        float sn, cs;
+                        __sincosf(ang, &sn, &cs);
+                        const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
+                        tot[c].x = fmaf(cs, gr, tot[c].x);
+                        tot[c].x = fmaf(-sn, gi, tot[c].x);
+                        tot[c].y = fmaf(cs, gi, tot[c].y);
+                        tot[c].y = fmaf(sn, gr, tot[c].y);
+                    }
+                }
+                ++u;
+            }
+            if (b < P.npy) {
+                float2 *dst = P.partial + (((size_t)it.b * P.ng * P.nzs + it.g * P.nzs + it.s) * P.npy + b) * P.npx;
+#pragma unroll
+                for (int c = 0; c < 64; ++c)
+                    if (a0 + c < P.npx) dst[a0 + c] = tot[c];
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
+    }
+}
+
 // I[b][a] = |ampscale * sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
 __global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
                                        const double *__restrict__ qy, double k, int npx, int npy, int nsplit,
@@ -766,7 +1030,8 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     SepTcPlan t;
     t.NY = (p.ny + 127) / 128 * 128;
     t.NXP = (p.nx + kKB - 1) / kKB * kKB;
-    t.NPXP = (npx + kNyz - 1) / kNyz * kNyz;
+    t.nyz = npx > kNyz ? 128 : kNyz;   // stage YZ accumulator width: 128 columns (full-rate UMMA) unless the grid is narrower
+    t.NPXP = (npx + t.nyz - 1) / t.nyz * t.nyz;
     t.NPYP = (npy + kM - 1) / kM * kM;
     t.ng = t.NY / 128;
     int L = 0;
@@ -779,7 +1044,7 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     if (nb * p.nz > 60000) nb = 60000 / (size_t)p.nz;   // global slice index and TMA row coordinates stay small
     t.nb = nb < 1 ? 1 : (int)nb;
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
-    const int base = (t.NPYP / kM) * (t.NPXP / kNyz) * t.ng * t.nb;
+    const int base = (t.NPYP / kM) * (t.NPXP / t.nyz) * t.ng * t.nb;
     int best = 1;
     double best_cost = 1e300;
     const int max_z = p.nz < 32 ? p.nz : 32;
@@ -811,10 +1076,11 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
                              const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
-    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;
+    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // both variants: 128 KB + 96 KB ring
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yz128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -830,7 +1096,7 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
         cuuint64_t dims[3] = {(cuuint64_t)t.NY, rows, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
-        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kNyz, 1};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)t.nyz, 1};
         ok = encode_map(&tmB, d_Hp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
     if (!ok) {
@@ -839,12 +1105,13 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     }
     SepYzParams P;
     P.nz = p.nz; P.nb = nb; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
-    P.ntb = t.NPYP / kM; P.nta = t.NPXP / kNyz; P.nkb = t.NY / kKB;
+    P.ntb = t.NPYP / kM; P.nta = t.NPXP / t.nyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
     P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
     const int nitems = P.ntb * P.nta * P.ng * P.nzs * nb;
     const int grid = nitems < num_sms ? nitems : num_sms;
-    sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
+    if (t.nyz == 128) sep_tc_yz128_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
+    else sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
     return cudaGetLastError();
 }
 
