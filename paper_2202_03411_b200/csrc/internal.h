@@ -76,7 +76,7 @@ struct SepTcPlan {
     int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
     int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
     int NX = 64, nsx = 1;                      // stage X: a columns per tile, z splits
-    int nyz = 64;                              // stage YZ: a columns per accumulator (128, or 64 for narrow grids)
+    int nyz = 64, yz_ncta = 1;                 // stage YZ: a columns per accumulator (128, or 64 for narrow grids), CTAs per work item
     int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);

@@ -14,6 +14,9 @@
 // turns = 4e-7 rad), and sin / cos come from the SFU on an argument in [-pi, pi) (absolute error ~4e-7).
 #include <cuda.h>
 
+#include <cstdio>
+#include <cstdlib>
+
 #include "internal.h"
 #include "ptx_sm100.h"
 
@@ -480,6 +483,22 @@ __device__ __forceinline__ YzItem yz_decode(int item, const SepYzParams &P) {
     return it;
 }
 
+// items of the CTA-pair variant: a pair index replaces the b tile, this CTA's tile is NCTA tp + rank
+template <int NCTA>
+__device__ __forceinline__ YzItem yz_decode_n(int item, const SepYzParams &P, int rank) {
+    YzItem it;
+    const int ntp = P.ntb / NCTA;
+    it.tb = (item % ntp) * NCTA + rank;
+    item /= ntp;
+    it.ta = item % P.nta;
+    item /= P.nta;
+    it.g = item % P.ng;
+    item /= P.ng;
+    it.s = item % P.nzs;
+    it.b = item / P.nzs;
+    return it;
+}
+
 __global__ void __launch_bounds__(kThreadsTc, 1)
 sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
     constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
@@ -749,24 +768,38 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 __device__ __forceinline__ void setmaxnreg_inc_224() { asm volatile("setmaxnreg.inc.sync.aligned.u32 224;"); }
 __device__ __forceinline__ void setmaxnreg_dec_48() { asm volatile("setmaxnreg.dec.sync.aligned.u32 48;"); }
 
+// NCTA = 2: a CTA pair per work item (tcgen05 cta_group::2, UMMA 256 x 128 x 16): each CTA owns one b tile (its Ey tile, its
+// accumulators, its epilogue) and HALF of every H tile (64 of the 128 a rows), so an instruction fetches 4 KB of A + 2 KB of B
+// per SM for its 64 tensor cycles -- at 128 B/clk that leaves the shared-memory port slack, where a single CTA (8 KB per 64
+// cycles) has none and measured 54 % tensor-pipe activity.  The leader (rank 0) issues every MMA; full barriers live in the
+// leader, empty barriers are signalled in both CTAs (the protocol of tensor_kernel.cu).
+template <int NCTA>
 __global__ void __launch_bounds__(kThreadsTc, 1)
 sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
     constexpr int kN = 128;
     constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
-    constexpr int kStages = 6;                        // single-plane 64-y blocks of an H tile: 128 rows x 128 bytes = 16 KB
+    constexpr int kSlotB = kSlotA / NCTA;             // this CTA's part of a single-plane 64-y block of an H tile (kN / NCTA rows)
+    // A stage = G planes of one 64-y block.  A pair's halves are small enough for all four planes (48 MMAs per barrier round
+    // trip); a single CTA streams plane by plane (8 or 4 MMAs per stage: the issue overhead shows).
+    constexpr int kG = NCTA == 2 ? 4 : 1;
+    constexpr int kStageB = kG * kSlotB;              // 32 KB (pair) / 16 KB (single)
+    constexpr int kStages = NCTA == 2 ? 3 : 6;
     constexpr int kNB = 2;                            // accumulator buffers (256 columns each)
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *sA = smem;
     uint8_t *sB = smem + kSmemA;
-    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kSlotA);
+    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kStageB);
     uint64_t *a_full = bars + 0, *a_empty = bars + 1;
     uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
     uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
     uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nitems = P.ntb * P.nta * P.ng * P.nzs * P.nb;
+    const uint32_t rank = NCTA == 2 ? ptx::cluster_ctarank() : 0u;
+    const bool leader = rank == 0;
+    const int cluster_id = blockIdx.x / NCTA, nclusters = gridDim.x / NCTA;
+    const int nitems = (P.ntb / NCTA) * P.nta * P.ng * P.nzs * P.nb;   // an item covers NCTA b tiles: tb = NCTA tp + rank
 
     if (warp == 0 && lane == 0) {
         ptx::tma_prefetch_desc(&tmA);
@@ -781,15 +814,19 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         }
         for (int i = 0; i < kNB; ++i) {
             ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 8);
+            ptx::mbar_init(t_empty + i, 8 * NCTA);
             ptx::mbar_init(first_done + i, 1);
         }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
     }
-    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
+    if (warp == 2) {
+        if (NCTA == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
+        else ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
+    }
     ptx::tc_fence_before();
     __syncthreads();
+    if (NCTA == 2) ptx::cluster_sync_all();   // peer barriers are initialised before anyone signals them
     ptx::tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
 
@@ -806,14 +843,17 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         int slot = 0;
         uint32_t phase = 0;
         int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const YzItem it = yz_decode(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
             ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
             if (ptx::elect_one()) {
-                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)kSmemA);
+                if (leader) ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(NCTA * kSmemA));
                 for (int pl = 0; pl < 4; ++pl)
-                    for (int kb = 0; kb < 2; ++kb)
-                        ptx::tma_load_3d(sA + (pl * 2 + kb) * kSlotA, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
+                    for (int kb = 0; kb < 2; ++kb) {
+                        void *dst = sA + (pl * 2 + kb) * kSlotA;
+                        if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
+                        else ptx::tma_load_3d(dst, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
+                    }
             }
             __syncwarp();
             int z0, z1;
@@ -826,12 +866,22 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                 const int j = z0 + n;
                 for (int kb = 0; kb < 2; ++kb) {
                     if (((f >> kb) & 1u) == 0u) continue;
-                    for (int pl = 0; pl < 4; ++pl) {
+                    for (int pg = 0; pg < 4 / kG; ++pg) {
                         ptx::mbar_wait(b_empty + slot, phase ^ 1);
                         if (ptx::elect_one()) {
-                            ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kSlotA);
-                            ptx::tma_load_3d(sB + slot * kSlotA, &tmB, b_full + slot, (it.g * 2 + kb) * kKB,
-                                             j * P.NPXP + it.ta * kN, pl);
+#ifdef SEPABL_YZ_NOLOAD   // debug-only ablation (built by _work scripts; never in the product build)
+                            if (leader) ptx::mbar_arrive(b_full + slot);
+                            (void)j;
+#else
+                            if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)(NCTA * kStageB));   // both halves land on the leader's barrier
+                            const int row = j * P.NPXP + it.ta * kN + (int)rank * (kN / NCTA);
+#pragma unroll
+                            for (int q = 0; q < kG; ++q) {
+                                void *dst = sB + slot * kStageB + q * kSlotB;
+                                if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
+                                else ptx::tma_load_3d(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
+                            }
+#endif
                         }
                         __syncwarp();
                         if (++slot == kStages) { slot = 0; phase ^= 1; }
@@ -839,19 +889,31 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                 }
             }
         }
-      } else if (warp == 1 || warp == 3) {
+      } else if ((warp == 1 || warp == 3) && leader) {
         // ===================================================================== MMA issuers (k-step ks belongs to issuer ks % 2)
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, kN, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, kN, true);
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM * NCTA, kN, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM * NCTA, kN, true);
+        auto mma = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
+            if (NCTA == 2) ptx::umma_f16_2sm(d, a, b, idesc, acc);
+            else ptx::umma_f16(d, a, b, idesc, acc);
+        };
+        auto commit = [](uint64_t *bar) {         // in every CTA of the pair
+            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x3);
+            else ptx::umma_commit(bar);
+        };
+        auto commit_local = [](uint64_t *bar) {   // this (leader) CTA's barrier only
+            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x1);
+            else ptx::umma_commit(bar);
+        };
         const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
         const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
-        constexpr uint64_t kA = kSlotA >> 4;
+        constexpr uint64_t kA = kSlotA >> 4, kB = kSlotB >> 4;
         const int iw = warp >> 1;
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const YzItem it = yz_decode(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
             ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             int z0, z1;
@@ -868,8 +930,8 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                 bool first = true;
                 for (int kb = 0; kb < 2; ++kb) {
                     if (((f >> kb) & 1u) == 0u) continue;
-                    for (int pl = 0; pl < 4; ++pl) {
-                        if (first && pl == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
+                    for (int pg = 0; pg < 4 / kG; ++pg) {
+                        if (first && pg == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
                             ptx::mbar_wait(first_done + buf, upar);
                             ptx::tc_fence_after();
                         }
@@ -879,42 +941,46 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
 #pragma unroll
                             for (int kk = 0; kk < 2; ++kk) {
                                 const int ks = 2 * kk + iw;
-                                const uint64_t b = descB0 + (uint64_t)slot * kA + (uint64_t)(ks * 2);
                                 const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
                                 const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
-                                const uint32_t acc0 = (first && pl == 0 && ks == 0) ? 0u : 1u;
-                                // (Ar + i Ai)(Br + i Bi), B = the H plane of this stage, three split products AhBh + AlBh + AhBl
-                                if (pl == 0) {          // B Re_hi
-                                    ptx::umma_f16(d_re, a_reh, b, idesc_pos, acc0);
-                                    ptx::umma_f16(d_im, a_imh, b, idesc_pos, acc0);
-                                    ptx::umma_f16(d_re, a_rel, b, idesc_pos, 1u);
-                                    ptx::umma_f16(d_im, a_iml, b, idesc_pos, 1u);
-                                } else if (pl == 1) {   // B Re_lo
-                                    ptx::umma_f16(d_re, a_reh, b, idesc_pos, 1u);
-                                    ptx::umma_f16(d_im, a_imh, b, idesc_pos, 1u);
-                                } else if (pl == 2) {   // B Im_hi
-                                    ptx::umma_f16(d_re, a_imh, b, idesc_neg, 1u);
-                                    ptx::umma_f16(d_im, a_reh, b, idesc_pos, 1u);
-                                    ptx::umma_f16(d_re, a_iml, b, idesc_neg, 1u);
-                                    ptx::umma_f16(d_im, a_rel, b, idesc_pos, 1u);
-                                } else {                // B Im_lo
-                                    ptx::umma_f16(d_re, a_imh, b, idesc_neg, 1u);
-                                    ptx::umma_f16(d_im, a_reh, b, idesc_pos, 1u);
+#pragma unroll
+                                for (int q = 0; q < kG; ++q) {
+                                    const int pl = pg * kG + q;
+                                    const uint64_t b = descB0 + (uint64_t)slot * (kStageB >> 4) + (uint64_t)q * kB + (uint64_t)(ks * 2);
+                                    const uint32_t acc0 = (first && pl == 0 && ks == 0) ? 0u : 1u;
+                                    // (Ar + i Ai)(Br + i Bi), B = H plane pl of this stage, three split products AhBh + AlBh + AhBl
+                                    if (pl == 0) {          // B Re_hi
+                                        mma(d_re, a_reh, b, idesc_pos, acc0);
+                                        mma(d_im, a_imh, b, idesc_pos, acc0);
+                                        mma(d_re, a_rel, b, idesc_pos, 1u);
+                                        mma(d_im, a_iml, b, idesc_pos, 1u);
+                                    } else if (pl == 1) {   // B Re_lo
+                                        mma(d_re, a_reh, b, idesc_pos, 1u);
+                                        mma(d_im, a_imh, b, idesc_pos, 1u);
+                                    } else if (pl == 2) {   // B Im_hi
+                                        mma(d_re, a_imh, b, idesc_neg, 1u);
+                                        mma(d_im, a_reh, b, idesc_pos, 1u);
+                                        mma(d_re, a_iml, b, idesc_neg, 1u);
+                                        mma(d_im, a_rel, b, idesc_pos, 1u);
+                                    } else {                // B Im_lo
+                                        mma(d_re, a_imh, b, idesc_neg, 1u);
+                                        mma(d_im, a_reh, b, idesc_pos, 1u);
+                                    }
                                 }
-                                if (first && pl == 0 && iw == 0 && kk == 0) ptx::umma_commit(first_done + buf);
+                                if (first && pg == 0 && iw == 0 && kk == 0) commit_local(first_done + buf);
                             }
-                            ptx::umma_commit(b_empty + slot);
+                            commit(b_empty + slot);
                         }
                         __syncwarp();
                         if (++slot == kStages) { slot = 0; phase ^= 1; }
                     }
                     first = false;
                 }
-                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
+                if (ptx::elect_one()) commit(t_full + buf);
                 __syncwarp();
                 ++u;
             }
-            if (ptx::elect_one()) ptx::umma_commit(a_empty);
+            if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
         }
       }
@@ -924,8 +990,8 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         const int lg = warp & 3, ch = (warp - 4) >> 2;
         const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 64);
         uint32_t u = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-            const YzItem it = yz_decode(item, P);
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
             const int b = it.tb * kM + lg * 32 + lane;
             const int a0 = it.ta * kN + ch * 64;
             const double qyb = b < P.npy ? P.qy[b] : 0.0;
@@ -960,6 +1026,17 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+#ifdef SEPABL_YZ_NOEPI
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);
+                    else ptx::mbar_arrive(t_empty + buf);
+                }
+                ++u;
+                tot[0].x += (float)(mult + t_im);
+                continue;
+#endif
 #pragma unroll
                 for (int q8 = 0; q8 < 8; ++q8) {
                     uint32_t gre[8], gim[8];
@@ -969,7 +1046,10 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                     if (q8 == 7) {
                         ptx::tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);
+                        if (lane == 0) {
+                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                            else ptx::mbar_arrive(t_empty + buf);
+                        }
                     }
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
@@ -996,9 +1076,11 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
     }
     ptx::tc_fence_before();
     __syncthreads();
+    if (NCTA == 2) ptx::cluster_sync_all();   // nobody leaves while the peer may still signal its barriers
     if (warp == 2) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
+        if (NCTA == 2) ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
+        else ptx::tmem_dealloc(tmem_base, kTmemColsTc);
     }
 }
 
@@ -1044,13 +1126,16 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     if (nb * p.nz > 60000) nb = 60000 / (size_t)p.nz;   // global slice index and TMA row coordinates stay small
     t.nb = nb < 1 ? 1 : (int)nb;
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
-    const int base = (t.NPYP / kM) * (t.NPXP / t.nyz) * t.ng * t.nb;
+    // stage YZ runs on CTA pairs (UMMA 256 x 128) when it uses 128-column accumulators and the b tiles pair up
+    t.yz_ncta = (t.nyz == 128 && (t.NPYP / kM) % 2 == 0) ? 2 : 1;
+    const int base = (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * t.ng * t.nb;
+    const int workers = num_sms / t.yz_ncta;
     int best = 1;
     double best_cost = 1e300;
     const int max_z = p.nz < 32 ? p.nz : 32;
     for (int z = 1; z <= max_z; ++z) {
         const long long items = (long long)base * z;
-        const long long waves = (items + num_sms - 1) / num_sms;
+        const long long waves = (items + workers - 1) / workers;
         const double cost = (double)waves * ((double)((p.nz + z - 1) / z) + 3.0);
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = z; }
     }
@@ -1073,17 +1158,37 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
     return cudaGetLastError();
 }
 
-cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
-                             const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
-                             const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
-    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // both variants: 128 KB + 96 KB ring
+template <int NCTA>
+static cudaError_t launch_yz128_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepYzParams &P, int nitems, int num_sms,
+                                        int smem, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yz128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz128_kernel<NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
+    const int max_clusters = num_sms / NCTA;
+    const int nclusters = nitems < max_clusters ? nitems : max_clusters;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(nclusters * NCTA));
+    cfg.blockDim = dim3(kThreadsTc);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = NCTA;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, sep_tc_yz128_kernel<NCTA>, tmA, tmB, P);
+}
+
+cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
+                             const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
+                             const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
+    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // every variant: 128 KB resident + 96 KB ring
+    const int ncta = t.nyz == 128 ? t.yz_ncta : 1;
     CUtensorMap tmA, tmB;
     bool ok;
     {
@@ -1092,11 +1197,11 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
         ok = encode_map(&tmA, d_Eyp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
-    if (ok) {
+    if (ok) {   // box = one CTA's rows of an H tile
         const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
         cuuint64_t dims[3] = {(cuuint64_t)t.NY, rows, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
-        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)t.nyz, 1};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)(t.nyz / ncta), 1};
         ok = encode_map(&tmB, d_Hp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
     if (!ok) {
@@ -1108,10 +1213,17 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     P.ntb = t.NPYP / kM; P.nta = t.NPXP / t.nyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
     P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
-    const int nitems = P.ntb * P.nta * P.ng * P.nzs * nb;
-    const int grid = nitems < num_sms ? nitems : num_sms;
-    if (t.nyz == 128) sep_tc_yz128_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
-    else sep_tc_yz_kernel<<<grid, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
+    const int nitems = (P.ntb / ncta) * P.nta * P.ng * P.nzs * nb;
+    if (t.nyz == 128)
+        return ncta == 2 ? launch_yz128_variant<2>(tmA, tmB, P, nitems, num_sms, kSmem, st)
+                         : launch_yz128_variant<1>(tmA, tmB, P, nitems, num_sms, kSmem, st);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    sep_tc_yz_kernel<<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
     return cudaGetLastError();
 }
 

@@ -171,6 +171,19 @@ def test_full_size_cfg3_sampled_points(sm, method):
     assert_parity(I[pix], ref, what=f"qgrid cfg3 full sampled {method}")
 
 
+def test_odd_number_of_row_tiles_runs_single_ctas(sm):
+    """Stage YZ pairs the b tiles (UMMA 256 x 128); 384 grid rows = 3 tiles cannot pair and use one CTA per item."""
+    w = W.config(2, scale=0.25)
+    g = w.grid(0)
+    vox = (w.dx, w.dy, w.dz)
+    qx, qy = _uniform_q(w.lam, w.theta_max_deg, 200), _uniform_q(w.lam, w.theta_max_deg, 384)
+    I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy), method=METHODS["tensor"]).cpu().numpy()
+    q, ok = O.qgrid_q(qx, qy, w.lam)
+    pix = W.sample_pixels(5, 200 * 384, 400)
+    ref = O.simulate_q(g, vox, w.lam, q[pix]) * ok[pix]
+    assert_parity(I.ravel()[pix], ref, what="qgrid 3 row tiles")
+
+
 def test_error_codes(sm):
     import torch
     from paper_2202_03411_b200 import binding as B
