@@ -237,7 +237,7 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "fit"],
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
                          "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
@@ -287,7 +287,7 @@ def main():
     stream = torch.cuda.current_stream()
 
     qmethod = args.method if args.method in (0, 1, 3) else 0
-    if args.route == "qgrid":
+    if args.route in ("qgrid", "shapes_qgrid"):
         kk = 2 * np.pi / w.lam
         qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
         qy = torch.from_numpy((np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)).cuda()
@@ -298,6 +298,13 @@ def main():
         ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
 
     shapes = None
+    if args.route == "shapes_qgrid":
+        shapes = w.shapes(items)
+        if shapes is None:
+            raise SystemExit(f"{w.name} is not one shape per item: --route shapes_qgrid does not apply")
+        need = C.c_size_t(0)
+        sm._check(sm.lib.scatman_shapes_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
+        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
     if args.route == "shapes":
         shapes = w.shapes(items)
         if shapes is None:
@@ -310,6 +317,10 @@ def main():
         if args.route == "shapes":
             sm.simulate_shapes(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method,
                                workspace=ws, out=out, stream=stream)
+            return
+        if args.route == "shapes_qgrid":
+            sm.simulate_shapes_qgrid(shapes, (w.nx, w.ny, w.nz), vox, w.lam, qx, qy, method=qmethod, workspace=ws, out=out,
+                                     stream=stream)
             return
         if args.route == "qgrid":
             sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=stream)
@@ -352,7 +363,7 @@ def main():
     e2e_steps = max(1, min(args.steps, 3))
 
     def e2e_step():
-        if args.route == "shapes":  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
+        if args.route in ("shapes", "shapes_qgrid"):  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
             step()
             h_I.copy_(out, non_blocking=True)
             torch.cuda.synchronize()
@@ -382,7 +393,7 @@ def main():
     peaks = load_peaks()
     k_ms = sum(kernel_ms) / len(kernel_ms)
     dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
-    if args.route == "qgrid":
+    if args.route in ("qgrid", "shapes_qgrid"):
         dense_sep = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)   # both stages, 8 flop per complex MAC
         if qmethod == 3:
             # two FP32 complex GEMMs per slice on CUDA cores, dense count (vacuum rows are skipped)
@@ -484,13 +495,13 @@ def main():
 
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32" if (args.route == "qgrid" and qmethod == 3) or (args.route != "qgrid" and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route == "qgrid" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
-                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route != "shapes" else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
+                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route not in ("shapes", "shapes_qgrid") else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
                     "d2h_bytes_per_step": int(h_I.numel() * 4)},
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line), flush=True)

@@ -25,6 +25,7 @@ EXPORTS = [
     "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
     "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
+    "scatman_shapes_qgrid_workspace_bytes", "scatman_simulate_shapes_qgrid",
     "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
@@ -93,6 +94,9 @@ def load_library() -> C.CDLL:
     L.scatman_shapes_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i64, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
     L.scatman_simulate_shapes.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), dbl, C.POINTER(Detector),
                                           C.POINTER(Options), vp, C.c_size_t, vp, vp]
+    L.scatman_shapes_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
+    L.scatman_simulate_shapes_qgrid.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), dbl, vp, i32, vp, i32,
+                                                C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
     L.scatman_fit_workspace_bytes.argtypes = [vp, i64, i32, C.POINTER(C.c_size_t)]
     L.scatman_discrepancy.argtypes = [vp, vp, vp, i64, vp, i64, i32, i32, vp, C.c_size_t, vp, vp]
@@ -323,6 +327,32 @@ class Scatman:
         self._check(self.lib.scatman_simulate_shapes(self._ctx, arr, batch, C.byref(grid), float(lam), C.byref(det), C.byref(opts),
                                                      C.c_void_p(workspace.data_ptr()), workspace.numel(),
                                                      C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out
+
+    def simulate_shapes_qgrid(self, shapes: Sequence[dict], dims, voxel, lam: float, qx, qy, rho_mode: int = RHO_LINEAR,
+                              method: int = METHOD_AUTO, workspace=None, out=None, stream=None):
+        """Shape descriptors -> I float32 [B][npy][npx] on the tensor grid (qx[a], qy[b]): rendered on the device, then the
+        separable route (scatman_simulate_shapes_qgrid)."""
+        import torch
+        for q in (qx, qy):
+            if not (q.is_cuda and q.dtype == torch.float64 and q.is_contiguous() and q.dim() == 1):
+                raise ValueError("qx, qy must be contiguous 1-D CUDA float64 tensors")
+        nx, ny, nz = (int(v) for v in dims)
+        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+        batch, npx, npy = len(shapes), int(qx.numel()), int(qy.numel())
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_shapes_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(opts),
+                                                                  C.byref(need)))
+        if workspace is None:
+            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=qx.device)
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=qx.device)
+        arr, keep = self._shape_array(shapes)
+        self._check(self.lib.scatman_simulate_shapes_qgrid(self._ctx, arr, batch, C.byref(grid), float(lam),
+                                                           C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy,
+                                                           C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
+                                                           C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
     def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,

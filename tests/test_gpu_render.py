@@ -162,6 +162,27 @@ def test_simulate_shapes_equals_render_then_simulate_and_matches_oracle(sm):
         assert_parity(I[i], ref, what=f"shapes item {items[i]}")
 
 
+def test_simulate_shapes_qgrid_equals_render_then_qgrid_and_matches_oracle(sm):
+    """scatman_simulate_shapes_qgrid = scatman_render + scatman_simulate_qgrid on the rendered grids, and matches the oracle's
+    direct sum at the grid points (cfg4 shapes at quarter scale on a uniform (qx, qy) grid)."""
+    import torch
+    w = W.config(3, scale=0.25)
+    items = [0, 1, 2, 3, 4]
+    shapes = w.shapes(items)
+    dims, vox = (w.nx, w.ny, w.nz), (w.dx, w.dy, w.dz)
+    k = 2 * np.pi / w.lam
+    q1 = (np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * k * np.sin(np.radians(w.theta_max_deg)) / w.npx)
+    qx = qy = torch.from_numpy(q1).cuda()
+    I = sm.simulate_shapes_qgrid(shapes, dims, vox, w.lam, qx, qy)
+    g = sm.render(shapes, dims, vox)
+    I2 = sm.simulate_qgrid(g, vox, w.lam, qx, qy)
+    assert torch.allclose(I, I2, rtol=1e-4, atol=1e-6 * float(I2.max()))
+    I = I.cpu().numpy()
+    for i in (0, 3):
+        ref = O.simulate_qgrid(g[i].cpu().numpy(), vox, w.lam, q1, q1)
+        assert_parity(I[i], ref, what=f"shapes qgrid item {items[i]}")
+
+
 def test_workload_shape_descriptors_describe_the_same_particles_as_the_grids(sm):
     """The descriptors of cfg1 / cfg3 (identity orientation) render to exactly the voxel grids the generators produce."""
     for idx, scale in ((0, 1.0), (2, 0.25)):
