@@ -75,7 +75,7 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
 struct SepTcPlan {
     int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
     int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
-    int NX = 64, nsx = 1;                      // stage X: a columns per tile, z splits
+    int NX = 64, nsx = 1, x_ncta = 1;          // stage X: a columns per resident Ex tile, z splits, CTAs per work item
     int nyz = 64, yz_ncta = 1;                 // stage YZ: a columns per accumulator (128, or 64 for narrow grids), CTAs per work item
     int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };

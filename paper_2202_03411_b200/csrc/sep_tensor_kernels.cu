@@ -457,6 +457,246 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
 }
 
+// ---- stage X on CTA pairs ------------------------------------------------------------------------------------------
+// tcgen05 cta_group::2, UMMA 256 x 2NX x 16: the two CTAs of a pair take two consecutive live row tiles (each streams its own
+// rho~ tile, 128 rows = its half of M) against the same 2 NX grid columns, of whose Ex tile each CTA keeps NX rows resident.
+// Per SM an instruction then fetches 4 KB of A + 2 KB of B for 64 tensor cycles (N = 128) instead of 6 KB for 32 (N = 64 from
+// one CTA, shared-memory bound at 48.7 cycles).  Stages hold two planes (Re hi + lo, then Im hi + lo: 24 MMAs per barrier round
+// trip).  Each CTA converts and stores the H rows of its own tile; an odd last tile is run twice (the peer repeats the
+// leader's tile and discards it).  Leader-side barriers as in tensor_kernel.cu.
+template <int NX>
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_x2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepXParams P) {
+    constexpr int kN = 2 * NX;                    // accumulator columns
+    constexpr int kSmemE = 131072;                // resident Ex planes of this CTA's NX columns: [4][nkx][NX rows x 128 bytes]
+    constexpr int kStages = 3;                    // ring of two-plane 64-x blocks of this CTA's rho~ row tile (32 KB each)
+    constexpr int kStage = 2 * kSlotA;
+    constexpr int kBlkE = NX * kKB * 2;
+    constexpr int kNB = 2;                        // accumulator buffers (D_re, D_im of up to 128 columns each)
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sE = smem;
+    uint8_t *sR = smem + kSmemE;
+    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kStage);
+    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
+    uint64_t *r_full = bars + 2, *r_empty = r_full + kStages;
+    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();
+    const bool leader = rank == 0;
+    const int cluster_id = blockIdx.x / 2, nclusters = gridDim.x / 2;
+    const int nitems = P.nta * P.nsx;             // nta = tiles of 2 NX columns
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(e_full, 1);
+        ptx::mbar_init(e_empty, 2);
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(r_full + i, 1);
+            ptx::mbar_init(r_empty + i, 2);
+        }
+        for (int i = 0; i < kNB; ++i) {
+            ptx::mbar_init(t_full + i, 2);
+            ptx::mbar_init(t_empty + i, 16);
+            ptx::mbar_init(first_done + i, 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    auto zrange = [&](int s, int &z0, int &z1) {
+        z0 = __ldg(P.zb + s);
+        z1 = __ldg(P.zb + s + 1);
+    };
+    // the next pair of live units: n0 for the leader, n1 for the peer (n1 = n0 and dup = true when only one is left)
+    auto next_pair = [&](LiveUnits &un, int &n0, int &n1, bool &dup) {
+        uint32_t f;
+        if (!un.next(n0, f)) return false;
+        dup = !un.next(n1, f);
+        if (dup) n1 = n0;
+        return true;
+    };
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer (both CTAs)
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const int ta = item % P.nta, s = item / P.nta;
+            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
+                if (leader) ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(2 * 4 * P.nkx * kBlkE));
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int kx = 0; kx < P.nkx; ++kx)
+                        ptx::tma_load_3d_2sm(sE + (pl * P.nkx + kx) * kBlkE, &tmB, e_full, kx * kKB, ta * kN + (int)rank * NX, pl);
+            }
+            __syncwarp();
+            int z0, z1;
+            zrange(s, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n0, n1;
+            bool dup;
+            while (next_pair(un, n0, n1, dup)) {
+                const int n = leader ? n0 : n1;
+                const int j = z0 + n / P.ng, g = n % P.ng;
+                for (int kx = 0; kx < P.nkx; ++kx)
+                    for (int ph = 0; ph < 2; ++ph) {   // Re planes, Im planes
+                        ptx::mbar_wait(r_empty + slot, phase ^ 1);
+                        if (ptx::elect_one()) {
+                            if (leader) ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)(2 * kStage));
+                            ptx::tma_load_3d_2sm(sR + slot * kStage, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, 2 * ph);
+                            ptx::tma_load_3d_2sm(sR + slot * kStage + kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, 2 * ph + 1);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+            }
+        }
+    } else if ((warp == 1 || warp == 3) && leader) {
+        // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
+        const uint64_t descR0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sR));
+        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
+        constexpr uint64_t kR = kSlotA >> 4, kSt = kStage >> 4, kE = kBlkE >> 4;
+        const int iw = warp >> 1;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        int it_local = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            const int s = item / P.nta;
+            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
+            ptx::tc_fence_after();
+            const uint64_t kEpl = (uint64_t)P.nkx * kE;
+            int z0, z1;
+            zrange(s, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n0, n1;
+            bool dup;
+            while (next_pair(un, n0, n1, dup)) {
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                for (int kx = 0; kx < P.nkx; ++kx)
+                    for (int ph = 0; ph < 2; ++ph) {
+                        if (iw == 1 && kx == 0 && ph == 0) {   // D must have been initialised by issuer 0
+                            ptx::mbar_wait(first_done + buf, upar);
+                            ptx::tc_fence_after();
+                        }
+                        ptx::mbar_wait(r_full + slot, phase);
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+#pragma unroll
+                            for (int kk = 0; kk < 2; ++kk) {
+                                const int ks = 2 * kk + iw;
+                                const uint64_t a_hi = descR0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2), a_lo = a_hi + kR;
+                                const uint64_t e_reh = descE0 + (uint64_t)kx * kE + (uint64_t)(ks * 2);
+                                const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
+                                const uint32_t acc0 = (kx == 0 && ph == 0 && ks == 0) ? 0u : 1u;
+                                // (Ar + i Ai)(Er + i Ei), A = the rho~ planes of this stage, three split products AhEh + AlEh + AhEl
+                                if (ph == 0) {   // Re hi, Re lo
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_reh, idesc_pos, acc0);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_imh, idesc_pos, acc0);
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_rel, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_iml, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_lo, e_reh, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_lo, e_imh, idesc_pos, 1u);
+                                } else {         // Im hi, Im lo
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_imh, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_reh, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_iml, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_rel, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_lo, e_imh, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_lo, e_reh, idesc_pos, 1u);
+                                }
+                                if (iw == 0 && kk == 0 && kx == 0 && ph == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
+                            }
+                            ptx::umma_commit_2sm(r_empty + slot, (uint16_t)0x3);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+                if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
+                __syncwarp();
+                ++u;
+            }
+            if (ptx::elect_one()) ptx::umma_commit_2sm(e_empty, (uint16_t)0x3);
+            __syncwarp();
+        }
+    } else if (warp >= 4) {
+        // ===================================================================== epilogue: H rows of this CTA's tile -> FP16 planes
+        const int lg = warp & 3, ch = (warp - 4) >> 2;   // TMEM lane group; column half: [ch NX, +NX) of the 2 NX columns
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * NX);
+        const size_t plane = (size_t)P.nz * P.NPXP * P.NY;
+        uint32_t u = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            const int ta = item % P.nta, s = item / P.nta;
+            const int a0 = ta * kN + ch * NX;
+            int z0, z1;
+            zrange(s, z0, z1);
+            LiveUnits un;
+            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
+            int n0, n1;
+            bool dup;
+            while (next_pair(un, n0, n1, dup)) {
+                const int n = leader ? n0 : n1;
+                const int j = z0 + n / P.ng, g = n % P.ng;
+                const bool store = leader || !dup;
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                ptx::mbar_wait(t_full + buf, upar);
+                ptx::tc_fence_after();
+                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+                __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
+#pragma unroll 1
+                for (int c0 = 0; c0 < NX; c0 += 8) {
+                    uint32_t gre[8], gim[8];
+                    ptx::tmem_ld8(t_re + c0, gre);
+                    ptx::tmem_ld8(t_im + c0, gim);
+                    ptx::tmem_ld_wait();
+                    if (c0 + 8 >= NX) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                    }
+                    if (store) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            __half h[4];
+                            split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
+                            __half *d = dst + (size_t)(c0 + i) * P.NY;
+#pragma unroll
+                            for (int pl = 0; pl < 4; ++pl) d[pl * plane] = h[pl];
+                        }
+                    }
+                }
+                ++u;
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ stage YZ
 struct SepYzParams {
     int nz, nb, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nz: slices per item, nb: items of the chunk, nkb = NY / 64
@@ -1143,8 +1383,9 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     t.nsplit = t.ng * t.nzs;
     // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for ~4 waves of a-tile items
     t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
-    const int nta = t.NPXP / t.NX;
-    int nsx = (2 * num_sms + nta - 1) / nta;   // two balanced items per CTA
+    t.x_ncta = t.NPXP % (2 * t.NX) == 0 ? 2 : 1;   // CTA pairs (UMMA 256 x 2NX) when the column tiles pair up
+    const int nta = t.NPXP / (t.NX * t.x_ncta);
+    int nsx = (2 * (num_sms / t.x_ncta) + nta - 1) / nta;   // two balanced items per CTA (pair)
     t.nsx = nsx < 1 ? 1 : nsx > p.nz * t.nb ? p.nz * t.nb : nsx;
     return t;
 }
@@ -1255,6 +1496,32 @@ static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &t
     return cudaGetLastError();
 }
 
+template <int NX>
+static cudaError_t launch_x2_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
+                                     cudaStream_t st) {
+    constexpr int kSmem = 1024 + 131072 + 6 * kSlotA + 256;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sep_tc_x2_kernel<NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int nitems = P.nta * P.nsx, max_clusters = num_sms / 2;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(2 * (nitems < max_clusters ? nitems : max_clusters)));
+    cfg.blockDim = dim3(kThreadsTc);
+    cfg.dynamicSmemBytes = kSmem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, sep_tc_x2_kernel<NX>, tmA, tmB, P);
+}
+
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
                             const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
                             cudaStream_t st, std::string *err) {
@@ -1278,10 +1545,18 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
         return cudaErrorUnknown;
     }
     SepXParams P;
-    P.nz = p.nz * nb; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / t.NX; P.nsx = t.nsx;
+    P.nz = p.nz * nb; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / (t.NX * t.x_ncta);
+    P.nsx = t.nsx;
     P.nkb = t.NY / kKB;
     P.hscale = ldexpf(1.f, -9 - t.L);
     P.flags = d_flags64; P.zb = d_bounds; P.Hp = d_Hp;
+    if (t.x_ncta == 2) {
+        switch (t.NX) {
+            case 64: return launch_x2_variant<64>(tmA, tmB, P, num_sms, st);
+            case 32: return launch_x2_variant<32>(tmA, tmB, P, num_sms, st);
+            default: return launch_x2_variant<16>(tmA, tmB, P, num_sms, st);
+        }
+    }
     switch (t.NX) {
         case 64: return launch_x_variant<64>(tmA, tmB, P, num_sms, st);
         case 32: return launch_x_variant<32>(tmA, tmB, P, num_sms, st);
