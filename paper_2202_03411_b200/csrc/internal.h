@@ -77,6 +77,7 @@ struct SepTcPlan {
     int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
     int NX = 64, nsx = 1, x_ncta = 1;          // stage X: a columns per resident Ex tile, z splits, CTAs per work item
     int nyz = 64, yz_ncta = 1;                 // stage YZ: a columns per accumulator (128, or 64 for narrow grids), CTAs per work item
+    bool yz_stream = false;                    // stage YZ: one accumulator per slice, both operands streamed (sep_tc_yzs_kernel)
     int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);

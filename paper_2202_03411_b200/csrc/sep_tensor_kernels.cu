@@ -25,6 +25,17 @@ namespace scatman {
 bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
                 const cuuint32_t *box, CUtensorMapSwizzle swizzle);   // tensor_kernel.cu
 
+#ifdef SEP_TIMING
+// debug-only cycle accounting of the stage YZ issuers (built by _work scripts with -DSEP_TIMING; never in the product build)
+__device__ long long g_sep_timing[74 * 2 * 8];
+extern "C" int scatman_debug_sep_timing(long long *h_out) {
+    return (int)cudaMemcpyFromSymbol(h_out, g_sep_timing, sizeof(long long) * 74 * 2 * 8);
+}
+#define SEP_TIMED(acc, stmt) do { long long _t0 = clock64(); stmt; acc += clock64() - _t0; } while (0)
+#else
+#define SEP_TIMED(acc, stmt) stmt
+#endif
+
 namespace {
 
 constexpr int kM = 128;              // UMMA M: rows of the A operand tile
@@ -154,8 +165,8 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // Balanced z splits.  Sequence 0 (stage X): weight of slice j = its live 128-y row tiles; sequence 1 + g (stage YZ, group g):
 // its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
 // every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam.
-__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int nsx, int nzs,
-                                     int *__restrict__ bx, int *__restrict__ by) {
+__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int ngs, int gw,
+                                     int nsx, int nzs, int *__restrict__ bx, int *__restrict__ by) {   // ngs YZ groups of gw flags
     // bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
     // One warp per sequence, 32 slices per step: warp scan of the weights; the lane of slice j writes the bounds with
     // E(j - 1) < target(s) <= E(j) (E(-1) = -1; j = nz is a last, weightless slice so that E(nz) = total is covered).
@@ -164,8 +175,8 @@ __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, in
     const int seq = blockIdx.x, lane = threadIdx.x;
     const int ns = seq == 0 ? nsx : nzs;
     int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
-    const int gsel = seq == 0 ? 0 : (seq - 1) % ng;
-    const int jbase = seq == 0 ? 0 : ((seq - 1) / ng) * nz1;
+    const int gsel = seq == 0 ? 0 : (seq - 1) % ngs;
+    const int jbase = seq == 0 ? 0 : ((seq - 1) / ngs) * nz1;
     const int nz = seq == 0 ? nzt : nz1;
     if (seq == 0 && nzt > 4096) {   // many stacked items: equal slice counts per range balance well enough, no scan
         for (int sidx = lane; sidx <= ns; sidx += 32) out[sidx] = (int)(((long long)nzt * sidx) / ns);
@@ -178,7 +189,7 @@ __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, in
         if (seq == 0) {
             for (int g = 0; g < ng; ++g) w += (fl[2 * g] | fl[2 * g + 1]) != 0;
         } else {
-            w = (fl[2 * gsel] != 0) + (fl[2 * gsel + 1] != 0);
+            for (int q = 0; q < gw; ++q) w += fl[gw * gsel + q] != 0;
         }
         return w;
     };
@@ -1152,9 +1163,13 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
+#ifdef SEP_TIMING
+        long long w_afull = 0, w_tempty = 0, w_first = 0, w_bfull = 0;
+        const long long t_begin = clock64();
+#endif
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
             const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
-            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
+            SEP_TIMED(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
             ptx::tc_fence_after();
             int z0, z1;
             zrange(it, z0, z1);
@@ -1164,7 +1179,7 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
             uint32_t f;
             while (un.next(n, f)) {
                 const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                SEP_TIMED(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                 bool first = true;
@@ -1172,10 +1187,10 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                     if (((f >> kb) & 1u) == 0u) continue;
                     for (int pg = 0; pg < 4 / kG; ++pg) {
                         if (first && pg == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
-                            ptx::mbar_wait(first_done + buf, upar);
+                            SEP_TIMED(w_first, ptx::mbar_wait(first_done + buf, upar));
                             ptx::tc_fence_after();
                         }
-                        ptx::mbar_wait(b_full + slot, phase);
+                        SEP_TIMED(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
 #pragma unroll
@@ -1223,6 +1238,12 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
             if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
         }
+#ifdef SEP_TIMING
+        if (lane == 0) {
+            long long *o = g_sep_timing + ((blockIdx.x / NCTA) * 2 + iw) * 8;
+            o[0] = clock64() - t_begin; o[1] = w_afull; o[2] = w_tempty; o[3] = w_first; o[4] = w_bfull; o[5] = u;
+        }
+#endif
       }
     } else {
         setmaxnreg_inc_224();
@@ -1324,6 +1345,297 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
     }
 }
 
+// ---- stage YZ with one accumulator per slice: both operands streamed -------------------------------------------------------
+// With the Ey tile resident, a slice needs one accumulator pass PER 128-y group, and the per-element slice phase of the epilogue
+// (two SFU calls for every accumulator element) then costs more than the group's MMAs: measured, the issuers wait 38 % of the
+// kernel for an accumulator buffer.  Here a unit is a whole slice: every live 64-y block of it is one stage holding this CTA's
+// Ey block (4 planes x 16 KB) AND its half of the H block (4 x 8 KB), 96 KB, two stages.  Ey is re-streamed for every slice (from
+// L2: the tables are ~1 MB), which triples the L2 -> SM traffic and halves the epilogue work and the partial sums.  CTA pairs
+// only (cta_group::2, UMMA 256 x 128 x 16), slices of at most 32 blocks (N_y <= 2048); other cases use sep_tc_yz128_kernel.
+struct LiveSlices {   // the live slices of a z range with the bit mask of their live 64-y blocks, warp-cooperative as LiveUnits
+    const unsigned char *fl;
+    int nkb, z0, total, base, lane;
+    uint32_t cur, ahead, live;
+    __device__ __forceinline__ uint32_t load(int n) const {
+        if (n >= total) return 0u;
+        const unsigned char *p = fl + (size_t)(z0 + n) * nkb;
+        uint32_t m = 0u;
+        for (int kb = 0; kb < nkb; ++kb) m |= (uint32_t)(__ldg(p + kb) != 0) << kb;
+        return m;
+    }
+    __device__ __forceinline__ void begin(const unsigned char *flags, int nkb_, int z0_, int z1, int lane_) {
+        fl = flags; nkb = nkb_; z0 = z0_; lane = lane_;
+        total = z1 - z0_;
+        base = 0;
+        cur = load(lane);
+        ahead = load(32 + lane);
+        live = __ballot_sync(0xffffffffu, cur != 0u);
+    }
+    __device__ __forceinline__ bool next(int &n, uint32_t &m) {
+        while (live == 0u) {
+            base += 32;
+            if (base >= total) return false;
+            cur = ahead;
+            ahead = load(base + 32 + lane);
+            live = __ballot_sync(0xffffffffu, cur != 0u);
+        }
+        const int pos = __ffs((int)live) - 1;
+        live &= live - 1;
+        m = __shfl_sync(0xffffffffu, cur, pos);
+        n = base + pos;
+        return true;
+    }
+};
+
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_yzs_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
+    constexpr int kN = 128;
+    constexpr int kPartA = 4 * kSlotA;                // 65536: this CTA's Ey block, four planes
+    constexpr int kSlotB = kSlotA / 2;                // 8192: this CTA's half (64 rows) of one plane of an H block
+    constexpr int kStage = kPartA + 4 * kSlotB;       // 98304
+    constexpr int kStages = 2;
+    constexpr int kNB = 2;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sS = smem;
+    uint64_t *bars = (uint64_t *)(smem + kStages * kStage);
+    uint64_t *s_full = bars + 0, *s_empty = s_full + kStages;
+    uint64_t *t_full = s_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();
+    const bool leader = rank == 0;
+    const int cluster_id = blockIdx.x / 2, nclusters = gridDim.x / 2;
+    const int ntp = P.ntb / 2;
+    const int nitems = ntp * P.nta * P.nzs * P.nb;   // item -> (tile pair tp, a tile, z split, batch item); no y groups
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(s_full + i, 1);
+            ptx::mbar_init(s_empty + i, 2);
+        }
+        for (int i = 0; i < kNB; ++i) {
+            ptx::mbar_init(t_full + i, 2);
+            ptx::mbar_init(t_empty + i, 16);
+            ptx::mbar_init(first_done + i, 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    auto decode = [&](int item, int &tb, int &ta, int &sp, int &bi) {
+        tb = (item % ntp) * 2 + (int)rank;
+        item /= ntp;
+        ta = item % P.nta;
+        item /= P.nta;
+        sp = item % P.nzs;
+        bi = item / P.nzs;
+    };
+    auto zrange = [&](int bi, int sp, int &z0, int &z1) {   // global slice indices
+        const int *zb = P.zb + (size_t)bi * (P.nzs + 1) + sp;
+        z0 = __ldg(zb);
+        z1 = __ldg(zb + 1);
+    };
+
+    if (warp < 4) {
+      setmaxnreg_dec_48();
+      if (warp == 0) {
+        // ===================================================================== TMA producer (both CTAs)
+        int slot = 0;
+        uint32_t phase = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            int tb, ta, sp, bi;
+            decode(item, tb, ta, sp, bi);
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const int j = z0 + n;
+                for (int kb = 0; kb < P.nkb; ++kb) {
+                    if (((m >> kb) & 1u) == 0u) continue;
+                    ptx::mbar_wait(s_empty + slot, phase ^ 1);
+                    if (ptx::elect_one()) {
+                        if (leader) ptx::mbar_arrive_expect_tx(s_full + slot, (uint32_t)(2 * kStage));   // both CTAs' parts
+                        uint8_t *st = sS + slot * kStage;
+                        const int row = j * P.NPXP + ta * kN + (int)rank * (kN / 2);
+#pragma unroll
+                        for (int pl = 0; pl < 4; ++pl) {
+                            ptx::tma_load_3d_2sm(st + pl * kSlotA, &tmA, s_full + slot, kb * kKB, tb * kM, pl);
+                            ptx::tma_load_3d_2sm(st + kPartA + pl * kSlotB, &tmB, s_full + slot, kb * kKB, row, pl);
+                        }
+                    }
+                    __syncwarp();
+                    if (++slot == kStages) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+      } else if ((warp == 1 || warp == 3) && leader) {
+        // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
+        const uint64_t descS0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sS));
+        constexpr uint64_t kA = kSlotA >> 4, kB = kSlotB >> 4, kSt = kStage >> 4, kPa = kPartA >> 4;
+        const int iw = warp >> 1;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            int tb, ta, sp, bi;
+            decode(item, tb, ta, sp, bi);
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                bool first = true;
+                for (int kb = 0; kb < P.nkb; ++kb) {
+                    if (((m >> kb) & 1u) == 0u) continue;
+                    if (first && iw == 1) {   // D must have been initialised by issuer 0's first k-step
+                        ptx::mbar_wait(first_done + buf, upar);
+                        ptx::tc_fence_after();
+                    }
+                    ptx::mbar_wait(s_full + slot, phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+                            const int ks = 2 * kk + iw;
+                            const uint64_t a_reh = descS0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2);
+                            const uint64_t a_rel = a_reh + kA, a_imh = a_rel + kA, a_iml = a_imh + kA;
+                            const uint64_t b_reh = descS0 + (uint64_t)slot * kSt + kPa + (uint64_t)(ks * 2);
+                            const uint64_t b_rel = b_reh + kB, b_imh = b_rel + kB, b_iml = b_imh + kB;
+                            const uint32_t acc0 = (first && ks == 0) ? 0u : 1u;
+                            ptx::umma_f16_2sm(d_re, a_reh, b_reh, idesc_pos, acc0);
+                            ptx::umma_f16_2sm(d_im, a_imh, b_reh, idesc_pos, acc0);
+                            ptx::umma_f16_2sm(d_re, a_rel, b_reh, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_im, a_iml, b_reh, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_re, a_reh, b_rel, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_im, a_imh, b_rel, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_re, a_imh, b_imh, idesc_neg, 1u);
+                            ptx::umma_f16_2sm(d_im, a_reh, b_imh, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_re, a_iml, b_imh, idesc_neg, 1u);
+                            ptx::umma_f16_2sm(d_im, a_rel, b_imh, idesc_pos, 1u);
+                            ptx::umma_f16_2sm(d_re, a_imh, b_iml, idesc_neg, 1u);
+                            ptx::umma_f16_2sm(d_im, a_reh, b_iml, idesc_pos, 1u);
+                            if (first && iw == 0 && kk == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
+                        }
+                        ptx::umma_commit_2sm(s_empty + slot, (uint16_t)0x3);
+                    }
+                    __syncwarp();
+                    first = false;
+                    if (++slot == kStages) { slot = 0; phase ^= 1; }
+                }
+                if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
+                __syncwarp();
+                ++u;
+            }
+        }
+      }
+    } else {
+        setmaxnreg_inc_224();
+        // ===================================================================== epilogue: Blocks 7-8, 64 columns per thread
+        const int lg = warp & 3, ch = (warp - 4) >> 2;
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 64);
+        uint32_t u = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            int tb, ta, sp, bi;
+            decode(item, tb, ta, sp, bi);
+            const int b = tb * kM + lg * 32 + lane;
+            const int a0 = ta * kN + ch * 64;
+            const double qyb = b < P.npy ? P.qy[b] : 0.0;
+            uint32_t dph[64];
+#pragma unroll
+            for (int c = 0; c < 64; ++c) {
+                const int a = a0 + c;
+                double t = 0.0;
+                if (a < P.npx && b < P.npy) {
+                    const double qxa = P.qx[a];
+                    const double qxy2 = qxa * qxa + qyb * qyb;
+                    const double kz2 = P.k * P.k - qxy2;
+                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
+                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
+                    t -= rint(t);
+                }
+                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
+            }
+            float2 tot[64];
+#pragma unroll
+            for (int c = 0; c < 64; ++c) tot[c] = make_float2(0.f, 0.f);
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const int j = z0 + n - bi * P.nz;
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
+                ptx::mbar_wait(t_full + buf, upar);
+                ptx::tc_fence_after();
+                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+#pragma unroll
+                for (int q8 = 0; q8 < 8; ++q8) {
+                    uint32_t gre[8], gim[8];
+                    ptx::tmem_ld8(t_re + q8 * 8, gre);
+                    ptx::tmem_ld8(t_im + q8 * 8, gim);
+                    ptx::tmem_ld_wait();
+                    if (q8 == 7) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int c = q8 * 8 + i;
+                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
+                        float sn, cs;
+                        __sincosf(ang, &sn, &cs);
+                        const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
+                        tot[c].x = fmaf(cs, gr, tot[c].x);
+                        tot[c].x = fmaf(-sn, gi, tot[c].x);
+                        tot[c].y = fmaf(cs, gi, tot[c].y);
+                        tot[c].y = fmaf(sn, gr, tot[c].y);
+                    }
+                }
+                ++u;
+            }
+            if (b < P.npy) {
+                float2 *dst = P.partial + (((size_t)bi * P.nzs + sp) * P.npy + b) * P.npx;
+#pragma unroll
+                for (int c = 0; c < 64; ++c)
+                    if (a0 + c < P.npx) dst[a0 + c] = tot[c];
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
+    }
+}
+
 // I[b][a] = |ampscale * sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
 __global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
                                        const double *__restrict__ qy, double k, int npx, int npy, int nsplit,
@@ -1368,7 +1680,8 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
     // stage YZ runs on CTA pairs (UMMA 256 x 128) when it uses 128-column accumulators and the b tiles pair up
     t.yz_ncta = (t.nyz == 128 && (t.NPYP / kM) % 2 == 0) ? 2 : 1;
-    const int base = (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * t.ng * t.nb;
+    t.yz_stream = t.yz_ncta == 2 && t.NY / kKB <= 32;   // one accumulator per slice, both operands streamed (sep_tc_yzs_kernel)
+    const int base = (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * (t.yz_stream ? 1 : t.ng) * t.nb;
     const int workers = num_sms / t.yz_ncta;
     int best = 1;
     double best_cost = 1e300;
@@ -1380,7 +1693,7 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = z; }
     }
     t.nzs = best;
-    t.nsplit = t.ng * t.nzs;
+    t.nsplit = (t.yz_stream ? 1 : t.ng) * t.nzs;
     // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for ~4 waves of a-tile items
     t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
     t.x_ncta = t.NPXP % (2 * t.NX) == 0 ? 2 : 1;   // CTA pairs (UMMA 256 x 2NX) when the column tiles pair up
@@ -1454,6 +1767,28 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     P.ntb = t.NPYP / kM; P.nta = t.NPXP / t.nyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
     P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
+    if (t.yz_stream) {
+        static bool attr_s = false;
+        if (!attr_s) {
+            cudaError_t e = cudaFuncSetAttribute(sep_tc_yzs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+            if (e != cudaSuccess) return e;
+            attr_s = true;
+        }
+        const int nit = (P.ntb / 2) * P.nta * P.nzs * nb, maxc = num_sms / 2;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
+        cfg.blockDim = dim3(kThreadsTc);
+        cfg.dynamicSmemBytes = kSmem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, sep_tc_yzs_kernel, tmA, tmB, P);
+    }
     const int nitems = (P.ntb / ncta) * P.nta * P.ng * P.nzs * nb;
     if (t.nyz == 128)
         return ncta == 2 ? launch_yz128_variant<2>(tmA, tmB, P, nitems, num_sms, kSmem, st)
@@ -1477,7 +1812,9 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
     sep_tc_pack_rho_kernel<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(d_rho, p.nx, p.ny, p.nz, nzt, t.NY, t.NXP, d_maxbits,
                                                                              d_Rp, d_flags64);
     sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
-    sep_tc_bounds_kernel<<<1 + nb * t.ng, 32, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, t.nsx, t.nzs, d_bounds, d_bounds + (t.nsx + 1));
+    const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;   // stage YZ's z splits: per item, or per item and 128-y group
+    sep_tc_bounds_kernel<<<1 + nb * ngs, 32, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, ngs, gw, t.nsx, t.nzs, d_bounds,
+                                                      d_bounds + (t.nsx + 1));
     return cudaGetLastError();
 }
 
