@@ -78,6 +78,8 @@ struct SepTcPlan {
     int NX = 64, nsx = 1, x_ncta = 1;          // stage X: a columns per resident Ex tile, z splits, CTAs per work item
     int nyz = 64, yz_ncta = 1;                 // stage YZ: a columns per accumulator (128, or 64 for narrow grids), CTAs per work item
     bool yz_stream = false;                    // stage YZ: one accumulator per slice, both operands streamed (sep_tc_yzs_kernel)
+    bool yz_t = false;                         // stage YZ transposed, Ey resident for all y (sep_tc_yzt_kernel<yzt_nb>)
+    int yzt_nb = 0;
     int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);

@@ -1636,6 +1636,295 @@ sep_tc_yzs_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
 }
 
+// ---- stage YZ transposed: D^T[a, b] = sum_y H_j[a, y] Ey[b, y], the Ey tile resident for ALL y -----------------------------
+// The roles of sep_tc_x2_kernel: the streamed A operand is each CTA's own H tile (128 grid columns a = the TMEM lanes, two
+// planes per stage), the resident B operand this CTA's NB rows of the Ey tile of 2 NB grid rows b, for every 64-y block
+// (NB nkb 8 KB <= 128 KB: NB = 64 for N_y <= 256, the only instance built; NB = 32 for N_y <= 512 ran UMMA N = 64 and measured
+// slower than the streamed form).  One accumulator per slice like sep_tc_yzs_kernel, but only H streams (2/3 of that kernel's
+// L2 -> SM traffic).  The epilogue thread owns one column a and NB rows b.
+template <int NB>
+__global__ void __launch_bounds__(kThreadsTc, 1)
+sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
+    constexpr int kN = 2 * NB;
+    constexpr int kSmemE = 131072;                // resident Ey planes of this CTA's NB rows: [4][nkb][NB rows x 128 bytes]
+    constexpr int kStages = 3;
+    constexpr int kStage = 2 * kSlotA;            // two planes of one 64-y block of this CTA's H tile
+    constexpr int kBlkE = NB * kKB * 2;
+    constexpr int kNB = 2;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *sE = smem;
+    uint8_t *sH = smem + kSmemE;
+    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kStage);
+    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
+    uint64_t *h_full = bars + 2, *h_empty = h_full + kStages;
+    uint64_t *t_full = h_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
+    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();
+    const bool leader = rank == 0;
+    const int cluster_id = blockIdx.x / 2, nclusters = gridDim.x / 2;
+    const int ntap = P.NPXP / (2 * kM);           // pairs of a tiles
+    const int ntbn = P.ntb * kM / kN;             // tiles of 2 NB grid rows
+    const int nitems = ntap * ntbn * P.nzs * P.nb;
+
+    if (warp == 0 && lane == 0) {
+        ptx::tma_prefetch_desc(&tmA);
+        ptx::tma_prefetch_desc(&tmB);
+    }
+    if (warp == 1 && lane == 0) {
+        ptx::mbar_init(e_full, 1);
+        ptx::mbar_init(e_empty, 2);
+        for (int i = 0; i < kStages; ++i) {
+            ptx::mbar_init(h_full + i, 1);
+            ptx::mbar_init(h_empty + i, 2);
+        }
+        for (int i = 0; i < kNB; ++i) {
+            ptx::mbar_init(t_full + i, 2);
+            ptx::mbar_init(t_empty + i, 16);
+            ptx::mbar_init(first_done + i, 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+    }
+    if (warp == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
+
+    auto decode = [&](int item, int &ta, int &tbn, int &sp, int &bi) {   // a pairs fastest: neighbours share the Ey tile
+        ta = (item % ntap) * 2 + (int)rank;
+        item /= ntap;
+        tbn = item % ntbn;
+        item /= ntbn;
+        sp = item % P.nzs;
+        bi = item / P.nzs;
+    };
+    auto zrange = [&](int bi, int sp, int &z0, int &z1) {
+        const int *zb = P.zb + (size_t)bi * (P.nzs + 1) + sp;
+        z0 = __ldg(zb);
+        z1 = __ldg(zb + 1);
+    };
+
+    if (warp < 4) {
+      setmaxnreg_dec_48();
+      if (warp == 0) {
+        // ===================================================================== TMA producer (both CTAs)
+        int slot = 0;
+        uint32_t phase = 0;
+        int it_local = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            int ta, tbn, sp, bi;
+            decode(item, ta, tbn, sp, bi);
+            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
+            if (ptx::elect_one()) {
+                if (leader) ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(2 * 4 * P.nkb * kBlkE));
+                for (int pl = 0; pl < 4; ++pl)
+                    for (int kb = 0; kb < P.nkb; ++kb)
+                        ptx::tma_load_3d_2sm(sE + (pl * P.nkb + kb) * kBlkE, &tmA, e_full, kb * kKB, tbn * kN + (int)rank * NB, pl);
+            }
+            __syncwarp();
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const int row = (z0 + n) * P.NPXP + ta * kM;
+                for (int kb = 0; kb < P.nkb; ++kb) {
+                    if (((m >> kb) & 1u) == 0u) continue;
+                    for (int ph = 0; ph < 2; ++ph) {   // Re planes, Im planes
+                        ptx::mbar_wait(h_empty + slot, phase ^ 1);
+                        if (ptx::elect_one()) {
+                            if (leader) ptx::mbar_arrive_expect_tx(h_full + slot, (uint32_t)(2 * kStage));
+                            ptx::tma_load_3d_2sm(sH + slot * kStage, &tmB, h_full + slot, kb * kKB, row, 2 * ph);
+                            ptx::tma_load_3d_2sm(sH + slot * kStage + kSlotA, &tmB, h_full + slot, kb * kKB, row, 2 * ph + 1);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+                }
+            }
+        }
+      } else if ((warp == 1 || warp == 3) && leader) {
+        // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
+        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
+        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
+        const uint64_t descH0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sH));
+        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
+        constexpr uint64_t kR = kSlotA >> 4, kSt = kStage >> 4, kE = kBlkE >> 4;
+        const int iw = warp >> 1;
+        int slot = 0;
+        uint32_t phase = 0, u = 0;
+        int it_local = 0;
+#ifdef SEP_TIMING
+        long long w_afull = 0, w_tempty = 0, w_first = 0, w_bfull = 0;
+        const long long t_begin = clock64();
+#endif
+        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
+            int ta, tbn, sp, bi;
+            decode(item, ta, tbn, sp, bi);
+            SEP_TIMED(w_afull, ptx::mbar_wait(e_full, (uint32_t)(it_local & 1)));
+            ptx::tc_fence_after();
+            const uint64_t kEpl = (uint64_t)P.nkb * kE;   // descriptor distance between Ey planes
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                SEP_TIMED(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
+                ptx::tc_fence_after();
+                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
+                bool first = true;
+                for (int kb = 0; kb < P.nkb; ++kb) {
+                    if (((m >> kb) & 1u) == 0u) continue;
+                    for (int ph = 0; ph < 2; ++ph) {
+                        if (first && ph == 0 && iw == 1) {   // D must have been initialised by issuer 0
+                            SEP_TIMED(w_first, ptx::mbar_wait(first_done + buf, upar));
+                            ptx::tc_fence_after();
+                        }
+                        SEP_TIMED(w_bfull, ptx::mbar_wait(h_full + slot, phase));
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+#pragma unroll
+                            for (int kk = 0; kk < 2; ++kk) {
+                                const int ks = 2 * kk + iw;
+                                const uint64_t a_hi = descH0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2), a_lo = a_hi + kR;
+                                const uint64_t e_reh = descE0 + (uint64_t)kb * kE + (uint64_t)(ks * 2);
+                                const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
+                                const uint32_t acc0 = (first && ph == 0 && ks == 0) ? 0u : 1u;
+                                // (Hr + i Hi)(Er + i Ei), the H planes of this stage as A, three split products HhEh + HlEh + HhEl
+                                if (ph == 0) {
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_reh, idesc_pos, acc0);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_imh, idesc_pos, acc0);
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_rel, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_iml, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_lo, e_reh, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_lo, e_imh, idesc_pos, 1u);
+                                } else {
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_imh, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_reh, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_hi, e_iml, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_hi, e_rel, idesc_pos, 1u);
+                                    ptx::umma_f16_2sm(d_re, a_lo, e_imh, idesc_neg, 1u);
+                                    ptx::umma_f16_2sm(d_im, a_lo, e_reh, idesc_pos, 1u);
+                                }
+                                if (first && ph == 0 && iw == 0 && kk == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
+                            }
+                            ptx::umma_commit_2sm(h_empty + slot, (uint16_t)0x3);
+                        }
+                        __syncwarp();
+                        if (++slot == kStages) { slot = 0; phase ^= 1; }
+                    }
+                    first = false;
+                }
+                if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
+                __syncwarp();
+                ++u;
+            }
+            if (ptx::elect_one()) ptx::umma_commit_2sm(e_empty, (uint16_t)0x3);
+            __syncwarp();
+        }
+#ifdef SEP_TIMING
+        if (lane == 0) {
+            long long *o = g_sep_timing + ((blockIdx.x / 2) * 2 + iw) * 8;
+            o[0] = clock64() - t_begin; o[1] = w_afull; o[2] = w_tempty; o[3] = w_first; o[4] = w_bfull; o[5] = u;
+        }
+#endif
+      }
+    } else {
+        setmaxnreg_inc_224();
+        // ===================================================================== epilogue: Blocks 7-8; thread = (column a, NB rows b)
+        const int lg = warp & 3, ch = (warp - 4) >> 2;
+        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * NB);
+        uint32_t u = 0;
+        for (int item = cluster_id; item < nitems; item += nclusters) {
+            int ta, tbn, sp, bi;
+            decode(item, ta, tbn, sp, bi);
+            const int a = ta * kM + lg * 32 + lane;
+            const int b0 = tbn * kN + ch * NB;
+            const double qxa = a < P.npx ? P.qx[a] : 0.0;
+            uint32_t dph[NB];
+#pragma unroll
+            for (int c = 0; c < NB; ++c) {
+                const int b = b0 + c;
+                double t = 0.0;
+                if (a < P.npx && b < P.npy) {
+                    const double qyb = P.qy[b];
+                    const double qxy2 = qxa * qxa + qyb * qyb;
+                    const double kz2 = P.k * P.k - qxy2;
+                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
+                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
+                    t -= rint(t);
+                }
+                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
+            }
+            float2 tot[NB];
+#pragma unroll
+            for (int c = 0; c < NB; ++c) tot[c] = make_float2(0.f, 0.f);
+            int z0, z1;
+            zrange(bi, sp, z0, z1);
+            LiveSlices un;
+            un.begin(P.flags, P.nkb, z0, z1, lane);
+            int n;
+            uint32_t m;
+            while (un.next(n, m)) {
+                const int j = z0 + n - bi * P.nz;
+                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
+                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
+                ptx::mbar_wait(t_full + buf, upar);
+                ptx::tc_fence_after();
+                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+#pragma unroll
+                for (int q8 = 0; q8 < NB / 8; ++q8) {
+                    uint32_t gre[8], gim[8];
+                    ptx::tmem_ld8(t_re + q8 * 8, gre);
+                    ptx::tmem_ld8(t_im + q8 * 8, gim);
+                    ptx::tmem_ld_wait();
+                    if (q8 == NB / 8 - 1) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int c = q8 * 8 + i;
+                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
+                        float sn, cs;
+                        __sincosf(ang, &sn, &cs);
+                        const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
+                        tot[c].x = fmaf(cs, gr, tot[c].x);
+                        tot[c].x = fmaf(-sn, gi, tot[c].x);
+                        tot[c].y = fmaf(cs, gi, tot[c].y);
+                        tot[c].y = fmaf(sn, gr, tot[c].y);
+                    }
+                }
+                ++u;
+            }
+            if (a < P.npx) {   // a warp stores 32 consecutive a of one grid row
+                float2 *dst = P.partial + ((size_t)bi * P.nzs + sp) * P.npy * P.npx + a;
+#pragma unroll
+                for (int c = 0; c < NB; ++c)
+                    if (b0 + c < P.npy) dst[(size_t)(b0 + c) * P.npx] = tot[c];
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    if (warp == 2) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
+    }
+}
+
 // I[b][a] = |ampscale * sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
 __global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
                                        const double *__restrict__ qy, double k, int npx, int npy, int nsplit,
@@ -1679,9 +1968,19 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     t.nb = nb < 1 ? 1 : (int)nb;
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
     // stage YZ runs on CTA pairs (UMMA 256 x 128) when it uses 128-column accumulators and the b tiles pair up
-    t.yz_ncta = (t.nyz == 128 && (t.NPYP / kM) % 2 == 0) ? 2 : 1;
-    t.yz_stream = t.yz_ncta == 2 && t.NY / kKB <= 32;   // one accumulator per slice, both operands streamed (sep_tc_yzs_kernel)
-    const int base = (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * (t.yz_stream ? 1 : t.ng) * t.nb;
+    // stage YZ variants, in order of preference (each needs its tiles to pair up for cta_group::2):
+    //   sep_tc_yzt_kernel   pairs of a tiles, Ey resident for all y (N_y <= 256)
+    //   sep_tc_yzs_kernel   pairs of b tiles, both operands streamed (N_y <= 2048)
+    //   sep_tc_yz128_kernel one CTA, Ey resident per 128-y group, one accumulator per (slice, group): any size
+    //   sep_tc_yz_kernel    the same with 64-column accumulators, for grids of at most 64 columns
+    t.yz_stream = t.nyz == 128 && (t.NPYP / kM) % 2 == 0 && t.NY / kKB <= 32;
+    t.yz_ncta = t.yz_stream ? 2 : 1;
+    // transposed form (sep_tc_yzt_kernel): pairs of a tiles, the Ey tile of 2 NB rows resident for all y
+    t.yzt_nb = t.NY / kKB <= 4 ? 64 : 0;   // (NB = 32 / 16 for taller grids run UMMA N = 64 / 32: measured slower than the streamed form)
+    t.yz_t = t.nyz == 128 && (t.NPXP / kM) % 2 == 0 && t.yzt_nb != 0;
+    if (t.yz_t) { t.yz_stream = true; t.yz_ncta = 2; }   // same bounds / partial layout as the streamed form
+    const int base = t.yz_t ? (t.NPXP / (2 * kM)) * (t.NPYP / (2 * t.yzt_nb)) * t.nb
+                            : (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * (t.yz_stream ? 1 : t.ng) * t.nb;
     const int workers = num_sms / t.yz_ncta;
     int best = 1;
     double best_cost = 1e300;
@@ -1767,6 +2066,41 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     P.ntb = t.NPYP / kM; P.nta = t.NPXP / t.nyz; P.nkb = t.NY / kKB;
     P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
     P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
+    if (t.yz_t) {
+        // A map: the Ey planes, box = this CTA's NB rows of one 64-y block; B map: the H planes, box = a whole a tile
+        cuuint64_t dimsA[3] = {(cuuint64_t)t.NY, (cuuint64_t)t.NPYP, 4};
+        cuuint64_t stridesA[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * (cuuint64_t)t.NPYP * 2};
+        cuuint32_t boxA[3] = {(cuuint32_t)kKB, (cuuint32_t)t.yzt_nb, 1};
+        const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
+        cuuint64_t dimsB[3] = {(cuuint64_t)t.NY, rows, 4};
+        cuuint64_t stridesB[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
+        cuuint32_t boxB[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
+        if (!encode_map(&tmA, d_Eyp, 3, dimsA, stridesA, boxA, CU_TENSOR_MAP_SWIZZLE_128B) ||
+            !encode_map(&tmB, d_Hp, 3, dimsB, stridesB, boxB, CU_TENSOR_MAP_SWIZZLE_128B)) {
+            if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
+            return cudaErrorUnknown;
+        }
+        const int nit = (t.NPXP / (2 * kM)) * (t.NPYP / (2 * t.yzt_nb)) * P.nzs * nb, maxc = num_sms / 2;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
+        cfg.blockDim = dim3(kThreadsTc);
+        cfg.dynamicSmemBytes = kSmem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        static bool attr_t = false;
+        if (!attr_t) {
+            cudaError_t e = cudaFuncSetAttribute(sep_tc_yzt_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
+            if (e != cudaSuccess) return e;
+            attr_t = true;
+        }
+        return cudaLaunchKernelEx(&cfg, sep_tc_yzt_kernel<64>, tmA, tmB, P);
+    }
     if (t.yz_stream) {
         static bool attr_s = false;
         if (!attr_s) {
@@ -1790,9 +2124,7 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         return cudaLaunchKernelEx(&cfg, sep_tc_yzs_kernel, tmA, tmB, P);
     }
     const int nitems = (P.ntb / ncta) * P.nta * P.ng * P.nzs * nb;
-    if (t.nyz == 128)
-        return ncta == 2 ? launch_yz128_variant<2>(tmA, tmB, P, nitems, num_sms, kSmem, st)
-                         : launch_yz128_variant<1>(tmA, tmB, P, nitems, num_sms, kSmem, st);
+    if (t.nyz == 128) return launch_yz128_variant<1>(tmA, tmB, P, nitems, num_sms, kSmem, st);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);

@@ -171,17 +171,19 @@ def test_full_size_cfg3_sampled_points(sm, method):
     assert_parity(I[pix], ref, what=f"qgrid cfg3 full sampled {method}")
 
 
-def test_odd_number_of_row_tiles_runs_single_ctas(sm):
-    """Stage YZ pairs the b tiles (UMMA 256 x 128); 384 grid rows = 3 tiles cannot pair and use one CTA per item."""
+@pytest.mark.parametrize("npx,npy", [(200, 384), (300, 200), (300, 384)])
+def test_tile_parities_select_the_stage_yz_variants(sm, npx, npy):
+    """Stage YZ pairs CTAs over two column tiles (2 x 3 tiles of 128: transposed form, Ey resident), else over two row tiles
+    (3 x 2: both operands streamed), else runs one CTA per item (3 x 3)."""
     w = W.config(2, scale=0.25)
     g = w.grid(0)
     vox = (w.dx, w.dy, w.dz)
-    qx, qy = _uniform_q(w.lam, w.theta_max_deg, 200), _uniform_q(w.lam, w.theta_max_deg, 384)
+    qx, qy = _uniform_q(w.lam, w.theta_max_deg, npx), _uniform_q(w.lam, w.theta_max_deg, npy)
     I = sm.simulate_qgrid(dev(g), vox, w.lam, dev(qx), dev(qy), method=METHODS["tensor"]).cpu().numpy()
     q, ok = O.qgrid_q(qx, qy, w.lam)
-    pix = W.sample_pixels(5, 200 * 384, 400)
+    pix = W.sample_pixels(5, npx * npy, 400)
     ref = O.simulate_q(g, vox, w.lam, q[pix]) * ok[pix]
-    assert_parity(I.ravel()[pix], ref, what="qgrid 3 row tiles")
+    assert_parity(I.ravel()[pix], ref, what=f"qgrid {npx} x {npy} points")
 
 
 def test_error_codes(sm):
