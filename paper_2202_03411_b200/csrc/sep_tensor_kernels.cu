@@ -1,13 +1,18 @@
 // sep_tensor_kernels.cu -- the separable tensor-grid route (Block 6 of Fig. 4 transforms every slice on a
 // uniform (qx, qy) grid) with both GEMM stages on tcgen05 tensor cores, FP16x3 split precision:
-//   stage X   H_j[a, y]  = sum_x rho~_j[y, x] e^{i qx[a] x}                  (M = 128 y rows, N = a columns, K = x)
-//   stage YZ  A[b, a]    = sum_j e^{i qz(a,b) z_j} sum_y e^{i qy[b] y} H_j[a, y]   (M = 128 b rows, N = 64 a columns, K = y)
+//   stage X   H_j[a, y]  = sum_x rho~_j[y, x] e^{i qx[a] x}                        (M = y rows, N = a columns, K = x)
+//   stage YZ  A[b, a]    = sum_j e^{i qz(a,b) z_j} sum_y e^{i qy[b] y} H_j[a, y]   (K = y; Blocks 7-8 in the epilogue)
 // Every operand is four FP16 planes (Re_hi, Re_lo, Im_hi, Im_lo) of a scaled FP32 value, K-major, fetched by TMA boxes of
 // 64 K x rows with the 128-byte swizzle; a complex product is the 12 real MMAs AhBh + AlBh + AhBl of tensor_kernel.cu
-// (the minus sign of Re = ArBr - AiBi is the instruction descriptor's negate-A bit).  Accumulators live in TMEM (four
-// buffers of D_re, D_im), FP32.  Stage X's epilogue rescales H and splits it into the FP16 planes stage YZ reads as its
-// B operand; stage YZ's epilogue is Blocks 7-8 of Fig. 4: the slice phase e^{i qz(a,b) z_j} applied to
-// the accumulator tile and the sum over slices, both in registers.  Vacuum is skipped in 64-y blocks (byte flags).
+// (the minus sign of Re = ArBr - AiBi is the instruction descriptor's negate-A bit).  Accumulators live in TMEM, FP32.
+// Stage X's epilogue rescales H and splits it into the FP16 planes stage YZ reads; stage YZ's epilogue applies the slice
+// phase e^{i qz(a,b) z_j} to the accumulator tile and sums over slices in registers.  Vacuum is skipped in 64-y blocks (byte
+// flags); batch items are stacked along z; z splits are balanced on the device by live tiles.
+// Kernels (each is selected by make_sep_tc_plan and covered by tests/test_gpu_qgrid.py):
+//   stage X   sep_tc_x2_kernel<NX>  CTA pairs, UMMA 256 x 2NX, Ex tile resident          | sep_tc_x_kernel<NX>  one CTA
+//   stage YZ  sep_tc_yzt_kernel<64> CTA pairs, transposed, Ey resident for all y (N_y <= 256)
+//             sep_tc_yzs_kernel     CTA pairs, both operands streamed (N_y <= 2048)
+//             sep_tc_yz128_kernel   one CTA, Ey resident per 128-y group (any size)      | sep_tc_yz_kernel  grids of <= 64 columns
 //
 // Slice phase: qz z_j = 2 pi t (2j - nz + 1) with t = qz dz / (4 pi) turns; frac(t) is kept as a 32-bit fixed-point
 // fraction of a turn, so the product with the integer (2j - nz + 1) wraps modulo one turn for free (error <= 512 * 2^-33
