@@ -418,7 +418,7 @@ def main():
                 issued += 24.0 * (grp.sum() * 128.0 * NXP * NPXP + blk.sum() * 64.0 * NPYP * NPXP)
             peak = peaks["sustained"]
             ach = issued / (k_ms * 1e-3) / 1e12
-            roofline = {"bound": "tensor", "kernel": "sep_tc_x_kernel + sep_tc_yz_kernel", "achieved": ach, "peak": peak,
+            roofline = {"bound": "tensor", "kernel": "sep_tc_x2_kernel + sep_tc_yzt_kernel (stage X + stage YZ variants of sep_tensor_kernels.cu)", "achieved": ach, "peak": peak,
                         "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
                         "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
                         "achieved_is": "issued tensor flop (24 per complex MAC of the live tiles: 8 flop x 3 split products) / "
