@@ -237,7 +237,7 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit"],
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit", "nufft"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
                          "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
@@ -297,6 +297,14 @@ def main():
         sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
         ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
 
+    nq = None
+    if args.route == "nufft":      # same flat detector, same result: 3-D type-2 NUFFT instead of the pixel x voxel contraction
+        det = B.Detector(w.npx, w.npy, w.theta_max_deg, 0.0, 0.0)
+        need = C.c_size_t(0)
+        sm._check(sm.lib.scatman_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)))
+        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+        nq = sm.nufft_grid_dims(grid, w.lam, det)
+
     shapes = None
     if args.route == "shapes_qgrid":
         shapes = w.shapes(items)
@@ -324,6 +332,9 @@ def main():
             return
         if args.route == "qgrid":
             sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=stream)
+            return
+        if args.route == "nufft":
+            sm.simulate_nufft(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, workspace=ws, out=out, stream=stream)
             return
         sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
                     workspace=ws, out=out, stream=stream)
@@ -367,7 +378,7 @@ def main():
             step()
             h_I.copy_(out, non_blocking=True)
             torch.cuda.synchronize()
-        elif args.route == "qgrid":   # no host-buffer C entry point for this route: the copies go through torch
+        elif args.route in ("qgrid", "nufft"):   # no host-buffer C entry point for this route: the copies go through torch
             d_dn.copy_(h_dn, non_blocking=True)
             step()
             h_I.copy_(out, non_blocking=True)
@@ -425,6 +436,17 @@ def main():
                                        "CUDA-event time of the per-item launches (pack, stage X, stage YZ, finalize)",
                         "issued_fraction_of_dense": issued / (3.0 * dense_sep),
                         "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12}
+    elif args.route == "nufft":
+        # three FP64 complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 12^3-point interpolation, CUDA cores:
+        # 8 flop per complex MAC of the GEMMs, 4 per (real weight x complex value) MAC of the interpolation.
+        nqx, nqy, nqz = nq
+        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * w.npix * 12 ** 3)
+        peak = 148 * 64 * 2 * 1.965e9 / 1e12           # FP64 FMA: 148 SMs x 64 lanes x 2 flop x max clock
+        ach = flop / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "nufft_zgemm_kernel (stages Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,
+                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms, "uniform_grid": [nqz, nqy, nqx],
+                    "achieved_is": "FP64 flop of the three GEMM stages and the interpolation / their CUDA-event time",
+                    "flop_vs_pixel_route": flop / (FLOP_PER_TERM * terms_per_pattern * batch)}
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
         # One extra, untimed call with the counting flag (same inputs, same schedule).
@@ -495,9 +517,9 @@ def main():
 
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f64" if args.route == "nufft" else "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route == "nufft" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",

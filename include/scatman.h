@@ -149,6 +149,24 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
                            int32_t batch, const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I,
                            void *cuda_stream);
 
+/* The flat detector by a 3-D type-2 non-uniform Fourier transform ("a type-2 NUFFT for the flat detector"):
+ * the SAME result as scatman_simulate -- A(p) = sum_r rho~(r) e^{i q(p).r} at every pixel's Ewald-sphere q (Eq. 2-4,
+ * PAPER.md:68-87), same a0 / a1 / a2 steps, conventions and output scale -- but rho~ is first transformed onto a small uniform
+ * (gz, gy, gx) grid covering the detector's q range (three FP64 complex GEMMs: slices, columns, rows; spacing 2 pi / (2 N d),
+ * Kaiser-Bessel pre-correction) and every pixel is then interpolated from its 12^3 nearest grid points.  The window's
+ * aliasing error is < 1e-9 of sum |rho~| dV per pixel; everything else is FP64, so north_star's tolerances against the direct
+ * sum hold (tests/test_gpu_nufft.py).  Work ~ N_vox * nqz + ... instead of N_vox * N_pix: ~1000x fewer multiply-adds.
+ * opts: rho_mode only (method, precision, flags ignored).  d_I[b][npy][npx].  The workspace depends on lambda and the
+ * detector (they fix the q range): scatman_nufft_workspace_bytes with the same arguments. */
+int scatman_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                                  int32_t batch, size_t *bytes);
+/* nq[3] = points per axis (x, y, z) of the uniform grid the route transforms onto (for work counts). */
+int scatman_nufft_grid_dims(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                            int32_t *nq);
+int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                           void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies h_dn to the device, runs
  * scatman_simulate on the context's own stream, copies I back into h_I and synchronises.  This entry
  * point alone owns device memory: a grow-only arena kept in the context until scatman_destroy.

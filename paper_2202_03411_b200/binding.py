@@ -26,6 +26,7 @@ EXPORTS = [
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
     "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
     "scatman_shapes_qgrid_workspace_bytes", "scatman_simulate_shapes_qgrid",
+    "scatman_nufft_workspace_bytes", "scatman_nufft_grid_dims", "scatman_simulate_nufft",
     "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
@@ -88,6 +89,10 @@ def load_library() -> C.CDLL:
                                      C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                         C.POINTER(Options), vp]
+    L.scatman_nufft_workspace_bytes.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), i32, C.POINTER(C.c_size_t)]
+    L.scatman_nufft_grid_dims.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(i32)]
+    L.scatman_simulate_nufft.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
+                                         C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
     L.scatman_simulate_qgrid.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i32, vp, i32, C.POINTER(dbl), i32,
                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
@@ -282,6 +287,33 @@ class Scatman:
         self._check(self.lib.scatman_simulate(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                               C.byref(det), qp, batch, C.byref(opts), C.c_void_p(workspace.data_ptr()),
                                               workspace.numel(), C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out if dn.dim() == 5 else out[0]
+
+    def nufft_grid_dims(self, grid, lam: float, det):
+        """(nqx, nqy, nqz): points per axis of the uniform grid scatman_simulate_nufft transforms onto."""
+        nq = (C.c_int32 * 3)()
+        self._check(self.lib.scatman_nufft_grid_dims(self._ctx, C.byref(grid), float(lam), C.byref(det), nq))
+        return int(nq[0]), int(nq[1]), int(nq[2])
+
+    def simulate_nufft(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
+                       rho_mode: int = RHO_LINEAR, cx: float = 0.0, cy: float = 0.0, workspace=None, out=None, stream=None):
+        """Same result as simulate() by the 3-D type-2 NUFFT route (scatman_simulate_nufft).  Asynchronous."""
+        import torch
+        self._check_dn(dn)
+        grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
+        opts = Options(int(rho_mode), 0, 0, 0)
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_nufft_workspace_bytes(self._ctx, C.byref(grid), float(lam), C.byref(det), batch,
+                                                           C.byref(need)))
+        if workspace is None:
+            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dn.device)
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_nufft(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
+                                                    C.byref(det), qp, batch, C.byref(opts), C.c_void_p(workspace.data_ptr()),
+                                                    workspace.numel(), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out if dn.dim() == 5 else out[0]
 
     def simulate_q(self, dn, voxel, lam: float, q, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,

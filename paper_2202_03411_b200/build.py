@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libscatman.so")
-SOURCES = ["api.cu", "fit_kernels.cu", "prep_kernels.cu", "render_kernels.cu", "sep_kernels.cu", "sep_tensor_kernels.cu", "simt_kernels.cu", "tensor_kernel.cu"]
+SOURCES = ["api.cu", "fit_kernels.cu", "nufft_kernels.cu", "prep_kernels.cu", "render_kernels.cu", "sep_kernels.cu", "sep_tensor_kernels.cu", "simt_kernels.cu", "tensor_kernel.cu"]
 HEADERS = ["internal.h", "ptx_sm100.h", os.path.join("..", "..", "include", "scatman.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false"]
 

@@ -600,6 +600,145 @@ int scatman_simulate_shapes_qgrid(scatman_ctx *ctx, const scatman_shape *h_shape
     return rc;
 }
 
+// ---- flat detector by a 3-D type-2 NUFFT (nufft_kernels.cu) ----------------------------------------------------------
+struct NufftLayout {
+    Plan p;
+    NufftPlan n;
+    size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_q = 0, off_tz = 0, off_tx = 0, off_ty = 0,
+           off_P = 0, off_H = 0, off_U = 0, total = 0;
+};
+// Range of q over the detector (host, FP64, a1's formula): q_x and q_y are monotonic along u and v and extremal in the other
+// coordinate on the rectangle's border; q_z <= 0 is monotonic in u^2 + v^2, so the border pixels plus q_z = 0 bound all three.
+static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const scatman_detector &det, int batch, int rho_mode) {
+    NufftLayout L;
+    Plan &p = L.p;
+    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
+    p.npix = (int64_t)det.npx * det.npy; p.batch = batch; p.rho_mode = rho_mode;
+    p.nvox = (int64_t)g.nx * g.ny * g.nz;
+    const double pi = 3.14159265358979323846;
+    const double k = 2.0 * pi / lambda;
+    const double pitch = 2.0 * tan(det.theta_max_deg * pi / 180.0) / (double)det.npx;
+    double lo[3] = {1e300, 1e300, 0.0}, hi[3] = {-1e300, -1e300, 0.0};
+    auto visit = [&](int ix, int iy) {
+        const double u = ((double)ix + 0.5 - 0.5 * (double)det.npx + det.cx) * pitch;
+        const double v = ((double)iy + 0.5 - 0.5 * (double)det.npy + det.cy) * pitch;
+        const double s2 = u * u + v * v, r = sqrt(s2 + 1.0);
+        const double q[3] = {k * u / r, k * v / r, -k * s2 / (r * (r + 1.0))};
+        for (int d = 0; d < 3; ++d) { lo[d] = q[d] < lo[d] ? q[d] : lo[d]; hi[d] = q[d] > hi[d] ? q[d] : hi[d]; }
+    };
+    for (int ix = 0; ix < det.npx; ++ix) { visit(ix, 0); visit(ix, det.npy - 1); }
+    for (int iy = 0; iy < det.npy; ++iy) { visit(0, iy); visit(det.npx - 1, iy); }
+    // the axes u = 0 and v = 0 cross the rectangle where |q_x| (|q_y|) along an edge peaks: cover them by the nearest pixels
+    for (int ix = 0; ix < det.npx; ++ix) {
+        int iy = (int)floor(0.5 * det.npy - det.cy);
+        for (int d = -1; d <= 1; ++d) if (iy + d >= 0 && iy + d < det.npy) visit(ix, iy + d);
+    }
+    for (int iy = 0; iy < det.npy; ++iy) {
+        int ix = (int)floor(0.5 * det.npx - det.cx);
+        for (int d = -1; d <= 1; ++d) if (ix + d >= 0 && ix + d < det.npx) visit(ix + d, iy);
+    }
+    const int N[3] = {g.nx, g.ny, g.nz};
+    const double dd[3] = {g.dx, g.dy, g.dz};
+    NufftAxis *ax[3] = {&L.n.ax, &L.n.ay, &L.n.az};
+    for (int d = 0; d < 3; ++d) {
+        const double h = 2.0 * pi / (2.0 * (double)N[d] * dd[d]);
+        ax[d]->inv_h = 1.0 / h;
+        const int m_lo = (int)floor(lo[d] / h - 0.5 * kNufftW) - 1;
+        const int m_hi = (int)ceil(hi[d] / h + 0.5 * kNufftW) + 1;
+        ax[d]->m_lo = m_lo;
+        ax[d]->nq = m_hi - m_lo + 1;
+    }
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
+    L.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
+    L.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
+    L.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    L.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    L.off_max = take(sizeof(unsigned) * (size_t)batch);
+    L.off_q = take(sizeof(double) * 3 * (size_t)p.npix);
+    L.off_tz = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz);
+    L.off_tx = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx);
+    L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
+    L.off_P = take(sizeof(double2) * (size_t)L.n.az.nq * g.ny * g.nx);
+    L.off_H = take(sizeof(double2) * (size_t)L.n.az.nq * g.ny * L.n.ax.nq);
+    L.off_U = take(sizeof(double2) * (size_t)L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
+    L.total = off;
+    return L;
+}
+
+int scatman_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                                  int32_t batch, size_t *bytes) {
+    if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
+    if (!valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) || batch < 1)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = make_nufft_layout(*grid, lambda, *det, batch, 0).total;
+    return SCATMAN_OK;
+}
+
+int scatman_nufft_grid_dims(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                            int32_t *nq) {
+    if (!ctx || !nq) return SCATMAN_INVALID_ARGUMENT;
+    if (!valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, 1, 0);
+    nq[0] = L.n.ax.nq; nq[1] = L.n.ay.nq; nq[2] = L.n.az.nq;
+    return SCATMAN_OK;
+}
+
+int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                           void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_dn || !d_I || !d_ws || !valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) ||
+        batch < 1 || batch > 65535 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    if (h_quat && !valid_quats(h_quat, batch)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "quaternion is not unit");
+    if (((uintptr_t)d_dn | (uintptr_t)d_ws | (uintptr_t)d_I) & 15)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
+    cudaSetDevice(ctx->device);
+    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, batch, o.rho_mode);
+    const Plan &p = L.p;
+    if (ws_bytes < L.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint8_t *ws = (uint8_t *)d_ws;
+    int nl = 0;
+    ctx->ev_valid = false;
+    ctx->d_count = nullptr;
+    double *q = (double *)(ws + L.off_q);
+    cudaError_t e = launch_qmap(*det, lambda, q, st);
+    ++nl;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+    const float *src = d_dn;
+    if (h_quat && !all_identity(h_quat, batch)) {
+        double *rm = (double *)(ws + L.off_rotmat);
+        e = upload_rotmats(h_quat, batch, rm, st, &nl);
+        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + L.off_rot), (int *)(ws + L.off_bbox), st);
+        nl += 3;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
+        src = (const float *)(ws + L.off_rot);
+    }
+    float *rho = (float *)(ws + L.off_rho);
+    e = launch_strength(src, p, batch, rho, (unsigned *)(ws + L.off_max), st);
+    ++nl;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    double2 *Tz = (double2 *)(ws + L.off_tz), *TxT = (double2 *)(ws + L.off_tx), *Ty = (double2 *)(ws + L.off_ty);
+    e = launch_nufft_tables(p, L.n, Tz, TxT, Ty, st);
+    nl += 3;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
+    cudaEventRecord(ctx->ev0, st);
+    for (int b = 0; b < batch; ++b) {
+        e = launch_nufft_item((const float2 *)rho + (size_t)b * p.nvox, p, L.n, Tz, TxT, Ty, q, (double2 *)(ws + L.off_P),
+                              (double2 *)(ws + L.off_H), (double2 *)(ws + L.off_U), d_I + (size_t)b * p.npix, st);
+        nl += 4;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");
+    }
+    cudaEventRecord(ctx->ev1, st);
+    ctx->ev_valid = true;
+    ctx->last_launches = nl;
+    return SCATMAN_OK;
+}
+
 // ---- forward-fitting pieces ---------------------------------------------------------------------------------------
 int scatman_fit_workspace_bytes(scatman_ctx *ctx, int64_t npix, int32_t batch, size_t *bytes) {
     if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;

@@ -1,0 +1,166 @@
+"""GPU parity of the flat-detector NUFFT route (scatman_simulate_nufft) against the FP64 oracle's direct sum:
+the same tolerances as the pixel x voxel contraction, on the same seeded inputs."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2202_03411_b200 import workloads as W
+from parity import assert_parity, metrics
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sm():
+    import torch
+    from paper_2202_03411_b200 import binding as B, build
+    build.build()
+    assert torch.cuda.is_available()
+    s = B.Scatman(0)
+    yield s
+    s.close()
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def test_cfg1_sphere_full_pattern(sm):
+    w = W.config(0)
+    g = w.grid(0)
+    I = sm.simulate_nufft(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg).cpu().numpy()
+    ref = O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg)
+    l2, pix = assert_parity(I, ref, what="nufft cfg1")
+    assert l2 <= 1e-6 and pix <= 1e-5      # FP64 throughout: only the FP32 store of rho~ and of I is left
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_ragged_random_batch_with_orientations(sm, mode):
+    """Odd sizes in x, y, z and on the detector (several GEMM tiles plus ragged tails), batch with quaternions."""
+    rng = np.random.default_rng(8)
+    nx, ny, nz, B = 150, 70, 13, 3
+    g = np.stack([W.random_grid(51 + i, nx, ny, nz, fill=0.5) for i in range(B)])
+    quat = W.random_quaternions(rng, B)
+    quat[1] = [1, 0, 0, 0]
+    voxel, lam = (2.0, 2.5, 3.0), 14.0
+    npx, npy, th = 23, 19, 35.0
+    I = sm.simulate_nufft(dev(g), voxel, lam, npx, npy, th, quat=quat, rho_mode=mode).cpu().numpy()
+    for b in range(B):
+        ref = O.simulate(g[b], voxel, lam, npx, npy, th, quat=quat[b], rho_mode=mode)
+        assert_parity(I[b], ref, what=f"nufft ragged b={b} mode={mode}")
+
+
+def test_off_axis_rectangular_detector_wide_angle(sm):
+    """Detector centre off the beam axis (the q range is not symmetric, the forward pixel is near a corner) at 70 degrees."""
+    g = W.random_grid(91, 40, 33, 29, fill=0.6)
+    voxel, lam = (1.0, 1.5, 1.25), 6.0
+    for (npx, npy, th, cx, cy) in [(31, 18, 70.0, 9.5, -7.0), (16, 40, 50.0, -30.0, 0.0), (1, 1, 20.0, 0.0, 0.0)]:
+        I = sm.simulate_nufft(dev(g), voxel, lam, npx, npy, th, cx=cx, cy=cy).cpu().numpy()
+        ref = O.simulate(g, voxel, lam, npx, npy, th, cx=cx, cy=cy)
+        assert_parity(I, ref, what=f"nufft off-axis {npx}x{npy}")
+
+
+def test_sparse_blobs(sm):
+    nx, ny, nz, B = 300, 200, 10, 2
+    g = np.stack([W.sparse_blobs_grid(71 + 10 * i, nx, ny, nz, nblobs=5 + 3 * i, max_extent=20 + 60 * i) for i in range(B)])
+    voxel, lam = (2.0, 2.0, 2.5), 11.0
+    npx, npy, th = 20, 17, 25.0
+    I = sm.simulate_nufft(dev(g), voxel, lam, npx, npy, th).cpu().numpy()
+    for b in range(B):
+        assert_parity(I[b], O.simulate(g[b], voxel, lam, npx, npy, th), what=f"nufft sparse blobs b={b}")
+
+
+def test_cfg2_ellipsoid_half_scale_oriented(sm):
+    w = W.config(1, scale=0.5)
+    g = w.grid(0)
+    I = sm.simulate_nufft(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat).cpu().numpy()
+    ref = O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat[0])
+    assert_parity(I, ref, what="nufft cfg2 half")
+
+
+def test_cfg3_droplet_quarter_scale(sm):
+    w = W.config(2, scale=0.25)
+    g = w.grid(0)
+    I = sm.simulate_nufft(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg).cpu().numpy()
+    assert_parity(I, O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg), what="nufft cfg3 quarter")
+
+
+def test_cfg5_coreshell_eighth_scale(sm):
+    w = W.config(4, scale=0.125)
+    g = w.grid(0)
+    I = sm.simulate_nufft(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg).cpu().numpy()
+    assert_parity(I, O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg), what="nufft cfg5 eighth")
+
+
+def test_empty_and_single_voxel(sm):
+    voxel, lam = (3.0, 3.0, 3.0), 12.0
+    z = np.zeros((8, 8, 8, 2), np.float32)
+    assert np.all(sm.simulate_nufft(dev(z), voxel, lam, 16, 16, 30.0).cpu().numpy() == 0)
+    one = z.copy()
+    one[2, 5, 1] = (0.03, 0.004)
+    I = sm.simulate_nufft(dev(one), voxel, lam, 16, 16, 30.0).cpu().numpy()
+    exact = abs((float(np.float32(0.03)) + 1j * float(np.float32(0.004))) * 27.0) ** 2
+    assert np.allclose(I, exact, rtol=1e-6)          # a corner voxel: |A| is flat only if the window correction is right
+
+
+def test_agrees_with_the_pixel_contraction_and_is_deterministic(sm):
+    import torch
+    w = W.config(1, scale=0.5)
+    d = dev(w.grid(0))
+    vox = (w.dx, w.dy, w.dz)
+    a = sm.simulate_nufft(d, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat).clone()
+    b = sm.simulate_nufft(d, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat).clone()
+    assert torch.equal(a, b)
+    c = sm.simulate(d, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat)
+    l2, pix = metrics(c.cpu().numpy(), a.cpu().numpy())
+    assert l2 <= 1e-4 and pix <= 1e-3
+
+
+def test_error_codes(sm):
+    import torch
+    from paper_2202_03411_b200 import binding as B
+    w = W.config(0)
+    d = dev(w.grid(0))
+    vox = (w.dx, w.dy, w.dz)
+    with pytest.raises(B.ScatmanError) as e:
+        sm.simulate_nufft(d, vox, w.lam, 64, 64, 30.0, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == B.WORKSPACE_TOO_SMALL
+    for bad in [dict(lam=-1.0), dict(theta=95.0), dict(quat=[[2.0, 0, 0, 0]]), dict(mode=7)]:
+        with pytest.raises(B.ScatmanError) as e:
+            sm.simulate_nufft(d, vox, bad.get("lam", w.lam), 64, 64, bad.get("theta", 30.0), quat=bad.get("quat"),
+                              rho_mode=bad.get("mode", 0))
+        assert e.value.status == B.INVALID_ARGUMENT
+
+
+# ------------------------------------------------------------------------------------------ full sizes, sampled pixels
+def _sampled_full(sm, idx, count, items=None):
+    w = W.config(idx)
+    vox = (w.dx, w.dy, w.dz)
+    items = [0] if items is None else items
+    g = w.grids(items)
+    quat = None if w.quat is None else w.quat[items]
+    I = sm.simulate_nufft(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat).cpu().numpy()
+    for i in range(len(items)):
+        flat = I[i].ravel()
+        c = w.npy // 2 * w.npx + w.npx // 2
+        pix = W.sample_pixels(w.seed + i, w.npix, count, always=[int(np.argmax(flat)), c, c - 1, c - w.npx, c - w.npx - 1,
+                                                                  0, w.npx - 1, w.npix - 1])
+        ref = O.simulate(g[i], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[i], pixels=pix)
+        assert_parity(flat[pix], ref, what=f"nufft {w.name} item {items[i]} sampled")
+
+
+def test_cfg2_full_size_sampled(sm):
+    _sampled_full(sm, 1, 512)
+
+
+def test_cfg3_full_size_sampled(sm):
+    _sampled_full(sm, 2, 192)
+
+
+def test_cfg4_full_size_items_sampled(sm):
+    _sampled_full(sm, 3, 128, items=[0, 1, 2, 3])
+
+
+def test_cfg5_full_size_sampled(sm):
+    _sampled_full(sm, 4, 48)
