@@ -437,10 +437,10 @@ def main():
                         "issued_fraction_of_dense": issued / (3.0 * dense_sep),
                         "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12}
     elif args.route == "nufft":
-        # three FP64 complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 12^3-point interpolation, CUDA cores:
+        # three FP64 complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 10^3-point interpolation, CUDA cores:
         # 8 flop per complex MAC of the GEMMs, 4 per (real weight x complex value) MAC of the interpolation.
         nqx, nqy, nqz = nq
-        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * w.npix * 12 ** 3)
+        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * w.npix * 10 ** 3)
         peak = 148 * 64 * 2 * 1.965e9 / 1e12           # FP64 FMA: 148 SMs x 64 lanes x 2 flop x max clock
         ach = flop / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "nufft_zgemm_kernel (stages Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,

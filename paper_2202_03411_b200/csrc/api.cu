@@ -644,9 +644,22 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
         const double h = 2.0 * pi / (2.0 * (double)N[d] * dd[d]);
         ax[d]->inv_h = 1.0 / h;
         const int m_lo = (int)floor(lo[d] / h - 0.5 * kNufftW) - 1;
-        const int m_hi = (int)ceil(hi[d] / h + 0.5 * kNufftW) + 1;
+        const int m_hi = (int)ceil(hi[d] / h + 0.5 * kNufftW) + 3;   // + 2: the interpolation's common window of W + 2 cells
         ax[d]->m_lo = m_lo;
         ax[d]->nq = m_hi - m_lo + 1;
+    }
+    // widest step between neighbouring pixels of a row, in grid cells: |dq/du| <= k on every axis (largest at the centre)
+    {
+        const double hmin = 2.0 * pi / (2.0 * fmax(fmax(g.nx * g.dx, g.ny * g.dy), g.nz * g.dz));
+        L.n.pixel_cells = k * pitch / hmin;
+    }
+    // batch items per chunk (one set of launches each): at most 2 GB of stage-Z planes
+    {
+        const double per_item = 16.0 * (double)L.n.az.nq * g.ny * g.nx;
+        int nb = (int)fmax(1.0, floor(2147483648.0 / per_item));
+        if (nb > batch) nb = batch;
+        if ((int64_t)nb * L.n.az.nq > 65535) nb = 65535 / L.n.az.nq > 0 ? 65535 / L.n.az.nq : 1;
+        L.n.nb = nb;
     }
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
@@ -659,9 +672,9 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
     L.off_tz = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz);
     L.off_tx = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx);
     L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
-    L.off_P = take(sizeof(double2) * (size_t)L.n.az.nq * g.ny * g.nx);
-    L.off_H = take(sizeof(double2) * (size_t)L.n.az.nq * g.ny * L.n.ax.nq);
-    L.off_U = take(sizeof(double2) * (size_t)L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
+    L.off_P = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx);
+    L.off_H = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq);
+    L.off_U = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
     L.total = off;
     return L;
 }
@@ -727,9 +740,11 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     nl += 3;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
     cudaEventRecord(ctx->ev0, st);
-    for (int b = 0; b < batch; ++b) {
-        e = launch_nufft_item((const float2 *)rho + (size_t)b * p.nvox, p, L.n, Tz, TxT, Ty, q, (double2 *)(ws + L.off_P),
-                              (double2 *)(ws + L.off_H), (double2 *)(ws + L.off_U), d_I + (size_t)b * p.npix, st);
+    for (int b0 = 0; b0 < batch; b0 += L.n.nb) {   // a chunk of items per set of launches
+        const int nb = batch - b0 < L.n.nb ? batch - b0 : L.n.nb;
+        e = launch_nufft_chunk((const float2 *)rho + (size_t)b0 * p.nvox, p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, Tz, TxT, Ty,
+                               q, (double2 *)(ws + L.off_P), (double2 *)(ws + L.off_H), (double2 *)(ws + L.off_U),
+                               d_I + (size_t)b0 * p.npix, st);
         nl += 4;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");
     }

@@ -99,13 +99,13 @@ cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, 
 int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
 
 // flat-detector route by a 3-D type-2 NUFFT (nufft_kernels.cu)
-constexpr int kNufftW = 12;                     // Kaiser-Bessel window width in grid cells (oversampling 2)
+constexpr int kNufftW = 10;                     // Kaiser-Bessel window width in grid cells (oversampling 2)
 struct NufftAxis { int m_lo = 0, nq = 0; double inv_h = 0; };   // uniform grid g_m = (m_lo + m) h, m = 0..nq-1; inv_h = 1 / h
-struct NufftPlan { NufftAxis ax, ay, az; };
+struct NufftPlan { NufftAxis ax, ay, az; int nb = 1; double pixel_cells = 0; };   // nb = batch items per chunk
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st);
-cudaError_t launch_nufft_item(const float2 *d_rho, const Plan &p, const NufftPlan &n, const double2 *d_Tz, const double2 *d_TxT,
-                              const double2 *d_Ty, const double *d_q, double2 *d_P, double2 *d_H, double2 *d_U, float *d_I,
-                              cudaStream_t st);
+cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
+                               const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
+                               double2 *d_H, double2 *d_U, float *d_I, cudaStream_t st);
 
 // forward-fitting pieces (fit_kernels.cu)
 size_t fit_workspace_bytes(int64_t npix, int batch);

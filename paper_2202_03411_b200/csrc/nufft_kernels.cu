@@ -4,16 +4,18 @@
 // contraction is replaced by
 //   (1) a SEPARABLE transform of rho~ onto a small uniform (g_z, g_y, g_x) grid that covers the q's of the detector with a margin,
 //       U[mz][my][mx] = sum_r c_z c_y c_x rho~(r) e^{i g_m . r}     -- three complex GEMMs (stage Z over slices, X over columns, Y over rows)
-//   (2) an interpolation from that grid to each pixel with a Kaiser-Bessel window of W = 12 grid cells per axis,
+//   (2) an interpolation from that grid to each pixel with a Kaiser-Bessel window of W = 10 grid cells per axis,
 //       A(p) = sum_{m near q(p)/h} phi(u_z - m_z) phi(u_y - m_y) phi(u_x - m_x) U[m],   u = q / h.
 // Grid spacing h_d = 2 pi / (2 N_d d_d) (oversampling 2), pre-correction c_i = 1 / Phi(h x_i) with Phi the window's Fourier transform:
 //   sum_m phi(u - m) e^{i m t} = sum_l Phi(t - 2 pi l) e^{i u (t - 2 pi l)}   (Poisson summation),   |t| = |h x_i| < pi / 2,
-// so the l = 0 term is the wanted e^{i u t} and the l = +-1 aliases are below 1e-10 of it for W = 12, beta = pi sqrt(W^2 (3/4)^2 - 0.8).
+// so the l = 0 term is the wanted e^{i u t} and the l = +-1 aliases are below 3e-9 of it for W = 10, beta = pi sqrt(W^2 (3/4)^2 - 0.8).
 // Everything is FP64 on the CUDA cores (the work is ~1000x smaller than the pixel contraction: 1.2e9 complex MACs for 256^3 on 512^2
 // pixels against 4.4e12), so the only approximation is the window's and the result meets the same tolerances against the oracle.
 #include "internal.h"
 
 namespace scatman {
+
+double nufft_inv_i0_beta();
 
 namespace {
 
@@ -45,15 +47,17 @@ __global__ void nufft_table_kernel(int N, int nq, int m_lo, int transposed, doub
 
 // ---- complex FP64 GEMM: C[b] (M x N) = A[b] (M x K, K contiguous) * B[b] (K x N, N contiguous); 64 x 64 tiles, K steps of 16,
 // 256 threads x (4 x 4) outputs at rows ty + 16 i, columns tx + 16 j (conflict-free 16-byte shared-memory reads).
-constexpr int BM = 64, BN = 64, BK = 16;
+constexpr int BN = 64, BK = 16;
 
 __device__ inline double2 ld_c(const double2 *p) { return __ldg(p); }
 __device__ inline double2 ld_c(const float2 *p) { const float2 v = __ldg(p); return make_double2((double)v.x, (double)v.y); }
 
-template <typename TA, typename TB>
-__global__ void __launch_bounds__(256)
+// RM = rows per thread: the row tile is BM = 16 RM (32, 48 or 64), picked per GEMM so that M pads least (stage Z has M = nqz ~ 40-150).
+template <typename TA, typename TB, int RM>
+__global__ void __launch_bounds__(256, RM <= 3 ? 2 : 1)
 nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *__restrict__ C, int M, int N, int K,
                    int64_t lda, int64_t ldb, int64_t ldc, int64_t strideA, int64_t strideB, int64_t strideC) {
+    constexpr int BM = 16 * RM;
     __shared__ double2 As[BK][BM + 1];
     __shared__ double2 Bs[BK][BN];
     const int t = threadIdx.x, tx = t & 15, ty = t >> 4;
@@ -61,18 +65,22 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
     A += (int64_t)blockIdx.z * strideA;
     B += (int64_t)blockIdx.z * strideB;
     C += (int64_t)blockIdx.z * strideC;
-    double2 acc[4][4];
+    double2 acc[RM][4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < RM; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
-    double2 ra[4], rb[4];
+    double2 ra[RM], rb[4];
     auto fetch = [&](int k0) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < RM; ++r) {
             const int idx = t + 256 * r;
             const int ak = idx & 15, am = idx >> 4;
             ra[r] = (m0 + am < M && k0 + ak < K) ? ld_c(A + (int64_t)(m0 + am) * lda + (k0 + ak)) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int idx = t + 256 * r;
             const int bn = idx & 63, bk = idx >> 6;
             rb[r] = (n0 + bn < N && k0 + bk < K) ? ld_c(B + (int64_t)(k0 + bk) * ldb + (n0 + bn)) : make_double2(0.0, 0.0);
         }
@@ -80,22 +88,26 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
     fetch(0);
     for (int k0 = 0; k0 < K; k0 += BK) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < RM; ++r) {
             const int idx = t + 256 * r;
             As[idx & 15][idx >> 4] = ra[r];
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int idx = t + 256 * r;
             Bs[idx >> 6][idx & 63] = rb[r];
         }
         __syncthreads();
         if (k0 + BK < K) fetch(k0 + BK);
 #pragma unroll
         for (int k = 0; k < BK; ++k) {
-            double2 a[4], b[4];
+            double2 a[RM], b[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = As[k][ty + 16 * i];
+            for (int i = 0; i < RM; ++i) a[i] = As[k][ty + 16 * i];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < RM; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     acc[i][j].x = fma(a[i].x, b[j].x, acc[i][j].x);
@@ -107,7 +119,7 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
         __syncthreads();
     }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < RM; ++i) {
         const int m = m0 + ty + 16 * i;
         if (m >= M) continue;
 #pragma unroll
@@ -118,65 +130,180 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
     }
 }
 
-template <typename TA, typename TB>
-cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
-                  int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
-    // grid.y carries the row tiles (<= 65535: M <= 4 M rows), grid.z the batch
-    for (int m_base = 0; m_base < M; m_base += 65535 * BM) {
-        const int rows = M - m_base < 65535 * BM ? M - m_base : 65535 * BM;
+template <typename TA, typename TB, int RM>
+cudaError_t zgemm_rm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
+                     int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
+    constexpr int BM = 16 * RM;
+    // grid.y carries the row tiles (<= 65535), grid.z the batch (<= 65535, the callers' concern)
+    for (int64_t m_base = 0; m_base < M; m_base += 65535LL * BM) {
+        const int rows = (int)(M - m_base < 65535LL * BM ? M - m_base : 65535LL * BM);
         dim3 grid((N + BN - 1) / BN, (rows + BM - 1) / BM, nbatch);
-        nufft_zgemm_kernel<TA, TB><<<grid, 256, 0, st>>>(A + (int64_t)m_base * lda, B, C + (int64_t)m_base * ldc, rows, N, K, lda, ldb,
-                                                         ldc, sA, sB, sC);
+        nufft_zgemm_kernel<TA, TB, RM><<<grid, 256, 0, st>>>(A + m_base * lda, B, C + m_base * ldc, rows, N, K, lda, ldb, ldc, sA, sB,
+                                                             sC);
     }
     return cudaGetLastError();
 }
 
-// ---- interpolation: one thread per pixel; A = sum over the W^3 nearest grid points, I = |A dV|^2 (Block 11).
+template <typename TA, typename TB>
+cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
+                  int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
+    auto padded = [&](int bm) { return (int64_t)((M + bm - 1) / bm) * bm; };
+    if (padded(64) <= padded(48) && padded(64) <= padded(32))
+        return zgemm_rm<TA, TB, 4>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (padded(48) <= padded(32)) return zgemm_rm<TA, TB, 3>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    return zgemm_rm<TA, TB, 2>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+}
+
+// ---- interpolation: A = sum over the W^3 nearest grid points, I = |A dV|^2 (Block 11).
+// A thread owns P consecutive pixels of a detector row: their windows overlap (a pixel is a fraction of a grid cell wide), so the
+// thread walks ONE common window of KU = W + 2 cells per axis, loads every grid value once and applies it to all P pixels with
+// per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the bytes it pulls through L1, and this divides
+// them by ~P.  A group whose windows do not fit the common one (pixels more than a cell apart: coarse detectors) takes its pixels
+// one by one.  Window weights of the y and z axes live in shared memory ([axis][pixel][cell][thread]).
 __device__ inline double kb_phi(double s, double beta, double inv_i0b) {
     const double a = 1.0 - (s / kHalfW) * (s / kHalfW);
     return a > 0.0 ? cyl_bessel_i0(beta * sqrt(a)) * inv_i0b : (a == 0.0 ? inv_i0b : 0.0);
 }
 
-__global__ void __launch_bounds__(128)
-nufft_interp_kernel(const double *__restrict__ q, int64_t npix, NufftAxis ax, NufftAxis ay, NufftAxis az,
-                    const double2 *__restrict__ U, double inv_i0b, double dV, float *__restrict__ I) {
-    __shared__ double wyz[2 * kW][128];
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= npix) return;
+constexpr int kInterpThreads = 64;
+
+template <int P>
+__global__ void __launch_bounds__(kInterpThreads)
+nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
+                    const double2 *__restrict__ U, int64_t strideU, double inv_i0b, double dV, float *__restrict__ I) {
+    constexpr int KU = P > 1 ? kW + 2 : kW;
+    extern __shared__ double wsm[];                       // [2][P][KU][kInterpThreads]
+    const int ngx = (npx + P - 1) / P;
+    const int64_t g = (int64_t)blockIdx.x * kInterpThreads + threadIdx.x;
+    if (g >= (int64_t)ngx * npy) return;
+    const int iy = (int)(g / ngx), ix0 = (int)(g % ngx) * P;
+    const int64_t p0 = (int64_t)iy * npx + ix0;
+    const int64_t npix = (int64_t)npx * npy;
+    U += (int64_t)blockIdx.y * strideU;
+    I += (int64_t)blockIdx.y * npix;
     const double beta = kb_beta();
-    const double ux = q[3 * p + 0] * ax.inv_h, uy = q[3 * p + 1] * ay.inv_h, uz = q[3 * p + 2] * az.inv_h;
-    const int mx0 = (int)ceil(ux - kHalfW), my0 = (int)ceil(uy - kHalfW), mz0 = (int)ceil(uz - kHalfW);
-    double wx[kW];
+    const int np = npx - ix0 < P ? npx - ix0 : P;
+    double u[P][3];
+    int m0[P][3], base[3], top[3];
 #pragma unroll
-    for (int i = 0; i < kW; ++i) {
-        wx[i] = kb_phi(ux - (double)(mx0 + i), beta, inv_i0b);
-        wyz[i][threadIdx.x] = kb_phi(uy - (double)(my0 + i), beta, inv_i0b);
-        wyz[kW + i][threadIdx.x] = kb_phi(uz - (double)(mz0 + i), beta, inv_i0b);
-    }
-    const int ix = mx0 - ax.m_lo, iy = my0 - ay.m_lo, iz = mz0 - az.m_lo;   // >= 0 and + kW <= nq by the margins of the plan
-    double are = 0.0, aim = 0.0;
-    for (int c = 0; c < kW; ++c) {
-        const double wz = wyz[kW + c][threadIdx.x];
-        double pre = 0.0, pim = 0.0;
-        for (int b = 0; b < kW; ++b) {
-            const double2 *row = U + ((int64_t)(iz + c) * ay.nq + (iy + b)) * ax.nq + ix;
-            double rre = 0.0, rim = 0.0;
+    for (int j = 0; j < P; ++j) {
+        const int64_t p = p0 + (j < np ? j : 0);
+        u[j][0] = q[3 * p + 0] * ax.inv_h; u[j][1] = q[3 * p + 1] * ay.inv_h; u[j][2] = q[3 * p + 2] * az.inv_h;
 #pragma unroll
-            for (int a = 0; a < kW; ++a) {
-                const double2 v = __ldg(row + a);
-                rre = fma(wx[a], v.x, rre);
-                rim = fma(wx[a], v.y, rim);
-            }
-            const double wy = wyz[b][threadIdx.x];
-            pre = fma(wy, rre, pre);
-            pim = fma(wy, rim, pim);
+        for (int d = 0; d < 3; ++d) {
+            m0[j][d] = (int)ceil(u[j][d] - kHalfW);
+            base[d] = j == 0 ? m0[j][d] : min(base[d], m0[j][d]);
+            top[d] = j == 0 ? m0[j][d] : max(top[d], m0[j][d]);
         }
-        are = fma(wz, pre, are);
-        aim = fma(wz, pim, aim);
     }
-    are *= dV;
-    aim *= dV;
-    I[p] = (float)(are * are + aim * aim);
+    const bool common = top[0] - base[0] + kW <= KU && top[1] - base[1] + kW <= KU && top[2] - base[2] + kW <= KU;
+    auto wy = [&](int j, int b) -> double & { return wsm[((0 * P + j) * KU + b) * kInterpThreads + threadIdx.x]; };
+    auto wz = [&](int j, int c) -> double & { return wsm[((1 * P + j) * KU + c) * kInterpThreads + threadIdx.x]; };
+    if (common) {
+        double wx[P][KU];
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+#pragma unroll
+            for (int a = 0; a < KU; ++a) {
+                wx[j][a] = kb_phi(u[j][0] - (double)(base[0] + a), beta, inv_i0b);
+                wy(j, a) = kb_phi(u[j][1] - (double)(base[1] + a), beta, inv_i0b);
+                wz(j, a) = kb_phi(u[j][2] - (double)(base[2] + a), beta, inv_i0b);
+            }
+        const int ix = base[0] - ax.m_lo, iyq = base[1] - ay.m_lo, iz = base[2] - az.m_lo;   // inside the grid by the plan's margins
+        double are[P], aim[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) are[j] = aim[j] = 0.0;
+        for (int c = 0; c < KU; ++c) {
+            double wzc[P];
+            bool any = false;
+#pragma unroll
+            for (int j = 0; j < P; ++j) { wzc[j] = wz(j, c); any |= wzc[j] != 0.0; }
+            if (!any) continue;
+            double pre[P], pim[P];
+#pragma unroll
+            for (int j = 0; j < P; ++j) pre[j] = pim[j] = 0.0;
+            for (int b = 0; b < KU; ++b) {
+                double wyb[P];
+                bool anyb = false;
+#pragma unroll
+                for (int j = 0; j < P; ++j) { wyb[j] = wy(j, b); anyb |= wyb[j] != 0.0; }
+                if (!anyb) continue;
+                const double2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
+                double2 v[KU];
+#pragma unroll
+                for (int a = 0; a < KU; ++a) v[a] = __ldg(row + a);
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    double rre = 0.0, rim = 0.0;
+#pragma unroll
+                    for (int a = 0; a < KU; ++a) {
+                        rre = fma(wx[j][a], v[a].x, rre);
+                        rim = fma(wx[j][a], v[a].y, rim);
+                    }
+                    pre[j] = fma(wyb[j], rre, pre[j]);
+                    pim[j] = fma(wyb[j], rim, pim[j]);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                are[j] = fma(wzc[j], pre[j], are[j]);
+                aim[j] = fma(wzc[j], pim[j], aim[j]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+            if (j < np) {
+                const double re = are[j] * dV, im = aim[j] * dV;
+                I[p0 + j] = (float)(re * re + im * im);
+            }
+        return;
+    }
+    // pixels one by one, each with its own W-cell window
+    for (int j = 0; j < np; ++j) {
+        double wx1[kW];
+#pragma unroll
+        for (int a = 0; a < kW; ++a) {
+            wx1[a] = kb_phi(u[j][0] - (double)(m0[j][0] + a), beta, inv_i0b);
+            wy(0, a) = kb_phi(u[j][1] - (double)(m0[j][1] + a), beta, inv_i0b);
+            wz(0, a) = kb_phi(u[j][2] - (double)(m0[j][2] + a), beta, inv_i0b);
+        }
+        const int ix = m0[j][0] - ax.m_lo, iyq = m0[j][1] - ay.m_lo, iz = m0[j][2] - az.m_lo;
+        double are = 0.0, aim = 0.0;
+        for (int c = 0; c < kW; ++c) {
+            double pre = 0.0, pim = 0.0;
+            for (int b = 0; b < kW; ++b) {
+                const double2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
+                double rre = 0.0, rim = 0.0;
+#pragma unroll
+                for (int a = 0; a < kW; ++a) {
+                    const double2 v = __ldg(row + a);
+                    rre = fma(wx1[a], v.x, rre);
+                    rim = fma(wx1[a], v.y, rim);
+                }
+                pre = fma(wy(0, b), rre, pre);
+                pim = fma(wy(0, b), rim, pim);
+            }
+            are = fma(wz(0, c), pre, are);
+            aim = fma(wz(0, c), pim, aim);
+        }
+        are *= dV;
+        aim *= dV;
+        I[p0 + j] = (float)(are * are + aim * aim);
+    }
+}
+
+template <int P>
+cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &n, const double2 *d_U, int64_t strideU, int nb,
+                          double dV, float *d_I, cudaStream_t st) {
+    constexpr int KU = P > 1 ? kW + 2 : kW;
+    const size_t smem = sizeof(double) * 2 * P * KU * kInterpThreads;
+    cudaError_t e = cudaFuncSetAttribute(nufft_interp_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t groups = (int64_t)((npx + P - 1) / P) * npy;
+    dim3 grid((unsigned)((groups + kInterpThreads - 1) / kInterpThreads), nb);
+    nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, nufft_inv_i0_beta(), dV,
+                                                                 d_I);
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -204,28 +331,34 @@ cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz
     return cudaGetLastError();
 }
 
-// One batch item: rho~ [nz][ny][nx] -> P [nqz][ny][nx] -> H [nqz][ny][nqx] -> U [nqz][nqy][nqx] -> I [npix].
-cudaError_t launch_nufft_item(const float2 *d_rho, const Plan &p, const NufftPlan &n, const double2 *d_Tz, const double2 *d_TxT,
-                              const double2 *d_Ty, const double *d_q, double2 *d_P, double2 *d_H, double2 *d_U, float *d_I,
-                              cudaStream_t st) {
+// A chunk of nb batch items: rho~ [nb][nz][ny][nx] -> P [nb][nqz][ny][nx] -> H [nb][nqz][ny][nqx] -> U [nb][nqz][nqy][nqx] -> I [nb][npix].
+// pixel_cells = the widest step between neighbouring pixels of a row, in grid cells of any axis (picks the pixels per thread).
+cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
+                               const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
+                               double2 *d_H, double2 *d_U, float *d_I, cudaStream_t st) {
     const int64_t nyx = (int64_t)p.ny * p.nx;
     cudaError_t e = cudaSuccess;
-    // stage Z: P (nqz x ny nx) = Tz (nqz x nz) * rho~ (nz x ny nx); the column dimension is cut so that grid.x stays in range
-    e = zgemm<double2, float2>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, 1, 0, 0, 0, st);
+    // stage Z, one GEMM per item: P_b (nqz x ny nx) = Tz (nqz x nz) * rho~_b (nz x ny nx)
+    e = zgemm<double2, float2>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, nb, 0, (int64_t)p.nz * nyx,
+                               (int64_t)n.az.nq * nyx, st);
     if (e != cudaSuccess) return e;
-    // stage X: H ((nqz ny) x nqx) = P ((nqz ny) x nx) * TxT (nx x nqx)
-    e = zgemm<double2, double2>(d_P, d_TxT, d_H, n.az.nq * p.ny, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
+    // stage X, all items and planes at once: H ((nb nqz ny) x nqx) = P ((nb nqz ny) x nx) * TxT (nx x nqx)
+    const int64_t rows = (int64_t)nb * n.az.nq * p.ny;     // < 2^31: the chunk holds at most 2 GB of P
+    e = zgemm<double2, double2>(d_P, d_TxT, d_H, (int)rows, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
     if (e != cudaSuccess) return e;
-    // stage Y, one GEMM per g_z plane: U_m (nqy x nqx) = Ty (nqy x ny) * H_m (ny x nqx)
-    for (int z0 = 0; z0 < n.az.nq; z0 += 65535) {
-        const int nzb = n.az.nq - z0 < 65535 ? n.az.nq - z0 : 65535;
+    // stage Y, one GEMM per (item, g_z plane): U_m (nqy x nqx) = Ty (nqy x ny) * H_m (ny x nqx)
+    const int planes = nb * n.az.nq;
+    for (int z0 = 0; z0 < planes; z0 += 65535) {
+        const int nzb = planes - z0 < 65535 ? planes - z0 : 65535;
         e = zgemm<double2, double2>(d_Ty, d_H + (int64_t)z0 * p.ny * n.ax.nq, d_U + (int64_t)z0 * n.ay.nq * n.ax.nq, n.ay.nq, n.ax.nq,
                                     p.ny, p.ny, n.ax.nq, n.ax.nq, nzb, 0, (int64_t)p.ny * n.ax.nq, (int64_t)n.ay.nq * n.ax.nq, st);
         if (e != cudaSuccess) return e;
     }
-    nufft_interp_kernel<<<(unsigned)((p.npix + 127) / 128), 128, 0, st>>>(d_q, p.npix, n.ax, n.ay, n.az, d_U, nufft_inv_i0_beta(),
-                                                                         p.dx * p.dy * p.dz, d_I);
-    return cudaGetLastError();
+    const int64_t strideU = (int64_t)n.az.nq * n.ay.nq * n.ax.nq;
+    const double dV = p.dx * p.dy * p.dz;
+    if (3.0 * pixel_cells <= 1.0) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    if (pixel_cells <= 1.0) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    return launch_interp<1>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
 }
 
 }  // namespace scatman
