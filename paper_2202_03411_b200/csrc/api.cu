@@ -197,7 +197,8 @@ int scatman_create(scatman_ctx **out, int device) {
     scatman_ctx *ctx = new scatman_ctx();
     ctx->device = device;
     ctx->num_sms = prop.multiProcessorCount;
-    if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) {
+    if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess ||
+        nufft_init_device() != cudaSuccess) {   // the NUFFT route's window polynomials -> constant memory of this device
         delete ctx;
         return SCATMAN_CUDA_ERROR;
     }

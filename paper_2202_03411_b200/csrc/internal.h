@@ -102,6 +102,7 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
 constexpr int kNufftW = 10;                     // Kaiser-Bessel window width in grid cells (oversampling 2)
 struct NufftAxis { int m_lo = 0, nq = 0; double inv_h = 0; };   // uniform grid g_m = (m_lo + m) h, m = 0..nq-1; inv_h = 1 / h
 struct NufftPlan { NufftAxis ax, ay, az; int nb = 1; double pixel_cells = 0; };   // nb = batch items per chunk
+cudaError_t nufft_init_device();   // once per device (scatman_create): uploads the window's piecewise polynomials
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st);
 cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,

@@ -160,9 +160,31 @@ cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int
 // per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the bytes it pulls through L1, and this divides
 // them by ~P.  A group whose windows do not fit the common one (pixels more than a cell apart: coarse detectors) takes its pixels
 // one by one.  Window weights of the y and z axes live in shared memory ([axis][pixel][cell][thread]).
-__device__ inline double kb_phi(double s, double beta, double inv_i0b) {
-    const double a = 1.0 - (s / kHalfW) * (s / kHalfW);
-    return a > 0.0 ? cyl_bessel_i0(beta * sqrt(a)) * inv_i0b : (a == 0.0 ? inv_i0b : 0.0);
+// The window phi(s) = I0(beta sqrt(1 - (s / (W/2))^2)) / I0(beta) is entire in s^2, so on each of its W unit cells it is a polynomial
+// to 2e-13 at degree 11 (Chebyshev fit on the host, nufft_init_device): the W weights of a point come from W Horner evaluations at
+// the one offset t = m0 - (u - W/2) in [0, 1), weight of cell m0 + c = phi(W/2 - c - t) = sum_k c_kb[c][k] (2 t - 1)^k.
+constexpr int kDeg = 11;
+__constant__ double c_kb[kW][kDeg + 1];
+
+__device__ inline void kb_weights(double u, int m0, double (&w)[kW]) {
+    const double x = 2.0 * ((double)m0 - (u - kHalfW)) - 1.0;
+#pragma unroll
+    for (int c = 0; c < kW; ++c) {
+        double v = c_kb[c][kDeg];
+#pragma unroll
+        for (int k = kDeg - 1; k >= 0; --k) v = fma(v, x, c_kb[c][k]);
+        w[c] = v;
+    }
+}
+
+// own[0..W) placed at cells shift..shift+W of a KU-cell window, zero elsewhere (static indices: selects, no local memory)
+template <int KU>
+__device__ inline double placed(const double (&own)[kW], int shift, int a) {
+    double v = 0.0;
+#pragma unroll
+    for (int s = 0; s <= KU - kW; ++s)
+        if (shift == s && a - s >= 0 && a - s < kW) v = own[a - s < 0 ? 0 : (a - s >= kW ? kW - 1 : a - s)];
+    return v;
 }
 
 constexpr int kInterpThreads = 64;
@@ -170,7 +192,7 @@ constexpr int kInterpThreads = 64;
 template <int P>
 __global__ void __launch_bounds__(kInterpThreads)
 nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
-                    const double2 *__restrict__ U, int64_t strideU, double inv_i0b, double dV, float *__restrict__ I) {
+                    const double2 *__restrict__ U, int64_t strideU, double dV, float *__restrict__ I) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     extern __shared__ double wsm[];                       // [2][P][KU][kInterpThreads]
     const int ngx = (npx + P - 1) / P;
@@ -181,7 +203,6 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     const int64_t npix = (int64_t)npx * npy;
     U += (int64_t)blockIdx.y * strideU;
     I += (int64_t)blockIdx.y * npix;
-    const double beta = kb_beta();
     const int np = npx - ix0 < P ? npx - ix0 : P;
     double u[P][3];
     int m0[P][3], base[3], top[3];
@@ -202,13 +223,18 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     if (common) {
         double wx[P][KU];
 #pragma unroll
-        for (int j = 0; j < P; ++j)
+        for (int j = 0; j < P; ++j) {
+            double own[kW];
+            kb_weights(u[j][0], m0[j][0], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) {
-                wx[j][a] = kb_phi(u[j][0] - (double)(base[0] + a), beta, inv_i0b);
-                wy(j, a) = kb_phi(u[j][1] - (double)(base[1] + a), beta, inv_i0b);
-                wz(j, a) = kb_phi(u[j][2] - (double)(base[2] + a), beta, inv_i0b);
-            }
+            for (int a = 0; a < KU; ++a) wx[j][a] = placed<KU>(own, m0[j][0] - base[0], a);
+            kb_weights(u[j][1], m0[j][1], own);
+#pragma unroll
+            for (int a = 0; a < KU; ++a) wy(j, a) = placed<KU>(own, m0[j][1] - base[1], a);
+            kb_weights(u[j][2], m0[j][2], own);
+#pragma unroll
+            for (int a = 0; a < KU; ++a) wz(j, a) = placed<KU>(own, m0[j][2] - base[2], a);
+        }
         const int ix = base[0] - ax.m_lo, iyq = base[1] - ay.m_lo, iz = base[2] - az.m_lo;   // inside the grid by the plan's margins
         double are[P], aim[P];
 #pragma unroll
@@ -260,13 +286,14 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     }
     // pixels one by one, each with its own W-cell window
     for (int j = 0; j < np; ++j) {
-        double wx1[kW];
+        double wx1[kW], own[kW];
+        kb_weights(u[j][0], m0[j][0], wx1);
+        kb_weights(u[j][1], m0[j][1], own);
 #pragma unroll
-        for (int a = 0; a < kW; ++a) {
-            wx1[a] = kb_phi(u[j][0] - (double)(m0[j][0] + a), beta, inv_i0b);
-            wy(0, a) = kb_phi(u[j][1] - (double)(m0[j][1] + a), beta, inv_i0b);
-            wz(0, a) = kb_phi(u[j][2] - (double)(m0[j][2] + a), beta, inv_i0b);
-        }
+        for (int a = 0; a < kW; ++a) wy(0, a) = own[a];
+        kb_weights(u[j][2], m0[j][2], own);
+#pragma unroll
+        for (int a = 0; a < kW; ++a) wz(0, a) = own[a];
         const int ix = m0[j][0] - ax.m_lo, iyq = m0[j][1] - ay.m_lo, iz = m0[j][2] - az.m_lo;
         double are = 0.0, aim = 0.0;
         for (int c = 0; c < kW; ++c) {
@@ -301,8 +328,7 @@ cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &
     if (e != cudaSuccess) return e;
     const int64_t groups = (int64_t)((npx + P - 1) / P) * npy;
     dim3 grid((unsigned)((groups + kInterpThreads - 1) / kInterpThreads), nb);
-    nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, nufft_inv_i0_beta(), dV,
-                                                                 d_I);
+    nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_I);
     return cudaGetLastError();
 }
 
@@ -318,6 +344,50 @@ double nufft_inv_i0_beta() {
         if (term < 1e-18 * sum) break;
     }
     return 1.0 / sum;
+}
+
+// Chebyshev fit of the window on each unit cell (degree kDeg, nodes cos(pi (k + 1/2) / n)), rewritten in powers of x = 2 t - 1.
+cudaError_t nufft_init_device() {
+    static double coef[kW][kDeg + 1];
+    static bool fitted = false;
+    if (!fitted) {
+        const double beta = kb_beta(), inv_i0b = nufft_inv_i0_beta();
+        auto i0 = [](double x) {
+            double term = 1.0, sum = 1.0;
+            for (int k = 1; k < 300; ++k) {
+                term *= (x * 0.5 / k) * (x * 0.5 / k);
+                sum += term;
+                if (term < 1e-18 * sum) break;
+            }
+            return sum;
+        };
+        constexpr int n = kDeg + 1;
+        for (int c = 0; c < kW; ++c) {
+            double f[n], cheb[n];
+            for (int k = 0; k < n; ++k) {
+                const double x = cos(kPi * (k + 0.5) / n);
+                const double s = kHalfW - c - 0.5 * (x + 1.0);
+                const double a = 1.0 - (s / kHalfW) * (s / kHalfW);
+                f[k] = i0(beta * sqrt(a > 0.0 ? a : 0.0)) * inv_i0b;
+            }
+            for (int j = 0; j < n; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < n; ++k) acc += f[k] * cos(j * kPi * (k + 0.5) / n);
+                cheb[j] = (j == 0 ? 1.0 : 2.0) / n * acc;
+            }
+            // sum_j cheb[j] T_j(x) in the monomial basis: T_0 = 1, T_1 = x, T_{j+1} = 2 x T_j - T_{j-1}
+            double t0[n] = {1.0}, t1[n] = {0.0, 1.0}, mono[n] = {0.0};
+            for (int k = 0; k < n; ++k) mono[k] = cheb[0] * t0[k] + (n > 1 ? cheb[1] * t1[k] : 0.0);
+            for (int j = 2; j < n; ++j) {
+                double t2[n];
+                for (int k = 0; k < n; ++k) t2[k] = (k > 0 ? 2.0 * t1[k - 1] : 0.0) - t0[k];
+                for (int k = 0; k < n; ++k) { mono[k] += cheb[j] * t2[k]; t0[k] = t1[k]; t1[k] = t2[k]; }
+            }
+            for (int k = 0; k < n; ++k) coef[c][k] = mono[k];
+        }
+        fitted = true;
+    }
+    return cudaMemcpyToSymbol(c_kb, coef, sizeof(coef));
 }
 
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st) {
