@@ -87,18 +87,24 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
     };
     fetch(0);
     for (int k0 = 0; k0 < K; k0 += BK) {
+        // A K step whose A tile or B tile is all zero (vacuum: rho~, and the planes and rows made from it, are exact zeros
+        // outside the particle) adds nothing: the block agrees on that with two barrier reductions and skips the arithmetic.
+        bool nza = false, nzb = false;
 #pragma unroll
         for (int r = 0; r < RM; ++r) {
             const int idx = t + 256 * r;
             As[idx & 15][idx >> 4] = ra[r];
+            nza |= ra[r].x != 0.0 || ra[r].y != 0.0;
         }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int idx = t + 256 * r;
             Bs[idx >> 6][idx & 63] = rb[r];
+            nzb |= rb[r].x != 0.0 || rb[r].y != 0.0;
         }
-        __syncthreads();
+        const bool live = __syncthreads_or(nzb) != 0 && __syncthreads_or(nza) != 0;   // the first one orders the stores above
         if (k0 + BK < K) fetch(k0 + BK);
+        if (!live) continue;
 #pragma unroll
         for (int k = 0; k < BK; ++k) {
             double2 a[RM], b[4];
