@@ -25,6 +25,8 @@ FLOP_PER_TERM = 8    # one complex MAC
 # dram__bytes_read.sum + dram__bytes_write.sum of one contraction launch, from the committed `ncu --set full` capture
 # (profiles/r01_contract_cfg3_full.md); only the workload that was captured has a number
 NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": 2.295495e9 + 8.534016e6}
+# the same for the four launches of one NUFFT pattern (stages Z, X, Y, interpolation; profiles/r01_nufft.md)
+NCU_DRAM_BYTES_NUFFT = {"cfg3_droplet_256": (134.436 + 22.964 + 46.631 + 0.980 + 20.852 + 0.0 + 9.708 + 0.0) * 1e6}
 
 
 def load_peaks():
@@ -444,8 +446,10 @@ def main():
         peak = 148 * 64 * 2 * 1.965e9 / 1e12           # FP64 FMA: 148 SMs x 64 lanes x 2 flop x max clock
         ach = flop / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "nufft_zgemm_kernel (stages Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,
-                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms, "uniform_grid": [nqz, nqy, nqx],
-                    "achieved_is": "FP64 flop of the three GEMM stages and the interpolation / their CUDA-event time",
+                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": NCU_DRAM_BYTES_NUFFT.get(w.name) if batch == 1 else None,
+                    "kernel_ms": k_ms, "uniform_grid": [nqz, nqy, nqx],
+                    "achieved_is": "dense FP64 flop of the three GEMM stages and the interpolation / their CUDA-event time; K steps over "
+                                   "vacuum are skipped, so the ALUs executed less than this (ncu: FP64 pipe 50-59 % active in the GEMMs)",
                     "flop_vs_pixel_route": flop / (FLOP_PER_TERM * terms_per_pattern * batch)}
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.

@@ -153,10 +153,17 @@ cudaError_t zgemm_rm(const TA *A, const TB *B, double2 *C, int M, int N, int K, 
 template <typename TA, typename TB>
 cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
                   int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
-    auto padded = [&](int bm) { return (int64_t)((M + bm - 1) / bm) * bm; };
-    if (padded(64) <= padded(48) && padded(64) <= padded(32))
-        return zgemm_rm<TA, TB, 4>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
-    if (padded(48) <= padded(32)) return zgemm_rm<TA, TB, 3>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    // Row tile by a makespan estimate: resident sets of 148 x (2 CTAs of RM <= 3, or 1 of RM = 4) run one after the other and a
+    // set takes ~ CTAs per SM x RM; ties go to the least padding, then to the taller tile.
+    auto cost = [&](int rm) {
+        const int64_t tiles = (int64_t)((M + 16 * rm - 1) / (16 * rm)) * ((N + BN - 1) / BN) * nbatch;
+        const int cps = rm <= 3 ? 2 : 1;
+        const int64_t sets = (tiles + 148 * cps - 1) / (148 * cps);
+        return sets * cps * rm * 1000000 + (int64_t)((M + 16 * rm - 1) / (16 * rm)) * 16 * rm % 1000000 * 10 + (4 - rm);
+    };
+    const int64_t c2 = cost(2), c3 = cost(3), c4 = cost(4);
+    if (c4 <= c3 && c4 <= c2) return zgemm_rm<TA, TB, 4>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (c3 <= c2) return zgemm_rm<TA, TB, 3>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
     return zgemm_rm<TA, TB, 2>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
 }
 
