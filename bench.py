@@ -239,7 +239,7 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit", "nufft"],
+    ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit", "nufft", "shapes_nufft"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
                          "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
@@ -300,7 +300,7 @@ def main():
         ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
 
     nq = None
-    if args.route == "nufft":      # same flat detector, same result: 3-D type-2 NUFFT instead of the pixel x voxel contraction
+    if args.route in ("nufft", "shapes_nufft"):      # same flat detector, same result: 3-D type-2 NUFFT instead of the pixel x voxel contraction
         det = B.Detector(w.npx, w.npy, w.theta_max_deg, 0.0, 0.0)
         need = C.c_size_t(0)
         sm._check(sm.lib.scatman_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)))
@@ -314,6 +314,13 @@ def main():
             raise SystemExit(f"{w.name} is not one shape per item: --route shapes_qgrid does not apply")
         need = C.c_size_t(0)
         sm._check(sm.lib.scatman_shapes_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
+        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+    if args.route == "shapes_nufft":
+        shapes = w.shapes(items)
+        if shapes is None:
+            raise SystemExit(f"{w.name} is not one shape per item: --route shapes_nufft does not apply")
+        need = C.c_size_t(0)
+        sm._check(sm.lib.scatman_shapes_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)))
         ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
     if args.route == "shapes":
         shapes = w.shapes(items)
@@ -334,6 +341,10 @@ def main():
             return
         if args.route == "qgrid":
             sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=stream)
+            return
+        if args.route == "shapes_nufft":
+            sm.simulate_shapes_nufft(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, workspace=ws, out=out,
+                                     stream=stream)
             return
         if args.route == "nufft":
             sm.simulate_nufft(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, workspace=ws, out=out, stream=stream)
@@ -376,7 +387,7 @@ def main():
     e2e_steps = max(1, min(args.steps, 3))
 
     def e2e_step():
-        if args.route in ("shapes", "shapes_qgrid"):  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
+        if args.route in ("shapes", "shapes_qgrid", "shapes_nufft"):  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
             step()
             h_I.copy_(out, non_blocking=True)
             torch.cuda.synchronize()
@@ -438,7 +449,7 @@ def main():
                                        "CUDA-event time of the per-item launches (pack, stage X, stage YZ, finalize)",
                         "issued_fraction_of_dense": issued / (3.0 * dense_sep),
                         "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12}
-    elif args.route == "nufft":
+    elif args.route in ("nufft", "shapes_nufft"):
         # three FP64 complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 10^3-point interpolation, CUDA cores:
         # 8 flop per complex MAC of the GEMMs, 4 per (real weight x complex value) MAC of the interpolation.
         nqx, nqy, nqz = nq
@@ -494,7 +505,7 @@ def main():
         from paper_2202_03411_b200 import workloads as W
         # size the sample for ~15 s of host-core work from a short probe
         g0, q0 = g[0], (None if quat is None else quat[0])
-        if args.route == "shapes":     # the oracle's own rendering of item 0 (already in the beam frame)
+        if args.route in ("shapes", "shapes_nufft"):     # the oracle's own rendering of item 0 (already in the beam frame)
             from oracle import render as OR
             g0, q0 = OR.render(shapes[0], (w.nx, w.ny, w.nz), vox), None
         probe = W.sample_pixels(w.seed + 99, w.npix, 32)
@@ -521,13 +532,13 @@ def main():
 
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if args.route == "nufft" else "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f64" if args.route in ("nufft", "shapes_nufft") else "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route == "nufft" else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route in ("nufft", "shapes_nufft") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
-                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route not in ("shapes", "shapes_qgrid") else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
+                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route not in ("shapes", "shapes_qgrid", "shapes_nufft") else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
                     "d2h_bytes_per_step": int(h_I.numel() * 4)},
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line), flush=True)

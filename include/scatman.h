@@ -265,6 +265,14 @@ int scatman_simulate_shapes_qgrid(scatman_ctx *ctx, const scatman_shape *h_shape
                                   double lambda, const double *d_qx, int32_t npx, const double *d_qy, int32_t npy,
                                   const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
 
+/* The same from shape descriptors on the NUFFT route for the flat detector: scatman_render followed by scatman_simulate_nufft
+ * (shapes are rendered in the beam frame, so a0 is skipped).  d_I[batch][npy][npx].  opts: rho_mode only. */
+int scatman_shapes_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                                         int32_t batch, size_t *bytes);
+int scatman_simulate_shapes_nufft(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
+                                  double lambda, const scatman_detector *det, const scatman_options *opts, void *d_ws,
+                                  size_t ws_bytes, float *d_I, void *cuda_stream);
+
 /* With SCATMAN_FLAG_COUNT_ISSUED: the number of 16-y x 16-x blocks of rho~ (256 voxels each) the contraction of the last
  * scatman_simulate* call multiplied against EVERY pixel, summed over slices and batch items; the dense count is
  * batch * nz * ceil(ny/16) * ceil(nx/16) blocks of the padded grid.  Issued tensor flop = blocks * 256 * npix_pad * 24.

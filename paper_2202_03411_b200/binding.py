@@ -27,6 +27,7 @@ EXPORTS = [
     "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
     "scatman_shapes_qgrid_workspace_bytes", "scatman_simulate_shapes_qgrid",
     "scatman_nufft_workspace_bytes", "scatman_nufft_grid_dims", "scatman_simulate_nufft",
+    "scatman_shapes_nufft_workspace_bytes", "scatman_simulate_shapes_nufft",
     "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
@@ -93,6 +94,9 @@ def load_library() -> C.CDLL:
     L.scatman_nufft_grid_dims.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(i32)]
     L.scatman_simulate_nufft.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
+    L.scatman_shapes_nufft_workspace_bytes.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), i32, C.POINTER(C.c_size_t)]
+    L.scatman_simulate_shapes_nufft.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), dbl, C.POINTER(Detector),
+                                                C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_qgrid_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i32, i32, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
     L.scatman_simulate_qgrid.argtypes = [vp, vp, C.POINTER(Grid), dbl, vp, i32, vp, i32, C.POINTER(dbl), i32,
                                          C.POINTER(Options), vp, C.c_size_t, vp, vp]
@@ -383,6 +387,29 @@ class Scatman:
         arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_simulate_shapes_qgrid(self._ctx, arr, batch, C.byref(grid), float(lam),
                                                            C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy,
+                                                           C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
+                                                           C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out
+
+    def simulate_shapes_nufft(self, shapes: Sequence[dict], dims, voxel, lam: float, npx: int, npy: int, theta_max_deg: float,
+                              rho_mode: int = RHO_LINEAR, cx: float = 0.0, cy: float = 0.0, workspace=None, out=None, stream=None):
+        """Shape descriptors -> I float32 [B][npy][npx] on the flat detector: rendered on the device, then the NUFFT route
+        (scatman_simulate_shapes_nufft)."""
+        import torch
+        nx, ny, nz = (int(v) for v in dims)
+        grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
+        det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
+        batch = len(shapes)
+        opts = Options(int(rho_mode), 0, 0, 0)
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_shapes_nufft_workspace_bytes(self._ctx, C.byref(grid), float(lam), C.byref(det), batch,
+                                                                  C.byref(need)))
+        if workspace is None:
+            workspace = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+        if out is None:
+            out = torch.empty((batch, npy, npx), dtype=torch.float32, device="cuda")
+        arr, keep = self._shape_array(shapes)
+        self._check(self.lib.scatman_simulate_shapes_nufft(self._ctx, arr, batch, C.byref(grid), float(lam), C.byref(det),
                                                            C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
                                                            C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out

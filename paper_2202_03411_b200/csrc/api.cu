@@ -755,6 +755,32 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     return SCATMAN_OK;
 }
 
+int scatman_shapes_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
+                                         int32_t batch, size_t *bytes) {
+    size_t inner = 0;
+    const int rc = scatman_nufft_workspace_bytes(ctx, grid, lambda, det, batch, &inner);
+    if (rc != SCATMAN_OK) return rc;
+    *bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024) + inner;
+    return SCATMAN_OK;
+}
+
+int scatman_simulate_shapes_nufft(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batch, const scatman_grid *grid,
+                                  double lambda, const scatman_detector *det, const scatman_options *opts, void *d_ws,
+                                  size_t ws_bytes, float *d_I, void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!h_shapes || !d_ws || !valid_grid(grid) || batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    const size_t dn_bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024);
+    if (ws_bytes < dn_bytes) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
+    float *d_dn = (float *)d_ws;
+    int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
+    if (rc != SCATMAN_OK) return rc;
+    const int rendered = ctx->last_launches;
+    rc = scatman_simulate_nufft(ctx, d_dn, grid, lambda, det, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes,
+                                d_I, cuda_stream);
+    if (rc == SCATMAN_OK) ctx->last_launches += rendered;
+    return rc;
+}
+
 // ---- forward-fitting pieces ---------------------------------------------------------------------------------------
 int scatman_fit_workspace_bytes(scatman_ctx *ctx, int64_t npix, int32_t batch, size_t *bytes) {
     if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;

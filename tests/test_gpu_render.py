@@ -183,6 +183,24 @@ def test_simulate_shapes_qgrid_equals_render_then_qgrid_and_matches_oracle(sm):
         assert_parity(I[i], ref, what=f"shapes qgrid item {items[i]}")
 
 
+def test_simulate_shapes_nufft_equals_render_then_nufft_and_matches_oracle(sm):
+    """scatman_simulate_shapes_nufft = scatman_render + scatman_simulate_nufft on the rendered grids (bit for bit), and matches the
+    oracle on the flat detector (cfg4 shapes at quarter scale)."""
+    import torch
+    w = W.config(3, scale=0.25)
+    items = [0, 1, 2, 3, 4, 5]
+    shapes = w.shapes(items)
+    dims, vox = (w.nx, w.ny, w.nz), (w.dx, w.dy, w.dz)
+    I = sm.simulate_shapes_nufft(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+    g = sm.render(shapes, dims, vox)
+    I2 = sm.simulate_nufft(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+    assert torch.equal(I, I2)
+    I = I.cpu().numpy()
+    for i in (0, 1, 4):
+        ref = O.simulate(g[i].cpu().numpy(), vox, w.lam, w.npx, w.npy, w.theta_max_deg)
+        assert_parity(I[i], ref, what=f"shapes nufft item {items[i]}")
+
+
 def test_workload_shape_descriptors_describe_the_same_particles_as_the_grids(sm):
     """The descriptors of cfg1 / cfg3 (identity orientation) render to exactly the voxel grids the generators produce."""
     for idx, scale in ((0, 1.0), (2, 0.25)):
