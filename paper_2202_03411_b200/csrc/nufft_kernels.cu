@@ -52,14 +52,19 @@ constexpr int BN = 64, BK = 16;
 __device__ inline double2 ld_c(const double2 *p) { return __ldg(p); }
 __device__ inline double2 ld_c(const float2 *p) { const float2 v = __ldg(p); return make_double2((double)v.x, (double)v.y); }
 
-// RM = rows per thread: the row tile is BM = 16 RM (32, 48 or 64), picked per GEMM so that M pads least (stage Z has M = nqz ~ 40-150).
-template <typename TA, typename TB, int RM>
+// RM = rows per thread: the row tile is BM = 16 RM (32, 48 or 64), picked per GEMM (zgemm below).  Shared memory is double-buffered, so a
+// K step costs ONE barrier: the tile of step s + 1 goes into the other buffer while slower warps still read step s.
+// A K step whose streamed tile is all zero (vacuum: rho~, and the planes and rows made from it, are exact zeros outside the particle) adds
+// nothing: the barrier doubles as a block-wide OR over "my part of the tile holds a non-zero", and the arithmetic is skipped.  ZERO_IN_A
+// says which operand can be vacuum (stage X: the P planes are A; stages Z and Y: rho~ / H are B); the other one is a phase table.
+template <typename TA, typename TB, int RM, bool ZERO_IN_A>
 __global__ void __launch_bounds__(256, RM <= 3 ? 2 : 1)
 nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *__restrict__ C, int M, int N, int K,
                    int64_t lda, int64_t ldb, int64_t ldc, int64_t strideA, int64_t strideB, int64_t strideC) {
     constexpr int BM = 16 * RM;
-    __shared__ double2 As[BK][BM + 1];
-    __shared__ double2 Bs[BK][BN];
+    extern __shared__ double2 zg_smem[];
+    double2 (*As)[BK][BM + 1] = reinterpret_cast<double2 (*)[BK][BM + 1]>(zg_smem);                          // [2][BK][BM + 1]
+    double2 (*Bs)[BK][BN] = reinterpret_cast<double2 (*)[BK][BN]>(zg_smem + 2 * BK * (BM + 1));              // [2][BK][BN]
     const int t = threadIdx.x, tx = t & 15, ty = t >> 4;
     const int n0 = blockIdx.x * BN, m0 = blockIdx.y * BM;
     A += (int64_t)blockIdx.z * strideA;
@@ -86,32 +91,31 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
         }
     };
     fetch(0);
-    for (int k0 = 0; k0 < K; k0 += BK) {
-        // A K step whose A tile or B tile is all zero (vacuum: rho~, and the planes and rows made from it, are exact zeros
-        // outside the particle) adds nothing: the block agrees on that with two barrier reductions and skips the arithmetic.
-        bool nza = false, nzb = false;
+    int buf = 0;
+    for (int k0 = 0; k0 < K; k0 += BK, buf ^= 1) {
+        bool nz = false;
 #pragma unroll
         for (int r = 0; r < RM; ++r) {
             const int idx = t + 256 * r;
-            As[idx & 15][idx >> 4] = ra[r];
-            nza |= ra[r].x != 0.0 || ra[r].y != 0.0;
+            As[buf][idx & 15][idx >> 4] = ra[r];
+            if (ZERO_IN_A) nz |= ra[r].x != 0.0 || ra[r].y != 0.0;
         }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int idx = t + 256 * r;
-            Bs[idx >> 6][idx & 63] = rb[r];
-            nzb |= rb[r].x != 0.0 || rb[r].y != 0.0;
+            Bs[buf][idx >> 6][idx & 63] = rb[r];
+            if (!ZERO_IN_A) nz |= rb[r].x != 0.0 || rb[r].y != 0.0;
         }
-        const bool live = __syncthreads_or(nzb) != 0 && __syncthreads_or(nza) != 0;   // the first one orders the stores above
+        const bool live = __syncthreads_or(nz) != 0;
         if (k0 + BK < K) fetch(k0 + BK);
         if (!live) continue;
 #pragma unroll
         for (int k = 0; k < BK; ++k) {
             double2 a[RM], b[4];
 #pragma unroll
-            for (int i = 0; i < RM; ++i) a[i] = As[k][ty + 16 * i];
+            for (int i = 0; i < RM; ++i) a[i] = As[buf][k][ty + 16 * i];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
+            for (int j = 0; j < 4; ++j) b[j] = Bs[buf][k][tx + 16 * j];
 #pragma unroll
             for (int i = 0; i < RM; ++i)
 #pragma unroll
@@ -122,7 +126,6 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
                     acc[i][j].y = fma(a[i].y, b[j].x, acc[i][j].y);
                 }
         }
-        __syncthreads();
     }
 #pragma unroll
     for (int i = 0; i < RM; ++i) {
@@ -136,21 +139,23 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
     }
 }
 
-template <typename TA, typename TB, int RM>
+template <typename TA, typename TB, int RM, bool ZERO_IN_A>
 cudaError_t zgemm_rm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
                      int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
     constexpr int BM = 16 * RM;
+    constexpr size_t smem = sizeof(double2) * 2 * BK * ((BM + 1) + BN);
+    // (the dynamic shared-memory limit of every instantiation is raised once per device, nufft_init_device)
     // grid.y carries the row tiles (<= 65535), grid.z the batch (<= 65535, the callers' concern)
     for (int64_t m_base = 0; m_base < M; m_base += 65535LL * BM) {
         const int rows = (int)(M - m_base < 65535LL * BM ? M - m_base : 65535LL * BM);
         dim3 grid((N + BN - 1) / BN, (rows + BM - 1) / BM, nbatch);
-        nufft_zgemm_kernel<TA, TB, RM><<<grid, 256, 0, st>>>(A + m_base * lda, B, C + m_base * ldc, rows, N, K, lda, ldb, ldc, sA, sB,
-                                                             sC);
+        nufft_zgemm_kernel<TA, TB, RM, ZERO_IN_A><<<grid, 256, smem, st>>>(A + m_base * lda, B, C + m_base * ldc, rows, N, K, lda, ldb, ldc,
+                                                                          sA, sB, sC);
     }
     return cudaGetLastError();
 }
 
-template <typename TA, typename TB>
+template <typename TA, typename TB, bool ZERO_IN_A>
 cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
                   int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
     // Row tile by a makespan estimate: resident sets of 148 x (2 CTAs of RM <= 3, or 1 of RM = 4) run one after the other and a
@@ -162,9 +167,9 @@ cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int
         return sets * cps * rm * 1000000 + (int64_t)((M + 16 * rm - 1) / (16 * rm)) * 16 * rm % 1000000 * 10 + (4 - rm);
     };
     const int64_t c2 = cost(2), c3 = cost(3), c4 = cost(4);
-    if (c4 <= c3 && c4 <= c2) return zgemm_rm<TA, TB, 4>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
-    if (c3 <= c2) return zgemm_rm<TA, TB, 3>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
-    return zgemm_rm<TA, TB, 2>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (c4 <= c3 && c4 <= c2) return zgemm_rm<TA, TB, 4, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (c3 <= c2) return zgemm_rm<TA, TB, 3, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    return zgemm_rm<TA, TB, 2, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
 }
 
 // ---- interpolation: A = sum over the W^3 nearest grid points, I = |A dV|^2 (Block 11).
@@ -337,8 +342,6 @@ cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &
                           double dV, float *d_I, cudaStream_t st) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     const size_t smem = sizeof(double) * 2 * P * KU * kInterpThreads;
-    cudaError_t e = cudaFuncSetAttribute(nufft_interp_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
     const int64_t groups = (int64_t)((npx + P - 1) / P) * npy;
     dim3 grid((unsigned)((groups + kInterpThreads - 1) / kInterpThreads), nb);
     nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_I);
@@ -400,7 +403,22 @@ cudaError_t nufft_init_device() {
         }
         fitted = true;
     }
-    return cudaMemcpyToSymbol(c_kb, coef, sizeof(coef));
+    cudaError_t e = cudaMemcpyToSymbol(c_kb, coef, sizeof(coef));
+    auto smem_gemm = [](int rm) { return (int)(sizeof(double2) * 2 * BK * ((16 * rm + 1) + BN)); };
+    auto smem_interp = [](int P) { return (int)(sizeof(double) * 2 * P * (P > 1 ? kW + 2 : kW) * kInterpThreads); };
+    const cudaFuncAttribute attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+#define SCATMAN_ZGEMM_ATTR(RM)                                                                                          \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, float2, RM, false>, attr, smem_gemm(RM));   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, RM, true>, attr, smem_gemm(RM));   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, RM, false>, attr, smem_gemm(RM));
+    SCATMAN_ZGEMM_ATTR(2)
+    SCATMAN_ZGEMM_ATTR(3)
+    SCATMAN_ZGEMM_ATTR(4)
+#undef SCATMAN_ZGEMM_ATTR
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<1>, attr, smem_interp(1));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<2>, attr, smem_interp(2));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<4>, attr, smem_interp(4));
+    return e;
 }
 
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st) {
@@ -422,18 +440,18 @@ cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPl
     const int64_t nyx = (int64_t)p.ny * p.nx;
     cudaError_t e = cudaSuccess;
     // stage Z, one GEMM per item: P_b (nqz x ny nx) = Tz (nqz x nz) * rho~_b (nz x ny nx)
-    e = zgemm<double2, float2>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, nb, 0, (int64_t)p.nz * nyx,
+    e = zgemm<double2, float2, false>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, nb, 0, (int64_t)p.nz * nyx,
                                (int64_t)n.az.nq * nyx, st);
     if (e != cudaSuccess) return e;
     // stage X, all items and planes at once: H ((nb nqz ny) x nqx) = P ((nb nqz ny) x nx) * TxT (nx x nqx)
     const int64_t rows = (int64_t)nb * n.az.nq * p.ny;     // < 2^31: the chunk holds at most 2 GB of P
-    e = zgemm<double2, double2>(d_P, d_TxT, d_H, (int)rows, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
+    e = zgemm<double2, double2, true>(d_P, d_TxT, d_H, (int)rows, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
     if (e != cudaSuccess) return e;
     // stage Y, one GEMM per (item, g_z plane): U_m (nqy x nqx) = Ty (nqy x ny) * H_m (ny x nqx)
     const int planes = nb * n.az.nq;
     for (int z0 = 0; z0 < planes; z0 += 65535) {
         const int nzb = planes - z0 < 65535 ? planes - z0 : 65535;
-        e = zgemm<double2, double2>(d_Ty, d_H + (int64_t)z0 * p.ny * n.ax.nq, d_U + (int64_t)z0 * n.ay.nq * n.ax.nq, n.ay.nq, n.ax.nq,
+        e = zgemm<double2, double2, false>(d_Ty, d_H + (int64_t)z0 * p.ny * n.ax.nq, d_U + (int64_t)z0 * n.ay.nq * n.ax.nq, n.ay.nq, n.ax.nq,
                                     p.ny, p.ny, n.ax.nq, n.ax.nq, nzb, 0, (int64_t)p.ny * n.ax.nq, (int64_t)n.ay.nq * n.ax.nq, st);
         if (e != cudaSuccess) return e;
     }

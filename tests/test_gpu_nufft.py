@@ -93,6 +93,21 @@ def test_cfg5_coreshell_eighth_scale(sm):
     assert_parity(I, O.simulate(g, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg), what="nufft cfg5 eighth")
 
 
+def test_batch_larger_than_one_chunk(sm):
+    """The stage-Z planes of a chunk are capped at 2 GB: nine wide, thin items (1024 x 1024 x 4 voxels, ~270 MB of planes each) run as a
+    chunk of seven or eight and a rest.  Checked at seeded pixels of three items, first and last included."""
+    nx, ny, nz, B_ = 1024, 1024, 4, 9
+    voxel, lam = (1.0, 1.0, 2.0), 9.0
+    g = np.stack([W.sparse_blobs_grid(400 + i, nx, ny, nz, nblobs=6, max_extent=40) for i in range(B_)])
+    npx, npy, th = 24, 20, 5.0
+    I = sm.simulate_nufft(dev(g), voxel, lam, npx, npy, th).cpu().numpy()
+    pix = W.sample_pixels(19, npx * npy, 40, always=[0, npx * npy - 1])
+    for b in (0, 6, 7, 8):
+        ref = O.simulate(g[b], voxel, lam, npx, npy, th, pixels=pix)
+        assert_parity(I[b].ravel()[pix], ref, what=f"nufft chunked batch item {b}")
+    assert not np.array_equal(I[7], I[8])
+
+
 def test_empty_and_single_voxel(sm):
     voxel, lam = (3.0, 3.0, 3.0), 12.0
     z = np.zeros((8, 8, 8, 2), np.float32)
