@@ -675,7 +675,7 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
     L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
     L.off_P = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx);
     L.off_H = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq);
-    L.off_U = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
+    L.off_U = take(sizeof(float2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
     L.total = off;
     return L;
 }
@@ -744,7 +744,7 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     for (int b0 = 0; b0 < batch; b0 += L.n.nb) {   // a chunk of items per set of launches
         const int nb = batch - b0 < L.n.nb ? batch - b0 : L.n.nb;
         e = launch_nufft_chunk((const float2 *)rho + (size_t)b0 * p.nvox, p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, Tz, TxT, Ty,
-                               q, (double2 *)(ws + L.off_P), (double2 *)(ws + L.off_H), (double2 *)(ws + L.off_U),
+                               q, (double2 *)(ws + L.off_P), (double2 *)(ws + L.off_H), (float2 *)(ws + L.off_U),
                                d_I + (size_t)b0 * p.npix, st);
         nl += 4;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");

@@ -106,7 +106,7 @@ cudaError_t nufft_init_device();   // once per device (scatman_create): uploads 
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st);
 cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
-                               double2 *d_H, double2 *d_U, float *d_I, cudaStream_t st);
+                               double2 *d_H, float2 *d_U, float *d_I, cudaStream_t st);
 
 // forward-fitting pieces (fit_kernels.cu)
 size_t fit_workspace_bytes(int64_t npix, int batch);

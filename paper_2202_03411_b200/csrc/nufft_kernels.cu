@@ -57,9 +57,12 @@ __device__ inline double2 ld_c(const float2 *p) { const float2 v = __ldg(p); ret
 // A K step whose streamed tile is all zero (vacuum: rho~, and the planes and rows made from it, are exact zeros outside the particle) adds
 // nothing: the barrier doubles as a block-wide OR over "my part of the tile holds a non-zero", and the arithmetic is skipped.  ZERO_IN_A
 // says which operand can be vacuum (stage X: the P planes are A; stages Z and Y: rho~ / H are B); the other one is a phase table.
-template <typename TA, typename TB, int RM, bool ZERO_IN_A>
+__device__ inline void st_c(double2 *p, double2 v) { *p = v; }
+__device__ inline void st_c(float2 *p, double2 v) { *p = make_float2((float)v.x, (float)v.y); }
+
+template <typename TA, typename TB, typename TC, int RM, bool ZERO_IN_A>
 __global__ void __launch_bounds__(256, RM <= 3 ? 2 : 1)
-nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *__restrict__ C, int M, int N, int K,
+nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, TC *__restrict__ C, int M, int N, int K,
                    int64_t lda, int64_t ldb, int64_t ldc, int64_t strideA, int64_t strideB, int64_t strideC) {
     constexpr int BM = 16 * RM;
     extern __shared__ double2 zg_smem[];
@@ -134,13 +137,13 @@ nufft_zgemm_kernel(const TA *__restrict__ A, const TB *__restrict__ B, double2 *
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int n = n0 + tx + 16 * j;
-            if (n < N) C[(int64_t)m * ldc + n] = acc[i][j];
+            if (n < N) st_c(C + (int64_t)m * ldc + n, acc[i][j]);
         }
     }
 }
 
-template <typename TA, typename TB, int RM, bool ZERO_IN_A>
-cudaError_t zgemm_rm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
+template <typename TA, typename TB, typename TC, int RM, bool ZERO_IN_A>
+cudaError_t zgemm_rm(const TA *A, const TB *B, TC *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
                      int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
     constexpr int BM = 16 * RM;
     constexpr size_t smem = sizeof(double2) * 2 * BK * ((BM + 1) + BN);
@@ -149,14 +152,14 @@ cudaError_t zgemm_rm(const TA *A, const TB *B, double2 *C, int M, int N, int K, 
     for (int64_t m_base = 0; m_base < M; m_base += 65535LL * BM) {
         const int rows = (int)(M - m_base < 65535LL * BM ? M - m_base : 65535LL * BM);
         dim3 grid((N + BN - 1) / BN, (rows + BM - 1) / BM, nbatch);
-        nufft_zgemm_kernel<TA, TB, RM, ZERO_IN_A><<<grid, 256, smem, st>>>(A + m_base * lda, B, C + m_base * ldc, rows, N, K, lda, ldb, ldc,
+        nufft_zgemm_kernel<TA, TB, TC, RM, ZERO_IN_A><<<grid, 256, smem, st>>>(A + m_base * lda, B, C + m_base * ldc, rows, N, K, lda, ldb, ldc,
                                                                           sA, sB, sC);
     }
     return cudaGetLastError();
 }
 
-template <typename TA, typename TB, bool ZERO_IN_A>
-cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
+template <typename TA, typename TB, typename TC, bool ZERO_IN_A>
+cudaError_t zgemm(const TA *A, const TB *B, TC *C, int M, int N, int K, int64_t lda, int64_t ldb, int64_t ldc, int nbatch,
                   int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
     // Row tile by a makespan estimate: resident sets of 148 x (2 CTAs of RM <= 3, or 1 of RM = 4) run one after the other and a
     // set takes ~ CTAs per SM x RM; ties go to the least padding, then to the taller tile.
@@ -167,12 +170,15 @@ cudaError_t zgemm(const TA *A, const TB *B, double2 *C, int M, int N, int K, int
         return sets * cps * rm * 1000000 + (int64_t)((M + 16 * rm - 1) / (16 * rm)) * 16 * rm % 1000000 * 10 + (4 - rm);
     };
     const int64_t c2 = cost(2), c3 = cost(3), c4 = cost(4);
-    if (c4 <= c3 && c4 <= c2) return zgemm_rm<TA, TB, 4, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
-    if (c3 <= c2) return zgemm_rm<TA, TB, 3, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
-    return zgemm_rm<TA, TB, 2, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (c4 <= c3 && c4 <= c2) return zgemm_rm<TA, TB, TC, 4, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    if (c3 <= c2) return zgemm_rm<TA, TB, TC, 3, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
+    return zgemm_rm<TA, TB, TC, 2, ZERO_IN_A>(A, B, C, M, N, K, lda, ldb, ldc, nbatch, sA, sB, sC, st);
 }
 
 // ---- interpolation: A = sum over the W^3 nearest grid points, I = |A dV|^2 (Block 11).
+// U is stored FP32 (stage Y rounds its FP64 accumulators on the way out): the window's weights are positive and A varies slowly over the
+// window, so a value's 6e-8 relative rounding stays relative to the LOCAL amplitude (unlike an error made before the transforms, which
+// would be relative to the whole particle); sums and weights stay FP64.  Halves the bytes this L1-bound kernel pulls.
 // A thread owns P consecutive pixels of a detector row: their windows overlap (a pixel is a fraction of a grid cell wide), so the
 // thread walks ONE common window of KU = W + 2 cells per axis, loads every grid value once and applies it to all P pixels with
 // per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the bytes it pulls through L1, and this divides
@@ -210,7 +216,7 @@ constexpr int kInterpThreads = 64;
 template <int P>
 __global__ void __launch_bounds__(kInterpThreads)
 nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
-                    const double2 *__restrict__ U, int64_t strideU, double dV, float *__restrict__ I) {
+                    const float2 *__restrict__ U, int64_t strideU, double dV, float *__restrict__ I) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     extern __shared__ double wsm[];                       // [2][P][KU][kInterpThreads]
     const int ngx = (npx + P - 1) / P;
@@ -272,8 +278,8 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
 #pragma unroll
                 for (int j = 0; j < P; ++j) { wyb[j] = wy(j, b); anyb |= wyb[j] != 0.0; }
                 if (!anyb) continue;
-                const double2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
-                double2 v[KU];
+                const float2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
+                float2 v[KU];
 #pragma unroll
                 for (int a = 0; a < KU; ++a) v[a] = __ldg(row + a);
 #pragma unroll
@@ -281,8 +287,8 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
                     double rre = 0.0, rim = 0.0;
 #pragma unroll
                     for (int a = 0; a < KU; ++a) {
-                        rre = fma(wx[j][a], v[a].x, rre);
-                        rim = fma(wx[j][a], v[a].y, rim);
+                        rre = fma(wx[j][a], (double)v[a].x, rre);
+                        rim = fma(wx[j][a], (double)v[a].y, rim);
                     }
                     pre[j] = fma(wyb[j], rre, pre[j]);
                     pim[j] = fma(wyb[j], rim, pim[j]);
@@ -317,13 +323,13 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
         for (int c = 0; c < kW; ++c) {
             double pre = 0.0, pim = 0.0;
             for (int b = 0; b < kW; ++b) {
-                const double2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
+                const float2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
                 double rre = 0.0, rim = 0.0;
 #pragma unroll
                 for (int a = 0; a < kW; ++a) {
-                    const double2 v = __ldg(row + a);
-                    rre = fma(wx1[a], v.x, rre);
-                    rim = fma(wx1[a], v.y, rim);
+                    const float2 v = __ldg(row + a);
+                    rre = fma(wx1[a], (double)v.x, rre);
+                    rim = fma(wx1[a], (double)v.y, rim);
                 }
                 pre = fma(wy(0, b), rre, pre);
                 pim = fma(wy(0, b), rim, pim);
@@ -338,7 +344,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
 }
 
 template <int P>
-cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &n, const double2 *d_U, int64_t strideU, int nb,
+cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &n, const float2 *d_U, int64_t strideU, int nb,
                           double dV, float *d_I, cudaStream_t st) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     const size_t smem = sizeof(double) * 2 * P * KU * kInterpThreads;
@@ -408,9 +414,9 @@ cudaError_t nufft_init_device() {
     auto smem_interp = [](int P) { return (int)(sizeof(double) * 2 * P * (P > 1 ? kW + 2 : kW) * kInterpThreads); };
     const cudaFuncAttribute attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
 #define SCATMAN_ZGEMM_ATTR(RM)                                                                                          \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, float2, RM, false>, attr, smem_gemm(RM));   \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, RM, true>, attr, smem_gemm(RM));   \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, RM, false>, attr, smem_gemm(RM));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, float2, double2, RM, false>, attr, smem_gemm(RM));   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, double2, RM, true>, attr, smem_gemm(RM));   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, double2, float2, RM, false>, attr, smem_gemm(RM));
     SCATMAN_ZGEMM_ATTR(2)
     SCATMAN_ZGEMM_ATTR(3)
     SCATMAN_ZGEMM_ATTR(4)
@@ -436,22 +442,22 @@ cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz
 // pixel_cells = the widest step between neighbouring pixels of a row, in grid cells of any axis (picks the pixels per thread).
 cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
-                               double2 *d_H, double2 *d_U, float *d_I, cudaStream_t st) {
+                               double2 *d_H, float2 *d_U, float *d_I, cudaStream_t st) {
     const int64_t nyx = (int64_t)p.ny * p.nx;
     cudaError_t e = cudaSuccess;
     // stage Z, one GEMM per item: P_b (nqz x ny nx) = Tz (nqz x nz) * rho~_b (nz x ny nx)
-    e = zgemm<double2, float2, false>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, nb, 0, (int64_t)p.nz * nyx,
+    e = zgemm<double2, float2, double2, false>(d_Tz, d_rho, d_P, n.az.nq, (int)nyx, p.nz, p.nz, nyx, nyx, nb, 0, (int64_t)p.nz * nyx,
                                (int64_t)n.az.nq * nyx, st);
     if (e != cudaSuccess) return e;
     // stage X, all items and planes at once: H ((nb nqz ny) x nqx) = P ((nb nqz ny) x nx) * TxT (nx x nqx)
     const int64_t rows = (int64_t)nb * n.az.nq * p.ny;     // < 2^31: the chunk holds at most 2 GB of P
-    e = zgemm<double2, double2, true>(d_P, d_TxT, d_H, (int)rows, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
+    e = zgemm<double2, double2, double2, true>(d_P, d_TxT, d_H, (int)rows, n.ax.nq, p.nx, p.nx, n.ax.nq, n.ax.nq, 1, 0, 0, 0, st);
     if (e != cudaSuccess) return e;
     // stage Y, one GEMM per (item, g_z plane): U_m (nqy x nqx) = Ty (nqy x ny) * H_m (ny x nqx)
     const int planes = nb * n.az.nq;
     for (int z0 = 0; z0 < planes; z0 += 65535) {
         const int nzb = planes - z0 < 65535 ? planes - z0 : 65535;
-        e = zgemm<double2, double2, false>(d_Ty, d_H + (int64_t)z0 * p.ny * n.ax.nq, d_U + (int64_t)z0 * n.ay.nq * n.ax.nq, n.ay.nq, n.ax.nq,
+        e = zgemm<double2, double2, float2, false>(d_Ty, d_H + (int64_t)z0 * p.ny * n.ax.nq, d_U + (int64_t)z0 * n.ay.nq * n.ax.nq, n.ay.nq, n.ax.nq,
                                     p.ny, p.ny, n.ax.nq, n.ax.nq, nzb, 0, (int64_t)p.ny * n.ax.nq, (int64_t)n.ay.nq * n.ax.nq, st);
         if (e != cudaSuccess) return e;
     }
