@@ -26,7 +26,7 @@ FLOP_PER_TERM = 8    # one complex MAC
 # (profiles/r01_contract_cfg3_full.md); only the workload that was captured has a number
 NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": 2.295495e9 + 8.534016e6}
 # the same for the four launches of one NUFFT pattern (stages Z, X, Y, interpolation; profiles/r01_nufft.md)
-NCU_DRAM_BYTES_NUFFT = {"cfg3_droplet_256": (134.436 + 22.964 + 46.631 + 0.980 + 20.852 + 0.0 + 9.708 + 0.0) * 1e6}
+NCU_DRAM_BYTES_NUFFT = {"cfg3_droplet_256": (134.46 + 24.46 + 46.63 + 0.91 + 20.85 + 0.0 + 8.27 + 0.0) * 1e6}
 
 
 def load_peaks():
