@@ -179,7 +179,7 @@ cudaError_t zgemm(const TA *A, const TB *B, TC *C, int M, int N, int K, int64_t 
 // U is stored FP32 (stage Y rounds its FP64 accumulators on the way out): the window's weights are positive and A varies slowly over the
 // window, so a value's 6e-8 relative rounding stays relative to the LOCAL amplitude (unlike an error made before the transforms, which
 // would be relative to the whole particle); sums and weights stay FP64.  Halves the bytes this L1-bound kernel pulls.
-// A thread owns P consecutive pixels of a detector row: their windows overlap (a pixel is a fraction of a grid cell wide), so the
+// A thread owns P = 4, 3, 2 or 1 consecutive pixels of a detector row: their windows overlap (a pixel is a fraction of a grid cell wide), so the
 // thread walks ONE common window of KU = W + 2 cells per axis, loads every grid value once and applies it to all P pixels with
 // per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the bytes it pulls through L1, and this divides
 // them by ~P.  A group whose windows do not fit the common one (pixels more than a cell apart: coarse detectors) takes its pixels
@@ -423,6 +423,7 @@ cudaError_t nufft_init_device() {
 #undef SCATMAN_ZGEMM_ATTR
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<1>, attr, smem_interp(1));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<2>, attr, smem_interp(2));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<3>, attr, smem_interp(3));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<4>, attr, smem_interp(4));
     return e;
 }
@@ -463,8 +464,11 @@ cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPl
     }
     const int64_t strideU = (int64_t)n.az.nq * n.ay.nq * n.ax.nq;
     const double dV = p.dx * p.dy * p.dz;
-    if (3.0 * pixel_cells <= 1.0) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
-    if (pixel_cells <= 1.0) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    // P pixels share a window of W + 2 cells if their first cells differ by at most 2, i.e. if they lie within 2 grid cells of each other
+    // on every axis: (P - 1) x pixel_cells < 2 (with a margin; a group that still does not fit takes its pixels one by one in the kernel)
+    if (3.0 * pixel_cells < 1.9) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    if (2.0 * pixel_cells < 1.9) return launch_interp<3>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    if (pixel_cells < 1.9) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
     return launch_interp<1>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
 }
 
