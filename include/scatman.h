@@ -154,7 +154,8 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
  * PAPER.md:68-87), same a0 / a1 / a2 steps, conventions and output scale -- but rho~ is first transformed onto a small uniform
  * (gz, gy, gx) grid covering the detector's q range (three FP64 complex GEMMs: slices, columns, rows; spacing 2 pi / (2 N d),
  * Kaiser-Bessel pre-correction) and every pixel is then interpolated from its 10^3 nearest grid points.  The window's
- * aliasing error is < 1e-8 of sum |rho~| dV per pixel; everything else is FP64, so north_star's tolerances against the direct
+ * aliasing error is < 1e-8 of sum |rho~| dV per pixel; all sums are FP64 (the uniform-grid values are stored FP32 for the
+ * interpolation, a rounding relative to the local amplitude), so north_star's tolerances against the direct
  * sum hold (tests/test_gpu_nufft.py).  Work ~ N_vox * nqz + ... instead of N_vox * N_pix: ~1000x fewer multiply-adds.
  * opts: rho_mode only (method, precision, flags ignored).  d_I[b][npy][npx].  The workspace depends on lambda and the
  * detector (they fix the q range): scatman_nufft_workspace_bytes with the same arguments. */

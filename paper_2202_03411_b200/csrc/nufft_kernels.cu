@@ -9,8 +9,11 @@
 // Grid spacing h_d = 2 pi / (2 N_d d_d) (oversampling 2), pre-correction c_i = 1 / Phi(h x_i) with Phi the window's Fourier transform:
 //   sum_m phi(u - m) e^{i m t} = sum_l Phi(t - 2 pi l) e^{i u (t - 2 pi l)}   (Poisson summation),   |t| = |h x_i| < pi / 2,
 // so the l = 0 term is the wanted e^{i u t} and the l = +-1 aliases are below 3e-9 of it for W = 10, beta = pi sqrt(W^2 (3/4)^2 - 0.8).
-// Everything is FP64 on the CUDA cores (the work is ~1000x smaller than the pixel contraction: 1.2e9 complex MACs for 256^3 on 512^2
-// pixels against 4.4e12), so the only approximation is the window's and the result meets the same tolerances against the oracle.
+// All sums, tables and window weights are FP64 on the CUDA cores (the work is ~3000x smaller than the pixel contraction: 1.2e9 complex MACs for
+// 256^3 on 512^2 pixels against 4.4e12); only U is stored FP32 for the interpolation (see nufft_interp_kernel).  The only approximation beyond
+// rounding is the window's, and the result meets the same tolerances against the oracle's direct sum (tests/test_gpu_nufft.py).
+// Kernels: nufft_table_kernel (phase tables with the window correction folded in), nufft_zgemm_kernel (the three GEMM stages),
+// nufft_interp_kernel<P> (P = 4, 3, 2, 1 pixels per thread); nufft_init_device fits the window's per-cell polynomials (host) once per device.
 #include "internal.h"
 
 namespace scatman {
