@@ -132,6 +132,40 @@ def test_agrees_with_the_pixel_contraction_and_is_deterministic(sm):
     assert l2 <= 1e-4 and pix <= 1e-3
 
 
+def test_call_is_capturable_in_a_cuda_graph(sm):
+    """The entry point only enqueues work on the caller's stream (no allocation, no synchronisation), so a whole call can be captured in
+    a CUDA graph and replayed on new input: the replay must give what an eager call gives (bit for bit), oriented batch included."""
+    import torch
+    w = W.config(1, scale=0.25)
+    vox = (w.dx, w.dy, w.dz)
+    g0, g1 = w.grid(0), W.random_grid(5, w.nx, w.ny, w.nz, fill=0.3)
+    static_in = dev(g0)
+    out = torch.empty((1, w.npy, w.npx), dtype=torch.float32, device="cuda")
+    from paper_2202_03411_b200 import binding as B
+    import ctypes as C
+    need = C.c_size_t(0)
+    grid = B.Grid(w.nx, w.ny, w.nz, *vox)
+    det = B.Detector(w.npx, w.npy, w.theta_max_deg, 0.0, 0.0)
+    sm._check(sm.lib.scatman_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), 1, C.byref(need)))
+    ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):                         # warm-up outside the capture
+        sm.simulate_nufft(static_in, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat, workspace=ws, out=out)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        sm.simulate_nufft(static_in, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat, workspace=ws, out=out)
+    for g in (g1, g0):
+        static_in.copy_(dev(g))
+        graph.replay()
+        torch.cuda.synchronize()
+        got = out.clone()
+        ref = sm.simulate_nufft(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=w.quat)
+        assert torch.equal(got[0], ref)
+
+
 def test_error_codes(sm):
     import torch
     from paper_2202_03411_b200 import binding as B
