@@ -239,6 +239,8 @@ def main():
     ap.add_argument("--method", type=int, default=1, help="1 tensor (default), 2 simt_sincos, 3 simt_table")
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", action="store_true",
+                    help="--route nufft only: capture one call in a CUDA graph after the warm-up and time its replays")
     ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit", "nufft", "shapes_nufft"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
@@ -365,9 +367,24 @@ def main():
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     kernel_ms, launches = [], 0
     torch.cuda.synchronize()
+    graph = None
+    if args.graph:
+        if args.route != "nufft":
+            raise SystemExit("--graph applies to --route nufft")
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):      # the call only enqueues on the capturing stream: the whole step becomes one graph
+            sm.simulate_nufft(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, workspace=ws, out=out)
+        graph_launches = sm.last_launch_count()
+        graph.replay()
+        torch.cuda.synchronize()
     for i in range(args.steps):
         flush.zero_()                      # L2 flush, outside the timed events
         ev[i][0].record(stream)
+        if graph is not None:
+            graph.replay()
+            ev[i][1].record(stream)
+            launches += graph_launches
+            continue
         step()
         ev[i][1].record(stream)
         launches += sm.last_launch_count()
@@ -415,7 +432,8 @@ def main():
     value = patterns / (total_ms * 1e-3)
     terms_per_pattern = w.nvox * w.npix
     peaks = load_peaks()
-    k_ms = sum(kernel_ms) / len(kernel_ms)
+    # graph replays have no per-kernel events: the roofline then takes the WHOLE step (a1, a2 and tables included) as the kernel time
+    k_ms = sum(kernel_ms) / len(kernel_ms) if kernel_ms else total_ms / args.steps
     dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
     if args.route in ("qgrid", "shapes_qgrid"):
         dense_sep = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)   # both stages, 8 flop per complex MAC
@@ -534,7 +552,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if args.route in ("nufft", "shapes_nufft") else "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route in ("nufft", "shapes_nufft") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "cuda_graph": bool(args.graph), "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route in ("nufft", "shapes_nufft") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
                        "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
             "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
