@@ -147,3 +147,141 @@ def test_volume_map_cells_and_layout():
     want = np.zeros((4, 6, 8), dtype=bool)
     want[2:4, 4:6, 6:8] = True
     assert np.array_equal(g[..., 0] > 0, want)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Anisotropic pins of the voxel -> (theta, phi) / (latitude, longitude) mappings ("the North-South axis is
+# along the z direction"; Eq. 10; RadialMap example).  An l = 0 shape or a constant map
+# cannot tell z from x or atan2(y, x) from atan2(x, y); these can.
+def _half_extents(g):
+    """Number of inside voxels strictly beyond the centre voxel along +x, -x, +y, -y, +z, -z (odd dims, centre inside)."""
+    occ = g[..., 0] > 0
+    nz, ny, nx = occ.shape
+    cz, cy, cx = nz // 2, ny // 2, nx // 2
+    assert occ[cz, cy, cx]
+    def run(line):
+        n = 0
+        for v in line:
+            if not v:
+                break
+            n += 1
+        return n
+    return (run(occ[cz, cy, cx + 1:]), run(occ[cz, cy, cx - 1::-1]), run(occ[cz, cy + 1:, cx]), run(occ[cz, cy - 1::-1, cx]),
+            run(occ[cz + 1:, cy, cx]), run(occ[cz - 1::-1, cy, cx]))
+
+
+_SH_DIMS, _SH_VOX = (81, 81, 81), (1.0, 1.0, 1.0)
+_R0, _S = 25.4, 6.2                           # R = R0 +- S along the dipole's axis: half extents 31 / 19, 25 elsewhere
+
+
+def _dipole(m):
+    c = _S / sqrt(3 / (4 * pi))
+    return R.render({"kind": "spherical_harmonics", "delta": 1.0, "beta": 0.0,
+                     "coeffs": [(0, 0, _R0 * sqrt(4 * pi)), (1, m, c)]}, _SH_DIMS, _SH_VOX)
+
+
+def test_sh_l1_m0_dipole_points_along_plus_z():
+    """Y_1^0 = sqrt(3/4pi) cos(theta), theta from body +z: R = R0 + S cos(theta) -> longer towards +z, shorter towards -z,
+    R0 along x and y."""
+    assert _half_extents(_dipole(0)) == (25, 25, 25, 25, 31, 19)
+
+
+def test_sh_l1_m1_dipole_points_along_minus_x():
+    """sqrt(2) Re Y_1^1 = -sqrt(3/4pi) sin(theta) cos(phi) (Condon-Shortley), phi from +x towards +y: for c > 0 the shape
+    is longer towards -x, shorter towards +x, R0 along y and z."""
+    assert _half_extents(_dipole(1)) == (19, 31, 25, 25, 25, 25)
+
+
+def test_sh_l1_mneg1_dipole_points_along_minus_y():
+    """sqrt(2) Im Y_1^1 = -sqrt(3/4pi) sin(theta) sin(phi): for c > 0 longer towards -y, shorter towards +y."""
+    assert _half_extents(_dipole(-1)) == (25, 25, 19, 31, 25, 25)
+
+
+def test_sh_l2_m2_distinguishes_x_from_y():
+    """sqrt(2) Re Y_2^2 = sqrt(15/16pi) sin^2(theta) cos(2 phi): +S along +-x, -S along +-y, nothing along z."""
+    c = _S / sqrt(15 / (16 * pi))
+    g = R.render({"kind": "spherical_harmonics", "delta": 1.0, "beta": 0.0,
+                  "coeffs": [(0, 0, _R0 * sqrt(4 * pi)), (2, 2, c)]}, _SH_DIMS, _SH_VOX)
+    assert _half_extents(g) == (31, 31, 19, 19, 25, 25)
+
+
+def _ray_count(g, d):
+    """Inside voxels at centre + n d, n = 1, 2, ... (d an integer direction), until the first outside one."""
+    occ = g[..., 0] > 0
+    nz, ny, nx = occ.shape
+    z, y, x = nz // 2, ny // 2, nx // 2
+    n = 0
+    while True:
+        x, y, z = x + d[0], y + d[1], z + d[2]
+        if not (0 <= x < nx and 0 <= y < ny and 0 <= z < nz) or not occ[z, y, x]:
+            return n
+        n += 1
+
+
+def test_radial_map_raised_sample_sits_at_its_latitude_and_longitude():
+    """in a 4 x 4 map the sample (i, j) = (3, 1) is the radius at latitude +pi/4, longitude pi/2, i.e. along
+    (0, +1, +1)/sqrt(2): above the equator (z is the North-South axis), on the +y meridian."""
+    radii = np.full((4, 4), 10.0)
+    radii[3, 1] = 20.0
+    g = R.render({"kind": "radial_map", "delta": 1.0, "beta": 0.0, "radii": radii}, (41, 41, 41), (1.0, 1.0, 1.0))
+    assert _ray_count(g, (0, 1, 1)) == 14                  # n sqrt(2) <= 20
+    for d in ((0, -1, 1), (0, 1, -1), (0, -1, -1), (1, 0, -1), (-1, 0, -1), (1, 1, 0), (-1, 1, 0)):
+        assert _ray_count(g, d) == 7, d                    # n sqrt(2) <= 10: untouched directions
+    # (1, 0, 1) and (-1, 0, 1) lie at latitude pi/4 a quarter turn of longitude from the bump: bilinear weight 0 there
+    assert _ray_count(g, (1, 0, 1)) == 7 and _ray_count(g, (-1, 0, 1)) == 7
+    # sample (1, 2): latitude -pi/4, longitude pi -> along (-1, 0, -1)/sqrt(2)
+    radii = np.full((4, 4), 10.0)
+    radii[1, 2] = 20.0
+    g = R.render({"kind": "radial_map", "delta": 1.0, "beta": 0.0, "radii": radii}, (41, 41, 41), (1.0, 1.0, 1.0))
+    assert _ray_count(g, (-1, 0, -1)) == 14
+    for d in ((1, 0, -1), (-1, 0, 1), (0, -1, -1), (0, 1, -1), (1, 0, 1)):
+        assert _ray_count(g, d) == 7, d
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# The (latitude, longitude, rotation) helper of the input generators (workloads.quat_from_lat_long_rot, DESIGN.md R11)
+# against Fig. 6's caption (PAPER.md:289) and PAPER.md:281.
+def test_lat_long_rot_helper_follows_fig6():
+    from paper_2202_03411_b200 import workloads as W
+    zb, xb = np.array([0.0, 0.0, 1.0]), np.array([1.0, 0.0, 0.0])
+    M = lambda la, lo, ro: R.rotation_matrix(W.quat_from_lat_long_rot(la, lo, ro))
+    # "90 deg latitude indicates a direction towards the incoming beam": the beam travels along +z, so the main axis
+    # (body z) points to -z; "-90 deg latitude towards the detector": +z
+    assert np.allclose(M(90, 0, 0) @ zb, [0, 0, -1], atol=1e-12)
+    assert np.allclose(M(90, 123, 0) @ zb, [0, 0, -1], atol=1e-12)
+    assert np.allclose(M(-90, 0, 0) @ zb, [0, 0, 1], atol=1e-12)
+    # "the equator, at 0 deg latitude, lies on the plane orthogonal to the beam": longitude 0 -> +x, 90 -> +y
+    assert np.allclose(M(0, 0, 0) @ zb, [1, 0, 0], atol=1e-12)
+    assert np.allclose(M(0, 90, 0) @ zb, [0, 1, 0], atol=1e-12)
+    assert np.allclose(M(0, 180, 0) @ zb, [-1, 0, 0], atol=1e-12)
+    la, lo = np.radians(30.0), np.radians(40.0)
+    assert np.allclose(M(30, 40, 0) @ zb, [np.cos(la) * np.cos(lo), np.cos(la) * np.sin(lo), -np.sin(la)], atol=1e-12)
+    # "once the main axis is oriented, a rotation is applied to the sample along this axis": the main axis stays, a
+    # body vector perpendicular to it turns by the rotation angle, right-handed about the main axis
+    for (a, b) in ((0, 0), (30, 40), (-55, 200), (90, 0)):
+        M0 = M(a, b, 0)
+        axis = M0 @ zb
+        for rot in (10.0, 90.0, 170.0):
+            M1 = M(a, b, rot)
+            assert np.allclose(M1 @ zb, axis, atol=1e-12)
+            u0, u1 = M0 @ xb, M1 @ xb
+            assert np.isclose(np.dot(u0, u1), np.cos(np.radians(rot)), atol=1e-12)
+            assert np.isclose(np.dot(np.cross(u0, u1), axis), np.sin(np.radians(rot)), atol=1e-12)
+            assert np.isclose(np.linalg.det(M1), 1.0, atol=1e-12)
+    # every quaternion is unit (the boundary rejects others)
+    assert np.isclose(np.linalg.norm(W.quat_from_lat_long_rot(12, 34, 56)), 1.0, atol=1e-15)
+
+
+def test_lat_long_rot_helper_orients_a_rendered_shape():
+    """An ellipsoid that is long along its main (body z) axis, rendered through the oracle with the helper's quaternion:
+    latitude 90 -> long along the beam (grid z); latitude 0, longitude 0 -> long along grid x; longitude 90 -> grid y."""
+    from paper_2202_03411_b200 import workloads as W
+    shape = {"kind": "ellipsoid", "delta": 1.0, "beta": 0.0, "a": 5.3, "b": 8.3, "c": 14.3}
+    dims, vox = (41, 41, 41), (1.0, 1.0, 1.0)
+    ext = lambda la, lo, ro: _half_extents(R.render({**shape, "quat": W.quat_from_lat_long_rot(la, lo, ro)}, dims, vox))
+    assert ext(90, 0, 0)[4:] == (14, 14)
+    assert ext(0, 0, 0)[:2] == (14, 14)
+    assert ext(0, 90, 0)[2:4] == (14, 14)
+    # rotation about the main axis exchanges the two short axes after a quarter turn
+    e0, e1 = ext(90, 0, 0), ext(90, 0, 90)
+    assert sorted((e0[0], e0[2])) == [5, 8] and (e1[0], e1[2]) == (e0[2], e0[0])
