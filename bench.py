@@ -228,6 +228,51 @@ def load_peaks_hbm():
     return 6500.0, "fallback of B200_PROFILING.md"
 
 
+def measure_peaks(args):
+    """--measure-peaks: dense GEMM peaks of the tensor pipe for the operand types the library's tcgen05 kernels use, with
+    MEASURED_PEAKS.json's protocol (torch.matmul 8192^3, 2 N^3 flop: best of 10 = burst, then back to back for 4 s =
+    sustained, SM clock sampled under load).  FP16 is the type of every contraction here (kind::f16); BF16 repeats the
+    driver's own measurement on this box for comparison; TF32 is the type SURVEY 8(d) sized its target on."""
+    import torch
+    n = 8192
+    out = {"how": "torch.matmul 8192^3 (2 N^3 flop): best of 10 (burst), back to back for 4 s (sustained); CUDA events",
+           "gpu": torch.cuda.get_device_name(0)}
+    for name, dt, tf32 in (("fp16", torch.float16, False), ("bf16", torch.bfloat16, False), ("tf32", torch.float32, True)):
+        torch.backends.cuda.matmul.allow_tf32 = tf32
+        a = torch.randn(n, n, device="cuda", dtype=dt)
+        b = torch.randn(n, n, device="cuda", dtype=dt)
+        c = torch.empty(n, n, device="cuda", dtype=dt)
+        for _ in range(5):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            torch.matmul(a, b, out=c)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        sampler = ClockSampler(0)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0, reps = time.perf_counter(), 0
+        e0.record()
+        while time.perf_counter() - t0 < 4.0:
+            for _ in range(20):
+                torch.matmul(a, b, out=c)
+            reps += 20
+            torch.cuda.synchronize()
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        out[name] = {"tflops_burst": 2.0 * n ** 3 / (best * 1e-3) / 1e12,
+                     "tflops_sustained": 2.0 * n ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12, "clocks": clocks}
+        del a, b, c
+    torch.backends.cuda.matmul.allow_tf32 = False
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -245,7 +290,13 @@ def main():
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
                          "go in as shape descriptors and are rendered on the device (scatman_simulate_shapes; not cfg5)")
+    ap.add_argument("--measure-peaks", action="store_true",
+                    help="measure the FP16 / BF16 / TF32 GEMM peaks with MEASURED_PEAKS.json's protocol and print them (no bench)")
     args = ap.parse_args()
+    if args.measure_peaks:
+        if int(os.environ.get("RANK", "0")) == 0:
+            measure_peaks(args)
+        return
     if args.impl == "reference":
         run_reference(args)
         return

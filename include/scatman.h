@@ -15,7 +15,8 @@
  * Conventions common to every entry point
  *   - Pointers named d_* are DEVICE pointers (16-byte aligned), h_* are HOST pointers.
  *   - The caller owns every device buffer, including the workspace; the library allocates no
- *     device memory in the d_* entry points.  Inputs are never modified.
+ *     device memory in the d_* entry points (only scatman_simulate*_host keep a device arena in the
+ *     context).  Inputs are never modified.
  *   - All device work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream).  No host synchronisation happens unless stated.
  *   - Every function returns a scatman_status.  No exceptions, no abort, NO CPU FALLBACK: without a
@@ -91,6 +92,15 @@ typedef struct {
  * scatman_last_issued_blocks.  The contraction skips 16-y steps of a (slice, 128-x tile, 128-y group) unit whose
  * rho~ values are all zero and narrows every unit to the range of its non-empty 16-x blocks. */
 #define SCATMAN_FLAG_COUNT_ISSUED 2u
+/* Every scatman_simulate* entry point: reuse the phase tables of the previous call.  The q-map (a1) and the phase tables (a3;
+ * the window-corrected tables of the NUFFT route, the Ex / Ey tables of the separable route) depend only on the grid geometry,
+ * lambda and the detector ("once per detector / lambda"); they sit at the start of the workspace, at offsets that do not depend
+ * on the batch.  With this flag the caller PROMISES that the workspace (same pointer) has not been written since the previous
+ * scatman_simulate* call on this context, and that explicit q arrays (d_q, d_qx, d_qy: same pointers) still hold the same
+ * values.  The library checks that grid, voxel size, lambda, detector / q pointers, method and workspace pointer equal those of
+ * the previous call and rebuilds the tables whenever anything differs, so the flag never changes a result: outputs are
+ * bit-identical with and without it.  It saves the table kernels (cfg3, pixel route: 0.54 GB of tables per call). */
+#define SCATMAN_FLAG_REUSE_TABLES 4u
 
 /* Create / destroy a context on CUDA device `device`.  Fails with SCATMAN_UNSUPPORTED_DEVICE unless the
  * device is compute capability 10.x.  scatman_destroy(NULL) is SCATMAN_OK. */
@@ -109,9 +119,11 @@ int scatman_qmap(scatman_ctx *ctx, const scatman_detector *det, double lambda, d
 /* Step a0, orientation (Block 5; Fig. 6; R11): beam-frame grid = trilinear
  * resample (FP64 coordinates, zero outside) of the body-frame grid at r_body = R^T r_beam, same dims.
  * h_quat[b][4] = (w,x,y,z) unit quaternion, body -> beam; read on the host before return.
- * d_dn_out must not alias d_dn_in. */
+ * d_dn_out must not alias d_dn_in.  d_ws: scatman_orient_workspace_bytes(batch) bytes (rotation matrices and the
+ * bounding boxes of the non-vacuum voxels), 16-byte aligned, owned by the caller like every device buffer. */
+int scatman_orient_workspace_bytes(scatman_ctx *ctx, int32_t batch, size_t *bytes);
 int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *grid, const double *h_quat,
-                   int32_t batch, float *d_dn_out, void *cuda_stream);
+                   int32_t batch, void *d_ws, size_t ws_bytes, float *d_dn_out, void *cuda_stream);
 
 /* Step a2, column prefix (Eq. 6/8/9; north_star (2)): effective scattering strength
  * d_rho[b][iz][iy][ix][2] = f(dn_j) exp(i k dz sum_{l<j} dn_l) as FP32 (Re, Im), WITHOUT the dV factor.
@@ -141,7 +153,7 @@ int scatman_simulate_q(scatman_ctx *ctx, const float *d_dn, const scatman_grid *
  * d_qx[npx], d_qy[npy]: FP64 device arrays (any values, e.g. the DFT grid 2 pi m / (N dx)).  d_I[b][npy][npx].
  * opts: rho_mode; method AUTO / TENSOR = both GEMMs on tcgen05 tensor cores with the FP16x3 split (grids with nx > 1024
  * use the CUDA-core stages), SIMT_TABLE = FP32 CUDA-core GEMMs; SIMT_SINCOS is INVALID_ARGUMENT here; precision and
- * flags are ignored.  The workspace size depends on the method: pass the same opts to both calls. */
+ * flags other than SCATMAN_FLAG_REUSE_TABLES are ignored.  The workspace size depends on the method: pass the same opts to both calls. */
 int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
                                   const scatman_options *opts, size_t *bytes);
 int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
@@ -157,7 +169,7 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
  * aliasing error is < 1e-8 of sum |rho~| dV per pixel; all sums are FP64 (the uniform-grid values are stored FP32 for the
  * interpolation, a rounding relative to the local amplitude), so north_star's tolerances against the direct
  * sum hold (tests/test_gpu_nufft.py).  Work ~ N_vox * nqz + ... instead of N_vox * N_pix: ~1000x fewer multiply-adds.
- * opts: rho_mode only (method, precision, flags ignored).  d_I[b][npy][npx].  The workspace depends on lambda and the
+ * opts: rho_mode and SCATMAN_FLAG_REUSE_TABLES (method, precision, other flags ignored).  d_I[b][npy][npx].  The workspace depends on lambda and the
  * detector (they fix the q range): scatman_nufft_workspace_bytes with the same arguments. */
 int scatman_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
                                   int32_t batch, size_t *bytes);
@@ -168,13 +180,23 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
                            const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
                            void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream);
 
-/* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies h_dn to the device, runs
- * scatman_simulate on the context's own stream, copies I back into h_I and synchronises.  This entry
- * point alone owns device memory: a grow-only arena kept in the context until scatman_destroy.
- * h_dn and h_I should be pinned for full copy bandwidth (pageable memory works). */
+/* End to end with HOST buffers (bench.py's e2e leg), one entry point per route: h_dn[batch][nz][ny][nx][2] in, h_I out, both
+ * in host memory (pinned for full copy bandwidth and for the overlap below; pageable memory works, serially).  The batch is cut
+ * into chunks of ~256 MB of input; the upload of chunk c + 1, the kernels of chunk c and the download of chunk c - 1 run
+ * concurrently on three streams of the context, so for a batch of several chunks the call costs max(copy, compute) per chunk
+ * instead of their sum.  The phase tables are built once and reused by every chunk and by later calls with the same geometry.
+ * These entry points alone own device memory: a grow-only arena kept in the context until scatman_destroy.  They return
+ * after h_I is complete (synchronous).  h_quat[batch][4] or NULL; h_qx[npx], h_qy[npy] are host arrays.
+ * scatman_last_launch_count then counts the kernels of all chunks. */
 int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
                           const scatman_detector *det, const double *h_quat, int32_t batch,
                           const scatman_options *opts, float *h_I);
+int scatman_simulate_nufft_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
+                                const scatman_detector *det, const double *h_quat, int32_t batch,
+                                const scatman_options *opts, float *h_I);
+int scatman_simulate_qgrid_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
+                                const double *h_qx, int32_t npx, const double *h_qy, int32_t npy, const double *h_quat,
+                                int32_t batch, const scatman_options *opts, float *h_I);
 
 /* ---- Forward-fitting pieces (simulate, compare with the measured pattern, improve) -------
  * scatman_discrepancy: one number per simulated pattern instead of an image.  d_I[batch][npix] FP32 simulated patterns;

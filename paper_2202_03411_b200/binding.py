@@ -20,10 +20,12 @@ LOSS_L2_NORMALISED, LOSS_POISSON_DEVIANCE = 0, 1
 PRECISION_AUTO, PRECISION_FP16X3 = 0, 1
 FLAG_SINGLE_CTA = 1
 FLAG_COUNT_ISSUED = 2
+FLAG_REUSE_TABLES = 4
 
 EXPORTS = [
-    "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient",
+    "scatman_create", "scatman_destroy", "scatman_workspace_bytes", "scatman_qmap", "scatman_orient_workspace_bytes", "scatman_orient",
     "scatman_effective_strength", "scatman_simulate", "scatman_simulate_q", "scatman_simulate_host",
+    "scatman_simulate_nufft_host", "scatman_simulate_qgrid_host",
     "scatman_qgrid_workspace_bytes", "scatman_simulate_qgrid", "scatman_shapes_workspace_bytes", "scatman_simulate_shapes",
     "scatman_shapes_qgrid_workspace_bytes", "scatman_simulate_shapes_qgrid",
     "scatman_nufft_workspace_bytes", "scatman_nufft_grid_dims", "scatman_simulate_nufft",
@@ -82,7 +84,8 @@ def load_library() -> C.CDLL:
     L.scatman_destroy.argtypes = [vp]
     L.scatman_workspace_bytes.argtypes = [vp, C.POINTER(Grid), i64, i32, C.POINTER(Options), C.POINTER(C.c_size_t)]
     L.scatman_qmap.argtypes = [vp, C.POINTER(Detector), dbl, vp, vp]
-    L.scatman_orient.argtypes = [vp, vp, C.POINTER(Grid), C.POINTER(dbl), i32, vp, vp]
+    L.scatman_orient_workspace_bytes.argtypes = [vp, i32, C.POINTER(C.c_size_t)]
+    L.scatman_orient.argtypes = [vp, vp, C.POINTER(Grid), C.POINTER(dbl), i32, vp, C.c_size_t, vp, vp]
     L.scatman_effective_strength.argtypes = [vp, vp, C.POINTER(Grid), dbl, i32, i32, vp, vp]
     L.scatman_simulate.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                    C.POINTER(Options), vp, C.c_size_t, vp, vp]
@@ -90,6 +93,9 @@ def load_library() -> C.CDLL:
                                      C.POINTER(Options), vp, C.c_size_t, vp, vp]
     L.scatman_simulate_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
                                         C.POINTER(Options), vp]
+    L.scatman_simulate_nufft_host.argtypes = L.scatman_simulate_host.argtypes
+    L.scatman_simulate_qgrid_host.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(dbl), i32, C.POINTER(dbl), i32,
+                                              C.POINTER(dbl), i32, C.POINTER(Options), vp]
     L.scatman_nufft_workspace_bytes.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), i32, C.POINTER(C.c_size_t)]
     L.scatman_nufft_grid_dims.argtypes = [vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(i32)]
     L.scatman_simulate_nufft.argtypes = [vp, vp, C.POINTER(Grid), dbl, C.POINTER(Detector), C.POINTER(dbl), i32,
@@ -170,6 +176,19 @@ class Scatman:
         return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
 
     @staticmethod
+    def _empty(shape, dtype, device, stream):
+        """torch.empty allocated in the ORDER OF `stream`: the caching allocator hands out blocks that are free in the order
+        of the stream that is current at allocation time, so a buffer the library's kernels use on `stream` must be allocated
+        (and is then freed) under that stream, not under whatever stream happens to be current."""
+        import torch
+        if stream is None:
+            return torch.empty(shape, dtype=dtype, device=device)
+        if not isinstance(stream, torch.cuda.Stream):
+            stream = torch.cuda.ExternalStream(int(stream))
+        with torch.cuda.stream(stream):
+            return torch.empty(shape, dtype=dtype, device=device)
+
+    @staticmethod
     def _grid_of(dn, voxel) -> Grid:
         if dn.dim() == 4:
             nz, ny, nx, two = dn.shape
@@ -197,7 +216,7 @@ class Scatman:
 
     def qmap(self, npx: int, npy: int, theta_max_deg: float, lam: float, cx: float = 0.0, cy: float = 0.0, stream=None):
         import torch
-        q = torch.empty((npx * npy, 3), dtype=torch.float64, device=f"cuda:{self.device}")
+        q = self._empty((npx * npy, 3), torch.float64, f"cuda:{self.device}", stream)
         det = Detector(npx, npy, float(theta_max_deg), float(cx), float(cy))
         self._check(self.lib.scatman_qmap(self._ctx, C.byref(det), float(lam), C.c_void_p(q.data_ptr()), self._stream(stream)))
         return q
@@ -206,17 +225,20 @@ class Scatman:
         import torch
         self._check_dn(dn)
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
-        out = torch.empty_like(dn)
+        out = self._empty(tuple(dn.shape), dn.dtype, dn.device, stream)
+        need = C.c_size_t(0)
+        self._check(self.lib.scatman_orient_workspace_bytes(self._ctx, batch, C.byref(need)))
+        ws = self._empty(int(need.value), torch.uint8, dn.device, stream)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_orient(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), qp, batch,
-                                            C.c_void_p(out.data_ptr()), self._stream(stream)))
+                                            C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
     def effective_strength(self, dn, voxel, lam: float, rho_mode: int = RHO_LINEAR, stream=None):
         import torch
         self._check_dn(dn)
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
-        out = torch.empty_like(dn)
+        out = self._empty(tuple(dn.shape), dn.dtype, dn.device, stream)
         self._check(self.lib.scatman_effective_strength(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                         int(rho_mode), batch, C.c_void_p(out.data_ptr()),
                                                         self._stream(stream)))
@@ -268,7 +290,7 @@ class Scatman:
         grid = Grid(nx, ny, nz, float(voxel[0]), float(voxel[1]), float(voxel[2]))
         batch = len(shapes)
         if out is None:
-            out = torch.empty((batch, nz, ny, nx, 2), dtype=torch.float32, device=f"cuda:{self.device}")
+            out = self._empty((batch, nz, ny, nx, 2), torch.float32, f"cuda:{self.device}", stream)
         arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_render(self._ctx, arr, batch, C.byref(grid), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
@@ -284,9 +306,9 @@ class Scatman:
         opts = Options(int(rho_mode), int(method), 0, int(flags))
         need = self.workspace_bytes(grid, npx * npy, batch, opts)
         if workspace is None:
-            workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
+            workspace = self._empty(need, torch.uint8, dn.device, stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+            out = self._empty((batch, npy, npx), torch.float32, dn.device, stream)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                               C.byref(det), qp, batch, C.byref(opts), C.c_void_p(workspace.data_ptr()),
@@ -300,20 +322,21 @@ class Scatman:
         return int(nq[0]), int(nq[1]), int(nq[2])
 
     def simulate_nufft(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
-                       rho_mode: int = RHO_LINEAR, cx: float = 0.0, cy: float = 0.0, workspace=None, out=None, stream=None):
+                       rho_mode: int = RHO_LINEAR, cx: float = 0.0, cy: float = 0.0, workspace=None, out=None, stream=None,
+                       flags: int = 0):
         """Same result as simulate() by the 3-D type-2 NUFFT route (scatman_simulate_nufft).  Asynchronous."""
         import torch
         self._check_dn(dn)
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
-        opts = Options(int(rho_mode), 0, 0, 0)
+        opts = Options(int(rho_mode), 0, 0, int(flags))
         need = C.c_size_t(0)
         self._check(self.lib.scatman_nufft_workspace_bytes(self._ctx, C.byref(grid), float(lam), C.byref(det), batch,
                                                            C.byref(need)))
         if workspace is None:
-            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dn.device)
+            workspace = self._empty(int(need.value), torch.uint8, dn.device, stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+            out = self._empty((batch, npy, npx), torch.float32, dn.device, stream)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate_nufft(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                     C.byref(det), qp, batch, C.byref(opts), C.c_void_p(workspace.data_ptr()),
@@ -332,9 +355,9 @@ class Scatman:
         opts = Options(int(rho_mode), int(method), 0, int(flags))
         need = self.workspace_bytes(grid, npix, batch, opts)
         if workspace is None:
-            workspace = torch.empty(need, dtype=torch.uint8, device=dn.device)
+            workspace = self._empty(need, torch.uint8, dn.device, stream)
         if out is None:
-            out = torch.empty((batch, npix), dtype=torch.float32, device=dn.device)
+            out = self._empty((batch, npix), torch.float32, dn.device, stream)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate_q(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                 C.c_void_p(q.data_ptr()), npix, qp, batch, C.byref(opts),
@@ -356,9 +379,9 @@ class Scatman:
         self._check(self.lib.scatman_shapes_workspace_bytes(self._ctx, C.byref(grid), npx * npy, batch, C.byref(opts), C.byref(need)))
         dev = f"cuda:{self.device}"
         if workspace is None:
-            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dev)
+            workspace = self._empty(int(need.value), torch.uint8, dev, stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dev)
+            out = self._empty((batch, npy, npx), torch.float32, dev, stream)
         arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_simulate_shapes(self._ctx, arr, batch, C.byref(grid), float(lam), C.byref(det), C.byref(opts),
                                                      C.c_void_p(workspace.data_ptr()), workspace.numel(),
@@ -381,9 +404,9 @@ class Scatman:
         self._check(self.lib.scatman_shapes_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(opts),
                                                                   C.byref(need)))
         if workspace is None:
-            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=qx.device)
+            workspace = self._empty(int(need.value), torch.uint8, qx.device, stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=qx.device)
+            out = self._empty((batch, npy, npx), torch.float32, qx.device, stream)
         arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_simulate_shapes_qgrid(self._ctx, arr, batch, C.byref(grid), float(lam),
                                                            C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy,
@@ -405,9 +428,9 @@ class Scatman:
         self._check(self.lib.scatman_shapes_nufft_workspace_bytes(self._ctx, C.byref(grid), float(lam), C.byref(det), batch,
                                                                   C.byref(need)))
         if workspace is None:
-            workspace = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+            workspace = self._empty(int(need.value), torch.uint8, "cuda", stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device="cuda")
+            out = self._empty((batch, npy, npx), torch.float32, "cuda", stream)
         arr, keep = self._shape_array(shapes)
         self._check(self.lib.scatman_simulate_shapes_nufft(self._ctx, arr, batch, C.byref(grid), float(lam), C.byref(det),
                                                            C.byref(opts), C.c_void_p(workspace.data_ptr()), workspace.numel(),
@@ -415,7 +438,7 @@ class Scatman:
         return out
 
     def simulate_qgrid(self, dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO,
-                       workspace=None, out=None, stream=None):
+                       workspace=None, out=None, stream=None, flags: int = 0):
         """I float32 [B][npy][npx] on the tensor grid (qx[a], qy[b]) of transverse momentum transfers (CUDA float64 1-D
         tensors): the separable route (scatman_simulate_qgrid).  method: AUTO / TENSOR = both GEMM stages on tcgen05,
         SIMT_TABLE = FP32 CUDA cores."""
@@ -427,13 +450,13 @@ class Scatman:
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         npx, npy = int(qx.numel()), int(qy.numel())
         need = C.c_size_t(0)
-        opts = Options(int(rho_mode), int(method), 0, 0)
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
         self._check(self.lib.scatman_qgrid_workspace_bytes(self._ctx, C.byref(grid), npx, npy, batch, C.byref(opts),
                                                            C.byref(need)))
         if workspace is None:
-            workspace = torch.empty(int(need.value), dtype=torch.uint8, device=dn.device)
+            workspace = self._empty(int(need.value), torch.uint8, dn.device, stream)
         if out is None:
-            out = torch.empty((batch, npy, npx), dtype=torch.float32, device=dn.device)
+            out = self._empty((batch, npy, npx), torch.float32, dn.device, stream)
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate_qgrid(self._ctx, C.c_void_p(dn.data_ptr()), C.byref(grid), float(lam),
                                                     C.c_void_p(qx.data_ptr()), npx, C.c_void_p(qy.data_ptr()), npy, qp, batch,
@@ -441,11 +464,17 @@ class Scatman:
                                                     C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out if dn.dim() == 5 else out[0]
 
-    def _fit_ws(self, npix: int, batch: int, device):
+    def _fit_ws(self, npix: int, batch: int, device, stream):
+        """Workspace of the fit entry points, kept per (size, stream) so that a fitting loop allocates it once."""
         import torch
         need = C.c_size_t(0)
         self._check(self.lib.scatman_fit_workspace_bytes(self._ctx, npix, batch, C.byref(need)))
-        return torch.empty(int(need.value), dtype=torch.uint8, device=device)
+        key = (int(need.value), str(device), int(self._stream(stream).value or 0))
+        cache = self.__dict__.setdefault("_fit_ws_cache", {})
+        if key not in cache:
+            cache.clear()
+            cache[key] = self._empty(int(need.value), torch.uint8, device, stream)
+        return cache[key]
 
     def discrepancy(self, I, M, mask=None, metric: int = LOSS_L2_NORMALISED, out=None, stream=None):
         """float64 [B]: discrepancy of each simulated pattern I[B][...] (CUDA float32) against the measured pattern M (same
@@ -459,9 +488,9 @@ class Scatman:
         m_stride = 0 if M.numel() == npix else npix
         if mask is not None and not (mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous() and mask.numel() == npix):
             raise ValueError("mask must be a contiguous CUDA uint8 tensor with one byte per pixel")
-        ws = self._fit_ws(npix, batch, I.device)
+        ws = self._fit_ws(npix, batch, I.device, stream)
         if out is None:
-            out = torch.empty(batch, dtype=torch.float64, device=I.device)
+            out = self._empty(batch, torch.float64, I.device, stream)
         self._check(self.lib.scatman_discrepancy(self._ctx, C.c_void_p(I.data_ptr()), C.c_void_p(M.data_ptr()), m_stride,
                                                  C.c_void_p(mask.data_ptr()) if mask is not None else None, npix, batch,
                                                  int(metric), C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()),
@@ -477,9 +506,9 @@ class Scatman:
             raise ValueError("I must be a contiguous CUDA float32 tensor [B][...pixels]")
         batch, npix = int(I.shape[0]), int(I[0].numel())
         ph = np.ascontiguousarray(np.broadcast_to(np.asarray(n_photons, dtype=np.float64), (batch,)))
-        ws = self._fit_ws(npix, batch, I.device)
+        ws = self._fit_ws(npix, batch, I.device, stream)
         if out is None:
-            out = torch.empty_like(I)
+            out = self._empty(tuple(I.shape), I.dtype, I.device, stream)
         self._check(self.lib.scatman_ideal_detector(self._ctx, C.c_void_p(I.data_ptr()), npix, batch,
                                                     ph.ctypes.data_as(C.POINTER(C.c_double)), C.c_uint64(int(seed) & (2 ** 64 - 1)),
                                                     C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()),
@@ -500,6 +529,43 @@ class Scatman:
         keep, qp = _quat_arg(quat, batch)
         self._check(self.lib.scatman_simulate_host(self._ctx, C.c_void_p(h_dn.data_ptr()), C.byref(grid), float(lam),
                                                    C.byref(det), qp, batch, C.byref(opts), C.c_void_p(h_out.data_ptr())))
+        return h_out
+
+    def simulate_nufft_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
+                            rho_mode: int = RHO_LINEAR, h_out=None):
+        """scatman_simulate_nufft_host: host tensors in and out, upload / compute / download overlapped chunk by chunk."""
+        import torch
+        if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
+            raise ValueError("h_dn must be a contiguous CPU float32 tensor")
+        grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
+        opts = Options(int(rho_mode), 0, 0, 0)
+        if h_out is None:
+            h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_nufft_host(self._ctx, C.c_void_p(h_dn.data_ptr()), C.byref(grid), float(lam),
+                                                         C.byref(det), qp, batch, C.byref(opts), C.c_void_p(h_out.data_ptr())))
+        return h_out
+
+    def simulate_qgrid_host(self, h_dn, voxel, lam: float, qx, qy, quat=None, rho_mode: int = RHO_LINEAR,
+                            method: int = METHOD_AUTO, h_out=None):
+        """scatman_simulate_qgrid_host: host tensors in and out; qx, qy are host sequences / numpy arrays of float64."""
+        import numpy as np
+        import torch
+        if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
+            raise ValueError("h_dn must be a contiguous CPU float32 tensor")
+        grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
+        qx = np.ascontiguousarray(np.asarray(qx, dtype=np.float64))
+        qy = np.ascontiguousarray(np.asarray(qy, dtype=np.float64))
+        npx, npy = int(qx.size), int(qy.size)
+        opts = Options(int(rho_mode), int(method), 0, 0)
+        if h_out is None:
+            h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
+        keep, qp = _quat_arg(quat, batch)
+        self._check(self.lib.scatman_simulate_qgrid_host(self._ctx, C.c_void_p(h_dn.data_ptr()), C.byref(grid), float(lam),
+                                                         qx.ctypes.data_as(C.POINTER(C.c_double)), npx,
+                                                         qy.ctypes.data_as(C.POINTER(C.c_double)), npy, qp, batch, C.byref(opts),
+                                                         C.c_void_p(h_out.data_ptr())))
         return h_out
 
     def last_launch_count(self) -> int:

@@ -9,19 +9,44 @@
 
 using namespace scatman;
 
+// What a set of phase tables was built for.  Tables live in the CALLER's workspace, ahead of everything that depends on the
+// batch, so the key holds the workspace pointer and no batch size.
+struct TableKey {
+    int route = 0;                       // 1 pixel contraction, 2 separable q-grid, 3 NUFFT
+    int32_t nx = 0, ny = 0, nz = 0;
+    double dx = 0, dy = 0, dz = 0, lambda = 0;
+    int32_t npx = 0, npy = 0;
+    double theta = 0, cx = 0, cy = 0;
+    int64_t npix = 0;
+    int method = 0, ncta = 0;
+    const void *q0 = nullptr, *q1 = nullptr;   // explicit q arrays (scatman_simulate_q, scatman_simulate_qgrid)
+    const void *ws = nullptr;
+    bool operator==(const TableKey &o) const {
+        return route == o.route && nx == o.nx && ny == o.ny && nz == o.nz && dx == o.dx && dy == o.dy && dz == o.dz &&
+               lambda == o.lambda && npx == o.npx && npy == o.npy && theta == o.theta && cx == o.cx && cy == o.cy &&
+               npix == o.npix && method == o.method && ncta == o.ncta && q0 == o.q0 && q1 == o.q1 && ws == o.ws;
+    }
+};
+
 struct scatman_ctx {
     int device = 0;
     int num_sms = 0;
     std::string last_error;
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    bool ev_valid = false;
+    bool ev_valid = false, ev_capturing = false;
     const unsigned long long *d_count = nullptr;   // issued-block counter of the last call (in its workspace)
     cudaStream_t count_stream = nullptr;
-    // arena of scatman_simulate_host (grow-only)
-    cudaStream_t host_stream = nullptr;
+    // Phase tables of the last call (a1 q-map + a3 tables: functions of the detector, lambda and the grid geometry only,
+    // "cacheable" in SURVEY section 3): what they were built for and where.  SCATMAN_FLAG_REUSE_TABLES skips rebuilding them.
+    TableKey tables_key;
+    bool tables_valid = false;
+    // scatman_simulate*_host: device arena (grow-only) and the three streams / events of the copy-compute pipeline
+    cudaStream_t host_stream = nullptr, in_stream = nullptr, out_stream = nullptr;
+    cudaEvent_t in_ready[2] = {nullptr, nullptr}, in_free[2] = {nullptr, nullptr}, out_free[2] = {nullptr, nullptr};
     void *arena = nullptr;
     size_t arena_bytes = 0;
+    std::vector<double> host_q;   // qx | qy of the last scatman_simulate_qgrid_host (its tables are valid for these values only)
 };
 
 namespace scatman {
@@ -75,7 +100,14 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
     }
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = align_up(off + bytes, 1024); return o2; };
+    // the phase tables first: their offsets and sizes do not depend on the batch (SCATMAN_FLAG_REUSE_TABLES)
     p.off_q = take(sizeof(double) * 3 * (size_t)npix);
+    if (p.method == SCATMAN_METHOD_TENSOR) {
+        p.off_A = take(sizeof(__half) * 4 * (size_t)p.npix_pad * p.ny_pad);
+        p.off_anchor = take(sizeof(float2) * (size_t)p.ntiles * p.nxa * kTileP);
+        p.off_fine = take(sizeof(float2) * (size_t)p.ntiles * kFine * kTileP);
+        p.off_zturn = take(sizeof(unsigned long long) * (size_t)p.ntiles * kTileP);
+    }
     p.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
     p.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     p.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
@@ -85,10 +117,6 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
     p.off_partial = take(sizeof(float2) * (size_t)batch * p.nsplit * (size_t)p.npix_pad);
     if (p.method == SCATMAN_METHOD_TENSOR) {
         p.off_B = take(sizeof(__half) * 4 * (size_t)p.nx_pad * p.ny_pad * (size_t)p.nz * batch);
-        p.off_A = take(sizeof(__half) * 4 * (size_t)p.npix_pad * p.ny_pad);
-        p.off_anchor = take(sizeof(float2) * (size_t)p.ntiles * p.nxa * kTileP);
-        p.off_fine = take(sizeof(float2) * (size_t)p.ntiles * kFine * kTileP);
-        p.off_mz = take(sizeof(float2) * (size_t)p.ntiles * p.nz * kTileP);
         p.off_mask = take(sizeof(unsigned long long) * (size_t)batch * p.nz * p.nxt * p.ngroups);
         p.off_count = take(sizeof(unsigned long long));
     }
@@ -103,6 +131,21 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
 }
 
 }  // namespace scatman
+
+// The contraction's CUDA events are skipped while the stream is being captured into a graph (an event recorded in a capture
+// cannot be synchronised on or timed afterwards): scatman_last_contraction_ms then reports -1.
+static bool stream_capturing(cudaStream_t st) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
+    return cs != cudaStreamCaptureStatusNone;
+}
+static void ev_begin(scatman_ctx *ctx, cudaStream_t st) {
+    ctx->ev_capturing = stream_capturing(st);
+    if (!ctx->ev_capturing) cudaEventRecord(ctx->ev0, st);
+}
+static void ev_end(scatman_ctx *ctx, cudaStream_t st) {
+    if (!ctx->ev_capturing) { cudaEventRecord(ctx->ev1, st); ctx->ev_valid = true; }
+}
 
 static int fail(scatman_ctx *ctx, int status, const std::string &msg) {
     if (ctx) ctx->last_error = msg;
@@ -122,7 +165,7 @@ static bool valid_detector(const scatman_detector *d) {
 }
 static bool valid_options(const scatman_options &o) {
     return (o.rho_mode == SCATMAN_RHO_LINEAR || o.rho_mode == SCATMAN_RHO_N2M1) && o.method >= 0 && o.method <= 3 &&
-           o.precision >= 0 && o.precision <= 1 && (o.flags & ~(uint32_t)(SCATMAN_FLAG_SINGLE_CTA | SCATMAN_FLAG_COUNT_ISSUED)) == 0;
+           o.precision >= 0 && o.precision <= 1 && (o.flags & ~(uint32_t)(SCATMAN_FLAG_SINGLE_CTA | SCATMAN_FLAG_COUNT_ISSUED | SCATMAN_FLAG_REUSE_TABLES)) == 0;
 }
 static bool valid_quats(const double *q, int batch) {
     for (int b = 0; b < batch; ++b) {
@@ -165,7 +208,7 @@ static cudaError_t upload_rotmats(const double *h_quat, int batch, double *d_rot
 
 extern "C" {
 
-int scatman_version(void) { return 100; }
+int scatman_version(void) { return 200; }
 
 const char *scatman_status_string(int status) {
     switch (status) {
@@ -198,7 +241,8 @@ int scatman_create(scatman_ctx **out, int device) {
     ctx->device = device;
     ctx->num_sms = prop.multiProcessorCount;
     if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess ||
-        nufft_init_device() != cudaSuccess) {   // the NUFFT route's window polynomials -> constant memory of this device
+        nufft_init_device() != cudaSuccess ||   // the NUFFT route's window polynomials -> constant memory of this device
+        tensor_init_device() != cudaSuccess || sep_init_device() != cudaSuccess || sep_tc_init_device() != cudaSuccess) {
         delete ctx;
         return SCATMAN_CUDA_ERROR;
     }
@@ -211,6 +255,13 @@ int scatman_destroy(scatman_ctx *ctx) {
     cudaSetDevice(ctx->device);
     if (ctx->arena) cudaFree(ctx->arena);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->in_stream) cudaStreamDestroy(ctx->in_stream);
+    if (ctx->out_stream) cudaStreamDestroy(ctx->out_stream);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->in_ready[i]) cudaEventDestroy(ctx->in_ready[i]);
+        if (ctx->in_free[i]) cudaEventDestroy(ctx->in_free[i]);
+        if (ctx->out_free[i]) cudaEventDestroy(ctx->out_free[i]);
+    }
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
@@ -234,22 +285,30 @@ int scatman_qmap(scatman_ctx *ctx, const scatman_detector *det, double lambda, d
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "qmap");
 }
 
+int scatman_orient_workspace_bytes(scatman_ctx *ctx, int32_t batch, size_t *bytes) {
+    if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
+    if (batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    *bytes = scatman::align_up(sizeof(double) * 9 * (size_t)batch, 256) + sizeof(int) * 6 * (size_t)batch;   // matrices + boxes
+    return SCATMAN_OK;
+}
+
 int scatman_orient(scatman_ctx *ctx, const float *d_dn_in, const scatman_grid *grid, const double *h_quat,
-                   int32_t batch, float *d_dn_out, void *cuda_stream) {
-    if (!ctx || !d_dn_in || !d_dn_out || d_dn_in == d_dn_out || !valid_grid(grid) || !h_quat || batch < 1 ||
-        !valid_quats(h_quat, batch))
+                   int32_t batch, void *d_ws, size_t ws_bytes, float *d_dn_out, void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_dn_in || !d_dn_out || !d_ws || d_dn_in == d_dn_out || !valid_grid(grid) || !h_quat || batch < 1 ||
+        !valid_quats(h_quat, batch) || ((uintptr_t)d_ws & 15))
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    size_t need = 0;
+    scatman_orient_workspace_bytes(ctx, batch, &need);
+    if (ws_bytes < need) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     cudaSetDevice(ctx->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    // the rotation matrices travel in a small stream-ordered allocation
-    double *d_rot = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&d_rot, (sizeof(double) * 9 + sizeof(int) * 6) * batch, st);   // matrices + boxes
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "orient: cudaMallocAsync");
+    double *d_rot = (double *)d_ws;
+    int *d_bbox = (int *)((uint8_t *)d_ws + scatman::align_up(sizeof(double) * 9 * (size_t)batch, 256));
     Plan p;
     p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.dx = grid->dx; p.dy = grid->dy; p.dz = grid->dz;
-    e = upload_rotmats(h_quat, batch, d_rot, st, nullptr);
-    if (e == cudaSuccess) e = launch_orient(d_dn_in, p, d_rot, batch, d_dn_out, (int *)(d_rot + 9 * batch), st);
-    cudaFreeAsync(d_rot, st);
+    cudaError_t e = upload_rotmats(h_quat, batch, d_rot, st, nullptr);
+    if (e == cudaSuccess) e = launch_orient(d_dn_in, p, d_rot, batch, d_dn_out, d_bbox, st);
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "orient");
 }
 
@@ -275,14 +334,10 @@ int scatman_effective_strength(scatman_ctx *ctx, const float *d_dn, const scatma
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
     cudaSetDevice(ctx->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    unsigned *d_max = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&d_max, sizeof(unsigned) * batch, st);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "effective_strength: cudaMallocAsync");
     Plan p;
     p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.dx = grid->dx; p.dy = grid->dy; p.dz = grid->dz;
     p.lambda = lambda; p.rho_mode = rho_mode;
-    e = launch_strength(d_dn, p, batch, d_rho, d_max, st);
-    cudaFreeAsync(d_max, st);
+    cudaError_t e = launch_strength(d_dn, p, batch, d_rho, nullptr, st);   // no per-item maximum wanted: no scratch needed
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "effective_strength");
 }
 
@@ -311,12 +366,21 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
     ctx->ev_valid = false;
     ctx->d_count = nullptr;
 
+    TableKey key;
+    key.route = 1;
+    key.nx = grid->nx; key.ny = grid->ny; key.nz = grid->nz; key.dx = grid->dx; key.dy = grid->dy; key.dz = grid->dz;
+    key.lambda = lambda; key.npix = npix; key.method = p.method; key.ncta = p.t_ncta; key.q0 = d_q_in; key.ws = d_ws;
+    if (det) { key.npx = det->npx; key.npy = det->npy; key.theta = det->theta_max_deg; key.cx = det->cx; key.cy = det->cy; }
+    const bool reuse = (o.flags & SCATMAN_FLAG_REUSE_TABLES) && ctx->tables_valid && ctx->tables_key == key;
+    ctx->tables_valid = false;
     const double *d_q = d_q_in;
     if (!d_q) {
         double *q = (double *)(ws + p.off_q);
-        e = launch_qmap(*det, lambda, q, st);
-        ++nl;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+        if (!reuse) {
+            e = launch_qmap(*det, lambda, q, st);
+            ++nl;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+        }
         d_q = q;
     }
     const float *src = d_dn;
@@ -348,42 +412,43 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
             ctx->d_count = (const unsigned long long *)(ws + p.off_count);
             ctx->count_stream = st;
         }
-        e = launch_tables(d_q, p, (__half *)(ws + p.off_A), (float2 *)(ws + p.off_anchor), (float2 *)(ws + p.off_fine),
-                          (float2 *)(ws + p.off_mz), st, &nl);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "tables");
+        if (!reuse) {
+            e = launch_tables(d_q, p, (__half *)(ws + p.off_A), (float2 *)(ws + p.off_anchor), (float2 *)(ws + p.off_fine),
+                              (unsigned long long *)(ws + p.off_zturn), st, &nl);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "tables");
+        }
         TensorLaunch t;
         t.d_A = ws + p.off_A; t.d_B = ws + p.off_B;
         t.d_anchor = (const float2 *)(ws + p.off_anchor); t.d_fine = (const float2 *)(ws + p.off_fine);
-        t.d_mz = (const float2 *)(ws + p.off_mz); t.d_partial = partial;
+        t.d_zturn = (const unsigned long long *)(ws + p.off_zturn); t.d_partial = partial;
         t.d_mask = (const unsigned long long *)(ws + p.off_mask); t.num_sms = ctx->num_sms;
         std::string err;
-        cudaEventRecord(ctx->ev0, st);
+        ev_begin(ctx, st);
         e = launch_tensor(p, t, st, &err);
-        cudaEventRecord(ctx->ev1, st);
         ++nl;
         if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "contract") : fail(ctx, SCATMAN_CUDA_ERROR, err);
-        ctx->ev_valid = true;
+        ev_end(ctx, st);
         e = launch_finalize(partial, p, ampscale, dV, d_I, st);
     } else if (p.method == SCATMAN_METHOD_SIMT_TABLE) {
-        cudaEventRecord(ctx->ev0, st);
+        ev_begin(ctx, st);
         e = launch_simt_table(rho, d_q, p, (float2 *)(ws + p.off_tab_y), (float2 *)(ws + p.off_tab_x), (float2 *)(ws + p.off_tab_z),
                               ws + p.off_flags, partial, st, &nl);
-        cudaEventRecord(ctx->ev1, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "simt_table");
-        ctx->ev_valid = true;
+        ev_end(ctx, st);
         e = launch_finalize(partial, p, nullptr, dV, d_I, st);
     } else {
-        cudaEventRecord(ctx->ev0, st);
+        ev_begin(ctx, st);
         e = launch_simt_sincos(rho, d_q, p, partial, st);
-        cudaEventRecord(ctx->ev1, st);
         ++nl;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "simt_sincos");
-        ctx->ev_valid = true;
+        ev_end(ctx, st);
         e = launch_finalize(partial, p, nullptr, dV, d_I, st);
     }
     ++nl;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "finalize");
     ctx->last_launches = nl;
+    ctx->tables_key = key;
+    ctx->tables_valid = true;
     return SCATMAN_OK;
 }
 
@@ -454,6 +519,14 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     if (sp.tensor) sp.tc = make_sep_tc_plan(p, npx, npy, num_sms);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
+    // the phase tables first: their offsets and sizes do not depend on the batch (SCATMAN_FLAG_REUSE_TABLES)
+    if (sp.tensor) {
+        sp.off_eyp = take(sizeof(__half) * 4 * (size_t)sp.tc.NPYP * sp.tc.NY);
+        sp.off_exp = take(sizeof(__half) * 4 * (size_t)sp.tc.NPXP * sp.tc.NXP);
+    } else {
+        sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
+        sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
+    }
     sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
     sp.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
@@ -461,8 +534,6 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
-        sp.off_eyp = take(sizeof(__half) * 4 * (size_t)t.NPYP * t.NY);
-        sp.off_exp = take(sizeof(__half) * 4 * (size_t)t.NPXP * t.NXP);
         sp.off_rp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NY * t.NXP);
         sp.off_hp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NPXP * t.NY);
         sp.off_flags = take((size_t)t.nb * g.nz * (t.NY / 64));
@@ -470,8 +541,6 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
         sp.off_bounds = take(sizeof(int) * (size_t)((t.nsx + 1) + (size_t)t.nb * t.ng * (t.nzs + 1)));
         sp.off_partial = take(sizeof(float2) * (size_t)t.nb * t.nsplit * npx * npy);
     } else {
-        sp.off_ex = take(sizeof(float2) * (size_t)g.nx * npx);
-        sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
         sp.off_h = take(sizeof(float2) * (size_t)g.nz * g.ny * npx);
         sp.off_flags = take((size_t)g.nz * ((g.ny + 15) / 16));
         sp.off_partial = take(sizeof(float2) * (size_t)sp.nzs * npx * npy);
@@ -516,6 +585,12 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     cudaError_t e = cudaSuccess;
     ctx->ev_valid = false;
     ctx->d_count = nullptr;
+    TableKey key;
+    key.route = 2;
+    key.nx = grid->nx; key.ny = grid->ny; key.nz = grid->nz; key.dx = grid->dx; key.dy = grid->dy; key.dz = grid->dz;
+    key.lambda = lambda; key.npx = npx; key.npy = npy; key.method = sp.tensor ? 1 : 3; key.q0 = d_qx; key.q1 = d_qy; key.ws = d_ws;
+    const bool reuse = (o.flags & SCATMAN_FLAG_REUSE_TABLES) && ctx->tables_valid && ctx->tables_key == key;
+    ctx->tables_valid = false;
     const float *src = d_dn;
     if (h_quat && !all_identity(h_quat, batch)) {
         double *rm = (double *)(ws + sp.off_rotmat);
@@ -536,10 +611,12 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
                *Hp = (__half *)(ws + sp.off_hp);
         float *ampscale = (float *)(ws + sp.off_scale);
         int *bounds = (int *)(ws + sp.off_bounds);
-        e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, Exp, Eyp, st);
-        nl += 2;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
-        cudaEventRecord(ctx->ev0, st);
+        if (!reuse) {
+            e = launch_sep_tc_tables(d_qx, npx, d_qy, npy, p, t, Exp, Eyp, st);
+            nl += 2;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
+        }
+        ev_begin(ctx, st);
         for (int b0 = 0; b0 < batch; b0 += t.nb) {   // a chunk of items per set of launches, stacked along z
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
             const float2 *rho_b = (const float2 *)rho + (size_t)b0 * p.nvox;
@@ -557,10 +634,12 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         }
     } else {
         float2 *Ex = (float2 *)(ws + sp.off_ex), *Ey = (float2 *)(ws + sp.off_ey);
-        e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
-        nl += 2;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
-        cudaEventRecord(ctx->ev0, st);
+        if (!reuse) {
+            e = launch_sep_tables(d_qx, npx, d_qy, npy, p, Ex, Ey, st);
+            nl += 2;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid tables");
+        }
+        ev_begin(ctx, st);
         for (int b = 0; b < batch; ++b) {
             e = launch_sep_item((const float2 *)rho + (size_t)b * p.nvox, p, Ex, Ey, d_qx, npx, d_qy, npy, sp.nzs,
                                 (float2 *)(ws + sp.off_h), ws + sp.off_flags, (float2 *)(ws + sp.off_partial),
@@ -569,9 +648,10 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
             if (e != cudaSuccess) return cuda_fail(ctx, e, "qgrid stages");
         }
     }
-    cudaEventRecord(ctx->ev1, st);
-    ctx->ev_valid = true;
+    ev_end(ctx, st);
     ctx->last_launches = nl;
+    ctx->tables_key = key;
+    ctx->tables_valid = true;
     return SCATMAN_OK;
 }
 
@@ -664,15 +744,16 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
     }
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
+    // q-map and window-corrected tables first: independent of the batch (SCATMAN_FLAG_REUSE_TABLES)
+    L.off_q = take(sizeof(double) * 3 * (size_t)p.npix);
+    L.off_tz = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz);
+    L.off_tx = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx);
+    L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
     L.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
     L.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     L.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     L.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     L.off_max = take(sizeof(unsigned) * (size_t)batch);
-    L.off_q = take(sizeof(double) * 3 * (size_t)p.npix);
-    L.off_tz = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz);
-    L.off_tx = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx);
-    L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
     L.off_P = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx);
     L.off_H = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq);
     L.off_U = take(sizeof(float2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
@@ -719,10 +800,20 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     int nl = 0;
     ctx->ev_valid = false;
     ctx->d_count = nullptr;
+    TableKey key;
+    key.route = 3;
+    key.nx = grid->nx; key.ny = grid->ny; key.nz = grid->nz; key.dx = grid->dx; key.dy = grid->dy; key.dz = grid->dz;
+    key.lambda = lambda; key.npx = det->npx; key.npy = det->npy; key.theta = det->theta_max_deg; key.cx = det->cx; key.cy = det->cy;
+    key.ws = d_ws;
+    const bool reuse = (o.flags & SCATMAN_FLAG_REUSE_TABLES) && ctx->tables_valid && ctx->tables_key == key;
+    ctx->tables_valid = false;
     double *q = (double *)(ws + L.off_q);
-    cudaError_t e = launch_qmap(*det, lambda, q, st);
-    ++nl;
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+    cudaError_t e = cudaSuccess;
+    if (!reuse) {
+        e = launch_qmap(*det, lambda, q, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
+    }
     const float *src = d_dn;
     if (h_quat && !all_identity(h_quat, batch)) {
         double *rm = (double *)(ws + L.off_rotmat);
@@ -737,10 +828,12 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     ++nl;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
     double2 *Tz = (double2 *)(ws + L.off_tz), *TxT = (double2 *)(ws + L.off_tx), *Ty = (double2 *)(ws + L.off_ty);
-    e = launch_nufft_tables(p, L.n, Tz, TxT, Ty, st);
-    nl += 3;
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
-    cudaEventRecord(ctx->ev0, st);
+    if (!reuse) {
+        e = launch_nufft_tables(p, L.n, Tz, TxT, Ty, st);
+        nl += 3;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
+    }
+    ev_begin(ctx, st);
     for (int b0 = 0; b0 < batch; b0 += L.n.nb) {   // a chunk of items per set of launches
         const int nb = batch - b0 < L.n.nb ? batch - b0 : L.n.nb;
         e = launch_nufft_chunk((const float2 *)rho + (size_t)b0 * p.nvox, p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, Tz, TxT, Ty,
@@ -749,9 +842,10 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         nl += 4;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");
     }
-    cudaEventRecord(ctx->ev1, st);
-    ctx->ev_valid = true;
+    ev_end(ctx, st);
     ctx->last_launches = nl;
+    ctx->tables_key = key;
+    ctx->tables_valid = true;
     return SCATMAN_OK;
 }
 
@@ -820,42 +914,173 @@ int scatman_ideal_detector(scatman_ctx *ctx, const float *d_I, int64_t npix, int
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "ideal detector");
 }
 
+}  // extern "C"
+
+// ---- host-buffer entry points: copy / compute pipeline ----------------------------------------------------------------
+// The batch is cut into chunks; chunk c + 1 is uploaded on `in_stream` while chunk c computes on `host_stream` and the
+// patterns of chunk c - 1 go back on `out_stream` (two input and two output buffers in the context's arena, one workspace:
+// compute is serial).  Phase tables are built by the first chunk and reused by the others and by later calls with the same
+// geometry (the arena belongs to the context, so nobody else can have touched them).
+static int host_prepare(scatman_ctx *ctx) {
+    if (ctx->host_stream) return SCATMAN_OK;
+    cudaError_t e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->in_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->out_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&ctx->in_ready[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->in_free[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->out_free[i], cudaEventDisableTiming);
+    }
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "host pipeline setup");
+}
+
+static int host_chunk_items(size_t in_item_bytes, int batch) {
+    // ~256 MB of input per chunk; a batch worth overlapping (>= 16 MB) is cut into at least two chunks
+    size_t n = ((size_t)256 << 20) / (in_item_bytes ? in_item_bytes : 1);
+    if (n < 1) n = 1;
+    if (n > (size_t)batch) n = (size_t)batch;
+    if (batch >= 2 && n == (size_t)batch && in_item_bytes * (size_t)batch >= ((size_t)16 << 20)) n = ((size_t)batch + 1) / 2;
+    return (int)n;
+}
+
+// run(d_dn, b0, nb, d_ws, d_I, stream): enqueue the simulation of items [b0, b0 + nb) on `stream`
+template <class Run>
+static int host_pipeline(scatman_ctx *ctx, const float *h_dn, size_t in_item_bytes, float *h_I, size_t out_item_bytes, int batch,
+                         int chunk, size_t ws_bytes, const void *h_extra, size_t extra_bytes, void **d_extra_out, Run run) {
+    int rc = host_prepare(ctx);
+    if (rc != SCATMAN_OK) return rc;
+    const size_t ws_b = scatman::align_up(ws_bytes, 1024), ex_b = scatman::align_up(extra_bytes, 1024);
+    const size_t in_b = scatman::align_up(in_item_bytes * (size_t)chunk, 1024), out_b = scatman::align_up(out_item_bytes * (size_t)chunk, 1024);
+    const size_t need = ws_b + ex_b + 2 * in_b + 2 * out_b;
+    cudaError_t e;
+    if (need > ctx->arena_bytes) {
+        if (ctx->arena) cudaFree(ctx->arena);
+        ctx->arena = nullptr;
+        ctx->arena_bytes = 0;
+        ctx->tables_valid = false;
+        if ((e = cudaMalloc(&ctx->arena, need)) != cudaSuccess) return cuda_fail(ctx, e, "arena cudaMalloc");
+        ctx->arena_bytes = need;
+    }
+    uint8_t *a = (uint8_t *)ctx->arena;
+    void *d_ws = a;
+    uint8_t *d_extra = a + ws_b;
+    uint8_t *d_in[2] = {a + ws_b + ex_b, a + ws_b + ex_b + in_b};
+    uint8_t *d_out[2] = {a + ws_b + ex_b + 2 * in_b, a + ws_b + ex_b + 2 * in_b + out_b};
+    if (d_extra_out) *d_extra_out = d_extra;
+    if (extra_bytes && (e = cudaMemcpyAsync(d_extra, h_extra, extra_bytes, cudaMemcpyHostToDevice, ctx->in_stream)) != cudaSuccess)
+        return cuda_fail(ctx, e, "H2D");
+    int launches = 0;
+    rc = SCATMAN_OK;
+    e = cudaSuccess;
+    for (int c = 0, b0 = 0; b0 < batch && rc == SCATMAN_OK && e == cudaSuccess; ++c, b0 += chunk) {
+        const int nb = batch - b0 < chunk ? batch - b0 : chunk, buf = c & 1;
+        if (c >= 2) e = cudaStreamWaitEvent(ctx->in_stream, ctx->in_free[buf], 0);      // the compute that read this buffer is done
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(d_in[buf], (const uint8_t *)h_dn + (size_t)b0 * in_item_bytes, (size_t)nb * in_item_bytes,
+                                cudaMemcpyHostToDevice, ctx->in_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->in_ready[buf], ctx->in_stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->host_stream, ctx->in_ready[buf], 0);
+        if (e == cudaSuccess && c >= 2) e = cudaStreamWaitEvent(ctx->host_stream, ctx->out_free[buf], 0);   // its patterns have left
+        if (e != cudaSuccess) break;
+        rc = run((const float *)d_in[buf], b0, nb, d_ws, (float *)d_out[buf], ctx->host_stream);
+        if (rc != SCATMAN_OK) break;
+        launches += ctx->last_launches;
+        e = cudaEventRecord(ctx->in_free[buf], ctx->host_stream);                       // input consumed = patterns ready
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->out_stream, ctx->in_free[buf], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync((uint8_t *)h_I + (size_t)b0 * out_item_bytes, d_out[buf], (size_t)nb * out_item_bytes,
+                                cudaMemcpyDeviceToHost, ctx->out_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->out_free[buf], ctx->out_stream);
+    }
+    // nothing of this call is left in flight when it returns, whatever happened
+    cudaError_t e1 = cudaStreamSynchronize(ctx->in_stream), e2 = cudaStreamSynchronize(ctx->host_stream),
+                e3 = cudaStreamSynchronize(ctx->out_stream);
+    if (rc != SCATMAN_OK) return rc;
+    if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : e2 != cudaSuccess ? e2 : e3;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "host pipeline");
+    ctx->last_launches = launches;
+    return SCATMAN_OK;
+}
+
+extern "C" {
+
 int scatman_simulate_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
                           float *h_I) {
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
-    if (!h_dn || !h_I || !valid_grid(grid) || !valid_detector(det) || batch < 1 || !valid_options(o) || !(lambda > 0.0))
+    if (!h_dn || !h_I || !valid_grid(grid) || !valid_detector(det) || batch < 1 || batch > 65535 || !valid_options(o) || !(lambda > 0.0))
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
     cudaSetDevice(ctx->device);
-    cudaError_t e;
-    if (!ctx->host_stream && (e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
-        return cuda_fail(ctx, e, "stream create");
+    o.flags |= SCATMAN_FLAG_REUSE_TABLES;
     const int64_t npix = (int64_t)det->npx * det->npy;
-    const Plan p = make_plan(*grid, lambda, npix, batch, o, ctx->num_sms);
-    const size_t dn_bytes = (sizeof(float) * 2 * (size_t)p.nvox * batch + 1023) / 1024 * 1024;
-    const size_t I_bytes = (sizeof(float) * (size_t)npix * batch + 1023) / 1024 * 1024;
-    const size_t need = dn_bytes + I_bytes + p.total;
-    if (need > ctx->arena_bytes) {
-        if (ctx->arena) cudaFree(ctx->arena);
-        ctx->arena = nullptr;
-        ctx->arena_bytes = 0;
-        if ((e = cudaMalloc(&ctx->arena, need)) != cudaSuccess) return cuda_fail(ctx, e, "arena cudaMalloc");
-        ctx->arena_bytes = need;
+    const size_t in_item = sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz, out_item = sizeof(float) * (size_t)npix;
+    const int chunk = host_chunk_items(in_item, batch);
+    size_t ws_bytes = make_plan(*grid, lambda, npix, chunk, o, ctx->num_sms).total;
+    if (batch % chunk) {
+        const size_t last = make_plan(*grid, lambda, npix, batch % chunk, o, ctx->num_sms).total;
+        ws_bytes = last > ws_bytes ? last : ws_bytes;
     }
-    uint8_t *a = (uint8_t *)ctx->arena;
-    float *d_dn = (float *)a;
-    float *d_I = (float *)(a + dn_bytes);
-    void *d_ws = a + dn_bytes + I_bytes;
-    cudaStream_t st = ctx->host_stream;
-    if ((e = cudaMemcpyAsync(d_dn, h_dn, sizeof(float) * 2 * (size_t)p.nvox * batch, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-        return cuda_fail(ctx, e, "H2D");
-    int rc = run_path(ctx, d_dn, grid, lambda, det, nullptr, npix, h_quat, batch, &o, d_ws, p.total, d_I, st);
-    if (rc != SCATMAN_OK) return rc;
-    if ((e = cudaMemcpyAsync(h_I, d_I, sizeof(float) * (size_t)npix * batch, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-        return cuda_fail(ctx, e, "D2H");
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "synchronize");
-    return SCATMAN_OK;
+    return host_pipeline(ctx, h_dn, in_item, h_I, out_item, batch, chunk, ws_bytes, nullptr, 0, nullptr,
+                         [&](const float *d_dn, int b0, int nb, void *d_ws, float *d_I, cudaStream_t st) {
+                             return run_path(ctx, d_dn, grid, lambda, det, nullptr, npix, h_quat ? h_quat + 4 * (size_t)b0 : nullptr, nb,
+                                             &o, d_ws, ws_bytes, d_I, st);
+                         });
+}
+
+int scatman_simulate_nufft_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda,
+                                const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                                float *h_I) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!h_dn || !h_I || !valid_grid(grid) || !valid_detector(det) || batch < 1 || batch > 65535 || !(lambda > 0.0) ||
+        !std::isfinite(lambda) || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    o.flags |= SCATMAN_FLAG_REUSE_TABLES;
+    const int64_t npix = (int64_t)det->npx * det->npy;
+    const size_t in_item = sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz, out_item = sizeof(float) * (size_t)npix;
+    const int chunk = host_chunk_items(in_item, batch);
+    size_t ws_bytes = make_nufft_layout(*grid, lambda, *det, chunk, o.rho_mode).total;   // grows with the batch
+    return host_pipeline(ctx, h_dn, in_item, h_I, out_item, batch, chunk, ws_bytes, nullptr, 0, nullptr,
+                         [&](const float *d_dn, int b0, int nb, void *d_ws, float *d_I, cudaStream_t st) {
+                             return scatman_simulate_nufft(ctx, d_dn, grid, lambda, det, h_quat ? h_quat + 4 * (size_t)b0 : nullptr, nb, &o,
+                                                           d_ws, ws_bytes, d_I, (void *)st);
+                         });
+}
+
+int scatman_simulate_qgrid_host(scatman_ctx *ctx, const float *h_dn, const scatman_grid *grid, double lambda, const double *h_qx,
+                                int32_t npx, const double *h_qy, int32_t npy, const double *h_quat, int32_t batch,
+                                const scatman_options *opts, float *h_I) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
+    if (!h_dn || !h_I || !h_qx || !h_qy || !valid_grid(grid) || npx < 1 || npy < 1 || batch < 1 || batch > 65535 || !(lambda > 0.0) ||
+        !std::isfinite(lambda) || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1) || !valid_qgrid_method(o.method))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    cudaSetDevice(ctx->device);
+    // the q arrays come from the host on every call: the tables are reused only if their VALUES are those of the last call
+    std::vector<double> qv((size_t)npx + npy);
+    std::memcpy(qv.data(), h_qx, sizeof(double) * npx);
+    std::memcpy(qv.data() + npx, h_qy, sizeof(double) * npy);
+    if (qv != ctx->host_q) ctx->tables_valid = false;
+    o.flags |= SCATMAN_FLAG_REUSE_TABLES;
+    const size_t in_item = sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz, out_item = sizeof(float) * (size_t)npx * npy;
+    const int chunk = host_chunk_items(in_item, batch);
+    size_t ws_bytes = make_sep_plan(*grid, lambda, npx, npy, chunk, o.rho_mode, o.method, ctx->num_sms).total;
+    if (batch % chunk) {
+        const size_t last = make_sep_plan(*grid, lambda, npx, npy, batch % chunk, o.rho_mode, o.method, ctx->num_sms).total;
+        ws_bytes = last > ws_bytes ? last : ws_bytes;
+    }
+    void *d_q = nullptr;
+    const int rc = host_pipeline(ctx, h_dn, in_item, h_I, out_item, batch, chunk, ws_bytes, qv.data(), sizeof(double) * qv.size(), &d_q,
+                                 [&](const float *d_dn, int b0, int nb, void *d_ws, float *d_I, cudaStream_t st) {
+                                     const double *d_qx = (const double *)d_q, *d_qy = d_qx + npx;
+                                     return scatman_simulate_qgrid(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy,
+                                                                   h_quat ? h_quat + 4 * (size_t)b0 : nullptr, nb, &o, d_ws, ws_bytes, d_I,
+                                                                   (void *)st);
+                                 });
+    if (rc == SCATMAN_OK) ctx->host_q.swap(qv); else ctx->host_q.clear();
+    return rc;
 }
 
 int scatman_last_launch_count(scatman_ctx *ctx, int32_t *count) {

@@ -196,6 +196,13 @@ __global__ void __launch_bounds__(kFitThreads) ideal_detector_kernel(const float
     counts[(size_t)b * npix + p] = (float)n;
 }
 
+struct PhotonChunk {
+    double v[256];
+};
+__global__ void store_photons_kernel(PhotonChunk c, int n, double *__restrict__ dst) {
+    if ((int)threadIdx.x < n) dst[threadIdx.x] = c.v[threadIdx.x];
+}
+
 // ------------------------------------------------------------------------------------------------ host
 int fit_nchunk(int64_t npix) { return (int)((npix + kFitChunk - 1) / kFitChunk); }
 
@@ -231,8 +238,13 @@ cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, con
     const int nchunk = fit_nchunk(npix);
     double *sums = d_ws + (size_t)batch * nchunk * 5;
     double *photons = sums + (size_t)batch * 5 + (size_t)batch * nchunk;
-    e = cudaMemcpyAsync(photons, h_photons, sizeof(double) * batch, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return e;
+    // the photon numbers travel as kernel arguments (read from h_photons before return whatever memory it is; capturable)
+    for (int b0 = 0; b0 < batch; b0 += 256) {
+        PhotonChunk c;
+        const int n = batch - b0 < 256 ? batch - b0 : 256;
+        for (int i = 0; i < n; ++i) c.v[i] = h_photons[b0 + i];
+        store_photons_kernel<<<1, 256, 0, st>>>(c, n, photons + b0);
+    }
     ideal_detector_kernel<<<dim3((unsigned)((npix + kFitThreads - 1) / kFitThreads), batch), kFitThreads, 0, st>>>(
         d_I, npix, sums, photons, seed, d_counts);
     return cudaGetLastError();

@@ -40,7 +40,7 @@ struct Plan {
     int t_ncta = 2;               // CTAs per work item: 2 = cta_group::2 pairs (default), 1 = single CTA
     // workspace offsets (bytes)
     size_t off_q = 0, off_rotmat = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ampscale = 0, off_B = 0,
-           off_A = 0, off_anchor = 0, off_fine = 0, off_mz = 0, off_partial = 0, off_mask = 0, off_count = 0, off_bbox = 0, off_tab_y = 0, off_tab_x = 0, off_tab_z = 0, off_flags = 0, total = 0;
+           off_A = 0, off_anchor = 0, off_fine = 0, off_zturn = 0, off_partial = 0, off_mask = 0, off_count = 0, off_bbox = 0, off_tab_y = 0, off_tab_x = 0, off_tab_z = 0, off_flags = 0, total = 0;
 };
 
 int simt_zsplit(const Plan &p, int num_sms);
@@ -57,7 +57,7 @@ cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_m
 cudaError_t launch_count_issued(const unsigned long long *d_mask, const Plan &p, unsigned long long *d_count,
                                 cudaStream_t st);
 cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
-                          float2 *d_mz, cudaStream_t st, int *nlaunch);
+                          unsigned long long *d_zturn, cudaStream_t st, int *nlaunch);
 cudaError_t launch_finalize(const float2 *d_partial, const Plan &p, const float *d_ampscale, double dV,
                             float *d_I, cudaStream_t st);
 cudaError_t launch_simt_sincos(const float *d_rho, const double *d_q, const Plan &p, float2 *d_partial,
@@ -103,6 +103,10 @@ constexpr int kNufftW = 10;                     // Kaiser-Bessel window width in
 struct NufftAxis { int m_lo = 0, nq = 0; double inv_h = 0; };   // uniform grid g_m = (m_lo + m) h, m = 0..nq-1; inv_h = 1 / h
 struct NufftPlan { NufftAxis ax, ay, az; int nb = 1; double pixel_cells = 0; };   // nb = batch items per chunk
 cudaError_t nufft_init_device();   // once per device (scatman_create): uploads the window's piecewise polynomials
+// per-device kernel attributes (dynamic shared memory limits) of the other translation units; called by scatman_create
+cudaError_t tensor_init_device();
+cudaError_t sep_init_device();
+cudaError_t sep_tc_init_device();
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st);
 cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
@@ -120,7 +124,8 @@ struct TensorMaps;  // opaque here
 struct TensorLaunch {
     const void *d_A;      // fp16 [4][npix_pad][ny_pad]
     const void *d_B;      // fp16 [batch][nz][4][nx_pad][ny_pad]
-    const float2 *d_anchor, *d_fine, *d_mz;
+    const float2 *d_anchor, *d_fine;
+    const unsigned long long *d_zturn;   // [tile][128] slice-phase turn fractions
     const unsigned long long *d_mask;  // occupancy [batch][nz][nxt][ngroups], bit 8*yi + xi: 16-y x 16-x block is non-zero
     float2 *d_partial;
     int num_sms;

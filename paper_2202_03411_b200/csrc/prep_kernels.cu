@@ -207,14 +207,16 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
     if (threadIdx.x == 0) {
         float m = 0.f;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmaxf(m, wmax[w]);
-        if (m > 0.f) atomicMax(maxbits + b, __float_as_uint(m));
+        if (m > 0.f && maxbits) atomicMax(maxbits + b, __float_as_uint(m));
     }
 }
 
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
                             cudaStream_t st) {
-    cudaError_t e = cudaMemsetAsync(d_maxbits, 0, sizeof(unsigned) * batch, st);
-    if (e != cudaSuccess) return e;
+    if (d_maxbits) {   // nullptr: the caller does not want the per-item maximum (scatman_effective_strength)
+        cudaError_t e = cudaMemsetAsync(d_maxbits, 0, sizeof(unsigned) * batch, st);
+        if (e != cudaSuccess) return e;
+    }
     const int threads = p.nx >= 128 ? 128 : 64;
     dim3 grid((p.nx + threads - 1) / threads, p.ny, batch);
     const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
@@ -341,7 +343,8 @@ cudaError_t launch_count_issued(const unsigned long long *d_mask, const Plan &p,
 //   A planes  fp16 [4][npix_pad][ny_pad]  = split(2^10 e^{i qy(p) y_i})   (the UMMA A operand)
 //   anchor    float2 [tile][nxa][128]     = e^{i qx(p) x_{16 a}}
 //   fine      float2 [tile][16][128]      = e^{i qx(p) b dx}
-//   mz        float2 [tile][nz][128]      = e^{i qz(p) z_j}
+//   zturn     uint64 [tile][128]          = frac(qz(p) dz / 4 pi) as a 64-bit fixed-point fraction of a turn: the slice phase
+//                                           e^{i qz z_j} is formed in the contraction's epilogue from it (no per-slice table)
 // One thread = one pixel x 16 consecutive coordinates: FP64 sincos of the first phase and of the step, then the
 // angle-addition recurrence in FP64 (15 complex products; the rounding it adds is ~1e-15, far below the FP32 / FP16-pair
 // storage) -- an FP64 sincos per entry made these kernels FP64-throughput-bound.
@@ -389,22 +392,35 @@ __global__ void table_a_kernel(const double *__restrict__ q, int64_t npix, int64
     }
 }
 
-// anchor, fine and mz in ONE launch: blockIdx.y ranges [0, ya) anchor runs, [ya, ya + 1) fine, the rest mz runs
-__global__ void table_small_all_kernel(const double *__restrict__ q, int64_t npix, int nxa, int nx, double dx, int nz, double dz,
-                                       int ya, float2 *__restrict__ anchor, float2 *__restrict__ fine, float2 *__restrict__ mz) {
+// anchor, fine and the slice-phase turn fraction in ONE launch: blockIdx.y ranges [0, ya) anchor runs, ya = fine, ya + 1 = zturn
+__global__ void table_small_all_kernel(const double *__restrict__ q, int64_t npix, int nxa, int nx, double dx, double dz,
+                                       int ya, float2 *__restrict__ anchor, float2 *__restrict__ fine,
+                                       unsigned long long *__restrict__ zturn) {
     const int lane = threadIdx.x, tile = blockIdx.x;
     const int64_t p = (int64_t)tile * kTileP + lane;
-    int which, y = blockIdx.y, count;
-    float2 *out;
-    if (y < ya) { which = 0; count = nxa; out = anchor; }
-    else if (y == ya) { which = 1; y = 0; count = kFine; out = fine; }
-    else { which = 2; y -= ya + 1; count = nz; out = mz; }
+    int y = blockIdx.y;
+    if (y == ya + 1) {
+        // t = qz dz / (4 pi) turns, reduced to [-1/2, 1/2) and stored as a 64-bit fixed-point fraction (two's complement wraps
+        // like the phase does); FP64 carries 53 bits of it, far more than the 32 the epilogue keeps after the multiplication
+        unsigned long long v = 0ull;
+        if (p < npix) {
+            double t = q[3 * p + 2] * dz * (0.25 / 3.14159265358979323846);
+            t -= rint(t);
+            v = (unsigned long long)(long long)rint(t * 18446744073709551616.0);   // 2^64; |t| <= 1/2 keeps it in int64 range
+            if (t >= 0.5) v = 0x8000000000000000ull;
+        }
+        zturn[(size_t)tile * kTileP + lane] = v;
+        return;
+    }
+    const bool is_fine = y == ya;
+    if (is_fine) y = 0;
+    const int count = is_fine ? kFine : nxa;
+    float2 *out = is_fine ? fine : anchor;
     const int idx0 = y * 16;
     double re[16], im[16];
     if (p < npix) {
-        if (which == 0) phase_run16(q[3 * p + 0], centre(idx0 * kFine, nx, dx), dx * (double)kFine, re, im);
-        else if (which == 1) phase_run16(q[3 * p + 0], 0.0, dx, re, im);
-        else phase_run16(q[3 * p + 2], centre(idx0, nz, dz), dz, re, im);
+        if (!is_fine) phase_run16(q[3 * p + 0], centre(idx0 * kFine, nx, dx), dx * (double)kFine, re, im);
+        else phase_run16(q[3 * p + 0], 0.0, dx, re, im);
     }
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -415,12 +431,11 @@ __global__ void table_small_all_kernel(const double *__restrict__ q, int64_t npi
 }
 
 cudaError_t launch_tables(const double *d_q, const Plan &p, __half *d_A, float2 *d_anchor, float2 *d_fine,
-                          float2 *d_mz, cudaStream_t st, int *nlaunch) {
+                          unsigned long long *d_zturn, cudaStream_t st, int *nlaunch) {
     const int64_t nthreads_a = p.npix_pad * (p.ny_pad / 16);
     table_a_kernel<<<(unsigned)((nthreads_a + 127) / 128), 128, 0, st>>>(d_q, p.npix, p.npix_pad, p.ny, p.ny_pad, p.dy, d_A);
     const int ya = (p.nxa + 15) / 16;
-    table_small_all_kernel<<<dim3(p.ntiles, ya + 1 + (p.nz + 15) / 16), kTileP, 0, st>>>(d_q, p.npix, p.nxa, p.nx, p.dx, p.nz, p.dz, ya,
-                                                                                       d_anchor, d_fine, d_mz);
+    table_small_all_kernel<<<dim3(p.ntiles, ya + 2), kTileP, 0, st>>>(d_q, p.npix, p.nxa, p.nx, p.dx, p.dz, ya, d_anchor, d_fine, d_zturn);
     if (nlaunch) *nlaunch += 2;
     return cudaGetLastError();
 }

@@ -414,6 +414,10 @@ int sep_zsplit(const Plan &p, int npx, int npy, int num_sms) {
     return nzs < 1 ? 1 : nzs;
 }
 
+cudaError_t sep_init_device() {   // per device (scatman_create)
+    return cudaFuncSetAttribute(sep_stage_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * 8);
+}
+
 // one batch item: rho (FP32 complex [nz][ny][nx], without dV) -> I[npy][npx]
 cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_Ex, const float2 *d_Ey, const double *d_qx,
                             int npx, const double *d_qy, int npy, int nzs, float2 *d_H, unsigned char *d_flags,
@@ -425,12 +429,6 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
     dim3 gx((M + kBM - 1) / kBM, (npx + kBN - 1) / kBN);
     sep_stage_x_kernel<<<gx, 256, 0, st>>>(d_rho, d_Ex, M, p.nx, npx, p.ny % 16 == 0 ? d_flags : nullptr, d_H);
     dim3 gy((npx + kBN - 1) / kBN, (npy + kBM - 1) / kBM, nzs);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t ea = cudaFuncSetAttribute(sep_stage_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * 8);
-        if (ea != cudaSuccess) return ea;
-        attr_set = true;
-    }
     sep_stage_yz_kernel<<<gy, 256, 16 * 256 * 8, st>>>(d_Ey, d_H, d_qx, d_qy, k, npx, npy, p.ny, p.nz, p.dz, nzs, d_flags, nyc,
                                             d_partial);
     const int64_t npix = (int64_t)npx * npy;

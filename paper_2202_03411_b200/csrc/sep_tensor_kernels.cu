@@ -30,17 +30,6 @@ namespace scatman {
 bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
                 const cuuint32_t *box, CUtensorMapSwizzle swizzle);   // tensor_kernel.cu
 
-#ifdef SEP_TIMING
-// debug-only cycle accounting of the stage YZ issuers (built by _work scripts with -DSEP_TIMING; never in the product build)
-__device__ long long g_sep_timing[74 * 2 * 8];
-extern "C" int scatman_debug_sep_timing(long long *h_out) {
-    return (int)cudaMemcpyFromSymbol(h_out, g_sep_timing, sizeof(long long) * 74 * 2 * 8);
-}
-#define SEP_TIMED(acc, stmt) do { long long _t0 = clock64(); stmt; acc += clock64() - _t0; } while (0)
-#else
-#define SEP_TIMED(acc, stmt) stmt
-#endif
-
 namespace {
 
 constexpr int kM = 128;              // UMMA M: rows of the A operand tile
@@ -319,12 +308,8 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                         for (int pl = 0; pl < 4; ++pl) {
                             ptx::mbar_wait(r_empty + slot, phase ^ 1);
                             if (ptx::elect_one()) {
-#ifdef SEPABL_X_NOLOAD   // debug-only ablation (built by _work scripts; never in the product build)
-                                ptx::mbar_arrive(r_full + slot);
-#else
                                 ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)kSlotA);
                                 ptx::tma_load_3d(sR + slot * kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, pl);
-#endif
                             }
                             __syncwarp();
                             if (++slot == kStages) { slot = 0; phase ^= 1; }
@@ -433,14 +418,6 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                     ptx::tc_fence_after();
                     const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
                     __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
-#ifdef SEPABL_X_NOEPI
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(t_empty + buf);
-                    ++u;
-                    if (dst == nullptr) *dst = __float2half(0.f);
-                    continue;
-#endif
 #pragma unroll 1
                     for (int c0 = 0; c0 < kCols; c0 += 8) {
                         uint32_t gre[8], gim[8];
@@ -831,14 +808,10 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                     if (((f >> kb) & 1u) == 0u) continue;
                     ptx::mbar_wait(b_empty + slot, phase ^ 1);
                     if (ptx::elect_one()) {
-#ifdef SEPABL_YZ_NOLOAD
-                        ptx::mbar_arrive(b_full + slot);
-#else
                         ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kStageB);
                         for (int pl = 0; pl < 4; ++pl)
                             ptx::tma_load_3d(sB + slot * kStageB + pl * (kStageB / 4), &tmB, b_full + slot,
                                              (it.g * 2 + kb) * kKB, j * P.NPXP + it.ta * kNyz, pl);
-#endif
                     }
                     __syncwarp();
                     if (++slot == kStages) { slot = 0; phase ^= 1; }
@@ -958,14 +931,6 @@ sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
-#ifdef SEPABL_YZ_NOEPI
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(t_empty + buf);
-                ++u;
-                tot[0].x += (float)(mult + t_im);
-                continue;
-#endif
                 uint32_t gre[2][8], gim[2][8];
                 ptx::tmem_ld8(t_re, gre[0]);
                 ptx::tmem_ld8(t_im, gim[0]);
@@ -1125,10 +1090,6 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                     for (int pg = 0; pg < 4 / kG; ++pg) {
                         ptx::mbar_wait(b_empty + slot, phase ^ 1);
                         if (ptx::elect_one()) {
-#ifdef SEPABL_YZ_NOLOAD   // debug-only ablation (built by _work scripts; never in the product build)
-                            if (leader) ptx::mbar_arrive(b_full + slot);
-                            (void)j;
-#else
                             if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)(NCTA * kStageB));   // both halves land on the leader's barrier
                             const int row = j * P.NPXP + it.ta * kN + (int)rank * (kN / NCTA);
 #pragma unroll
@@ -1137,7 +1098,6 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                                 if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
                                 else ptx::tma_load_3d(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
                             }
-#endif
                         }
                         __syncwarp();
                         if (++slot == kStages) { slot = 0; phase ^= 1; }
@@ -1168,13 +1128,9 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
-#ifdef SEP_TIMING
-        long long w_afull = 0, w_tempty = 0, w_first = 0, w_bfull = 0;
-        const long long t_begin = clock64();
-#endif
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
             const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
-            SEP_TIMED(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
+            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             int z0, z1;
             zrange(it, z0, z1);
@@ -1184,7 +1140,7 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
             uint32_t f;
             while (un.next(n, f)) {
                 const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                SEP_TIMED(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                 bool first = true;
@@ -1192,10 +1148,10 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                     if (((f >> kb) & 1u) == 0u) continue;
                     for (int pg = 0; pg < 4 / kG; ++pg) {
                         if (first && pg == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
-                            SEP_TIMED(w_first, ptx::mbar_wait(first_done + buf, upar));
+                            ptx::mbar_wait(first_done + buf, upar);
                             ptx::tc_fence_after();
                         }
-                        SEP_TIMED(w_bfull, ptx::mbar_wait(b_full + slot, phase));
+                        ptx::mbar_wait(b_full + slot, phase);
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
 #pragma unroll
@@ -1243,12 +1199,6 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
             if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
         }
-#ifdef SEP_TIMING
-        if (lane == 0) {
-            long long *o = g_sep_timing + ((blockIdx.x / NCTA) * 2 + iw) * 8;
-            o[0] = clock64() - t_begin; o[1] = w_afull; o[2] = w_tempty; o[3] = w_first; o[4] = w_bfull; o[5] = u;
-        }
-#endif
       }
     } else {
         setmaxnreg_inc_224();
@@ -1292,17 +1242,6 @@ sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
-#ifdef SEPABL_YZ_NOEPI
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) {
-                    if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);
-                    else ptx::mbar_arrive(t_empty + buf);
-                }
-                ++u;
-                tot[0].x += (float)(mult + t_im);
-                continue;
-#endif
 #pragma unroll
                 for (int q8 = 0; q8 < 8; ++q8) {
                     uint32_t gre[8], gim[8];
@@ -1766,14 +1705,10 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         int slot = 0;
         uint32_t phase = 0, u = 0;
         int it_local = 0;
-#ifdef SEP_TIMING
-        long long w_afull = 0, w_tempty = 0, w_first = 0, w_bfull = 0;
-        const long long t_begin = clock64();
-#endif
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
             int ta, tbn, sp, bi;
             decode(item, ta, tbn, sp, bi);
-            SEP_TIMED(w_afull, ptx::mbar_wait(e_full, (uint32_t)(it_local & 1)));
+            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             const uint64_t kEpl = (uint64_t)P.nkb * kE;   // descriptor distance between Ey planes
             int z0, z1;
@@ -1784,7 +1719,7 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             uint32_t m;
             while (un.next(n, m)) {
                 const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                SEP_TIMED(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
+                ptx::mbar_wait(t_empty + buf, upar ^ 1);
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                 bool first = true;
@@ -1792,10 +1727,10 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     if (((m >> kb) & 1u) == 0u) continue;
                     for (int ph = 0; ph < 2; ++ph) {
                         if (first && ph == 0 && iw == 1) {   // D must have been initialised by issuer 0
-                            SEP_TIMED(w_first, ptx::mbar_wait(first_done + buf, upar));
+                            ptx::mbar_wait(first_done + buf, upar);
                             ptx::tc_fence_after();
                         }
-                        SEP_TIMED(w_bfull, ptx::mbar_wait(h_full + slot, phase));
+                        ptx::mbar_wait(h_full + slot, phase);
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
 #pragma unroll
@@ -1837,12 +1772,6 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             if (ptx::elect_one()) ptx::umma_commit_2sm(e_empty, (uint16_t)0x3);
             __syncwarp();
         }
-#ifdef SEP_TIMING
-        if (lane == 0) {
-            long long *o = g_sep_timing + ((blockIdx.x / 2) * 2 + iw) * 8;
-            o[0] = clock64() - t_begin; o[1] = w_afull; o[2] = w_tempty; o[3] = w_first; o[4] = w_bfull; o[5] = u;
-        }
-#endif
       }
     } else {
         setmaxnreg_inc_224();
@@ -2007,6 +1936,25 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     return t;
 }
 
+constexpr int kSmemYz = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // every stage YZ variant: 128 KB resident + 96 KB ring
+constexpr int kSmemX = 1024 + 131072 + 6 * kSlotA + 256;                           // every stage X variant
+
+// Function attributes belong to a device's context: set for the CURRENT device by scatman_create.
+cudaError_t sep_tc_init_device() {
+    const cudaFuncAttribute attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, attr, kSmemYz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yz128_kernel<1>, attr, kSmemYz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yzs_kernel, attr, kSmemYz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yzt_kernel<64>, attr, kSmemYz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<64>, attr, kSmemX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<32>, attr, kSmemX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<16>, attr, kSmemX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<64>, attr, kSmemX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<32>, attr, kSmemX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<16>, attr, kSmemX);
+    return e;
+}
+
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st) {
     const int64_t nye = (int64_t)t.NPYP * t.NY;
@@ -2019,12 +1967,6 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 template <int NCTA>
 static cudaError_t launch_yz128_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepYzParams &P, int nitems, int num_sms,
                                         int smem, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz128_kernel<NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     const int max_clusters = num_sms / NCTA;
     const int nclusters = nitems < max_clusters ? nitems : max_clusters;
     cudaLaunchConfig_t cfg = {};
@@ -2045,7 +1987,7 @@ static cudaError_t launch_yz128_variant(const CUtensorMap &tmA, const CUtensorMa
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
                              const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
-    constexpr int kSmem = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // every variant: 128 KB resident + 96 KB ring
+    constexpr int kSmem = kSmemYz;
     const int ncta = t.nyz == 128 ? t.yz_ncta : 1;
     CUtensorMap tmA, tmB;
     bool ok;
@@ -2098,21 +2040,9 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
         attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        static bool attr_t = false;
-        if (!attr_t) {
-            cudaError_t e = cudaFuncSetAttribute(sep_tc_yzt_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-            if (e != cudaSuccess) return e;
-            attr_t = true;
-        }
         return cudaLaunchKernelEx(&cfg, sep_tc_yzt_kernel<64>, tmA, tmB, P);
     }
     if (t.yz_stream) {
-        static bool attr_s = false;
-        if (!attr_s) {
-            cudaError_t e = cudaFuncSetAttribute(sep_tc_yzs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-            if (e != cudaSuccess) return e;
-            attr_s = true;
-        }
         const int nit = (P.ntb / 2) * P.nta * P.nzs * nb, maxc = num_sms / 2;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
@@ -2130,12 +2060,6 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     }
     const int nitems = (P.ntb / ncta) * P.nta * P.ng * P.nzs * nb;
     if (t.nyz == 128) return launch_yz128_variant<1>(tmA, tmB, P, nitems, num_sms, kSmem, st);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     sep_tc_yz_kernel<<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
     return cudaGetLastError();
 }
@@ -2158,13 +2082,7 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
 template <int NX>
 static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
                                     cudaStream_t st) {
-    constexpr int kSmem = 1024 + 131072 + 6 * kSlotA + 256;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sep_tc_x_kernel<NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    constexpr int kSmem = kSmemX;
     const int nitems = P.nta * P.nsx;
     sep_tc_x_kernel<NX><<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
     return cudaGetLastError();
@@ -2173,13 +2091,7 @@ static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &t
 template <int NX>
 static cudaError_t launch_x2_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
                                      cudaStream_t st) {
-    constexpr int kSmem = 1024 + 131072 + 6 * kSlotA + 256;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sep_tc_x2_kernel<NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    constexpr int kSmem = kSmemX;
     const int nitems = P.nta * P.nsx, max_clusters = num_sms / 2;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(2 * (nitems < max_clusters ? nitems : max_clusters)));

@@ -11,9 +11,13 @@
 // accumulators (tcgen05.ld) and reduce them over x against e^{i qx x} = anchor[x/16] * fine[x%16],
 // multiply by e^{i qz z_j} and accumulate over slices in FP32 registers (the fused epilogue).
 //
-// Roles: warp 0 lane 0 = TMA producer, warp 1 lane 0 = MMA issuer, warp 2 = TMEM allocator,
-// warps 4-7 = epilogue (TMEM lane group = warp % 4).  Pipelines: A-resident (a_full/a_empty),
-// B ring of kStagesB 16-KB slots (b_full/b_empty), two TMEM accumulator buffers (t_full/t_empty).
+// Roles: warp 0 = TMA producer, warps 1 and 3 = MMA issuers (k-step n of a unit belongs to issuer n % 2), warp 2 = TMEM
+// allocator, warps 4-7 = epilogue (TMEM lane group = warp % 4).  Pipelines: A-resident (a_full/a_empty), B ring of
+// kStagesB slots (b_full/b_empty), two TMEM accumulator buffers (t_full/t_empty), first_done orders issuer 1 behind the
+// unit's first k-step.  Ordering between the two issuing threads (tcgen05.mma is ordered only within one thread): a
+// unit's accumulator is initialised by issuer 0's first k-step and issuer 1 waits for its completion (first_done);
+// after that both threads only ACCUMULATE into D, and FP32 accumulation order differences are within the tolerance
+// budget; both commit t_full (count 2), so the epilogue sees every MMA of both threads.
 #include <cuda.h>
 
 #include "internal.h"
@@ -32,20 +36,11 @@ constexpr int kMaxStagesB = 12;
 
 size_t tensor_smem_bytes() { return kSmemTotal; }
 
-#ifdef SCATMAN_TIMING
-// debug-only cycle accounting (built by _work scripts with -DSCATMAN_TIMING; never in the product build)
-__device__ long long g_timing[148 * 8];
-#define TIMING_DECL(name) long long name = 0, name##_long = 0, name##_n = 0
-#define TIMED_WAIT(acc, stmt) do { long long _t0 = clock64(); stmt; long long _d = clock64() - _t0; acc += _d; if (_d > 400) { acc##_long += _d; ++acc##_n; } } while (0)
-#else
-#define TIMING_DECL(name)
-#define TIMED_WAIT(acc, stmt) stmt
-#endif
-
 struct TensorParams {
     int nz, nxt, nyb, ny16, ngroups, ntiles, batch, nchunks, bpc, nzs, nxa;
     int64_t npix_pad;
-    const float2 *anchor, *fine, *mz;
+    const float2 *anchor, *fine;
+    const unsigned long long *zturn;  // [tile][128]: frac(qz dz / 4 pi) of the pixel as a 64-bit fixed-point fraction of a turn
     const unsigned long long *mask;   // [batch][nz][nxt][ngroups]: bit 8*yi + xi = 16-y x 16-x block of rho~ is non-zero
     float2 *partial;
 };
@@ -185,7 +180,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         ptx::mbar_init(a_empty, 2);      // both MMA issuers
         for (int i = 0; i < kStagesB; ++i) {
             ptx::mbar_init(b_full + i, 1);
-            ptx::mbar_init(b_empty + i, 1);
+            ptx::mbar_init(b_empty + i, 2);   // both MMA issuers (see the issuer loop)
         }
         for (int i = 0; i < 2; ++i) {
             ptx::mbar_init(t_full + i, 2);   // both MMA issuers
@@ -250,20 +245,12 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // this 16-y step of the slice tile is empty
                     ptx::mbar_wait(b_empty + slot, phase ^ 1);
                     if (ptx::elect_one()) {
-#ifdef SCATMAN_ABL_NOLOAD
-                        if (leader) ptx::mbar_arrive(b_full + slot);
-#else
                         if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, tx_bytes);
-#endif
                         void *dst = sB + slot * kSlotB;
                         const int cg = uxt * 16 + (NCTA == 2 ? (int)rank * 8 + xa : 0);
                         const int cs = (ub * P.nz + uj) * P.ny16 + it.g * (kGroupYB * kBlockY / 16) + yi;
-#ifndef SCATMAN_ABL_NOLOAD
                         if (NCTA == 2) ptx::tma_load_4d_2sm(dst, tmb, b_full + slot, 0, 0, cg, cs);
                         else ptx::tma_load_4d(dst, tmb, b_full + slot, 0, 0, cg, cs);
-#else
-                        (void)dst; (void)cg; (void)cs; (void)tmb;
-#endif
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
@@ -298,14 +285,10 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         uint32_t phase = 0;
         uint32_t u = 0;
         int it_local = 0;
-        TIMING_DECL(w_tempty); TIMING_DECL(w_bfull); TIMING_DECL(w_afull);
-#ifdef SCATMAN_TIMING
-        const long long t_begin = clock64();
-#endif
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
             const Item it = decode_item(item, P, ntp);
             const int nybg = min(kGroupYB, P.nyb - it.g * kGroupYB);
-            TIMED_WAIT(w_afull, ptx::mbar_wait(a_full, (uint32_t)(it_local & 1)));
+            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
             ptx::tc_fence_after();
             // All-zero units never appear: no MMA, no accumulator hand-over.
             // TWO issuers (warps 1 and 3) share every unit: k-step n of a unit belongs to issuer n % 2.  For N < 112 a
@@ -320,7 +303,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                 {
                     const uint32_t buf = u & 1;
                     const uint32_t upar = (u >> 1) & 1;
-                    TIMED_WAIT(w_tempty, ptx::mbar_wait(t_empty + buf, upar ^ 1));
+                    ptx::mbar_wait(t_empty + buf, upar ^ 1);
                     ptx::tc_fence_after();
                     const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
                     int xa, xm;
@@ -331,14 +314,24 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     int kidx = 0;            // k-step index within the unit
                     for (int yi = 0; yi < 4 * nybg; ++yi) {
                         if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // empty 16-y step: never loaded
-                        if ((kidx & 1) == iw) {
-#ifndef SCATMAN_ABL_NOFIRST
+                        // BOTH issuers observe every pass of every slot's full barrier and BOTH release the slot (b_empty
+                        // counts 2: the owner's tcgen05.commit + a plain arrive of the other issuer).  A parity wait tells
+                        // pass R from pass R - 1 only: were a slot re-armed while one issuer had not seen its previous pass
+                        // (units with odd k-step counts shift the ownership of a slot between the issuers), that issuer
+                        // could take "pass R - 2 complete" for "pass R complete" and consume stale data.  With both
+                        // arrivals the producer cannot run more than one pass ahead of either issuer, whatever order the
+                        // TMA loads complete in.  The extra wait runs while the issuer's own MMAs execute.
+                        ptx::mbar_wait(b_full + slot, phase);
+                        if ((kidx & 1) != iw) {
+                            if (ptx::elect_one()) {
+                                ptx::mbar_arrive(b_empty + slot);
+                                if (NCTA == 2) ptx::mbar_arrive_cluster(b_empty + slot, 1);
+                            }
+                            __syncwarp();
+                        } else {
                             if (kidx == 1) {   // issuer 1's first k-step of the unit: D must have been initialised
                                 ptx::mbar_wait(first_done + buf, upar);
-                                ptx::tc_fence_after();
                             }
-#endif
-                            TIMED_WAIT(w_bfull, ptx::mbar_wait(b_full + slot, phase));
                             ptx::tc_fence_after();
                             if (ptx::elect_one()) {
                                 // A planes 0 Re_hi, 1 Re_lo, 2 Im_hi, 3 Im_lo of this k-step (32 bytes = 2 descriptor units per step)
@@ -377,18 +370,6 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             if (ptx::elect_one()) commit(a_empty);
             __syncwarp();
         }
-#ifdef SCATMAN_TIMING
-        if (lane == 0 && iw == 0) {
-            g_timing[blockIdx.x * 8 + 0] = clock64() - t_begin;
-            g_timing[blockIdx.x * 8 + 1] = w_tempty;
-            g_timing[blockIdx.x * 8 + 2] = w_bfull;
-            g_timing[blockIdx.x * 8 + 3] = w_afull;
-            g_timing[blockIdx.x * 8 + 7] = w_bfull_long;
-            g_timing[blockIdx.x * 8 + 6] = w_bfull_n;
-            g_timing[blockIdx.x * 8 + 5] = w_tempty_long;
-            g_timing[blockIdx.x * 8 + 4] = w_tempty_n;
-        }
-#endif
       }
     } else if (warp >= 4) {
         // ========================================================================= epilogue
@@ -396,10 +377,6 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         const int el = ew * 32 + lane;  // pixel within the tile = TMEM lane
         const uint32_t lane_base = tmem_base + ((uint32_t)(ew * 32) << 16);
         uint32_t u = 0;
-        TIMING_DECL(w_tfull);
-#ifdef SCATMAN_TIMING
-        const long long e_begin = clock64();
-#endif
         for (int item = cluster_id; item < nitems; item += nclusters) {
             const Item it = decode_item(item, P, ntp);
             const int tile = it.tp * NCTA + (int)rank;
@@ -408,7 +385,10 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #pragma unroll
             for (int i = 0; i < kFine; ++i) fine[i] = __ldg(P.fine + ((size_t)tile * kFine + i) * kTileP + el);
             const float2 *anchor_t = P.anchor + (size_t)tile * P.nxa * kTileP + el;
-            const float2 *mz_t = P.mz + (size_t)tile * P.nz * kTileP + el;
+            // slice phase e^{i qz z_j}, z_j = (j - (nz-1)/2) dz: qz z_j = 2 pi t (2j - nz + 1) with t = qz dz / 4 pi turns.  frac(t) is a
+            // 64-bit fixed-point fraction of a turn, so the integer product wraps modulo one turn for free; its top 32 bits go
+            // to the SFU as an angle in [-pi, pi) (error <= 2^-32 turn + 4e-7 rad of __sincosf, for any nz).
+            const unsigned long long zt = __ldg(P.zturn + (size_t)tile * kTileP + el);
             float2 *partial_t = P.partial + (size_t)(it.g * P.nzs + it.s) * P.npix_pad + (size_t)tile * kTileP + el;
             const size_t partial_b = (size_t)(P.ngroups * P.nzs) * P.npix_pad;   // stride between batch items
             // Flat walk over the non-empty units; f = row-dot of the current slice, acc = amplitude of the current
@@ -437,7 +417,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                                 acc_im = 0.f;
                             }
                             cj = uj;
-                            mz = __ldg(mz_t + (size_t)uj * kTileP);
+                            const unsigned long long turn = zt * (unsigned long long)(long long)(2 * uj - P.nz + 1);
+                            __sincosf((float)(int)(uint32_t)(turn >> 32) * 1.4629180792671596e-9f, &mz.y, &mz.x);   // pi / 2^31
                         }
                         const uint32_t buf = u & 1;
                         int xa, xm;
@@ -446,7 +427,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 #pragma unroll
                         for (int a = 0; a < kTileX / kFine; ++a)
                             anc[a] = __ldg(anchor_t + (size_t)(xt * (kTileX / kFine) + min(xa + a, kTileX / kFine - 1)) * kTileP);
-                        TIMED_WAIT(w_tfull, ptx::mbar_wait(t_full + buf, (u >> 1) & 1));
+                        ptx::mbar_wait(t_full + buf, (u >> 1) & 1);
                         ptx::tc_fence_after();
                         const uint32_t t_re = lane_base + buf * 256, t_im = t_re + 128;
                         // Column layout of an accumulator (N = 16 xm): x block a = columns [8a, 8a+8) (its x 0..7) and
@@ -454,17 +435,6 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         const uint32_t half = 8u * (uint32_t)xm;
                         // software-pipelined: the loads of block a+1 are in flight while block a is reduced; the
                         // accumulator buffer is handed back to the MMA warp as soon as its last column has landed
-#ifdef SCATMAN_ABL_NOEPI
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) {
-                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);
-                            else ptx::mbar_arrive(t_empty + buf);
-                        }
-                        ++u;
-                        f_re += anc[0].x + (float)half + (float)t_im;
-                        continue;
-#endif
                         uint32_t gre[2][16], gim[2][16];
                         ptx::tmem_ld8(t_re, gre[0]);
                         ptx::tmem_ld8(t_re + half, gre[0] + 8);
@@ -524,13 +494,6 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                 acc_im = 0.f;
             }
         }
-#ifdef SCATMAN_TIMING
-        if (warp == 4 && lane == 0 && (blockIdx.x & 1)) {
-            g_timing[blockIdx.x * 8 + 4] = clock64() - e_begin;
-            g_timing[blockIdx.x * 8 + 5] = w_tfull;
-            g_timing[blockIdx.x * 8 + 6] = u;
-        }
-#endif
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -569,16 +532,16 @@ bool encode_map(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *d
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Function attributes belong to a device's context: set for the CURRENT device by scatman_create (one context per device).
+cudaError_t tensor_init_device() {
+    cudaError_t e = cudaFuncSetAttribute(msft_contract_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTotal);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(msft_contract_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemTotal);
+    return e;
+}
+
 template <int NCTA>
 static cudaError_t launch_variant(const CUtensorMap &tmA, const TmapsB &tmB, const TensorParams &P, int num_sms,
                                   cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(msft_contract_kernel<NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             kSmemTotal);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     const int nitems = P.nchunks * P.nzs * P.ngroups * (P.ntiles / NCTA);
     const int max_clusters = num_sms / NCTA;
     const int nclusters = nitems < max_clusters ? nitems : max_clusters;
@@ -628,14 +591,9 @@ cudaError_t launch_tensor(const Plan &p, const TensorLaunch &t, cudaStream_t st,
     P.nchunks = (p.batch + P.bpc - 1) / P.bpc;
     P.nxa = p.nxa;
     P.npix_pad = p.npix_pad;
-    P.anchor = t.d_anchor; P.fine = t.d_fine; P.mz = t.d_mz; P.partial = t.d_partial; P.mask = t.d_mask;
+    P.anchor = t.d_anchor; P.fine = t.d_fine; P.zturn = t.d_zturn; P.partial = t.d_partial; P.mask = t.d_mask;
     return ncta == 2 ? launch_variant<2>(tmA, tmB, P, t.num_sms, st) : launch_variant<1>(tmA, tmB, P, t.num_sms, st);
 }
 
-#ifdef SCATMAN_TIMING
-extern "C" int scatman_debug_timing(long long *h_out) {
-    return (int)cudaMemcpyFromSymbol(h_out, g_timing, sizeof(long long) * 148 * 8);
-}
-#endif
 
 }  // namespace scatman

@@ -5,7 +5,7 @@ import pytest
 
 from oracle import oracle as O
 from paper_2202_03411_b200 import workloads as W
-from parity import assert_parity, metrics
+from parity import FULL_SIZE_SAMPLES, assert_parity, metrics, oracle_at_pixels, sampled_pixels
 
 pytestmark = pytest.mark.gpu
 
@@ -183,7 +183,7 @@ def test_error_codes(sm):
 
 
 # ------------------------------------------------------------------------------------------ full sizes, sampled pixels
-def _sampled_full(sm, idx, count, items=None):
+def _sampled_full(sm, idx, items=None):
     w = W.config(idx)
     vox = (w.dx, w.dy, w.dz)
     items = [0] if items is None else items
@@ -192,24 +192,22 @@ def _sampled_full(sm, idx, count, items=None):
     I = sm.simulate_nufft(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat).cpu().numpy()
     for i in range(len(items)):
         flat = I[i].ravel()
-        c = w.npy // 2 * w.npx + w.npx // 2
-        pix = W.sample_pixels(w.seed + i, w.npix, count, always=[int(np.argmax(flat)), c, c - 1, c - w.npx, c - w.npx - 1,
-                                                                  0, w.npx - 1, w.npix - 1])
-        ref = O.simulate(g[i], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[i], pixels=pix)
+        pix = sampled_pixels(w, items[i], flat, FULL_SIZE_SAMPLES[idx])
+        ref = oracle_at_pixels(w, items[i], g[i], None if quat is None else quat[i], pix)
         assert_parity(flat[pix], ref, what=f"nufft {w.name} item {items[i]} sampled")
 
 
 def test_cfg2_full_size_sampled(sm):
-    _sampled_full(sm, 1, 512)
+    _sampled_full(sm, 1)
 
 
 def test_cfg3_full_size_sampled(sm):
-    _sampled_full(sm, 2, 192)
+    _sampled_full(sm, 2)
 
 
 def test_cfg4_full_size_items_sampled(sm):
-    _sampled_full(sm, 3, 128, items=[0, 1, 2, 3])
+    _sampled_full(sm, 3, items=[0, 1, 2, 3])
 
 
 def test_cfg5_full_size_sampled(sm):
-    _sampled_full(sm, 4, 48)
+    _sampled_full(sm, 4)

@@ -4,7 +4,7 @@ import pytest
 
 from oracle import oracle as O
 from paper_2202_03411_b200 import workloads as W
-from parity import assert_parity, metrics
+from parity import FULL_SIZE_SAMPLES, assert_parity, metrics, oracle_at_pixels, sampled_pixels
 
 pytestmark = pytest.mark.gpu
 
@@ -230,6 +230,123 @@ def test_deterministic_and_workspace_reuse(sm):
     assert sm.last_launch_count() == 7   # q-map, prefix, pack, 2 table launches, contraction, finalize
 
 
+def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
+    """SCATMAN_FLAG_REUSE_TABLES skips the q-map and phase-table kernels when grid geometry, lambda, detector, method and
+    workspace equal the previous call's -- never otherwise: results are bit-identical with and without the flag, on every route."""
+    import torch
+    from paper_2202_03411_b200 import binding as B
+    w = W.config(0)
+    vox = (w.dx, w.dy, w.dz)
+    g1, g2 = dev(w.grid(0)), dev(W.random_grid(5, w.nx, w.ny, w.nz))
+    g3 = dev(np.stack([W.random_grid(6 + i, w.nx, w.ny, w.nz) for i in range(3)]))
+    R = B.FLAG_REUSE_TABLES
+    k = 2 * np.pi / w.lam
+    q1 = torch.from_numpy((np.arange(48) + 0.5 - 24) * (2 * k * np.sin(np.radians(30.0)) / 48)).cuda()
+    q2 = (q1 * 0.5).contiguous()
+    routes = {
+        "pixels": lambda g, lam, th, ws, fl: sm.simulate(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl),
+        "pixels_1cta": lambda g, lam, th, ws, fl: sm.simulate(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl | B.FLAG_SINGLE_CTA),
+        "nufft": lambda g, lam, th, ws, fl: sm.simulate_nufft(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl),
+        "qgrid": lambda g, lam, th, ws, fl: sm.simulate_qgrid(g, vox, lam, q1 if th == 30.0 else q2, q1, workspace=ws, flags=fl),
+    }
+    for name, run in routes.items():
+        ws = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+        ws2 = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+        fresh = lambda g, lam=w.lam, th=30.0: run(g, lam, th, ws2, 0).clone()       # tables rebuilt, other workspace
+        a = run(g1, w.lam, 30.0, ws, 0).clone()
+        n_full = sm.last_launch_count()
+        b = run(g1, w.lam, 30.0, ws, R).clone()                                     # same everything: tables reused
+        n_reuse = sm.last_launch_count()
+        assert n_reuse < n_full, (name, n_reuse, n_full)
+        assert torch.equal(a, b), name
+        assert torch.equal(run(g2, w.lam, 30.0, ws, R), fresh(g2)), name            # new particle, same tables
+        assert sm.last_launch_count() == n_reuse
+        assert torch.equal(run(g3, w.lam, 30.0, ws, R), fresh(g3)), name            # another batch size: same tables (they sit first)
+        assert torch.equal(run(g2, 0.8 * w.lam, 30.0, ws, R), fresh(g2, lam=0.8 * w.lam)), name   # lambda changed: rebuilt
+        assert sm.last_launch_count() == n_full
+        assert torch.equal(run(g2, 0.8 * w.lam, 25.0, ws, R), fresh(g2, lam=0.8 * w.lam, th=25.0)), name   # detector / qx changed
+        assert sm.last_launch_count() == n_full
+        run(g2, 0.8 * w.lam, 25.0, ws2, R)                                          # other workspace: rebuilt there
+        assert sm.last_launch_count() == n_full
+        assert torch.equal(run(g1, w.lam, 30.0, ws, R), a), name                    # back: key differs from the last call's -> rebuilt
+
+
+@pytest.mark.parametrize("route", ["pixels", "qgrid"])
+def test_calls_are_capturable_in_a_cuda_graph(sm, route):
+    """A whole scatman_simulate / scatman_simulate_qgrid call (oriented batch) only enqueues on the caller's stream, so it can
+    be captured in a CUDA graph; a replay on new input in the same buffers equals the eager call within summation order."""
+    import torch
+    rng = np.random.default_rng(12)
+    nx, ny, nz, Bn = 70, 40, 24, 3
+    g = [np.stack([W.random_grid(900 + 10 * r + i, nx, ny, nz, fill=0.4) for i in range(Bn)]) for r in range(2)]
+    quat = W.random_quaternions(rng, Bn)
+    vox, lam = (2.0, 2.0, 2.5), 13.0
+    k = 2 * np.pi / lam
+    q1 = torch.from_numpy((np.arange(40) + 0.5 - 20) * (2 * k * np.sin(np.radians(25.0)) / 40)).cuda()
+    d = dev(g[0])
+    ws = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+    out = torch.empty((Bn, 40, 40), dtype=torch.float32, device="cuda")
+
+    def call(stream=None):
+        if route == "pixels":
+            sm.simulate(d, vox, lam, 40, 40, 25.0, quat=quat, workspace=ws, out=out, stream=stream)
+        else:
+            sm.simulate_qgrid(d, vox, lam, q1, q1, quat=quat, workspace=ws, out=out, stream=stream)
+
+    call()
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        call()
+    assert sm.last_contraction_ms() == -1.0          # events are not recorded inside a capture
+    d.copy_(dev(g[1]))
+    graph.replay()
+    torch.cuda.synchronize()
+    replayed = out.clone()
+    call()
+    torch.cuda.synchronize()
+    assert torch.allclose(replayed, out, rtol=1e-5, atol=1e-6 * float(out.max()))
+    assert sm.last_contraction_ms() > 0.0
+    ref = O.simulate(g[1][1], vox, lam, 40, 40, 25.0, quat=quat[1]) if route == "pixels" else None
+    if ref is not None:
+        assert_parity(replayed[1].cpu().numpy(), ref, what="graph replay")
+
+
+def test_host_entry_points_pipeline_matches_device_paths(sm):
+    """scatman_simulate_host / _nufft_host / _qgrid_host on a batch that is cut into several chunks (17 items of 2.1 MB: the
+    pipeline cuts batches above 16 MB in two; plus a 1-item call): equal to the device entry points item by item."""
+    import torch
+    rng = np.random.default_rng(21)
+    nx, ny, nz, Bn = 64, 64, 64, 17
+    g = np.stack([W.sparse_blobs_grid(700 + i, nx, ny, nz, nblobs=4, max_extent=30) for i in range(Bn)])
+    quat = W.random_quaternions(rng, Bn)
+    vox, lam = (3.0, 3.0, 3.0), 15.0
+    k = 2 * np.pi / lam
+    q1 = (np.arange(40) + 0.5 - 20) * (2 * k * np.sin(np.radians(25.0)) / 40)
+    h = torch.from_numpy(g).pin_memory()
+    for nb in (Bn, 1):
+        hh, qq = h[:nb], quat[:nb]
+        d = dev(g[:nb])
+        I_h = sm.simulate_host(hh, vox, lam, 24, 20, 25.0, quat=qq)
+        I_d = sm.simulate(d, vox, lam, 24, 20, 25.0, quat=qq).cpu()
+        assert torch.allclose(I_h, I_d, rtol=1e-5, atol=1e-6 * float(I_d.max()))
+        N_h = sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq)
+        N_d = sm.simulate_nufft(d, vox, lam, 24, 20, 25.0, quat=qq).cpu()
+        assert torch.equal(N_h, N_d)
+        Q_h = sm.simulate_qgrid_host(hh, vox, lam, q1, q1, quat=qq)
+        Q_d = sm.simulate_qgrid(d, vox, lam, torch.from_numpy(q1).cuda(), torch.from_numpy(q1).cuda(), quat=qq).cpu()
+        assert torch.allclose(Q_h, Q_d, rtol=1e-5, atol=1e-6 * float(Q_d.max()))
+        # a second call reuses the tables kept in the context's arena; new q values rebuild them
+        assert torch.equal(sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq), N_h)
+        Q2 = sm.simulate_qgrid_host(hh, vox, lam, 0.5 * q1, q1, quat=qq)
+        Q2_d = sm.simulate_qgrid(d, vox, lam, torch.from_numpy(0.5 * q1).cuda(), torch.from_numpy(q1).cuda(), quat=qq).cpu()
+        assert torch.allclose(Q2, Q2_d, rtol=1e-5, atol=1e-6 * float(Q2_d.max()))
+        for b in {0, nb - 1}:
+            ref = O.simulate(g[b], vox, lam, 24, 20, 25.0, quat=quat[b])
+            assert_parity(N_h[b].numpy(), ref, what=f"host nufft item {b}")
+            assert_parity(I_h[b].numpy(), ref, what=f"host pixels item {b}")
+
+
 def test_simulate_host_matches_device_path(sm):
     import torch
     w = W.config(0)
@@ -238,6 +355,68 @@ def test_simulate_host_matches_device_path(sm):
     I_h = sm.simulate_host(h, (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg)
     I_d = sm.simulate(dev(g), (w.dx, w.dy, w.dz), w.lam, w.npx, w.npy, w.theta_max_deg).cpu()
     assert torch.equal(I_h[0], I_d)
+
+
+def test_issuers_stay_in_step_on_mixed_odd_even_kstep_units(sm):
+    """The two MMA issuer warps of the contraction share the k-steps of a unit by parity, so units with an odd number of
+    live 16-y steps shift which issuer owns a ring slot.  Grid: 40 slices x 3 x-tiles whose live y steps number 1..8 in a
+    scrambled order (several hundred k-steps per CTA pair: the 12-slot ring wraps dozens of times, through every
+    ownership pattern), checked against the oracle, run to run and between the two tensor kernels."""
+    rng = np.random.default_rng(1234)
+    nx, ny, nz = 300, 128, 40
+    g = np.zeros((nz, ny, nx, 2), np.float32)
+    for j in range(nz):
+        for xt in range(3):
+            nsteps = int(rng.integers(1, 9))
+            for ys in rng.choice(8, size=nsteps, replace=False):
+                x0 = 128 * xt + int(rng.integers(0, min(128, nx - 128 * xt) - 8))
+                y0 = 16 * int(ys) + int(rng.integers(0, 12))
+                g[j, y0:y0 + 3, x0:x0 + 6, 0] = rng.uniform(0.01, 0.05)
+                g[j, y0:y0 + 3, x0:x0 + 6, 1] = rng.uniform(0.0, 0.01)
+    voxel, lam = (2.0, 2.0, 2.0), 12.0
+    npx, npy, th = 32, 16, 30.0                     # 512 pixels = 2 CTA pairs
+    ref = O.simulate(g, voxel, lam, npx, npy, th)
+    outs = {}
+    for name in ("tensor", "tensor_1cta"):
+        runs = [sm.simulate(dev(g), voxel, lam, npx, npy, th, method=METHODS[name][0], flags=METHODS[name][1]).cpu().numpy()
+                for _ in range(6)]
+        for r in runs:
+            assert_parity(r, ref, what=f"mixed k-steps {name}")
+            # Two issuing threads accumulate into one FP32 accumulator in whatever order their MMAs reach the tensor pipe, so
+            # runs may differ by FP32 summation order (~1e-7 of the amplitude); a stale operand tile would be orders above.
+            assert np.max(np.abs(r - runs[0])) <= 3e-6 * ref.max(), f"{name}: run-to-run difference beyond summation order"
+        outs[name] = runs[0]
+    assert np.allclose(outs["tensor"], outs["tensor_1cta"], rtol=1e-4, atol=1e-6 * ref.max())
+
+
+def test_create_destroy_create_runs_every_route():
+    """Kernel attributes (dynamic shared memory limits) are set per context creation, not once per process: a second
+    context, and one created after the first was destroyed, run every route."""
+    import torch
+    from paper_2202_03411_b200 import binding as B, build
+    build.build()
+    w = W.config(0)
+    g = w.grid(0)
+    vox = (w.dx, w.dy, w.dz)
+    k = 2 * np.pi / w.lam
+    q1 = torch.from_numpy((np.arange(48) + 0.5 - 24) * (2 * k * np.sin(np.radians(30.0)) / 48)).cuda()
+    results = []
+    first = B.Scatman(0)
+    second = B.Scatman(0)          # two live contexts on one device
+    for round_, s in enumerate((first, second, None)):
+        if s is None:
+            first.close()
+            second.close()
+            s = B.Scatman(0)       # created after both were destroyed
+        r = [s.simulate(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=m, flags=fl).cpu() for m, fl in METHODS.values()]
+        r.append(s.simulate_nufft(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg).cpu())
+        r.append(s.simulate_qgrid(dev(g), vox, w.lam, q1, q1).cpu())
+        r.append(s.simulate_qgrid(dev(g), vox, w.lam, q1, q1, method=B.METHOD_SIMT_TABLE).cpu())
+        results.append(r)
+        if round_ == 2:
+            s.close()
+    for r in results[1:]:
+        assert all(torch.equal(a, b) for a, b in zip(results[0], r))
 
 
 def test_error_codes(sm):
@@ -257,33 +436,34 @@ def test_error_codes(sm):
 
 
 # ------------------------------------------------------------------------------------------ full sizes, sampled pixels
-def _sampled_full(sm, idx, count, items=None):
-    import torch
+def _sampled_full(sm, idx, items=None, method="tensor"):
     w = W.config(idx)
     vox = (w.dx, w.dy, w.dz)
     items = [0] if items is None else items
     g = w.grids(items)
     quat = None if w.quat is None else w.quat[items]
-    I = sm.simulate(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat).cpu().numpy()
+    I = sm.simulate(dev(g), vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=METHODS[method][0],
+                    flags=METHODS[method][1]).cpu().numpy()
     for i in range(len(items)):
         flat = I[i].ravel()
-        c = w.npy // 2 * w.npx + w.npx // 2
-        pix = W.sample_pixels(w.seed + i, w.npix, count, always=[int(np.argmax(flat)), c, c - 1, c - w.npx, c - w.npx - 1])
-        ref = O.simulate(g[i], vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=None if quat is None else quat[i], pixels=pix)
-        assert_parity(flat[pix], ref, what=f"{w.name} item {items[i]} sampled")
+        pix = sampled_pixels(w, items[i], flat, FULL_SIZE_SAMPLES[idx])
+        ref = oracle_at_pixels(w, items[i], g[i], None if quat is None else quat[i], pix)
+        assert_parity(flat[pix], ref, what=f"{w.name} item {items[i]} sampled {method}")
 
 
 def test_cfg2_full_size_sampled(sm):
-    _sampled_full(sm, 1, 512)
+    _sampled_full(sm, 1)
 
 
 def test_cfg3_full_size_sampled(sm):
-    _sampled_full(sm, 2, 192)
+    _sampled_full(sm, 2)
 
 
 def test_cfg4_full_size_items_sampled(sm):
-    _sampled_full(sm, 3, 128, items=[0, 1, 2, 3, 4, 5, 6, 7, 8])
+    _sampled_full(sm, 3, items=[0, 1, 2, 3, 4, 5, 6, 7, 8])
 
 
-def test_cfg5_full_size_sampled(sm):
-    _sampled_full(sm, 4, 48)
+@pytest.mark.parametrize("method", ["tensor", "tensor_1cta"])
+def test_cfg5_full_size_sampled(sm, method):
+    """The 298-rad-phase, opaque-core stress case at full size (512^3 on 1024^2), both tensor kernels, 1024 + 9 pixels."""
+    _sampled_full(sm, 4, method=method)
