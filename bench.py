@@ -273,6 +273,25 @@ def measure_peaks(args):
     print(json.dumps(out), flush=True)
 
 
+# GEMM peaks measured on this pool with MEASURED_PEAKS.json's protocol (`python bench.py --measure-peaks`, profiles/r02_peaks.md):
+# the operand type of every contraction here is FP16 (kind::f16); context beside the driver-written BF16 figures.
+MEASURED_FP16 = {"burst": 1466.2, "sustained": 1286.0, "sm_mhz_under_load": 1207.0, "source": "profiles/r02_peaks.md"}
+PIPE_FLOP_PER_CLK_SM = 8192          # dense FP16/BF16 tensor flop per clock and SM (2250 TFLOP/s nominal = 148 SMs x 8192 x 1.855 GHz)
+
+
+def tensor_roofline_extras(achieved, clocks, peaks):
+    """Context for a tensor-bound roofline entry.  `frac` divides by MEASURED_PEAKS.json's bf16 BURST figure (the kernel is timed by
+    its own CUDA events; kind::f16 runs at the bf16 rate).  That cuBLAS figure was measured power-capped at ~1.3 GHz, so a kernel
+    that holds a higher clock can exceed it; `frac_of_pipe_ceiling` divides by what the tensor pipes can issue at the clock sampled
+    during THIS run and is <= 1 by construction."""
+    mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    ceiling = 148 * PIPE_FLOP_PER_CLK_SM * mhz * 1e6 / 1e12
+    return {"peak_sustained": peaks["sustained"], "frac_of_sustained": achieved / peaks["sustained"],
+            "peak_nominal": 2250.0, "frac_of_nominal": achieved / 2250.0,
+            "pipe_ceiling_at_sampled_clock": ceiling, "frac_of_pipe_ceiling": achieved / ceiling, "sampled_sm_mhz": mhz,
+            "peak_fp16_measured": MEASURED_FP16}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -285,7 +304,15 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=0, help="pixels per step of the CPU oracle sample (0 = sized for ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--graph", action="store_true",
-                    help="--route nufft only: capture one call in a CUDA graph after the warm-up and time its replays")
+                    help="capture one call in a CUDA graph after the warm-up and time its replays (routes pixels, qgrid, nufft)")
+    ap.add_argument("--reuse-tables", action="store_true",
+                    help="time with SCATMAN_FLAG_REUSE_TABLES (q-map and phase tables kept from the previous call); the default "
+                         "rebuilds them every step and reports the cached figure beside it")
+    ap.add_argument("--shard", default="items", choices=["items", "pixels"],
+                    help="N > 1: items = every rank runs the whole workload (weak scaling, the paper's scheme); pixels = every rank "
+                         "simulates its row band of the detector and rank 0 gathers the pattern (strong scaling)")
+    ap.add_argument("--e2e-batch", type=int, default=4,
+                    help="patterns per end-to-end call (the host entry points overlap upload, compute and download chunk by chunk)")
     ap.add_argument("--route", default="pixels", choices=["pixels", "qgrid", "shapes", "shapes_qgrid", "fit", "nufft", "shapes_nufft"],
                     help="pixels: the flat detector of BASELINE.json (default, the headline); qgrid: the separable route on a "
                          "uniform (qx, qy) grid of the same size and angular reach (scatman_simulate_qgrid); shapes: the particles "
@@ -308,6 +335,7 @@ def main():
     import numpy as np
     import torch
     from paper_2202_03411_b200 import binding as B, build as lib_build
+    from paper_2202_03411_b200.sharding import shard_detector_rows, shard_range
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -322,152 +350,187 @@ def main():
     if dist:
         dist.barrier()
     sm = B.Scatman(local)
+    shapes_route = args.route in ("shapes", "shapes_qgrid", "shapes_nufft")
+    shard_pixels = args.shard == "pixels"
+    if shard_pixels and args.route not in ("pixels", "nufft"):
+        raise SystemExit("--shard pixels applies to the flat-detector routes (pixels, nufft)")
 
     w, items = workload_for(args)
     vox = (w.dx, w.dy, w.dz)
-    # weak scaling: the global job is `world` copies of the batch; shapes shard across ranks with no collective
-    from paper_2202_03411_b200.sharding import shard_range
-    global_items = [i for _ in range(world) for i in items]
-    lo, hi = shard_range(len(global_items), rank, world)
-    items = global_items[lo:hi]
+    if shard_pixels:
+        # strong scaling: every rank holds the whole (small) volume and simulates its row band of the detector
+        y0, y1, cy_band = shard_detector_rows(w.npy, 0.0, rank, world)
+        npy_r = y1 - y0
+    else:
+        # weak scaling: the global job is `world` copies of the batch; shapes shard across ranks with no collective
+        global_items = [i for _ in range(world) for i in items]
+        lo, hi = shard_range(len(global_items), rank, world)
+        items = global_items[lo:hi]
+        y0, y1, cy_band, npy_r = 0, w.npy, 0.0, w.npy
     g = w.grids(items)
     quat = None if w.quat is None else w.quat[items]
     batch = len(items)
+    npix_r = npy_r * w.npx
     d_dn = torch.from_numpy(g).cuda()
     grid = B.Grid(w.nx, w.ny, w.nz, *vox)
+    det = B.Detector(w.npx, npy_r, w.theta_max_deg, 0.0, cy_band)
     opts = B.Options(0, args.method, 0, 0)
-    ws = torch.empty(sm.workspace_bytes(grid, w.npix, batch, opts), dtype=torch.uint8, device="cuda")
-    out = torch.empty((batch, w.npy, w.npx), dtype=torch.float32, device="cuda")
+    out = torch.empty((batch, npy_r, w.npx), dtype=torch.float32, device="cuda")
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
-
     qmethod = args.method if args.method in (0, 1, 3) else 0
+    qopts = B.Options(0, qmethod, 0, 0)
+    qx = qy = qx_h = qy_h = nq = shapes = None
+    need = C.c_size_t(0)
     if args.route in ("qgrid", "shapes_qgrid"):
         kk = 2 * np.pi / w.lam
-        qx = torch.from_numpy((np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)).cuda()
-        qy = torch.from_numpy((np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)).cuda()
-        need = C.c_size_t(0)
-        qmethod = args.method if args.method in (0, 1, 3) else 0
-        qopts = B.Options(0, qmethod, 0, 0)
-        sm._check(sm.lib.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
-        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
-
-    nq = None
-    if args.route in ("nufft", "shapes_nufft"):      # same flat detector, same result: 3-D type-2 NUFFT instead of the pixel x voxel contraction
-        det = B.Detector(w.npx, w.npy, w.theta_max_deg, 0.0, 0.0)
-        need = C.c_size_t(0)
-        sm._check(sm.lib.scatman_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)))
-        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+        qx_h = (np.arange(w.npx) + 0.5 - 0.5 * w.npx) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npx)
+        qy_h = (np.arange(w.npy) + 0.5 - 0.5 * w.npy) * (2 * kk * np.sin(np.radians(w.theta_max_deg)) / w.npy)
+        qx, qy = torch.from_numpy(qx_h).cuda(), torch.from_numpy(qy_h).cuda()
+    if shapes_route:
+        shapes = w.shapes(items)
+        if shapes is None:
+            raise SystemExit(f"{w.name} is not one shape per item: --route {args.route} does not apply")
+    L = sm.lib
+    ws_calls = {
+        "pixels": lambda: L.scatman_workspace_bytes(sm._ctx, C.byref(grid), npix_r, batch, C.byref(opts), C.byref(need)),
+        "qgrid": lambda: L.scatman_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)),
+        "nufft": lambda: L.scatman_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)),
+        "shapes": lambda: L.scatman_shapes_workspace_bytes(sm._ctx, C.byref(grid), npix_r, batch, C.byref(opts), C.byref(need)),
+        "shapes_qgrid": lambda: L.scatman_shapes_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)),
+        "shapes_nufft": lambda: L.scatman_shapes_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)),
+    }
+    sm._check(ws_calls[args.route]())
+    ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
+    if args.route in ("nufft", "shapes_nufft"):
         nq = sm.nufft_grid_dims(grid, w.lam, det)
+    dims = (w.nx, w.ny, w.nz)
+    gathered = [torch.empty((batch, (w.npy + world - 1) // world, w.npx), dtype=torch.float32, device="cuda") for _ in range(world)] \
+        if (shard_pixels and dist and rank == 0) else None
+    band_pad = torch.zeros((batch, (w.npy + world - 1) // world, w.npx), dtype=torch.float32, device="cuda") if (shard_pixels and dist) else None
 
-    shapes = None
-    if args.route == "shapes_qgrid":
-        shapes = w.shapes(items)
-        if shapes is None:
-            raise SystemExit(f"{w.name} is not one shape per item: --route shapes_qgrid does not apply")
-        need = C.c_size_t(0)
-        sm._check(sm.lib.scatman_shapes_qgrid_workspace_bytes(sm._ctx, C.byref(grid), w.npx, w.npy, batch, C.byref(qopts), C.byref(need)))
-        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
-    if args.route == "shapes_nufft":
-        shapes = w.shapes(items)
-        if shapes is None:
-            raise SystemExit(f"{w.name} is not one shape per item: --route shapes_nufft does not apply")
-        need = C.c_size_t(0)
-        sm._check(sm.lib.scatman_shapes_nufft_workspace_bytes(sm._ctx, C.byref(grid), w.lam, C.byref(det), batch, C.byref(need)))
-        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
-    if args.route == "shapes":
-        shapes = w.shapes(items)
-        if shapes is None:
-            raise SystemExit(f"{w.name} is not one shape per item: --route shapes does not apply")
-        need = C.c_size_t(0)
-        sm._check(sm.lib.scatman_shapes_workspace_bytes(sm._ctx, C.byref(grid), w.npix, batch, C.byref(opts), C.byref(need)))
-        ws = torch.empty(int(need.value), dtype=torch.uint8, device="cuda")
-
-    def step():
+    def step(flags=0, st=stream):
         if args.route == "shapes":
-            sm.simulate_shapes(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method,
-                               workspace=ws, out=out, stream=stream)
-            return
-        if args.route == "shapes_qgrid":
-            sm.simulate_shapes_qgrid(shapes, (w.nx, w.ny, w.nz), vox, w.lam, qx, qy, method=qmethod, workspace=ws, out=out,
-                                     stream=stream)
-            return
-        if args.route == "qgrid":
-            sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=stream)
-            return
-        if args.route == "shapes_nufft":
-            sm.simulate_shapes_nufft(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, workspace=ws, out=out,
-                                     stream=stream)
-            return
-        if args.route == "nufft":
-            sm.simulate_nufft(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, workspace=ws, out=out, stream=stream)
-            return
-        sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method,
-                    workspace=ws, out=out, stream=stream)
+            sm.simulate_shapes(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method, workspace=ws, out=out,
+                               stream=st, flags=flags)
+        elif args.route == "shapes_qgrid":
+            sm.simulate_shapes_qgrid(shapes, dims, vox, w.lam, qx, qy, method=qmethod, workspace=ws, out=out, stream=st)
+        elif args.route == "qgrid":
+            sm.simulate_qgrid(d_dn, vox, w.lam, qx, qy, quat=quat, method=qmethod, workspace=ws, out=out, stream=st, flags=flags)
+        elif args.route == "shapes_nufft":
+            sm.simulate_shapes_nufft(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg, workspace=ws, out=out, stream=st)
+        elif args.route == "nufft":
+            sm.simulate_nufft(d_dn, vox, w.lam, w.npx, npy_r, w.theta_max_deg, quat=quat, cy=cy_band, workspace=ws, out=out, stream=st,
+                              flags=flags)
+        else:
+            sm.simulate(d_dn, vox, w.lam, w.npx, npy_r, w.theta_max_deg, quat=quat, method=args.method, cy=cy_band, workspace=ws,
+                        out=out, stream=st, flags=flags)
+        if band_pad is not None:       # pixel sharding: rank 0 gathers the row bands (NCCL gather of equal-sized padded bands)
+            band_pad[:, :npy_r] = out
+            dist.gather(band_pad, gathered, dst=0)
 
+    def timed(nsteps, flags=0, graph=None):
+        """nsteps steps, L2 flushed before each (outside its events); returns (total ms, launches, contraction ms per step)."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        k_ms, n = [], 0
+        torch.cuda.synchronize()
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            if graph is not None:
+                graph.replay()
+                b.record(stream)
+                continue
+            step(flags)
+            b.record(stream)
+            n += sm.last_launch_count()
+            k_ms.append(sm.last_contraction_ms())   # the library's events on the launch stream; waits for this step
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev), n, k_ms
+
+    base_flags = B.FLAG_REUSE_TABLES if args.reuse_tables else 0
     for _ in range(args.warmup):
         flush.zero_()
-        step()
+        step(base_flags)
     torch.cuda.synchronize()
+    graph = None
+    graph_launches = 0
+    if args.graph:
+        if shapes_route or dist:
+            raise SystemExit("--graph applies to the single-GPU routes pixels, qgrid, nufft")
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):      # the call only enqueues on the capturing stream: the whole step becomes one graph
+            step(base_flags, st=None)
+        graph_launches = sm.last_launch_count()
+        graph.replay()
+        torch.cuda.synchronize()
     if dist:
         dist.barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kernel_ms, launches = [], 0
-    torch.cuda.synchronize()
-    graph = None
-    if args.graph:
-        if args.route != "nufft":
-            raise SystemExit("--graph applies to --route nufft")
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):      # the call only enqueues on the capturing stream: the whole step becomes one graph
-            sm.simulate_nufft(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, workspace=ws, out=out)
-        graph_launches = sm.last_launch_count()
-        graph.replay()
-        torch.cuda.synchronize()
-    for i in range(args.steps):
-        flush.zero_()                      # L2 flush, outside the timed events
-        ev[i][0].record(stream)
-        if graph is not None:
-            graph.replay()
-            ev[i][1].record(stream)
-            launches += graph_launches
-            continue
-        step()
-        ev[i][1].record(stream)
-        launches += sm.last_launch_count()
-        kernel_ms.append(sm.last_contraction_ms())   # events on the launch stream; waits for this step
-    torch.cuda.synchronize()
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    total_ms, launches, kernel_ms = timed(args.steps, base_flags, graph)
+    if graph is not None:
+        launches = graph_launches * args.steps
     if dist:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
         dist.barrier()
     clocks = sampler.stop() if rank == 0 else None
+    # the same step with the phase tables of the previous call kept (SCATMAN_FLAG_REUSE_TABLES): reported beside the headline
+    cached = None
+    if not args.reuse_tables and graph is None and not shapes_route and not dist:
+        step(B.FLAG_REUSE_TABLES)
+        c_ms, _, _ = timed(min(args.steps, 5), B.FLAG_REUSE_TABLES)
+        cached = {"ms_per_step": c_ms / min(args.steps, 5), "value": batch * min(args.steps, 5) / (c_ms * 1e-3), "unit": "patterns/s",
+                  "what": "same step with SCATMAN_FLAG_REUSE_TABLES: q-map and phase tables kept from the previous call"}
 
-    # end to end through the host-buffer C entry point: pinned host grid in, pinned host intensity out
-    h_dn = torch.from_numpy(g).pin_memory()
-    h_I = torch.empty((batch, w.npy, w.npx), dtype=torch.float32).pin_memory()
-    e2e_steps = max(1, min(args.steps, 3))
+    # ---- end to end through the host-buffer C entry points: pinned host grids in, pinned host patterns out, every step
+    e2e = None
+    if shapes_route:
+        # the inputs ARE the descriptors (host structs, marshalled per call); the patterns come back to pinned host memory
+        h_I = torch.empty((batch, npy_r, w.npx), dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
 
-    def e2e_step():
-        if args.route in ("shapes", "shapes_qgrid", "shapes_nufft"):  # the inputs are the descriptors (host structs, marshalled per call); results to pinned host
+        def e2e_step():
             step()
             h_I.copy_(out, non_blocking=True)
             torch.cuda.synchronize()
-        elif args.route in ("qgrid", "nufft"):   # no host-buffer C entry point for this route: the copies go through torch
-            d_dn.copy_(h_dn, non_blocking=True)
-            step()
-            h_I.copy_(out, non_blocking=True)
-            torch.cuda.synchronize()
-        else:
-            sm.simulate_host(h_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, h_out=h_I)
+        e2e_batch = batch
+        h2d = int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes))
+        copy_bound = None
+    else:
+        e2e_batch = batch if batch >= args.e2e_batch else args.e2e_batch      # small batches are replicated: the pipeline needs chunks
+        rep = (e2e_batch + batch - 1) // batch
+        e2e_batch = rep * batch
+        h_dn = torch.from_numpy(np.concatenate([g] * rep)).pin_memory()
+        quat_e = None if quat is None else np.concatenate([quat] * rep)
+        h_I = torch.empty((e2e_batch, npy_r, w.npx), dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
 
+        def e2e_step():
+            if args.route == "qgrid":
+                sm.simulate_qgrid_host(h_dn, vox, w.lam, qx_h, qy_h, quat=quat_e, method=qmethod, h_out=h_I)
+            elif args.route == "nufft":
+                sm.simulate_nufft_host(h_dn, vox, w.lam, w.npx, npy_r, w.theta_max_deg, quat=quat_e, h_out=h_I, cy=cy_band)
+            else:
+                sm.simulate_host(h_dn, vox, w.lam, w.npx, npy_r, w.theta_max_deg, quat=quat_e, method=args.method, h_out=h_I, cy=cy_band)
+        h2d = int(h_dn.numel() * 4)
+        # the copy bound: the same bytes through one pinned H2D copy and one D2H copy, nothing else
+        d_tmp = torch.empty_like(h_dn, device="cuda")
+        d_tmp.copy_(h_dn, non_blocking=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        d_tmp.copy_(h_dn, non_blocking=True)
+        torch.cuda.synchronize()
+        copy_s = time.perf_counter() - t0
+        del d_tmp
+        copy_bound = {"h2d_s": copy_s, "h2d_gbps": h2d / copy_s / 1e9, "patterns_per_s": e2e_batch / copy_s}
     e2e_step()
+    if dist:
+        dist.barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         e2e_step()
@@ -478,14 +541,22 @@ def main():
         e2e_s = float(t.item())
     if rank != 0:
         return
+    e2e_patterns = e2e_batch * e2e_steps * (1 if shard_pixels else world)
+    e2e = {"value": e2e_patterns / e2e_s, "unit": "patterns/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(h_I.numel() * 4),
+           "patterns_per_step": e2e_batch, "copy_bound": copy_bound,
+           "through": "descriptors marshalled per call + pattern read-back" if shapes_route else
+                      {"pixels": "scatman_simulate_host", "nufft": "scatman_simulate_nufft_host", "qgrid": "scatman_simulate_qgrid_host"}[args.route]}
+    if copy_bound:
+        e2e["frac_of_copy_bound"] = e2e["value"] / (copy_bound["patterns_per_s"] * (1 if shard_pixels else world))
 
-    patterns = batch * args.steps * world
+    patterns = batch * args.steps * (1 if shard_pixels else world)
     value = patterns / (total_ms * 1e-3)
     terms_per_pattern = w.nvox * w.npix
+    terms_issued_per_pattern = None
     peaks = load_peaks()
     # graph replays have no per-kernel events: the roofline then takes the WHOLE step (a1, a2 and tables included) as the kernel time
     k_ms = sum(kernel_ms) / len(kernel_ms) if kernel_ms else total_ms / args.steps
-    dense = SPLITS * FLOP_PER_TERM * terms_per_pattern * batch           # tensor flop of the dense sum per launch
+    dense = SPLITS * FLOP_PER_TERM * w.nvox * npix_r * batch           # tensor flop of the dense sum per launch (this rank's pixels)
     if args.route in ("qgrid", "shapes_qgrid"):
         dense_sep = 8.0 * batch * (w.nz * w.ny * w.nx * w.npx + w.nz * w.npy * w.ny * w.npx)   # both stages, 8 flop per complex MAC
         if qmethod == 3:
@@ -509,62 +580,57 @@ def main():
                 blk = occ.reshape(w.nz, NY // 64, 64).any(axis=2)                 # live 64-y blocks
                 grp = blk.reshape(w.nz, NY // 128, 2).any(axis=2)                 # live 128-y row tiles of stage X
                 issued += 24.0 * (grp.sum() * 128.0 * NXP * NPXP + blk.sum() * 64.0 * NPYP * NPXP)
-            peak = peaks["sustained"]
             ach = issued / (k_ms * 1e-3) / 1e12
-            roofline = {"bound": "tensor", "kernel": "sep_tc_x2_kernel + sep_tc_yzt_kernel (stage X + stage YZ variants of sep_tensor_kernels.cu)", "achieved": ach, "peak": peak,
-                        "unit": "TFLOP/s", "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
-                        "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
+            roofline = {"bound": "tensor", "kernel": "sep_tc_x2_kernel + sep_tc_yzt_kernel (stage X + stage YZ variants of sep_tensor_kernels.cu)",
+                        "achieved": ach, "peak": peaks["burst"], "unit": "TFLOP/s", "frac": ach / peaks["burst"], "traffic": None, "kernel_ms": k_ms,
+                        "peak_source": f"MEASURED_PEAKS.json bf16 burst ({peaks['source']}); kind::f16 runs at the bf16 rate",
                         "achieved_is": "issued tensor flop (24 per complex MAC of the live tiles: 8 flop x 3 split products) / "
-                                       "CUDA-event time of the per-item launches (pack, stage X, stage YZ, finalize)",
+                                       "CUDA-event time of the per-chunk launches (pack, stage X, stage YZ, finalize)",
                         "issued_fraction_of_dense": issued / (3.0 * dense_sep),
-                        "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12}
+                        "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12, **tensor_roofline_extras(ach, clocks, peaks)}
     elif args.route in ("nufft", "shapes_nufft"):
-        # three FP64 complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 10^3-point interpolation, CUDA cores:
+        # three complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 10^3-point interpolation:
         # 8 flop per complex MAC of the GEMMs, 4 per (real weight x complex value) MAC of the interpolation.
         nqx, nqy, nqz = nq
-        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * w.npix * 10 ** 3)
+        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * npix_r * 10 ** 3)
         peak = 148 * 64 * 2 * 1.965e9 / 1e12           # FP64 FMA: 148 SMs x 64 lanes x 2 flop x max clock
         ach = flop / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "nufft_zgemm_kernel (stages Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,
+        roofline = {"bound": "alu", "kernel": "NUFFT stages (GEMMs Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,
                     "unit": "TFLOP/s", "frac": ach / peak, "traffic": NCU_DRAM_BYTES_NUFFT.get(w.name) if batch == 1 else None,
                     "kernel_ms": k_ms, "uniform_grid": [nqz, nqy, nqx],
-                    "achieved_is": "dense FP64 flop of the three GEMM stages and the interpolation / their CUDA-event time; K steps over "
-                                   "vacuum are skipped, so the ALUs executed less than this (ncu: FP64 pipe 50-59 % active in the GEMMs)",
+                    "achieved_is": "dense flop of the three GEMM stages (8 per complex MAC) and the interpolation / their CUDA-event time, "
+                                   "against the FP64 ALU peak the interpolation runs on",
                     "flop_vs_pixel_route": flop / (FLOP_PER_TERM * terms_per_pattern * batch)}
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
         # One extra, untimed call with the counting flag (same inputs, same schedule).
-        if args.route == "shapes":
-            sm.simulate_shapes(shapes, (w.nx, w.ny, w.nz), vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method,
-                               workspace=ws, out=out, stream=stream, flags=B.FLAG_COUNT_ISSUED)
-        else:
-            sm.simulate(d_dn, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, method=args.method, workspace=ws, out=out,
-                        stream=stream, flags=B.FLAG_COUNT_ISSUED)
+        step(B.FLAG_COUNT_ISSUED) if args.route == "pixels" else \
+            sm.simulate_shapes(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg, method=args.method, workspace=ws, out=out,
+                               stream=stream, flags=B.FLAG_COUNT_ISSUED)
         blocks = sm.last_issued_blocks()
-        npix_pad = (w.npix + 255) // 256 * 256
+        npix_pad = (npix_r + 255) // 256 * 256
         issued = blocks * 256 * npix_pad * SPLITS * FLOP_PER_TERM         # tensor flop per contraction launch
+        terms_issued_per_pattern = blocks * 256 * npix_pad / batch
         achieved = issued / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "tensor", "kernel": "msft_contract_kernel", "achieved": achieved, "peak": peaks["sustained"],
-                    "unit": "TFLOP/s", "frac": achieved / peaks["sustained"],
-                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name),
-                    "peak_source": f"MEASURED_PEAKS.json bf16 sustained ({peaks['source']}); kind::f16 runs at the bf16 rate",
+        roofline = {"bound": "tensor", "kernel": "msft_contract_kernel", "achieved": achieved, "peak": peaks["burst"],
+                    "unit": "TFLOP/s", "frac": achieved / peaks["burst"],
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if not shard_pixels or world == 1 else None,
+                    "peak_source": f"MEASURED_PEAKS.json bf16 burst ({peaks['source']}): the kernel is timed alone by its own CUDA "
+                                   "events; kind::f16 runs at the bf16 rate",
                     "achieved_is": "issued tensor flop (24 per issued voxel-pixel term: 8 flop x 3 split products) / kernel time",
                     "issued_fraction_of_dense": issued / dense, "dense_equivalent_tflops": dense / (k_ms * 1e-3) / 1e12,
                     "useful_dense_tflops": dense / SPLITS / (k_ms * 1e-3) / 1e12, "kernel_ms": k_ms,
-                    "kernel_share_of_step": k_ms * args.steps / total_ms,
-                    # context: the measured cuBLAS peak is power-limited (SM clock ~1.3 GHz under its load); this kernel skips
-                    # vacuum, draws less power and holds the full clock, hence frac > 1.  Nominal dense FP16/BF16 is 2250 TFLOP/s.
-                    "peak_nominal": 2250.0, "frac_of_nominal": achieved / 2250.0, "peak_burst": peaks["burst"]}
+                    "kernel_share_of_step": k_ms * args.steps / total_ms, **tensor_roofline_extras(achieved, clocks, peaks)}
     elif args.method == 3:
         # FP32 FMA against phase tables: 8 flop per term (dense count; vacuum y chunks are skipped); FP32 peak as for qgrid
         peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        ach = FLOP_PER_TERM * terms_per_pattern * batch / (k_ms * 1e-3) / 1e12
+        ach = FLOP_PER_TERM * w.nvox * npix_r * batch / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "simt_table_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                     "frac": ach / peak, "traffic": None, "kernel_ms": k_ms}
     else:
         # direct sincos: 2 MUFU per term; SFU peak = 148 SMs x 16 MUFU/clk x max clock
         peak = 148 * 16 * 1.965e9 / 2 / 1e12
-        ach = terms_per_pattern * batch / (k_ms * 1e-3) / 1e12
+        ach = w.nvox * npix_r * batch / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "simt_sincos_kernel", "achieved": ach, "peak": peak, "unit": "Tterm/s",
                     "frac": ach / peak, "traffic": None, "kernel_ms": k_ms}
 
@@ -572,26 +638,26 @@ def main():
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         from paper_2202_03411_b200 import workloads as W
-        # size the sample for ~15 s of host-core work from a short probe
+        # size the sample for ~15 s of host-core work from a short probe; pixels of THIS rank's band, in full-detector numbering
         g0, q0 = g[0], (None if quat is None else quat[0])
         if args.route in ("shapes", "shapes_nufft"):     # the oracle's own rendering of item 0 (already in the beam frame)
             from oracle import render as OR
-            g0, q0 = OR.render(shapes[0], (w.nx, w.ny, w.nz), vox), None
+            g0, q0 = OR.render(shapes[0], dims, vox), None
         probe = W.sample_pixels(w.seed + 99, w.npix, 32)
         t0 = time.perf_counter()
         O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=probe)
         per_pixel = (time.perf_counter() - t0) / len(probe)
         npix_s = args.ref_pixels if args.ref_pixels > 0 else int(min(8192, max(256, 15.0 / per_pixel)))
-        pix = W.sample_pixels(w.seed, w.npix, npix_s)
+        pix = W.sample_pixels(w.seed, npix_r, npix_s) + y0 * w.npx
         t0 = time.perf_counter()
         ref = O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=pix)
         dt = time.perf_counter() - t0
         if args.route == "qgrid":
-            qg, okg = O.qgrid_q(qx.cpu().numpy(), qy.cpu().numpy(), w.lam)
+            qg, okg = O.qgrid_q(qx_h, qy_h, w.lam)
             t0 = time.perf_counter()
             ref = O.simulate_q(g0, vox, w.lam, qg[pix], quat=q0) * okg[pix]
             dt = time.perf_counter() - t0
-        got = out[0].flatten()[torch.from_numpy(pix).cuda()].cpu().numpy().astype(np.float64)
+        got = out[0].flatten()[torch.from_numpy(pix - y0 * w.npx).cuda()].cpu().numpy().astype(np.float64)
         rel = float(np.sqrt(np.sum((got - ref) ** 2) / np.sum(ref ** 2)))
         m = ref > 1e-6 * ref.max()
         pixerr = float(np.max(np.abs(got[m] - ref[m]) / ref[m]))
@@ -599,16 +665,26 @@ def main():
                "sample": f"{len(pix)} seeded pixels of item 0 of {w.name} ({dt:.1f} s)",
                "terms_per_s": w.nvox * len(pix) / dt, "parity_rel_l2": rel, "parity_max_pixel_rel": pixerr}
 
+    if args.route in ("nufft", "shapes_nufft"):
+        dtype, method_name = "fp16x3 split GEMM stages (fp32 accumulate) + f64 interpolation", "nufft"
+    elif args.route in ("qgrid", "shapes_qgrid"):
+        dtype, method_name = ("f32", "separable_simt") if qmethod == 3 else ("fp16x3 split (fp32 accumulate)", "separable_tensor")
+    else:
+        dtype = "fp16x3 split (fp32 accumulate)" if args.method == 1 else "f32"
+        method_name = {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method]
+    parallelism = f"replicas x{world}" if not shard_pixels else f"detector row bands x{world} (rank 0: rows {y0}..{y1 - 1}), pattern gathered on rank 0"
     line = {"metric": "msft_patterns_per_s", "value": value, "unit": "patterns/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if args.route in ("nufft", "shapes_nufft") else "f32" if (args.route in ("qgrid", "shapes_qgrid") and qmethod == 3) or (args.route not in ("qgrid", "shapes_qgrid") and args.method != 1) else "fp16x3 split (fp32 accumulate)", "data": "synthetic",
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong" if shard_pixels else "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nz, w.ny, w.nx], "detector": [w.npy, w.npx], "batch": batch,
-                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "cuda_graph": bool(args.graph), "method": ("separable_simt" if qmethod == 3 else "separable_tensor") if args.route in ("qgrid", "shapes_qgrid") else "nufft_fp64" if args.route in ("nufft", "shapes_nufft") else {1: "tensor", 2: "simt_sincos", 3: "simt_table"}[args.method],
-                       "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": f"replicas x{world}"},
-            "terms_per_s": value * terms_per_pattern, "roofline": roofline, "cpu_baseline": cpu,
-            "e2e": {"value": batch * e2e_steps * world / e2e_s, "unit": "patterns/s",
-                    "h2d_bytes_per_step": int(h_dn.numel() * 4) if args.route not in ("shapes", "shapes_qgrid", "shapes_nufft") else int(C.sizeof(B.Shape) * batch + sum(24 * len(sh.get("coeffs", ())) for sh in shapes)),
-                    "d2h_bytes_per_step": int(h_I.numel() * 4)},
+                       "lambda": w.lam, "theta_max_deg": w.theta_max_deg, "route": args.route, "cuda_graph": bool(args.graph),
+                       "reuse_tables": bool(args.reuse_tables), "method": method_name, "shard": args.shard,
+                       "l2": "flushed between steps (192 MiB write); inputs 134 MB > L2", "parallelism": parallelism},
+            # the term rate of the work really multiplied (the contraction skips vacuum); the dense-grid count of north_star beside it
+            "terms_per_s": value * (terms_issued_per_pattern if terms_issued_per_pattern else terms_per_pattern),
+            "terms_per_s_dense_equivalent": value * terms_per_pattern,
+            "terms_counted": "issued (voxel, pixel) terms" if terms_issued_per_pattern else "dense grid (this route does not issue per-term work)",
+            "roofline": roofline, "with_table_cache": cached, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line), flush=True)
 

@@ -516,13 +516,13 @@ class Scatman:
         return out
 
     def simulate_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
-                      rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None, flags: int = 0):
+                      rho_mode: int = RHO_LINEAR, method: int = METHOD_AUTO, h_out=None, flags: int = 0, cx: float = 0.0, cy: float = 0.0):
         """Host-buffer end-to-end call: h_dn / h_out are CPU float32 tensors (pinned for speed). Synchronous."""
         import torch
         if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
             raise ValueError("h_dn must be a contiguous CPU float32 tensor")
         grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
-        det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
         opts = Options(int(rho_mode), int(method), 0, int(flags))
         if h_out is None:
             h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
@@ -532,13 +532,13 @@ class Scatman:
         return h_out
 
     def simulate_nufft_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
-                            rho_mode: int = RHO_LINEAR, h_out=None):
+                            rho_mode: int = RHO_LINEAR, h_out=None, cx: float = 0.0, cy: float = 0.0):
         """scatman_simulate_nufft_host: host tensors in and out, upload / compute / download overlapped chunk by chunk."""
         import torch
         if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
             raise ValueError("h_dn must be a contiguous CPU float32 tensor")
         grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
-        det = Detector(int(npx), int(npy), float(theta_max_deg), 0.0, 0.0)
+        det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
         opts = Options(int(rho_mode), 0, 0, 0)
         if h_out is None:
             h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()

@@ -18,8 +18,11 @@ def shard_range(n: int, rank: int, world: int) -> Tuple[int, int]:
     return lo, lo + base + (1 if rank < rem else 0)
 
 
-def shard_pixel_tiles(npix: int, rank: int, world: int, tile: int = 128) -> Tuple[int, int]:
-    """Pixel range [lo, hi) owned by `rank`, aligned to whole 128-pixel tiles of the contraction kernel."""
-    ntiles = (npix + tile - 1) // tile
-    t0, t1 = shard_range(ntiles, rank, world)
-    return min(t0 * tile, npix), min(t1 * tile, npix)
+def shard_detector_rows(npy: int, cy: float, rank: int, world: int) -> Tuple[int, int, float]:
+    """Pixel sharding ("partition pixel tiles across GPUs, each GPU writes its slice of I"): rank `rank` of `world`
+    simulates the rows [y0, y1) of the flat detector.  A row band IS a detector of the C ABI: same npx, theta_max_deg and cx
+    (the pixel pitch depends on npx only), npy = y1 - y0 rows and the centre offset cy_band returned here, which puts band row
+    iy at the v of full-detector row y0 + iy:  (iy + 1/2 - (y1-y0)/2 + cy_band) = (y0 + iy + 1/2 - npy/2 + cy).
+    Returns (y0, y1, cy_band); bands are contiguous, balanced, disjoint and cover every row."""
+    y0, y1 = shard_range(npy, rank, world)
+    return y0, y1, float(y0) - 0.5 * float(npy) + 0.5 * float(y1 - y0) + float(cy)

@@ -347,6 +347,26 @@ def test_host_entry_points_pipeline_matches_device_paths(sm):
             assert_parity(I_h[b].numpy(), ref, what=f"host pixels item {b}")
 
 
+@pytest.mark.parametrize("route", ["pixels", "nufft"])
+def test_detector_row_bands_equal_the_full_detector(sm, route):
+    """Pixel sharding on one device: the row bands of shard_detector_rows (each a detector of the C ABI with its own npy and
+    cy), run back to back and stacked, give the full-detector pattern (ragged band sizes, off-axis detector)."""
+    from paper_2202_03411_b200.sharding import shard_detector_rows
+    g = W.random_grid(91, 60, 44, 20, fill=0.4)
+    vox, lam, npx, npy, th, cx, cy = (2.0, 2.0, 2.5), 12.0, 37, 29, 35.0, 1.5, -2.0
+    run = sm.simulate if route == "pixels" else sm.simulate_nufft
+    full = run(dev(g), vox, lam, npx, npy, th, cx=cx, cy=cy).cpu().numpy()
+    for world in (2, 3):
+        bands = []
+        for r in range(world):
+            y0, y1, cyb = shard_detector_rows(npy, cy, r, world)
+            bands.append(run(dev(g), vox, lam, npx, y1 - y0, th, cx=cx, cy=cyb).cpu().numpy())
+        stacked = np.concatenate(bands, axis=0)
+        assert stacked.shape == full.shape
+        assert_parity(stacked, full, l2_tol=2e-6, pix_tol=5e-5, what=f"{route} bands x{world} vs full")
+    assert_parity(full, O.simulate(g, vox, lam, npx, npy, th, cx=cx, cy=cy), what=f"{route} off-axis full")
+
+
 def test_simulate_host_matches_device_path(sm):
     import torch
     w = W.config(0)
