@@ -16,6 +16,14 @@ SOURCES = ["api.cu", "fit_kernels.cu", "nufft_kernels.cu", "prep_kernels.cu", "r
            "sep_kernels.cu", "sep_tensor_kernels.cu", "simt_kernels.cu", "tensor_kernel.cu"]
 HEADERS = ["internal.h", "ptx_sm100.h", os.path.join("..", "..", "include", "scatman.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17"]
+# SCATMAN_CHECKED=1: the same library with device-side checks compiled in (mbarrier watchdog, bounds assertions before stores
+# and TMA loads; csrc/ptx_sm100.h).  compute-sanitizer is not available on the GPU pool, so this is the build the sanitize
+# subset of the tests runs on (profiles/r02_sanitizers.md).  Objects go to their own directory; the output is still LIB.
+CHECKED = os.environ.get("SCATMAN_CHECKED", "") not in ("", "0")
+if CHECKED:
+    NVCC_FLAGS = NVCC_FLAGS + ["-DSCATMAN_CHECKED"]
+    OBJ = os.path.join(CSRC, "build_checked")
+STAMP = LIB + ".mode"                # which mode LIB was last linked in ("checked" / "normal"); travels with LIB
 
 
 def _sources():
@@ -29,6 +37,8 @@ def _headers_mtime() -> float:
 def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
+    if not os.path.exists(STAMP) or open(STAMP).read().strip() != ("checked" if CHECKED else "normal"):
+        return True                  # LIB was linked in the other mode
     t = os.path.getmtime(LIB)
     return _headers_mtime() > t or any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in _sources())
 
@@ -53,6 +63,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(compile_one, _sources()))
     subprocess.run([nvcc, *NVCC_FLAGS, "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB, *objs], check=True)
+    with open(STAMP, "w") as f:
+        f.write("checked\n" if CHECKED else "normal\n")
     return LIB
 
 

@@ -3,6 +3,7 @@
 // Bit layouts follow the PTX ISA "tcgen05" chapter (matrix descriptor, instruction descriptor).
 #pragma once
 #include <cstdint>
+#include <cstdio>
 
 namespace scatman {
 namespace ptx {
@@ -45,10 +46,37 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+#ifdef SCATMAN_CHECKED
+// Checked build (SCATMAN_CHECKED=1 python -m paper_2202_03411_b200.build; profiles/r02_sanitizers.md): a barrier that does not
+// complete within ~2 s of SM clock is a protocol error (a lost arrival, a wrong phase, a transaction count that never adds up).
+// Report which barrier of which CTA and trap, instead of hanging the GPU.
+static __device__ __noinline__ void mbar_timeout(uint64_t *bar, uint32_t parity, int line) {
+    printf("scatman checked build: mbarrier wait timed out: block %d thread %d smem 0x%x parity %u (ptx_sm100.h caller line %d)\n",
+           (int)blockIdx.x, (int)threadIdx.x, smem_u32(bar), parity, line);
+    __trap();
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity, int line = __builtin_LINE()) {
+    if (mbar_try_wait(bar, parity)) return;
+    const long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+        if (clock64() - t0 > 4000000000ll) mbar_timeout(bar, parity, line);
+    }
+}
+#define SCATMAN_ASSERT(cond)                                                                                              \
+    do {                                                                                                                  \
+        if (!(cond)) {                                                                                                    \
+            printf("scatman checked build: %s:%d: assertion `%s` failed (block %d thread %d)\n", __FILE__, __LINE__, #cond, \
+                   (int)blockIdx.x, (int)threadIdx.x);                                                                    \
+            __trap();                                                                                                     \
+        }                                                                                                                 \
+    } while (0)
+#else
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
     }
 }
+#define SCATMAN_ASSERT(cond) ((void)0)
+#endif
 
 // ---- TMA ---------------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_prefetch_desc(const void *tmap) {

@@ -417,6 +417,7 @@ sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                     ptx::mbar_wait(t_full + buf, upar);
                     ptx::tc_fence_after();
                     const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
+                    SCATMAN_ASSERT(j >= 0 && j < P.nz && a0 + kCols <= P.NPXP && g * kM + kM <= P.NY);
                     __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
 #pragma unroll 1
                     for (int c0 = 0; c0 < kCols; c0 += 8) {
@@ -654,6 +655,7 @@ sep_tc_x2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
+                SCATMAN_ASSERT(j >= 0 && j < P.nz && a0 + NX <= P.NPXP && g * kM + kM <= P.NY);
                 __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
 #pragma unroll 1
                 for (int c0 = 0; c0 < NX; c0 += 8) {
@@ -1811,6 +1813,7 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             uint32_t m;
             while (un.next(n, m)) {
                 const int j = z0 + n - bi * P.nz;
+                SCATMAN_ASSERT(j >= 0 && j < P.nz && bi < P.nb && sp < P.nzs);
                 const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
                 const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
                 ptx::mbar_wait(t_full + buf, upar);

@@ -249,6 +249,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                         void *dst = sB + slot * kSlotB;
                         const int cg = uxt * 16 + (NCTA == 2 ? (int)rank * 8 + xa : 0);
                         const int cs = (ub * P.nz + uj) * P.ny16 + it.g * (kGroupYB * kBlockY / 16) + yi;
+                        SCATMAN_ASSERT(xm >= 1 && xm <= 8 && xa >= 0 && xa + xm <= 8);
+                        SCATMAN_ASSERT(ub < P.batch && uj < P.nz && cs < P.batch * P.nz * P.ny16 && cg + (NCTA == 2 ? xm : 16) <= P.nxt * 16);
                         if (NCTA == 2) ptx::tma_load_4d_2sm(dst, tmb, b_full + slot, 0, 0, cg, cs);
                         else ptx::tma_load_4d(dst, tmb, b_full + slot, 0, 0, cg, cs);
                     }
@@ -389,6 +391,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             // 64-bit fixed-point fraction of a turn, so the integer product wraps modulo one turn for free; its top 32 bits go
             // to the SFU as an angle in [-pi, pi) (error <= 2^-32 turn + 4e-7 rad of __sincosf, for any nz).
             const unsigned long long zt = __ldg(P.zturn + (size_t)tile * kTileP + el);
+            SCATMAN_ASSERT(tile < P.ntiles && it.g < P.ngroups && it.s < P.nzs && b1 <= P.batch);
             float2 *partial_t = P.partial + (size_t)(it.g * P.nzs + it.s) * P.npix_pad + (size_t)tile * kTileP + el;
             const size_t partial_b = (size_t)(P.ngroups * P.nzs) * P.npix_pad;   // stride between batch items
             // Flat walk over the non-empty units; f = row-dot of the current slice, acc = amplitude of the current
@@ -411,6 +414,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                             acc_im = fmaf(mz.y, f_re, acc_im);
                             f_re = 0.f;
                             f_im = 0.f;
+                            SCATMAN_ASSERT(ub >= cb && ub < b1 && uj >= 0 && uj < P.nz);
                             for (; cb < ub; ++cb) {                 // finished (or empty) batch items
                                 partial_t[(size_t)cb * partial_b] = make_float2(acc_re, acc_im);
                                 acc_re = 0.f;

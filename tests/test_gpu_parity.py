@@ -252,23 +252,26 @@ def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
     for name, run in routes.items():
         ws = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
         ws2 = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
-        fresh = lambda g, lam=w.lam, th=30.0: run(g, lam, th, ws2, 0).clone()       # tables rebuilt, other workspace
-        a = run(g1, w.lam, 30.0, ws, 0).clone()
+        # references first: every one rebuilds its tables (no flag) in another workspace
+        ref = {(gi, lam, th): run(g, lam, th, ws2, 0).clone()
+               for gi, g in (("g1", g1), ("g2", g2), ("g3", g3)) for lam, th in ((w.lam, 30.0), (0.8 * w.lam, 30.0), (0.8 * w.lam, 25.0))}
         n_full = sm.last_launch_count()
-        b = run(g1, w.lam, 30.0, ws, R).clone()                                     # same everything: tables reused
-        n_reuse = sm.last_launch_count()
-        assert n_reuse < n_full, (name, n_reuse, n_full)
-        assert torch.equal(a, b), name
-        assert torch.equal(run(g2, w.lam, 30.0, ws, R), fresh(g2)), name            # new particle, same tables
-        assert sm.last_launch_count() == n_reuse
-        assert torch.equal(run(g3, w.lam, 30.0, ws, R), fresh(g3)), name            # another batch size: same tables (they sit first)
-        assert torch.equal(run(g2, 0.8 * w.lam, 30.0, ws, R), fresh(g2, lam=0.8 * w.lam)), name   # lambda changed: rebuilt
-        assert sm.last_launch_count() == n_full
-        assert torch.equal(run(g2, 0.8 * w.lam, 25.0, ws, R), fresh(g2, lam=0.8 * w.lam, th=25.0)), name   # detector / qx changed
-        assert sm.last_launch_count() == n_full
-        run(g2, 0.8 * w.lam, 25.0, ws2, R)                                          # other workspace: rebuilt there
-        assert sm.last_launch_count() == n_full
-        assert torch.equal(run(g1, w.lam, 30.0, ws, R), a), name                    # back: key differs from the last call's -> rebuilt
+        seq = [(g1, "g1", w.lam, 30.0, ws, True),            # first call on ws after calls on ws2: rebuilt
+               (g1, "g1", w.lam, 30.0, ws, False),           # same everything: tables reused
+               (g2, "g2", w.lam, 30.0, ws, False),           # new particle, same tables
+               (g3, "g3", w.lam, 30.0, ws, False),           # another batch size: same tables (they sit first in the workspace)
+               (g2, "g2", 0.8 * w.lam, 30.0, ws, True),      # lambda changed: rebuilt
+               (g2, "g2", 0.8 * w.lam, 25.0, ws, True),      # detector / qx changed: rebuilt
+               (g2, "g2", 0.8 * w.lam, 25.0, ws2, True),     # other workspace: rebuilt there
+               (g2, "g2", 0.8 * w.lam, 25.0, ws, True),      # back: the key is the last call's (ws2) -> rebuilt
+               (g1, "g1", 0.8 * w.lam, 25.0, ws, False)]     # and reused again
+        for i, (g, gi, lam, th, wsp, rebuilt) in enumerate(seq):
+            got = run(g, lam, th, wsp, R)
+            n = sm.last_launch_count()
+            extra = n - n_full if gi != "g3" else None         # a batch of 3 may launch more kernels per chunk; compare only equals
+            assert torch.equal(got, ref[(gi, lam, th)]), (name, i)
+            if extra is not None:
+                assert (n == n_full) == rebuilt and n <= n_full, (name, i, n, n_full)
 
 
 @pytest.mark.parametrize("route", ["pixels", "qgrid"])
