@@ -323,13 +323,14 @@ class Scatman:
 
     def simulate_nufft(self, dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
                        rho_mode: int = RHO_LINEAR, cx: float = 0.0, cy: float = 0.0, workspace=None, out=None, stream=None,
-                       flags: int = 0):
-        """Same result as simulate() by the 3-D type-2 NUFFT route (scatman_simulate_nufft).  Asynchronous."""
+                       flags: int = 0, method: int = METHOD_AUTO):
+        """Same result as simulate() by the 3-D type-2 NUFFT route (scatman_simulate_nufft).  Asynchronous.
+        method: AUTO / TENSOR = GEMM stages on tcgen05 (FP16x3), SIMT_TABLE = FP64 CUDA-core stages."""
         import torch
         self._check_dn(dn)
         grid, batch = self._grid_of(dn, voxel), self._batch_of(dn)
         det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
-        opts = Options(int(rho_mode), 0, 0, int(flags))
+        opts = Options(int(rho_mode), int(method), 0, int(flags))
         need = C.c_size_t(0)
         self._check(self.lib.scatman_nufft_workspace_bytes(self._ctx, C.byref(grid), float(lam), C.byref(det), batch,
                                                            C.byref(need)))
@@ -532,14 +533,14 @@ class Scatman:
         return h_out
 
     def simulate_nufft_host(self, h_dn, voxel, lam: float, npx: int, npy: int, theta_max_deg: float, quat=None,
-                            rho_mode: int = RHO_LINEAR, h_out=None, cx: float = 0.0, cy: float = 0.0):
+                            rho_mode: int = RHO_LINEAR, h_out=None, cx: float = 0.0, cy: float = 0.0, method: int = METHOD_AUTO):
         """scatman_simulate_nufft_host: host tensors in and out, upload / compute / download overlapped chunk by chunk."""
         import torch
         if h_dn.is_cuda or h_dn.dtype != torch.float32 or not h_dn.is_contiguous():
             raise ValueError("h_dn must be a contiguous CPU float32 tensor")
         grid, batch = self._grid_of(h_dn, voxel), self._batch_of(h_dn)
         det = Detector(int(npx), int(npy), float(theta_max_deg), float(cx), float(cy))
-        opts = Options(int(rho_mode), 0, 0, 0)
+        opts = Options(int(rho_mode), int(method), 0, 0)
         if h_out is None:
             h_out = torch.empty((batch, npy, npx), dtype=torch.float32).pin_memory()
         keep, qp = _quat_arg(quat, batch)

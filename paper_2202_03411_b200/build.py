@@ -12,9 +12,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libscatman.so")
-SOURCES = ["api.cu", "fit_kernels.cu", "nufft_kernels.cu", "prep_kernels.cu", "render_kernels.cu",
+SOURCES = ["api.cu", "fit_kernels.cu", "nufft_kernels.cu", "nufft_tensor_kernels.cu", "prep_kernels.cu", "render_kernels.cu",
            "sep_kernels.cu", "sep_tensor_kernels.cu", "simt_kernels.cu", "tensor_kernel.cu"]
-HEADERS = ["internal.h", "ptx_sm100.h", os.path.join("..", "..", "include", "scatman.h")]
+HEADERS = ["internal.h", "ptx_sm100.h", "tc_cgemm.cuh", os.path.join("..", "..", "include", "scatman.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17"]
 # SCATMAN_CHECKED=1: the same library with device-side checks compiled in (mbarrier watchdog, bounds assertions before stores
 # and TMA loads; csrc/ptx_sm100.h).  compute-sanitizer is not available on the GPU pool, so this is the build the sanitize

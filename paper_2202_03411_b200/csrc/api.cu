@@ -147,6 +147,17 @@ static void ev_end(scatman_ctx *ctx, cudaStream_t st) {
     if (!ctx->ev_capturing) { cudaEventRecord(ctx->ev1, st); ctx->ev_valid = true; }
 }
 
+// Checked build only (SCATMAN_CHECKED=1): wait for the stream after a stage and name the stage that failed.
+#ifdef SCATMAN_CHECKED
+#define SCATMAN_STAGE_CHECK(e, st, what)                                                             \
+    do {                                                                                             \
+        if ((e) == cudaSuccess) (e) = cudaStreamSynchronize(st);                                     \
+        if ((e) != cudaSuccess) fprintf(stderr, "scatman checked build: stage '%s' failed: %s\n", what, cudaGetErrorString(e)); \
+    } while (0)
+#else
+#define SCATMAN_STAGE_CHECK(e, st, what) ((void)0)
+#endif
+
 static int fail(scatman_ctx *ctx, int status, const std::string &msg) {
     if (ctx) ctx->last_error = msg;
     return status;
@@ -242,7 +253,8 @@ int scatman_create(scatman_ctx **out, int device) {
     ctx->num_sms = prop.multiProcessorCount;
     if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess ||
         nufft_init_device() != cudaSuccess ||   // the NUFFT route's window polynomials -> constant memory of this device
-        tensor_init_device() != cudaSuccess || sep_init_device() != cudaSuccess || sep_tc_init_device() != cudaSuccess) {
+        tensor_init_device() != cudaSuccess || sep_init_device() != cudaSuccess || sep_tc_init_device() != cudaSuccess ||
+        nufft_tc_init_device() != cudaSuccess) {
         delete ctx;
         return SCATMAN_CUDA_ERROR;
     }
@@ -685,12 +697,18 @@ int scatman_simulate_shapes_qgrid(scatman_ctx *ctx, const scatman_shape *h_shape
 struct NufftLayout {
     Plan p;
     NufftPlan n;
+    NufftTcPlan tc;      // the GEMM stages on tensor cores (tc.ok) ...
+    bool tensor = false; // ... and whether this call uses them (method AUTO / TENSOR) or the FP64 CUDA-core stages (SIMT_TABLE)
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_q = 0, off_tz = 0, off_tx = 0, off_ty = 0,
            off_P = 0, off_H = 0, off_U = 0, total = 0;
+    // tensor-core stages: table planes, rho~ planes, H planes, V planes, flags, z-split bounds, per-item scales
+    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0;
+    size_t hp_bytes = 0;
 };
 // Range of q over the detector (host, FP64, a1's formula): q_x and q_y are monotonic along u and v and extremal in the other
 // coordinate on the rectangle's border; q_z <= 0 is monotonic in u^2 + v^2, so the border pixels plus q_z = 0 bound all three.
-static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const scatman_detector &det, int batch, int rho_mode) {
+static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const scatman_detector &det, int batch, int rho_mode,
+                                     int method, int num_sms) {
     NufftLayout L;
     Plan &p = L.p;
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
@@ -742,22 +760,51 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
         if ((int64_t)nb * L.n.az.nq > 65535) nb = 65535 / L.n.az.nq > 0 ? 65535 / L.n.az.nq : 1;
         L.n.nb = nb;
     }
-    size_t off = 0;
-    auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
-    // q-map and window-corrected tables first: independent of the batch (SCATMAN_FLAG_REUSE_TABLES)
-    L.off_q = take(sizeof(double) * 3 * (size_t)p.npix);
-    L.off_tz = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz);
-    L.off_tx = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx);
-    L.off_ty = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
-    L.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
-    L.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
-    L.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
-    L.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
-    L.off_max = take(sizeof(unsigned) * (size_t)batch);
-    L.off_P = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx);
-    L.off_H = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq);
-    L.off_U = take(sizeof(float2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
-    L.total = off;
+    L.tc = make_nufft_tc_plan(p, L.n, batch, num_sms);
+    L.tensor = L.tc.ok && method != SCATMAN_METHOD_SIMT_TABLE;
+    // Two layouts share the head (q-map, then the phase tables of the method in use: batch-independent, SCATMAN_FLAG_REUSE_TABLES);
+    // the workspace size is the larger of the two so that one buffer serves both methods.
+    size_t total[2] = {0, 0};
+    for (int tensor = 0; tensor < 2; ++tensor) {
+        if (tensor && !L.tc.ok) continue;
+        const bool mine = (tensor != 0) == L.tensor;
+        size_t off = 0;
+        auto take = [&](size_t bytes) { size_t o2 = off; off = scatman::align_up(off + bytes, 1024); return o2; };
+        const size_t o_q = take(sizeof(double) * 3 * (size_t)p.npix);
+        if (mine) L.off_q = o_q;
+        if (!tensor) {
+            const size_t a = take(sizeof(double2) * (size_t)L.n.az.nq * g.nz), b = take(sizeof(double2) * (size_t)L.n.ax.nq * g.nx),
+                         c = take(sizeof(double2) * (size_t)L.n.ay.nq * g.ny);
+            if (mine) { L.off_tz = a; L.off_tx = b; L.off_ty = c; }
+        } else {
+            const NufftTcPlan &t = L.tc;
+            const size_t a = take(sizeof(__half) * 4 * (size_t)t.NPXP * t.sep.NXP), b = take(sizeof(__half) * 4 * (size_t)t.NQYP * t.NY),
+                         c = take(sizeof(__half) * 4 * (size_t)t.NQZP * t.NZP);
+            if (mine) { L.off_txp = a; L.off_typ = b; L.off_tzp = c; }
+        }
+        const size_t o_rm = take(sizeof(double) * 9 * (size_t)batch), o_bb = take(sizeof(int) * 6 * (size_t)batch),
+                     o_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch), o_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch),
+                     o_max = take(sizeof(unsigned) * (size_t)batch);
+        if (mine) { L.off_rotmat = o_rm; L.off_bbox = o_bb; L.off_rot = o_rot; L.off_rho = o_rho; L.off_max = o_max; }
+        if (!tensor) {
+            const size_t a = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx),
+                         b = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq),
+                         c = take(sizeof(float2) * (size_t)L.n.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
+            if (mine) { L.off_P = a; L.off_H = b; L.off_U = c; }
+        } else {
+            const NufftTcPlan &t = L.tc;
+            const size_t slices = (size_t)t.nb * g.nz;
+            const size_t hp = sizeof(__half) * 4 * slices * t.NPXP * t.NY;
+            const size_t a = take(sizeof(__half) * 4 * slices * t.NY * t.sep.NXP), b = take(hp),
+                         c = take(sizeof(__half) * 4 * (size_t)t.NPXP * t.NQYP * t.NZT), d = take(slices * (t.NY / 64)),
+                         e2 = take(sizeof(int) * (size_t)((t.sep.nsx + 1) + (size_t)t.nb * t.sep.ng * (t.sep.nzs + 1))),
+                         f = take(sizeof(float) * (size_t)batch),
+                         u = take(sizeof(float2) * (size_t)t.nb * L.n.az.nq * L.n.ay.nq * L.n.ax.nq);
+            if (mine) { L.off_rp = a; L.off_hp = b; L.hp_bytes = hp; L.off_vp = c; L.off_flags = d; L.off_bounds = e2; L.off_scale = f; L.off_U = u; }
+        }
+        total[tensor] = off;
+    }
+    L.total = total[0] > total[1] ? total[0] : total[1];
     return L;
 }
 
@@ -766,7 +813,7 @@ int scatman_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, do
     if (!ctx || !bytes) return SCATMAN_INVALID_ARGUMENT;
     if (!valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) || batch < 1)
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
-    *bytes = make_nufft_layout(*grid, lambda, *det, batch, 0).total;
+    *bytes = make_nufft_layout(*grid, lambda, *det, batch, 0, SCATMAN_METHOD_AUTO, ctx->num_sms).total;
     return SCATMAN_OK;
 }
 
@@ -775,7 +822,7 @@ int scatman_nufft_grid_dims(scatman_ctx *ctx, const scatman_grid *grid, double l
     if (!ctx || !nq) return SCATMAN_INVALID_ARGUMENT;
     if (!valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda))
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
-    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, 1, 0);
+    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, 1, 0, SCATMAN_METHOD_AUTO, ctx->num_sms);
     nq[0] = L.n.ax.nq; nq[1] = L.n.ay.nq; nq[2] = L.n.az.nq;
     return SCATMAN_OK;
 }
@@ -786,13 +833,13 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) ||
-        batch < 1 || batch > 65535 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1))
+        batch < 1 || batch > 65535 || (o.rho_mode != SCATMAN_RHO_LINEAR && o.rho_mode != SCATMAN_RHO_N2M1) || !valid_qgrid_method(o.method))
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
     if (h_quat && !valid_quats(h_quat, batch)) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "quaternion is not unit");
     if (((uintptr_t)d_dn | (uintptr_t)d_ws | (uintptr_t)d_I) & 15)
         return fail(ctx, SCATMAN_INVALID_ARGUMENT, "device pointers must be 16-byte aligned");
     cudaSetDevice(ctx->device);
-    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, batch, o.rho_mode);
+    const NufftLayout L = make_nufft_layout(*grid, lambda, *det, batch, o.rho_mode, o.method, ctx->num_sms);
     const Plan &p = L.p;
     if (ws_bytes < L.total) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -804,6 +851,7 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     key.route = 3;
     key.nx = grid->nx; key.ny = grid->ny; key.nz = grid->nz; key.dx = grid->dx; key.dy = grid->dy; key.dz = grid->dz;
     key.lambda = lambda; key.npx = det->npx; key.npy = det->npy; key.theta = det->theta_max_deg; key.cx = det->cx; key.cy = det->cy;
+    key.method = L.tensor ? 1 : 3;
     key.ws = d_ws;
     const bool reuse = (o.flags & SCATMAN_FLAG_REUSE_TABLES) && ctx->tables_valid && ctx->tables_key == key;
     ctx->tables_valid = false;
@@ -827,20 +875,57 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     e = launch_strength(src, p, batch, rho, (unsigned *)(ws + L.off_max), st);
     ++nl;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
-    double2 *Tz = (double2 *)(ws + L.off_tz), *TxT = (double2 *)(ws + L.off_tx), *Ty = (double2 *)(ws + L.off_ty);
-    if (!reuse) {
-        e = launch_nufft_tables(p, L.n, Tz, TxT, Ty, st);
-        nl += 3;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
-    }
-    ev_begin(ctx, st);
-    for (int b0 = 0; b0 < batch; b0 += L.n.nb) {   // a chunk of items per set of launches
-        const int nb = batch - b0 < L.n.nb ? batch - b0 : L.n.nb;
-        e = launch_nufft_chunk((const float2 *)rho + (size_t)b0 * p.nvox, p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, Tz, TxT, Ty,
-                               q, (double2 *)(ws + L.off_P), (double2 *)(ws + L.off_H), (float2 *)(ws + L.off_U),
-                               d_I + (size_t)b0 * p.npix, st);
-        nl += 4;
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");
+    if (L.tensor) {
+        // GEMM stages on tcgen05 (nufft_tensor_kernels.cu): pack -> stage X (the separable route's) -> stage Y -> stage Z -> interpolation
+        const NufftTcPlan &t = L.tc;
+        __half *Txp = (__half *)(ws + L.off_txp), *Typ = (__half *)(ws + L.off_typ), *Tzp = (__half *)(ws + L.off_tzp);
+        __half *Rp = (__half *)(ws + L.off_rp), *Hp = (__half *)(ws + L.off_hp), *Vp = (__half *)(ws + L.off_vp);
+        float *ampscale = (float *)(ws + L.off_scale);
+        int *bounds = (int *)(ws + L.off_bounds);
+        float2 *U = (float2 *)(ws + L.off_U);
+        if (!reuse) {
+            e = launch_nufft_tc_tables(p, L.n, t, Txp, Typ, Tzp, st);
+            nl += 3;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
+        }
+        int Ly = 0;
+        while ((1 << Ly) < p.ny) ++Ly;
+        ev_begin(ctx, st);
+        for (int b0 = 0; b0 < batch; b0 += t.nb) {
+            const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
+            std::string err;
+            e = launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, (const unsigned *)(ws + L.off_max) + b0, p, t.sep, nb, Rp,
+                                   ws + L.off_flags, bounds, ampscale + b0, st);
+            // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero
+            SCATMAN_STAGE_CHECK(e, st, "nufft pack");
+            if (e == cudaSuccess) e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);
+            if (e == cudaSuccess) e = launch_sep_tc_x(p, t.sep, Rp, Txp, ws + L.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
+            SCATMAN_STAGE_CHECK(e, st, "nufft stage X");
+            if (e == cudaSuccess) e = launch_nufft_tc_yz(p, L.n, t, nb, Hp, Typ, Tzp, Vp, U, ctx->num_sms, st, &err);
+            SCATMAN_STAGE_CHECK(e, st, "nufft stages Y, Z");
+            // amplitude = accumulator x (the separable route's per-item scale) / (2^10 of Tz x stage Y's 2^(-11 - Ly))
+            if (e == cudaSuccess)
+                e = launch_nufft_interp(p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, q, U, ampscale + b0, ldexp(1.0, 1 + Ly),
+                                        d_I + (size_t)b0 * p.npix, st);
+            nl += 8;
+            if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "nufft stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
+        }
+    } else {
+        double2 *Tz = (double2 *)(ws + L.off_tz), *TxT = (double2 *)(ws + L.off_tx), *Ty = (double2 *)(ws + L.off_ty);
+        if (!reuse) {
+            e = launch_nufft_tables(p, L.n, Tz, TxT, Ty, st);
+            nl += 3;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft tables");
+        }
+        ev_begin(ctx, st);
+        for (int b0 = 0; b0 < batch; b0 += L.n.nb) {   // a chunk of items per set of launches
+            const int nb = batch - b0 < L.n.nb ? batch - b0 : L.n.nb;
+            e = launch_nufft_chunk((const float2 *)rho + (size_t)b0 * p.nvox, p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, Tz, TxT, Ty,
+                                   q, (double2 *)(ws + L.off_P), (double2 *)(ws + L.off_H), (float2 *)(ws + L.off_U),
+                                   d_I + (size_t)b0 * p.npix, st);
+            nl += 4;
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "nufft stages");
+        }
     }
     ev_end(ctx, st);
     ctx->last_launches = nl;
@@ -1041,7 +1126,7 @@ int scatman_simulate_nufft_host(scatman_ctx *ctx, const float *h_dn, const scatm
     const int64_t npix = (int64_t)det->npx * det->npy;
     const size_t in_item = sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz, out_item = sizeof(float) * (size_t)npix;
     const int chunk = host_chunk_items(in_item, batch);
-    size_t ws_bytes = make_nufft_layout(*grid, lambda, *det, chunk, o.rho_mode).total;   // grows with the batch
+    size_t ws_bytes = make_nufft_layout(*grid, lambda, *det, chunk, o.rho_mode, o.method, ctx->num_sms).total;   // grows with the batch
     return host_pipeline(ctx, h_dn, in_item, h_I, out_item, batch, chunk, ws_bytes, nullptr, 0, nullptr,
                          [&](const float *d_dn, int b0, int nb, void *d_ws, float *d_I, cudaStream_t st) {
                              return scatman_simulate_nufft(ctx, d_dn, grid, lambda, det, h_quat ? h_quat + 4 * (size_t)b0 : nullptr, nb, &o,

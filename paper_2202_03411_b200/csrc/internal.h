@@ -112,6 +112,26 @@ cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPl
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,
                                double2 *d_H, float2 *d_U, float *d_I, cudaStream_t st);
 
+// the NUFFT route's GEMM stages on tensor cores (nufft_tensor_kernels.cu)
+struct NufftTcPlan {
+    bool ok = false;                 // the grid fits the resident operands (nx, ny, nz <= 1024); else the FP64 stages run
+    SepTcPlan sep;                   // stage X = the separable route's stage X on the nqx uniform-grid columns
+    int NY = 0, NPXP = 0;            // padded y (x128) and uniform-grid columns, as in sep
+    int nky = 0, nkz = 0, NZP = 0;   // 64-blocks of y and of one item's slices; padded slices of the Tz planes
+    int nby = 0, nbz = 0;            // resident table rows per CTA in stages Y and Z (64 / 32 / 16)
+    int NQYP = 0, NQZP = 0;          // padded uniform-grid rows and planes (multiples of 2 nby, 2 nbz)
+    int nb = 1, NZI = 0, NZT = 0;    // items per chunk; slices per item padded to 8; row length of V (nb NZI)
+};
+NufftTcPlan make_nufft_tc_plan(const Plan &p, const NufftPlan &n, int batch, int num_sms);
+cudaError_t nufft_tc_init_device();
+cudaError_t launch_nufft_tc_tables(const Plan &p, const NufftPlan &n, const NufftTcPlan &t, __half *d_Tx, __half *d_Ty, __half *d_Tz,
+                                   cudaStream_t st);
+cudaError_t launch_nufft_tc_yz(const Plan &p, const NufftPlan &n, const NufftTcPlan &t, int nb, const __half *d_Hp, const __half *d_Ty,
+                               const __half *d_Tz, __half *d_Vp, float2 *d_U, int num_sms, cudaStream_t st, std::string *err);
+// interpolation of a chunk from U (FP32 complex [nb][nqz][nqy][nqx]); amplitude scale = ampscale[b] * scale_mul, or dV if ampscale is null
+cudaError_t launch_nufft_interp(const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells, const double *d_q,
+                                const float2 *d_U, const float *d_ampscale, double scale_mul, float *d_I, cudaStream_t st);
+
 // forward-fitting pieces (fit_kernels.cu)
 size_t fit_workspace_bytes(int64_t npix, int batch);
 cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,

