@@ -328,14 +328,14 @@ int scatman_render(scatman_ctx *ctx, const scatman_shape *h_shapes, int32_t batc
                    void *cuda_stream) {
     if (!ctx || !h_shapes || !d_dn || !valid_grid(grid) || batch < 1) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
     cudaSetDevice(ctx->device);
-    const size_t per_item = (size_t)grid->nx * grid->ny * grid->nz * 2;
-    for (int b = 0; b < batch; ++b) {
-        cudaError_t e = cudaSuccess;
-        if (launch_render(h_shapes[b], *grid, d_dn + (size_t)b * per_item, (cudaStream_t)cuda_stream, &e))
-            return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad shape descriptor " + std::to_string(b));
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "render");
-    }
-    ctx->last_launches = batch;
+    if ((size_t)((uint64_t)grid->nx * grid->ny * grid->nz + 255) / 256 > 0x7fffffffull || batch > 65535)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "grid or batch too large for one render launch");
+    cudaError_t e = cudaSuccess;
+    int nl = 0;
+    const int bad = launch_render_batch(h_shapes, batch, *grid, d_dn, (cudaStream_t)cuda_stream, &e, &nl);
+    if (bad) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad shape descriptor " + std::to_string(bad - 1));
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "render");
+    ctx->last_launches = nl;
     return SCATMAN_OK;
 }
 
@@ -895,7 +895,7 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
             std::string err;
             e = launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, (const unsigned *)(ws + L.off_max) + b0, p, t.sep, nb, Rp,
-                                   ws + L.off_flags, bounds, ampscale + b0, st);
+                                   ws + L.off_flags, bounds, ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero
             SCATMAN_STAGE_CHECK(e, st, "nufft pack");
             if (e == cudaSuccess) e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);

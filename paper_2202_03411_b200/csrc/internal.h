@@ -86,7 +86,8 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
-                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st);
+                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
+                               bool x_only = false);   // x_only: z-split bounds of stage X only (the NUFFT route)
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
                             const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
                             cudaStream_t st, std::string *err);
@@ -96,7 +97,8 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, int npx, const double *d_qy, int npy,
                                    const Plan &p, const SepTcPlan &t, int nb, const float *d_ampscale, float *d_I,
                                    cudaStream_t st);
-int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err);
+int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_grid &g, float *d_dn, cudaStream_t st,
+                        cudaError_t *err, int *nlaunch);   // 0, or 1 + index of the first bad descriptor
 
 // flat-detector route by a 3-D type-2 NUFFT (nufft_kernels.cu)
 constexpr int kNufftW = 10;                     // Kaiser-Bessel window width in grid cells (oversampling 2)

@@ -214,30 +214,46 @@ __device__ inline double placed(const double (&own)[kW], int shift, int a) {
     return v;
 }
 
-constexpr int kInterpThreads = 64;
+constexpr int kInterpThreads = 128;
+constexpr int kTX = 8, kTY = 16;         // a block = 8 groups of P pixels along a detector row x 16 rows
+constexpr int kTileCap = 4096;           // float2 elements of shared memory for the block's window of U (32 KB)
 
+// A block owns a TILE of 8 P x 8 pixels.  Its pixels' windows overlap heavily, so the block first copies the box of U that covers
+// all of them into shared memory (coalesced, every thread loading: the whole box is in flight at once) and the per-thread sums
+// then read shared memory -- the earlier version read U through L1 from a loop whose every iteration waited for an L2 round
+// trip, with one wave of 8-12 warps per SM to hide it.  A tile whose box exceeds kTileCap (coarse detectors, where neighbouring
+// pixels are cells apart) reads U from global memory as before.
 template <int P>
 __global__ void __launch_bounds__(kInterpThreads)
 nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
                     const float2 *__restrict__ U, int64_t strideU, double dV, const float *__restrict__ ampscale,
                     float *__restrict__ I) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
-    extern __shared__ double wsm[];                       // [2][P][KU][kInterpThreads]
+    extern __shared__ float wsm[];                        // [2][P][KU][kInterpThreads] y and z weights (FP32), then the tile of U
+    float2 *tile = reinterpret_cast<float2 *>(wsm + 2 * P * KU * kInterpThreads);
+    __shared__ int red[8];                                // lo[3], hi[3], every thread's pixels share a window, any valid thread
     const int ngx = (npx + P - 1) / P;
-    const int64_t g = (int64_t)blockIdx.x * kInterpThreads + threadIdx.x;
-    if (g >= (int64_t)ngx * npy) return;
-    const int iy = (int)(g / ngx), ix0 = (int)(g % ngx) * P;
+    const int tiles_x = (ngx + kTX - 1) / kTX;
+    const int gx = (blockIdx.x % tiles_x) * kTX + (threadIdx.x % kTX), iy = (blockIdx.x / tiles_x) * kTY + threadIdx.x / kTX;
+    const bool valid = gx < ngx && iy < npy;
+    const int ix0 = gx * P;
     const int64_t p0 = (int64_t)iy * npx + ix0;
     const int64_t npix = (int64_t)npx * npy;
     U += (int64_t)blockIdx.y * strideU;
     I += (int64_t)blockIdx.y * npix;
     if (ampscale) dV *= (double)__ldg(ampscale + blockIdx.y);   // tensor-core stages: U carries the item's operand scales
-    const int np = npx - ix0 < P ? npx - ix0 : P;
+    const int np = valid ? (npx - ix0 < P ? npx - ix0 : P) : 0;
     double u[P][3];
     int m0[P][3], base[3], top[3];
+    if (threadIdx.x == 0) {
+        red[0] = red[1] = red[2] = 0x7fffffff;
+        red[3] = red[4] = red[5] = -0x7fffffff;
+        red[6] = 1;
+    }
+    __syncthreads();
 #pragma unroll
     for (int j = 0; j < P; ++j) {
-        const int64_t p = p0 + (j < np ? j : 0);
+        const int64_t p = valid ? p0 + (j < np ? j : 0) : 0;     // threads past the detector's edge look at pixel 0 and stay out of the sums
         u[j][0] = q[3 * p + 0] * ax.inv_h; u[j][1] = q[3 * p + 1] * ay.inv_h; u[j][2] = q[3 * p + 2] * az.inv_h;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -246,25 +262,63 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
             top[d] = j == 0 ? m0[j][d] : max(top[d], m0[j][d]);
         }
     }
-    const bool common = top[0] - base[0] + kW <= KU && top[1] - base[1] + kW <= KU && top[2] - base[2] + kW <= KU;
-    auto wy = [&](int j, int b) -> double & { return wsm[((0 * P + j) * KU + b) * kInterpThreads + threadIdx.x]; };
-    auto wz = [&](int j, int c) -> double & { return wsm[((1 * P + j) * KU + c) * kInterpThreads + threadIdx.x]; };
+    const bool common = valid && top[0] - base[0] + kW <= KU && top[1] - base[1] + kW <= KU && top[2] - base[2] + kW <= KU;
+    if (valid) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            atomicMin(&red[d], base[d]);
+            atomicMax(&red[3 + d], base[d] + KU - 1);    // last cell a common window of KU cells can touch
+        }
+        if (!common) atomicAnd(&red[6], 0);
+    }
+    __syncthreads();
+    const int lo0 = red[0], lo1 = red[1], lo2 = red[2];
+    const int e0 = red[3] - lo0 + 1, e1 = red[4] - lo1 + 1, e2 = red[5] - lo2 + 1;
+    // the box must also lie inside the uniform grid (a thread's common window can reach 2 cells past its pixels' own windows)
+    const bool tiled = red[6] != 0 && red[3] >= lo0 && (int64_t)e0 * e1 * e2 <= kTileCap && lo0 - ax.m_lo >= 0 && lo1 - ay.m_lo >= 0 &&
+                       lo2 - az.m_lo >= 0 && red[3] - ax.m_lo < ax.nq && red[4] - ay.m_lo < ay.nq && red[5] - az.m_lo < az.nq;
+    if (tiled) {
+        const int rows = e1 * e2;
+        for (int e = threadIdx.x; e < rows * e0; e += kInterpThreads) {
+            const int x = e % e0, yz = e / e0;
+            const int y = yz % e1, z = yz / e1;
+            tile[e] = __ldg(U + ((int64_t)(lo2 - az.m_lo + z) * ay.nq + (lo1 - ay.m_lo + y)) * ax.nq + (lo0 - ax.m_lo + x));
+        }
+        __syncthreads();
+    }
+    if (!valid) return;
+    auto wy = [&](int j, int b) -> float & { return wsm[((0 * P + j) * KU + b) * kInterpThreads + threadIdx.x]; };
+    auto wz = [&](int j, int c) -> float & { return wsm[((1 * P + j) * KU + c) * kInterpThreads + threadIdx.x]; };
     if (common) {
-        double wx[P][KU];
+        // The x weights and the row sums over x (12 of the 14 multiply-adds of a grid value) are FP32: a row sum of <= 12 terms of
+        // one sign pattern rounds at ~1e-7 of its own magnitude, the same size as the FP32 rounding U already carries; the sums over
+        // y and z (where rows of different phase combine) stay FP64.
+        float wx[P][KU];
 #pragma unroll
         for (int j = 0; j < P; ++j) {
             double own[kW];
             kb_weights(u[j][0], m0[j][0], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) wx[j][a] = placed<KU>(own, m0[j][0] - base[0], a);
+            for (int a = 0; a < KU; ++a) wx[j][a] = (float)placed<KU>(own, m0[j][0] - base[0], a);
             kb_weights(u[j][1], m0[j][1], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) wy(j, a) = placed<KU>(own, m0[j][1] - base[1], a);
+            for (int a = 0; a < KU; ++a) wy(j, a) = (float)placed<KU>(own, m0[j][1] - base[1], a);
             kb_weights(u[j][2], m0[j][2], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) wz(j, a) = placed<KU>(own, m0[j][2] - base[2], a);
+            for (int a = 0; a < KU; ++a) wz(j, a) = (float)placed<KU>(own, m0[j][2] - base[2], a);
         }
-        const int ix = base[0] - ax.m_lo, iyq = base[1] - ay.m_lo, iz = base[2] - az.m_lo;   // inside the grid by the plan's margins
+        // first grid value of the thread's window and the strides between its rows and planes, in the tile or in U
+        const float2 *win;
+        int sy, sz;                    // < 2^31: a plane of the uniform grid is at most a few 10^5 points
+        if (tiled) {
+            win = tile + ((base[2] - lo2) * e1 + (base[1] - lo1)) * e0 + (base[0] - lo0);
+            sy = e0;
+            sz = e0 * e1;
+        } else {
+            win = U + ((int64_t)(base[2] - az.m_lo) * ay.nq + (base[1] - ay.m_lo)) * ax.nq + (base[0] - ax.m_lo);   // inside the grid by the plan's margins
+            sy = ax.nq;
+            sz = ax.nq * ay.nq;
+        }
         double are[P], aim[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) are[j] = aim[j] = 0.0;
@@ -272,7 +326,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
             double wzc[P];
             bool any = false;
 #pragma unroll
-            for (int j = 0; j < P; ++j) { wzc[j] = wz(j, c); any |= wzc[j] != 0.0; }
+            for (int j = 0; j < P; ++j) { wzc[j] = (double)wz(j, c); any |= wzc[j] != 0.0; }
             if (!any) continue;
             double pre[P], pim[P];
 #pragma unroll
@@ -281,22 +335,22 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
                 double wyb[P];
                 bool anyb = false;
 #pragma unroll
-                for (int j = 0; j < P; ++j) { wyb[j] = wy(j, b); anyb |= wyb[j] != 0.0; }
+                for (int j = 0; j < P; ++j) { wyb[j] = (double)wy(j, b); anyb |= wyb[j] != 0.0; }
                 if (!anyb) continue;
-                const float2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
+                const float2 *row = win + c * sz + b * sy;
                 float2 v[KU];
 #pragma unroll
-                for (int a = 0; a < KU; ++a) v[a] = __ldg(row + a);
+                for (int a = 0; a < KU; ++a) v[a] = row[a];
 #pragma unroll
                 for (int j = 0; j < P; ++j) {
-                    double rre = 0.0, rim = 0.0;
+                    float rre = 0.f, rim = 0.f;
 #pragma unroll
                     for (int a = 0; a < KU; ++a) {
-                        rre = fma(wx[j][a], (double)v[a].x, rre);
-                        rim = fma(wx[j][a], (double)v[a].y, rim);
+                        rre = fmaf(wx[j][a], v[a].x, rre);
+                        rim = fmaf(wx[j][a], v[a].y, rim);
                     }
-                    pre[j] = fma(wyb[j], rre, pre[j]);
-                    pim[j] = fma(wyb[j], rim, pim[j]);
+                    pre[j] = fma(wyb[j], (double)rre, pre[j]);
+                    pim[j] = fma(wyb[j], (double)rim, pim[j]);
                 }
             }
 #pragma unroll
@@ -314,33 +368,38 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
         return;
     }
     // pixels one by one, each with its own W-cell window
-    for (int j = 0; j < np; ++j) {
-        double wx1[kW], own[kW];
-        kb_weights(u[j][0], m0[j][0], wx1);
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        if (j >= np) break;
+        double own[kW];
+        float wx1[kW];
+        kb_weights(u[j][0], m0[j][0], own);
+#pragma unroll
+        for (int a = 0; a < kW; ++a) wx1[a] = (float)own[a];
         kb_weights(u[j][1], m0[j][1], own);
 #pragma unroll
-        for (int a = 0; a < kW; ++a) wy(0, a) = own[a];
+        for (int a = 0; a < kW; ++a) wy(0, a) = (float)own[a];
         kb_weights(u[j][2], m0[j][2], own);
 #pragma unroll
-        for (int a = 0; a < kW; ++a) wz(0, a) = own[a];
+        for (int a = 0; a < kW; ++a) wz(0, a) = (float)own[a];
         const int ix = m0[j][0] - ax.m_lo, iyq = m0[j][1] - ay.m_lo, iz = m0[j][2] - az.m_lo;
         double are = 0.0, aim = 0.0;
         for (int c = 0; c < kW; ++c) {
             double pre = 0.0, pim = 0.0;
             for (int b = 0; b < kW; ++b) {
                 const float2 *row = U + ((int64_t)(iz + c) * ay.nq + (iyq + b)) * ax.nq + ix;
-                double rre = 0.0, rim = 0.0;
+                float rre = 0.f, rim = 0.f;
 #pragma unroll
                 for (int a = 0; a < kW; ++a) {
                     const float2 v = __ldg(row + a);
-                    rre = fma(wx1[a], (double)v.x, rre);
-                    rim = fma(wx1[a], (double)v.y, rim);
+                    rre = fmaf(wx1[a], v.x, rre);
+                    rim = fmaf(wx1[a], v.y, rim);
                 }
-                pre = fma(wy(0, b), rre, pre);
-                pim = fma(wy(0, b), rim, pim);
+                pre = fma((double)wy(0, b), (double)rre, pre);
+                pim = fma((double)wy(0, b), (double)rim, pim);
             }
-            are = fma(wz(0, c), pre, are);
-            aim = fma(wz(0, c), pim, aim);
+            are = fma((double)wz(0, c), pre, are);
+            aim = fma((double)wz(0, c), pim, aim);
         }
         are *= dV;
         aim *= dV;
@@ -352,9 +411,9 @@ template <int P>
 cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &n, const float2 *d_U, int64_t strideU, int nb,
                           double dV, const float *d_ampscale, float *d_I, cudaStream_t st) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
-    const size_t smem = sizeof(double) * 2 * P * KU * kInterpThreads;
-    const int64_t groups = (int64_t)((npx + P - 1) / P) * npy;
-    dim3 grid((unsigned)((groups + kInterpThreads - 1) / kInterpThreads), nb);
+    const size_t smem = sizeof(float) * 2 * P * KU * kInterpThreads + sizeof(float2) * kTileCap;
+    const int64_t tiles = (int64_t)(((npx + P - 1) / P + kTX - 1) / kTX) * ((npy + kTY - 1) / kTY);
+    dim3 grid((unsigned)tiles, nb);
     nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_ampscale, d_I);
     return cudaGetLastError();
 }
@@ -416,7 +475,7 @@ cudaError_t nufft_init_device() {
     }
     cudaError_t e = cudaMemcpyToSymbol(c_kb, coef, sizeof(coef));
     auto smem_gemm = [](int rm) { return (int)(sizeof(double2) * 2 * BK * ((16 * rm + 1) + BN)); };
-    auto smem_interp = [](int P) { return (int)(sizeof(double) * 2 * P * (P > 1 ? kW + 2 : kW) * kInterpThreads); };
+    auto smem_interp = [](int P) { return (int)(sizeof(float) * 2 * P * (P > 1 ? kW + 2 : kW) * kInterpThreads + sizeof(float2) * kTileCap); };
     const cudaFuncAttribute attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
 #define SCATMAN_ZGEMM_ATTR(RM)                                                                                          \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_zgemm_kernel<double2, float2, double2, RM, false>, attr, smem_gemm(RM));   \
@@ -428,8 +487,6 @@ cudaError_t nufft_init_device() {
 #undef SCATMAN_ZGEMM_ATTR
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<1>, attr, smem_interp(1));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<2>, attr, smem_interp(2));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<3>, attr, smem_interp(3));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(nufft_interp_kernel<4>, attr, smem_interp(4));
     return e;
 }
 
@@ -477,8 +534,8 @@ cudaError_t launch_nufft_interp(const Plan &p, const NufftPlan &n, int nb, int n
     (void)p;
     // P pixels share a window of W + 2 cells if their first cells differ by at most 2, i.e. if they lie within 2 grid cells of each other
     // on every axis: (P - 1) x pixel_cells < 2 (with a margin; a group that still does not fit takes its pixels one by one in the kernel)
-    if (3.0 * pixel_cells < 1.9) return launch_interp<4>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
-    if (2.0 * pixel_cells < 1.9) return launch_interp<3>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
+    // (measured on B200: two pixels per thread and twice the threads beat four pixels per thread -- the same instruction count, but
+    // the per-thread chains are half as long and twice as many warps hide them; profiles/r02_nufft_tensor.md)
     if (pixel_cells < 1.9) return launch_interp<2>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
     return launch_interp<1>(d_q, npx, npy, n, d_U, strideU, nb, dV, d_ampscale, d_I, st);
 }

@@ -36,16 +36,36 @@ cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q,
 // initialised by the launcher to {INT_MAX x3, -1 x3}.  One block per (b, z) slice.  The resampling below gathers 8 corners
 // along a slanted line (its cost is cache wavefronts, not bytes); beam-frame voxels that land outside this box are vacuum
 // without looking.
-__global__ void bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox) {
+__global__ void __launch_bounds__(256)
+bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox) {
     const int iz = blockIdx.x % nz, b = blockIdx.x / nz;
     const float2 *src = in + ((size_t)b * nz + iz) * (size_t)nx * ny;
     int x0 = 0x7fffffff, y0 = 0x7fffffff, x1 = -1, y1 = -1;
-    for (int e = threadIdx.x; e < nx * ny; e += blockDim.x) {
-        const float2 v = __ldg(src + e);
-        if (v.x != 0.f || v.y != 0.f) {
-            const int x = e % nx, y = e / nx;
-            x0 = min(x0, x); x1 = max(x1, x);
-            y0 = min(y0, y); y1 = max(y1, y);
+    const int n = nx * ny;
+    // two voxels per 16-byte load (slices start 16-byte aligned when nx ny is even; the odd case takes the scalar path), four
+    // loads in flight per thread: the pass is bound by HBM bandwidth, not by load latency
+    auto seen = [&](int e) {
+        const int x = e % nx, y = e / nx;
+        x0 = min(x0, x); x1 = max(x1, x);
+        y0 = min(y0, y); y1 = max(y1, y);
+    };
+    if ((n & 1) == 0) {
+        const float4 *src4 = (const float4 *)src;
+        const int n2 = n >> 1;
+        for (int e0 = threadIdx.x; e0 < n2; e0 += 4 * 256) {
+            float4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = e0 + u * 256 < n2 ? __ldg(src4 + e0 + u * 256) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (v[u].x != 0.f || v[u].y != 0.f) seen(2 * (e0 + u * 256));
+                if (v[u].z != 0.f || v[u].w != 0.f) seen(2 * (e0 + u * 256) + 1);
+            }
+        }
+    } else {
+        for (int e = threadIdx.x; e < n; e += 256) {
+            const float2 v = __ldg(src + e);
+            if (v.x != 0.f || v.y != 0.f) seen(e);
         }
     }
     for (int off = 16; off > 0; off >>= 1) {
@@ -78,8 +98,44 @@ __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int
     const int bz = blk % nbz;
     const int b = blk / nbz;
     const int ix = bx * 16 + (threadIdx.x & 15), iy = by * 4 + ((threadIdx.x >> 4) & 3), iz = bz * 4 + (threadIdx.x >> 6);
-    if (ix >= nx || iy >= ny || iz >= nz) return;
     const double *R = rotmat + 9 * b;
+    // Most blocks of a grid lie outside the particle: the eight corners of this block of 16 x 4 x 4 output voxels go to the body
+    // frame (threads 0-7), and if their bounding range misses the box of non-vacuum voxels (widened by the voxel of the
+    // interpolation cell) on any axis, every output voxel of the block is vacuum: store zeros, skip the per-voxel arithmetic.
+    {
+        bool hit = false;
+        if (threadIdx.x < 32) {
+            const int c = threadIdx.x & 7;
+            const double xc = centre(min(bx * 16 + ((c & 1) ? 15 : 0), nx - 1), nx, dx);
+            const double yc = centre(min(by * 4 + ((c & 2) ? 3 : 0), ny - 1), ny, dy);
+            const double zc = centre(min(bz * 4 + ((c & 4) ? 3 : 0), nz - 1), nz, dz);
+            double f[3];
+            f[0] = (R[0] * xc + R[3] * yc + R[6] * zc) * inv.x + 0.5 * (double)(nx - 1);
+            f[1] = (R[1] * xc + R[4] * yc + R[7] * zc) * inv.y + 0.5 * (double)(ny - 1);
+            f[2] = (R[2] * xc + R[5] * yc + R[8] * zc) * inv.z + 0.5 * (double)(nz - 1);
+            const int *bb = bbox + 6 * b;
+            bool miss = false;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double lo = f[d], hi = f[d];
+#pragma unroll
+                for (int off = 1; off < 8; off <<= 1) {
+                    lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+                    hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+                }
+                // the per-voxel test below is f > bb_lo - 1 && f < bb_hi + 1: no voxel of the block can pass it if the whole
+                // range lies at or beyond one of the two limits (an affine map takes the block into the hull of its corners)
+                miss |= hi <= (double)(bb[d] - 1) || lo >= (double)(bb[3 + d] + 1);
+            }
+            hit = !miss;
+        }
+        if (!__syncthreads_or(hit ? 1 : 0)) {
+            if (ix < nx && iy < ny && iz < nz)
+                out[(size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx + ix] = make_float2(0.f, 0.f);
+            return;
+        }
+    }
+    if (ix >= nx || iy >= ny || iz >= nz) return;
     // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = f0 + ix * step (one row of R^T per axis)
     const double yb = centre(iy, ny, dy), zb = centre(iz, nz, dz), xb0 = centre(0, nx, dx);
     const double ix_dx = inv.x, iy_dy = inv.y, iz_dz = inv.z;   // reciprocals from the host: an FP64 division costs ~40 instructions
@@ -97,6 +153,22 @@ __global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int
             fz > (double)(bb[2] - 1) && fz < (double)(bb[5] + 1)) {
             const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
             const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
+            // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
+            // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
+            // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
+            if (x0 >= 0 && y0 >= 0 && z0 >= 0 && x0 + 1 < nx && y0 + 1 < ny && z0 + 1 < nz) {
+                const float2 *c0 = src + ((size_t)z0 * ny + y0) * nx + x0;
+                const size_t sy = (size_t)nx, sz = (size_t)nx * ny;
+                const float2 v000 = __ldg(c0), v001 = __ldg(c0 + 1), v010 = __ldg(c0 + sy), v011 = __ldg(c0 + sy + 1);
+                const float2 v100 = __ldg(c0 + sz), v101 = __ldg(c0 + sz + 1), v110 = __ldg(c0 + sz + sy), v111 = __ldg(c0 + sz + sy + 1);
+                const bool same = v001.x == v000.x && v001.y == v000.y && v010.x == v000.x && v010.y == v000.y && v011.x == v000.x &&
+                                  v011.y == v000.y && v100.x == v000.x && v100.y == v000.y && v101.x == v000.x && v101.y == v000.y &&
+                                  v110.x == v000.x && v110.y == v000.y && v111.x == v000.x && v111.y == v000.y;
+                if (same) {
+                    dst[ix] = v000;
+                    return;
+                }
+            }
             const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
             const double wx[2] = {1.0 - tx, tx}, wy[2] = {1.0 - ty, ty}, wz[2] = {1.0 - tz, tz};
             double are = 0.0, aim = 0.0;

@@ -1,7 +1,9 @@
 // render_kernels.cu -- shape rendering on the GPU (Block 5 of Fig. 4; shape models PAPER.md:279-281,
 // 405-425): Ellipsoid, SphericalHarmonics, RadialMap, VolumeMap -> (delta, beta) grid, rendered directly
 // in the beam frame at r_body = R^T r_beam (no resampling step), binary voxelisation at voxel centres, all FP64.
-// Readings R18-R21 of DESIGN.md.  One launch per shape, one thread per voxel, x fastest (coalesced 8-byte stores).
+// Readings R18-R21 of DESIGN.md.  One thread per voxel, x fastest (coalesced 8-byte stores); the shapes of a batch are rendered by ONE
+// launch per ~30 KB of descriptors (blockIdx.y = shape): the descriptors travel as a __grid_constant__ kernel parameter (no device
+// allocation, no host buffer that must outlive the call), the harmonic coefficients of all shapes of a launch in one pool.
 #include <cmath>
 #include <utility>
 
@@ -18,9 +20,7 @@ struct RenderArgs {
     double dx, dy, dz;
     double Rt[9];            // row-major R^T: r_body = Rt r_beam
     double a, b, c;          // ellipsoid: 1 / semi-axis
-    int ncoef;               // spherical harmonics: value = sum cn[i] P_{l[i]}^{m[i]}(cos theta) {1, cos m phi, sin m phi}
-    signed char l[kMaxCoef], m[kMaxCoef];   // m as given (sign selects cos / sin)
-    double cn[kMaxCoef];     // c * N_lm * (m != 0 ? sqrt 2 : 1)
+    int ncoef, coef0;        // spherical harmonics: value = sum cn[coef0 + i] P_{l}^{|m|}(cos theta) {1, cos m phi, sin m phi}, i < ncoef
     double r_lo, r_hi;       // every voxel with |r| < r_lo is inside, with |r| > r_hi outside
     int nlat, nlon;          // radial map
     const double *radii;
@@ -29,16 +29,27 @@ struct RenderArgs {
     double vdx;
 };
 
+// The shapes of one launch: descriptors + the pooled harmonic coefficients (sorted per shape by (|m|, l)); < 32 KB of kernel parameters.
+constexpr int kBatchShapes = 96, kPoolCoef = 1024;
+struct RenderBatch {
+    int n;
+    RenderArgs a[kBatchShapes];
+    double cn[kPoolCoef];                 // c * N_lm * (m != 0 ? sqrt 2 : 1)
+    signed char l[kPoolCoef], m[kPoolCoef];   // m as given (sign selects cos / sin)
+};
+static_assert(sizeof(RenderBatch) <= 32000, "kernel parameters are limited to 32764 bytes");
+
 // R(theta, phi) = sum_i cn[i] P_{l_i}^{|m_i|}(cos theta) {1 | cos |m| phi | sin |m| phi}, the triplets sorted by (|m|, l):
 // P_m^m and (cos m phi, sin m phi) advance with m, P_l^m by the upward recurrence in l
 //   (l + 1 - m) P_{l+1}^m = (2l + 1) x P_l^m - (l + m) P_{l-1}^m        (Condon-Shortley phase, Eq. 10),
 // so one voxel costs O(l_max^2) FP64 operations and no trigonometric call.
-__device__ double sh_radius(const RenderArgs &A, double ct, double cphi, double sphi) {
+__device__ double sh_radius(const RenderArgs &A, const double *__restrict__ Acn, const signed char *__restrict__ Al,
+                            const signed char *__restrict__ Am, double ct, double cphi, double sphi) {
     const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
     double R = 0.0, pmm = 1.0, cm = 1.0, sm = 0.0;
     int am = 0, i = 0;
     while (i < A.ncoef) {
-        const int target = A.m[i] < 0 ? -A.m[i] : A.m[i];
+        const int target = Am[i] < 0 ? -Am[i] : Am[i];
         while (am < target) {
             ++am;
             pmm = -pmm * (double)(2 * am - 1) * st;
@@ -48,27 +59,29 @@ __device__ double sh_radius(const RenderArgs &A, double ct, double cphi, double 
         }
         double pl = pmm, pl_prev = 0.0;
         int lcur = am;
-        while (i < A.ncoef && (A.m[i] < 0 ? -A.m[i] : A.m[i]) == am) {
-            const int l = A.l[i];
+        while (i < A.ncoef && (Am[i] < 0 ? -Am[i] : Am[i]) == am) {
+            const int l = Al[i];
             while (lcur < l) {
                 const double pn = ((double)(2 * lcur + 1) * ct * pl - (double)(lcur + am) * pl_prev) / (double)(lcur + 1 - am);
                 pl_prev = pl;
                 pl = pn;
                 ++lcur;
             }
-            const double ang = A.m[i] > 0 ? cm : (A.m[i] < 0 ? sm : 1.0);
-            R = fma(A.cn[i] * pl, ang, R);
+            const double ang = Am[i] > 0 ? cm : (Am[i] < 0 ? sm : 1.0);
+            R = fma(Acn[i] * pl, ang, R);
             ++i;
         }
     }
     return R;
 }
 
-__global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
+__global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out) {
     const double kPi = 3.14159265358979323846;
+    const RenderArgs &A = Bt.a[blockIdx.y];
     const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t nvox = (size_t)A.nx * A.ny * A.nz;
     if (v >= nvox) return;
+    out += (size_t)blockIdx.y * nvox;
     const int ix = (int)(v % A.nx), iy = (int)((v / A.nx) % A.ny), iz = (int)(v / ((size_t)A.nx * A.ny));
     const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
     const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
@@ -87,7 +100,7 @@ __global__ void render_kernel(const RenderArgs A, float2 *__restrict__ out) {
             const double ct = r > 0.0 ? zb / r : 1.0;
             const double rho = sqrt(xb * xb + yb * yb);
             const double cphi = rho > 0.0 ? xb / rho : 1.0, sphi = rho > 0.0 ? yb / rho : 0.0;   // phi = atan2(y, x)
-            const double R = sh_radius(A, ct, cphi, sphi);
+            const double R = sh_radius(A, Bt.cn + A.coef0, Bt.l + A.coef0, Bt.m + A.coef0, ct, cphi, sphi);
             inside = r <= R;
         }
     } else if (A.kind == SCATMAN_SHAPE_RADIAL_MAP) {
@@ -121,11 +134,10 @@ static double factorial_d(int n) {
     return f;
 }
 
-// 0 ok, 1 bad argument
-int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err) {
+// Fills descriptor A (and, for harmonics, coefficients at coef0 of the pool arrays).  0 ok, 1 bad argument.
+static int fill_render_args(const scatman_shape &s, const scatman_grid &g, RenderArgs &A, double *Acn, signed char *Al, signed char *Am) {
     const double kPi = 3.14159265358979323846;
-    *err = cudaSuccess;
-    RenderArgs A = {};
+    A = RenderArgs{};
     A.kind = s.kind;
     A.delta = s.delta;
     A.beta = s.beta;
@@ -156,9 +168,9 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
                     return 1;
                 const int am = m < 0 ? -m : m;
                 const double n = std::sqrt((2 * l + 1) / (4 * kPi) * factorial_d(l - am) / factorial_d(l + am));
-                A.l[i] = (signed char)l;
-                A.m[i] = (signed char)m;
-                A.cn[i] = cv * n * (m != 0 ? std::sqrt(2.0) : 1.0);
+                Al[i] = (signed char)l;
+                Am[i] = (signed char)m;
+                Acn[i] = cv * n * (m != 0 ? std::sqrt(2.0) : 1.0);
                 if (l == 0) r00 += cv * n;
                 else norm2[l] += cv * cv;
             }
@@ -167,12 +179,12 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
             A.ncoef = s.ncoef;
             for (int i = 1; i < A.ncoef; ++i)   // insertion sort by (|m|, l): the order sh_radius walks
                 for (int j = i; j > 0; --j) {
-                    const int ka = (A.m[j] < 0 ? -A.m[j] : A.m[j]) * 64 + A.l[j];
-                    const int kb = (A.m[j - 1] < 0 ? -A.m[j - 1] : A.m[j - 1]) * 64 + A.l[j - 1];
+                    const int ka = (Am[j] < 0 ? -Am[j] : Am[j]) * 64 + Al[j];
+                    const int kb = (Am[j - 1] < 0 ? -Am[j - 1] : Am[j - 1]) * 64 + Al[j - 1];
                     if (ka >= kb) break;
-                    std::swap(A.l[j], A.l[j - 1]);
-                    std::swap(A.m[j], A.m[j - 1]);
-                    std::swap(A.cn[j], A.cn[j - 1]);
+                    std::swap(Al[j], Al[j - 1]);
+                    std::swap(Am[j], Am[j - 1]);
+                    std::swap(Acn[j], Acn[j - 1]);
                 }
             A.r_lo = (r00 - bound) * (1.0 - 1e-9) - 1e-300;
             A.r_hi = (r00 + bound) * (1.0 + 1e-9) + 1e-300;
@@ -188,9 +200,38 @@ int launch_render(const scatman_shape &s, const scatman_grid &g, float *d_dn, cu
             break;
         default: return 1;
     }
+    return 0;
+}
+
+// Renders h_shapes[0 .. batch) into d_dn[batch][nz][ny][nx][2]: one launch per RenderBatch of descriptors.
+// Returns 0, or 1 + the index of the first bad descriptor; *err = the CUDA status; *nlaunch = kernels launched.
+int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err,
+                        int *nlaunch) {
+    *err = cudaSuccess;
+    *nlaunch = 0;
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    render_kernel<<<(unsigned)((nvox + 255) / 256), 256, 0, st>>>(A, (float2 *)d_dn);
-    *err = cudaGetLastError();
+    static thread_local RenderBatch Bt;       // 31 KB: not on the stack
+    int b = 0;
+    while (b < batch) {
+        const int first = b;
+        int pool = 0;
+        Bt.n = 0;
+        while (b < batch && Bt.n < kBatchShapes) {
+            const scatman_shape &s = h_shapes[b];
+            const int nc = s.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS ? s.ncoef : 0;
+            if (nc < 0 || nc > kMaxCoef) return 1 + b;
+            if (pool + nc > kPoolCoef) break;
+            if (fill_render_args(s, g, Bt.a[Bt.n], Bt.cn + pool, Bt.l + pool, Bt.m + pool)) return 1 + b;
+            Bt.a[Bt.n].coef0 = pool;
+            pool += nc;
+            ++Bt.n;
+            ++b;
+        }
+        render_kernel<<<dim3((unsigned)((nvox + 255) / 256), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox);
+        ++*nlaunch;
+        *err = cudaGetLastError();
+        if (*err != cudaSuccess) return 0;
+    }
     return 0;
 }
 

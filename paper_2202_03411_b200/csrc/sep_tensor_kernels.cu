@@ -158,26 +158,27 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 
 // Balanced z splits.  Sequence 0 (stage X): weight of slice j = its live 128-y row tiles; sequence 1 + g (stage YZ, group g):
 // its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
-// every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam.
-__global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int ngs, int gw,
-                                     int nsx, int nzs, int *__restrict__ bx, int *__restrict__ by) {   // ngs YZ groups of gw flags
-    // bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
-    // One warp per sequence, 32 slices per step: warp scan of the weights; the lane of slice j writes the bounds with
-    // E(j - 1) < target(s) <= E(j) (E(-1) = -1; j = nz is a last, weightless slice so that E(nz) = total is covered).
-    // sequence 0: stage X over all nzt slices of the chunk; sequence 1 + b ng + g: stage YZ of item b, group g (its nz1 slices).
-    // Bounds are GLOBAL slice indices (jbase + j).
-    const int seq = blockIdx.x, lane = threadIdx.x;
+// every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam:
+// bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
+// One block of 256 threads per sequence: every thread sums a contiguous run of slices (all flag loads of the block are in
+// flight together), a block scan gives E at the run starts, and each thread then places the bounds that fall into its run.
+// sequence 0: stage X over all nzt slices of the chunk; sequence 1 + b ngs + g: stage YZ of item b, group g (its nz1 slices).
+// Bounds are GLOBAL slice indices (jbase + j).  nyz_seq = 0 skips the stage YZ sequences (the NUFFT route needs only stage X's).
+constexpr int kBoundsThreads = 256;
+__global__ void __launch_bounds__(kBoundsThreads)
+sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int ngs, int gw,
+                     int nsx, int nzs, int *__restrict__ bx, int *__restrict__ by) {   // ngs YZ groups of gw flags
+    const int seq = blockIdx.x, tid = threadIdx.x;
     const int ns = seq == 0 ? nsx : nzs;
     int *out = seq == 0 ? bx : by + (size_t)(seq - 1) * (nzs + 1);
     const int gsel = seq == 0 ? 0 : (seq - 1) % ngs;
     const int jbase = seq == 0 ? 0 : ((seq - 1) / ngs) * nz1;
     const int nz = seq == 0 ? nzt : nz1;
-    if (seq == 0 && nzt > 4096) {   // many stacked items: equal slice counts per range balance well enough, no scan
-        for (int sidx = lane; sidx <= ns; sidx += 32) out[sidx] = (int)(((long long)nzt * sidx) / ns);
+    if (seq == 0 && nzt > 65536) {   // very many stacked slices: equal slice counts per range balance well enough
+        for (int sidx = tid; sidx <= ns; sidx += kBoundsThreads) out[sidx] = (int)(((long long)nzt * sidx) / ns);
         return;
     }
     auto weight = [&](int j) -> unsigned {
-        if (j >= nz) return 0u;
         const unsigned char *fl = flags + (size_t)(jbase + j) * nkb;
         unsigned w = 0;
         if (seq == 0) {
@@ -187,38 +188,47 @@ __global__ void sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, in
         }
         return w;
     };
-    long long total = 0;
-    for (int j0 = 0; j0 < nz; j0 += 32) {
-        unsigned w = weight(j0 + lane);
-        for (int off = 16; off > 0; off >>= 1) w += __shfl_xor_sync(0xffffffffu, w, off);
-        total += w;
+    const int run = (nz + kBoundsThreads - 1) / kBoundsThreads;          // slices per thread
+    const int j0 = min(tid * run, nz), j1 = min(j0 + run, nz);
+    unsigned mine = 0;
+    for (int j = j0; j < j1; ++j) mine += weight(j);
+    // exclusive block scan of `mine` -> E(j0)
+    __shared__ unsigned wsum[kBoundsThreads / 32];
+    unsigned inc = mine;
+    const int lane = tid & 31, wid = tid >> 5;
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += v;
     }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    unsigned before = 0, tot = 0;
+    for (int w = 0; w < kBoundsThreads / 32; ++w) {
+        if (w < wid) before += wsum[w];
+        tot += wsum[w];
+    }
+    const long long total = tot;
     auto target = [&](int sidx) { return (total * sidx) / ns; };
-    long long carry = 0;    // E(j0)
-    unsigned wlast = 0;     // weight of slice j0 - 1
-    for (int j0 = 0; j0 <= nz; j0 += 32) {
-        const int j = j0 + lane;
-        const unsigned w = weight(j);
-        unsigned inc = w;
-        for (int off = 1; off < 32; off <<= 1) {
-            const unsigned v = __shfl_up_sync(0xffffffffu, inc, off);
-            if (lane >= off) inc += v;
-        }
-        unsigned wprev = __shfl_up_sync(0xffffffffu, w, 1);
-        if (lane == 0) wprev = wlast;
-        const long long hi = carry + (long long)(inc - w);             // E(j)
-        const long long lo = j == 0 ? -1 : hi - (long long)wprev;      // E(j - 1)
-        if (j <= nz && lo < hi) {
-            int sidx = total > 0 ? (int)(((lo + 1) * ns) / total) : 0;
-            if (sidx > ns) sidx = ns;
-            while (sidx > 0 && target(sidx - 1) > lo) --sidx;
-            while (sidx < ns && target(sidx) <= lo) ++sidx;
-            for (; sidx < ns && target(sidx) <= hi; ++sidx) out[sidx] = jbase + j;
-        }
-        carry += (long long)__shfl_sync(0xffffffffu, inc, 31);
-        wlast = __shfl_sync(0xffffffffu, w, 31);
+    long long E = (long long)before + (inc - mine);                      // E(j0)
+    // slice j (or the weightless last slice j = nz) receives the bounds with E(j - 1) < target <= E(j), E(-1) = -1
+    auto place = [&](int j, long long lo, long long hi) {
+        if (lo >= hi) return;
+        int sidx = total > 0 ? (int)(((lo + 1) * ns) / total) : 0;
+        if (sidx > ns) sidx = ns;
+        while (sidx > 0 && target(sidx - 1) > lo) --sidx;
+        while (sidx < ns && target(sidx) <= lo) ++sidx;
+        for (; sidx < ns && target(sidx) <= hi; ++sidx) out[sidx] = jbase + j;
+    };
+    // this thread's slices j0 .. j1-1: E(j) for j = j0 is E; E(j - 1) for j0 is E minus the weight of slice j0 - 1
+    long long prev = j0 == 0 ? -1 : E - (long long)weight(j0 - 1);
+    for (int j = j0; j < j1; ++j) {
+        place(j, prev, E);
+        prev = E;
+        E += weight(j);
     }
-    if (lane == 0) out[ns] = jbase + nz;
+    if (j0 < nz && j1 == nz) place(nz, prev, E);                         // the thread owning the last slice: E(nz) = total
+    if (nz == 0 && tid == 0) place(0, -1, 0);
+    if (tid == 0) out[ns] = jbase + nz;
 }
 
 // ------------------------------------------------------------------------------------------------ stage X
@@ -2068,7 +2078,8 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 }
 
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
-                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st) {
+                               __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
+                               bool x_only) {
     const int nyb = t.NY / kKB, nzt = p.nz * nb;
     cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
     if (e != cudaSuccess) return e;
@@ -2077,8 +2088,8 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
                                                                              d_Rp, d_flags64);
     sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
     const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;   // stage YZ's z splits: per item, or per item and 128-y group
-    sep_tc_bounds_kernel<<<1 + nb * ngs, 32, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, ngs, gw, t.nsx, t.nzs, d_bounds,
-                                                      d_bounds + (t.nsx + 1));
+    sep_tc_bounds_kernel<<<x_only ? 1 : 1 + nb * ngs, kBoundsThreads, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, ngs, gw, t.nsx, t.nzs,
+                                                                              d_bounds, d_bounds + (t.nsx + 1));
     return cudaGetLastError();
 }
 
