@@ -254,7 +254,7 @@ int scatman_create(scatman_ctx **out, int device) {
     if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess ||
         nufft_init_device() != cudaSuccess ||   // the NUFFT route's window polynomials -> constant memory of this device
         tensor_init_device() != cudaSuccess || sep_init_device() != cudaSuccess || sep_tc_init_device() != cudaSuccess ||
-        nufft_tc_init_device() != cudaSuccess) {
+        nufft_tc_init_device() != cudaSuccess || render_init_device() != cudaSuccess) {
         delete ctx;
         return SCATMAN_CUDA_ERROR;
     }

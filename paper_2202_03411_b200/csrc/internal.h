@@ -109,6 +109,7 @@ cudaError_t nufft_init_device();   // once per device (scatman_create): uploads 
 cudaError_t tensor_init_device();
 cudaError_t sep_init_device();
 cudaError_t sep_tc_init_device();
+cudaError_t render_init_device();
 cudaError_t launch_nufft_tables(const Plan &p, const NufftPlan &n, double2 *d_Tz, double2 *d_TxT, double2 *d_Ty, cudaStream_t st);
 cudaError_t launch_nufft_chunk(const float2 *d_rho, const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells,
                                const double2 *d_Tz, const double2 *d_TxT, const double2 *d_Ty, const double *d_q, double2 *d_P,

@@ -86,123 +86,138 @@ __global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
     if (i < n) bbox[i] = (i % 6) < 3 ? 0x7fffffff : -1;
 }
 
-// Threads are grouped as 16 x 4 x 4 output voxels per block so that the 2x2x2 source cells of a block share cache lines
-// for any rotation (row-shaped blocks gather along a slanted line and read 30x more sectors than they use).
-__global__ void orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz,
-                              double3 inv, const double *__restrict__ rotmat, const int *__restrict__ bbox,
-                              float2 *__restrict__ out) {
+// Output voxels are handled in TILES of 16 x 4 x 4 (256 threads, one voxel each) so that the 2x2x2 source cells of a tile share
+// cache lines for any rotation (row-shaped tiles gather along a slanted line and read 30x more sectors than they use).
+// A block owns one layer of tiles (fixed item b and tile row bz) and walks it: first every thread decides for ONE tile whether it
+// can hold material at all -- the tile's image in the body frame is a parallelepiped whose extent along each body axis follows
+// from three signed edge vectors, compared with the box of non-vacuum voxels widened by the interpolation cell -- then the block
+// zero-fills the tiles that cannot and resamples the others.  (One launch-sized block per tile, each loading the rotation and the
+// box and deciding on its own, was bound by that start-up latency, not by arithmetic or bytes: profiles/r02_orient_render.md.)
+__global__ void __launch_bounds__(256)
+orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz, double3 inv,
+              const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out) {
     const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
-    int blk = blockIdx.x;
-    const int bx = blk % nbx; blk /= nbx;
-    const int by = blk % nby; blk /= nby;
-    const int bz = blk % nbz;
-    const int b = blk / nbz;
-    const int ix = bx * 16 + (threadIdx.x & 15), iy = by * 4 + ((threadIdx.x >> 4) & 3), iz = bz * 4 + (threadIdx.x >> 6);
-    const double *R = rotmat + 9 * b;
-    // Most blocks of a grid lie outside the particle: the eight corners of this block of 16 x 4 x 4 output voxels go to the body
-    // frame (threads 0-7), and if their bounding range misses the box of non-vacuum voxels (widened by the voxel of the
-    // interpolation cell) on any axis, every output voxel of the block is vacuum: store zeros, skip the per-voxel arithmetic.
-    {
-        bool hit = false;
-        if (threadIdx.x < 32) {
-            const int c = threadIdx.x & 7;
-            const double xc = centre(min(bx * 16 + ((c & 1) ? 15 : 0), nx - 1), nx, dx);
-            const double yc = centre(min(by * 4 + ((c & 2) ? 3 : 0), ny - 1), ny, dy);
-            const double zc = centre(min(bz * 4 + ((c & 4) ? 3 : 0), nz - 1), nz, dz);
-            double f[3];
-            f[0] = (R[0] * xc + R[3] * yc + R[6] * zc) * inv.x + 0.5 * (double)(nx - 1);
-            f[1] = (R[1] * xc + R[4] * yc + R[7] * zc) * inv.y + 0.5 * (double)(ny - 1);
-            f[2] = (R[2] * xc + R[5] * yc + R[8] * zc) * inv.z + 0.5 * (double)(nz - 1);
-            const int *bb = bbox + 6 * b;
-            bool miss = false;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                double lo = f[d], hi = f[d];
-#pragma unroll
-                for (int off = 1; off < 8; off <<= 1) {
-                    lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, off));
-                    hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, off));
-                }
-                // the per-voxel test below is f > bb_lo - 1 && f < bb_hi + 1: no voxel of the block can pass it if the whole
-                // range lies at or beyond one of the two limits (an affine map takes the block into the hull of its corners)
-                miss |= hi <= (double)(bb[d] - 1) || lo >= (double)(bb[3 + d] + 1);
-            }
-            hit = !miss;
-        }
-        if (!__syncthreads_or(hit ? 1 : 0)) {
-            if (ix < nx && iy < ny && iz < nz)
-                out[(size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx + ix] = make_float2(0.f, 0.f);
-            return;
-        }
-    }
-    if (ix >= nx || iy >= ny || iz >= nz) return;
-    // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = f0 + ix * step (one row of R^T per axis)
-    const double yb = centre(iy, ny, dy), zb = centre(iz, nz, dz), xb0 = centre(0, nx, dx);
-    const double ix_dx = inv.x, iy_dy = inv.y, iz_dz = inv.z;   // reciprocals from the host: an FP64 division costs ~40 instructions
-    const double fx0 = (R[0] * xb0 + R[3] * yb + R[6] * zb) * ix_dx + 0.5 * (double)(nx - 1), sx = R[0] * dx * ix_dx;
-    const double fy0 = (R[1] * xb0 + R[4] * yb + R[7] * zb) * iy_dy + 0.5 * (double)(ny - 1), sy = R[1] * dx * iy_dy;
-    const double fz0 = (R[2] * xb0 + R[5] * yb + R[8] * zb) * iz_dz + 0.5 * (double)(nz - 1), sz = R[2] * dx * iz_dz;
+    const int bz = blockIdx.x % nbz, b = blockIdx.x / nbz;
+    __shared__ double sR[9];
+    __shared__ int sbb[6];
+    __shared__ unsigned char hit[256];
+    if (threadIdx.x < 9) sR[threadIdx.x] = rotmat[9 * b + threadIdx.x];
+    if (threadIdx.x >= 32 && threadIdx.x < 38) sbb[threadIdx.x - 32] = bbox[6 * b + threadIdx.x - 32];
+    __syncthreads();
+    const double *R = sR;
+    // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = origin + ix ex + iy ey + iz ez (one row of R^T per axis)
+    const double ex[3] = {R[0] * dx * inv.x, R[1] * dx * inv.y, R[2] * dx * inv.z};
+    const double ey[3] = {R[3] * dy * inv.x, R[4] * dy * inv.y, R[5] * dy * inv.z};
+    const double ez[3] = {R[6] * dz * inv.x, R[7] * dz * inv.y, R[8] * dz * inv.z};
+    const double xb0 = centre(0, nx, dx), yb0 = centre(0, ny, dy), zb0 = centre(0, nz, dz);
+    const double org[3] = {(R[0] * xb0 + R[3] * yb0 + R[6] * zb0) * inv.x + 0.5 * (double)(nx - 1),
+                           (R[1] * xb0 + R[4] * yb0 + R[7] * zb0) * inv.y + 0.5 * (double)(ny - 1),
+                           (R[2] * xb0 + R[5] * yb0 + R[8] * zb0) * inv.z + 0.5 * (double)(nz - 1)};
+    const int n3[3] = {nx, ny, nz};
     const float2 *src = in + (size_t)b * nx * ny * nz;
-    float2 *dst = out + (size_t)b * nx * ny * nz + ((size_t)iz * ny + iy) * nx;
-    {
-        const double fx = fma((double)ix, sx, fx0), fy = fma((double)ix, sy, fy0), fz = fma((double)ix, sz, fz0);
-        float2 o = make_float2(0.f, 0.f);
-        // the 2x2x2 cell holds material only if every coordinate lies within one voxel of the box of non-vacuum voxels
-        const int *bb = bbox + 6 * b;
-        if (fx > (double)(bb[0] - 1) && fx < (double)(bb[3] + 1) && fy > (double)(bb[1] - 1) && fy < (double)(bb[4] + 1) &&
-            fz > (double)(bb[2] - 1) && fz < (double)(bb[5] + 1)) {
-            const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
-            const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
-            // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
-            // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
-            // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
-            if (x0 >= 0 && y0 >= 0 && z0 >= 0 && x0 + 1 < nx && y0 + 1 < ny && z0 + 1 < nz) {
-                const float2 *c0 = src + ((size_t)z0 * ny + y0) * nx + x0;
-                const size_t sy = (size_t)nx, sz = (size_t)nx * ny;
-                const float2 v000 = __ldg(c0), v001 = __ldg(c0 + 1), v010 = __ldg(c0 + sy), v011 = __ldg(c0 + sy + 1);
-                const float2 v100 = __ldg(c0 + sz), v101 = __ldg(c0 + sz + 1), v110 = __ldg(c0 + sz + sy), v111 = __ldg(c0 + sz + sy + 1);
-                const bool same = v001.x == v000.x && v001.y == v000.y && v010.x == v000.x && v010.y == v000.y && v011.x == v000.x &&
-                                  v011.y == v000.y && v100.x == v000.x && v100.y == v000.y && v101.x == v000.x && v101.y == v000.y &&
-                                  v110.x == v000.x && v110.y == v000.y && v111.x == v000.x && v111.y == v000.y;
-                if (same) {
-                    dst[ix] = v000;
-                    return;
+    float2 *dstb = out + (size_t)b * nx * ny * nz;
+    const int lx = threadIdx.x & 15, ly = (threadIdx.x >> 4) & 3, lz = threadIdx.x >> 6;
+    const int iz = bz * 4 + lz;
+    const int wz = min(3, nz - 1 - bz * 4);                         // tile extent - 1 along z
+    const int ntile = nbx * nby;
+    for (int t0 = 0; t0 < ntile; t0 += 256) {
+        {   // phase 1: thread t decides tile t0 + t
+            const int t = t0 + threadIdx.x;
+            bool h = false;
+            if (t < ntile) {
+                const int bx = t % nbx, by = t / nbx;
+                const int wx = min(15, nx - 1 - bx * 16), wy = min(3, ny - 1 - by * 4);
+                h = true;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const double f0 = org[d] + (double)(bx * 16) * ex[d] + (double)(by * 4) * ey[d] + (double)(bz * 4) * ez[d];
+                    const double sx = (double)wx * ex[d], sy = (double)wy * ey[d], sz = (double)wz * ez[d];
+                    const double lo = f0 + fmin(sx, 0.0) + fmin(sy, 0.0) + fmin(sz, 0.0);
+                    const double hi = f0 + fmax(sx, 0.0) + fmax(sy, 0.0) + fmax(sz, 0.0);
+                    // the per-voxel test below is f > bb_lo - 1 && f < bb_hi + 1; a slack of 1e-9 voxels covers the rounding of this
+                    // bound against the per-voxel evaluation (a wrongly kept tile only costs time)
+                    if (hi <= (double)(sbb[d] - 1) - 1e-9 || lo >= (double)(sbb[3 + d] + 1) + 1e-9 || sbb[3 + d] < 0) h = false;
                 }
+                (void)n3;
             }
-            const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
-            const double wx[2] = {1.0 - tx, tx}, wy[2] = {1.0 - ty, ty}, wz[2] = {1.0 - tz, tz};
-            double are = 0.0, aim = 0.0;
-#pragma unroll
-            for (int cz = 0; cz < 2; ++cz) {
-                const int zi = z0 + cz;
-                if (zi < 0 || zi >= nz) continue;
-#pragma unroll
-                for (int cy = 0; cy < 2; ++cy) {
-                    const int yi = y0 + cy;
-                    if (yi < 0 || yi >= ny) continue;
-                    const double wyz = wy[cy] * wz[cz];
-                    const float2 *row = src + ((size_t)zi * ny + yi) * nx;
-#pragma unroll
-                    for (int cx = 0; cx < 2; ++cx) {
-                        const int xi = x0 + cx;
-                        if (xi < 0 || xi >= nx) continue;
-                        const float2 v = __ldg(row + xi);
-                        if (v.x == 0.f && v.y == 0.f) continue;   // most of a grid is vacuum: skip the FP64 conversions
-                        const double w = wx[cx] * wyz;
-                        are = fma(w, (double)v.x, are);
-                        aim = fma(w, (double)v.y, aim);
+            hit[threadIdx.x] = h ? 1 : 0;
+        }
+        __syncthreads();
+        const int tend = min(256, ntile - t0);
+        for (int tt = 0; tt < tend; ++tt) {
+            const int t = t0 + tt;
+            const int bx = t % nbx, by = t / nbx;
+            const int ix = bx * 16 + lx, iy = by * 4 + ly;
+            if (ix >= nx || iy >= ny || iz >= nz) continue;
+            float2 *dst = dstb + ((size_t)iz * ny + iy) * nx;
+            if (!hit[tt]) {
+                dst[ix] = make_float2(0.f, 0.f);
+                continue;
+            }
+            const double fx = org[0] + (double)ix * ex[0] + (double)iy * ey[0] + (double)iz * ez[0];
+            const double fy = org[1] + (double)ix * ex[1] + (double)iy * ey[1] + (double)iz * ez[1];
+            const double fz = org[2] + (double)ix * ex[2] + (double)iy * ey[2] + (double)iz * ez[2];
+            float2 o = make_float2(0.f, 0.f);
+            // the 2x2x2 cell holds material only if every coordinate lies within one voxel of the box of non-vacuum voxels
+            if (fx > (double)(sbb[0] - 1) && fx < (double)(sbb[3] + 1) && fy > (double)(sbb[1] - 1) && fy < (double)(sbb[4] + 1) &&
+                fz > (double)(sbb[2] - 1) && fz < (double)(sbb[5] + 1)) {
+                const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
+                const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
+                // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
+                // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
+                // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
+                bool done = false;
+                if (x0 >= 0 && y0 >= 0 && z0 >= 0 && x0 + 1 < nx && y0 + 1 < ny && z0 + 1 < nz) {
+                    const float2 *c0 = src + ((size_t)z0 * ny + y0) * nx + x0;
+                    const size_t sy = (size_t)nx, sz = (size_t)nx * ny;
+                    const float2 v000 = __ldg(c0), v001 = __ldg(c0 + 1), v010 = __ldg(c0 + sy), v011 = __ldg(c0 + sy + 1);
+                    const float2 v100 = __ldg(c0 + sz), v101 = __ldg(c0 + sz + 1), v110 = __ldg(c0 + sz + sy), v111 = __ldg(c0 + sz + sy + 1);
+                    const bool same = v001.x == v000.x && v001.y == v000.y && v010.x == v000.x && v010.y == v000.y && v011.x == v000.x &&
+                                      v011.y == v000.y && v100.x == v000.x && v100.y == v000.y && v101.x == v000.x && v101.y == v000.y &&
+                                      v110.x == v000.x && v110.y == v000.y && v111.x == v000.x && v111.y == v000.y;
+                    if (same) {
+                        o = v000;
+                        done = true;
                     }
                 }
+                if (!done) {
+                    const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
+                    const double wxx[2] = {1.0 - tx, tx}, wyy[2] = {1.0 - ty, ty}, wzz[2] = {1.0 - tz, tz};
+                    double are = 0.0, aim = 0.0;
+#pragma unroll
+                    for (int cz = 0; cz < 2; ++cz) {
+                        const int zi = z0 + cz;
+                        if (zi < 0 || zi >= nz) continue;
+#pragma unroll
+                        for (int cy = 0; cy < 2; ++cy) {
+                            const int yi = y0 + cy;
+                            if (yi < 0 || yi >= ny) continue;
+                            const double wyz = wyy[cy] * wzz[cz];
+                            const float2 *row = src + ((size_t)zi * ny + yi) * nx;
+#pragma unroll
+                            for (int cx = 0; cx < 2; ++cx) {
+                                const int xi = x0 + cx;
+                                if (xi < 0 || xi >= nx) continue;
+                                const float2 v = __ldg(row + xi);
+                                if (v.x == 0.f && v.y == 0.f) continue;   // most of a grid is vacuum: skip the FP64 conversions
+                                const double w = wxx[cx] * wyz;
+                                are = fma(w, (double)v.x, are);
+                                aim = fma(w, (double)v.y, aim);
+                            }
+                        }
+                    }
+                    o = make_float2((float)are, (float)aim);
+                }
             }
-            o = make_float2((float)are, (float)aim);
+            dst[ix] = o;
         }
-        dst[ix] = o;
+        __syncthreads();
     }
 }
 
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
                           cudaStream_t st) {
-    const size_t blocks = (size_t)((p.nx + 15) / 16) * ((p.ny + 3) / 4) * ((p.nz + 3) / 4) * batch;
+    const size_t blocks = (size_t)((p.nz + 3) / 4) * batch;     // one block per layer of 16 x 4 x 4 tiles
     if (blocks > 0x7fffffffull || (size_t)p.nz * batch > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     bbox_init_kernel<<<(6 * batch + 255) / 256, 256, 0, st>>>(d_bbox, 6 * batch);
     bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox);

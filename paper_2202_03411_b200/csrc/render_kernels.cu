@@ -22,6 +22,7 @@ struct RenderArgs {
     double a, b, c;          // ellipsoid: 1 / semi-axis
     int ncoef, coef0;        // spherical harmonics: value = sum cn[coef0 + i] P_{l}^{|m|}(cos theta) {1, cos m phi, sin m phi}, i < ncoef
     double r_lo, r_hi;       // every voxel with |r| < r_lo is inside, with |r| > r_hi outside
+    double r2_in, r2_out;    // any kind: |r|^2 < r2_in is inside, |r|^2 > r2_out outside, without rotating (-1 / +inf: no such sphere)
     int nlat, nlon;          // radial map
     const double *radii;
     int nvx, nvy, nvz;       // volume map
@@ -30,14 +31,16 @@ struct RenderArgs {
 };
 
 // The shapes of one launch: descriptors + the pooled harmonic coefficients (sorted per shape by (|m|, l)); < 32 KB of kernel parameters.
-constexpr int kBatchShapes = 96, kPoolCoef = 1024;
+constexpr int kBatchShapes = 88, kPoolCoef = 1024;
 struct RenderBatch {
     int n;
     RenderArgs a[kBatchShapes];
     double cn[kPoolCoef];                 // c * N_lm * (m != 0 ? sqrt 2 : 1)
     signed char l[kPoolCoef], m[kPoolCoef];   // m as given (sign selects cos / sin)
 };
-static_assert(sizeof(RenderBatch) <= 32000, "kernel parameters are limited to 32764 bytes");
+static_assert(sizeof(RenderBatch) <= 32700, "kernel parameters are limited to 32764 bytes");
+
+__constant__ double c_rcp[40];   // 1 / n, n = 1 .. 39 (l <= 32); filled by render_init_device
 
 // R(theta, phi) = sum_i cn[i] P_{l_i}^{|m_i|}(cos theta) {1 | cos |m| phi | sin |m| phi}, the triplets sorted by (|m|, l):
 // P_m^m and (cos m phi, sin m phi) advance with m, P_l^m by the upward recurrence in l
@@ -62,7 +65,9 @@ __device__ double sh_radius(const RenderArgs &A, const double *__restrict__ Acn,
         while (i < A.ncoef && (Am[i] < 0 ? -Am[i] : Am[i]) == am) {
             const int l = Al[i];
             while (lcur < l) {
-                const double pn = ((double)(2 * lcur + 1) * ct * pl - (double)(lcur + am) * pl_prev) / (double)(lcur + 1 - am);
+                // (an FP64 division costs ~40 instructions; 1 / n comes from a table, one rounding more than the quotient,
+                // far inside the surface-tie margin of the rendering)
+                const double pn = ((double)(2 * lcur + 1) * ct * pl - (double)(lcur + am) * pl_prev) * c_rcp[lcur + 1 - am];
                 pl_prev = pl;
                 pl = pn;
                 ++lcur;
@@ -82,10 +87,26 @@ __global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__
     const size_t nvox = (size_t)A.nx * A.ny * A.nz;
     if (v >= nvox) return;
     out += (size_t)blockIdx.y * nvox;
-    const int ix = (int)(v % A.nx), iy = (int)((v / A.nx) % A.ny), iz = (int)(v / ((size_t)A.nx * A.ny));
+    int ix, iy, iz;
+    if (nvox <= 0x7fffffffull) {   // 32-bit divisions (the usual case)
+        const unsigned v32 = (unsigned)v, row = v32 / (unsigned)A.nx;
+        ix = (int)(v32 - row * (unsigned)A.nx);
+        iz = (int)(row / (unsigned)A.ny);
+        iy = (int)(row - (unsigned)iz * (unsigned)A.ny);
+    } else {
+        ix = (int)(v % A.nx); iy = (int)((v / A.nx) % A.ny); iz = (int)(v / ((size_t)A.nx * A.ny));
+    }
     const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
     const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
     const double z = ((double)iz - 0.5 * (double)(A.nz - 1)) * A.dz;
+    // |r| does not change under the rotation: voxels inside the shape's inscribed sphere or outside its circumscribed one are
+    // decided from x^2 + y^2 + z^2 alone (most of a grid); the margins of 1e-12 leave every close call to the full test below,
+    // so the rendering is voxel for voxel what the full test gives.
+    const double r2 = x * x + y * y + z * z;
+    if (r2 > A.r2_out || r2 < A.r2_in) {
+        out[v] = r2 < A.r2_in ? make_float2(A.delta, A.beta) : make_float2(0.f, 0.f);
+        return;
+    }
     const double xb = A.Rt[0] * x + A.Rt[1] * y + A.Rt[2] * z;
     const double yb = A.Rt[3] * x + A.Rt[4] * y + A.Rt[5] * z;
     const double zb = A.Rt[6] * x + A.Rt[7] * y + A.Rt[8] * z;
@@ -97,9 +118,11 @@ __global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__
         const double r = sqrt(xb * xb + yb * yb + zb * zb);
         if (r < A.r_lo) inside = true;
         else if (r <= A.r_hi) {
-            const double ct = r > 0.0 ? zb / r : 1.0;
+            const double ir = r > 0.0 ? 1.0 / r : 0.0;
+            const double ct = r > 0.0 ? zb * ir : 1.0;
             const double rho = sqrt(xb * xb + yb * yb);
-            const double cphi = rho > 0.0 ? xb / rho : 1.0, sphi = rho > 0.0 ? yb / rho : 0.0;   // phi = atan2(y, x)
+            const double irho = rho > 0.0 ? 1.0 / rho : 0.0;
+            const double cphi = rho > 0.0 ? xb * irho : 1.0, sphi = yb * irho;   // phi = atan2(y, x)
             const double R = sh_radius(A, Bt.cn + A.coef0, Bt.l + A.coef0, Bt.m + A.coef0, ct, cphi, sphi);
             inside = r <= R;
         }
@@ -128,6 +151,13 @@ __global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__
     out[v] = inside ? make_float2(A.delta, A.beta) : make_float2(0.f, 0.f);
 }
 
+cudaError_t render_init_device() {   // per device (scatman_create)
+    double rcp[40];
+    rcp[0] = 0.0;
+    for (int n = 1; n < 40; ++n) rcp[n] = 1.0 / (double)n;
+    return cudaMemcpyToSymbol(c_rcp, rcp, sizeof(rcp));
+}
+
 static double factorial_d(int n) {
     double f = 1.0;
     for (int i = 2; i <= n; ++i) f *= (double)i;
@@ -138,6 +168,8 @@ static double factorial_d(int n) {
 static int fill_render_args(const scatman_shape &s, const scatman_grid &g, RenderArgs &A, double *Acn, signed char *Al, signed char *Am) {
     const double kPi = 3.14159265358979323846;
     A = RenderArgs{};
+    A.r2_in = -1.0;
+    A.r2_out = INFINITY;
     A.kind = s.kind;
     A.delta = s.delta;
     A.beta = s.beta;
@@ -154,6 +186,11 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
         case SCATMAN_SHAPE_ELLIPSOID:
             if (!(s.a > 0.0 && s.b > 0.0 && s.c > 0.0)) return 1;
             A.a = 1.0 / s.a; A.b = 1.0 / s.b; A.c = 1.0 / s.c;
+            {
+                const double rmin = std::fmin(s.a, std::fmin(s.b, s.c)), rmax = std::fmax(s.a, std::fmax(s.b, s.c));
+                A.r2_in = rmin * rmin * (1.0 - 1e-12);
+                A.r2_out = rmax * rmax * (1.0 + 1e-12);
+            }
             break;
         case SCATMAN_SHAPE_SPHERICAL_HARMONICS: {
             if (s.ncoef < 1 || s.ncoef > kMaxCoef || !s.h_coef) return 1;
@@ -188,6 +225,8 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
                 }
             A.r_lo = (r00 - bound) * (1.0 - 1e-9) - 1e-300;
             A.r_hi = (r00 + bound) * (1.0 + 1e-9) + 1e-300;
+            A.r2_in = A.r_lo > 0.0 ? A.r_lo * A.r_lo * (1.0 - 1e-12) : -1.0;
+            A.r2_out = A.r_hi > 0.0 ? A.r_hi * A.r_hi * (1.0 + 1e-12) : 0.0;   // r_hi <= 0: the radius is nowhere positive
             break;
         }
         case SCATMAN_SHAPE_RADIAL_MAP:
@@ -197,6 +236,7 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
         case SCATMAN_SHAPE_VOLUME_MAP:
             if (s.nvx < 1 || s.nvy < 1 || s.nvz < 1 || !s.d_volume || !(s.vdx > 0.0)) return 1;
             A.nvx = s.nvx; A.nvy = s.nvy; A.nvz = s.nvz; A.vol = s.d_volume; A.vdx = 1.0 / s.vdx;
+            A.r2_out = 0.25 * s.vdx * s.vdx * ((double)s.nvx * s.nvx + (double)s.nvy * s.nvy + (double)s.nvz * s.nvz) * (1.0 + 1e-12);
             break;
         default: return 1;
     }
