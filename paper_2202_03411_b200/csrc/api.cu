@@ -526,7 +526,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.dx = g.dx; p.dy = g.dy; p.dz = g.dz; p.lambda = lambda;
     p.npix = (int64_t)npx * npy; p.batch = batch; p.rho_mode = rho_mode;
     p.nvox = (int64_t)g.nx * g.ny * g.nz;
-    sp.tensor = method != SCATMAN_METHOD_SIMT_TABLE && g.nx <= 1024;   // stage X keeps an Ex tile of >= 16 columns resident
+    sp.tensor = method != SCATMAN_METHOD_SIMT_TABLE && g.nx <= 1024 && g.ny <= 2048;   // stage X keeps an Ex tile of >= 16 columns resident; stage YZ's slice masks hold 32 64-y blocks
     sp.nzs = sep_zsplit(p, npx, npy, num_sms);
     if (sp.tensor) sp.tc = make_sep_tc_plan(p, npx, npy, num_sms);
     size_t off = 0;

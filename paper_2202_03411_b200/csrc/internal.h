@@ -73,12 +73,12 @@ cudaError_t launch_sep_item(const float2 *d_rho, const Plan &p, const float2 *d_
                             float2 *d_partial, float *d_I, cudaStream_t st);
 // separable route on tensor cores (sep_tensor_kernels.cu)
 struct SepTcPlan {
-    int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x64), grid rows (x128)
-    int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits, partial sums per point, ceil(log2 nx)
-    int NX = 64, nsx = 1, x_ncta = 1;          // stage X: a columns per resident Ex tile, z splits, CTAs per work item
-    int nyz = 64, yz_ncta = 1;                 // stage YZ: a columns per accumulator (128, or 64 for narrow grids), CTAs per work item
-    bool yz_stream = false;                    // stage YZ: one accumulator per slice, both operands streamed (sep_tc_yzs_kernel)
-    bool yz_t = false;                         // stage YZ transposed, Ey resident for all y (sep_tc_yzt_kernel<yzt_nb>)
+    int NY = 0, NXP = 0, NPXP = 0, NPYP = 0;   // padded y (x128), x (x64), grid columns (x128), grid rows (x128; x256 in the streamed form)
+    int ng = 0, nzs = 1, nsplit = 1, L = 0;    // 128-y groups, z splits of stage YZ (= partial sums per point), ceil(log2 nx)
+    int NX = 64, nsx = 1, x_ncta = 2;          // stage X: a columns per resident Ex tile, z splits, CTAs per work item (always pairs)
+    int nyz = 128, yz_ncta = 2;                // stage YZ: a columns per tile, CTAs per work item (always pairs)
+    bool yz_stream = true;                     // stage YZ keeps one accumulator per slice (both forms): bounds and partial sums per item
+    bool yz_t = false;                         // stage YZ transposed, Ey resident for all y (SepYztPolicy<yzt_nb>); else sep_tc_yzs_kernel
     int yzt_nb = 0;
     int nb = 1;                                // batch items per chunk (stacked along z, one set of launches per chunk)
 };

@@ -79,6 +79,8 @@ struct GItem {
 template <int NB_>
 struct StageY {
     static constexpr int NB = NB_;
+    static constexpr bool kUnrollEpilogue = false;
+    static constexpr int kEpilogueRegs = 0;
     using Params = YParams;
     using Item = GItem;
     __device__ static int nitems(const Params &P) { return P.ntb * P.nsplit; }
@@ -139,6 +141,8 @@ struct ZParams {
 template <int NB_>
 struct StageZ {
     static constexpr int NB = NB_;
+    static constexpr bool kUnrollEpilogue = false;
+    static constexpr int kEpilogueRegs = 0;
     using Params = ZParams;
     using Item = GItem;
     __device__ static int nitems(const Params &P) { return P.ntb * P.nsplit; }

@@ -8,11 +8,13 @@
 // Stage X's epilogue rescales H and splits it into the FP16 planes stage YZ reads; stage YZ's epilogue applies the slice
 // phase e^{i qz(a,b) z_j} to the accumulator tile and sums over slices in registers.  Vacuum is skipped in 64-y blocks (byte
 // flags); batch items are stacked along z; z splits are balanced on the device by live tiles.
-// Kernels (each is selected by make_sep_tc_plan and covered by tests/test_gpu_qgrid.py):
-//   stage X   sep_tc_x2_kernel<NX>  CTA pairs, UMMA 256 x 2NX, Ex tile resident          | sep_tc_x_kernel<NX>  one CTA
-//   stage YZ  sep_tc_yzt_kernel<64> CTA pairs, transposed, Ey resident for all y (N_y <= 256)
-//             sep_tc_yzs_kernel     CTA pairs, both operands streamed (N_y <= 2048)
-//             sep_tc_yz128_kernel   one CTA, Ey resident per 128-y group (any size)      | sep_tc_yz_kernel  grids of <= 64 columns
+// Kernels (selected by make_sep_tc_plan, covered by tests/test_gpu_qgrid.py):
+//   stage X   tcg::cgemm_kernel<SepXPolicy<NX>>     CTA pairs, UMMA 256 x 2NX, Ex tile resident (NX = 64 / 32 / 16 for N_x <= 256 / 512 / 1024)
+//   stage YZ  tcg::cgemm_kernel<SepYztPolicy<64>>   CTA pairs, transposed, Ey resident for all y (N_y <= 256)
+//             sep_tc_yzs_kernel                     CTA pairs, both operands streamed (N_y <= 2048)
+// Stage X and the transposed stage YZ are instances of ONE producer / issuer / epilogue pipeline (tc_cgemm.cuh), which also runs
+// the NUFFT route's stages Y and Z; odd tile counts are handled by running the last tile twice in the pair, so no single-CTA
+// variants exist.  Grids with N_x > 1024 or N_y > 2048 use the CUDA-core stages (sep_kernels.cu).
 //
 // Slice phase: qz z_j = 2 pi t (2j - nz + 1) with t = qz dz / (4 pi) turns; frac(t) is kept as a 32-bit fixed-point
 // fraction of a turn, so the product with the integer (2j - nz + 1) wraps modulo one turn for free (error <= 512 * 2^-33
@@ -24,6 +26,7 @@
 
 #include "internal.h"
 #include "ptx_sm100.h"
+#include "tc_cgemm.cuh"
 
 namespace scatman {
 
@@ -35,10 +38,8 @@ namespace {
 constexpr int kM = 128;              // UMMA M: rows of the A operand tile
 constexpr int kKB = 64;              // K per block (one 128-byte swizzle row of FP16)
 constexpr int kSlotA = kM * kKB * 2; // 16384: one plane, one K block of an A tile
-constexpr int kNyz = 64;             // stage YZ: a columns per accumulator
 constexpr int kThreadsTc = 384;      // warp 0 TMA, 1 and 3 MMA issuers, 2 TMEM, 4-11 epilogue
 constexpr uint32_t kTmemColsTc = 512;
-constexpr int kNBuf = 4;             // accumulator buffers (128 columns each: D_re 64 + D_im 64)
 
 __device__ __forceinline__ double centre_t(int i, int n, double d) { return ((double)i - 0.5 * (double)(n - 1)) * d; }
 
@@ -232,1074 +233,99 @@ sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, 
 }
 
 // ------------------------------------------------------------------------------------------------ stage X
+// H_j[a, y] = sum_x rho~_j[y, x] e^{i qx[a] x}: the streamed-A x resident-B pipeline of tc_cgemm.cuh.  A unit = one live 128-y row tile
+// of a slice (rows y = TMEM lanes, K = x); the resident operand = NX rows per CTA of the Ex tile of 2 NX grid columns a
+// (NX * NXP * 8 bytes <= 128 KB: NX = 64 / 32 / 16 for N_x <= 256 / 512 / 1024).  A work item = (column tile, balanced z range);
+// the pair takes two consecutive live tiles (an odd last one is run twice, the peer's copy discarded).  The epilogue rescales the
+// accumulator by the constant 2^(-9 - ceil(log2 N_x)) (|H| <= 2^14.5 whatever the data), splits it hi / lo and stores H as the
+// planes [4][N_z][NPXP][NY], y fastest = K-major for stage YZ (a warp stores 32 consecutive y).
 struct SepXParams {
-    int nz, NY, NPXP, ng, nkx, nta, nsx, nkb;   // nkx = NXP / 64, nta = a tiles of NX columns, nsx = z splits, nkb = NY / 64
+    int nk;                                     // NXP / 64
+    int nz, NY, NPXP, ng, nta, nsx, nkb;        // nta = tiles of 2 NX columns, nsx = z splits, nkb = NY / 64
     float hscale;                               // 2^(-9 - L): accumulator (2^10 sR H) -> stored H (sH H)
     const unsigned char *flags;                 // [nz][nkb]
     const int *zb;                              // [nsx + 1] balanced z split bounds (sep_tc_bounds_kernel)
     __half *Hp;                                 // [4][nz][NPXP][NY]
 };
 
-// NX = a columns per accumulator = rows of the resident Ex tile (NX * NXP * 8 bytes <= 128 KB)
 template <int NX>
-__global__ void __launch_bounds__(kThreadsTc, 1)
-sep_tc_x_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepXParams P) {
-    constexpr int kSmemE = 131072;                // resident Ex planes: [4][nkx][NX rows x 128 bytes]
-    constexpr int kStages = 6;                    // ring of single-plane 64-x blocks of a rho~ row tile (16 KB each)
-    constexpr int kBlkE = NX * kKB * 2;           // bytes of one plane, one K block of the Ex tile
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *sE = smem;
-    uint8_t *sR = smem + kSmemE;
-    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kSlotA);
-    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
-    uint64_t *r_full = bars + 2, *r_empty = r_full + kStages;
-    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNBuf, *first_done = t_empty + kNBuf;
-    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNBuf);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nitems = P.nta * P.nsx;
-
-    if (warp == 0 && lane == 0) {
-        ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
-    }
-    if (warp == 1 && lane == 0) {
-        ptx::mbar_init(e_full, 1);
-        ptx::mbar_init(e_empty, 2);          // both MMA issuers
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(r_full + i, 1);
-            ptx::mbar_init(r_empty + i, 2);
-        }
-        for (int i = 0; i < kNBuf; ++i) {
-            ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 8);
-            ptx::mbar_init(first_done + i, 1);
-        }
-        ptx::fence_barrier_init();
-        ptx::fence_proxy_async();
-    }
-    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::tc_fence_after();
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
-
-    // units of an item: (slice j of its z range, 128-y group g) with a non-empty 64-y block; u = (j - z0) * ng + g
-    auto zrange = [&](int s, int &z0, int &z1) {
-        z0 = __ldg(P.zb + s);
-        z1 = __ldg(P.zb + s + 1);
+struct SepXPolicy {
+    static constexpr int NB = NX;
+    static constexpr bool kUnrollEpilogue = false;
+    static constexpr int kEpilogueRegs = 0;
+    using Params = SepXParams;
+    struct Item {
+        int ta, z0, z1;
     };
-
-    if (warp == 0) {
-        // ===================================================================== TMA producer
-        int slot = 0;
-        uint32_t phase = 0;
-        int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const int ta = item % P.nta, s = item / P.nta;   // a tiles fastest: concurrent CTAs stream the same rho~ tiles
-            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
-            if (ptx::elect_one()) {
-                ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(4 * P.nkx * kBlkE));
-                for (int pl = 0; pl < 4; ++pl)
-                    for (int kx = 0; kx < P.nkx; ++kx)
-                        ptx::tma_load_3d(sE + (pl * P.nkx + kx) * kBlkE, &tmB, e_full, kx * kKB, ta * NX, pl);
-            }
-            __syncwarp();
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n;
+    __device__ static int nitems(const Params &P) { return P.nta * P.nsx; }
+    __device__ static Item item(const Params &P, int index) {
+        Item it;
+        it.ta = index % P.nta;   // column tiles fastest: concurrent pairs stream the same rho~ tiles
+        const int sp = index / P.nta;
+        it.z0 = __ldg(P.zb + sp);
+        it.z1 = __ldg(P.zb + sp + 1);
+        return it;
+    }
+    __device__ static int b_row0(const Params &, const Item &it) { return it.ta * 2 * NX; }
+    // unit id = slice * ng + 128-y group
+    struct Units {
+        LiveUnits lu;
+        int base;
+        __device__ void begin(const Params &P, const Item &it, int lane) {
+            lu.begin(P.flags, P.nkb, it.z0, it.z1, P.ng, 0, lane);
+            base = it.z0 * P.ng;
+        }
+        __device__ bool next(int &u0, int &u1, bool &dup, uint32_t &kmask) {
+            kmask = 0xffffffffu;
+            int n0, n1;
             uint32_t f;
-            while (un.next(n, f)) {
-                    const int j = z0 + n / P.ng, g = n % P.ng;
-                    for (int kx = 0; kx < P.nkx; ++kx)
-                        for (int pl = 0; pl < 4; ++pl) {
-                            ptx::mbar_wait(r_empty + slot, phase ^ 1);
-                            if (ptx::elect_one()) {
-                                ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)kSlotA);
-                                ptx::tma_load_3d(sR + slot * kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, pl);
-                            }
-                            __syncwarp();
-                            if (++slot == kStages) { slot = 0; phase ^= 1; }
-                        }
-                }
+            if (!lu.next(n0, f)) return false;
+            dup = !lu.next(n1, f);
+            u0 = base + n0;
+            u1 = dup ? u0 : base + n1;
+            return true;
         }
-    } else if (warp == 1 || warp == 3) {
-        // ===================================================================== MMA issuers
-        // Two issuer warps share every stage: k-step ks belongs to issuer ks % 2.  At N = 64 a tcgen05.mma is bound by its
-        // shared-memory operand fetch (48 cycles) and a single issuing thread exposes whatever it spends between stages
-        // (measured 72-107 cycles per MMA with one issuer); two threads hide each other's gaps (as in tensor_kernel.cu).
-        // The unit's first k-step (accumulate = 0) is issuer 0's; issuer 1 starts on the unit once it has completed.
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, NX, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, NX, true);
-        const uint64_t descR0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sR));
-        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
-        constexpr uint64_t kR = kSlotA >> 4, kE = kBlkE >> 4;
-        const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
-        int slot = 0;
-        uint32_t phase = 0, u = 0;
-        int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const int s = item / P.nta;
-            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
-            ptx::tc_fence_after();
-            const uint64_t kEpl = (uint64_t)P.nkx * kE;   // descriptor distance between Ex planes
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                    const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
-                    ptx::mbar_wait(t_empty + buf, upar ^ 1);
-                    ptx::tc_fence_after();
-                    const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
-                    for (int kx = 0; kx < P.nkx; ++kx)
-                        for (int pl = 0; pl < 4; ++pl) {
-                            if (iw == 1 && kx == 0 && pl == 0) {   // D must have been initialised by issuer 0
-                                ptx::mbar_wait(first_done + buf, upar);
-                                ptx::tc_fence_after();
-                            }
-                            ptx::mbar_wait(r_full + slot, phase);
-                            ptx::tc_fence_after();
-                            if (ptx::elect_one()) {
-#pragma unroll
-                                for (int kk = 0; kk < 2; ++kk) {
-                                    const int ks = 2 * kk + iw;
-                                    const uint64_t a = descR0 + (uint64_t)slot * kR + (uint64_t)(ks * 2);
-                                    const uint64_t e_reh = descE0 + (uint64_t)kx * kE + (uint64_t)(ks * 2);
-                                    const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
-                                    const uint32_t acc0 = (kx == 0 && ks == 0) ? 0u : 1u;
-                                    // (Ar + i Ai)(Er + i Ei), A = rho~ plane of this stage, three split products AhEh + AlEh + AhEl
-                                    if (pl == 0) {          // Re_hi
-                                        ptx::umma_f16(d_re, a, e_reh, idesc_pos, acc0);
-                                        ptx::umma_f16(d_im, a, e_imh, idesc_pos, acc0);
-                                        ptx::umma_f16(d_re, a, e_rel, idesc_pos, 1u);
-                                        ptx::umma_f16(d_im, a, e_iml, idesc_pos, 1u);
-                                    } else if (pl == 1) {   // Re_lo
-                                        ptx::umma_f16(d_re, a, e_reh, idesc_pos, 1u);
-                                        ptx::umma_f16(d_im, a, e_imh, idesc_pos, 1u);
-                                    } else if (pl == 2) {   // Im_hi
-                                        ptx::umma_f16(d_re, a, e_imh, idesc_neg, 1u);
-                                        ptx::umma_f16(d_im, a, e_reh, idesc_pos, 1u);
-                                        ptx::umma_f16(d_re, a, e_iml, idesc_neg, 1u);
-                                        ptx::umma_f16(d_im, a, e_rel, idesc_pos, 1u);
-                                    } else {                // Im_lo
-                                        ptx::umma_f16(d_re, a, e_imh, idesc_neg, 1u);
-                                        ptx::umma_f16(d_im, a, e_reh, idesc_pos, 1u);
-                                    }
-                                    if (iw == 0 && kk == 0 && kx == 0 && pl == 0) ptx::umma_commit(first_done + buf);
-                                }
-                                ptx::umma_commit(r_empty + slot);
-                            }
-                            __syncwarp();
-                            if (++slot == kStages) { slot = 0; phase ^= 1; }
-                        }
-                    if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
-                    __syncwarp();
-                    ++u;
-                }
-            if (ptx::elect_one()) ptx::umma_commit(e_empty);
-            __syncwarp();
-        }
-    } else if (warp >= 4) {
-        // ===================================================================== epilogue: H -> FP16 planes [j][a][y]
-        constexpr int kCols = NX / 2;                    // columns of this warp's half
-        const int lg = warp & 3, ch = (warp - 4) >> 2;
-        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * kCols);
-        const size_t plane = (size_t)P.nz * P.NPXP * P.NY;
-        uint32_t u = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-            const int ta = item % P.nta, s = item / P.nta;
-            const int a0 = ta * NX + ch * kCols;
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                    const int j = z0 + n / P.ng, g = n % P.ng;
-                    const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
-                    ptx::mbar_wait(t_full + buf, upar);
-                    ptx::tc_fence_after();
-                    const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
-                    SCATMAN_ASSERT(j >= 0 && j < P.nz && a0 + kCols <= P.NPXP && g * kM + kM <= P.NY);
-                    __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
-#pragma unroll 1
-                    for (int c0 = 0; c0 < kCols; c0 += 8) {
-                        uint32_t gre[8], gim[8];
-                        ptx::tmem_ld8(t_re + c0, gre);
-                        ptx::tmem_ld8(t_im + c0, gim);
-                        ptx::tmem_ld_wait();
-                        if (c0 + 8 >= kCols) {
-                            ptx::tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) ptx::mbar_arrive(t_empty + buf);
-                        }
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            __half h[4];
-                            split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
-                            __half *d = dst + (size_t)(c0 + i) * P.NY;
-#pragma unroll
-                            for (int pl = 0; pl < 4; ++pl) d[pl * plane] = h[pl];
-                        }
-                    }
-                    ++u;
-                }
-        }
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    if (warp == 2) {
-        ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
-    }
-}
-
-// ---- stage X on CTA pairs ------------------------------------------------------------------------------------------
-// tcgen05 cta_group::2, UMMA 256 x 2NX x 16: the two CTAs of a pair take two consecutive live row tiles (each streams its own
-// rho~ tile, 128 rows = its half of M) against the same 2 NX grid columns, of whose Ex tile each CTA keeps NX rows resident.
-// Per SM an instruction then fetches 4 KB of A + 2 KB of B for 64 tensor cycles (N = 128) instead of 6 KB for 32 (N = 64 from
-// one CTA, shared-memory bound at 48.7 cycles).  Stages hold two planes (Re hi + lo, then Im hi + lo: 24 MMAs per barrier round
-// trip).  Each CTA converts and stores the H rows of its own tile; an odd last tile is run twice (the peer repeats the
-// leader's tile and discards it).  Leader-side barriers as in tensor_kernel.cu.
-template <int NX>
-__global__ void __launch_bounds__(kThreadsTc, 1)
-sep_tc_x2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepXParams P) {
-    constexpr int kN = 2 * NX;                    // accumulator columns
-    constexpr int kSmemE = 131072;                // resident Ex planes of this CTA's NX columns: [4][nkx][NX rows x 128 bytes]
-    constexpr int kStages = 3;                    // ring of two-plane 64-x blocks of this CTA's rho~ row tile (32 KB each)
-    constexpr int kStage = 2 * kSlotA;
-    constexpr int kBlkE = NX * kKB * 2;
-    constexpr int kNB = 2;                        // accumulator buffers (D_re, D_im of up to 128 columns each)
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *sE = smem;
-    uint8_t *sR = smem + kSmemE;
-    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kStage);
-    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
-    uint64_t *r_full = bars + 2, *r_empty = r_full + kStages;
-    uint64_t *t_full = r_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
-    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = ptx::cluster_ctarank();
-    const bool leader = rank == 0;
-    const int cluster_id = blockIdx.x / 2, nclusters = gridDim.x / 2;
-    const int nitems = P.nta * P.nsx;             // nta = tiles of 2 NX columns
-
-    if (warp == 0 && lane == 0) {
-        ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
-    }
-    if (warp == 1 && lane == 0) {
-        ptx::mbar_init(e_full, 1);
-        ptx::mbar_init(e_empty, 2);
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(r_full + i, 1);
-            ptx::mbar_init(r_empty + i, 2);
-        }
-        for (int i = 0; i < kNB; ++i) {
-            ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 16);
-            ptx::mbar_init(first_done + i, 1);
-        }
-        ptx::fence_barrier_init();
-        ptx::fence_proxy_async();
-    }
-    if (warp == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::cluster_sync_all();
-    ptx::tc_fence_after();
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
-
-    auto zrange = [&](int s, int &z0, int &z1) {
-        z0 = __ldg(P.zb + s);
-        z1 = __ldg(P.zb + s + 1);
     };
-    // the next pair of live units: n0 for the leader, n1 for the peer (n1 = n0 and dup = true when only one is left)
-    auto next_pair = [&](LiveUnits &un, int &n0, int &n1, bool &dup) {
-        uint32_t f;
-        if (!un.next(n0, f)) return false;
-        dup = !un.next(n1, f);
-        if (dup) n1 = n0;
-        return true;
+    __device__ static void a_coords(const Params &P, const Item &, int unit, int kb, int (&c)[3]) {
+        c[0] = kb * kKB;
+        c[1] = (unit / P.ng) * P.NY + (unit % P.ng) * kM;
+        c[2] = 0;
+    }
+    struct Epilogue {
+        __half *dst;
+        size_t plane;
+        __device__ void begin(const Params &P, const Item &, const tcg::EpiThread &) { plane = (size_t)P.nz * P.NPXP * P.NY; }
+        __device__ void unit_begin(const Params &P, const Item &it, const tcg::EpiThread &et, int unit) {
+            const int j = unit / P.ng, g = unit % P.ng;
+            SCATMAN_ASSERT(j >= 0 && j < P.nz && it.ta * 2 * NX + et.col0 + NX <= P.NPXP && g * kM + kM <= P.NY);
+            dst = P.Hp + ((size_t)j * P.NPXP + it.ta * 2 * NX + et.col0) * P.NY + g * kM + et.lane_row;
+        }
+        __device__ __forceinline__ void columns(const Params &P, const Item &, const tcg::EpiThread &, int, int c0,
+                                                const uint32_t (&gre)[8], const uint32_t (&gim)[8]) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                __half h[4];
+                split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
+                __half *d = dst + (size_t)(c0 + i) * P.NY;
+#pragma unroll
+                for (int pl = 0; pl < 4; ++pl) d[pl * plane] = h[pl];
+            }
+        }
+        __device__ void end(const Params &, const Item &, const tcg::EpiThread &) {}
     };
-
-    if (warp == 0) {
-        // ===================================================================== TMA producer (both CTAs)
-        int slot = 0;
-        uint32_t phase = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            const int ta = item % P.nta, s = item / P.nta;
-            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
-            if (ptx::elect_one()) {
-                if (leader) ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(2 * 4 * P.nkx * kBlkE));
-                for (int pl = 0; pl < 4; ++pl)
-                    for (int kx = 0; kx < P.nkx; ++kx)
-                        ptx::tma_load_3d_2sm(sE + (pl * P.nkx + kx) * kBlkE, &tmB, e_full, kx * kKB, ta * kN + (int)rank * NX, pl);
-            }
-            __syncwarp();
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n0, n1;
-            bool dup;
-            while (next_pair(un, n0, n1, dup)) {
-                const int n = leader ? n0 : n1;
-                const int j = z0 + n / P.ng, g = n % P.ng;
-                for (int kx = 0; kx < P.nkx; ++kx)
-                    for (int ph = 0; ph < 2; ++ph) {   // Re planes, Im planes
-                        ptx::mbar_wait(r_empty + slot, phase ^ 1);
-                        if (ptx::elect_one()) {
-                            if (leader) ptx::mbar_arrive_expect_tx(r_full + slot, (uint32_t)(2 * kStage));
-                            ptx::tma_load_3d_2sm(sR + slot * kStage, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, 2 * ph);
-                            ptx::tma_load_3d_2sm(sR + slot * kStage + kSlotA, &tmA, r_full + slot, kx * kKB, j * P.NY + g * kM, 2 * ph + 1);
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-            }
-        }
-    } else if ((warp == 1 || warp == 3) && leader) {
-        // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
-        const uint64_t descR0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sR));
-        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
-        constexpr uint64_t kR = kSlotA >> 4, kSt = kStage >> 4, kE = kBlkE >> 4;
-        const int iw = warp >> 1;
-        int slot = 0;
-        uint32_t phase = 0, u = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            const int s = item / P.nta;
-            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
-            ptx::tc_fence_after();
-            const uint64_t kEpl = (uint64_t)P.nkx * kE;
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n0, n1;
-            bool dup;
-            while (next_pair(un, n0, n1, dup)) {
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                ptx::mbar_wait(t_empty + buf, upar ^ 1);
-                ptx::tc_fence_after();
-                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                for (int kx = 0; kx < P.nkx; ++kx)
-                    for (int ph = 0; ph < 2; ++ph) {
-                        if (iw == 1 && kx == 0 && ph == 0) {   // D must have been initialised by issuer 0
-                            ptx::mbar_wait(first_done + buf, upar);
-                            ptx::tc_fence_after();
-                        }
-                        ptx::mbar_wait(r_full + slot, phase);
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-#pragma unroll
-                            for (int kk = 0; kk < 2; ++kk) {
-                                const int ks = 2 * kk + iw;
-                                const uint64_t a_hi = descR0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2), a_lo = a_hi + kR;
-                                const uint64_t e_reh = descE0 + (uint64_t)kx * kE + (uint64_t)(ks * 2);
-                                const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
-                                const uint32_t acc0 = (kx == 0 && ph == 0 && ks == 0) ? 0u : 1u;
-                                // (Ar + i Ai)(Er + i Ei), A = the rho~ planes of this stage, three split products AhEh + AlEh + AhEl
-                                if (ph == 0) {   // Re hi, Re lo
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_reh, idesc_pos, acc0);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_imh, idesc_pos, acc0);
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_rel, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_iml, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_lo, e_reh, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_lo, e_imh, idesc_pos, 1u);
-                                } else {         // Im hi, Im lo
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_imh, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_reh, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_iml, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_rel, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_lo, e_imh, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_lo, e_reh, idesc_pos, 1u);
-                                }
-                                if (iw == 0 && kk == 0 && kx == 0 && ph == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
-                            }
-                            ptx::umma_commit_2sm(r_empty + slot, (uint16_t)0x3);
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-                if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
-                __syncwarp();
-                ++u;
-            }
-            if (ptx::elect_one()) ptx::umma_commit_2sm(e_empty, (uint16_t)0x3);
-            __syncwarp();
-        }
-    } else if (warp >= 4) {
-        // ===================================================================== epilogue: H rows of this CTA's tile -> FP16 planes
-        const int lg = warp & 3, ch = (warp - 4) >> 2;   // TMEM lane group; column half: [ch NX, +NX) of the 2 NX columns
-        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * NX);
-        const size_t plane = (size_t)P.nz * P.NPXP * P.NY;
-        uint32_t u = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters) {
-            const int ta = item % P.nta, s = item / P.nta;
-            const int a0 = ta * kN + ch * NX;
-            int z0, z1;
-            zrange(s, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, P.ng, 0, lane);
-            int n0, n1;
-            bool dup;
-            while (next_pair(un, n0, n1, dup)) {
-                const int n = leader ? n0 : n1;
-                const int j = z0 + n / P.ng, g = n % P.ng;
-                const bool store = leader || !dup;
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                ptx::mbar_wait(t_full + buf, upar);
-                ptx::tc_fence_after();
-                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
-                SCATMAN_ASSERT(j >= 0 && j < P.nz && a0 + NX <= P.NPXP && g * kM + kM <= P.NY);
-                __half *dst = P.Hp + ((size_t)j * P.NPXP + a0) * P.NY + g * kM + lg * 32 + lane;
-#pragma unroll 1
-                for (int c0 = 0; c0 < NX; c0 += 8) {
-                    uint32_t gre[8], gim[8];
-                    ptx::tmem_ld8(t_re + c0, gre);
-                    ptx::tmem_ld8(t_im + c0, gim);
-                    ptx::tmem_ld_wait();
-                    if (c0 + 8 >= NX) {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                    }
-                    if (store) {
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            __half h[4];
-                            split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
-                            __half *d = dst + (size_t)(c0 + i) * P.NY;
-#pragma unroll
-                            for (int pl = 0; pl < 4; ++pl) d[pl * plane] = h[pl];
-                        }
-                    }
-                }
-                ++u;
-            }
-        }
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::cluster_sync_all();
-    if (warp == 2) {
-        ptx::tc_fence_after();
-        ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
-    }
-}
+};
 
 // ------------------------------------------------------------------------------------------------ stage YZ
 struct SepYzParams {
-    int nz, nb, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nz: slices per item, nb: items of the chunk, nkb = NY / 64
+    int nk;                       // NY / 64 (K blocks of the transposed form)
+    int nz, nb, npx, npy, NY, NPXP, ng, nzs, ntb, nta, nkb;   // nz: slices per item, nb: items of the chunk, nkb = NY / 64; ntb / nta: 128-row b / a tiles
+    int ntap, ntbn;               // transposed form: pairs of a tiles, tiles of 2 NB grid rows
     double k, dz;
     const double *qx, *qy;
     const unsigned char *flags;   // [nz][nkb]
-    const int *zb;                // [nb][ng][nzs + 1] balanced z split bounds (global slice indices) per item and 128-y group
-    float2 *partial;              // [nb][ng * nzs][npy][npx]
+    const int *zb;                // [nb][nzs + 1] balanced z split bounds (global slice indices) per item
+    float2 *partial;              // [nb][nzs][npy][npx]
 };
-
-struct YzItem {
-    int tb, ta, g, s, b;
-};
-__device__ __forceinline__ YzItem yz_decode(int item, const SepYzParams &P) {
-    YzItem it;
-    it.tb = item % P.ntb;   // b tiles fastest: concurrent CTAs stream the same H tiles
-    item /= P.ntb;
-    it.ta = item % P.nta;
-    item /= P.nta;
-    it.g = item % P.ng;
-    item /= P.ng;
-    it.s = item % P.nzs;
-    it.b = item / P.nzs;
-    return it;
-}
-
-// items of the CTA-pair variant: a pair index replaces the b tile, this CTA's tile is NCTA tp + rank
-template <int NCTA>
-__device__ __forceinline__ YzItem yz_decode_n(int item, const SepYzParams &P, int rank) {
-    YzItem it;
-    const int ntp = P.ntb / NCTA;
-    it.tb = (item % ntp) * NCTA + rank;
-    item /= ntp;
-    it.ta = item % P.nta;
-    item /= P.nta;
-    it.g = item % P.ng;
-    item /= P.ng;
-    it.s = item % P.nzs;
-    it.b = item / P.nzs;
-    return it;
-}
-
-__global__ void __launch_bounds__(kThreadsTc, 1)
-sep_tc_yz_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
-    constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
-    constexpr int kStageB = 4 * kNyz * kKB * 2;       // 32768: four planes of one 64-y block of an H tile
-    constexpr int kStages = 3;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *sA = smem;
-    uint8_t *sB = smem + kSmemA;
-    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kStageB);
-    uint64_t *a_full = bars + 0, *a_empty = bars + 1;
-    uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
-    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNBuf, *first_done = t_empty + kNBuf;
-    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNBuf);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nitems = P.ntb * P.nta * P.ng * P.nzs * P.nb;
-
-    if (warp == 0 && lane == 0) {
-        ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
-    }
-    if (warp == 1 && lane == 0) {
-        ptx::mbar_init(a_full, 1);
-        ptx::mbar_init(a_empty, 2);          // both MMA issuers
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(b_full + i, 1);
-            ptx::mbar_init(b_empty + i, 2);
-        }
-        for (int i = 0; i < kNBuf; ++i) {
-            ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 8);
-            ptx::mbar_init(first_done + i, 1);
-        }
-        ptx::fence_barrier_init();
-        ptx::fence_proxy_async();
-    }
-    if (warp == 2) ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::tc_fence_after();
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
-
-    auto zrange = [&](const YzItem &it, int &z0, int &z1) {   // global slice indices
-        const int *zb = P.zb + (size_t)(it.b * P.ng + it.g) * (P.nzs + 1) + it.s;
-        z0 = __ldg(zb);
-        z1 = __ldg(zb + 1);
-    };
-
-    if (warp == 0) {
-        // ===================================================================== TMA producer
-        int slot = 0;
-        uint32_t phase = 0;
-        int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const YzItem it = yz_decode(item, P);
-            ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
-            if (ptx::elect_one()) {
-                ptx::mbar_arrive_expect_tx(a_full, (uint32_t)kSmemA);
-                for (int pl = 0; pl < 4; ++pl)
-                    for (int kb = 0; kb < 2; ++kb)
-                        ptx::tma_load_3d(sA + (pl * 2 + kb) * kSlotA, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
-            }
-            __syncwarp();
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const int j = z0 + n;
-                for (int kb = 0; kb < 2; ++kb) {
-                    if (((f >> kb) & 1u) == 0u) continue;
-                    ptx::mbar_wait(b_empty + slot, phase ^ 1);
-                    if (ptx::elect_one()) {
-                        ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)kStageB);
-                        for (int pl = 0; pl < 4; ++pl)
-                            ptx::tma_load_3d(sB + slot * kStageB + pl * (kStageB / 4), &tmB, b_full + slot,
-                                             (it.g * 2 + kb) * kKB, j * P.NPXP + it.ta * kNyz, pl);
-                    }
-                    __syncwarp();
-                    if (++slot == kStages) { slot = 0; phase ^= 1; }
-                }
-            }
-        }
-    } else if (warp == 1 || warp == 3) {
-        // ===================================================================== MMA issuers (k-step ks belongs to issuer ks % 2)
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM, kNyz, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM, kNyz, true);
-        const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
-        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
-        constexpr uint64_t kA = kSlotA >> 4, kBst = kStageB >> 4, kBpl = (kStageB / 4) >> 4;
-        const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
-        int slot = 0;
-        uint32_t phase = 0, u = 0;
-        int it_local = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it_local) {
-            const YzItem it = yz_decode(item, P);
-            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
-            ptx::tc_fence_after();
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
-                ptx::mbar_wait(t_empty + buf, upar ^ 1);
-                ptx::tc_fence_after();
-                const uint32_t d_re = tmem_base + buf * 128, d_im = d_re + 64;
-                bool first = true;
-                for (int kb = 0; kb < 2; ++kb) {
-                    if (((f >> kb) & 1u) == 0u) continue;
-                    if (first && iw == 1) {   // D must have been initialised by issuer 0's first k-step
-                        ptx::mbar_wait(first_done + buf, upar);
-                        ptx::tc_fence_after();
-                    }
-                    ptx::mbar_wait(b_full + slot, phase);
-                    ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-#pragma unroll
-                        for (int kk = 0; kk < 2; ++kk) {
-                            const int ks = 2 * kk + iw;
-                            const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
-                            const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
-                            const uint64_t b_reh = descB0 + (uint64_t)slot * kBst + (uint64_t)(ks * 2);
-                            const uint64_t b_rel = b_reh + kBpl, b_imh = b_rel + kBpl, b_iml = b_imh + kBpl;
-                            const uint32_t acc0 = (first && ks == 0) ? 0u : 1u;
-                            ptx::umma_f16(d_re, a_reh, b_reh, idesc_pos, acc0);
-                            ptx::umma_f16(d_im, a_imh, b_reh, idesc_pos, acc0);
-                            ptx::umma_f16(d_re, a_rel, b_reh, idesc_pos, 1u);
-                            ptx::umma_f16(d_im, a_iml, b_reh, idesc_pos, 1u);
-                            ptx::umma_f16(d_re, a_reh, b_rel, idesc_pos, 1u);
-                            ptx::umma_f16(d_im, a_imh, b_rel, idesc_pos, 1u);
-                            ptx::umma_f16(d_re, a_imh, b_imh, idesc_neg, 1u);
-                            ptx::umma_f16(d_im, a_reh, b_imh, idesc_pos, 1u);
-                            ptx::umma_f16(d_re, a_iml, b_imh, idesc_neg, 1u);
-                            ptx::umma_f16(d_im, a_rel, b_imh, idesc_pos, 1u);
-                            ptx::umma_f16(d_re, a_imh, b_iml, idesc_neg, 1u);
-                            ptx::umma_f16(d_im, a_reh, b_iml, idesc_pos, 1u);
-                            if (first && iw == 0 && kk == 0) ptx::umma_commit(first_done + buf);
-                        }
-                        ptx::umma_commit(b_empty + slot);
-                    }
-                    __syncwarp();
-                    first = false;
-                    if (++slot == kStages) { slot = 0; phase ^= 1; }
-                }
-                if (ptx::elect_one()) ptx::umma_commit(t_full + buf);
-                __syncwarp();
-                ++u;
-            }
-            if (ptx::elect_one()) ptx::umma_commit(a_empty);
-            __syncwarp();
-        }
-    } else if (warp >= 4) {
-        // ===================================================================== epilogue: Blocks 7-8
-        const int lg = warp & 3, ch = (warp - 4) >> 2;   // TMEM lane group, column half
-        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 32);
-        uint32_t u = 0;
-        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-            const YzItem it = yz_decode(item, P);
-            const int b = it.tb * kM + lg * 32 + lane;
-            const int a0 = it.ta * kNyz + ch * 32;
-            const double qyb = b < P.npy ? P.qy[b] : 0.0;
-            uint32_t dph[32];
-#pragma unroll
-            for (int c = 0; c < 32; ++c) {
-                const int a = a0 + c;
-                double t = 0.0;
-                if (a < P.npx && b < P.npy) {
-                    const double qxa = P.qx[a];
-                    const double qxy2 = qxa * qxa + qyb * qyb;
-                    const double kz2 = P.k * P.k - qxy2;
-                    // qz = -(k - sqrt(k^2 - qxy^2)) = -qxy^2 / (k + sqrt(k^2 - qxy^2)): no cancellation near forward
-                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
-                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
-                    t -= rint(t);
-                }
-                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
-            }
-            float2 tot[32];
-#pragma unroll
-            for (int c = 0; c < 32; ++c) tot[c] = make_float2(0.f, 0.f);
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const int j = z0 + n - it.b * P.nz;   // slice within its item
-                const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
-                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
-                ptx::mbar_wait(t_full + buf, upar);
-                ptx::tc_fence_after();
-                const uint32_t t_re = t_lane + buf * 128, t_im = t_re + 64;
-                uint32_t gre[2][8], gim[2][8];
-                ptx::tmem_ld8(t_re, gre[0]);
-                ptx::tmem_ld8(t_im, gim[0]);
-                ptx::tmem_ld_wait();
-#pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4) {
-                    const int cur = q4 & 1, nxt = cur ^ 1;
-                    if (q4 < 3) {
-                        ptx::tmem_ld8(t_re + (q4 + 1) * 8, gre[nxt]);
-                        ptx::tmem_ld8(t_im + (q4 + 1) * 8, gim[nxt]);
-                    } else {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(t_empty + buf);   // every column of this warp has landed
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int c = q4 * 8 + i;
-                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
-                        float sn, cs;
-                        __sincosf(ang, &sn, &cs);
-                        const float gr = __uint_as_float(gre[cur][i]), gi = __uint_as_float(gim[cur][i]);
-                        tot[c].x = fmaf(cs, gr, tot[c].x);
-                        tot[c].x = fmaf(-sn, gi, tot[c].x);
-                        tot[c].y = fmaf(cs, gi, tot[c].y);
-                        tot[c].y = fmaf(sn, gr, tot[c].y);
-                    }
-                    if (q4 < 3) ptx::tmem_ld_wait();
-                }
-                ++u;
-            }
-            if (b < P.npy) {
-                float2 *dst = P.partial + (((size_t)it.b * P.ng * P.nzs + it.g * P.nzs + it.s) * P.npy + b) * P.npx;
-#pragma unroll
-                for (int c = 0; c < 32; ++c)
-                    if (a0 + c < P.npx) dst[a0 + c] = tot[c];
-            }
-        }
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    if (warp == 2) {
-        ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemColsTc);
-    }
-}
-
-// ---- stage YZ with 128-column accumulators ------------------------------------------------------------------------
-// Same work as sep_tc_yz_kernel with UMMA 128 x 128 x 16: at N = 128 the instruction's 64 tensor cycles cover its
-// shared-memory operand fetch (8 KB), at N = 64 they do not (48.7 cycles for 32 of work).  H tiles of 128 columns stream
-// plane by plane through a ring of 6 x 16 KB (as the rho~ tiles of stage X); two accumulator buffers of D_re, D_im x 128
-// columns.  An epilogue thread now carries 64 columns: 128 running totals + 64 phase fractions, more than the 168 registers
-// a 384-thread CTA gives each thread, so the register file is re-split with setmaxnreg: the producer / issuer warpgroup
-// drops to 48 registers per thread, the two epilogue warpgroups rise to 224: 128 x 48 + 256 x 224 = 63488 <= the 384 x 168 =
-// 64512 registers the CTA owns (an increase can only take what the CTA's own warps released, or it waits forever).
-__device__ __forceinline__ void setmaxnreg_inc_224() { asm volatile("setmaxnreg.inc.sync.aligned.u32 224;"); }
-__device__ __forceinline__ void setmaxnreg_dec_48() { asm volatile("setmaxnreg.dec.sync.aligned.u32 48;"); }
-
-// NCTA = 2: a CTA pair per work item (tcgen05 cta_group::2, UMMA 256 x 128 x 16): each CTA owns one b tile (its Ey tile, its
-// accumulators, its epilogue) and HALF of every H tile (64 of the 128 a rows), so an instruction fetches 4 KB of A + 2 KB of B
-// per SM for its 64 tensor cycles -- at 128 B/clk that leaves the shared-memory port slack, where a single CTA (8 KB per 64
-// cycles) has none and measured 54 % tensor-pipe activity.  The leader (rank 0) issues every MMA; full barriers live in the
-// leader, empty barriers are signalled in both CTAs (the protocol of tensor_kernel.cu).
-template <int NCTA>
-__global__ void __launch_bounds__(kThreadsTc, 1)
-sep_tc_yz128_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
-    constexpr int kN = 128;
-    constexpr int kSmemA = 4 * 2 * kSlotA;            // 131072: resident Ey planes of one b tile, one 128-y group
-    constexpr int kSlotB = kSlotA / NCTA;             // this CTA's part of a single-plane 64-y block of an H tile (kN / NCTA rows)
-    // A stage = G planes of one 64-y block.  A pair's halves are small enough for all four planes (48 MMAs per barrier round
-    // trip); a single CTA streams plane by plane (8 or 4 MMAs per stage: the issue overhead shows).
-    constexpr int kG = NCTA == 2 ? 4 : 1;
-    constexpr int kStageB = kG * kSlotB;              // 32 KB (pair) / 16 KB (single)
-    constexpr int kStages = NCTA == 2 ? 3 : 6;
-    constexpr int kNB = 2;                            // accumulator buffers (256 columns each)
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *sA = smem;
-    uint8_t *sB = smem + kSmemA;
-    uint64_t *bars = (uint64_t *)(smem + kSmemA + kStages * kStageB);
-    uint64_t *a_full = bars + 0, *a_empty = bars + 1;
-    uint64_t *b_full = bars + 2, *b_empty = b_full + kStages;
-    uint64_t *t_full = b_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
-    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = NCTA == 2 ? ptx::cluster_ctarank() : 0u;
-    const bool leader = rank == 0;
-    const int cluster_id = blockIdx.x / NCTA, nclusters = gridDim.x / NCTA;
-    const int nitems = (P.ntb / NCTA) * P.nta * P.ng * P.nzs * P.nb;   // an item covers NCTA b tiles: tb = NCTA tp + rank
-
-    if (warp == 0 && lane == 0) {
-        ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
-    }
-    if (warp == 1 && lane == 0) {
-        ptx::mbar_init(a_full, 1);
-        ptx::mbar_init(a_empty, 2);
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(b_full + i, 1);
-            ptx::mbar_init(b_empty + i, 2);
-        }
-        for (int i = 0; i < kNB; ++i) {
-            ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 8 * NCTA);
-            ptx::mbar_init(first_done + i, 1);
-        }
-        ptx::fence_barrier_init();
-        ptx::fence_proxy_async();
-    }
-    if (warp == 2) {
-        if (NCTA == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
-        else ptx::tmem_alloc(tmem_ptr, kTmemColsTc);
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    if (NCTA == 2) ptx::cluster_sync_all();   // peer barriers are initialised before anyone signals them
-    ptx::tc_fence_after();
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
-
-    auto zrange = [&](const YzItem &it, int &z0, int &z1) {
-        const int *zb = P.zb + (size_t)(it.b * P.ng + it.g) * (P.nzs + 1) + it.s;
-        z0 = __ldg(zb);
-        z1 = __ldg(zb + 1);
-    };
-
-    if (warp < 4) {
-      setmaxnreg_dec_48();
-      if (warp == 0) {
-        // ===================================================================== TMA producer
-        int slot = 0;
-        uint32_t phase = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
-            ptx::mbar_wait(a_empty, (uint32_t)((it_local & 1) ^ 1));
-            if (ptx::elect_one()) {
-                if (leader) ptx::mbar_arrive_expect_tx(a_full, (uint32_t)(NCTA * kSmemA));
-                for (int pl = 0; pl < 4; ++pl)
-                    for (int kb = 0; kb < 2; ++kb) {
-                        void *dst = sA + (pl * 2 + kb) * kSlotA;
-                        if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
-                        else ptx::tma_load_3d(dst, &tmA, a_full, (it.g * 2 + kb) * kKB, it.tb * kM, pl);
-                    }
-            }
-            __syncwarp();
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const int j = z0 + n;
-                for (int kb = 0; kb < 2; ++kb) {
-                    if (((f >> kb) & 1u) == 0u) continue;
-                    for (int pg = 0; pg < 4 / kG; ++pg) {
-                        ptx::mbar_wait(b_empty + slot, phase ^ 1);
-                        if (ptx::elect_one()) {
-                            if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, (uint32_t)(NCTA * kStageB));   // both halves land on the leader's barrier
-                            const int row = j * P.NPXP + it.ta * kN + (int)rank * (kN / NCTA);
-#pragma unroll
-                            for (int q = 0; q < kG; ++q) {
-                                void *dst = sB + slot * kStageB + q * kSlotB;
-                                if (NCTA == 2) ptx::tma_load_3d_2sm(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
-                                else ptx::tma_load_3d(dst, &tmB, b_full + slot, (it.g * 2 + kb) * kKB, row, pg * kG + q);
-                            }
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-                }
-            }
-        }
-      } else if ((warp == 1 || warp == 3) && leader) {
-        // ===================================================================== MMA issuers (k-step ks belongs to issuer ks % 2)
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(kM * NCTA, kN, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(kM * NCTA, kN, true);
-        auto mma = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
-            if (NCTA == 2) ptx::umma_f16_2sm(d, a, b, idesc, acc);
-            else ptx::umma_f16(d, a, b, idesc, acc);
-        };
-        auto commit = [](uint64_t *bar) {         // in every CTA of the pair
-            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x3);
-            else ptx::umma_commit(bar);
-        };
-        auto commit_local = [](uint64_t *bar) {   // this (leader) CTA's barrier only
-            if (NCTA == 2) ptx::umma_commit_2sm(bar, (uint16_t)0x1);
-            else ptx::umma_commit(bar);
-        };
-        const uint64_t descA0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sA));
-        const uint64_t descB0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sB));
-        constexpr uint64_t kA = kSlotA >> 4, kB = kSlotB >> 4;
-        const int iw = warp >> 1;
-        int slot = 0;
-        uint32_t phase = 0, u = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
-            ptx::mbar_wait(a_full, (uint32_t)(it_local & 1));
-            ptx::tc_fence_after();
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                ptx::mbar_wait(t_empty + buf, upar ^ 1);
-                ptx::tc_fence_after();
-                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                bool first = true;
-                for (int kb = 0; kb < 2; ++kb) {
-                    if (((f >> kb) & 1u) == 0u) continue;
-                    for (int pg = 0; pg < 4 / kG; ++pg) {
-                        if (first && pg == 0 && iw == 1) {   // D must have been initialised by issuer 0's first k-step
-                            ptx::mbar_wait(first_done + buf, upar);
-                            ptx::tc_fence_after();
-                        }
-                        ptx::mbar_wait(b_full + slot, phase);
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-#pragma unroll
-                            for (int kk = 0; kk < 2; ++kk) {
-                                const int ks = 2 * kk + iw;
-                                const uint64_t a_reh = descA0 + (uint64_t)kb * kA + (uint64_t)(ks * 2);
-                                const uint64_t a_rel = a_reh + 2 * kA, a_imh = a_reh + 4 * kA, a_iml = a_reh + 6 * kA;
-#pragma unroll
-                                for (int q = 0; q < kG; ++q) {
-                                    const int pl = pg * kG + q;
-                                    const uint64_t b = descB0 + (uint64_t)slot * (kStageB >> 4) + (uint64_t)q * kB + (uint64_t)(ks * 2);
-                                    const uint32_t acc0 = (first && pl == 0 && ks == 0) ? 0u : 1u;
-                                    // (Ar + i Ai)(Br + i Bi), B = H plane pl of this stage, three split products AhBh + AlBh + AhBl
-                                    if (pl == 0) {          // B Re_hi
-                                        mma(d_re, a_reh, b, idesc_pos, acc0);
-                                        mma(d_im, a_imh, b, idesc_pos, acc0);
-                                        mma(d_re, a_rel, b, idesc_pos, 1u);
-                                        mma(d_im, a_iml, b, idesc_pos, 1u);
-                                    } else if (pl == 1) {   // B Re_lo
-                                        mma(d_re, a_reh, b, idesc_pos, 1u);
-                                        mma(d_im, a_imh, b, idesc_pos, 1u);
-                                    } else if (pl == 2) {   // B Im_hi
-                                        mma(d_re, a_imh, b, idesc_neg, 1u);
-                                        mma(d_im, a_reh, b, idesc_pos, 1u);
-                                        mma(d_re, a_iml, b, idesc_neg, 1u);
-                                        mma(d_im, a_rel, b, idesc_pos, 1u);
-                                    } else {                // B Im_lo
-                                        mma(d_re, a_imh, b, idesc_neg, 1u);
-                                        mma(d_im, a_reh, b, idesc_pos, 1u);
-                                    }
-                                }
-                                if (first && pg == 0 && iw == 0 && kk == 0) commit_local(first_done + buf);
-                            }
-                            commit(b_empty + slot);
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-                    first = false;
-                }
-                if (ptx::elect_one()) commit(t_full + buf);
-                __syncwarp();
-                ++u;
-            }
-            if (ptx::elect_one()) commit(a_empty);
-            __syncwarp();
-        }
-      }
-    } else {
-        setmaxnreg_inc_224();
-        // ===================================================================== epilogue: Blocks 7-8, 64 columns per thread
-        const int lg = warp & 3, ch = (warp - 4) >> 2;
-        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 64);
-        uint32_t u = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters) {
-            const YzItem it = yz_decode_n<NCTA>(item, P, (int)rank);
-            const int b = it.tb * kM + lg * 32 + lane;
-            const int a0 = it.ta * kN + ch * 64;
-            const double qyb = b < P.npy ? P.qy[b] : 0.0;
-            uint32_t dph[64];
-#pragma unroll
-            for (int c = 0; c < 64; ++c) {
-                const int a = a0 + c;
-                double t = 0.0;
-                if (a < P.npx && b < P.npy) {
-                    const double qxa = P.qx[a];
-                    const double qxy2 = qxa * qxa + qyb * qyb;
-                    const double kz2 = P.k * P.k - qxy2;
-                    const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
-                    t = qz * P.dz * (0.25 / 3.14159265358979323846);
-                    t -= rint(t);
-                }
-                dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
-            }
-            float2 tot[64];
-#pragma unroll
-            for (int c = 0; c < 64; ++c) tot[c] = make_float2(0.f, 0.f);
-            int z0, z1;
-            zrange(it, z0, z1);
-            LiveUnits un;
-            un.begin(P.flags, P.nkb, z0, z1, 1, it.g, lane);
-            int n;
-            uint32_t f;
-            while (un.next(n, f)) {
-                const int j = z0 + n - it.b * P.nz;
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
-                ptx::mbar_wait(t_full + buf, upar);
-                ptx::tc_fence_after();
-                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
-#pragma unroll
-                for (int q8 = 0; q8 < 8; ++q8) {
-                    uint32_t gre[8], gim[8];
-                    ptx::tmem_ld8(t_re + q8 * 8, gre);
-                    ptx::tmem_ld8(t_im + q8 * 8, gim);
-                    ptx::tmem_ld_wait();
-                    if (q8 == 7) {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) {
-                            if (NCTA == 2) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                            else ptx::mbar_arrive(t_empty + buf);
-                        }
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int c = q8 * 8 + i;
-                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
-                        float sn, cs;
-                        __sincosf(ang, &sn, &cs);
-                        const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
-                        tot[c].x = fmaf(cs, gr, tot[c].x);
-                        tot[c].x = fmaf(-sn, gi, tot[c].x);
-                        tot[c].y = fmaf(cs, gi, tot[c].y);
-                        tot[c].y = fmaf(sn, gr, tot[c].y);
-                    }
-                }
-                ++u;
-            }
-            if (b < P.npy) {
-                float2 *dst = P.partial + (((size_t)it.b * P.ng * P.nzs + it.g * P.nzs + it.s) * P.npy + b) * P.npx;
-#pragma unroll
-                for (int c = 0; c < 64; ++c)
-                    if (a0 + c < P.npx) dst[a0 + c] = tot[c];
-            }
-        }
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    if (NCTA == 2) ptx::cluster_sync_all();   // nobody leaves while the peer may still signal its barriers
-    if (warp == 2) {
-        ptx::tc_fence_after();
-        if (NCTA == 2) ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
-        else ptx::tmem_dealloc(tmem_base, kTmemColsTc);
-    }
-}
 
 // ---- stage YZ with one accumulator per slice: both operands streamed -------------------------------------------------------
 // With the Ey tile resident, a slice needs one accumulator pass PER 128-y group, and the per-element slice phase of the epilogue
@@ -1405,7 +431,7 @@ sep_tc_yzs_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     };
 
     if (warp < 4) {
-      setmaxnreg_dec_48();
+      tcg::setmaxnreg_dec_48();
       if (warp == 0) {
         // ===================================================================== TMA producer (both CTAs)
         int slot = 0;
@@ -1507,7 +533,7 @@ sep_tc_yzs_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
       }
     } else {
-        setmaxnreg_inc_224();
+        tcg::setmaxnreg_inc<224>();
         // ===================================================================== epilogue: Blocks 7-8, 64 columns per thread
         const int lg = warp & 3, ch = (warp - 4) >> 2;
         const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * 64);
@@ -1593,211 +619,68 @@ sep_tc_yzs_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 }
 
 // ---- stage YZ transposed: D^T[a, b] = sum_y H_j[a, y] Ey[b, y], the Ey tile resident for ALL y -----------------------------
-// The roles of sep_tc_x2_kernel: the streamed A operand is each CTA's own H tile (128 grid columns a = the TMEM lanes, two
-// planes per stage), the resident B operand this CTA's NB rows of the Ey tile of 2 NB grid rows b, for every 64-y block
-// (NB nkb 8 KB <= 128 KB: NB = 64 for N_y <= 256, the only instance built; NB = 32 for N_y <= 512 ran UMMA N = 64 and measured
-// slower than the streamed form).  One accumulator per slice like sep_tc_yzs_kernel, but only H streams (2/3 of that kernel's
-// L2 -> SM traffic).  The epilogue thread owns one column a and NB rows b.
-template <int NB>
-__global__ void __launch_bounds__(kThreadsTc, 1)
-sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const SepYzParams P) {
-    constexpr int kN = 2 * NB;
-    constexpr int kSmemE = 131072;                // resident Ey planes of this CTA's NB rows: [4][nkb][NB rows x 128 bytes]
-    constexpr int kStages = 3;
-    constexpr int kStage = 2 * kSlotA;            // two planes of one 64-y block of this CTA's H tile
-    constexpr int kBlkE = NB * kKB * 2;
-    constexpr int kNB = 2;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *sE = smem;
-    uint8_t *sH = smem + kSmemE;
-    uint64_t *bars = (uint64_t *)(smem + kSmemE + kStages * kStage);
-    uint64_t *e_full = bars + 0, *e_empty = bars + 1;
-    uint64_t *h_full = bars + 2, *h_empty = h_full + kStages;
-    uint64_t *t_full = h_empty + kStages, *t_empty = t_full + kNB, *first_done = t_empty + kNB;
-    uint32_t *tmem_ptr = (uint32_t *)(first_done + kNB);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = ptx::cluster_ctarank();
-    const bool leader = rank == 0;
-    const int cluster_id = blockIdx.x / 2, nclusters = gridDim.x / 2;
-    const int ntap = P.NPXP / (2 * kM);           // pairs of a tiles
-    const int ntbn = P.ntb * kM / kN;             // tiles of 2 NB grid rows
-    const int nitems = ntap * ntbn * P.nzs * P.nb;
-
-    if (warp == 0 && lane == 0) {
-        ptx::tma_prefetch_desc(&tmA);
-        ptx::tma_prefetch_desc(&tmB);
-    }
-    if (warp == 1 && lane == 0) {
-        ptx::mbar_init(e_full, 1);
-        ptx::mbar_init(e_empty, 2);
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(h_full + i, 1);
-            ptx::mbar_init(h_empty + i, 2);
-        }
-        for (int i = 0; i < kNB; ++i) {
-            ptx::mbar_init(t_full + i, 2);
-            ptx::mbar_init(t_empty + i, 16);
-            ptx::mbar_init(first_done + i, 1);
-        }
-        ptx::fence_barrier_init();
-        ptx::fence_proxy_async();
-    }
-    if (warp == 2) ptx::tmem_alloc_2sm(tmem_ptr, kTmemColsTc);
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::cluster_sync_all();
-    ptx::tc_fence_after();
-    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
-
-    auto decode = [&](int item, int &ta, int &tbn, int &sp, int &bi) {   // a pairs fastest: neighbours share the Ey tile
-        ta = (item % ntap) * 2 + (int)rank;
-        item /= ntap;
-        tbn = item % ntbn;
-        item /= ntbn;
-        sp = item % P.nzs;
-        bi = item / P.nzs;
+// The same pipeline (tc_cgemm.cuh): the streamed A operand is each CTA's own H tile (128 grid columns a = the TMEM lanes), the
+// resident B operand this CTA's NB rows of the Ey tile of 2 NB grid rows b for every 64-y block (NB nkb 8 KB <= 128 KB: NB = 64 for
+// N_y <= 256, the only instance built; NB = 32 for N_y <= 512 ran UMMA N = 64 and measured slower than the streamed form).  A work
+// item = (pair of a tiles, b tile, z range, batch item); a unit = (live slice, a tile): the pair takes the two a tiles of the
+// same slice (an odd last a tile is run twice and the copy discarded), and 64-y blocks of a slice that hold nothing are never
+// loaded.  One accumulator per slice, so the epilogue -- Blocks 7-8: slice phase, sum over slices -- runs once per slice; its
+// thread owns one column a and NB rows b: 2 NB running totals + NB phase fractions, hence the setmaxnreg re-split (224 registers).
+template <int NB_>
+struct SepYztPolicy {
+    static constexpr int NB = NB_;
+    static constexpr bool kUnrollEpilogue = true;
+    static constexpr int kEpilogueRegs = 224;
+    using Params = SepYzParams;
+    struct Item {
+        int ta0, tbn, sp, bi, z0, z1;
     };
-    auto zrange = [&](int bi, int sp, int &z0, int &z1) {
-        const int *zb = P.zb + (size_t)bi * (P.nzs + 1) + sp;
-        z0 = __ldg(zb);
-        z1 = __ldg(zb + 1);
+    __device__ static int nitems(const Params &P) { return P.ntap * P.ntbn * P.nzs * P.nb; }
+    __device__ static Item item(const Params &P, int index) {   // a pairs fastest: neighbours share the Ey tile
+        Item it;
+        it.ta0 = (index % P.ntap) * 2;
+        index /= P.ntap;
+        it.tbn = index % P.ntbn;
+        index /= P.ntbn;
+        it.sp = index % P.nzs;
+        it.bi = index / P.nzs;
+        const int *zb = P.zb + (size_t)it.bi * (P.nzs + 1) + it.sp;
+        it.z0 = __ldg(zb);
+        it.z1 = __ldg(zb + 1);
+        return it;
+    }
+    __device__ static int b_row0(const Params &, const Item &it) { return it.tbn * 2 * NB; }
+    // unit id = global slice * nta + a tile
+    struct Units {
+        LiveSlices ls;
+        int z0, ta0, nta;
+        __device__ void begin(const Params &P, const Item &it, int lane) {
+            ls.begin(P.flags, P.nkb, it.z0, it.z1, lane);
+            z0 = it.z0; ta0 = it.ta0; nta = P.nta;
+        }
+        __device__ bool next(int &u0, int &u1, bool &dup, uint32_t &kmask) {
+            int n;
+            if (!ls.next(n, kmask)) return false;
+            u0 = (z0 + n) * nta + ta0;
+            dup = ta0 + 1 >= nta;
+            u1 = dup ? u0 : u0 + 1;
+            return true;
+        }
     };
-
-    if (warp < 4) {
-      setmaxnreg_dec_48();
-      if (warp == 0) {
-        // ===================================================================== TMA producer (both CTAs)
-        int slot = 0;
-        uint32_t phase = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            int ta, tbn, sp, bi;
-            decode(item, ta, tbn, sp, bi);
-            ptx::mbar_wait(e_empty, (uint32_t)((it_local & 1) ^ 1));
-            if (ptx::elect_one()) {
-                if (leader) ptx::mbar_arrive_expect_tx(e_full, (uint32_t)(2 * 4 * P.nkb * kBlkE));
-                for (int pl = 0; pl < 4; ++pl)
-                    for (int kb = 0; kb < P.nkb; ++kb)
-                        ptx::tma_load_3d_2sm(sE + (pl * P.nkb + kb) * kBlkE, &tmA, e_full, kb * kKB, tbn * kN + (int)rank * NB, pl);
-            }
-            __syncwarp();
-            int z0, z1;
-            zrange(bi, sp, z0, z1);
-            LiveSlices un;
-            un.begin(P.flags, P.nkb, z0, z1, lane);
-            int n;
-            uint32_t m;
-            while (un.next(n, m)) {
-                const int row = (z0 + n) * P.NPXP + ta * kM;
-                for (int kb = 0; kb < P.nkb; ++kb) {
-                    if (((m >> kb) & 1u) == 0u) continue;
-                    for (int ph = 0; ph < 2; ++ph) {   // Re planes, Im planes
-                        ptx::mbar_wait(h_empty + slot, phase ^ 1);
-                        if (ptx::elect_one()) {
-                            if (leader) ptx::mbar_arrive_expect_tx(h_full + slot, (uint32_t)(2 * kStage));
-                            ptx::tma_load_3d_2sm(sH + slot * kStage, &tmB, h_full + slot, kb * kKB, row, 2 * ph);
-                            ptx::tma_load_3d_2sm(sH + slot * kStage + kSlotA, &tmB, h_full + slot, kb * kKB, row, 2 * ph + 1);
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-                }
-            }
-        }
-      } else if ((warp == 1 || warp == 3) && leader) {
-        // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
-        constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
-        constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
-        const uint64_t descH0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sH));
-        const uint64_t descE0 = ptx::umma_smem_desc_sw128(ptx::smem_u32(sE));
-        constexpr uint64_t kR = kSlotA >> 4, kSt = kStage >> 4, kE = kBlkE >> 4;
-        const int iw = warp >> 1;
-        int slot = 0;
-        uint32_t phase = 0, u = 0;
-        int it_local = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
-            int ta, tbn, sp, bi;
-            decode(item, ta, tbn, sp, bi);
-            ptx::mbar_wait(e_full, (uint32_t)(it_local & 1));
-            ptx::tc_fence_after();
-            const uint64_t kEpl = (uint64_t)P.nkb * kE;   // descriptor distance between Ey planes
-            int z0, z1;
-            zrange(bi, sp, z0, z1);
-            LiveSlices un;
-            un.begin(P.flags, P.nkb, z0, z1, lane);
-            int n;
-            uint32_t m;
-            while (un.next(n, m)) {
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                ptx::mbar_wait(t_empty + buf, upar ^ 1);
-                ptx::tc_fence_after();
-                const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                bool first = true;
-                for (int kb = 0; kb < P.nkb; ++kb) {
-                    if (((m >> kb) & 1u) == 0u) continue;
-                    for (int ph = 0; ph < 2; ++ph) {
-                        if (first && ph == 0 && iw == 1) {   // D must have been initialised by issuer 0
-                            ptx::mbar_wait(first_done + buf, upar);
-                            ptx::tc_fence_after();
-                        }
-                        ptx::mbar_wait(h_full + slot, phase);
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-#pragma unroll
-                            for (int kk = 0; kk < 2; ++kk) {
-                                const int ks = 2 * kk + iw;
-                                const uint64_t a_hi = descH0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2), a_lo = a_hi + kR;
-                                const uint64_t e_reh = descE0 + (uint64_t)kb * kE + (uint64_t)(ks * 2);
-                                const uint64_t e_rel = e_reh + kEpl, e_imh = e_rel + kEpl, e_iml = e_imh + kEpl;
-                                const uint32_t acc0 = (first && ph == 0 && ks == 0) ? 0u : 1u;
-                                // (Hr + i Hi)(Er + i Ei), the H planes of this stage as A, three split products HhEh + HlEh + HhEl
-                                if (ph == 0) {
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_reh, idesc_pos, acc0);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_imh, idesc_pos, acc0);
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_rel, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_iml, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_lo, e_reh, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_lo, e_imh, idesc_pos, 1u);
-                                } else {
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_imh, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_reh, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_hi, e_iml, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_hi, e_rel, idesc_pos, 1u);
-                                    ptx::umma_f16_2sm(d_re, a_lo, e_imh, idesc_neg, 1u);
-                                    ptx::umma_f16_2sm(d_im, a_lo, e_reh, idesc_pos, 1u);
-                                }
-                                if (first && ph == 0 && iw == 0 && kk == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
-                            }
-                            ptx::umma_commit_2sm(h_empty + slot, (uint16_t)0x3);
-                        }
-                        __syncwarp();
-                        if (++slot == kStages) { slot = 0; phase ^= 1; }
-                    }
-                    first = false;
-                }
-                if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
-                __syncwarp();
-                ++u;
-            }
-            if (ptx::elect_one()) ptx::umma_commit_2sm(e_empty, (uint16_t)0x3);
-            __syncwarp();
-        }
-      }
-    } else {
-        setmaxnreg_inc_224();
-        // ===================================================================== epilogue: Blocks 7-8; thread = (column a, NB rows b)
-        const int lg = warp & 3, ch = (warp - 4) >> 2;
-        const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * NB);
-        uint32_t u = 0;
-        for (int item = cluster_id; item < nitems; item += nclusters) {
-            int ta, tbn, sp, bi;
-            decode(item, ta, tbn, sp, bi);
-            const int a = ta * kM + lg * 32 + lane;
-            const int b0 = tbn * kN + ch * NB;
+    __device__ static void a_coords(const Params &P, const Item &, int unit, int kb, int (&c)[3]) {
+        c[0] = kb * kKB;
+        c[1] = (unit / P.nta) * P.NPXP + (unit % P.nta) * kM;
+        c[2] = 0;
+    }
+    struct Epilogue {
+        uint32_t dph[NB], mult;
+        float2 tot[NB];
+        int a, b0;
+        __device__ __forceinline__ void begin(const Params &P, const Item &it, const tcg::EpiThread &et) {
+            const int ta = it.ta0 + ((et.rank != 0 && it.ta0 + 1 < P.nta) ? 1 : 0);
+            a = ta * kM + et.lane_row;
+            b0 = it.tbn * 2 * NB + et.col0;
             const double qxa = a < P.npx ? P.qx[a] : 0.0;
-            uint32_t dph[NB];
 #pragma unroll
             for (int c = 0; c < NB; ++c) {
                 const int b = b0 + c;
@@ -1806,71 +689,46 @@ sep_tc_yzt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     const double qyb = P.qy[b];
                     const double qxy2 = qxa * qxa + qyb * qyb;
                     const double kz2 = P.k * P.k - qxy2;
+                    // qz = -(k - sqrt(k^2 - qxy^2)) = -qxy^2 / (k + sqrt(k^2 - qxy^2)): no cancellation near forward
                     const double qz = kz2 >= 0.0 ? -qxy2 / (P.k + sqrt(kz2)) : 0.0;
                     t = qz * P.dz * (0.25 / 3.14159265358979323846);
                     t -= rint(t);
                 }
                 dph[c] = (uint32_t)(long long)rint(t * 4294967296.0);
+                tot[c] = make_float2(0.f, 0.f);
             }
-            float2 tot[NB];
+        }
+        __device__ __forceinline__ void unit_begin(const Params &P, const Item &it, const tcg::EpiThread &, int unit) {
+            const int j = unit / P.nta - it.bi * P.nz;   // slice within its item
+            SCATMAN_ASSERT(j >= 0 && j < P.nz && it.bi < P.nb && it.sp < P.nzs);
+            mult = (uint32_t)(2 * j - P.nz + 1);
+        }
+        __device__ __forceinline__ void columns(const Params &, const Item &, const tcg::EpiThread &, int, int c0,
+                                                const uint32_t (&gre)[8], const uint32_t (&gim)[8]) {
 #pragma unroll
-            for (int c = 0; c < NB; ++c) tot[c] = make_float2(0.f, 0.f);
-            int z0, z1;
-            zrange(bi, sp, z0, z1);
-            LiveSlices un;
-            un.begin(P.flags, P.nkb, z0, z1, lane);
-            int n;
-            uint32_t m;
-            while (un.next(n, m)) {
-                const int j = z0 + n - bi * P.nz;
-                SCATMAN_ASSERT(j >= 0 && j < P.nz && bi < P.nb && sp < P.nzs);
-                const uint32_t buf = u % kNB, upar = (u / kNB) & 1;
-                const uint32_t mult = (uint32_t)(2 * j - P.nz + 1);
-                ptx::mbar_wait(t_full + buf, upar);
-                ptx::tc_fence_after();
-                const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
-#pragma unroll
-                for (int q8 = 0; q8 < NB / 8; ++q8) {
-                    uint32_t gre[8], gim[8];
-                    ptx::tmem_ld8(t_re + q8 * 8, gre);
-                    ptx::tmem_ld8(t_im + q8 * 8, gim);
-                    ptx::tmem_ld_wait();
-                    if (q8 == NB / 8 - 1) {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int c = q8 * 8 + i;
-                        const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
-                        float sn, cs;
-                        __sincosf(ang, &sn, &cs);
-                        const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
-                        tot[c].x = fmaf(cs, gr, tot[c].x);
-                        tot[c].x = fmaf(-sn, gi, tot[c].x);
-                        tot[c].y = fmaf(cs, gi, tot[c].y);
-                        tot[c].y = fmaf(sn, gr, tot[c].y);
-                    }
-                }
-                ++u;
+            for (int i = 0; i < 8; ++i) {
+                const int c = c0 + i;
+                const float ang = (float)(int)(dph[c] * mult) * 1.4629180792671596e-9f;   // pi / 2^31
+                float sn, cs;
+                __sincosf(ang, &sn, &cs);
+                const float gr = __uint_as_float(gre[i]), gi = __uint_as_float(gim[i]);
+                tot[c].x = fmaf(cs, gr, tot[c].x);
+                tot[c].x = fmaf(-sn, gi, tot[c].x);
+                tot[c].y = fmaf(cs, gi, tot[c].y);
+                tot[c].y = fmaf(sn, gr, tot[c].y);
             }
+        }
+        __device__ __forceinline__ void end(const Params &P, const Item &it, const tcg::EpiThread &et) {
+            if (et.rank != 0 && it.ta0 + 1 >= P.nta) return;   // the peer repeated the leader's tile
             if (a < P.npx) {   // a warp stores 32 consecutive a of one grid row
-                float2 *dst = P.partial + ((size_t)bi * P.nzs + sp) * P.npy * P.npx + a;
+                float2 *dst = P.partial + ((size_t)it.bi * P.nzs + it.sp) * P.npy * P.npx + a;
 #pragma unroll
                 for (int c = 0; c < NB; ++c)
                     if (b0 + c < P.npy) dst[(size_t)(b0 + c) * P.npx] = tot[c];
             }
         }
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::cluster_sync_all();
-    if (warp == 2) {
-        ptx::tc_fence_after();
-        ptx::tmem_dealloc_2sm(tmem_base, kTmemColsTc);
-    }
-}
+    };
+};
 
 // I[b][a] = |ampscale * sum of partials|^2; evanescent grid points (qx^2 + qy^2 > k^2: no scattering direction) give 0
 __global__ void sep_tc_finalize_kernel(const float2 *__restrict__ partial, const double *__restrict__ qx,
@@ -1900,13 +758,22 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     SepTcPlan t;
     t.NY = (p.ny + 127) / 128 * 128;
     t.NXP = (p.nx + kKB - 1) / kKB * kKB;
-    t.nyz = npx > kNyz ? 128 : kNyz;   // stage YZ accumulator width: 128 columns (full-rate UMMA) unless the grid is narrower
-    t.NPXP = (npx + t.nyz - 1) / t.nyz * t.nyz;
-    t.NPYP = (npy + kM - 1) / kM * kM;
+    t.nyz = 128;                                  // stage YZ accumulator width (columns a per tile)
+    t.NPXP = (npx + kM - 1) / kM * kM;            // whole 128-column tiles: stage X's tiles of 2 NX columns and stage YZ's a tiles divide it
     t.ng = t.NY / 128;
     int L = 0;
     while ((1 << L) < p.nx) ++L;
     t.L = L;
+    // Stage YZ, in order of preference:
+    //   transposed (SepYztPolicy<64>)  pairs of a tiles, Ey resident for all y: N_y <= 256
+    //   streamed   (sep_tc_yzs_kernel) pairs of b tiles, both operands streamed: N_y <= 2048 (taller grids use the CUDA-core stages)
+    t.yzt_nb = t.NY / kKB <= 4 ? 64 : 0;
+    t.yz_t = t.yzt_nb != 0;
+    t.yz_stream = true;                           // both forms: one accumulator per slice, z-split bounds and partial sums per item
+    t.yz_ncta = 2;
+    // the streamed form pairs b tiles: an odd count is padded by one all-zero tile of Ey rows
+    t.NPYP = (npy + kM - 1) / kM * kM;
+    if (!t.yz_t && (t.NPYP / kM) % 2 != 0) t.NPYP += kM;
     // items per chunk (stacked along z, one set of launches per chunk): as many as keep the H planes of a chunk under 4 GB
     const size_t h_item = (size_t)8 * p.nz * t.NPXP * t.NY;
     size_t nb = ((size_t)4 << 30) / (h_item ? h_item : 1);
@@ -1914,21 +781,8 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
     if (nb * p.nz > 60000) nb = 60000 / (size_t)p.nz;   // global slice index and TMA row coordinates stay small
     t.nb = nb < 1 ? 1 : (int)nb;
     // z splits: minimise waves x (slices per item + ~3 slice-equivalents of fill: Ey tile load, pipeline ramp, partial store)
-    // stage YZ runs on CTA pairs (UMMA 256 x 128) when it uses 128-column accumulators and the b tiles pair up
-    // stage YZ variants, in order of preference (each needs its tiles to pair up for cta_group::2):
-    //   sep_tc_yzt_kernel   pairs of a tiles, Ey resident for all y (N_y <= 256)
-    //   sep_tc_yzs_kernel   pairs of b tiles, both operands streamed (N_y <= 2048)
-    //   sep_tc_yz128_kernel one CTA, Ey resident per 128-y group, one accumulator per (slice, group): any size
-    //   sep_tc_yz_kernel    the same with 64-column accumulators, for grids of at most 64 columns
-    t.yz_stream = t.nyz == 128 && (t.NPYP / kM) % 2 == 0 && t.NY / kKB <= 32;
-    t.yz_ncta = t.yz_stream ? 2 : 1;
-    // transposed form (sep_tc_yzt_kernel): pairs of a tiles, the Ey tile of 2 NB rows resident for all y
-    t.yzt_nb = t.NY / kKB <= 4 ? 64 : 0;   // (NB = 32 / 16 for taller grids run UMMA N = 64 / 32: measured slower than the streamed form)
-    t.yz_t = t.nyz == 128 && (t.NPXP / kM) % 2 == 0 && t.yzt_nb != 0;
-    if (t.yz_t) { t.yz_stream = true; t.yz_ncta = 2; }   // same bounds / partial layout as the streamed form
-    const int base = t.yz_t ? (t.NPXP / (2 * kM)) * (t.NPYP / (2 * t.yzt_nb)) * t.nb
-                            : (t.NPYP / kM / t.yz_ncta) * (t.NPXP / t.nyz) * (t.yz_stream ? 1 : t.ng) * t.nb;
-    const int workers = num_sms / t.yz_ncta;
+    const int base = t.yz_t ? ((t.NPXP / kM + 1) / 2) * (t.NPYP / (2 * t.yzt_nb)) * t.nb : (t.NPYP / kM / 2) * (t.NPXP / t.nyz) * t.nb;
+    const int workers = num_sms / 2;
     int best = 1;
     double best_cost = 1e300;
     const int max_z = p.nz < 32 ? p.nz : 32;
@@ -1939,32 +793,25 @@ SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms) {
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = z; }
     }
     t.nzs = best;
-    t.nsplit = (t.yz_stream ? 1 : t.ng) * t.nzs;
-    // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for ~4 waves of a-tile items
+    t.nsplit = t.nzs;
+    // stage X: a columns per resident Ex tile (NX * NXP * 8 bytes <= 128 KB), z splits for two balanced items per CTA pair
     t.NX = t.NXP <= 256 ? 64 : t.NXP <= 512 ? 32 : 16;
-    t.x_ncta = t.NPXP % (2 * t.NX) == 0 ? 2 : 1;   // CTA pairs (UMMA 256 x 2NX) when the column tiles pair up
-    const int nta = t.NPXP / (t.NX * t.x_ncta);
-    int nsx = (2 * (num_sms / t.x_ncta) + nta - 1) / nta;   // two balanced items per CTA (pair)
+    t.x_ncta = 2;
+    const int nta = t.NPXP / (2 * t.NX);
+    int nsx = (2 * (num_sms / 2) + nta - 1) / nta;
     t.nsx = nsx < 1 ? 1 : nsx > p.nz * t.nb ? p.nz * t.nb : nsx;
     return t;
 }
 
-constexpr int kSmemYz = 1024 + 4 * 2 * kSlotA + 3 * (4 * kNyz * kKB * 2) + 256;   // every stage YZ variant: 128 KB resident + 96 KB ring
-constexpr int kSmemX = 1024 + 131072 + 6 * kSlotA + 256;                           // every stage X variant
+constexpr int kSmemYzs = 1024 + 2 * (4 * kSlotA + 4 * (kSlotA / 2)) + 256;   // streamed stage YZ: two stages of 96 KB
 
 // Function attributes belong to a device's context: set for the CURRENT device by scatman_create.
 cudaError_t sep_tc_init_device() {
-    const cudaFuncAttribute attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
-    cudaError_t e = cudaFuncSetAttribute(sep_tc_yz_kernel, attr, kSmemYz);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yz128_kernel<1>, attr, kSmemYz);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yzs_kernel, attr, kSmemYz);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_yzt_kernel<64>, attr, kSmemYz);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<64>, attr, kSmemX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<32>, attr, kSmemX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x_kernel<16>, attr, kSmemX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<64>, attr, kSmemX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<32>, attr, kSmemX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sep_tc_x2_kernel<16>, attr, kSmemX);
+    cudaError_t e = cudaFuncSetAttribute(sep_tc_yzs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemYzs);
+    if (e == cudaSuccess) e = tcg::cgemm_init_device<SepYztPolicy<64>>();
+    if (e == cudaSuccess) e = tcg::cgemm_init_device<SepXPolicy<64>>();
+    if (e == cudaSuccess) e = tcg::cgemm_init_device<SepXPolicy<32>>();
+    if (e == cudaSuccess) e = tcg::cgemm_init_device<SepXPolicy<16>>();
     return e;
 }
 
@@ -1977,104 +824,67 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
     return cudaGetLastError();
 }
 
-template <int NCTA>
-static cudaError_t launch_yz128_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepYzParams &P, int nitems, int num_sms,
-                                        int smem, cudaStream_t st) {
-    const int max_clusters = num_sms / NCTA;
-    const int nclusters = nitems < max_clusters ? nitems : max_clusters;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(nclusters * NCTA));
-    cfg.blockDim = dim3(kThreadsTc);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = NCTA;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, sep_tc_yz128_kernel<NCTA>, tmA, tmB, P);
-}
-
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
                              const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err) {
-    constexpr int kSmem = kSmemYz;
-    const int ncta = t.nyz == 128 ? t.yz_ncta : 1;
+    SepYzParams P;
+    P.nk = t.NY / kKB;
+    P.nz = p.nz; P.nb = nb; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
+    P.ntb = t.NPYP / kM; P.nta = t.NPXP / kM; P.nkb = t.NY / kKB;
+    P.ntap = (P.nta + 1) / 2;
+    P.ntbn = t.yz_t ? t.NPYP / (2 * t.yzt_nb) : 0;
+    P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
+    P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
+    const cuuint64_t hrows = (cuuint64_t)p.nz * nb * t.NPXP;
     CUtensorMap tmA, tmB;
     bool ok;
-    {
+    if (t.yz_t) {
+        // streamed operand: the H planes [4][slices NPXP][NY], box = 64 y x a whole 128-column a tile; resident: the Ey planes,
+        // box = this CTA's NB rows of one 64-y block
+        cuuint64_t dimsA[4] = {(cuuint64_t)t.NY, hrows, 1, 4};
+        cuuint64_t stridesA[3] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * hrows * 2, (cuuint64_t)t.NY * hrows * 2};
+        cuuint32_t boxA[4] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1, 1};
+        cuuint64_t dimsB[3] = {(cuuint64_t)t.NY, (cuuint64_t)t.NPYP, 4};
+        cuuint64_t stridesB[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * (cuuint64_t)t.NPYP * 2};
+        cuuint32_t boxB[3] = {(cuuint32_t)kKB, (cuuint32_t)t.yzt_nb, 1};
+        ok = encode_map(&tmA, d_Hp, 4, dimsA, stridesA, boxA, CU_TENSOR_MAP_SWIZZLE_128B) &&
+             encode_map(&tmB, d_Eyp, 3, dimsB, stridesB, boxB, CU_TENSOR_MAP_SWIZZLE_128B);
+        if (!ok) {
+            if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
+            return cudaErrorUnknown;
+        }
+        return tcg::cgemm_launch<SepYztPolicy<64>>(tmA, tmB, P, P.ntap * P.ntbn * P.nzs * nb, num_sms, st);
+    }
+    {   // streamed form: A = Ey planes (box = a 128-row b tile), B = H planes (box = this CTA's 64 rows of an a tile)
         cuuint64_t dims[3] = {(cuuint64_t)t.NY, (cuuint64_t)t.NPYP, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * (cuuint64_t)t.NPYP * 2};
         cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
         ok = encode_map(&tmA, d_Eyp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
-    if (ok) {   // box = one CTA's rows of an H tile
-        const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
-        cuuint64_t dims[3] = {(cuuint64_t)t.NY, rows, 4};
-        cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
-        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)(t.nyz / ncta), 1};
+    if (ok) {
+        cuuint64_t dims[3] = {(cuuint64_t)t.NY, hrows, 4};
+        cuuint64_t strides[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * hrows * 2};
+        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)(t.nyz / 2), 1};
         ok = encode_map(&tmB, d_Hp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
     if (!ok) {
         if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
         return cudaErrorUnknown;
     }
-    SepYzParams P;
-    P.nz = p.nz; P.nb = nb; P.npx = npx; P.npy = npy; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nzs = t.nzs;
-    P.ntb = t.NPYP / kM; P.nta = t.NPXP / t.nyz; P.nkb = t.NY / kKB;
-    P.k = 2.0 * 3.14159265358979323846 / p.lambda; P.dz = p.dz;
-    P.qx = d_qx; P.qy = d_qy; P.flags = d_flags64; P.zb = d_bounds + (t.nsx + 1); P.partial = d_partial;
-    if (t.yz_t) {
-        // A map: the Ey planes, box = this CTA's NB rows of one 64-y block; B map: the H planes, box = a whole a tile
-        cuuint64_t dimsA[3] = {(cuuint64_t)t.NY, (cuuint64_t)t.NPYP, 4};
-        cuuint64_t stridesA[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * (cuuint64_t)t.NPYP * 2};
-        cuuint32_t boxA[3] = {(cuuint32_t)kKB, (cuuint32_t)t.yzt_nb, 1};
-        const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NPXP;
-        cuuint64_t dimsB[3] = {(cuuint64_t)t.NY, rows, 4};
-        cuuint64_t stridesB[2] = {(cuuint64_t)t.NY * 2, (cuuint64_t)t.NY * rows * 2};
-        cuuint32_t boxB[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
-        if (!encode_map(&tmA, d_Eyp, 3, dimsA, stridesA, boxA, CU_TENSOR_MAP_SWIZZLE_128B) ||
-            !encode_map(&tmB, d_Hp, 3, dimsB, stridesB, boxB, CU_TENSOR_MAP_SWIZZLE_128B)) {
-            if (err) *err = "cuTensorMapEncodeTiled failed or is unavailable";
-            return cudaErrorUnknown;
-        }
-        const int nit = (t.NPXP / (2 * kM)) * (t.NPYP / (2 * t.yzt_nb)) * P.nzs * nb, maxc = num_sms / 2;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
-        cfg.blockDim = dim3(kThreadsTc);
-        cfg.dynamicSmemBytes = kSmem;
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 2;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, sep_tc_yzt_kernel<64>, tmA, tmB, P);
-    }
-    if (t.yz_stream) {
-        const int nit = (P.ntb / 2) * P.nta * P.nzs * nb, maxc = num_sms / 2;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
-        cfg.blockDim = dim3(kThreadsTc);
-        cfg.dynamicSmemBytes = kSmem;
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 2;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, sep_tc_yzs_kernel, tmA, tmB, P);
-    }
-    const int nitems = (P.ntb / ncta) * P.nta * P.ng * P.nzs * nb;
-    if (t.nyz == 128) return launch_yz128_variant<1>(tmA, tmB, P, nitems, num_sms, kSmem, st);
-    sep_tc_yz_kernel<<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
-    return cudaGetLastError();
+    const int nit = (P.ntb / 2) * P.nta * P.nzs * nb, maxc = num_sms / 2;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(2 * (nit < maxc ? nit : maxc)));
+    cfg.blockDim = dim3(kThreadsTc);
+    cfg.dynamicSmemBytes = kSmemYzs;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, sep_tc_yzs_kernel, tmA, tmB, P);
 }
 
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
@@ -2093,48 +903,19 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
     return cudaGetLastError();
 }
 
-template <int NX>
-static cudaError_t launch_x_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
-                                    cudaStream_t st) {
-    constexpr int kSmem = kSmemX;
-    const int nitems = P.nta * P.nsx;
-    sep_tc_x_kernel<NX><<<nitems < num_sms ? nitems : num_sms, kThreadsTc, kSmem, st>>>(tmA, tmB, P);
-    return cudaGetLastError();
-}
-
-template <int NX>
-static cudaError_t launch_x2_variant(const CUtensorMap &tmA, const CUtensorMap &tmB, const SepXParams &P, int num_sms,
-                                     cudaStream_t st) {
-    constexpr int kSmem = kSmemX;
-    const int nitems = P.nta * P.nsx, max_clusters = num_sms / 2;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(2 * (nitems < max_clusters ? nitems : max_clusters)));
-    cfg.blockDim = dim3(kThreadsTc);
-    cfg.dynamicSmemBytes = kSmem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, sep_tc_x2_kernel<NX>, tmA, tmB, P);
-}
-
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
                             const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
                             cudaStream_t st, std::string *err) {
     CUtensorMap tmA, tmB;
     bool ok;
-    {
+    {   // streamed: the rho~ planes [4][slices NY][NXP], box = 64 x of a 128-row tile
         const cuuint64_t rows = (cuuint64_t)p.nz * nb * t.NY;
-        cuuint64_t dims[3] = {(cuuint64_t)t.NXP, rows, 4};
-        cuuint64_t strides[2] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * rows * 2};
-        cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1};
-        ok = encode_map(&tmA, d_Rp, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+        cuuint64_t dims[4] = {(cuuint64_t)t.NXP, rows, 1, 4};
+        cuuint64_t strides[3] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * rows * 2, (cuuint64_t)t.NXP * rows * 2};
+        cuuint32_t box[4] = {(cuuint32_t)kKB, (cuuint32_t)kM, 1, 1};
+        ok = encode_map(&tmA, d_Rp, 4, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
     }
-    if (ok) {
+    if (ok) {   // resident: the Ex planes [4][NPXP][NXP], box = this CTA's NX rows of one 64-x block
         cuuint64_t dims[3] = {(cuuint64_t)t.NXP, (cuuint64_t)t.NPXP, 4};
         cuuint64_t strides[2] = {(cuuint64_t)t.NXP * 2, (cuuint64_t)t.NXP * (cuuint64_t)t.NPXP * 2};
         cuuint32_t box[3] = {(cuuint32_t)kKB, (cuuint32_t)t.NX, 1};
@@ -2145,22 +926,17 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
         return cudaErrorUnknown;
     }
     SepXParams P;
-    P.nz = p.nz * nb; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nkx = t.NXP / kKB; P.nta = t.NPXP / (t.NX * t.x_ncta);
+    P.nk = t.NXP / kKB;
+    P.nz = p.nz * nb; P.NY = t.NY; P.NPXP = t.NPXP; P.ng = t.ng; P.nta = t.NPXP / (2 * t.NX);
     P.nsx = t.nsx;
     P.nkb = t.NY / kKB;
     P.hscale = ldexpf(1.f, -9 - t.L);
     P.flags = d_flags64; P.zb = d_bounds; P.Hp = d_Hp;
-    if (t.x_ncta == 2) {
-        switch (t.NX) {
-            case 64: return launch_x2_variant<64>(tmA, tmB, P, num_sms, st);
-            case 32: return launch_x2_variant<32>(tmA, tmB, P, num_sms, st);
-            default: return launch_x2_variant<16>(tmA, tmB, P, num_sms, st);
-        }
-    }
+    const int nitems = P.nta * P.nsx;
     switch (t.NX) {
-        case 64: return launch_x_variant<64>(tmA, tmB, P, num_sms, st);
-        case 32: return launch_x_variant<32>(tmA, tmB, P, num_sms, st);
-        default: return launch_x_variant<16>(tmA, tmB, P, num_sms, st);
+        case 64: return tcg::cgemm_launch<SepXPolicy<64>>(tmA, tmB, P, nitems, num_sms, st);
+        case 32: return tcg::cgemm_launch<SepXPolicy<32>>(tmA, tmB, P, nitems, num_sms, st);
+        default: return tcg::cgemm_launch<SepXPolicy<16>>(tmA, tmB, P, nitems, num_sms, st);
     }
 }
 

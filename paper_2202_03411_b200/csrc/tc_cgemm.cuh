@@ -26,12 +26,14 @@
 //         static Item item(const Params &, int index);
 //         static int b_row0(const Params &, const Item &);                       // first B row (column of C) of the item's column tile
 //         Units: void begin(const Params &, const Item &, int lane);
-//                bool next(int &u0, int &u1, bool &dup);                         // units of leader / peer; false at the end
+//                bool next(int &u0, int &u1, bool &dup, uint32_t &kmask);        // units of leader / peer, live 64-k blocks; false at the end
+//         static constexpr bool kUnrollEpilogue;         // column loop of the epilogue fully unrolled (register-array accumulators)
+//         static constexpr int kEpilogueRegs;            // 0, or registers per epilogue thread after setmaxnreg (the other warps drop to 48)
 //         static void a_coords(const Params &, const Item &, int unit, int kb, int (&c)[3]);   // TMA coordinates {k, row, outer} of a 64-k block
 //         struct Epilogue { begin(P, item, ...), unit(...), end(...) };          // see the users
 //     };
-// Users: nufft_tensor_kernels.cu (stages Y and Z of the NUFFT route).  The separable route's stage kernels
-// (sep_tensor_kernels.cu) are older hand-written instances of the same pipeline.
+// Users: sep_tensor_kernels.cu (stage X and the transposed stage YZ of the separable route), nufft_tensor_kernels.cu (stages Y
+// and Z of the NUFFT route).
 #pragma once
 #include <cuda.h>
 
@@ -58,6 +60,12 @@ struct EpiThread {
     int col0;         // first of the NB accumulator columns this thread reads
     uint32_t rank;    // CTA rank in the pair
 };
+
+// The register file is re-split when the epilogue needs more than the 168 registers a 384-thread CTA gives each thread: the
+// producer / issuer warpgroup drops to 48, the two epilogue warpgroups rise to N: 128 x 48 + 256 x N must not exceed the
+// 384 x 168 the CTA owns (an increase can only take what the CTA's own warps released, or it waits forever) -> N <= 224.
+template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void setmaxnreg_dec_48() { asm volatile("setmaxnreg.dec.sync.aligned.u32 48;"); }
 
 template <class Policy>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -108,7 +116,10 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
     ptx::tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_ptr, 0);
 
-    if (warp == 0) {
+    // (each role's code must be DOMINATED by its setmaxnreg: ptxas allots the raised register count only to such code)
+    if (warp < 4) {
+      if constexpr (Policy::kEpilogueRegs != 0) setmaxnreg_dec_48();
+      if (warp == 0) {
         // ===================================================================== TMA producer (both CTAs)
         int slot = 0;
         uint32_t phase = 0;
@@ -128,9 +139,11 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
             un.begin(P, it, lane);
             int u0, u1;
             bool dup;
-            while (un.next(u0, u1, dup)) {
+            uint32_t kmask;
+            while (un.next(u0, u1, dup, kmask)) {
                 const int u = leader ? u0 : u1;
                 for (int kb = 0; kb < nk; ++kb) {
+                    if (((kmask >> kb) & 1u) == 0u) continue;   // a 64-k block that holds nothing: never loaded, never multiplied
                     int c[3];
                     Policy::a_coords(P, it, u, kb, c);
                     for (int ph = 0; ph < 2; ++ph) {   // Re planes, Im planes
@@ -146,7 +159,7 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
                 }
             }
         }
-    } else if ((warp == 1 || warp == 3) && leader) {
+      } else if ((warp == 1 || warp == 3) && leader) {
         // ===================================================================== MMA issuers (leader; k-step ks belongs to issuer ks % 2)
         constexpr uint32_t idesc_pos = ptx::umma_idesc_f16(2 * kM, kN, false);
         constexpr uint32_t idesc_neg = ptx::umma_idesc_f16(2 * kM, kN, true);
@@ -166,14 +179,17 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
             un.begin(P, it, lane);
             int u0, u1;
             bool dup;
-            while (un.next(u0, u1, dup)) {
+            uint32_t kmask;
+            while (un.next(u0, u1, dup, kmask)) {
                 const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
                 ptx::mbar_wait(t_empty + buf, upar ^ 1);
                 ptx::tc_fence_after();
                 const uint32_t d_re = tmem_base + buf * 256, d_im = d_re + 128;
-                for (int kb = 0; kb < nk; ++kb)
+                bool first = true;                             // the unit's first live k block
+                for (int kb = 0; kb < nk; ++kb) {
+                    if (((kmask >> kb) & 1u) == 0u) continue;
                     for (int ph = 0; ph < 2; ++ph) {
-                        if (iw == 1 && kb == 0 && ph == 0) {   // D must have been initialised by issuer 0
+                        if (iw == 1 && first && ph == 0) {     // D must have been initialised by issuer 0
                             ptx::mbar_wait(first_done + buf, upar);
                             ptx::tc_fence_after();
                         }
@@ -186,7 +202,7 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
                                 const uint64_t a_hi = descA0 + (uint64_t)slot * kSt + (uint64_t)(ks * 2), a_lo = a_hi + kA;
                                 const uint64_t b_reh = descB0 + (uint64_t)kb * kB + (uint64_t)(ks * 2);
                                 const uint64_t b_rel = b_reh + kBpl, b_imh = b_rel + kBpl, b_iml = b_imh + kBpl;
-                                const uint32_t acc0 = (kb == 0 && ph == 0 && ks == 0) ? 0u : 1u;
+                                const uint32_t acc0 = (first && ph == 0 && ks == 0) ? 0u : 1u;
                                 // (Ar + i Ai)(Br + i Bi) with the A planes of this stage: AhBh + AhBl + AlBh
                                 if (ph == 0) {   // A Re hi, Re lo
                                     ptx::umma_f16_2sm(d_re, a_hi, b_reh, idesc_pos, acc0);
@@ -203,13 +219,15 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
                                     ptx::umma_f16_2sm(d_re, a_lo, b_imh, idesc_neg, 1u);
                                     ptx::umma_f16_2sm(d_im, a_lo, b_reh, idesc_pos, 1u);
                                 }
-                                if (iw == 0 && kk == 0 && kb == 0 && ph == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
+                                if (iw == 0 && kk == 0 && first && ph == 0) ptx::umma_commit_2sm(first_done + buf, (uint16_t)0x1);
                             }
                             ptx::umma_commit_2sm(a_empty + slot, (uint16_t)0x3);
                         }
                         __syncwarp();
                         if (++slot == kStages) { slot = 0; phase ^= 1; }
                     }
+                    first = false;
+                }
                 if (ptx::elect_one()) ptx::umma_commit_2sm(t_full + buf, (uint16_t)0x3);
                 __syncwarp();
                 ++u;
@@ -217,7 +235,9 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
             if (ptx::elect_one()) ptx::umma_commit_2sm(b_empty, (uint16_t)0x3);
             __syncwarp();
         }
-    } else if (warp >= 4) {
+      }
+    } else {
+        if constexpr (Policy::kEpilogueRegs != 0) setmaxnreg_inc<Policy::kEpilogueRegs != 0 ? Policy::kEpilogueRegs : 168>();
         // ===================================================================== epilogue: this CTA's 128 rows x 2 NB columns
         const int lg = warp & 3, ch = (warp - 4) >> 2;     // TMEM lane group; column half [ch NB, +NB)
         const uint32_t t_lane = tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(ch * NB);
@@ -234,27 +254,36 @@ cgemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CU
             un.begin(P, it, lane);
             int u0, u1;
             bool dup;
-            while (un.next(u0, u1, dup)) {
+            uint32_t kmask;
+            while (un.next(u0, u1, dup, kmask)) {
                 const int unit = leader ? u0 : u1;
                 const bool keep = leader || !dup;
                 const uint32_t buf = u % kNBuf, upar = (u / kNBuf) & 1;
+                epi.unit_begin(P, it, et, unit);
                 ptx::mbar_wait(t_full + buf, upar);
                 ptx::tc_fence_after();
                 const uint32_t t_re = t_lane + buf * 256, t_im = t_re + 128;
-                epi.unit_begin(P, it, et, unit);
+#define SCATMAN_EPILOGUE_EIGHT_COLUMNS(c0)                                                                            \
+    {                                                                                                                    \
+        uint32_t gre[8], gim[8];                                                                                         \
+        ptx::tmem_ld8(t_re + (c0), gre);                                                                                 \
+        ptx::tmem_ld8(t_im + (c0), gim);                                                                                 \
+        ptx::tmem_ld_wait();                                                                                             \
+        if ((c0) + 8 >= NB) { /* every column of this warp has landed: hand the buffer back */                           \
+            ptx::tc_fence_before();                                                                                      \
+            __syncwarp();                                                                                                \
+            if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0); /* the leader's barrier */                        \
+        }                                                                                                                \
+        if (keep) epi.columns(P, it, et, unit, (c0), gre, gim);                                                          \
+    }
+                if constexpr (Policy::kUnrollEpilogue) {   // register-array accumulators: every column index must be static
+#pragma unroll
+                    for (int c0 = 0; c0 < NB; c0 += 8) SCATMAN_EPILOGUE_EIGHT_COLUMNS(c0)
+                } else {
 #pragma unroll 1
-                for (int c0 = 0; c0 < NB; c0 += 8) {
-                    uint32_t gre[8], gim[8];
-                    ptx::tmem_ld8(t_re + c0, gre);
-                    ptx::tmem_ld8(t_im + c0, gim);
-                    ptx::tmem_ld_wait();
-                    if (c0 + 8 >= NB) {                    // every column of this warp has landed: hand the buffer back
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive_cluster(t_empty + buf, 0);   // the leader's barrier
-                    }
-                    if (keep) epi.columns(P, it, et, unit, c0, gre, gim);
+                    for (int c0 = 0; c0 < NB; c0 += 8) SCATMAN_EPILOGUE_EIGHT_COLUMNS(c0)
                 }
+#undef SCATMAN_EPILOGUE_EIGHT_COLUMNS
                 ++u;
             }
             epi.end(P, it, et);
@@ -297,7 +326,8 @@ inline cudaError_t cgemm_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, 
 struct RangeUnits {
     int cur, end;
     __device__ __forceinline__ void set(int b, int e) { cur = b; end = e; }
-    __device__ __forceinline__ bool next(int &u0, int &u1, bool &dup) {
+    __device__ __forceinline__ bool next(int &u0, int &u1, bool &dup, uint32_t &kmask) {
+        kmask = 0xffffffffu;
         if (cur >= end) return false;
         u0 = cur;
         dup = cur + 1 >= end;
