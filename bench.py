@@ -23,10 +23,10 @@ sys.path.insert(0, ROOT)
 SPLITS = 3           # FP16x3: AhBh + AlBh + AhBl
 FLOP_PER_TERM = 8    # one complex MAC
 # dram__bytes_read.sum + dram__bytes_write.sum of one contraction launch, from the committed `ncu --set full` capture
-# (profiles/r01_contract_cfg3_full.md); only the workload that was captured has a number
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": 2.295495e9 + 8.534016e6}
-# the same for the four launches of one NUFFT pattern (stages Z, X, Y, interpolation; profiles/r01_nufft.md)
-NCU_DRAM_BYTES_NUFFT = {"cfg3_droplet_256": (134.46 + 24.46 + 46.63 + 0.91 + 20.85 + 0.0 + 8.27 + 0.0) * 1e6}
+# (profiles/r02_contract_cfg3_full.md); only the workload that was captured has a number
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg3_droplet_256": 970.813952e6 + 8.573184e6}   # profiles/r02_contract_cfg3_full.md (r01: 2.30e9, with the M_z table)
+# the same for the kernels of one NUFFT pattern (strength, pack, stages X, Y, Z, interpolation; profiles/r02_nufft_tensor.md)
+NCU_DRAM_BYTES_NUFFT = {"cfg3_droplet_256": (134.25 + 91.21 + 134.23 + 88.48 + 104.12 + 17.44 + 59.54 + 3.20 + 29.79 + 0.0 + 8.68 + 0.0) * 1e6}
 
 
 def load_peaks():
@@ -107,11 +107,16 @@ def run_reference(args):
     vox = (w.dx, w.dy, w.dz)
     if args.ref_pixels > 0:
         npix_s = max(8, int(args.ref_pixels))
-    else:   # ~10 s per step from a short probe
-        probe = W.sample_pixels(w.seed + 99, w.npix, 32)
-        t0 = time.perf_counter()
-        O.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, pixels=probe)
-        npix_s = int(min(8192, max(128, 10.0 / ((time.perf_counter() - t0) / len(probe)))))
+    else:   # ~10 s per step; two probes separate the per-call set-up from the per-pixel cost
+        tp = []
+        for n_probe in (16, 80):
+            probe = W.sample_pixels(w.seed + 99, w.npix, n_probe)
+            t0 = time.perf_counter()
+            O.simulate(g, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=quat, pixels=probe)
+            tp.append((len(probe), time.perf_counter() - t0))
+        per_pixel = max(1e-9, (tp[1][1] - tp[0][1]) / (tp[1][0] - tp[0][0]))
+        setup = max(0.0, tp[0][1] - tp[0][0] * per_pixel)
+        npix_s = int(min(8192, max(128, (10.0 - setup) / per_pixel)))
     pix = W.sample_pixels(w.seed, w.npix, npix_s)
     times = []
     for i in range(args.warmup + args.steps):
@@ -589,17 +594,22 @@ def main():
                         "issued_fraction_of_dense": issued / (3.0 * dense_sep),
                         "useful_dense_tflops": dense_sep / (k_ms * 1e-3) / 1e12, **tensor_roofline_extras(ach, clocks, peaks)}
     elif args.route in ("nufft", "shapes_nufft"):
-        # three complex GEMMs (slices -> g_z planes, columns -> g_x, rows -> g_y) + the 10^3-point interpolation:
-        # 8 flop per complex MAC of the GEMMs, 4 per (real weight x complex value) MAC of the interpolation.
+        # The route moves 8 B per voxel in and 4 B per pixel out and does ~3e-4 of the pixel route's arithmetic: its speed of light
+        # is the HBM time of those bytes.  Algorithmic bytes per launch set = batch x (8 nvox + 4 npix); the GEMM stages' tensor
+        # rate (24 issued flop per complex MAC of the dense transform) and the flop count are reported beside it.
         nqx, nqy, nqz = nq
-        flop = batch * (8.0 * (nqz * w.nz * w.ny * w.nx + nqz * w.ny * w.nx * nqx + nqz * nqy * w.ny * nqx) + 4.0 * npix_r * 10 ** 3)
-        peak = 148 * 64 * 2 * 1.965e9 / 1e12           # FP64 FMA: 148 SMs x 64 lanes x 2 flop x max clock
-        ach = flop / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "NUFFT stages (GEMMs Z, X, Y) + nufft_interp_kernel", "achieved": ach, "peak": peak,
-                    "unit": "TFLOP/s", "frac": ach / peak, "traffic": NCU_DRAM_BYTES_NUFFT.get(w.name) if batch == 1 else None,
+        hbm, hbm_src = load_peaks_hbm()
+        abytes = batch * (8.0 * w.nvox + 4.0 * npix_r)
+        ach = abytes / (k_ms * 1e-3) / 1e9
+        cmacs = batch * (w.nz * w.ny * w.nx * nqx + w.nz * nqx * w.ny * nqy + w.nz * nqx * nqy * nqz)     # stages X, Y, Z as run
+        flop = 8.0 * cmacs + 4.0 * batch * npix_r * 10 ** 3
+        roofline = {"bound": "hbm", "kernel": "strength + pack + GEMM stages X, Y, Z (tcgen05) + nufft_interp_kernel", "achieved": ach,
+                    "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "peak_source": hbm_src,
+                    "traffic": NCU_DRAM_BYTES_NUFFT.get(w.name) if batch == 1 else None,
                     "kernel_ms": k_ms, "uniform_grid": [nqz, nqy, nqx],
-                    "achieved_is": "dense flop of the three GEMM stages (8 per complex MAC) and the interpolation / their CUDA-event time, "
-                                   "against the FP64 ALU peak the interpolation runs on",
+                    "achieved_is": "algorithmic bytes (8 B per voxel read + 4 B per pixel written) / CUDA-event time of the per-chunk launches "
+                                   "(pack, stages X, Y, Z, interpolation); the prefix kernel a2 runs before the events",
+                    "gemm_stages_issued_tflops_upper": 24.0 * cmacs / (k_ms * 1e-3) / 1e12,
                     "flop_vs_pixel_route": flop / (FLOP_PER_TERM * terms_per_pattern * batch)}
     elif args.method == 1:
         # what the contraction really issued: it skips all-zero 16-y steps and narrows units to their non-empty x range.
@@ -643,11 +653,16 @@ def main():
         if args.route in ("shapes", "shapes_nufft"):     # the oracle's own rendering of item 0 (already in the beam frame)
             from oracle import render as OR
             g0, q0 = OR.render(shapes[0], dims, vox), None
-        probe = W.sample_pixels(w.seed + 99, w.npix, 32)
-        t0 = time.perf_counter()
-        O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=probe)
-        per_pixel = (time.perf_counter() - t0) / len(probe)
-        npix_s = args.ref_pixels if args.ref_pixels > 0 else int(min(8192, max(256, 15.0 / per_pixel)))
+        # two probes separate the per-call set-up (orientation, prefix) from the per-pixel cost
+        tp = []
+        for n_probe in (16, 80):
+            probe = W.sample_pixels(w.seed + 99, w.npix, n_probe)
+            t0 = time.perf_counter()
+            O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=probe)
+            tp.append((len(probe), time.perf_counter() - t0))
+        per_pixel = max(1e-9, (tp[1][1] - tp[0][1]) / (tp[1][0] - tp[0][0]))
+        setup = max(0.0, tp[0][1] - tp[0][0] * per_pixel)
+        npix_s = args.ref_pixels if args.ref_pixels > 0 else int(min(8192, max(256, (15.0 - setup) / per_pixel)))
         pix = W.sample_pixels(w.seed, npix_r, npix_s) + y0 * w.npx
         t0 = time.perf_counter()
         ref = O.simulate(g0, vox, w.lam, w.npx, w.npy, w.theta_max_deg, quat=q0, pixels=pix)

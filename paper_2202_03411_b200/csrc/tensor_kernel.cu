@@ -13,11 +13,13 @@
 //
 // Roles: warp 0 = TMA producer, warps 1 and 3 = MMA issuers (k-step n of a unit belongs to issuer n % 2), warp 2 = TMEM
 // allocator, warps 4-7 = epilogue (TMEM lane group = warp % 4).  Pipelines: A-resident (a_full/a_empty), B ring of
-// kStagesB slots (b_full/b_empty), two TMEM accumulator buffers (t_full/t_empty), first_done orders issuer 1 behind the
+// kStagesB slots (b_full[issuer]/b_empty), two TMEM accumulator buffers (t_full/t_empty), first_done orders issuer 1 behind the
 // unit's first k-step.  Ordering between the two issuing threads (tcgen05.mma is ordered only within one thread): a
 // unit's accumulator is initialised by issuer 0's first k-step and issuer 1 waits for its completion (first_done);
-// after that both threads only ACCUMULATE into D, and FP32 accumulation order differences are within the tolerance
-// budget; both commit t_full (count 2), so the epilogue sees every MMA of both threads.
+// after that both threads only ACCUMULATE into D, in whatever order their MMAs reach the tensor pipe -- results are
+// reproducible to FP32 summation order, not bit for bit; both commit t_full (count 2), so the epilogue
+// sees every MMA of both threads.  A B slot is filled for ONE issuer (the owner of its k-step) and signalled on that issuer's
+// own full barrier, so each issuer sees every completion of the barriers it waits on and a parity can never alias.
 #include <cuda.h>
 
 #include "internal.h"
@@ -160,8 +162,12 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     uint8_t *sB = smem + kSmemA;
     uint64_t *bars = (uint64_t *)(smem + kSmemA + kSmemB);
     uint64_t *a_full = bars + 0, *a_empty = bars + 1;
-    uint64_t *b_full = bars + 2, *b_empty = bars + 2 + kMaxStagesB;
-    uint64_t *t_full = bars + 2 + 2 * kMaxStagesB, *t_empty = t_full + 2, *first_done = t_empty + 2;
+    // b_full[i][slot]: "slot filled" for a k-step owned by MMA issuer i.  Each issuer has its OWN full barriers: it waits on every
+    // completion of each of them, in order, so a parity wait can never take an older pass for the current one (with one shared
+    // barrier per slot an issuer saw only the passes of its own k-steps -- every other one where units have odd k-step counts --
+    // and "pass R - 2 complete" is indistinguishable from "pass R complete" by parity).
+    uint64_t *b_full = bars + 2, *b_empty = bars + 2 + 2 * kMaxStagesB;
+    uint64_t *t_full = bars + 2 + 3 * kMaxStagesB, *t_empty = t_full + 2, *first_done = t_empty + 2;
     uint32_t *tmem_ptr = (uint32_t *)(first_done + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -180,7 +186,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         ptx::mbar_init(a_empty, 2);      // both MMA issuers
         for (int i = 0; i < kStagesB; ++i) {
             ptx::mbar_init(b_full + i, 1);
-            ptx::mbar_init(b_empty + i, 2);   // both MMA issuers (see the issuer loop)
+            ptx::mbar_init(b_full + kMaxStagesB + i, 1);
+            ptx::mbar_init(b_empty + i, 1);
         }
         for (int i = 0; i < 2; ++i) {
             ptx::mbar_init(t_full + i, 2);   // both MMA issuers
@@ -241,18 +248,21 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                 // one box = one 16-y step: {256-byte atom, 4 planes, xm x-groups of this CTA's half (16 for one CTA)}
                 const CUtensorMap *tmb = &tmB.m[xm - 1];
                 const uint32_t tx_bytes = NCTA == 2 ? (uint32_t)(2 * xm * 1024) : (uint32_t)kSlotBytes;
+                int kidx = 0;                                                   // k-step index within the unit: its parity = the issuer that owns it
                 for (int yi = 0; yi < 4 * nybg; ++yi) {
                     if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // this 16-y step of the slice tile is empty
                     ptx::mbar_wait(b_empty + slot, phase ^ 1);
+                    uint64_t *full = b_full + (kidx & 1) * kMaxStagesB + slot;
+                    ++kidx;
                     if (ptx::elect_one()) {
-                        if (leader) ptx::mbar_arrive_expect_tx(b_full + slot, tx_bytes);
+                        if (leader) ptx::mbar_arrive_expect_tx(full, tx_bytes);
                         void *dst = sB + slot * kSlotB;
                         const int cg = uxt * 16 + (NCTA == 2 ? (int)rank * 8 + xa : 0);
                         const int cs = (ub * P.nz + uj) * P.ny16 + it.g * (kGroupYB * kBlockY / 16) + yi;
                         SCATMAN_ASSERT(xm >= 1 && xm <= 8 && xa >= 0 && xa + xm <= 8);
                         SCATMAN_ASSERT(ub < P.batch && uj < P.nz && cs < P.batch * P.nz * P.ny16 && cg + (NCTA == 2 ? xm : 16) <= P.nxt * 16);
-                        if (NCTA == 2) ptx::tma_load_4d_2sm(dst, tmb, b_full + slot, 0, 0, cg, cs);
-                        else ptx::tma_load_4d(dst, tmb, b_full + slot, 0, 0, cg, cs);
+                        if (NCTA == 2) ptx::tma_load_4d_2sm(dst, tmb, full, 0, 0, cg, cs);
+                        else ptx::tma_load_4d(dst, tmb, full, 0, 0, cg, cs);
                     }
                     __syncwarp();
                     if (++slot == kStagesB) { slot = 0; phase ^= 1; }
@@ -284,7 +294,8 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
         };
         const int iw = warp >> 1;   // issuer 0 = warp 1, issuer 1 = warp 3
         int slot = 0;
-        uint32_t phase = 0;
+        uint32_t full_phase = 0;                                   // bit s: parity of the next pass of my_full[s]
+        uint64_t *my_full = b_full + iw * kMaxStagesB;
         uint32_t u = 0;
         int it_local = 0;
         for (int item = cluster_id; item < nitems; item += nclusters, ++it_local) {
@@ -316,21 +327,9 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                     int kidx = 0;            // k-step index within the unit
                     for (int yi = 0; yi < 4 * nybg; ++yi) {
                         if (((uint32_t)(m >> (8 * yi)) & 0xffu) == 0u) continue;   // empty 16-y step: never loaded
-                        // BOTH issuers observe every pass of every slot's full barrier and BOTH release the slot (b_empty
-                        // counts 2: the owner's tcgen05.commit + a plain arrive of the other issuer).  A parity wait tells
-                        // pass R from pass R - 1 only: were a slot re-armed while one issuer had not seen its previous pass
-                        // (units with odd k-step counts shift the ownership of a slot between the issuers), that issuer
-                        // could take "pass R - 2 complete" for "pass R complete" and consume stale data.  With both
-                        // arrivals the producer cannot run more than one pass ahead of either issuer, whatever order the
-                        // TMA loads complete in.  The extra wait runs while the issuer's own MMAs execute.
-                        ptx::mbar_wait(b_full + slot, phase);
-                        if ((kidx & 1) != iw) {
-                            if (ptx::elect_one()) {
-                                ptx::mbar_arrive(b_empty + slot);
-                                if (NCTA == 2) ptx::mbar_arrive_cluster(b_empty + slot, 1);
-                            }
-                            __syncwarp();
-                        } else {
+                        if ((kidx & 1) == iw) {
+                            ptx::mbar_wait(my_full + slot, (full_phase >> slot) & 1u);   // this issuer's own barrier of the slot
+                            full_phase ^= 1u << slot;
                             if (kidx == 1) {   // issuer 1's first k-step of the unit: D must have been initialised
                                 ptx::mbar_wait(first_done + buf, upar);
                             }
@@ -362,7 +361,7 @@ msft_contract_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
                             __syncwarp();
                         }
                         ++kidx;
-                        if (++slot == kStagesB) { slot = 0; phase ^= 1; }
+                        if (++slot == kStagesB) slot = 0;
                     }
                     if (ptx::elect_one()) commit(t_full + buf);
                     __syncwarp();
