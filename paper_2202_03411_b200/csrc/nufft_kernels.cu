@@ -216,7 +216,8 @@ __device__ inline double placed(const double (&own)[kW], int shift, int a) {
 
 constexpr int kInterpThreads = 128;
 constexpr int kTX = 8, kTY = 16;         // a block = 8 groups of P pixels along a detector row x 16 rows
-constexpr int kTileCap = 4096;           // float2 elements of shared memory for the block's window of U (32 KB)
+constexpr int kTileCap = 6144;           // float2 elements of shared memory for the block's window of U (48 KB: with the 24 KB of weights,
+                                         // three blocks per SM either way)
 
 // A block owns a TILE of 8 P x 8 pixels.  Its pixels' windows overlap heavily, so the block first copies the box of U that covers
 // all of them into shared memory (coalesced, every thread loading: the whole box is in flight at once) and the per-thread sums
@@ -267,7 +268,9 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             atomicMin(&red[d], base[d]);
-            atomicMax(&red[3 + d], base[d] + KU - 1);    // last cell a common window of KU cells can touch
+            // last cell the thread reads: along x every row is read over the whole common window of KU cells; along y and z
+            // rows and planes whose weights are all zero are skipped, so only the pixels' own windows count
+            atomicMax(&red[3 + d], d == 0 ? base[d] + KU - 1 : top[d] + kW - 1);
         }
         if (!common) atomicAnd(&red[6], 0);
     }
@@ -293,13 +296,17 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
         // The x weights and the row sums over x (12 of the 14 multiply-adds of a grid value) are FP32: a row sum of <= 12 terms of
         // one sign pattern rounds at ~1e-7 of its own magnitude, the same size as the FP32 rounding U already carries; the sums over
         // y and z (where rows of different phase combine) stay FP64.
-        float wx[P][KU];
+        // kept as (w, w) pairs: one packed fma.rn.f32x2 (sm_100) multiplies a grid value's (Re, Im) by the real weight
+        float2 wx[P][KU];
 #pragma unroll
         for (int j = 0; j < P; ++j) {
             double own[kW];
             kb_weights(u[j][0], m0[j][0], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) wx[j][a] = (float)placed<KU>(own, m0[j][0] - base[0], a);
+            for (int a = 0; a < KU; ++a) {
+                const float w = (float)placed<KU>(own, m0[j][0] - base[0], a);
+                wx[j][a] = make_float2(w, w);
+            }
             kb_weights(u[j][1], m0[j][1], own);
 #pragma unroll
             for (int a = 0; a < KU; ++a) wy(j, a) = (float)placed<KU>(own, m0[j][1] - base[1], a);
@@ -343,14 +350,14 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
                 for (int a = 0; a < KU; ++a) v[a] = row[a];
 #pragma unroll
                 for (int j = 0; j < P; ++j) {
-                    float rre = 0.f, rim = 0.f;
+                    float2 ra = make_float2(0.f, 0.f), rb = make_float2(0.f, 0.f);   // two chains per pixel
 #pragma unroll
-                    for (int a = 0; a < KU; ++a) {
-                        rre = fmaf(wx[j][a], v[a].x, rre);
-                        rim = fmaf(wx[j][a], v[a].y, rim);
+                    for (int a = 0; a < KU; a += 2) {
+                        ra = __ffma2_rn(wx[j][a], v[a], ra);
+                        rb = __ffma2_rn(wx[j][a + 1], v[a + 1], rb);
                     }
-                    pre[j] = fma(wyb[j], (double)rre, pre[j]);
-                    pim[j] = fma(wyb[j], (double)rim, pim[j]);
+                    pre[j] = fma(wyb[j], (double)(ra.x + rb.x), pre[j]);
+                    pim[j] = fma(wyb[j], (double)(ra.y + rb.y), pim[j]);
                 }
             }
 #pragma unroll
