@@ -93,7 +93,7 @@ __global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
 // from three signed edge vectors, compared with the box of non-vacuum voxels widened by the interpolation cell -- then the block
 // zero-fills the tiles that cannot and resamples the others.  (One launch-sized block per tile, each loading the rotation and the
 // box and deciding on its own, was bound by that start-up latency, not by arithmetic or bytes: profiles/r02_orient_render.md.)
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)   // 64 registers: four CTAs per SM (at 100 registers two CTAs left the issue slots half empty)
 orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz, double3 inv,
               const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out) {
     const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
