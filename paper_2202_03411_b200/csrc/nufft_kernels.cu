@@ -216,8 +216,8 @@ __device__ inline double placed(const double (&own)[kW], int shift, int a) {
 
 constexpr int kInterpThreads = 128;
 constexpr int kTX = 8, kTY = 16;         // a block = 8 groups of P pixels along a detector row x 16 rows
-constexpr int kTileCap = 6144;           // float2 elements of shared memory for the block's window of U (48 KB: with the 24 KB of weights,
-                                         // three blocks per SM either way)
+constexpr int kTileCap = 3968;           // float2 elements of shared memory for the block's window of U (31 KB: with the 24 KB of weights
+                                         // and the 1 KB the driver reserves per block, four blocks fit an SM)
 
 // A block owns a TILE of 8 P x 8 pixels.  Its pixels' windows overlap heavily, so the block first copies the box of U that covers
 // all of them into shared memory (coalesced, every thread loading: the whole box is in flight at once) and the per-thread sums
