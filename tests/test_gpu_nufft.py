@@ -122,6 +122,19 @@ def test_batch_larger_than_one_chunk(sm, sim):
     assert not np.array_equal(I[7], I[8])
 
 
+def test_grids_beyond_the_tensor_stages_limits_fall_back_to_the_fp64_stages(sm):
+    """The tcgen05 stages keep a table tile resident in shared memory, which bounds every grid dimension (1024 x, 1024 y, 1024 z);
+    a taller grid runs the FP64 CUDA-core stages whatever method is asked for -- same result, silently."""
+    voxel, lam = (2.0, 0.5, 2.0), 9.0
+    g = W.sparse_blobs_grid(55, 24, 1100, 5, nblobs=5, max_extent=60)
+    npx, npy, th = 12, 40, 20.0
+    ref = O.simulate(g, voxel, lam, npx, npy, th)
+    for method in (0, 3):
+        I = sm.simulate_nufft(dev(g), voxel, lam, npx, npy, th, method=method).cpu().numpy()
+        l2, pix = assert_parity(I, ref, what=f"tall grid method {method}")
+        assert l2 <= 1e-6          # both are the FP64 stages
+
+
 def test_empty_and_single_voxel(sm, sim):
     voxel, lam = (3.0, 3.0, 3.0), 12.0
     z = np.zeros((8, 8, 8, 2), np.float32)

@@ -116,6 +116,21 @@ def test_wide_grids_use_narrower_stage_x_tiles(sm, nx):
     assert_parity(I, ref, what=f"qgrid tensor nx={nx}")
 
 
+@pytest.mark.parametrize("ny", [300, 530, 2100])
+def test_tall_grids_use_the_streamed_stage_yz_and_beyond_it_the_cuda_core_stages(sm, ny):
+    """N_y > 256: stage YZ streams both operands (odd numbers of 128-row b tiles are padded to pairs); N_y > 2048 falls back to the
+    CUDA-core stages."""
+    g = W.random_grid(98, 20, ny, 3, fill=0.5)
+    voxel, lam = (2.0, 0.4, 2.5), 9.0
+    qx, qy = _uniform_q(lam, 30.0, 19), _uniform_q(lam, 20.0, 150)      # 150 rows: two b tiles; 19 columns: one (odd) a tile
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS["tensor"]).cpu().numpy()
+    ref = O.simulate_qgrid(g, voxel, lam, qx, qy)
+    assert_parity(I, ref, what=f"qgrid tensor ny={ny}")
+    qy3 = _uniform_q(lam, 20.0, 300)                                     # three b tiles: an odd count
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy3), method=METHODS["tensor"]).cpu().numpy()
+    assert_parity(I, O.simulate_qgrid(g, voxel, lam, qx, qy3), what=f"qgrid tensor ny={ny}, 300 rows")
+
+
 @both_methods
 def test_cfg1_sphere_on_a_uniform_q_grid(sm, method):
     w = W.config(0)
