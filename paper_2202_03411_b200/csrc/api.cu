@@ -186,6 +186,11 @@ static bool valid_quats(const double *q, int batch) {
     }
     return true;
 }
+// One thread per (x, y) column walks z in the fused prefix -> planes kernel (launch_sep_tc_prefix_prep): it beats strength + pack
+// once a chunk's columns fill the SMs (measured: one item of 256^2 columns loses 22 us, one of 128^2 37 us; a chunk of 8 x 128^2 or
+// more gains 8 %).
+static bool fused_prefix_pays(const Plan &p, int chunk_items) { return (size_t)chunk_items * p.nx * p.ny >= (size_t)4 << 16; }
+
 static bool all_identity(const double *q, int batch) {
     for (int b = 0; b < batch; ++b)
         if (std::fabs(q[4 * b]) != 1.0 || q[4 * b + 1] != 0.0 || q[4 * b + 2] != 0.0 || q[4 * b + 3] != 0.0) return false;
@@ -215,6 +220,32 @@ static cudaError_t upload_rotmats(const double *h_quat, int batch, double *d_rot
         if (nlaunch) ++*nlaunch;
     }
     return cudaGetLastError();
+}
+
+// Extremes of grids the host already knows (rendered shapes: one (delta, beta) per item) reach the device as kernel arguments.
+struct StatsChunk {
+    unsigned v[3 * 256];
+};
+__global__ void store_stats_kernel(StatsChunk c, int n, unsigned *__restrict__ dst) {
+    for (int i = threadIdx.x; i < 3 * n; i += blockDim.x) dst[i] = c.v[i];
+}
+static cudaError_t upload_stats(const float *h_stats, int batch, unsigned *d_stats, cudaStream_t st, int *nlaunch) {
+    for (int b0 = 0; b0 < batch; b0 += 256) {
+        StatsChunk c;
+        const int n = batch - b0 < 256 ? batch - b0 : 256;
+        for (int i = 0; i < 3 * n; ++i) std::memcpy(&c.v[i], &h_stats[3 * b0 + i], sizeof(unsigned));
+        store_stats_kernel<<<1, 256, 0, st>>>(c, n, d_stats + 3 * b0);
+        if (nlaunch) ++*nlaunch;
+    }
+    return cudaGetLastError();
+}
+static void shape_stats(const scatman_shape *h_shapes, int batch, std::vector<float> &stats) {
+    stats.resize(3 * (size_t)batch);
+    for (int b = 0; b < batch; ++b) {
+        stats[3 * b] = std::fabs(h_shapes[b].delta);
+        stats[3 * b + 1] = std::fabs(h_shapes[b].beta);
+        stats[3 * b + 2] = h_shapes[b].beta < 0.f ? -h_shapes[b].beta : 0.f;
+    }
 }
 
 extern "C" {
@@ -515,9 +546,10 @@ struct SepPlan {
     Plan p;
     SepTcPlan tc;
     bool tensor = true;   // both GEMM stages on tcgen05 (method AUTO / TENSOR) or FP32 CUDA cores (SIMT_TABLE)
+    bool fused_ok = false;   // tensor stages: a chunk is large enough for the fused prefix -> planes pass (fused_prefix_pays)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, off_stats = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
                              int num_sms) {
@@ -542,8 +574,12 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
     sp.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
     sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
-    sp.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
+    // FP32 rho~: always for the CUDA-core stages; for the tensor stages only where chunks are too small for the fused pass (when they
+    // are not, strength + pack runs only on un-oriented input and borrows the orientation's buffer)
+    sp.fused_ok = sp.tensor && fused_prefix_pays(p, batch < sp.tc.nb ? batch : sp.tc.nb);
+    sp.off_rho = sp.fused_ok ? sp.off_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
+    sp.off_stats = take(sizeof(unsigned) * 3 * (size_t)batch);
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
         sp.off_rp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NY * t.NXP);
@@ -575,9 +611,12 @@ int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, in
     return SCATMAN_OK;
 }
 
-int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_qx,
-                           int32_t npx, const double *d_qy, int32_t npy, const double *h_quat, int32_t batch,
-                           const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+}  // extern "C"
+
+// h_stats: extremes of the grids when the host knows them (rendered shapes), else null (measured on the device)
+static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_qx,
+                      int32_t npx, const double *d_qy, int32_t npy, const double *h_quat, int32_t batch,
+                      const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats) {
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !d_qx || !d_qy || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) ||
@@ -604,19 +643,36 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     const bool reuse = (o.flags & SCATMAN_FLAG_REUSE_TABLES) && ctx->tables_valid && ctx->tables_key == key;
     ctx->tables_valid = false;
     const float *src = d_dn;
-    if (h_quat && !all_identity(h_quat, batch)) {
+    unsigned *stats = (unsigned *)(ws + sp.off_stats);
+    const bool oriented = h_quat && !all_identity(h_quat, batch);
+    if (oriented) {
         double *rm = (double *)(ws + sp.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
-        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), (int *)(ws + sp.off_bbox), st);
+        if (e == cudaSuccess)
+            e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), (int *)(ws + sp.off_bbox), st,
+                              sp.fused_ok ? stats : nullptr);
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + sp.off_rot);
     }
+    // Tensor stages, two ways to the FP16 planes of rho~:  fused (prefix -> planes in one pass, the FP32 rho~ never exists; the scale
+    // of the planes then comes from a bound of max |rho~| that needs the extremes of (delta, beta) BEFORE the prefix) when those
+    // extremes are free -- a0's bounding-box pass measures them, the host knows them for rendered shapes -- and the chunk has
+    // enough columns to fill the machine with one thread per column; else strength + pack (rho~ in FP32, in the buffer the
+    // orientation does not use then), which is faster for single grids (profiles/r02_orient_render.md).
+    const bool fused = sp.fused_ok && (oriented || h_stats);
     float *rho = (float *)(ws + sp.off_rho);
     unsigned *maxbits = (unsigned *)(ws + sp.off_max);
-    e = launch_strength(src, p, batch, rho, maxbits, st);
-    ++nl;
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    if (fused) {
+        if (h_stats) e = upload_stats(h_stats, batch, stats, st, &nl);
+        if (e == cudaSuccess) e = launch_prefix_bound(stats, p, batch, maxbits, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "prefix bound");
+    } else {
+        e = launch_strength(src, p, batch, rho, maxbits, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    }
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
         __half *Eyp = (__half *)(ws + sp.off_eyp), *Exp = (__half *)(ws + sp.off_exp), *Rp = (__half *)(ws + sp.off_rp),
@@ -631,9 +687,11 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         ev_begin(ctx, st);
         for (int b0 = 0; b0 < batch; b0 += t.nb) {   // a chunk of items per set of launches, stacked along z
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
-            const float2 *rho_b = (const float2 *)rho + (size_t)b0 * p.nvox;
             std::string err;
-            e = launch_sep_tc_prep(rho_b, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds, ampscale + b0, st);
+            e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags,
+                                                  bounds, ampscale + b0, st)
+                      : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds,
+                                           ampscale + b0, st);
             if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
             if (e == cudaSuccess)
                 e = launch_sep_tc_yz(p, t, Eyp, Hp, ws + sp.off_flags, bounds, nb, d_qx, npx, d_qy, npy,
@@ -667,6 +725,14 @@ int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     return SCATMAN_OK;
 }
 
+extern "C" {
+
+int scatman_simulate_qgrid(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_qx,
+                           int32_t npx, const double *d_qy, int32_t npy, const double *h_quat, int32_t batch,
+                           const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+    return qgrid_impl(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy, h_quat, batch, opts, d_ws, ws_bytes, d_I, cuda_stream, nullptr);
+}
+
 int scatman_shapes_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, int32_t npx, int32_t npy, int32_t batch,
                                          const scatman_options *opts, size_t *bytes) {
     size_t inner = 0;
@@ -687,8 +753,10 @@ int scatman_simulate_shapes_qgrid(scatman_ctx *ctx, const scatman_shape *h_shape
     int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
     if (rc != SCATMAN_OK) return rc;
     const int rendered = ctx->last_launches;
-    rc = scatman_simulate_qgrid(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes,
-                                ws_bytes - dn_bytes, d_I, cuda_stream);
+    std::vector<float> stats;
+    shape_stats(h_shapes, batch, stats);
+    rc = qgrid_impl(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes,
+                    ws_bytes - dn_bytes, d_I, cuda_stream, stats.data());
     if (rc == SCATMAN_OK) ctx->last_launches += rendered;
     return rc;
 }
@@ -698,11 +766,12 @@ struct NufftLayout {
     Plan p;
     NufftPlan n;
     NufftTcPlan tc;      // the GEMM stages on tensor cores (tc.ok) ...
+    bool fused_ok = false;   // as SepPlan::fused_ok
     bool tensor = false; // ... and whether this call uses them (method AUTO / TENSOR) or the FP64 CUDA-core stages (SIMT_TABLE)
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_q = 0, off_tz = 0, off_tx = 0, off_ty = 0,
            off_P = 0, off_H = 0, off_U = 0, total = 0;
     // tensor-core stages: table planes, rho~ planes, H planes, V planes, flags, z-split bounds, per-item scales
-    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0;
+    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0, off_stats = 0;
     size_t hp_bytes = 0;
 };
 // Range of q over the detector (host, FP64, a1's formula): q_x and q_y are monotonic along u and v and extremal in the other
@@ -783,9 +852,11 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
             if (mine) { L.off_txp = a; L.off_typ = b; L.off_tzp = c; }
         }
         const size_t o_rm = take(sizeof(double) * 9 * (size_t)batch), o_bb = take(sizeof(int) * 6 * (size_t)batch),
-                     o_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch), o_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch),
-                     o_max = take(sizeof(unsigned) * (size_t)batch);
-        if (mine) { L.off_rotmat = o_rm; L.off_bbox = o_bb; L.off_rot = o_rot; L.off_rho = o_rho; L.off_max = o_max; }
+                     o_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch),
+                     o_rho = tensor && fused_prefix_pays(p, batch < L.tc.nb ? batch : L.tc.nb)   // see make_sep_plan
+                                 ? o_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch),
+                     o_max = take(sizeof(unsigned) * (size_t)batch), o_st = take(sizeof(unsigned) * 3 * (size_t)batch);
+        if (mine) { L.off_rotmat = o_rm; L.off_bbox = o_bb; L.off_rot = o_rot; L.off_rho = o_rho; L.off_max = o_max; L.off_stats = o_st; L.fused_ok = tensor && o_rho == o_rot; }
         if (!tensor) {
             const size_t a = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx),
                          b = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq),
@@ -827,9 +898,11 @@ int scatman_nufft_grid_dims(scatman_ctx *ctx, const scatman_grid *grid, double l
     return SCATMAN_OK;
 }
 
-int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
-                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
-                           void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+}  // extern "C"
+
+static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                      const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                      void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats) {
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) ||
@@ -863,18 +936,30 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         if (e != cudaSuccess) return cuda_fail(ctx, e, "qmap");
     }
     const float *src = d_dn;
-    if (h_quat && !all_identity(h_quat, batch)) {
+    unsigned *stats = (unsigned *)(ws + L.off_stats), *maxbits = (unsigned *)(ws + L.off_max);
+    const bool oriented = h_quat && !all_identity(h_quat, batch);
+    if (oriented) {
         double *rm = (double *)(ws + L.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
-        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + L.off_rot), (int *)(ws + L.off_bbox), st);
+        if (e == cudaSuccess)
+            e = launch_orient(d_dn, p, rm, batch, (float *)(ws + L.off_rot), (int *)(ws + L.off_bbox), st,
+                              L.fused_ok ? stats : nullptr);
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + L.off_rot);
     }
+    const bool fused = L.fused_ok && (oriented || h_stats);   // see qgrid_impl
     float *rho = (float *)(ws + L.off_rho);
-    e = launch_strength(src, p, batch, rho, (unsigned *)(ws + L.off_max), st);
-    ++nl;
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    if (fused) {
+        if (h_stats) e = upload_stats(h_stats, batch, stats, st, &nl);
+        if (e == cudaSuccess) e = launch_prefix_bound(stats, p, batch, maxbits, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "prefix bound");
+    } else {
+        e = launch_strength(src, p, batch, rho, maxbits, st);
+        ++nl;
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "strength");
+    }
     if (L.tensor) {
         // GEMM stages on tcgen05 (nufft_tensor_kernels.cu): pack -> stage X (the separable route's) -> stage Y -> stage Z -> interpolation
         const NufftTcPlan &t = L.tc;
@@ -894,8 +979,10 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
         for (int b0 = 0; b0 < batch; b0 += t.nb) {
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
             std::string err;
-            e = launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, (const unsigned *)(ws + L.off_max) + b0, p, t.sep, nb, Rp,
-                                   ws + L.off_flags, bounds, ampscale + b0, st, true);
+            e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags,
+                                                  bounds, ampscale + b0, st, true)
+                      : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags, bounds,
+                                           ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero
             SCATMAN_STAGE_CHECK(e, st, "nufft pack");
             if (e == cudaSuccess) e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);
@@ -934,6 +1021,14 @@ int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_gr
     return SCATMAN_OK;
 }
 
+extern "C" {
+
+int scatman_simulate_nufft(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
+                           const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
+                           void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream) {
+    return nufft_impl(ctx, d_dn, grid, lambda, det, h_quat, batch, opts, d_ws, ws_bytes, d_I, cuda_stream, nullptr);
+}
+
 int scatman_shapes_nufft_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, double lambda, const scatman_detector *det,
                                          int32_t batch, size_t *bytes) {
     size_t inner = 0;
@@ -954,8 +1049,10 @@ int scatman_simulate_shapes_nufft(scatman_ctx *ctx, const scatman_shape *h_shape
     int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
     if (rc != SCATMAN_OK) return rc;
     const int rendered = ctx->last_launches;
-    rc = scatman_simulate_nufft(ctx, d_dn, grid, lambda, det, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes,
-                                d_I, cuda_stream);
+    std::vector<float> stats;
+    shape_stats(h_shapes, batch, stats);
+    rc = nufft_impl(ctx, d_dn, grid, lambda, det, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes, d_I, cuda_stream,
+                    stats.data());
     if (rc == SCATMAN_OK) ctx->last_launches += rendered;
     return rc;
 }

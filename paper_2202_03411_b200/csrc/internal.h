@@ -49,7 +49,9 @@ void tensor_schedule(const Plan &p, int num_workers, int *nchunks, int *nzs);
 // ---- kernels launchers (all asynchronous on `st`; return cudaGetLastError()) -------------------
 cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
-                          cudaStream_t st);
+                          cudaStream_t st, unsigned *d_stats = nullptr);   // d_stats[batch][3]: also the extremes of the input, FP32 bits
+// the bound of max |rho~| per item that its extremes {max |delta|, max |beta|, max(0, -beta)} give (p.lambda, dz, nz, rho_mode)
+cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batch, unsigned *d_maxbits, cudaStream_t st);
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
                             cudaStream_t st);
 cudaError_t launch_pack_b(const float *d_rho, const Plan &p, const unsigned *d_maxbits, float *d_ampscale,
@@ -85,6 +87,11 @@ struct SepTcPlan {
 SepTcPlan make_sep_tc_plan(const Plan &p, int npx, int npy, int num_sms);
 cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy, int npy, const Plan &p,
                                  const SepTcPlan &t, __half *d_Exp, __half *d_Eyp, cudaStream_t st);
+// a2 fused with the operand pack: (delta, beta) grids -> FP16 planes of rho~ + flags + per-item scale + z-split bounds; d_maxbits = bounds of
+// max |rho~| per item (launch_prefix_bound).  Replaces launch_strength + launch_sep_tc_prep on the routes that only need the planes.
+cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
+                                      __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
+                                      bool x_only = false);
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
                                bool x_only = false);   // x_only: z-split bounds of stage X only (the NUFFT route)

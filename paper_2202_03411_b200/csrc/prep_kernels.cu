@@ -36,11 +36,36 @@ cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q,
 // initialised by the launcher to {INT_MAX x3, -1 x3}.  One block per (b, z) slice.  The resampling below gathers 8 corners
 // along a slanted line (its cost is cache wavefronts, not bytes); beam-frame voxels that land outside this box are vacuum
 // without looking.
+// Per-item extremes of a grid: stats[b] = {max |delta|, max |beta|, max(0, -beta)} as FP32 bit patterns (non-negative floats order
+// like their bits, so atomicMax works; zeroed by the launcher).  They bound |rho~| BEFORE the prefix runs (prefix_bound_kernel),
+// which lets the separable and NUFFT routes write their FP16 operand planes straight from the prefix kernel.
+struct Extremes {
+    float d = 0.f, b = 0.f, nb = 0.f;
+    __device__ __forceinline__ void see(float delta, float beta) {
+        d = fmaxf(d, fabsf(delta));
+        b = fmaxf(b, fabsf(beta));
+        nb = fmaxf(nb, -beta);
+    }
+    __device__ __forceinline__ void reduce_warp() {   // whole warps call this
+        for (int off = 16; off > 0; off >>= 1) {
+            d = fmaxf(d, __shfl_xor_sync(0xffffffffu, d, off));
+            b = fmaxf(b, __shfl_xor_sync(0xffffffffu, b, off));
+            nb = fmaxf(nb, __shfl_xor_sync(0xffffffffu, nb, off));
+        }
+    }
+    __device__ __forceinline__ void store(unsigned *__restrict__ stats) const {
+        if (d > 0.f) atomicMax(stats + 0, __float_as_uint(d));
+        if (b > 0.f) atomicMax(stats + 1, __float_as_uint(b));
+        if (nb > 0.f) atomicMax(stats + 2, __float_as_uint(nb));
+    }
+};
+
 __global__ void __launch_bounds__(256)
-bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox) {
+bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox, unsigned *__restrict__ stats) {
     const int iz = blockIdx.x % nz, b = blockIdx.x / nz;
     const float2 *src = in + ((size_t)b * nz + iz) * (size_t)nx * ny;
     int x0 = 0x7fffffff, y0 = 0x7fffffff, x1 = -1, y1 = -1;
+    Extremes ex;
     const int n = nx * ny;
     // two voxels per 16-byte load (slices start 16-byte aligned when nx ny is even; the odd case takes the scalar path), four
     // loads in flight per thread: the pass is bound by HBM bandwidth, not by load latency
@@ -60,24 +85,45 @@ bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restri
             for (int u = 0; u < 4; ++u) {
                 if (v[u].x != 0.f || v[u].y != 0.f) seen(2 * (e0 + u * 256));
                 if (v[u].z != 0.f || v[u].w != 0.f) seen(2 * (e0 + u * 256) + 1);
+                ex.see(v[u].x, v[u].y);
+                ex.see(v[u].z, v[u].w);
             }
         }
     } else {
         for (int e = threadIdx.x; e < n; e += 256) {
             const float2 v = __ldg(src + e);
             if (v.x != 0.f || v.y != 0.f) seen(e);
+            ex.see(v.x, v.y);
         }
     }
+    // warp -> block -> one set of atomics per block (a slice's eight warps hitting the same words serialise in L2 otherwise)
     for (int off = 16; off > 0; off >>= 1) {
         x0 = min(x0, __shfl_xor_sync(0xffffffffu, x0, off));
         y0 = min(y0, __shfl_xor_sync(0xffffffffu, y0, off));
         x1 = max(x1, __shfl_xor_sync(0xffffffffu, x1, off));
         y1 = max(y1, __shfl_xor_sync(0xffffffffu, y1, off));
     }
-    if ((threadIdx.x & 31) == 0 && x1 >= 0) {
-        int *o = bbox + 6 * b;
-        atomicMin(o + 0, x0); atomicMin(o + 1, y0); atomicMin(o + 2, iz);
-        atomicMax(o + 3, x1); atomicMax(o + 4, y1); atomicMax(o + 5, iz);
+    ex.reduce_warp();
+    __shared__ int sbox[8][4];
+    __shared__ float sext[8][3];
+    const int warp = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) {
+        sbox[warp][0] = x0; sbox[warp][1] = y0; sbox[warp][2] = x1; sbox[warp][3] = y1;
+        sext[warp][0] = ex.d; sext[warp][1] = ex.b; sext[warp][2] = ex.nb;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) {
+            x0 = min(x0, sbox[w][0]); y0 = min(y0, sbox[w][1]);
+            x1 = max(x1, sbox[w][2]); y1 = max(y1, sbox[w][3]);
+            ex.d = fmaxf(ex.d, sext[w][0]); ex.b = fmaxf(ex.b, sext[w][1]); ex.nb = fmaxf(ex.nb, sext[w][2]);
+        }
+        if (x1 >= 0) {
+            int *o = bbox + 6 * b;
+            atomicMin(o + 0, x0); atomicMin(o + 1, y0); atomicMin(o + 2, iz);
+            atomicMax(o + 3, x1); atomicMax(o + 4, y1); atomicMax(o + 5, iz);
+            if (stats) ex.store(stats + 3 * b);
+        }
     }
 }
 
@@ -119,8 +165,9 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
     const int lx = threadIdx.x & 15, ly = (threadIdx.x >> 4) & 3, lz = threadIdx.x >> 6;
     const int iz = bz * 4 + lz;
     const int wz = min(3, nz - 1 - bz * 4);                         // tile extent - 1 along z
-    const int ntile = nbx * nby;
-    for (int t0 = 0; t0 < ntile; t0 += 256) {
+    // gridDim.y blocks share a layer (single grids: a layer per block leaves most SMs without one)
+    const int ntile = (int)(((long long)nbx * nby * (blockIdx.y + 1)) / gridDim.y);
+    for (int t0 = (int)(((long long)nbx * nby * blockIdx.y) / gridDim.y); t0 < ntile; t0 += 256) {
         {   // phase 1: thread t decides tile t0 + t
             const int t = t0 + threadIdx.x;
             bool h = false;
@@ -215,13 +262,43 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
     }
 }
 
+// maxbits[b] = FP32 bits of an upper bound of max |component of rho~| of item b (without dV): |f(dn)| <= fb from the extremes, and
+// |T_j| = exp(-k dz sum beta) <= exp(k dz nz max(0, -beta)) (1 for absorbing material, beta >= 0).  The bound only sets the FP16
+// operand scale: it may be loose by orders of magnitude without costing accuracy that matters.
+__global__ void prefix_bound_kernel(const unsigned *__restrict__ stats, int batch, int rho_mode, double kdz_nz, unsigned *__restrict__ maxbits) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const double D = (double)__uint_as_float(stats[3 * b]), B = (double)__uint_as_float(stats[3 * b + 1]),
+                 nb = (double)__uint_as_float(stats[3 * b + 2]);
+    double fb = fmax(D, B);
+    if (rho_mode == SCATMAN_RHO_N2M1) fb = fmax(D * (2.0 + D) + B * B, 2.0 * B * (1.0 + D));   // c (2 - c), c = delta + i beta
+    double bound = fb * exp(fmin(kdz_nz * nb, 80.0));
+    if (!(bound < 3.0e38)) bound = 3.0e38;
+    maxbits[b] = __float_as_uint((float)bound);
+}
+
+cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batch, unsigned *d_maxbits, cudaStream_t st) {
+    const double kdz_nz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz * (double)p.nz;
+    prefix_bound_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d_stats, batch, p.rho_mode, kdz_nz, d_maxbits);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
-                          cudaStream_t st) {
+                          cudaStream_t st, unsigned *d_stats) {
+    if (d_stats) {   // extremes of the body-frame grids: the trilinear samples of the beam-frame grid lie within them
+        cudaError_t e = cudaMemsetAsync(d_stats, 0, sizeof(unsigned) * 3 * (size_t)batch, st);
+        if (e != cudaSuccess) return e;
+    }
     const size_t blocks = (size_t)((p.nz + 3) / 4) * batch;     // one block per layer of 16 x 4 x 4 tiles
     if (blocks > 0x7fffffffull || (size_t)p.nz * batch > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     bbox_init_kernel<<<(6 * batch + 255) / 256, 256, 0, st>>>(d_bbox, 6 * batch);
-    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox);
-    orient_kernel<<<(unsigned)blocks, 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
+    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats);
+    // four resident blocks per SM; at least 16 tiles per block
+    const int ntile = ((p.nx + 15) / 16) * ((p.ny + 3) / 4);
+    int nsplit = (int)((4 * 148 + blocks - 1) / blocks);
+    if (nsplit > ntile / 16) nsplit = ntile / 16;
+    if (nsplit < 1) nsplit = 1;
+    orient_kernel<<<dim3((unsigned)blocks, (unsigned)nsplit), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
                                                    make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
                                                    (float2 *)d_out);
     return cudaGetLastError();

@@ -157,6 +157,73 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
     if (any) flags[(size_t)j * (NY / kKB) + y / kKB] = 1;
 }
 
+// Step a2 (Eq. 6/8/9) fused with the pack above: the exclusive z-prefix of strength_kernel (prep_kernels.cu: T_j
+// as a running FP64 product of the per-voxel factors exp(i k dz dn), the factor of the last (delta, beta) seen reused) writes the
+// scaled FP16 planes and the flags directly -- rho~ never goes to memory in FP32.  The scale 2^(13 - e) comes from an upper BOUND of
+// max |rho~| known before the prefix runs (prefix_bound_kernel).  One thread = one column (x, y) of one item, walking z, x fastest:
+// every slice access of a warp is 256 contiguous bytes in and 64 contiguous bytes per plane out; the loads of eight slices are in
+// flight before the (serial) FP64 chain of those slices starts.
+__global__ void __launch_bounds__(128)
+sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz1, int nb, int NY, int NXP, double kdz, int rho_mode,
+                            const unsigned *__restrict__ maxbits, __half *__restrict__ R, unsigned char *__restrict__ flags) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, b = blockIdx.z;
+    if (x >= NXP) return;
+    const float m = __uint_as_float(maxbits[b]);
+    int e = 0;
+    if (m > 0.f) frexpf(m, &e);
+    const float s = ldexpf(1.f, kScaleBExp - e);
+    const size_t plane = (size_t)nb * nz1 * NY * NXP;
+    __half *out = R + ((size_t)b * nz1 * NY + y) * NXP + x;             // + j NY NXP per slice, + plane per plane
+    const size_t ostride = (size_t)NY * NXP;
+    const bool inside = y < ny && x < nx;
+    const float2 *src = dn + (size_t)b * nx * ny * nz1 + (size_t)y * nx + x;
+    const size_t sstride = (size_t)nx * ny;
+    double Tre = 1.0, Tim = 0.0, gre = 1.0, gim = 0.0;
+    float ld = 0.f, lb = 0.f;
+    const int nkb = NY / kKB;
+    for (int j0 = 0; j0 < nz1; j0 += 8) {
+        float2 cin[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            cin[i] = (inside && j0 + i < nz1) ? __ldg(src + (size_t)(j0 + i) * sstride) : make_float2(0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (j0 + i >= nz1) break;
+            const float2 v = cin[i];
+            float2 o = make_float2(0.f, 0.f);
+            if (v.x != 0.f || v.y != 0.f) {
+                const double d = (double)v.x, be = (double)v.y;
+                double fre = d, fim = be;
+                if (rho_mode == SCATMAN_RHO_N2M1) {   // c (2 - c)
+                    fre = d * (2.0 - d) + be * be;
+                    fim = 2.0 * be * (1.0 - d);
+                }
+                o.x = (float)(fre * Tre - fim * Tim);
+                o.y = (float)(fre * Tim + fim * Tre);
+                if (v.x != ld || v.y != lb) {
+                    double sn, co;
+                    sincos(kdz * d, &sn, &co);
+                    const double mag = exp(-kdz * be);
+                    gre = mag * co;
+                    gim = mag * sn;
+                    ld = v.x;
+                    lb = v.y;
+                }
+                const double t = Tre * gre - Tim * gim;
+                Tim = Tre * gim + Tim * gre;
+                Tre = t;
+            }
+            __half h[4];
+            split4(o.x * s, o.y * s, h);
+            __half *dst = out + (size_t)(j0 + i) * ostride;
+#pragma unroll
+            for (int pl = 0; pl < 4; ++pl) dst[pl * plane] = h[pl];
+            if ((o.x != 0.f) | (o.y != 0.f)) flags[((size_t)b * nz1 + j0 + i) * nkb + y / kKB] = 1;
+        }
+    }
+}
+
 // Balanced z splits.  Sequence 0 (stage X): weight of slice j = its live 128-y row tiles; sequence 1 + g (stage YZ, group g):
 // its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
 // every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam:
@@ -885,6 +952,22 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, sep_tc_yzs_kernel, tmA, tmB, P);
+}
+
+cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
+                                      __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
+                                      bool x_only) {
+    const int nyb = t.NY / kKB, nzt = p.nz * nb;
+    cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
+    if (e != cudaSuccess) return e;
+    const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
+    dim3 grid((unsigned)((t.NXP + 127) / 128), (unsigned)t.NY, (unsigned)nb);
+    sep_tc_prefix_planes_kernel<<<grid, 128, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits, d_Rp, d_flags64);
+    sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
+    const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;
+    sep_tc_bounds_kernel<<<x_only ? 1 : 1 + nb * ngs, kBoundsThreads, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, ngs, gw, t.nsx, t.nzs,
+                                                                              d_bounds, d_bounds + (t.nsx + 1));
+    return cudaGetLastError();
 }
 
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,

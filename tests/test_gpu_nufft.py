@@ -135,6 +135,20 @@ def test_grids_beyond_the_tensor_stages_limits_fall_back_to_the_fp64_stages(sm):
         assert l2 <= 1e-6          # both are the FP64 stages
 
 
+def test_gain_medium_and_weak_items_keep_their_accuracy(sm, sim):
+    """The FP16 operand scale of the tensor stages comes from a BOUND of max |rho~| taken before the prefix runs (extremes of
+    (delta, beta), gain factor for beta < 0).  A batch with an amplifying item (beta < 0: |T| grows along z), a strongly absorbing
+    one whose bound is loose by orders of magnitude, and a weak one: every item keeps the parity tolerances."""
+    nx, ny, nz = 70, 50, 24
+    voxel, lam = (2.0, 2.0, 2.0), 10.0
+    g = np.stack([W.random_grid(61, nx, ny, nz, fill=0.5, delta=(-0.01, 0.03), beta=(-0.02, 0.0)),      # gain
+                  W.random_grid(62, nx, ny, nz, fill=0.9, delta=(0.01, 0.05), beta=(0.2, 0.4)),          # opaque after a few slices
+                  W.random_grid(63, nx, ny, nz, fill=0.3, delta=(-1e-6, 1e-6), beta=(0.0, 1e-7))])       # weak
+    I = sim(dev(g), voxel, lam, 21, 18, 30.0).cpu().numpy()
+    for b in range(3):
+        assert_parity(I[b], O.simulate(g[b], voxel, lam, 21, 18, 30.0), what=f"nufft scale bound item {b}")
+
+
 def test_empty_and_single_voxel(sm, sim):
     voxel, lam = (3.0, 3.0, 3.0), 12.0
     z = np.zeros((8, 8, 8, 2), np.float32)

@@ -116,6 +116,20 @@ def test_wide_grids_use_narrower_stage_x_tiles(sm, nx):
     assert_parity(I, ref, what=f"qgrid tensor nx={nx}")
 
 
+@both_methods
+def test_gain_medium_and_weak_items_keep_their_accuracy(sm, method):
+    """As in test_gpu_nufft.py: the tensor stages' FP16 scale comes from a bound of max |rho~| taken before the prefix runs."""
+    nx, ny, nz = 70, 50, 24
+    voxel, lam = (2.0, 2.0, 2.0), 10.0
+    g = np.stack([W.random_grid(61, nx, ny, nz, fill=0.5, delta=(-0.01, 0.03), beta=(-0.02, 0.0)),
+                  W.random_grid(62, nx, ny, nz, fill=0.9, delta=(0.01, 0.05), beta=(0.2, 0.4)),
+                  W.random_grid(63, nx, ny, nz, fill=0.3, delta=(-1e-6, 1e-6), beta=(0.0, 1e-7))])
+    qx, qy = _uniform_q(lam, 30.0, 40), _uniform_q(lam, 25.0, 33)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), method=METHODS[method]).cpu().numpy()
+    for b in range(3):
+        assert_parity(I[b], O.simulate_qgrid(g[b], voxel, lam, qx, qy), what=f"qgrid {method} scale bound item {b}")
+
+
 @pytest.mark.parametrize("ny", [300, 530, 2100])
 def test_tall_grids_use_the_streamed_stage_yz_and_beyond_it_the_cuda_core_stages(sm, ny):
     """N_y > 256: stage YZ streams both operands (odd numbers of 128-row b tiles are padded to pairs); N_y > 2048 falls back to the
