@@ -108,7 +108,7 @@ int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_
                         cudaError_t *err, int *nlaunch);   // 0, or 1 + index of the first bad descriptor
 
 // flat-detector route by a 3-D type-2 NUFFT (nufft_kernels.cu)
-constexpr int kNufftW = 10;                     // Kaiser-Bessel window width in grid cells (oversampling 2)
+constexpr int kNufftW = 8;                      // Kaiser-Bessel window width in grid cells (oversampling 2); R25
 struct NufftAxis { int m_lo = 0, nq = 0; double inv_h = 0; };   // uniform grid g_m = (m_lo + m) h, m = 0..nq-1; inv_h = 1 / h
 struct NufftPlan { NufftAxis ax, ay, az; int nb = 1; double pixel_cells = 0; };   // nb = batch items per chunk
 cudaError_t nufft_init_device();   // once per device (scatman_create): uploads the window's piecewise polynomials

@@ -4,11 +4,11 @@
 // contraction is replaced by
 //   (1) a SEPARABLE transform of rho~ onto a small uniform (g_z, g_y, g_x) grid that covers the q's of the detector with a margin,
 //       U[mz][my][mx] = sum_r c_z c_y c_x rho~(r) e^{i g_m . r}     -- three complex GEMMs (stage Z over slices, X over columns, Y over rows)
-//   (2) an interpolation from that grid to each pixel with a Kaiser-Bessel window of W = 10 grid cells per axis,
+//   (2) an interpolation from that grid to each pixel with a Kaiser-Bessel window of W = 8 grid cells per axis,
 //       A(p) = sum_{m near q(p)/h} phi(u_z - m_z) phi(u_y - m_y) phi(u_x - m_x) U[m],   u = q / h.
 // Grid spacing h_d = 2 pi / (2 N_d d_d) (oversampling 2), pre-correction c_i = 1 / Phi(h x_i) with Phi the window's Fourier transform:
 //   sum_m phi(u - m) e^{i m t} = sum_l Phi(t - 2 pi l) e^{i u (t - 2 pi l)}   (Poisson summation),   |t| = |h x_i| < pi / 2,
-// so the l = 0 term is the wanted e^{i u t} and the l = +-1 aliases are below 3e-9 of it for W = 10, beta = pi sqrt(W^2 (3/4)^2 - 0.8).
+// so the l = 0 term is the wanted e^{i u t} and the l = +-1 aliases are below 2.4e-7 of it for W = 8, beta = pi sqrt(W^2 (3/4)^2 - 0.8).
 // All sums, tables and window weights are FP64 on the CUDA cores (the work is ~3000x smaller than the pixel contraction: 1.2e9 complex MACs for
 // 256^3 on 512^2 pixels against 4.4e12); only U is stored FP32 for the interpolation (see nufft_interp_kernel).  The only approximation beyond
 // rounding is the window's, and the result meets the same tolerances against the oracle's direct sum (tests/test_gpu_nufft.py).

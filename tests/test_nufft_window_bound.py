@@ -1,10 +1,10 @@
 """The error bound DESIGN.md (R25, section 5) states for the NUFFT route's window, checked with numpy / scipy alone (no CUDA, no oracle):
-e^{i u t} = (1 / Phi(t)) sum_m phi(u - m) e^{i m t} up to the aliases, for the Kaiser-Bessel window of 10 cells at oversampling 2
+e^{i u t} = (1 / Phi(t)) sum_m phi(u - m) e^{i m t} up to the aliases, for the Kaiser-Bessel window of 8 cells at oversampling 2
 (|t| <= pi / 2), and the degree-11 per-cell polynomials reproduce the window to 1e-12."""
 import numpy as np
 from scipy.special import i0
 
-W = 10
+W = 8
 HALF = W / 2.0
 BETA = np.pi * np.sqrt(HALF * HALF * 2.25 - 0.8)
 
@@ -31,7 +31,7 @@ def test_window_identity_error_is_below_the_stated_bound():
         m = np.arange(m0, m0 + W)
         approx = np.sum(phi(u - m) * np.exp(1j * m * t)) / Phi(t)
         worst = max(worst, abs(approx - np.exp(1j * u * t)))
-    assert worst <= 5e-9, worst
+    assert worst <= 4e-7, worst   # 2.4e-7 measured; three factors per voxel -> 7e-7 of sum |rho~|, below the 1e-3 per-pixel tolerance at 1e-6 of the peak
 
 
 def test_Phi_is_the_windows_fourier_transform():
