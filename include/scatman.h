@@ -213,6 +213,23 @@ int scatman_discrepancy(scatman_ctx *ctx, const float *d_I, const float *d_M, in
                         int64_t npix, int32_t batch, int32_t metric, void *d_ws, size_t ws_bytes, double *d_out,
                         void *cuda_stream);
 
+/* scatman_discrepancy for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same kernels and the same result, bit for bit, with the scratch in a static device array of
+ * SCATMAN_STATIC_SCRATCH_BYTES inside the library instead of a caller's workspace.  The call allocates nothing, on the host
+ * side of CUDA or the device.  Limits and rules:
+ *   - scatman_fit_workspace_bytes(npix, batch) must not exceed SCATMAN_STATIC_SCRATCH_BYTES (1 MiB: e.g. 256 patterns of up
+ *     to 2.7 M pixels, or 4096 of 128 k); beyond that the call fails with SCATMAN_WORKSPACE_TOO_SMALL and a message naming both
+ *     numbers, and nothing is launched.
+ *   - every GPU that loads the library holds the array until the process exits; ALL calls on a device share it, from any
+ *     context or stream.  It keeps the last call's contents (each call overwrites what it reads: nothing needs clearing), so
+ *     two calls that overlap on the GPU (different streams, or graphs replayed concurrently) race: serialise them.
+ *   - the array's device address is resolved per device in scatman_create (cudaGetSymbolAddress with that device current);
+ *     if that failed, this call returns SCATMAN_CUDA_ERROR with the reason and every other entry point is unaffected.
+ * Arguments as scatman_discrepancy, without d_ws / ws_bytes.  Asynchronous on cuda_stream. */
+#define SCATMAN_STATIC_SCRATCH_BYTES (1u << 20)
+int scatman_discrepancy_static(scatman_ctx *ctx, const float *d_I, const float *d_M, int64_t m_stride, const uint8_t *d_mask,
+                               int64_t npix, int32_t batch, int32_t metric, double *d_out, void *cuda_stream);
+
 /* The Ideal detector ("even a perfect real-life detector is subjected to Poisson statistics of photons";
  * the paper's photon estimate is in its unavailable supplement, so the caller states it, reading R23): d_counts[b][p] =
  * Poisson(h_photons[b] * I[b][p] / sum_p I[b][p]) as FP32 integers, h_photons[batch] = expected detected photons per pattern

@@ -30,7 +30,7 @@ EXPORTS = [
     "scatman_shapes_qgrid_workspace_bytes", "scatman_simulate_shapes_qgrid",
     "scatman_nufft_workspace_bytes", "scatman_nufft_grid_dims", "scatman_simulate_nufft",
     "scatman_shapes_nufft_workspace_bytes", "scatman_simulate_shapes_nufft",
-    "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
+    "scatman_render", "scatman_fit_workspace_bytes", "scatman_discrepancy", "scatman_discrepancy_static", "scatman_ideal_detector", "scatman_last_launch_count", "scatman_last_contraction_ms", "scatman_last_issued_blocks", "scatman_status_string", "scatman_last_error",
     "scatman_version",
 ]
 
@@ -49,6 +49,7 @@ class Options(C.Structure):
     _fields_ = [("rho_mode", C.c_int32), ("method", C.c_int32), ("precision", C.c_int32), ("flags", C.c_uint32)]
 
 
+STATIC_SCRATCH_BYTES = 1 << 20     # SCATMAN_STATIC_SCRATCH_BYTES
 SHAPE_ELLIPSOID, SHAPE_SPHERICAL_HARMONICS, SHAPE_RADIAL_MAP, SHAPE_VOLUME_MAP = range(4)
 
 
@@ -115,6 +116,7 @@ def load_library() -> C.CDLL:
     L.scatman_render.argtypes = [vp, C.POINTER(Shape), i32, C.POINTER(Grid), vp, vp]
     L.scatman_fit_workspace_bytes.argtypes = [vp, i64, i32, C.POINTER(C.c_size_t)]
     L.scatman_discrepancy.argtypes = [vp, vp, vp, i64, vp, i64, i32, i32, vp, C.c_size_t, vp, vp]
+    L.scatman_discrepancy_static.argtypes = [vp, vp, vp, i64, vp, i64, i32, i32, vp, vp]
     L.scatman_ideal_detector.argtypes = [vp, vp, i64, i32, C.POINTER(dbl), C.c_uint64, vp, C.c_size_t, vp, vp]
     L.scatman_last_launch_count.argtypes = [vp, C.POINTER(i32)]
     L.scatman_last_contraction_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -496,6 +498,25 @@ class Scatman:
                                                  C.c_void_p(mask.data_ptr()) if mask is not None else None, npix, batch,
                                                  int(metric), C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(out.data_ptr()),
                                                  self._stream(stream)))
+        return out
+
+    def discrepancy_static(self, I, M, out, mask=None, metric: int = LOSS_L2_NORMALISED, stream=None):
+        """discrepancy() without any allocation: the scratch is the library's static device array of STATIC_SCRATCH_BYTES
+        (scatman_discrepancy_static), `out` (CUDA float64 [B]) is the caller's.  Calls share that array: do not overlap them."""
+        import torch
+        if not (I.is_cuda and I.dtype == torch.float32 and I.is_contiguous() and I.dim() >= 2):
+            raise ValueError("I must be a contiguous CUDA float32 tensor [B][...pixels]")
+        batch, npix = int(I.shape[0]), int(I[0].numel())
+        if not (M.is_cuda and M.dtype == torch.float32 and M.is_contiguous() and M.numel() in (npix, batch * npix)):
+            raise ValueError("M must be a contiguous CUDA float32 tensor with the pixels of one pattern or of every item")
+        if mask is not None and not (mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous() and mask.numel() == npix):
+            raise ValueError("mask must be a contiguous CUDA uint8 tensor with one byte per pixel")
+        if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == batch):
+            raise ValueError("out must be a contiguous CUDA float64 tensor [B]")
+        self._check(self.lib.scatman_discrepancy_static(self._ctx, C.c_void_p(I.data_ptr()), C.c_void_p(M.data_ptr()),
+                                                        0 if M.numel() == npix else npix,
+                                                        C.c_void_p(mask.data_ptr()) if mask is not None else None, npix, batch,
+                                                        int(metric), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
     def ideal_detector(self, I, n_photons, seed: int, out=None, stream=None):

@@ -47,6 +47,10 @@ struct scatman_ctx {
     void *arena = nullptr;
     size_t arena_bytes = 0;
     std::vector<double> host_q;   // qx | qy of the last scatman_simulate_qgrid_host (its tables are valid for these values only)
+    // scatman_discrepancy_static: this device's address of the library's static scratch array (null + the error if it could not
+    // be resolved at set-up; only that entry point minds)
+    double *fit_static = nullptr;
+    cudaError_t fit_static_err = cudaSuccess;
 };
 
 namespace scatman {
@@ -289,6 +293,8 @@ int scatman_create(scatman_ctx **out, int device) {
         delete ctx;
         return SCATMAN_CUDA_ERROR;
     }
+    ctx->fit_static_err = fit_static_scratch(device, &ctx->fit_static);   // `device` is current
+    if (ctx->fit_static_err != cudaSuccess) cudaGetLastError();
     *out = ctx;
     return SCATMAN_OK;
 }
@@ -1079,6 +1085,29 @@ int scatman_discrepancy(scatman_ctx *ctx, const float *d_I, const float *d_M, in
                                        (cudaStream_t)cuda_stream);
     ctx->last_launches = 4;
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "discrepancy");
+}
+
+// The same kernels as scatman_discrepancy on the library's static scratch array: no allocation anywhere on this path.
+int scatman_discrepancy_static(scatman_ctx *ctx, const float *d_I, const float *d_M, int64_t m_stride, const uint8_t *d_mask,
+                               int64_t npix, int32_t batch, int32_t metric, double *d_out, void *cuda_stream) {
+    if (!ctx) return SCATMAN_INVALID_ARGUMENT;
+    if (!d_I || !d_M || !d_out || npix < 1 || batch < 1 || batch > 65535 || (m_stride != 0 && m_stride != npix) ||
+        (metric != SCATMAN_LOSS_L2_NORMALISED && metric != SCATMAN_LOSS_POISSON_DEVIANCE))
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad argument");
+    if ((uintptr_t)d_out & 7) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "d_out must be 8-byte aligned");
+    const size_t need = fit_workspace_bytes(npix, batch);
+    if (need > (size_t)SCATMAN_STATIC_SCRATCH_BYTES)
+        return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL,
+                    "scatman_discrepancy_static: npix = " + std::to_string(npix) + ", batch = " + std::to_string(batch) + " need " +
+                        std::to_string(need) + " bytes of scratch, the static array holds " +
+                        std::to_string((size_t)SCATMAN_STATIC_SCRATCH_BYTES) + " (use scatman_discrepancy with a workspace)");
+    if (!ctx->fit_static)
+        return cuda_fail(ctx, ctx->fit_static_err != cudaSuccess ? ctx->fit_static_err : cudaErrorInvalidSymbol, "static scratch address");
+    cudaSetDevice(ctx->device);
+    // every word of the scratch that is read (partials, sums) is written first by this call's own kernels: nothing to clear
+    cudaError_t e = launch_discrepancy(d_I, d_M, m_stride, d_mask, npix, batch, metric, ctx->fit_static, d_out, (cudaStream_t)cuda_stream);
+    ctx->last_launches = 4;
+    return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "discrepancy (static scratch)");
 }
 
 int scatman_ideal_detector(scatman_ctx *ctx, const float *d_I, int64_t npix, int32_t batch, const double *h_photons,

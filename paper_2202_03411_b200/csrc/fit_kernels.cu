@@ -7,6 +7,8 @@
 //     the counter (pixel lo, pixel hi, item, draw) and the seed as key -- every pixel's draw is independent of the launch shape.
 // HBM-bound: one or two passes over the patterns (4 B per pixel and item, + 4 B for the measured pattern, + 1 B mask),
 // FP64 accumulation (free at this intensity), deterministic two-level sums (per-block partials, summed in index order).
+#include <mutex>
+
 #include "internal.h"
 
 namespace scatman {
@@ -209,6 +211,30 @@ int fit_nchunk(int64_t npix) { return (int)((npix + kFitChunk - 1) / kFitChunk);
 size_t fit_workspace_bytes(int64_t npix, int batch) {
     // partial[b][nchunk][5] + sums[b][5] + partial2[b][nchunk] + photons[b]
     return sizeof(double) * ((size_t)batch * fit_nchunk(npix) * 6 + (size_t)batch * 6);
+}
+
+// ---- static scratch (scatman_discrepancy_static) ----------------------------------------------------------------------
+// The scratch of the discrepancy kernels for callers that cannot allocate: a file-scope device array, held by every GPU
+// that loads the library until the process exits.  In HOST code the name g_fit_static_scratch is a host-side stand-in, not
+// a device address: kernels are handed the address cudaGetSymbolAddress returns for the CURRENT device, resolved once per
+// device (call with that device current) and kept here.
+static __device__ __align__(256) unsigned char g_fit_static_scratch[SCATMAN_STATIC_SCRATCH_BYTES];
+
+cudaError_t fit_static_scratch(int device, double **d_ptr) {
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static double *resolved[kMaxDevices] = {};
+    *d_ptr = nullptr;
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!resolved[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_fit_static_scratch);
+        if (e != cudaSuccess) return e;
+        resolved[device] = (double *)p;
+    }
+    *d_ptr = resolved[device];
+    return cudaSuccess;
 }
 
 cudaError_t launch_fit_sums(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,

@@ -148,6 +148,9 @@ cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_str
                                int batch, int metric, double *d_ws, double *d_out, cudaStream_t st);
 cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, const double *h_photons, uint64_t seed, double *d_ws,
                                   float *d_counts, cudaStream_t st);
+// device address, on `device` (which must be current), of the library's static scratch array (SCATMAN_STATIC_SCRATCH_BYTES;
+// scatman_discrepancy_static): resolved with cudaGetSymbolAddress once per device
+cudaError_t fit_static_scratch(int device, double **d_ptr);
 
 // tensor path: tensor maps are encoded on the host through the driver entry point
 struct TensorMaps;  // opaque here
