@@ -163,12 +163,28 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // max |rho~| known before the prefix runs (prefix_bound_kernel).  One thread = one column (x, y) of one item, walking z, x fastest:
 // every slice access of a warp is 256 contiguous bytes in and 64 contiguous bytes per plane out; the loads of eight slices are in
 // flight before the (serial) FP64 chain of those slices starts.
-__global__ void __launch_bounds__(128)
+constexpr int kPrefThreads = 128, kPrefStages = 3;
+template <int C> struct PrefVec;                       // C columns of (delta, beta) / of one FP16 plane
+template <> struct PrefVec<1> { using In = float2; using Out = unsigned short; };
+template <> struct PrefVec<4> { using In = float4; using Out = uint2; };
+
+// C = 4 columns per thread (two 16-byte copies per slice in, one 8-byte store per plane out; needs even nx) or C = 1 (any nx).
+template <int C>
+__global__ void __launch_bounds__(kPrefThreads, C == 1 ? 8 : 5)
 sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz1, int nb, int NY, int NXP, double kdz, int rho_mode,
                             const unsigned *__restrict__ maxbits, __half *__restrict__ R, unsigned char *__restrict__ flags) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y, b = blockIdx.z;
-    if (x >= NXP) return;
+    // The column's voxels reach the thread through a ring of cp.async stages in shared memory (every thread reads back only what it
+    // copied itself: no barrier, only its own wait_group): two batches of slices are in flight while a third is worked on, and the
+    // loop over the slices of a batch is NOT unrolled -- the unrolled register version (eight inlined FP64 sincos / exp) ran at
+    // 128 registers, four warps per scheduler, and was bound by load latency at 45 % of the HBM rate; one column per thread with
+    // 2-byte stores was then bound by the load/store instruction queue.
+    constexpr int kBatch = C == 1 ? 8 : 3;             // 24 / 36 KB of shared memory: 8 / 5 blocks per SM
+    constexpr int kCopies = C == 1 ? 1 : 2;            // cp.async per slice
+    __shared__ __align__(16) float2 ring[kPrefStages][kBatch][kCopies][kPrefThreads][C / kCopies];
+    const int ncg = NXP / C;                            // column groups of a row (NXP is a multiple of 64)
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int x = (t % ncg) * C, y = t / ncg, b = blockIdx.y;
+    if (y >= NY) return;
     const float m = __uint_as_float(maxbits[b]);
     int e = 0;
     if (m > 0.f) frexpf(m, &e);
@@ -176,50 +192,100 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
     const size_t plane = (size_t)nb * nz1 * NY * NXP;
     __half *out = R + ((size_t)b * nz1 * NY + y) * NXP + x;             // + j NY NXP per slice, + plane per plane
     const size_t ostride = (size_t)NY * NXP;
-    const bool inside = y < ny && x < nx;
-    const float2 *src = dn + (size_t)b * nx * ny * nz1 + (size_t)y * nx + x;
+    const float2 *src = dn + (size_t)b * nx * ny * nz1 + (y < ny ? (size_t)y * nx : 0);
     const size_t sstride = (size_t)nx * ny;
-    double Tre = 1.0, Tim = 0.0, gre = 1.0, gim = 0.0;
-    float ld = 0.f, lb = 0.f;
     const int nkb = NY / kKB;
-    for (int j0 = 0; j0 < nz1; j0 += 8) {
-        float2 cin[8];
+    unsigned char *fl = flags + (size_t)b * nz1 * nkb + y / kKB;
+    const int nbatch = (nz1 + kBatch - 1) / kBatch;
+    auto fetch = [&](int k) {   // batch k -> stage k % kPrefStages; padding columns and slices past the end are zero-filled
+        if (k < nbatch) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
-            cin[i] = (inside && j0 + i < nz1) ? __ldg(src + (size_t)(j0 + i) * sstride) : make_float2(0.f, 0.f);
+            for (int i = 0; i < kBatch; ++i) {
+                const int j = k * kBatch + i;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            if (j0 + i >= nz1) break;
-            const float2 v = cin[i];
-            float2 o = make_float2(0.f, 0.f);
-            if (v.x != 0.f || v.y != 0.f) {
-                const double d = (double)v.x, be = (double)v.y;
-                double fre = d, fim = be;
-                if (rho_mode == SCATMAN_RHO_N2M1) {   // c (2 - c)
-                    fre = d * (2.0 - d) + be * be;
-                    fim = 2.0 * be * (1.0 - d);
+                for (int c = 0; c < kCopies; ++c) {
+                    const int xc = x + c * (C / kCopies);
+                    const bool ok = y < ny && xc < nx && j < nz1;      // (C = 4: nx is even, a pair of columns is in or out as a whole)
+                    const float2 *g = src + (ok ? (size_t)j * sstride + xc : 0);
+                    if (C == 1) ptx::cp_async_8(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
+                    else ptx::cp_async_16(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
                 }
-                o.x = (float)(fre * Tre - fim * Tim);
-                o.y = (float)(fre * Tim + fim * Tre);
-                if (v.x != ld || v.y != lb) {
-                    double sn, co;
-                    sincos(kdz * d, &sn, &co);
-                    const double mag = exp(-kdz * be);
-                    gre = mag * co;
-                    gim = mag * sn;
-                    ld = v.x;
-                    lb = v.y;
-                }
-                const double t = Tre * gre - Tim * gim;
-                Tim = Tre * gim + Tim * gre;
-                Tre = t;
             }
-            __half h[4];
-            split4(o.x * s, o.y * s, h);
-            __half *dst = out + (size_t)(j0 + i) * ostride;
+        }
+        ptx::cp_async_commit();   // (an empty group past the end keeps the wait counts uniform)
+    };
+    fetch(0);
+    fetch(1);
+    double Tre[C], Tim[C], gre[C], gim[C];
+    float ld[C], lb[C];
 #pragma unroll
-            for (int pl = 0; pl < 4; ++pl) dst[pl * plane] = h[pl];
-            if ((o.x != 0.f) | (o.y != 0.f)) flags[((size_t)b * nz1 + j0 + i) * nkb + y / kKB] = 1;
+    for (int c = 0; c < C; ++c) { Tre[c] = 1.0; Tim[c] = 0.0; gre[c] = 1.0; gim[c] = 0.0; ld[c] = lb[c] = 0.f; }
+    for (int k = 0; k < nbatch; ++k) {
+        fetch(k + 2);
+        ptx::cp_async_wait<2>();   // batch k has landed
+        const int jn = min(kBatch, nz1 - k * kBatch);
+        __half *dst = out + (size_t)(k * kBatch) * ostride;
+        float2 v[C], vn[C];
+#pragma unroll
+        for (int c = 0; c < C; ++c) vn[c] = ring[k % kPrefStages][0][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
+#pragma unroll 1
+        for (int i = 0; i < jn; ++i, dst += ostride) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) v[c] = vn[c];
+            if (i + 1 < jn) {   // the next slice's values leave shared memory while this one is worked on
+#pragma unroll
+                for (int c = 0; c < C; ++c) vn[c] = ring[k % kPrefStages][i + 1][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
+            }
+            bool any = false;
+#pragma unroll
+            for (int c = 0; c < C; ++c) any |= (v[c].x != 0.f) | (v[c].y != 0.f);
+            typename PrefVec<C>::Out pk[4];
+#pragma unroll
+            for (int pl = 0; pl < 4; ++pl) pk[pl] = typename PrefVec<C>::Out();
+            if (any) {   // (vacuum: rho~ = 0, T unchanged)
+                __half h[C][4];
+                bool live = false;
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    float ox = 0.f, oy = 0.f;
+                    if (v[c].x != 0.f || v[c].y != 0.f) {
+                        const double d = (double)v[c].x, be = (double)v[c].y;
+                        double fre = d, fim = be;
+                        if (rho_mode == SCATMAN_RHO_N2M1) {   // c (2 - c)
+                            fre = d * (2.0 - d) + be * be;
+                            fim = 2.0 * be * (1.0 - d);
+                        }
+                        ox = (float)(fre * Tre[c] - fim * Tim[c]);
+                        oy = (float)(fre * Tim[c] + fim * Tre[c]);
+                        if (v[c].x != ld[c] || v[c].y != lb[c]) {
+                            double sn, co;
+                            sincos(kdz * d, &sn, &co);
+                            const double mag = exp(-kdz * be);
+                            gre[c] = mag * co;
+                            gim[c] = mag * sn;
+                            ld[c] = v[c].x;
+                            lb[c] = v[c].y;
+                        }
+                        const double t = Tre[c] * gre[c] - Tim[c] * gim[c];
+                        Tim[c] = Tre[c] * gim[c] + Tim[c] * gre[c];
+                        Tre[c] = t;
+                    }
+                    split4(ox * s, oy * s, h[c]);
+                    live |= (ox != 0.f) | (oy != 0.f);
+                }
+#pragma unroll
+                for (int pl = 0; pl < 4; ++pl) {
+                    if constexpr (C == 1) {
+                        pk[pl] = __half_as_ushort(h[0][pl]);
+                    } else {
+                        pk[pl].x = (unsigned)__half_as_ushort(h[0][pl]) | ((unsigned)__half_as_ushort(h[1][pl]) << 16);
+                        pk[pl].y = (unsigned)__half_as_ushort(h[2][pl]) | ((unsigned)__half_as_ushort(h[3][pl]) << 16);
+                    }
+                }
+                if (live) fl[(size_t)(k * kBatch + i) * nkb] = 1;
+            }
+#pragma unroll
+            for (int pl = 0; pl < 4; ++pl) *reinterpret_cast<typename PrefVec<C>::Out *>(dst + pl * plane) = pk[pl];
         }
     }
 }
@@ -961,8 +1027,15 @@ cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxb
     cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
     if (e != cudaSuccess) return e;
     const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
-    dim3 grid((unsigned)((t.NXP + 127) / 128), (unsigned)t.NY, (unsigned)nb);
-    sep_tc_prefix_planes_kernel<<<grid, 128, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits, d_Rp, d_flags64);
+    if (p.nx % 2 == 0) {
+        dim3 grid((unsigned)(((size_t)(t.NXP / 4) * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
+        sep_tc_prefix_planes_kernel<4><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
+                                                                    d_Rp, d_flags64);
+    } else {
+        dim3 grid((unsigned)(((size_t)t.NXP * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
+        sep_tc_prefix_planes_kernel<1><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
+                                                                    d_Rp, d_flags64);
+    }
     sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
     const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;
     sep_tc_bounds_kernel<<<x_only ? 1 : 1 + nb * ngs, kBoundsThreads, 0, st>>>(d_flags64, p.nz, nzt, nyb, t.ng, ngs, gw, t.nsx, t.nzs,
