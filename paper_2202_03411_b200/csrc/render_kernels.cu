@@ -21,6 +21,7 @@ struct RenderArgs {
     double Rt[9];            // row-major R^T: r_body = Rt r_beam
     double a, b, c;          // ellipsoid: 1 / semi-axis
     int ncoef, coef0;        // spherical harmonics: value = sum cn[coef0 + i] P_{l}^{|m|}(cos theta) {1, cos m phi, sin m phi}, i < ncoef
+    int dense_L;             // 4, 6, 8: cn[coef0 ...] holds the dense cos | sin tables of sh_radius_dense<dense_L> instead (0: the triplets)
     double r_lo, r_hi;       // every voxel with |r| < r_lo is inside, with |r| > r_hi outside
     double r2_in, r2_out;    // any kind: |r|^2 < r2_in is inside, |r|^2 > r2_out outside, without rotating (-1 / +inf: no such sphere)
     int nlat, nlon;          // radial map
@@ -80,53 +81,76 @@ __device__ double sh_radius(const RenderArgs &A, const double *__restrict__ Acn,
     return R;
 }
 
-__global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out) {
+// The same sum for harmonics up to degree L <= 8 from DENSE coefficient tables -- cc / cs[p(m, l)] = the cos (or m = 0) and sin
+// coefficients of the pair (l, m >= 0), pairs enumerated m-major (p = 0: (0,0), 1: (1,0) ... L: (L,0), L+1: (1,1) ...), zeros where
+// the shape has no such triplet -- as straight-line code: the loops below unroll completely, the recurrence factors
+// (2l-1)/(l-m), (l+m-1)/(l-m) and (2m-1) are compile-time constants, nothing is indexed by data.  (The walker above spends most of
+// its time in loop control and in loads of l, m from the parameter bank, not in arithmetic: profiles/r02_orient_render.md.)
+template <int L>
+__device__ __forceinline__ double sh_radius_dense(const double *__restrict__ cc, const double *__restrict__ cs, double ct, double st,
+                                                   double cphi, double sphi) {
+    double R = 0.0, pmm = 1.0, cm = 1.0, sm = 0.0;
+    int p = 0;
+#pragma unroll
+    for (int m = 0; m <= L; ++m) {
+        if (m > 0) {
+            pmm = -pmm * (double)(2 * m - 1) * st;
+            const double t = cm * cphi - sm * sphi;
+            sm = sm * cphi + cm * sphi;
+            cm = t;
+        }
+        double pl = pmm, pl_prev = 0.0, S = 0.0, T = 0.0;
+#pragma unroll
+        for (int l = m; l <= L; ++l) {
+            if (l > m) {
+                const double pn = (double)(2 * l - 1) / (double)(l - m) * ct * pl - (double)(l + m - 1) / (double)(l - m) * pl_prev;
+                pl_prev = pl;
+                pl = pn;
+            }
+            S = fma(cc[p], pl, S);
+            if (m > 0) T = fma(cs[p], pl, T);
+            ++p;
+        }
+        R = fma(S, cm, R);
+        if (m > 0) R = fma(T, sm, R);
+    }
+    return R;
+}
+__host__ __device__ constexpr int sh_pairs(int L) { return (L + 1) * (L + 2) / 2; }
+
+// Is the voxel centre (x, y, z) (beam frame) inside shape A?  The full test, after the sphere tests of the caller.
+__device__ bool render_inside(const RenderBatch &Bt, const RenderArgs &A, double x, double y, double z) {
     const double kPi = 3.14159265358979323846;
-    const RenderArgs &A = Bt.a[blockIdx.y];
-    const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const size_t nvox = (size_t)A.nx * A.ny * A.nz;
-    if (v >= nvox) return;
-    out += (size_t)blockIdx.y * nvox;
-    int ix, iy, iz;
-    if (nvox <= 0x7fffffffull) {   // 32-bit divisions (the usual case)
-        const unsigned v32 = (unsigned)v, row = v32 / (unsigned)A.nx;
-        ix = (int)(v32 - row * (unsigned)A.nx);
-        iz = (int)(row / (unsigned)A.ny);
-        iy = (int)(row - (unsigned)iz * (unsigned)A.ny);
-    } else {
-        ix = (int)(v % A.nx); iy = (int)((v / A.nx) % A.ny); iz = (int)(v / ((size_t)A.nx * A.ny));
-    }
-    const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
-    const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
-    const double z = ((double)iz - 0.5 * (double)(A.nz - 1)) * A.dz;
-    // |r| does not change under the rotation: voxels inside the shape's inscribed sphere or outside its circumscribed one are
-    // decided from x^2 + y^2 + z^2 alone (most of a grid); the margins of 1e-12 leave every close call to the full test below,
-    // so the rendering is voxel for voxel what the full test gives.
-    const double r2 = x * x + y * y + z * z;
-    if (r2 > A.r2_out || r2 < A.r2_in) {
-        out[v] = r2 < A.r2_in ? make_float2(A.delta, A.beta) : make_float2(0.f, 0.f);
-        return;
-    }
     const double xb = A.Rt[0] * x + A.Rt[1] * y + A.Rt[2] * z;
     const double yb = A.Rt[3] * x + A.Rt[4] * y + A.Rt[5] * z;
     const double zb = A.Rt[6] * x + A.Rt[7] * y + A.Rt[8] * z;
-    bool inside = false;
     if (A.kind == SCATMAN_SHAPE_ELLIPSOID) {
         const double u = xb * A.a, w = yb * A.b, t = zb * A.c;   // A.a, A.b, A.c hold the reciprocal semi-axes
-        inside = u * u + w * w + t * t <= 1.0;
-    } else if (A.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS) {
-        const double r = sqrt(xb * xb + yb * yb + zb * zb);
-        if (r < A.r_lo) inside = true;
-        else if (r <= A.r_hi) {
-            const double ir = r > 0.0 ? 1.0 / r : 0.0;
-            const double ct = r > 0.0 ? zb * ir : 1.0;
-            const double rho = sqrt(xb * xb + yb * yb);
-            const double irho = rho > 0.0 ? 1.0 / rho : 0.0;
-            const double cphi = rho > 0.0 ? xb * irho : 1.0, sphi = yb * irho;   // phi = atan2(y, x)
-            const double R = sh_radius(A, Bt.cn + A.coef0, Bt.l + A.coef0, Bt.m + A.coef0, ct, cphi, sphi);
-            inside = r <= R;
+        return u * u + w * w + t * t <= 1.0;
+    }
+    if (A.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS) {
+        const double rho2 = xb * xb + yb * yb;
+        const double r = sqrt(rho2 + zb * zb);
+        if (r < A.r_lo) return true;
+        if (r > A.r_hi) return false;
+        const double ir = r > 0.0 ? 1.0 / r : 0.0;
+        const double ct = r > 0.0 ? zb * ir : 1.0;
+        const double rho = sqrt(rho2);
+        const double irho = rho > 0.0 ? 1.0 / rho : 0.0;
+        const double cphi = rho > 0.0 ? xb * irho : 1.0, sphi = yb * irho;   // phi = atan2(y, x)
+        double R;
+        if (A.dense_L > 0) {
+            const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+            const double *cc = Bt.cn + A.coef0;
+            if (A.dense_L == 4) R = sh_radius_dense<4>(cc, cc + sh_pairs(4), ct, st, cphi, sphi);
+            else if (A.dense_L == 6) R = sh_radius_dense<6>(cc, cc + sh_pairs(6), ct, st, cphi, sphi);
+            else R = sh_radius_dense<8>(cc, cc + sh_pairs(8), ct, st, cphi, sphi);
+        } else {
+            R = sh_radius(A, Bt.cn + A.coef0, Bt.l + A.coef0, Bt.m + A.coef0, ct, cphi, sphi);
         }
-    } else if (A.kind == SCATMAN_SHAPE_RADIAL_MAP) {
+        return r <= R;
+    }
+    if (A.kind == SCATMAN_SHAPE_RADIAL_MAP) {
         const double r = sqrt(xb * xb + yb * yb + zb * zb);
         const double sl = r > 0.0 ? fmin(1.0, fmax(-1.0, zb / r)) : 0.0;
         const double lat = asin(sl);
@@ -140,15 +164,53 @@ __global__ void render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__
         const int j0 = (((int)j0f % A.nlon) + A.nlon) % A.nlon, j1 = (j0 + 1) % A.nlon;
         const double lo = A.radii[(size_t)i0 * A.nlon + j0] * (1.0 - tj) + A.radii[(size_t)i0 * A.nlon + j1] * tj;
         const double hi = A.radii[(size_t)i1 * A.nlon + j0] * (1.0 - tj) + A.radii[(size_t)i1 * A.nlon + j1] * tj;
-        inside = r <= lo * (1.0 - ti) + hi * ti;
-    } else {
-        const double fx = xb * A.vdx + 0.5 * (double)A.nvx, fy = yb * A.vdx + 0.5 * (double)A.nvy,
-                     fz = zb * A.vdx + 0.5 * (double)A.nvz;   // A.vdx holds 1 / cell size
-        const double cx = floor(fx), cy = floor(fy), cz = floor(fz);
-        if (cx >= 0.0 && cx < (double)A.nvx && cy >= 0.0 && cy < (double)A.nvy && cz >= 0.0 && cz < (double)A.nvz)
-            inside = A.vol[((size_t)cz * A.nvy + (size_t)cy) * A.nvx + (size_t)cx] != 0;
+        return r <= lo * (1.0 - ti) + hi * ti;
     }
-    out[v] = inside ? make_float2(A.delta, A.beta) : make_float2(0.f, 0.f);
+    const double fx = xb * A.vdx + 0.5 * (double)A.nvx, fy = yb * A.vdx + 0.5 * (double)A.nvy,
+                 fz = zb * A.vdx + 0.5 * (double)A.nvz;   // A.vdx holds 1 / cell size
+    const double cx = floor(fx), cy = floor(fy), cz = floor(fz);
+    if (cx >= 0.0 && cx < (double)A.nvx && cy >= 0.0 && cy < (double)A.nvy && cz >= 0.0 && cz < (double)A.nvz)
+        return A.vol[((size_t)cz * A.nvy + (size_t)cy) * A.nvx + (size_t)cx] != 0;
+    return false;
+}
+
+// A WARP renders a run of up to 128 consecutive x of one row (y, z) of one shape (blockIdx.y): lane i takes x0 + i, x0 + i + 32, ...,
+// so that every store of the warp is 256 contiguous bytes, the row's index arithmetic is done once per four voxels, and a row that
+// misses the shape's circumscribed sphere altogether (most rows of most grids) is zero-filled without looking at its voxels.
+constexpr int kRenderRun = 128;
+__global__ void __launch_bounds__(256)
+render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out) {
+    const RenderArgs &A = Bt.a[blockIdx.y];
+    const int lane = threadIdx.x & 31;
+    const unsigned runs = (unsigned)(A.nx + kRenderRun - 1) / kRenderRun;      // runs per row
+    const unsigned long long w = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // run index
+    const unsigned long long nrows = (unsigned long long)A.ny * A.nz;
+    if (w >= nrows * runs) return;
+    const unsigned row = (unsigned)(w / runs), run = (unsigned)(w - (unsigned long long)row * runs);       // nrows < 2^32 (ny <= 8192, nz <= 65535)
+    const int iz = (int)(row / (unsigned)A.ny), iy = (int)(row - (unsigned)iz * (unsigned)A.ny);
+    const int x0 = (int)run * kRenderRun, x1 = min(A.nx, x0 + kRenderRun);
+    float2 *dst = out + (size_t)blockIdx.y * A.nx * A.ny * A.nz + (size_t)row * A.nx;
+    const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
+    const double z = ((double)iz - 0.5 * (double)(A.nz - 1)) * A.dz;
+    // |r| does not change under the rotation: voxels inside the shape's inscribed sphere or outside its circumscribed one are
+    // decided from x^2 + y^2 + z^2 alone (most of a grid); the margins of 1e-12 leave every close call to the full test,
+    // so the rendering is voxel for voxel what the full test gives.
+    const double yz2 = y * y + z * z;
+    const float2 vac = make_float2(0.f, 0.f), mat = make_float2(A.delta, A.beta);
+    if (yz2 > A.r2_out) {
+        for (int ix = x0 + lane; ix < x1; ix += 32) dst[ix] = vac;
+        return;
+    }
+#pragma unroll 1
+    for (int ix = x0 + lane; ix < x1; ix += 32) {
+        const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
+        const double r2 = x * x + yz2;
+        bool inside;
+        if (r2 > A.r2_out) inside = false;
+        else if (r2 < A.r2_in) inside = true;
+        else inside = render_inside(Bt, A, x, y, z);
+        dst[ix] = inside ? mat : vac;
+    }
 }
 
 cudaError_t render_init_device() {   // per device (scatman_create)
@@ -164,8 +226,25 @@ static double factorial_d(int n) {
     return f;
 }
 
+// Slots of the coefficient pool a harmonics shape takes: the dense tables of sh_radius_dense (degrees <= 8) or its triplets.
+static int sh_dense_degree(const scatman_shape &s) {
+    int lmax = 0;
+    for (int i = 0; i < s.ncoef; ++i) {
+        const double l = s.h_coef[3 * i];
+        if (!(l >= 0.0 && l <= 32.0)) return 0;      // (rejected by fill_render_args)
+        lmax = (int)l > lmax ? (int)l : lmax;
+    }
+    return lmax <= 4 ? 4 : lmax <= 6 ? 6 : lmax <= 8 ? 8 : 0;
+}
+static int sh_pool_need(const scatman_shape &s) {
+    if (s.ncoef < 1 || s.ncoef > kMaxCoef || !s.h_coef) return -1;
+    const int L = sh_dense_degree(s);
+    return L ? 2 * sh_pairs(L) : s.ncoef;
+}
+
 // Fills descriptor A (and, for harmonics, coefficients at coef0 of the pool arrays).  0 ok, 1 bad argument.
-static int fill_render_args(const scatman_shape &s, const scatman_grid &g, RenderArgs &A, double *Acn, signed char *Al, signed char *Am) {
+static int fill_render_args(const scatman_shape &s, const scatman_grid &g, RenderArgs &A, double *Acn_pool, signed char *Al, signed char *Am) {
+    double *Acn = Acn_pool;
     const double kPi = 3.14159265358979323846;
     A = RenderArgs{};
     A.r2_in = -1.0;
@@ -194,6 +273,11 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
             break;
         case SCATMAN_SHAPE_SPHERICAL_HARMONICS: {
             if (s.ncoef < 1 || s.ncoef > kMaxCoef || !s.h_coef) return 1;
+            const int L = sh_dense_degree(s);
+            double tcn[kMaxCoef];
+            signed char tl[kMaxCoef], tm[kMaxCoef];
+            if (L) { Acn = tcn; Al = tl; Am = tm; }   // the triplets are scattered into the dense tables below
+            double *pool_cn = L ? Acn_pool : nullptr;
             // |sum_m c_lm Y_lm| <= sqrt(sum_m c_lm^2) sqrt((2l+1)/4pi) (addition theorem): brackets R around its l = 0 part
             double norm2[33] = {0};
             double r00 = 0.0;
@@ -223,6 +307,16 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
                     std::swap(Am[j], Am[j - 1]);
                     std::swap(Acn[j], Acn[j - 1]);
                 }
+            if (L) {
+                const int np = sh_pairs(L);
+                for (int i = 0; i < 2 * np; ++i) pool_cn[i] = 0.0;
+                for (int i = 0; i < s.ncoef; ++i) {
+                    const int l = Al[i], m = Am[i], am = m < 0 ? -m : m;
+                    const int pi = am * (L + 1) - am * (am - 1) / 2 + (l - am);      // m-major enumeration of the pairs (l, m >= 0)
+                    pool_cn[(m < 0 ? np : 0) + pi] += Acn[i];
+                }
+                A.dense_L = L;
+            }
             A.r_lo = (r00 - bound) * (1.0 - 1e-9) - 1e-300;
             A.r_hi = (r00 + bound) * (1.0 + 1e-9) + 1e-300;
             A.r2_in = A.r_lo > 0.0 ? A.r_lo * A.r_lo * (1.0 - 1e-12) : -1.0;
@@ -258,8 +352,8 @@ int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_
         Bt.n = 0;
         while (b < batch && Bt.n < kBatchShapes) {
             const scatman_shape &s = h_shapes[b];
-            const int nc = s.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS ? s.ncoef : 0;
-            if (nc < 0 || nc > kMaxCoef) return 1 + b;
+            const int nc = s.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS ? sh_pool_need(s) : 0;
+            if (nc < 0) return 1 + b;
             if (pool + nc > kPoolCoef) break;
             if (fill_render_args(s, g, Bt.a[Bt.n], Bt.cn + pool, Bt.l + pool, Bt.m + pool)) return 1 + b;
             Bt.a[Bt.n].coef0 = pool;
@@ -267,7 +361,8 @@ int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_
             ++Bt.n;
             ++b;
         }
-        render_kernel<<<dim3((unsigned)((nvox + 255) / 256), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox);
+        const size_t nruns = (size_t)g.ny * g.nz * ((g.nx + kRenderRun - 1) / kRenderRun);      // one warp each
+        render_kernel<<<dim3((unsigned)((nruns + 7) / 8), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox);
         ++*nlaunch;
         *err = cudaGetLastError();
         if (*err != cudaSuccess) return 0;

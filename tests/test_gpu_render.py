@@ -78,7 +78,14 @@ def test_spherical_harmonics_droplets(sm):
               {"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.01, "quat": quats[0], "coeffs": _droplet_coeffs(rng, 25.0, 4, 0.15)},
               {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "quat": quats[1],
                "coeffs": [(0, 0, 100.0), (8, 5, 30.0), (8, -8, 25.0), (3, -2, 20.0), (5, 0, -15.0)]},
-              {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "quat": quats[2], "coeffs": [(0, 0, 33.0 * sqrt(4 * pi))]}]
+              {"kind": "spherical_harmonics", "delta": 0.01, "beta": 0.0, "quat": quats[2], "coeffs": [(0, 0, 33.0 * sqrt(4 * pi))]},
+              # degrees above 8 take the triplet walker, 5 and 7 the dense tables of the next even degree; a repeated (l, m) adds up
+              {"kind": "spherical_harmonics", "delta": 0.02, "beta": 0.001, "quat": quats[1],
+               "coeffs": [(0, 0, 110.0), (12, 7, 22.0), (10, -3, 18.0), (9, 0, 12.0), (2, 1, -9.0)]},
+              {"kind": "spherical_harmonics", "delta": 0.02, "beta": 0.001, "quat": quats[0],
+               "coeffs": [(0, 0, 105.0), (5, -4, 16.0), (5, 5, -14.0), (1, 0, 6.0), (3, 3, 9.0), (5, -4, 5.0)]},
+              {"kind": "spherical_harmonics", "delta": 0.02, "beta": 0.001, "quat": quats[2],
+               "coeffs": [(0, 0, 105.0), (7, -7, 13.0), (7, 2, -15.0), (6, -1, 11.0), (4, 4, 9.0)]}]
     _check(sm, shapes, (64, 60, 56), (1.6, 1.6, 1.6))
 
 
