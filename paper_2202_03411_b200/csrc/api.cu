@@ -555,7 +555,7 @@ struct SepPlan {
     bool fused_ok = false;   // tensor stages: a chunk is large enough for the fused prefix -> planes pass (fused_prefix_pays)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, off_stats = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, off_stats = 0, off_tilemap = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
                              int num_sms) {
@@ -586,6 +586,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_rho = sp.fused_ok ? sp.off_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
     sp.off_stats = take(sizeof(unsigned) * 3 * (size_t)batch);
+    if (sp.fused_ok) sp.off_tilemap = take(orient_tilemap_bytes(p, batch));   // sparse orientation output (launch_orient)
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
         sp.off_rp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NY * t.NXP);
@@ -656,7 +657,7 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
         if (e == cudaSuccess)
             e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), (int *)(ws + sp.off_bbox), st,
-                              sp.fused_ok ? stats : nullptr);
+                              sp.fused_ok ? stats : nullptr, sp.fused_ok ? ws + sp.off_tilemap : nullptr);
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + sp.off_rot);
@@ -695,7 +696,8 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags,
-                                                  bounds, ampscale + b0, st)
+                                                  bounds, ampscale + b0, st, false,
+                                                  oriented ? ws + sp.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds,
                                            ampscale + b0, st);
             if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
@@ -777,7 +779,7 @@ struct NufftLayout {
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_q = 0, off_tz = 0, off_tx = 0, off_ty = 0,
            off_P = 0, off_H = 0, off_U = 0, total = 0;
     // tensor-core stages: table planes, rho~ planes, H planes, V planes, flags, z-split bounds, per-item scales
-    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0, off_stats = 0;
+    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0, off_stats = 0, off_tilemap = 0;
     size_t hp_bytes = 0;
 };
 // Range of q over the detector (host, FP64, a1's formula): q_x and q_y are monotonic along u and v and extremal in the other
@@ -863,6 +865,10 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
                                  ? o_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch),
                      o_max = take(sizeof(unsigned) * (size_t)batch), o_st = take(sizeof(unsigned) * 3 * (size_t)batch);
         if (mine) { L.off_rotmat = o_rm; L.off_bbox = o_bb; L.off_rot = o_rot; L.off_rho = o_rho; L.off_max = o_max; L.off_stats = o_st; L.fused_ok = tensor && o_rho == o_rot; }
+        {
+            const size_t o_tm = tensor && o_rho == o_rot ? take(orient_tilemap_bytes(p, batch)) : 0;
+            if (mine) L.off_tilemap = o_tm;
+        }
         if (!tensor) {
             const size_t a = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx),
                          b = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * L.n.ax.nq),
@@ -949,7 +955,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
         if (e == cudaSuccess)
             e = launch_orient(d_dn, p, rm, batch, (float *)(ws + L.off_rot), (int *)(ws + L.off_bbox), st,
-                              L.fused_ok ? stats : nullptr);
+                              L.fused_ok ? stats : nullptr, L.fused_ok ? ws + L.off_tilemap : nullptr);
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + L.off_rot);
@@ -986,7 +992,8 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             const int nb = batch - b0 < t.nb ? batch - b0 : t.nb;
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags,
-                                                  bounds, ampscale + b0, st, true)
+                                                  bounds, ampscale + b0, st, true,
+                                                  oriented ? ws + L.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags, bounds,
                                            ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero

@@ -49,7 +49,14 @@ void tensor_schedule(const Plan &p, int num_workers, int *nchunks, int *nzs);
 // ---- kernels launchers (all asynchronous on `st`; return cudaGetLastError()) -------------------
 cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
-                          cudaStream_t st, unsigned *d_stats = nullptr);   // d_stats[batch][3]: also the extremes of the input, FP32 bits
+                          cudaStream_t st, unsigned *d_stats = nullptr,   // d_stats[batch][3]: also the extremes of the input, FP32 bits
+                          unsigned char *d_tilemap = nullptr);
+// d_tilemap = null: d_out is written everywhere.  Else SPARSE output: only the 16 x 4 x 4-voxel tiles that can hold material are
+// written, d_tilemap[b][ceil(nz/4)][ceil(ny/4)][ceil(nx/16)] says which (1) -- the rest of d_out is left as it was and must be read
+// as vacuum (launch_sep_tc_prefix_prep does)
+inline size_t orient_tilemap_bytes(const Plan &p, int batch) {
+    return (size_t)batch * ((p.nz + 3) / 4) * ((p.ny + 3) / 4) * ((p.nx + 15) / 16);
+}
 // the bound of max |rho~| per item that its extremes {max |delta|, max |beta|, max(0, -beta)} give (p.lambda, dz, nz, rho_mode)
 cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batch, unsigned *d_maxbits, cudaStream_t st);
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
@@ -91,7 +98,7 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 // max |rho~| per item (launch_prefix_bound).  Replaces launch_strength + launch_sep_tc_prep on the routes that only need the planes.
 cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                       __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
-                                      bool x_only = false);
+                                      bool x_only = false, const unsigned char *d_tilemap = nullptr);   // d_tilemap: of these nb items (launch_orient)
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
                                bool x_only = false);   // x_only: z-split bounds of stage X only (the NUFFT route)

@@ -134,129 +134,192 @@ __global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
 
 // Output voxels are handled in TILES of 16 x 4 x 4 (256 threads, one voxel each) so that the 2x2x2 source cells of a tile share
 // cache lines for any rotation (row-shaped tiles gather along a slanted line and read 30x more sectors than they use).
-// A block owns one layer of tiles (fixed item b and tile row bz) and walks it: first every thread decides for ONE tile whether it
-// can hold material at all -- the tile's image in the body frame is a parallelepiped whose extent along each body axis follows
-// from three signed edge vectors, compared with the box of non-vacuum voxels widened by the interpolation cell -- then the block
-// zero-fills the tiles that cannot and resamples the others.  (One launch-sized block per tile, each loading the rotation and the
-// box and deciding on its own, was bound by that start-up latency, not by arithmetic or bytes: profiles/r02_orient_render.md.)
+// A block owns one layer of tiles (fixed item b and tile row bz) and walks it in chunks of 256 tiles: first every thread decides
+// for ONE tile whether it can hold material at all -- the tile's image in the body frame is a parallelepiped whose extent along
+// each body axis follows from three signed edge vectors, compared with the box of non-vacuum voxels widened by the interpolation
+// cell -- and leaves the tile's origin in the body frame, its offset in the slice and its extent in shared memory; the live tiles
+// are compacted (ballot); then the block resamples the live tiles -- a voxel's body-frame index is its tile's origin plus a
+// per-thread constant: no index division, no integer -> FP64 conversion (the XU pipe's 4 lanes per scheduler were the limit) --
+// and, for dense output, zero-fills the others with 16-byte stores.
+// tilemap != null: SPARSE output -- the other tiles are not written at all and tilemap[b][bz][tile] says which are (see internal.h).
+// (One launch-sized block per tile, each loading the rotation and the box and deciding on its own, was bound by that start-up
+// latency, not by arithmetic or bytes: profiles/r02_orient_render.md.)
+__device__ __forceinline__ void floor_split(double f, int &i, double &t) {   // f = i + t, i = floor(f), |f| < 2^31: FP64 adds only
+    const double kMagic = 6755399441055744.0;                              // 1.5 * 2^52: f + kMagic holds round(f) in its low word
+    const double r = f + kMagic;
+    double n = r - kMagic;
+    i = __double2loint(r);
+    if (n > f) { n -= 1.0; --i; }
+    t = f - n;
+}
+
 __global__ void __launch_bounds__(256, 4)   // 64 registers: four CTAs per SM (at 100 registers two CTAs left the issue slots half empty)
 orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz, double3 inv,
-              const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out) {
+              const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out, unsigned char *__restrict__ tilemap) {
     const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
     const int bz = blockIdx.x % nbz, b = blockIdx.x / nbz;
     __shared__ double sR[9];
     __shared__ int sbb[6];
+    __shared__ double sbd[6];              // the box of non-vacuum voxels widened by one cell: lo - 1 (x, y, z), hi + 1
+    __shared__ double tile_f[256][3];      // body-frame index of the tile's first voxel
+    __shared__ int tile_off[256];          // offset of that voxel in its slice
+    __shared__ unsigned char tile_ext[256];   // (extent - 1) of the tile along x | along y << 4 (ragged edges)
     __shared__ unsigned char hit[256];
+    __shared__ unsigned short live[256];   // the chunk's tiles that can hold material, in order
+    __shared__ int wcount[8];
     if (threadIdx.x < 9) sR[threadIdx.x] = rotmat[9 * b + threadIdx.x];
-    if (threadIdx.x >= 32 && threadIdx.x < 38) sbb[threadIdx.x - 32] = bbox[6 * b + threadIdx.x - 32];
+    if (threadIdx.x >= 32 && threadIdx.x < 38) {
+        const int k = threadIdx.x - 32, v = bbox[6 * b + k];
+        sbb[k] = v;
+        sbd[k] = (double)(k < 3 ? v - 1 : v + 1);
+    }
     __syncthreads();
     const double *R = sR;
-    // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = origin + ix ex + iy ey + iz ez (one row of R^T per axis)
-    const double ex[3] = {R[0] * dx * inv.x, R[1] * dx * inv.y, R[2] * dx * inv.z};
-    const double ey[3] = {R[3] * dy * inv.x, R[4] * dy * inv.y, R[5] * dy * inv.z};
-    const double ez[3] = {R[6] * dz * inv.x, R[7] * dz * inv.y, R[8] * dz * inv.z};
-    const double xb0 = centre(0, nx, dx), yb0 = centre(0, ny, dy), zb0 = centre(0, nz, dz);
-    const double org[3] = {(R[0] * xb0 + R[3] * yb0 + R[6] * zb0) * inv.x + 0.5 * (double)(nx - 1),
-                           (R[1] * xb0 + R[4] * yb0 + R[7] * zb0) * inv.y + 0.5 * (double)(ny - 1),
-                           (R[2] * xb0 + R[5] * yb0 + R[8] * zb0) * inv.z + 0.5 * (double)(nz - 1)};
-    const int n3[3] = {nx, ny, nz};
-    const float2 *src = in + (size_t)b * nx * ny * nz;
-    float2 *dstb = out + (size_t)b * nx * ny * nz;
+    // fractional body-frame index of beam-frame voxel (ix, iy, iz): f = origin + ix ex + iy ey + iz ez (one row of R^T per axis);
+    // kept in shared memory (the registers go to the resampling loop)
+    __shared__ double sE[12];              // ex[3], ey[3], ez[3], origin[3]
+    if (threadIdx.x < 9) {
+        const int row = threadIdx.x / 3, d = threadIdx.x % 3;
+        sE[threadIdx.x] = R[threadIdx.x] * (row == 0 ? dx : row == 1 ? dy : dz) * (d == 0 ? inv.x : d == 1 ? inv.y : inv.z);
+    } else if (threadIdx.x < 12) {
+        const int d = threadIdx.x - 9;
+        const double xb0 = centre(0, nx, dx), yb0 = centre(0, ny, dy), zb0 = centre(0, nz, dz);
+        sE[threadIdx.x] = (R[d] * xb0 + R[3 + d] * yb0 + R[6 + d] * zb0) * (d == 0 ? inv.x : d == 1 ? inv.y : inv.z) +
+                          0.5 * (double)((d == 0 ? nx : d == 1 ? ny : nz) - 1);
+    }
+    __syncthreads();
+    const double *ex = sE, *ey = sE + 3, *ez = sE + 6;
     const int lx = threadIdx.x & 15, ly = (threadIdx.x >> 4) & 3, lz = threadIdx.x >> 6;
     const int iz = bz * 4 + lz;
     const int wz = min(3, nz - 1 - bz * 4);                         // tile extent - 1 along z
+    const bool empty = sbb[3] < 0;                                  // an all-vacuum item
+    const float2 *src = in + (size_t)b * nx * ny * nz;
+    float2 *dstb = out + (size_t)b * nx * ny * nz;
+    float2 *dstt = dstb + ((size_t)iz * ny + ly) * nx + lx;         // + tile_off
+    // this thread's voxel relative to its tile's first one, in body-frame index units
+    const double lo0 = (double)lx * ex[0] + (double)ly * ey[0] + (double)lz * ez[0];
+    const double lo1 = (double)lx * ex[1] + (double)ly * ey[1] + (double)lz * ez[1];
+    const double lo2 = (double)lx * ex[2] + (double)ly * ey[2] + (double)lz * ez[2];
     // gridDim.y blocks share a layer (single grids: a layer per block leaves most SMs without one)
     const int ntile = (int)(((long long)nbx * nby * (blockIdx.y + 1)) / gridDim.y);
     for (int t0 = (int)(((long long)nbx * nby * blockIdx.y) / gridDim.y); t0 < ntile; t0 += 256) {
+        int nlive;
         {   // phase 1: thread t decides tile t0 + t
             const int t = t0 + threadIdx.x;
             bool h = false;
             if (t < ntile) {
                 const int bx = t % nbx, by = t / nbx;
                 const int wx = min(15, nx - 1 - bx * 16), wy = min(3, ny - 1 - by * 4);
-                h = true;
+                h = !empty;
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
-                    const double f0 = org[d] + (double)(bx * 16) * ex[d] + (double)(by * 4) * ey[d] + (double)(bz * 4) * ez[d];
+                    const double f0 = sE[9 + d] + (double)(bx * 16) * ex[d] + (double)(by * 4) * ey[d] + (double)(bz * 4) * ez[d];
+                    tile_f[threadIdx.x][d] = f0;
                     const double sx = (double)wx * ex[d], sy = (double)wy * ey[d], sz = (double)wz * ez[d];
                     const double lo = f0 + fmin(sx, 0.0) + fmin(sy, 0.0) + fmin(sz, 0.0);
                     const double hi = f0 + fmax(sx, 0.0) + fmax(sy, 0.0) + fmax(sz, 0.0);
                     // the per-voxel test below is f > bb_lo - 1 && f < bb_hi + 1; a slack of 1e-9 voxels covers the rounding of this
                     // bound against the per-voxel evaluation (a wrongly kept tile only costs time)
-                    if (hi <= (double)(sbb[d] - 1) - 1e-9 || lo >= (double)(sbb[3 + d] + 1) + 1e-9 || sbb[3 + d] < 0) h = false;
+                    if (hi <= sbd[d] - 1e-9 || lo >= sbd[3 + d] + 1e-9) h = false;
                 }
-                (void)n3;
+                tile_off[threadIdx.x] = by * 4 * nx + bx * 16;
+                tile_ext[threadIdx.x] = (unsigned char)(wx | (wy << 4));
+                if (tilemap) tilemap[((size_t)b * nbz + bz) * ((size_t)nbx * nby) + t] = h ? 1 : 0;
             }
             hit[threadIdx.x] = h ? 1 : 0;
+            // compact the live tiles (ballot + warp counts): the resampling loop below visits only those
+            const unsigned bal = __ballot_sync(0xffffffffu, h);
+            if ((threadIdx.x & 31) == 0) wcount[threadIdx.x >> 5] = __popc(bal);
+            __syncthreads();
+            int before = 0, total = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) {
+                before += w < (int)(threadIdx.x >> 5) ? wcount[w] : 0;
+                total += wcount[w];
+            }
+            if (h) live[before + __popc(bal & ((1u << (threadIdx.x & 31)) - 1u))] = (unsigned short)threadIdx.x;
+            nlive = total;
         }
         __syncthreads();
-        const int tend = min(256, ntile - t0);
-        for (int tt = 0; tt < tend; ++tt) {
-            const int t = t0 + tt;
-            const int bx = t % nbx, by = t / nbx;
-            const int ix = bx * 16 + lx, iy = by * 4 + ly;
-            if (ix >= nx || iy >= ny || iz >= nz) continue;
-            float2 *dst = dstb + ((size_t)iz * ny + iy) * nx;
-            if (!hit[tt]) {
-                dst[ix] = make_float2(0.f, 0.f);
-                continue;
-            }
-            const double fx = org[0] + (double)ix * ex[0] + (double)iy * ey[0] + (double)iz * ez[0];
-            const double fy = org[1] + (double)ix * ex[1] + (double)iy * ey[1] + (double)iz * ez[1];
-            const double fz = org[2] + (double)ix * ex[2] + (double)iy * ey[2] + (double)iz * ez[2];
-            float2 o = make_float2(0.f, 0.f);
-            // the 2x2x2 cell holds material only if every coordinate lies within one voxel of the box of non-vacuum voxels
-            if (fx > (double)(sbb[0] - 1) && fx < (double)(sbb[3] + 1) && fy > (double)(sbb[1] - 1) && fy < (double)(sbb[4] + 1) &&
-                fz > (double)(sbb[2] - 1) && fz < (double)(sbb[5] + 1)) {
-                const double flx = floor(fx), fly = floor(fy), flz = floor(fz);
-                const int x0 = (int)flx, y0 = (int)fly, z0 = (int)flz;
-                // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
-                // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
-                // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
-                bool done = false;
-                if (x0 >= 0 && y0 >= 0 && z0 >= 0 && x0 + 1 < nx && y0 + 1 < ny && z0 + 1 < nz) {
-                    const float2 *c0 = src + ((size_t)z0 * ny + y0) * nx + x0;
-                    const size_t sy = (size_t)nx, sz = (size_t)nx * ny;
-                    const float2 v000 = __ldg(c0), v001 = __ldg(c0 + 1), v010 = __ldg(c0 + sy), v011 = __ldg(c0 + sy + 1);
-                    const float2 v100 = __ldg(c0 + sz), v101 = __ldg(c0 + sz + 1), v110 = __ldg(c0 + sz + sy), v111 = __ldg(c0 + sz + sy + 1);
-                    const bool same = v001.x == v000.x && v001.y == v000.y && v010.x == v000.x && v010.y == v000.y && v011.x == v000.x &&
-                                      v011.y == v000.y && v100.x == v000.x && v100.y == v000.y && v101.x == v000.x && v101.y == v000.y &&
-                                      v110.x == v000.x && v110.y == v000.y && v111.x == v000.x && v111.y == v000.y;
-                    if (same) {
-                        o = v000;
-                        done = true;
-                    }
+        if (!tilemap) {
+            // dense output: zero-fill the tiles that cannot hold material, a 128-byte tile row per 8 threads (16-byte stores when
+            // the rows are 16-byte aligned, i.e. nx is even)
+            const int tend = min(256, ntile - t0);
+            for (int e = threadIdx.x; e < tend * 128; e += 256) {
+                const int tt = e >> 7, r = (e >> 3) & 15, c = e & 7;       // tile, row of the tile (ly + 4 lz), 2-voxel chunk
+                if (hit[tt]) continue;
+                const int ext = tile_ext[tt];
+                const int cx = 2 * c, cy = r & 3, izr = bz * 4 + (r >> 2);
+                if (cx > (ext & 15) || cy > (ext >> 4) || izr >= nz) continue;
+                float2 *d2 = dstb + ((size_t)izr * ny + cy) * nx + tile_off[tt] + cx;
+                if ((nx & 1) == 0) *reinterpret_cast<float4 *>(d2) = make_float4(0.f, 0.f, 0.f, 0.f);
+                else {
+                    d2[0] = make_float2(0.f, 0.f);
+                    if (cx + 1 <= (ext & 15)) d2[1] = make_float2(0.f, 0.f);
                 }
-                if (!done) {
-                    const double tx = fx - flx, ty = fy - fly, tz = fz - flz;
-                    const double wxx[2] = {1.0 - tx, tx}, wyy[2] = {1.0 - ty, ty}, wzz[2] = {1.0 - tz, tz};
-                    double are = 0.0, aim = 0.0;
-#pragma unroll
-                    for (int cz = 0; cz < 2; ++cz) {
-                        const int zi = z0 + cz;
-                        if (zi < 0 || zi >= nz) continue;
-#pragma unroll
-                        for (int cy = 0; cy < 2; ++cy) {
-                            const int yi = y0 + cy;
-                            if (yi < 0 || yi >= ny) continue;
-                            const double wyz = wyy[cy] * wzz[cz];
-                            const float2 *row = src + ((size_t)zi * ny + yi) * nx;
-#pragma unroll
-                            for (int cx = 0; cx < 2; ++cx) {
-                                const int xi = x0 + cx;
-                                if (xi < 0 || xi >= nx) continue;
-                                const float2 v = __ldg(row + xi);
-                                if (v.x == 0.f && v.y == 0.f) continue;   // most of a grid is vacuum: skip the FP64 conversions
-                                const double w = wxx[cx] * wyz;
-                                are = fma(w, (double)v.x, are);
-                                aim = fma(w, (double)v.y, aim);
-                            }
+            }
+        }
+        if (iz < nz) {
+            for (int li = 0; li < nlive; ++li) {
+                const int tt = live[li];
+                const int ext = tile_ext[tt];
+                if (lx > (ext & 15) || ly > (ext >> 4)) continue;
+                const double fx = tile_f[tt][0] + lo0, fy = tile_f[tt][1] + lo1, fz = tile_f[tt][2] + lo2;
+                float2 o = make_float2(0.f, 0.f);
+                // the 2x2x2 cell holds material only if every coordinate lies within one voxel of the box of non-vacuum voxels
+                if (fx > sbd[0] && fx < sbd[3] && fy > sbd[1] && fy < sbd[4] && fz > sbd[2] && fz < sbd[5]) {
+                    int x0, y0, z0;
+                    double tx, ty, tz;
+                    floor_split(fx, x0, tx);
+                    floor_split(fy, y0, ty);
+                    floor_split(fz, z0, tz);
+                    // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
+                    // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
+                    // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
+                    bool done = false;
+                    if (x0 >= 0 && y0 >= 0 && z0 >= 0 && x0 + 1 < nx && y0 + 1 < ny && z0 + 1 < nz) {
+                        const float2 *c0 = src + ((size_t)z0 * ny + y0) * nx + x0;
+                        const size_t sy = (size_t)nx, sz = (size_t)nx * ny;
+                        const float2 v000 = __ldg(c0), v001 = __ldg(c0 + 1), v010 = __ldg(c0 + sy), v011 = __ldg(c0 + sy + 1);
+                        const float2 v100 = __ldg(c0 + sz), v101 = __ldg(c0 + sz + 1), v110 = __ldg(c0 + sz + sy), v111 = __ldg(c0 + sz + sy + 1);
+                        const bool same = v001.x == v000.x && v001.y == v000.y && v010.x == v000.x && v010.y == v000.y && v011.x == v000.x &&
+                                          v011.y == v000.y && v100.x == v000.x && v100.y == v000.y && v101.x == v000.x && v101.y == v000.y &&
+                                          v110.x == v000.x && v110.y == v000.y && v111.x == v000.x && v111.y == v000.y;
+                        if (same) {
+                            o = v000;
+                            done = true;
                         }
                     }
-                    o = make_float2((float)are, (float)aim);
+                    if (!done) {
+                        const double wxx[2] = {1.0 - tx, tx}, wyy[2] = {1.0 - ty, ty}, wzz[2] = {1.0 - tz, tz};
+                        double are = 0.0, aim = 0.0;
+#pragma unroll
+                        for (int cz = 0; cz < 2; ++cz) {
+                            const int zi = z0 + cz;
+                            if (zi < 0 || zi >= nz) continue;
+#pragma unroll
+                            for (int cy = 0; cy < 2; ++cy) {
+                                const int yi = y0 + cy;
+                                if (yi < 0 || yi >= ny) continue;
+                                const double wyz = wyy[cy] * wzz[cz];
+                                const float2 *row = src + ((size_t)zi * ny + yi) * nx;
+#pragma unroll
+                                for (int cx = 0; cx < 2; ++cx) {
+                                    const int xi = x0 + cx;
+                                    if (xi < 0 || xi >= nx) continue;
+                                    const float2 v = __ldg(row + xi);
+                                    if (v.x == 0.f && v.y == 0.f) continue;   // most of a grid is vacuum: skip the FP64 conversions
+                                    const double w = wxx[cx] * wyz;
+                                    are = fma(w, (double)v.x, are);
+                                    aim = fma(w, (double)v.y, aim);
+                                }
+                            }
+                        }
+                        o = make_float2((float)are, (float)aim);
+                    }
                 }
+                dstt[tile_off[tt]] = o;
             }
-            dst[ix] = o;
         }
         __syncthreads();
     }
@@ -284,7 +347,7 @@ cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batc
 }
 
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
-                          cudaStream_t st, unsigned *d_stats) {
+                          cudaStream_t st, unsigned *d_stats, unsigned char *d_tilemap) {
     if (d_stats) {   // extremes of the body-frame grids: the trilinear samples of the beam-frame grid lie within them
         cudaError_t e = cudaMemsetAsync(d_stats, 0, sizeof(unsigned) * 3 * (size_t)batch, st);
         if (e != cudaSuccess) return e;
@@ -300,7 +363,7 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
     if (nsplit < 1) nsplit = 1;
     orient_kernel<<<dim3((unsigned)blocks, (unsigned)nsplit), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
                                                    make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
-                                                   (float2 *)d_out);
+                                                   (float2 *)d_out, d_tilemap);
     return cudaGetLastError();
 }
 

@@ -172,7 +172,8 @@ template <> struct PrefVec<4> { using In = float4; using Out = uint2; };
 template <int C>
 __global__ void __launch_bounds__(kPrefThreads, C == 1 ? 8 : 5)
 sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz1, int nb, int NY, int NXP, double kdz, int rho_mode,
-                            const unsigned *__restrict__ maxbits, __half *__restrict__ R, unsigned char *__restrict__ flags) {
+                            const unsigned *__restrict__ maxbits, __half *__restrict__ R, unsigned char *__restrict__ flags,
+                            const unsigned char *__restrict__ tilemap) {
     // The column's voxels reach the thread through a ring of cp.async stages in shared memory (every thread reads back only what it
     // copied itself: no barrier, only its own wait_group): two batches of slices are in flight while a third is worked on, and the
     // loop over the slices of a batch is NOT unrolled -- the unrolled register version (eight inlined FP64 sincos / exp) ran at
@@ -197,15 +198,34 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
     const int nkb = NY / kKB;
     unsigned char *fl = flags + (size_t)b * nz1 * nkb + y / kKB;
     const int nbatch = (nz1 + kBatch - 1) / kBatch;
+    // Sparse input (launch_orient with a tile map): tiles of 16 x 4 x 4 voxels that were not written are vacuum and are not read --
+    // the copy is issued with source size 0, which zero-fills.  The thread's C columns lie in one tile column; the map byte of the
+    // layer after the one being fetched is already in flight.
+    const unsigned char *tm = nullptr;
+    size_t tm_stride = 0;
+    int tm_layer = -1, tm_layers = 0;
+    unsigned char tm_cur = 1, tm_next = 1;
+    if (tilemap && y < ny && x < nx) {
+        const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4;
+        tm_layers = (nz1 + 3) / 4;
+        tm_stride = (size_t)nbx * nby;
+        tm = tilemap + (size_t)b * tm_layers * tm_stride + (size_t)(y >> 2) * nbx + (x >> 4);
+        tm_next = __ldg(tm);
+    }
     auto fetch = [&](int k) {   // batch k -> stage k % kPrefStages; padding columns and slices past the end are zero-filled
         if (k < nbatch) {
 #pragma unroll
             for (int i = 0; i < kBatch; ++i) {
                 const int j = k * kBatch + i;
+                if (tm && (j >> 2) != tm_layer && j < nz1) {
+                    tm_layer = j >> 2;
+                    tm_cur = tm_next;
+                    if (tm_layer + 1 < tm_layers) tm_next = __ldg(tm + (size_t)(tm_layer + 1) * tm_stride);
+                }
 #pragma unroll
                 for (int c = 0; c < kCopies; ++c) {
                     const int xc = x + c * (C / kCopies);
-                    const bool ok = y < ny && xc < nx && j < nz1;      // (C = 4: nx is even, a pair of columns is in or out as a whole)
+                    const bool ok = y < ny && xc < nx && j < nz1 && tm_cur;      // (C = 4: nx is even, a pair of columns is in or out as a whole)
                     const float2 *g = src + (ok ? (size_t)j * sstride + xc : 0);
                     if (C == 1) ptx::cp_async_8(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
                     else ptx::cp_async_16(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
@@ -1022,7 +1042,7 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 
 cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                       __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
-                                      bool x_only) {
+                                      bool x_only, const unsigned char *d_tilemap) {
     const int nyb = t.NY / kKB, nzt = p.nz * nb;
     cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
     if (e != cudaSuccess) return e;
@@ -1030,11 +1050,11 @@ cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxb
     if (p.nx % 2 == 0) {
         dim3 grid((unsigned)(((size_t)(t.NXP / 4) * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
         sep_tc_prefix_planes_kernel<4><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
-                                                                    d_Rp, d_flags64);
+                                                                    d_Rp, d_flags64, d_tilemap);
     } else {
         dim3 grid((unsigned)(((size_t)t.NXP * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
         sep_tc_prefix_planes_kernel<1><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
-                                                                    d_Rp, d_flags64);
+                                                                    d_Rp, d_flags64, d_tilemap);
     }
     sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
     const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;
