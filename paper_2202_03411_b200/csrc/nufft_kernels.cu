@@ -215,7 +215,7 @@ __device__ inline double placed(const double (&own)[kW], int shift, int a) {
 }
 
 constexpr int kInterpThreads = 128;
-constexpr int kTX = 8, kTY = 16;         // a block = 8 groups of P pixels along a detector row x 16 rows
+constexpr int kTX = 16, kTY = 8;         // a block = 16 pixels along a detector row x 8 groups of P rows
 constexpr int kTileCap = 3968;           // float2 elements of shared memory for the block's window of U (31 KB: with the 24 KB of weights
                                          // and the 1 KB the driver reserves per block, four blocks fit an SM)
 
@@ -233,17 +233,20 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     extern __shared__ float wsm[];                        // [2][P][KU][kInterpThreads] y and z weights (FP32), then the tile of U
     float2 *tile = reinterpret_cast<float2 *>(wsm + 2 * P * KU * kInterpThreads);
     __shared__ int red[8];                                // lo[3], hi[3], every thread's pixels share a window, any valid thread
-    const int ngx = (npx + P - 1) / P;
-    const int tiles_x = (ngx + kTX - 1) / kTX;
-    const int gx = (blockIdx.x % tiles_x) * kTX + (threadIdx.x % kTX), iy = (blockIdx.x / tiles_x) * kTY + threadIdx.x / kTX;
-    const bool valid = gx < ngx && iy < npy;
-    const int ix0 = gx * P;
-    const int64_t p0 = (int64_t)iy * npx + ix0;
+    // A thread's P pixels are neighbours along y (same column ix), a half-warp = 16 consecutive ix of one row group: at the usual
+    // pixel spacing (< 1 grid cell) its 16 lanes then read one run of <= 16 cells of a tile row per load -- one shared-memory
+    // wavefront.  (P pixels along x and 8 x 4 thread groups per warp cost 3 wavefronts per load: the kernel's limit.)
+    const int ngy = (npy + P - 1) / P;
+    const int tiles_x = (npx + kTX - 1) / kTX;
+    const int ix = (blockIdx.x % tiles_x) * kTX + (threadIdx.x % kTX), gy = (blockIdx.x / tiles_x) * kTY + threadIdx.x / kTX;
+    const bool valid = ix < npx && gy < ngy;
+    const int iy0 = gy * P;
+    const int64_t p0 = (int64_t)iy0 * npx + ix;     // pixel j of the thread: p0 + j npx
     const int64_t npix = (int64_t)npx * npy;
     U += (int64_t)blockIdx.y * strideU;
     I += (int64_t)blockIdx.y * npix;
     if (ampscale) dV *= (double)__ldg(ampscale + blockIdx.y);   // tensor-core stages: U carries the item's operand scales
-    const int np = valid ? (npx - ix0 < P ? npx - ix0 : P) : 0;
+    const int np = valid ? (npy - iy0 < P ? npy - iy0 : P) : 0;
     double u[P][3];
     int m0[P][3], base[3], top[3];
     if (threadIdx.x == 0) {
@@ -254,7 +257,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < P; ++j) {
-        const int64_t p = valid ? p0 + (j < np ? j : 0) : 0;     // threads past the detector's edge look at pixel 0 and stay out of the sums
+        const int64_t p = valid ? p0 + (int64_t)(j < np ? j : 0) * npx : 0;     // threads past the detector's edge look at pixel 0 and stay out of the sums
         u[j][0] = q[3 * p + 0] * ax.inv_h; u[j][1] = q[3 * p + 1] * ay.inv_h; u[j][2] = q[3 * p + 2] * az.inv_h;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -370,7 +373,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
         for (int j = 0; j < P; ++j)
             if (j < np) {
                 const double re = are[j] * dV, im = aim[j] * dV;
-                I[p0 + j] = (float)(re * re + im * im);
+                I[p0 + (int64_t)j * npx] = (float)(re * re + im * im);
             }
         return;
     }
@@ -410,7 +413,7 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
         }
         are *= dV;
         aim *= dV;
-        I[p0 + j] = (float)(are * are + aim * aim);
+        I[p0 + (int64_t)j * npx] = (float)(are * are + aim * aim);
     }
 }
 
@@ -419,7 +422,7 @@ cudaError_t launch_interp(const double *d_q, int npx, int npy, const NufftPlan &
                           double dV, const float *d_ampscale, float *d_I, cudaStream_t st) {
     constexpr int KU = P > 1 ? kW + 2 : kW;
     const size_t smem = sizeof(float) * 2 * P * KU * kInterpThreads + sizeof(float2) * kTileCap;
-    const int64_t tiles = (int64_t)(((npx + P - 1) / P + kTX - 1) / kTX) * ((npy + kTY - 1) / kTY);
+    const int64_t tiles = (int64_t)((npx + kTX - 1) / kTX) * (((npy + P - 1) / P + kTY - 1) / kTY);
     dim3 grid((unsigned)tiles, nb);
     nufft_interp_kernel<P><<<grid, kInterpThreads, smem, st>>>(d_q, npx, npy, n.ax, n.ay, n.az, d_U, strideU, dV, d_ampscale, d_I);
     return cudaGetLastError();
