@@ -296,9 +296,8 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     auto wy = [&](int j, int b) -> float & { return wsm[((0 * P + j) * KU + b) * kInterpThreads + threadIdx.x]; };
     auto wz = [&](int j, int c) -> float & { return wsm[((1 * P + j) * KU + c) * kInterpThreads + threadIdx.x]; };
     if (common) {
-        // The x weights and the row sums over x (12 of the 14 multiply-adds of a grid value) are FP32: a row sum of <= 12 terms of
-        // one sign pattern rounds at ~1e-7 of its own magnitude, the same size as the FP32 rounding U already carries; the sums over
-        // y and z (where rows of different phase combine) stay FP64.
+        // The x weights and the row sums over x are FP32: a row sum of <= 10 terms of one sign pattern rounds at ~1e-7 of its own
+        // magnitude, the same size as the FP32 rounding U already carries.
         // kept as (w, w) pairs: one packed fma.rn.f32x2 (sm_100) multiplies a grid value's (Re, Im) by the real weight
         float2 wx[P][KU];
 #pragma unroll
@@ -317,58 +316,54 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
 #pragma unroll
             for (int a = 0; a < KU; ++a) wz(j, a) = (float)placed<KU>(own, m0[j][2] - base[2], a);
         }
-        // first grid value of the thread's window and the strides between its rows and planes, in the tile or in U
-        const float2 *win;
-        int sy, sz;                    // < 2^31: a plane of the uniform grid is at most a few 10^5 points
-        if (tiled) {
-            win = tile + ((base[2] - lo2) * e1 + (base[1] - lo1)) * e0 + (base[0] - lo0);
-            sy = e0;
-            sz = e0 * e1;
-        } else {
-            win = U + ((int64_t)(base[2] - az.m_lo) * ay.nq + (base[1] - ay.m_lo)) * ax.nq + (base[0] - ax.m_lo);   // inside the grid by the plan's margins
-            sy = ax.nq;
-            sz = ax.nq * ay.nq;
-        }
+        // The window's rows: FP32 over x (above) and over y -- eight more roundings of 6e-8 each on sums of one plane, the size of the
+        // rounding U already carries -- FP64 over z and for the intensity.  Called once with a pointer into the tile and once with one
+        // into U, so that each copy of the loop uses its own address space (shared loads for the tile, not generic ones).
         double are[P], aim[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) are[j] = aim[j] = 0.0;
-        for (int c = 0; c < KU; ++c) {
-            double wzc[P];
-            bool any = false;
+        auto walk = [&](const float2 *__restrict__ win, int sy, int sz) {   // strides < 2^31: a plane of the grid is a few 10^5 points
+            for (int c = 0; c < KU; ++c) {
+                float wzc[P];
+                bool any = false;
 #pragma unroll
-            for (int j = 0; j < P; ++j) { wzc[j] = (double)wz(j, c); any |= wzc[j] != 0.0; }
-            if (!any) continue;
-            double pre[P], pim[P];
+                for (int j = 0; j < P; ++j) { wzc[j] = wz(j, c); any |= wzc[j] != 0.f; }
+                if (!any) continue;
+                float2 pl[P];
 #pragma unroll
-            for (int j = 0; j < P; ++j) pre[j] = pim[j] = 0.0;
-            for (int b = 0; b < KU; ++b) {
-                double wyb[P];
-                bool anyb = false;
+                for (int j = 0; j < P; ++j) pl[j] = make_float2(0.f, 0.f);
+                for (int b = 0; b < KU; ++b) {
+                    float wyb[P];
+                    bool anyb = false;
 #pragma unroll
-                for (int j = 0; j < P; ++j) { wyb[j] = (double)wy(j, b); anyb |= wyb[j] != 0.0; }
-                if (!anyb) continue;
-                const float2 *row = win + c * sz + b * sy;
-                float2 v[KU];
+                    for (int j = 0; j < P; ++j) { wyb[j] = wy(j, b); anyb |= wyb[j] != 0.f; }
+                    if (!anyb) continue;
+                    const float2 *row = win + c * sz + b * sy;
+                    float2 v[KU];
 #pragma unroll
-                for (int a = 0; a < KU; ++a) v[a] = row[a];
+                    for (int a = 0; a < KU; ++a) v[a] = row[a];
+#pragma unroll
+                    for (int j = 0; j < P; ++j) {
+                        float2 ra = make_float2(0.f, 0.f), rb = make_float2(0.f, 0.f);   // two chains per pixel
+#pragma unroll
+                        for (int a = 0; a < KU; a += 2) {
+                            ra = __ffma2_rn(wx[j][a], v[a], ra);
+                            rb = __ffma2_rn(wx[j][a + 1], v[a + 1], rb);
+                        }
+                        const float2 w2 = make_float2(wyb[j], wyb[j]);
+                        pl[j] = __ffma2_rn(w2, ra, __ffma2_rn(w2, rb, pl[j]));
+                    }
+                }
 #pragma unroll
                 for (int j = 0; j < P; ++j) {
-                    float2 ra = make_float2(0.f, 0.f), rb = make_float2(0.f, 0.f);   // two chains per pixel
-#pragma unroll
-                    for (int a = 0; a < KU; a += 2) {
-                        ra = __ffma2_rn(wx[j][a], v[a], ra);
-                        rb = __ffma2_rn(wx[j][a + 1], v[a + 1], rb);
-                    }
-                    pre[j] = fma(wyb[j], (double)(ra.x + rb.x), pre[j]);
-                    pim[j] = fma(wyb[j], (double)(ra.y + rb.y), pim[j]);
+                    are[j] = fma((double)wzc[j], (double)pl[j].x, are[j]);
+                    aim[j] = fma((double)wzc[j], (double)pl[j].y, aim[j]);
                 }
             }
-#pragma unroll
-            for (int j = 0; j < P; ++j) {
-                are[j] = fma(wzc[j], pre[j], are[j]);
-                aim[j] = fma(wzc[j], pim[j], aim[j]);
-            }
-        }
+        };
+        if (tiled) walk(tile + ((base[2] - lo2) * e1 + (base[1] - lo1)) * e0 + (base[0] - lo0), e0, e0 * e1);
+        else   // inside the grid by the plan's margins
+            walk(U + ((int64_t)(base[2] - az.m_lo) * ay.nq + (base[1] - ay.m_lo)) * ax.nq + (base[0] - ax.m_lo), ax.nq, ax.nq * ay.nq);
 #pragma unroll
         for (int j = 0; j < P; ++j)
             if (j < np) {
