@@ -179,13 +179,14 @@ cudaError_t zgemm(const TA *A, const TB *B, TC *C, int M, int N, int K, int64_t 
 }
 
 // ---- interpolation: A = sum over the W^3 nearest grid points, I = |A dV|^2 (Block 11).
-// U is stored FP32 (stage Y rounds its FP64 accumulators on the way out): the window's weights are positive and A varies slowly over the
-// window, so a value's 6e-8 relative rounding stays relative to the LOCAL amplitude (unlike an error made before the transforms, which
-// would be relative to the whole particle); sums and weights stay FP64.  Halves the bytes this L1-bound kernel pulls.
-// A thread owns P = 4, 3, 2 or 1 consecutive pixels of a detector row: their windows overlap (a pixel is a fraction of a grid cell wide), so the
-// thread walks ONE common window of KU = W + 2 cells per axis, loads every grid value once and applies it to all P pixels with
-// per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the bytes it pulls through L1, and this divides
-// them by ~P.  A group whose windows do not fit the common one (pixels more than a cell apart: coarse detectors) takes its pixels
+// U is stored FP32 (the last GEMM stage rounds its accumulators on the way out): the window's weights are positive and A varies slowly
+// over the window, so a value's 6e-8 relative rounding stays relative to the LOCAL amplitude (unlike an error made before the
+// transforms, which would be relative to the whole particle).  The sums over x and y are FP32 (packed fma.rn.f32x2: (Re, Im) times a
+// real weight), the sum over z and the intensity FP64; the weights are evaluated in FP64.
+// A thread owns P = 2 (or 1) pixels that are neighbours along y: their windows overlap (a pixel is a fraction of a grid cell wide), so
+// the thread walks ONE common window (W + 1 cells along x, W + 2 along y and z), loads every grid value once and applies it to both
+// pixels with per-pixel weights (zero outside a pixel's own support) -- the kernel is bound by the shared-memory wavefronts of
+// those loads.  A pair whose windows do not fit the common one (pixels more than a cell apart: coarse detectors) takes its pixels
 // one by one.  Window weights of the y and z axes live in shared memory ([axis][pixel][cell][thread]).
 // The window phi(s) = I0(beta sqrt(1 - (s / (W/2))^2)) / I0(beta) is entire in s^2, so on each of its W unit cells it is a polynomial
 // to 2e-13 at degree 11 (Chebyshev fit on the host, nufft_init_device): the W weights of a point come from W Horner evaluations at
@@ -229,7 +230,8 @@ __global__ void __launch_bounds__(kInterpThreads)
 nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax, NufftAxis ay, NufftAxis az,
                     const float2 *__restrict__ U, int64_t strideU, double dV, const float *__restrict__ ampscale,
                     float *__restrict__ I) {
-    constexpr int KU = P > 1 ? kW + 2 : kW;
+    constexpr int KU = P > 1 ? kW + 2 : kW;              // common window along y, z: the thread's pixels are up to 1.9 cells apart
+    constexpr int KX = P > 1 ? kW + 1 : kW;              // ... along x: neighbours along y sit at nearly the same q_x (< 1 cell apart)
     extern __shared__ float wsm[];                        // [2][P][KU][kInterpThreads] y and z weights (FP32), then the tile of U
     float2 *tile = reinterpret_cast<float2 *>(wsm + 2 * P * KU * kInterpThreads);
     __shared__ int red[8];                                // lo[3], hi[3], every thread's pixels share a window, any valid thread
@@ -266,14 +268,14 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
             top[d] = j == 0 ? m0[j][d] : max(top[d], m0[j][d]);
         }
     }
-    const bool common = valid && top[0] - base[0] + kW <= KU && top[1] - base[1] + kW <= KU && top[2] - base[2] + kW <= KU;
+    const bool common = valid && top[0] - base[0] + kW <= KX && top[1] - base[1] + kW <= KU && top[2] - base[2] + kW <= KU;
     if (valid) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             atomicMin(&red[d], base[d]);
-            // last cell the thread reads: along x every row is read over the whole common window of KU cells; along y and z
+            // last cell the thread reads: along x every row is read over the whole common window of KX cells; along y and z
             // rows and planes whose weights are all zero are skipped, so only the pixels' own windows count
-            atomicMax(&red[3 + d], d == 0 ? base[d] + KU - 1 : top[d] + kW - 1);
+            atomicMax(&red[3 + d], d == 0 ? base[d] + KX - 1 : top[d] + kW - 1);
         }
         if (!common) atomicAnd(&red[6], 0);
     }
@@ -296,17 +298,17 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
     auto wy = [&](int j, int b) -> float & { return wsm[((0 * P + j) * KU + b) * kInterpThreads + threadIdx.x]; };
     auto wz = [&](int j, int c) -> float & { return wsm[((1 * P + j) * KU + c) * kInterpThreads + threadIdx.x]; };
     if (common) {
-        // The x weights and the row sums over x are FP32: a row sum of <= 10 terms of one sign pattern rounds at ~1e-7 of its own
+        // The x weights and the row sums over x are FP32: a row sum of <= 9 terms of one sign pattern rounds at ~1e-7 of its own
         // magnitude, the same size as the FP32 rounding U already carries.
         // kept as (w, w) pairs: one packed fma.rn.f32x2 (sm_100) multiplies a grid value's (Re, Im) by the real weight
-        float2 wx[P][KU];
+        float2 wx[P][KX];
 #pragma unroll
         for (int j = 0; j < P; ++j) {
             double own[kW];
             kb_weights(u[j][0], m0[j][0], own);
 #pragma unroll
-            for (int a = 0; a < KU; ++a) {
-                const float w = (float)placed<KU>(own, m0[j][0] - base[0], a);
+            for (int a = 0; a < KX; ++a) {
+                const float w = (float)placed<KX>(own, m0[j][0] - base[0], a);
                 wx[j][a] = make_float2(w, w);
             }
             kb_weights(u[j][1], m0[j][1], own);
@@ -339,16 +341,16 @@ nufft_interp_kernel(const double *__restrict__ q, int npx, int npy, NufftAxis ax
                     for (int j = 0; j < P; ++j) { wyb[j] = wy(j, b); anyb |= wyb[j] != 0.f; }
                     if (!anyb) continue;
                     const float2 *row = win + c * sz + b * sy;
-                    float2 v[KU];
+                    float2 v[KX];
 #pragma unroll
-                    for (int a = 0; a < KU; ++a) v[a] = row[a];
+                    for (int a = 0; a < KX; ++a) v[a] = row[a];
 #pragma unroll
                     for (int j = 0; j < P; ++j) {
                         float2 ra = make_float2(0.f, 0.f), rb = make_float2(0.f, 0.f);   // two chains per pixel
 #pragma unroll
-                        for (int a = 0; a < KU; a += 2) {
-                            ra = __ffma2_rn(wx[j][a], v[a], ra);
-                            rb = __ffma2_rn(wx[j][a + 1], v[a + 1], rb);
+                        for (int a = 0; a < KX; ++a) {
+                            if (a & 1) rb = __ffma2_rn(wx[j][a], v[a], rb);
+                            else ra = __ffma2_rn(wx[j][a], v[a], ra);
                         }
                         const float2 w2 = make_float2(wyb[j], wyb[j]);
                         pl[j] = __ffma2_rn(w2, ra, __ffma2_rn(w2, rb, pl[j]));
