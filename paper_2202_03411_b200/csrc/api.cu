@@ -620,10 +620,26 @@ int scatman_qgrid_workspace_bytes(scatman_ctx *ctx, const scatman_grid *grid, in
 
 }  // extern "C"
 
-// h_stats: extremes of the grids when the host knows them (rendered shapes), else null (measured on the device)
+// Renders h_shapes into d_dn on `st`; sparse (tile map at d_tilemap) if that is non-null.  SCATMAN_OK or the failure, *nl += launches.
+static int render_into(scatman_ctx *ctx, const scatman_shape *h_shapes, int batch, const scatman_grid &grid, float *d_dn,
+                       unsigned char *d_tilemap, cudaStream_t st, int *nl) {
+    if ((size_t)((uint64_t)grid.nx * grid.ny * grid.nz + 255) / 256 > 0x7fffffffull || batch > 65535)
+        return fail(ctx, SCATMAN_INVALID_ARGUMENT, "grid or batch too large for one render launch");
+    cudaError_t e = cudaSuccess;
+    int n = 0;
+    const int bad = launch_render_batch(h_shapes, batch, grid, d_dn, st, &e, &n, d_tilemap);
+    if (bad) return fail(ctx, SCATMAN_INVALID_ARGUMENT, "bad shape descriptor " + std::to_string(bad - 1));
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "render");
+    *nl += n;
+    return SCATMAN_OK;
+}
+
+// h_stats: extremes of the grids when the host knows them (rendered shapes), else null (measured on the device).
+// h_shapes: non-null -> the grids are rendered into d_dn first (scatman_simulate_shapes_qgrid), sparsely when the fused prefix pass reads them.
 static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda, const double *d_qx,
                       int32_t npx, const double *d_qy, int32_t npy, const double *h_quat, int32_t batch,
-                      const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats) {
+                      const scatman_options *opts, void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats,
+                      const scatman_shape *h_shapes = nullptr) {
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !d_qx || !d_qy || !valid_grid(grid) || !(lambda > 0.0) || !std::isfinite(lambda) ||
@@ -652,6 +668,12 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
     const float *src = d_dn;
     unsigned *stats = (unsigned *)(ws + sp.off_stats);
     const bool oriented = h_quat && !all_identity(h_quat, batch);
+    bool src_sparse = oriented;          // src is read through the tile map
+    if (h_shapes) {
+        src_sparse = sp.fused_ok;
+        const int rc = render_into(ctx, h_shapes, batch, *grid, const_cast<float *>(d_dn), src_sparse ? ws + sp.off_tilemap : nullptr, st, &nl);
+        if (rc != SCATMAN_OK) return rc;
+    }
     if (oriented) {
         double *rm = (double *)(ws + sp.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
@@ -697,7 +719,7 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags,
                                                   bounds, ampscale + b0, st, false,
-                                                  oriented ? ws + sp.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
+                                                  src_sparse ? ws + sp.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds,
                                            ampscale + b0, st);
             if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
@@ -758,15 +780,10 @@ int scatman_simulate_shapes_qgrid(scatman_ctx *ctx, const scatman_shape *h_shape
     const size_t dn_bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024);
     if (ws_bytes < dn_bytes) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     float *d_dn = (float *)d_ws;
-    int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
-    if (rc != SCATMAN_OK) return rc;
-    const int rendered = ctx->last_launches;
     std::vector<float> stats;
     shape_stats(h_shapes, batch, stats);
-    rc = qgrid_impl(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes,
-                    ws_bytes - dn_bytes, d_I, cuda_stream, stats.data());
-    if (rc == SCATMAN_OK) ctx->last_launches += rendered;
-    return rc;
+    return qgrid_impl(ctx, d_dn, grid, lambda, d_qx, npx, d_qy, npy, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes,
+                      ws_bytes - dn_bytes, d_I, cuda_stream, stats.data(), h_shapes);
 }
 
 // ---- flat detector by a 3-D type-2 NUFFT (nufft_kernels.cu) ----------------------------------------------------------
@@ -914,7 +931,8 @@ int scatman_nufft_grid_dims(scatman_ctx *ctx, const scatman_grid *grid, double l
 
 static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *grid, double lambda,
                       const scatman_detector *det, const double *h_quat, int32_t batch, const scatman_options *opts,
-                      void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats) {
+                      void *d_ws, size_t ws_bytes, float *d_I, void *cuda_stream, const float *h_stats,
+                      const scatman_shape *h_shapes = nullptr) {   // h_stats, h_shapes: see qgrid_impl
     scatman_options o = opts ? *opts : scatman_options{0, 0, 0, 0};
     if (!ctx) return SCATMAN_INVALID_ARGUMENT;
     if (!d_dn || !d_I || !d_ws || !valid_grid(grid) || !valid_detector(det) || !(lambda > 0.0) || !std::isfinite(lambda) ||
@@ -950,6 +968,12 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
     const float *src = d_dn;
     unsigned *stats = (unsigned *)(ws + L.off_stats), *maxbits = (unsigned *)(ws + L.off_max);
     const bool oriented = h_quat && !all_identity(h_quat, batch);
+    bool src_sparse = oriented;
+    if (h_shapes) {
+        src_sparse = L.fused_ok;
+        const int rc = render_into(ctx, h_shapes, batch, *grid, const_cast<float *>(d_dn), src_sparse ? ws + L.off_tilemap : nullptr, st, &nl);
+        if (rc != SCATMAN_OK) return rc;
+    }
     if (oriented) {
         double *rm = (double *)(ws + L.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
@@ -993,7 +1017,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags,
                                                   bounds, ampscale + b0, st, true,
-                                                  oriented ? ws + L.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
+                                                  src_sparse ? ws + L.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags, bounds,
                                            ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero
@@ -1059,15 +1083,10 @@ int scatman_simulate_shapes_nufft(scatman_ctx *ctx, const scatman_shape *h_shape
     const size_t dn_bytes = scatman::align_up(sizeof(float) * 2 * (size_t)grid->nx * grid->ny * grid->nz * batch, 1024);
     if (ws_bytes < dn_bytes) return fail(ctx, SCATMAN_WORKSPACE_TOO_SMALL, "workspace too small");
     float *d_dn = (float *)d_ws;
-    int rc = scatman_render(ctx, h_shapes, batch, grid, d_dn, cuda_stream);
-    if (rc != SCATMAN_OK) return rc;
-    const int rendered = ctx->last_launches;
     std::vector<float> stats;
     shape_stats(h_shapes, batch, stats);
-    rc = nufft_impl(ctx, d_dn, grid, lambda, det, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes, d_I, cuda_stream,
-                    stats.data());
-    if (rc == SCATMAN_OK) ctx->last_launches += rendered;
-    return rc;
+    return nufft_impl(ctx, d_dn, grid, lambda, det, nullptr, batch, opts, (uint8_t *)d_ws + dn_bytes, ws_bytes - dn_bytes, d_I, cuda_stream,
+                      stats.data(), h_shapes);
 }
 
 // ---- forward-fitting pieces ---------------------------------------------------------------------------------------

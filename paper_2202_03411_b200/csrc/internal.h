@@ -112,7 +112,8 @@ cudaError_t launch_sep_tc_finalize(const float2 *d_partial, const double *d_qx, 
                                    const Plan &p, const SepTcPlan &t, int nb, const float *d_ampscale, float *d_I,
                                    cudaStream_t st);
 int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_grid &g, float *d_dn, cudaStream_t st,
-                        cudaError_t *err, int *nlaunch);   // 0, or 1 + index of the first bad descriptor
+                        cudaError_t *err, int *nlaunch,    // 0, or 1 + index of the first bad descriptor
+                        unsigned char *d_tilemap = nullptr);   // non-null: sparse output + tile map, as launch_orient's
 
 // flat-detector route by a 3-D type-2 NUFFT (nufft_kernels.cu)
 constexpr int kNufftW = 8;                      // Kaiser-Bessel window width in grid cells (oversampling 2); R25

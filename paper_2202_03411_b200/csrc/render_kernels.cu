@@ -177,9 +177,18 @@ __device__ bool render_inside(const RenderBatch &Bt, const RenderArgs &A, double
 // A WARP renders a run of up to 128 consecutive x of one row (y, z) of one shape (blockIdx.y): lane i takes x0 + i, x0 + i + 32, ...,
 // so that every store of the warp is 256 contiguous bytes, the row's index arithmetic is done once per four voxels, and a row that
 // misses the shape's circumscribed sphere altogether (most rows of most grids) is zero-filled without looking at its voxels.
+// tilemap != null: SPARSE output for launch_sep_tc_prefix_prep, as launch_orient's -- a tile of 16 x 4 x 4 voxels whose nearest point to
+// the centre lies outside the circumscribed sphere is not written at all, tilemap[shape][z / 4][y / 4][x / 16] = 0 says so (every row of
+// a tile takes the same decision: it depends on the tile's indices only).
 constexpr int kRenderRun = 128;
+// min of coordinate^2 over cells i0 .. i0 + len - 1.  FP32: the decision only has to be the same in every row of a tile (it is a
+// function of the tile's indices) and must never drop a tile that holds a voxel inside the sphere -- the sphere is widened by 1e-5.
+__device__ __forceinline__ float nearest_sq(int i0, int n, float d, int len) {
+    const float a = ((float)i0 - 0.5f * (float)(n - 1)) * d, b = a + (float)(len - 1) * d;
+    return a > 0.f ? a * a : (b < 0.f ? b * b : 0.f);
+}
 __global__ void __launch_bounds__(256)
-render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out) {
+render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out, unsigned char *__restrict__ tilemap) {
     const RenderArgs &A = Bt.a[blockIdx.y];
     const int lane = threadIdx.x & 31;
     const unsigned runs = (unsigned)(A.nx + kRenderRun - 1) / kRenderRun;      // runs per row
@@ -197,19 +206,39 @@ render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out) 
     // so the rendering is voxel for voxel what the full test gives.
     const double yz2 = y * y + z * z;
     const float2 vac = make_float2(0.f, 0.f), mat = make_float2(A.delta, A.beta);
+    auto classify = [&](int ix) -> bool {
+        const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
+        const double r2 = x * x + yz2;
+        if (r2 > A.r2_out) return false;
+        if (r2 < A.r2_in) return true;
+        return render_inside(Bt, A, x, y, z);
+    };
+    if (tilemap) {
+        const int nbx = (A.nx + 15) / 16, nby = (A.ny + 3) / 4, nbz = (A.nz + 3) / 4;
+        const float fdx = (float)A.dx, r2o = (float)A.r2_out * 1.00001f;
+        const float tyz2 = nearest_sq(iy & ~3, A.ny, (float)A.dy, 4) + nearest_sq(iz & ~3, A.nz, (float)A.dz, 4);
+        const bool row_out = tyz2 > r2o;        // every tile of this row lies outside the sphere (most rows of most grids)
+        if (((iy | iz) & 3) == 0) {                  // the first row of its tiles writes their map bytes: lane = tile of the run
+            const int tx = (x0 >> 4) + lane;
+            if (tx < nbx && tx * 16 < x1)
+                tilemap[(((size_t)blockIdx.y * nbz + (iz >> 2)) * nby + (iy >> 2)) * nbx + tx] =
+                    !row_out && !(nearest_sq(tx * 16, A.nx, fdx, 16) + tyz2 > r2o) ? 1 : 0;
+        }
+        if (row_out) return;
+#pragma unroll 1
+        for (int ix = x0 + lane; ix < x1; ix += 32) {
+            if (nearest_sq(ix & ~15, A.nx, fdx, 16) + tyz2 > r2o) continue;      // the tile cannot hold material: not written
+            dst[ix] = classify(ix) ? mat : vac;
+        }
+        return;
+    }
     if (yz2 > A.r2_out) {
         for (int ix = x0 + lane; ix < x1; ix += 32) dst[ix] = vac;
         return;
     }
 #pragma unroll 1
     for (int ix = x0 + lane; ix < x1; ix += 32) {
-        const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
-        const double r2 = x * x + yz2;
-        bool inside;
-        if (r2 > A.r2_out) inside = false;
-        else if (r2 < A.r2_in) inside = true;
-        else inside = render_inside(Bt, A, x, y, z);
-        dst[ix] = inside ? mat : vac;
+        dst[ix] = classify(ix) ? mat : vac;
     }
 }
 
@@ -340,7 +369,7 @@ static int fill_render_args(const scatman_shape &s, const scatman_grid &g, Rende
 // Renders h_shapes[0 .. batch) into d_dn[batch][nz][ny][nx][2]: one launch per RenderBatch of descriptors.
 // Returns 0, or 1 + the index of the first bad descriptor; *err = the CUDA status; *nlaunch = kernels launched.
 int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_grid &g, float *d_dn, cudaStream_t st, cudaError_t *err,
-                        int *nlaunch) {
+                        int *nlaunch, unsigned char *d_tilemap) {
     *err = cudaSuccess;
     *nlaunch = 0;
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
@@ -362,7 +391,9 @@ int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_
             ++b;
         }
         const size_t nruns = (size_t)g.ny * g.nz * ((g.nx + kRenderRun - 1) / kRenderRun);      // one warp each
-        render_kernel<<<dim3((unsigned)((nruns + 7) / 8), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox);
+        const size_t tiles = (size_t)((g.nz + 3) / 4) * ((g.ny + 3) / 4) * ((g.nx + 15) / 16);
+        render_kernel<<<dim3((unsigned)((nruns + 7) / 8), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox,
+                                                                                      d_tilemap ? d_tilemap + (size_t)first * tiles : nullptr);
         ++*nlaunch;
         *err = cudaGetLastError();
         if (*err != cudaSuccess) return 0;
