@@ -129,18 +129,19 @@ __device__ bool render_inside(const RenderBatch &Bt, const RenderArgs &A, double
         return u * u + w * w + t * t <= 1.0;
     }
     if (A.kind == SCATMAN_SHAPE_SPHERICAL_HARMONICS) {
-        const double rho2 = xb * xb + yb * yb;
-        const double r = sqrt(rho2 + zb * zb);
+        // two reciprocal square roots instead of three square roots and two divisions (each ~30 FP64 instructions): r = r^2 / r,
+        // cos theta = z / r, sin theta = rho / r, (cos phi, sin phi) = (x, y) / rho
+        const double rho2 = xb * xb + yb * yb, r2 = rho2 + zb * zb;
+        const double ir = r2 > 0.0 ? rsqrt(r2) : 0.0;
+        const double r = r2 * ir;
         if (r < A.r_lo) return true;
         if (r > A.r_hi) return false;
-        const double ir = r > 0.0 ? 1.0 / r : 0.0;
-        const double ct = r > 0.0 ? zb * ir : 1.0;
-        const double rho = sqrt(rho2);
-        const double irho = rho > 0.0 ? 1.0 / rho : 0.0;
-        const double cphi = rho > 0.0 ? xb * irho : 1.0, sphi = yb * irho;   // phi = atan2(y, x)
+        const double ct = r2 > 0.0 ? zb * ir : 1.0;
+        const double irho = rho2 > 0.0 ? rsqrt(rho2) : 0.0;
+        const double cphi = rho2 > 0.0 ? xb * irho : 1.0, sphi = yb * irho;   // phi = atan2(y, x)
         double R;
         if (A.dense_L > 0) {
-            const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+            const double st = rho2 * irho * ir;
             const double *cc = Bt.cn + A.coef0;
             if (A.dense_L == 4) R = sh_radius_dense<4>(cc, cc + sh_pairs(4), ct, st, cphi, sphi);
             else if (A.dense_L == 6) R = sh_radius_dense<6>(cc, cc + sh_pairs(6), ct, st, cphi, sphi);
@@ -174,13 +175,15 @@ __device__ bool render_inside(const RenderBatch &Bt, const RenderArgs &A, double
     return false;
 }
 
-// A WARP renders a run of up to 128 consecutive x of one row (y, z) of one shape (blockIdx.y): lane i takes x0 + i, x0 + i + 32, ...,
-// so that every store of the warp is 256 contiguous bytes, the row's index arithmetic is done once per four voxels, and a row that
-// misses the shape's circumscribed sphere altogether (most rows of most grids) is zero-filled without looking at its voxels.
+// A WARP renders a run of up to 128 consecutive x of EIGHT consecutive rows (y .. y + 7, one z) of one shape (blockIdx.y): lane i takes
+// x0 + i, x0 + i + 32, ..., so that every store of the warp is 256 contiguous bytes; the index arithmetic of a work item (integer
+// divisions, the descriptor's fields from the parameter bank) is done once per 8 x 128 voxels -- with one row per warp it was most
+// of the ~230 instructions that a row outside the shape cost, and those rows are most of a grid; a row that misses the shape's
+// circumscribed sphere altogether is zero-filled without looking at its voxels.
 // tilemap != null: SPARSE output for launch_sep_tc_prefix_prep, as launch_orient's -- a tile of 16 x 4 x 4 voxels whose nearest point to
 // the centre lies outside the circumscribed sphere is not written at all, tilemap[shape][z / 4][y / 4][x / 16] = 0 says so (every row of
 // a tile takes the same decision: it depends on the tile's indices only).
-constexpr int kRenderRun = 128;
+constexpr int kRenderRun = 128, kRenderRows = 8;
 // min of coordinate^2 over cells i0 .. i0 + len - 1.  FP32: the decision only has to be the same in every row of a tile (it is a
 // function of the tile's indices) and must never drop a tile that holds a voxel inside the sphere -- the sphere is widened by 1e-5.
 __device__ __forceinline__ float nearest_sq(int i0, int n, float d, int len) {
@@ -192,53 +195,62 @@ render_kernel(const __grid_constant__ RenderBatch Bt, float2 *__restrict__ out, 
     const RenderArgs &A = Bt.a[blockIdx.y];
     const int lane = threadIdx.x & 31;
     const unsigned runs = (unsigned)(A.nx + kRenderRun - 1) / kRenderRun;      // runs per row
-    const unsigned long long w = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // run index
-    const unsigned long long nrows = (unsigned long long)A.ny * A.nz;
-    if (w >= nrows * runs) return;
-    const unsigned row = (unsigned)(w / runs), run = (unsigned)(w - (unsigned long long)row * runs);       // nrows < 2^32 (ny <= 8192, nz <= 65535)
-    const int iz = (int)(row / (unsigned)A.ny), iy = (int)(row - (unsigned)iz * (unsigned)A.ny);
+    const unsigned ygroups = (unsigned)(A.ny + kRenderRows - 1) / kRenderRows;
+    const unsigned long long w = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // work item
+    const unsigned long long ngroups = (unsigned long long)ygroups * A.nz;     // < 2^32 (ny <= 8192, nz <= 65535)
+    if (w >= ngroups * runs) return;
+    unsigned grp, run;                                                         // (a 64-bit division costs ~70 instructions: only if needed)
+    if (runs == 1) { grp = (unsigned)w; run = 0; }
+    else if (w <= 0xffffffffull) { grp = (unsigned)w / runs; run = (unsigned)w - grp * runs; }
+    else { grp = (unsigned)(w / runs); run = (unsigned)(w - (unsigned long long)grp * runs); }
+    const int iz = (int)(grp / ygroups), iy0 = (int)(grp - (unsigned)iz * ygroups) * kRenderRows;
     const int x0 = (int)run * kRenderRun, x1 = min(A.nx, x0 + kRenderRun);
-    float2 *dst = out + (size_t)blockIdx.y * A.nx * A.ny * A.nz + (size_t)row * A.nx;
-    const double y = ((double)iy - 0.5 * (double)(A.ny - 1)) * A.dy;
+    const int nx = A.nx, ny = A.ny;
+    const double dx = A.dx, dy = A.dy, r2_out = A.r2_out, r2_in = A.r2_in;
     const double z = ((double)iz - 0.5 * (double)(A.nz - 1)) * A.dz;
-    // |r| does not change under the rotation: voxels inside the shape's inscribed sphere or outside its circumscribed one are
-    // decided from x^2 + y^2 + z^2 alone (most of a grid); the margins of 1e-12 leave every close call to the full test,
-    // so the rendering is voxel for voxel what the full test gives.
-    const double yz2 = y * y + z * z;
     const float2 vac = make_float2(0.f, 0.f), mat = make_float2(A.delta, A.beta);
-    auto classify = [&](int ix) -> bool {
-        const double x = ((double)ix - 0.5 * (double)(A.nx - 1)) * A.dx;
-        const double r2 = x * x + yz2;
-        if (r2 > A.r2_out) return false;
-        if (r2 < A.r2_in) return true;
-        return render_inside(Bt, A, x, y, z);
-    };
-    if (tilemap) {
-        const int nbx = (A.nx + 15) / 16, nby = (A.ny + 3) / 4, nbz = (A.nz + 3) / 4;
-        const float fdx = (float)A.dx, r2o = (float)A.r2_out * 1.00001f;
-        const float tyz2 = nearest_sq(iy & ~3, A.ny, (float)A.dy, 4) + nearest_sq(iz & ~3, A.nz, (float)A.dz, 4);
-        const bool row_out = tyz2 > r2o;        // every tile of this row lies outside the sphere (most rows of most grids)
-        if (((iy | iz) & 3) == 0) {                  // the first row of its tiles writes their map bytes: lane = tile of the run
-            const int tx = (x0 >> 4) + lane;
-            if (tx < nbx && tx * 16 < x1)
-                tilemap[(((size_t)blockIdx.y * nbz + (iz >> 2)) * nby + (iy >> 2)) * nbx + tx] =
-                    !row_out && !(nearest_sq(tx * 16, A.nx, fdx, 16) + tyz2 > r2o) ? 1 : 0;
+    float2 *dst = out + ((size_t)blockIdx.y * A.nz + iz) * ((size_t)nx * ny) + (size_t)iy0 * nx;
+    // sparse output: the tiles' decisions
+    const int nbx = (nx + 15) / 16;
+    const float fdx = (float)dx, r2o = (float)r2_out * 1.00001f;
+    const float tz2 = tilemap ? nearest_sq(iz & ~3, A.nz, (float)A.dz, 4) : 0.f;
+    unsigned char *tm = tilemap ? tilemap + (((size_t)blockIdx.y * ((A.nz + 3) / 4) + (iz >> 2)) * ((ny + 3) / 4) + (iy0 >> 2)) * nbx : nullptr;
+    float tyz2 = 0.f;
+    bool rows_out = false;
+#pragma unroll 1
+    for (int r = 0; r < kRenderRows && iy0 + r < ny; ++r, dst += nx) {
+        const int iy = iy0 + r;
+        const double y = ((double)iy - 0.5 * (double)(ny - 1)) * dy;
+        // |r| does not change under the rotation: voxels inside the shape's inscribed sphere or outside its circumscribed one are
+        // decided from x^2 + y^2 + z^2 alone (most of a grid); the margins of 1e-12 leave every close call to the full test,
+        // so the rendering is voxel for voxel what the full test gives.
+        const double yz2 = y * y + z * z;
+        if (tilemap) {
+            if ((r & 3) == 0) {                          // a new row of tiles (iy0 is a multiple of 8)
+                tyz2 = nearest_sq(iy, ny, (float)dy, 4) + tz2;
+                rows_out = tyz2 > r2o;                   // every tile of these rows lies outside the sphere (most rows of most grids)
+                if ((iz & 3) == 0) {                     // the first row of its tiles writes their map bytes: lane = tile of the run
+                    const int tx = (x0 >> 4) + lane;
+                    if (tx < nbx && tx * 16 < x1)
+                        tm[(size_t)(r >> 2) * nbx + tx] = !rows_out && !(nearest_sq(tx * 16, nx, fdx, 16) + tyz2 > r2o) ? 1 : 0;
+                }
+            }
+            if (rows_out) continue;
+        } else if (yz2 > r2_out) {
+            for (int ix = x0 + lane; ix < x1; ix += 32) dst[ix] = vac;
+            continue;
         }
-        if (row_out) return;
 #pragma unroll 1
         for (int ix = x0 + lane; ix < x1; ix += 32) {
-            if (nearest_sq(ix & ~15, A.nx, fdx, 16) + tyz2 > r2o) continue;      // the tile cannot hold material: not written
-            dst[ix] = classify(ix) ? mat : vac;
+            if (tilemap && nearest_sq(ix & ~15, nx, fdx, 16) + tyz2 > r2o) continue;      // the tile cannot hold material: not written
+            const double x = ((double)ix - 0.5 * (double)(nx - 1)) * dx;
+            const double r2 = x * x + yz2;
+            bool inside;
+            if (r2 > r2_out) inside = false;
+            else if (r2 < r2_in) inside = true;
+            else inside = render_inside(Bt, A, x, y, z);
+            dst[ix] = inside ? mat : vac;
         }
-        return;
-    }
-    if (yz2 > A.r2_out) {
-        for (int ix = x0 + lane; ix < x1; ix += 32) dst[ix] = vac;
-        return;
-    }
-#pragma unroll 1
-    for (int ix = x0 + lane; ix < x1; ix += 32) {
-        dst[ix] = classify(ix) ? mat : vac;
     }
 }
 
@@ -390,7 +402,7 @@ int launch_render_batch(const scatman_shape *h_shapes, int batch, const scatman_
             ++Bt.n;
             ++b;
         }
-        const size_t nruns = (size_t)g.ny * g.nz * ((g.nx + kRenderRun - 1) / kRenderRun);      // one warp each
+        const size_t nruns = (size_t)((g.ny + kRenderRows - 1) / kRenderRows) * g.nz * ((g.nx + kRenderRun - 1) / kRenderRun);      // one warp each
         const size_t tiles = (size_t)((g.nz + 3) / 4) * ((g.ny + 3) / 4) * ((g.nx + 15) / 16);
         render_kernel<<<dim3((unsigned)((nruns + 7) / 8), (unsigned)Bt.n), 256, 0, st>>>(Bt, (float2 *)d_dn + (size_t)first * nvox,
                                                                                       d_tilemap ? d_tilemap + (size_t)first * tiles : nullptr);
