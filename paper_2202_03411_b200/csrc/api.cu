@@ -1022,10 +1022,12 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
                                            ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero
             SCATMAN_STAGE_CHECK(e, st, "nufft pack");
-            if (e == cudaSuccess) e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);
+            // (when a slice is a single 128-y tile, stage Y zeroes the rows of unwritten slices itself: no pass over the 2 GB of H)
+            if (e == cudaSuccess && nufft_tc_needs_h_memset(t))
+                e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);
             if (e == cudaSuccess) e = launch_sep_tc_x(p, t.sep, Rp, Txp, ws + L.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
             SCATMAN_STAGE_CHECK(e, st, "nufft stage X");
-            if (e == cudaSuccess) e = launch_nufft_tc_yz(p, L.n, t, nb, Hp, Typ, Tzp, Vp, U, ctx->num_sms, st, &err);
+            if (e == cudaSuccess) e = launch_nufft_tc_yz(p, L.n, t, nb, Hp, Typ, Tzp, Vp, U, ctx->num_sms, st, &err, ws + L.off_flags);
             SCATMAN_STAGE_CHECK(e, st, "nufft stages Y, Z");
             // amplitude = accumulator x (the separable route's per-item scale) / (2^10 of Tz x stage Y's 2^(-11 - Ly))
             if (e == cudaSuccess)

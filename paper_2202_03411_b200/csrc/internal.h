@@ -145,7 +145,9 @@ cudaError_t nufft_tc_init_device();
 cudaError_t launch_nufft_tc_tables(const Plan &p, const NufftPlan &n, const NufftTcPlan &t, __half *d_Tx, __half *d_Ty, __half *d_Tz,
                                    cudaStream_t st);
 cudaError_t launch_nufft_tc_yz(const Plan &p, const NufftPlan &n, const NufftTcPlan &t, int nb, const __half *d_Hp, const __half *d_Ty,
-                               const __half *d_Tz, __half *d_Vp, float2 *d_U, int num_sms, cudaStream_t st, std::string *err);
+                               const __half *d_Tz, __half *d_Vp, float2 *d_U, int num_sms, cudaStream_t st, std::string *err,
+                               const unsigned char *d_flags64 = nullptr);
+bool nufft_tc_needs_h_memset(const NufftTcPlan &t);   // false: pass d_flags64 above instead of zeroing the H planes
 // interpolation of a chunk from U (FP32 complex [nb][nqz][nqy][nqx]); amplitude scale = ampscale[b] * scale_mul, or dV if ampscale is null
 cudaError_t launch_nufft_interp(const Plan &p, const NufftPlan &n, int nb, int npx, int npy, double pixel_cells, const double *d_q,
                                 const float2 *d_U, const float *d_ampscale, double scale_mul, float *d_I, cudaStream_t st);

@@ -69,6 +69,8 @@ struct YParams {
                             // that stage Z's TMA boxes start 16-byte aligned (a box start that is not raises an illegal-instruction fault)
     int NQYP, NZT;          // padded columns; row length of V (nb NZI)
     float hscale;           // accumulator -> stored V
+    const unsigned char *flags;   // non-null (NY = 128 only): flags64[jg][2] of the separable pack; a slice with no flag set was not
+                            // written by stage X at all -- its rows of H hold whatever was there and its rows of V are written as zeros
     __half *Vp;
     size_t plane;           // elements per V plane
 };
@@ -105,11 +107,14 @@ struct StageY {
     struct Epilogue {
         __device__ void begin(const Params &, const Item &, const tcg::EpiThread &) {}
         int jg, jv, mx;      // global slice; its position in a V row; uniform-grid column
+        bool dead;           // the slice holds no material: stage X left its rows of H unwritten (row j of the product depends on row j only)
         __device__ void unit_begin(const Params &P, const Item &, const tcg::EpiThread &et, int unit) {
             jg = (unit % P.njt) * tcg::kM + et.lane_row;
             const int b = jg / P.nz;
             jv = b * P.NZI + (jg - b * P.nz);
             mx = unit / P.njt;
+            dead = false;
+            if (P.flags && jg < P.ntot) dead = (P.flags[2 * (size_t)jg] | P.flags[2 * (size_t)jg + 1]) == 0;
         }
         __device__ void columns(const Params &P, const Item &it, const tcg::EpiThread &et, int, int c0, const uint32_t (&gre)[8],
                                 const uint32_t (&gim)[8]) {
@@ -120,7 +125,7 @@ struct StageY {
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 __half h[4];
-                tcg::split4h(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
+                tcg::split4h(dead ? 0.f : __uint_as_float(gre[i]) * P.hscale, dead ? 0.f : __uint_as_float(gim[i]) * P.hscale, h);
                 __half *d = dst + (size_t)i * P.NZT;
 #pragma unroll
                 for (int pl = 0; pl < 4; ++pl) d[pl * P.plane] = h[pl];
@@ -268,9 +273,13 @@ static cudaError_t run_stage_z(const CUtensorMap &tmA, const CUtensorMap &tmB, c
     return tcg::cgemm_launch<StageZ<NB>>(tmA, tmB, P, P.ntb * P.nsplit, num_sms, st);
 }
 
-// Stages Y and Z for a chunk of nb items whose H planes [4][nb nz][NPXP][NY] stage X has written (dead tiles zeroed by the caller).
+// Stages Y and Z for a chunk of nb items whose H planes [4][nb nz][NPXP][NY] stage X has written.  The tiles stage X did not write
+// (no material) must read as zero: the caller zeroes H first -- or, when a slice is one 128-y tile (NY = 128), passes the flags of
+// the pack (d_flags64) and stage Y writes the rows of such slices as zeros whatever H holds (nufft_tc_needs_h_memset).
+bool nufft_tc_needs_h_memset(const NufftTcPlan &t) { return t.NY != tcg::kM; }
 cudaError_t launch_nufft_tc_yz(const Plan &p, const NufftPlan &n, const NufftTcPlan &t, int nb, const __half *d_Hp, const __half *d_Ty,
-                               const __half *d_Tz, __half *d_Vp, float2 *d_U, int num_sms, cudaStream_t st, std::string *err) {
+                               const __half *d_Tz, __half *d_Vp, float2 *d_U, int num_sms, cudaStream_t st, std::string *err,
+                               const unsigned char *d_flags64) {
     const int ntot = nb * p.nz;
     const size_t h_plane = (size_t)ntot * t.NPXP * t.NY, v_plane = (size_t)t.NPXP * t.NQYP * t.NZT;
     CUtensorMap tmA, tmB;
@@ -307,6 +316,7 @@ cudaError_t launch_nufft_tc_yz(const Plan &p, const NufftPlan &n, const NufftTcP
     Y.hscale = ldexpf(1.f, -11 - Ly);     // |acc| <= 2^14.5 (H) x 2^10.5 (Ty) x 2^Ly  ->  |V| <= 2^14
     Y.Vp = d_Vp;
     Y.plane = v_plane;
+    Y.flags = nufft_tc_needs_h_memset(t) ? nullptr : d_flags64;
     cudaError_t e = cudaSuccess;
     if (t.NZI != p.nz) {   // the padding between the items' slices is read by stage Z (against zero table entries): it must be finite
         e = cudaMemsetAsync(d_Vp, 0, sizeof(__half) * 4 * v_plane, st);
