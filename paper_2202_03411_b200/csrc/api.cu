@@ -555,7 +555,7 @@ struct SepPlan {
     bool fused_ok = false;   // tensor stages: a chunk is large enough for the fused prefix -> planes pass (fused_prefix_pays)
     int nzs = 1;
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_ex = 0, off_ey = 0, off_h = 0, off_flags = 0,
-           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, off_stats = 0, off_tilemap = 0, total = 0;
+           off_partial = 0, off_eyp = 0, off_exp = 0, off_rp = 0, off_hp = 0, off_scale = 0, off_bounds = 0, off_stats = 0, off_tilemap = 0, off_layers = 0, total = 0;
 };
 static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int npy, int batch, int rho_mode, int method,
                              int num_sms) {
@@ -586,7 +586,10 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
     sp.off_rho = sp.fused_ok ? sp.off_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     sp.off_max = take(sizeof(unsigned) * (size_t)batch);
     sp.off_stats = take(sizeof(unsigned) * 3 * (size_t)batch);
-    if (sp.fused_ok) sp.off_tilemap = take(orient_tilemap_bytes(p, batch));   // sparse orientation output (launch_orient)
+    if (sp.fused_ok) {   // sparse orientation / render output (launch_orient)
+        sp.off_tilemap = take(orient_tilemap_bytes(p, batch));
+        sp.off_layers = take(tile_layers_bytes(p, batch));
+    }
     if (sp.tensor) {
         const SepTcPlan &t = sp.tc;
         sp.off_rp = take(sizeof(__half) * 4 * (size_t)t.nb * g.nz * t.NY * t.NXP);
@@ -719,7 +722,7 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags,
                                                   bounds, ampscale + b0, st, false,
-                                                  src_sparse ? ws + sp.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
+                                                  src_sparse ? ws + sp.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr, ws + sp.off_layers)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t, nb, Rp, ws + sp.off_flags, bounds,
                                            ampscale + b0, st);
             if (e == cudaSuccess) e = launch_sep_tc_x(p, t, Rp, Exp, ws + sp.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
@@ -796,7 +799,7 @@ struct NufftLayout {
     size_t off_rotmat = 0, off_bbox = 0, off_rot = 0, off_rho = 0, off_max = 0, off_q = 0, off_tz = 0, off_tx = 0, off_ty = 0,
            off_P = 0, off_H = 0, off_U = 0, total = 0;
     // tensor-core stages: table planes, rho~ planes, H planes, V planes, flags, z-split bounds, per-item scales
-    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0, off_stats = 0, off_tilemap = 0;
+    size_t off_txp = 0, off_typ = 0, off_tzp = 0, off_rp = 0, off_hp = 0, off_vp = 0, off_flags = 0, off_bounds = 0, off_scale = 0, off_stats = 0, off_tilemap = 0, off_layers = 0;
     size_t hp_bytes = 0;
 };
 // Range of q over the detector (host, FP64, a1's formula): q_x and q_y are monotonic along u and v and extremal in the other
@@ -884,7 +887,8 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
         if (mine) { L.off_rotmat = o_rm; L.off_bbox = o_bb; L.off_rot = o_rot; L.off_rho = o_rho; L.off_max = o_max; L.off_stats = o_st; L.fused_ok = tensor && o_rho == o_rot; }
         {
             const size_t o_tm = tensor && o_rho == o_rot ? take(orient_tilemap_bytes(p, batch)) : 0;
-            if (mine) L.off_tilemap = o_tm;
+            const size_t o_ly = tensor && o_rho == o_rot ? take(tile_layers_bytes(p, batch)) : 0;
+            if (mine) { L.off_tilemap = o_tm; L.off_layers = o_ly; }
         }
         if (!tensor) {
             const size_t a = take(sizeof(double2) * (size_t)L.n.nb * L.n.az.nq * g.ny * g.nx),
@@ -1017,7 +1021,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             std::string err;
             e = fused ? launch_sep_tc_prefix_prep((const float2 *)src + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags,
                                                   bounds, ampscale + b0, st, true,
-                                                  src_sparse ? ws + L.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr)
+                                                  src_sparse ? ws + L.off_tilemap + orient_tilemap_bytes(p, b0) : nullptr, ws + L.off_layers)
                       : launch_sep_tc_prep((const float2 *)rho + (size_t)b0 * p.nvox, maxbits + b0, p, t.sep, nb, Rp, ws + L.off_flags, bounds,
                                            ampscale + b0, st, true);
             // stage X writes only the live 128-y tiles of H; stage Y reads whole slices: the rest must be zero

@@ -57,6 +57,7 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
 inline size_t orient_tilemap_bytes(const Plan &p, int batch) {
     return (size_t)batch * ((p.nz + 3) / 4) * ((p.ny + 3) / 4) * ((p.nx + 15) / 16);
 }
+inline size_t tile_layers_bytes(const Plan &p, int batch) { return (size_t)batch * ((p.nz + 3) / 4); }
 // the bound of max |rho~| per item that its extremes {max |delta|, max |beta|, max(0, -beta)} give (p.lambda, dz, nz, rho_mode)
 cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batch, unsigned *d_maxbits, cudaStream_t st);
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
@@ -98,7 +99,8 @@ cudaError_t launch_sep_tc_tables(const double *d_qx, int npx, const double *d_qy
 // max |rho~| per item (launch_prefix_bound).  Replaces launch_strength + launch_sep_tc_prep on the routes that only need the planes.
 cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                       __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
-                                      bool x_only = false, const unsigned char *d_tilemap = nullptr);   // d_tilemap: of these nb items (launch_orient)
+                                      bool x_only = false, const unsigned char *d_tilemap = nullptr,    // d_tilemap: of these nb items (launch_orient)
+                                      unsigned char *d_layer_live = nullptr);   // scratch, nb ceil(nz / 4) bytes: with a tile map, layers without a written tile are not packed
 cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
                                bool x_only = false);   // x_only: z-split bounds of stage X only (the NUFFT route)

@@ -163,6 +163,15 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // max |rho~| known before the prefix runs (prefix_bound_kernel).  One thread = one column (x, y) of one item, walking z, x fastest:
 // every slice access of a warp is 256 contiguous bytes in and 64 contiguous bytes per plane out; the loads of eight slices are in
 // flight before the (serial) FP64 chain of those slices starts.
+// layer_live[l] = any tile of layer l (four slices of one item) of the tile map was written
+__global__ void tile_layers_kernel(const unsigned char *__restrict__ tilemap, int tiles, unsigned char *__restrict__ layer_live) {
+    const unsigned char *t = tilemap + (size_t)blockIdx.x * tiles;
+    int any = 0;
+    for (int i = threadIdx.x; i < tiles; i += blockDim.x) any |= t[i];
+    any = __syncthreads_or(any);
+    if (threadIdx.x == 0) layer_live[blockIdx.x] = any ? 1 : 0;
+}
+
 constexpr int kPrefThreads = 128, kPrefStages = 3;
 template <int C> struct PrefVec;                       // C columns of (delta, beta) / of one FP16 plane
 template <> struct PrefVec<1> { using In = float2; using Out = unsigned short; };
@@ -173,7 +182,7 @@ template <int C>
 __global__ void __launch_bounds__(kPrefThreads, C == 1 ? 8 : 5)
 sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz1, int nb, int NY, int NXP, double kdz, int rho_mode,
                             const unsigned *__restrict__ maxbits, __half *__restrict__ R, unsigned char *__restrict__ flags,
-                            const unsigned char *__restrict__ tilemap) {
+                            const unsigned char *__restrict__ tilemap, const unsigned char *__restrict__ layer_live) {
     // The column's voxels reach the thread through a ring of cp.async stages in shared memory (every thread reads back only what it
     // copied itself: no barrier, only its own wait_group): two batches of slices are in flight while a third is worked on, and the
     // loop over the slices of a batch is NOT unrolled -- the unrolled register version (eight inlined FP64 sincos / exp) ran at
@@ -205,6 +214,9 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
     size_t tm_stride = 0;
     int tm_layer = -1, tm_layers = 0;
     unsigned char tm_cur = 1, tm_next = 1;
+    // ... and a layer of four slices none of whose tiles was written holds no material anywhere: its planes are not written either
+    // (no flag is raised for it, so no stage reads them)
+    const unsigned char *ll = layer_live ? layer_live + (size_t)b * ((nz1 + 3) / 4) : nullptr;
     if (tilemap && y < ny && x < nx) {
         const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4;
         tm_layers = (nz1 + 3) / 4;
@@ -245,17 +257,12 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
         ptx::cp_async_wait<2>();   // batch k has landed
         const int jn = min(kBatch, nz1 - k * kBatch);
         __half *dst = out + (size_t)(k * kBatch) * ostride;
-        float2 v[C], vn[C];
-#pragma unroll
-        for (int c = 0; c < C; ++c) vn[c] = ring[k % kPrefStages][0][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
+        float2 v[C];
 #pragma unroll 1
         for (int i = 0; i < jn; ++i, dst += ostride) {
+            if (ll && !__ldg(ll + ((k * kBatch + i) >> 2))) continue;
 #pragma unroll
-            for (int c = 0; c < C; ++c) v[c] = vn[c];
-            if (i + 1 < jn) {   // the next slice's values leave shared memory while this one is worked on
-#pragma unroll
-                for (int c = 0; c < C; ++c) vn[c] = ring[k % kPrefStages][i + 1][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
-            }
+            for (int c = 0; c < C; ++c) v[c] = ring[k % kPrefStages][i][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
             bool any = false;
 #pragma unroll
             for (int c = 0; c < C; ++c) any |= (v[c].x != 0.f) | (v[c].y != 0.f);
@@ -1042,19 +1049,25 @@ cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_
 
 cudaError_t launch_sep_tc_prefix_prep(const float2 *d_dn, const unsigned *d_maxbits, const Plan &p, const SepTcPlan &t, int nb,
                                       __half *d_Rp, unsigned char *d_flags64, int *d_bounds, float *d_ampscale, cudaStream_t st,
-                                      bool x_only, const unsigned char *d_tilemap) {
+                                      bool x_only, const unsigned char *d_tilemap, unsigned char *d_layer_live) {
     const int nyb = t.NY / kKB, nzt = p.nz * nb;
+    if (d_tilemap && d_layer_live) {
+        const int layers = nb * ((p.nz + 3) / 4), tiles = ((p.ny + 3) / 4) * ((p.nx + 15) / 16);
+        tile_layers_kernel<<<layers, 128, 0, st>>>(d_tilemap, tiles, d_layer_live);
+    } else {
+        d_layer_live = nullptr;
+    }
     cudaError_t e = cudaMemsetAsync(d_flags64, 0, (size_t)nzt * nyb, st);
     if (e != cudaSuccess) return e;
     const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
     if (p.nx % 2 == 0) {
         dim3 grid((unsigned)(((size_t)(t.NXP / 4) * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
         sep_tc_prefix_planes_kernel<4><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
-                                                                    d_Rp, d_flags64, d_tilemap);
+                                                                    d_Rp, d_flags64, d_tilemap, d_layer_live);
     } else {
         dim3 grid((unsigned)(((size_t)t.NXP * t.NY + kPrefThreads - 1) / kPrefThreads), (unsigned)nb);
         sep_tc_prefix_planes_kernel<1><<<grid, kPrefThreads, 0, st>>>(d_dn, p.nx, p.ny, p.nz, nb, t.NY, t.NXP, kdz, p.rho_mode, d_maxbits,
-                                                                    d_Rp, d_flags64, d_tilemap);
+                                                                    d_Rp, d_flags64, d_tilemap, d_layer_live);
     }
     sep_tc_scale_kernel<<<(nb + 127) / 128, 128, 0, st>>>(d_maxbits, nb, t.L, (float)(p.dx * p.dy * p.dz), d_ampscale);
     const int ngs = t.yz_stream ? 1 : t.ng, gw = t.yz_stream ? nyb : 2;
