@@ -22,7 +22,9 @@ SANITIZE = (
     "test_gpu_qgrid.py::test_wide_grids_use_narrower_stage_x_tiles", "test_gpu_qgrid.py::test_cfg1_sphere_on_a_uniform_q_grid",
     "test_gpu_qgrid.py::test_tile_parities_select_the_stage_yz_variants",
     "test_gpu_nufft.py::test_cfg1_sphere_full_pattern", "test_gpu_nufft.py::test_ragged_random_batch_with_orientations",
-    "test_gpu_nufft.py::test_empty_and_single_voxel",
+    "test_gpu_nufft.py::test_empty_and_single_voxel", "test_gpu_nufft.py::test_fused_prefix_pass_on_an_oriented_batch",
+    "test_gpu_qgrid.py::test_fused_prefix_pass_on_an_oriented_batch",
+    "test_gpu_render.py::test_shape_batches_large_enough_for_the_sparse_render_and_fused_prefix_pass",
     "test_gpu_render.py::test_ellipsoids_ragged_dims_random_orientations", "test_gpu_render.py::test_spherical_harmonics_droplets",
     "test_gpu_render.py::test_radial_maps", "test_gpu_render.py::test_volume_maps",
     "test_gpu_fitting.py::test_discrepancy_matches_oracle_over_several_chunks_and_a_ragged_tail",

@@ -149,6 +149,37 @@ def test_gain_medium_and_weak_items_keep_their_accuracy(sm, sim):
         assert_parity(I[b], O.simulate(g[b], voxel, lam, 21, 18, 30.0), what=f"nufft scale bound item {b}")
 
 
+def _fused_batch(nx, ny, nz, B_):
+    """20 grids whose chunk has more than 4 * 2^16 columns, so the tensor stages take the FUSED prefix -> planes pass (api.cu
+    fused_prefix_pays): sparse blobs, a gain medium, a weak item, an all-vacuum item; random orientations, one identity."""
+    g = np.stack([W.sparse_blobs_grid(700 + i, nx, ny, nz, nblobs=5, max_extent=30) for i in range(B_)])
+    g[3] = W.random_grid(703, nx, ny, nz, fill=0.4, delta=(-0.01, 0.03), beta=(-0.02, 0.0))      # gain
+    g[5] = W.random_grid(705, nx, ny, nz, fill=0.2, delta=(-1e-6, 1e-6), beta=(0.0, 1e-7))        # weak
+    g[7] = 0.0                                                                                    # vacuum
+    quat = W.random_quaternions(np.random.default_rng(77), B_)
+    quat[2] = [1, 0, 0, 0]
+    return g, quat
+
+
+@pytest.mark.parametrize("nx", [126, 125])
+def test_fused_prefix_pass_on_an_oriented_batch(sm, sim, nx):
+    """Orientation with SPARSE output + tile map, operand scale from the bound of max |rho~|, layers without material not packed,
+    four columns per thread (even N_x) or one (odd); ragged tiles in every dimension (126 = 7 tiles + 14, 22 = 5 layers + 2).
+    Items of every kind against the oracle; the all-vacuum item exactly 0."""
+    ny, nz, B_ = 120, 22, 20
+    g, quat = _fused_batch(nx, ny, nz, B_)
+    voxel, lam = (2.0, 2.0, 2.5), 12.0
+    npx, npy, th = 21, 18, 30.0
+    I = sim(dev(g), voxel, lam, npx, npy, th, quat=quat).cpu().numpy()
+    assert np.all(I[7] == 0)
+    for b in (0, 2, 3, 5, 11, 19):
+        assert_parity(I[b], O.simulate(g[b], voxel, lam, npx, npy, th, quat=quat[b]), what=f"nufft fused oriented batch item {b} nx={nx}")
+    # the same grids without orientation and without known extremes take strength + pack: both passes give the same patterns
+    I0 = sim(dev(g), voxel, lam, npx, npy, th).cpu().numpy()
+    assert_parity(I0[3], O.simulate(g[3], voxel, lam, npx, npy, th), what="nufft plain batch item 3")
+    assert np.allclose(I[2], I0[2], rtol=2e-4, atol=1e-6 * I0[2].max())      # item 2 has the identity orientation
+
+
 def test_empty_and_single_voxel(sm, sim):
     voxel, lam = (3.0, 3.0, 3.0), 12.0
     z = np.zeros((8, 8, 8, 2), np.float32)

@@ -54,6 +54,27 @@ def test_ragged_batch_with_orientations(sm, mode, method):
 
 
 @both_methods
+@pytest.mark.parametrize("nx", [126, 125])
+def test_fused_prefix_pass_on_an_oriented_batch(sm, method, nx):
+    """A batch whose chunk has more than 4 * 2^16 columns: the tensor stages take the fused prefix -> planes pass on the orientation's
+    sparse output (tile map, scale from the bound of max |rho~|, layers without material not packed); see test_gpu_nufft.py."""
+    ny, nz, B_ = 120, 22, 20
+    g = np.stack([W.sparse_blobs_grid(700 + i, nx, ny, nz, nblobs=5, max_extent=30) for i in range(B_)])
+    g[3] = W.random_grid(703, nx, ny, nz, fill=0.4, delta=(-0.01, 0.03), beta=(-0.02, 0.0))      # gain
+    g[5] = W.random_grid(705, nx, ny, nz, fill=0.2, delta=(-1e-6, 1e-6), beta=(0.0, 1e-7))        # weak
+    g[7] = 0.0                                                                                    # vacuum
+    quat = W.random_quaternions(np.random.default_rng(77), B_)
+    quat[2] = [1, 0, 0, 0]
+    voxel, lam = (2.0, 2.0, 2.5), 12.0
+    qx, qy = _uniform_q(lam, 30.0, 23), _uniform_q(lam, 25.0, 19)
+    I = sm.simulate_qgrid(dev(g), voxel, lam, dev(qx), dev(qy), quat=quat, method=METHODS[method]).cpu().numpy()
+    assert np.all(I[7] == 0)
+    for b in (0, 2, 3, 5, 11, 19):
+        ref = O.simulate_qgrid(g[b], voxel, lam, qx, qy, quat=quat[b])
+        assert_parity(I[b], ref, what=f"qgrid {method} fused oriented batch item {b} nx={nx}")
+
+
+@both_methods
 def test_sparse_blobs_and_evanescent_points(sm, method):
     """Mostly empty grid (the kernels skip vacuum rows); a q grid that runs past |q_xy| = k: those points must be exactly 0."""
     g = W.sparse_blobs_grid(91, 150, 130, 9, nblobs=6, max_extent=40)

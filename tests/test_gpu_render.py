@@ -208,6 +208,50 @@ def test_simulate_shapes_nufft_equals_render_then_nufft_and_matches_oracle(sm):
         assert_parity(I[i], ref, what=f"shapes nufft item {items[i]}")
 
 
+def test_shape_batches_large_enough_for_the_sparse_render_and_fused_prefix_pass(sm):
+    """24 shapes on 128 x 120 x 24 voxels: the chunk has more than 4 * 2^16 columns, so scatman_simulate_shapes_nufft / _qgrid render
+    SPARSELY (tiles outside the circumscribed sphere are neither written nor read: tile map) into a workspace that is poisoned
+    first, and the fused prefix pass packs the planes.  Equal (to FP32 summation order) to render -> simulate on dense grids, and
+    items of each kind against the oracle."""
+    import torch
+    rng = np.random.default_rng(401)
+    quats = W.random_quaternions(rng, 24)
+    shapes = []
+    for i in range(24):
+        if i % 3 == 0:
+            shapes.append({"kind": "ellipsoid", "delta": 0.01 + 0.001 * i, "beta": 0.002, "quat": quats[i],
+                           "a": 20.0 + 3 * i, "b": 16.0 + 2 * i, "c": 12.0 + i})
+        elif i % 3 == 1:
+            shapes.append({"kind": "spherical_harmonics", "delta": 0.02, "beta": 0.004, "quat": quats[i],
+                           "coeffs": _droplet_coeffs(rng, 25.0 + 2.5 * i, 4, 0.08)})
+        else:
+            shapes.append({"kind": "spherical_harmonics", "delta": 0.03, "beta": 0.0, "quat": quats[i],
+                           "coeffs": [(0, 0, (15.0 + 2 * i) * sqrt(4 * pi)), (10, 4, 6.0), (3, -1, 4.0)]})     # degree > 8: the triplet walker
+    shapes[5] = {"kind": "ellipsoid", "delta": 0.02, "beta": 0.001, "a": 0.4, "b": 0.4, "c": 0.4}      # smaller than a voxel, off every centre: vacuum
+    dims, vox, lam = (128, 120, 24), (2.0, 2.0, 2.5), 12.0
+    npx, npy, th = 21, 18, 30.0
+    g = sm.render(shapes, dims, vox)
+    # poison the caches of freed blocks: the sparse renderer must not depend on what its workspace held
+    junk = torch.full((64 << 20,), float("nan"), dtype=torch.float32, device="cuda")
+    del junk
+    I = sm.simulate_shapes_nufft(shapes, dims, vox, lam, npx, npy, th)
+    I2 = sm.simulate_nufft(g, vox, lam, npx, npy, th)
+    assert bool(torch.isfinite(I).all())
+    assert torch.allclose(I, I2, rtol=2e-4, atol=1e-6 * float(I2.max()))
+    assert float(I[5].abs().max()) == 0.0
+    In = I.cpu().numpy()
+    for i in (0, 1, 2, 23):
+        assert_parity(In[i], O.simulate(g[i].cpu().numpy(), vox, lam, npx, npy, th), what=f"sparse-rendered nufft item {i}")
+    k = 2 * np.pi / lam
+    qx = (np.arange(23) + 0.5 - 11.5) * (2 * k * np.sin(np.radians(30.0)) / 23)
+    qy = (np.arange(19) + 0.5 - 9.5) * (2 * k * np.sin(np.radians(25.0)) / 19)
+    dqx, dqy = torch.from_numpy(qx).cuda(), torch.from_numpy(qy).cuda()
+    J = sm.simulate_shapes_qgrid(shapes, dims, vox, lam, dqx, dqy)
+    J2 = sm.simulate_qgrid(g, vox, lam, dqx, dqy)
+    assert torch.allclose(J, J2, rtol=2e-4, atol=1e-6 * float(J2.max()))
+    assert_parity(J[1].cpu().numpy(), O.simulate_qgrid(g[1].cpu().numpy(), vox, lam, qx, qy), what="sparse-rendered qgrid item 1")
+
+
 def test_workload_shape_descriptors_describe_the_same_particles_as_the_grids(sm):
     """The descriptors of cfg1 / cfg3 (identity orientation) render to exactly the voxel grids the generators produce."""
     for idx, scale in ((0, 1.0), (2, 0.25)):
