@@ -732,7 +732,7 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             if (e == cudaSuccess)
                 e = launch_sep_tc_finalize((const float2 *)(ws + sp.off_partial), d_qx, npx, d_qy, npy, p, t, nb, ampscale + b0,
                                            d_I + (size_t)b0 * npx * npy, st);
-            nl += 6;
+            nl += 6 + (fused && src_sparse ? 1 : 0);   // pack | prefix, scale, bounds, stage X, stage YZ, finalize (+ the tile map's layer reduction)
             if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "qgrid stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         }
     } else {
@@ -1037,7 +1037,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             if (e == cudaSuccess)
                 e = launch_nufft_interp(p, L.n, nb, det->npx, det->npy, L.n.pixel_cells, q, U, ampscale + b0, ldexp(1.0, 1 + Ly),
                                         d_I + (size_t)b0 * p.npix, st);
-            nl += 8;
+            nl += 7 + (fused && src_sparse ? 1 : 0);   // pack | prefix, scale, bounds, stages X, Y, Z, interpolation (+ the tile map's layer reduction)
             if (e != cudaSuccess) return err.empty() ? cuda_fail(ctx, e, "nufft stages") : fail(ctx, SCATMAN_CUDA_ERROR, err);
         }
     } else {
