@@ -160,9 +160,8 @@ __global__ void sep_tc_pack_rho_kernel(const float2 *__restrict__ rho, int nx, i
 // Step a2 (Eq. 6/8/9) fused with the pack above: the exclusive z-prefix of strength_kernel (prep_kernels.cu: T_j
 // as a running FP64 product of the per-voxel factors exp(i k dz dn), the factor of the last (delta, beta) seen reused) writes the
 // scaled FP16 planes and the flags directly -- rho~ never goes to memory in FP32.  The scale 2^(13 - e) comes from an upper BOUND of
-// max |rho~| known before the prefix runs (prefix_bound_kernel).  One thread = one column (x, y) of one item, walking z, x fastest:
-// every slice access of a warp is 256 contiguous bytes in and 64 contiguous bytes per plane out; the loads of eight slices are in
-// flight before the (serial) FP64 chain of those slices starts.
+// max |rho~| known before the prefix runs (prefix_bound_kernel).  One thread = C adjacent columns (x .. x + C - 1, y) of one item,
+// walking z, x fastest (sep_tc_prefix_planes_kernel below).
 // layer_live[l] = any tile of layer l (four slices of one item) of the tile map was written
 __global__ void tile_layers_kernel(const unsigned char *__restrict__ tilemap, int tiles, unsigned char *__restrict__ layer_live) {
     const unsigned char *t = tilemap + (size_t)blockIdx.x * tiles;
