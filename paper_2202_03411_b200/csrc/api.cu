@@ -1029,7 +1029,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
             // (when a slice is a single 128-y tile, stage Y zeroes the rows of unwritten slices itself: no pass over the 2 GB of H)
             if (e == cudaSuccess && nufft_tc_needs_h_memset(t))
                 e = cudaMemsetAsync(Hp, 0, sizeof(__half) * 4 * (size_t)nb * p.nz * t.NPXP * t.NY, st);
-            if (e == cudaSuccess) e = launch_sep_tc_x(p, t.sep, Rp, Txp, ws + L.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err);
+            if (e == cudaSuccess) e = launch_sep_tc_x(p, t.sep, Rp, Txp, ws + L.off_flags, bounds, nb, Hp, ctx->num_sms, st, &err, L.n.ax.nq);
             SCATMAN_STAGE_CHECK(e, st, "nufft stage X");
             if (e == cudaSuccess) e = launch_nufft_tc_yz(p, L.n, t, nb, Hp, Typ, Tzp, Vp, U, ctx->num_sms, st, &err, ws + L.off_flags);
             SCATMAN_STAGE_CHECK(e, st, "nufft stages Y, Z");

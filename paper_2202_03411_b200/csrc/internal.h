@@ -106,7 +106,8 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
                                bool x_only = false);   // x_only: z-split bounds of stage X only (the NUFFT route)
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
                             const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
-                            cudaStream_t st, std::string *err);
+                            cudaStream_t st, std::string *err,
+                            int ncols = 0);   // > 0: only columns a < ncols of H are stored (nobody reads the padding)
 cudaError_t launch_sep_tc_yz(const Plan &p, const SepTcPlan &t, const __half *d_Eyp, const __half *d_Hp,
                              const unsigned char *d_flags64, const int *d_bounds, int nb, const double *d_qx, int npx,
                              const double *d_qy, int npy, float2 *d_partial, int num_sms, cudaStream_t st, std::string *err);

@@ -68,6 +68,7 @@ struct YParams {
     int nz, NZI;            // slices per item; the same padded to 8: item b's slices sit at [b NZI, b NZI + nz) of a V row, so
                             // that stage Z's TMA boxes start 16-byte aligned (a box start that is not raises an illegal-instruction fault)
     int NQYP, NZT;          // padded columns; row length of V (nb NZI)
+    int nqy;                // columns my < nqy are stored (stage Z reads no others)
     float hscale;           // accumulator -> stored V
     const unsigned char *flags;   // non-null (NY = 128 only): flags64[jg][2] of the separable pack; a slice with no flag set was not
                             // written by stage X at all -- its rows of H hold whatever was there and its rows of V are written as zeros
@@ -124,6 +125,7 @@ struct StageY {
             __half *dst = P.Vp + ((size_t)mx * P.NQYP + my0) * P.NZT + jv;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
+                if (my0 + i >= P.nqy) break;
                 __half h[4];
                 tcg::split4h(dead ? 0.f : __uint_as_float(gre[i]) * P.hscale, dead ? 0.f : __uint_as_float(gim[i]) * P.hscale, h);
                 __half *d = dst + (size_t)i * P.NZT;
@@ -310,6 +312,7 @@ cudaError_t launch_nufft_tc_yz(const Plan &p, const NufftPlan &n, const NufftTcP
     Y.nz = p.nz;
     Y.NZI = t.NZI;
     Y.NQYP = t.NQYP;
+    Y.nqy = n.ay.nq;
     Y.NZT = t.NZT;
     int Ly = 0;
     while ((1 << Ly) < p.ny) ++Ly;

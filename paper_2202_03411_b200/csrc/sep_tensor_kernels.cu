@@ -401,6 +401,7 @@ sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, 
 struct SepXParams {
     int nk;                                     // NXP / 64
     int nz, NY, NPXP, ng, nta, nsx, nkb;        // nta = tiles of 2 NX columns, nsx = z splits, nkb = NY / 64
+    int ncols;                                  // columns a < ncols are stored (the NUFFT route's stage Y reads no others)
     float hscale;                               // 2^(-9 - L): accumulator (2^10 sR H) -> stored H (sH H)
     const unsigned char *flags;                 // [nz][nkb]
     const int *zb;                              // [nsx + 1] balanced z split bounds (sep_tc_bounds_kernel)
@@ -453,16 +454,20 @@ struct SepXPolicy {
     struct Epilogue {
         __half *dst;
         size_t plane;
+        int ncol;            // columns of this thread's range that are stored
         __device__ void begin(const Params &P, const Item &, const tcg::EpiThread &) { plane = (size_t)P.nz * P.NPXP * P.NY; }
         __device__ void unit_begin(const Params &P, const Item &it, const tcg::EpiThread &et, int unit) {
             const int j = unit / P.ng, g = unit % P.ng;
             SCATMAN_ASSERT(j >= 0 && j < P.nz && it.ta * 2 * NX + et.col0 + NX <= P.NPXP && g * kM + kM <= P.NY);
             dst = P.Hp + ((size_t)j * P.NPXP + it.ta * 2 * NX + et.col0) * P.NY + g * kM + et.lane_row;
+            ncol = P.ncols - (it.ta * 2 * NX + et.col0);
         }
         __device__ __forceinline__ void columns(const Params &P, const Item &, const tcg::EpiThread &, int, int c0,
                                                 const uint32_t (&gre)[8], const uint32_t (&gim)[8]) {
+            if (c0 >= ncol) return;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
+                if (c0 + i >= ncol) break;
                 __half h[4];
                 split4(__uint_as_float(gre[i]) * P.hscale, __uint_as_float(gim[i]) * P.hscale, h);
                 __half *d = dst + (size_t)(c0 + i) * P.NY;
@@ -1093,7 +1098,7 @@ cudaError_t launch_sep_tc_prep(const float2 *d_rho, const unsigned *d_maxbits, c
 
 cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_Rp, const __half *d_Exp,
                             const unsigned char *d_flags64, const int *d_bounds, int nb, __half *d_Hp, int num_sms,
-                            cudaStream_t st, std::string *err) {
+                            cudaStream_t st, std::string *err, int ncols) {
     CUtensorMap tmA, tmB;
     bool ok;
     {   // streamed: the rho~ planes [4][slices NY][NXP], box = 64 x of a 128-row tile
@@ -1120,6 +1125,7 @@ cudaError_t launch_sep_tc_x(const Plan &p, const SepTcPlan &t, const __half *d_R
     P.nkb = t.NY / kKB;
     P.hscale = ldexpf(1.f, -9 - t.L);
     P.flags = d_flags64; P.zb = d_bounds; P.Hp = d_Hp;
+    P.ncols = ncols > 0 && ncols < t.NPXP ? ncols : t.NPXP;
     const int nitems = P.nta * P.nsx;
     switch (t.NX) {
         case 64: return tcg::cgemm_launch<SepXPolicy<64>>(tmA, tmB, P, nitems, num_sms, st);
