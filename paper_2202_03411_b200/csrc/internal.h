@@ -52,7 +52,7 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
                           cudaStream_t st, unsigned *d_stats = nullptr,   // d_stats[batch][3]: also the extremes of the input, FP32 bits
                           unsigned char *d_tilemap = nullptr);
 // d_tilemap = null: d_out is written everywhere.  Else SPARSE output: only the 16 x 4 x 4-voxel tiles that can hold material are
-// written, d_tilemap[b][ceil(nz/4)][ceil(ny/4)][ceil(nx/16)] says which (1) -- the rest of d_out is left as it was and must be read
+// written, and d_tilemap[b][ceil(nz/4)][ceil(ny/4)][ceil(nx/16)] = 1 for those of them that received material -- the rest of d_out is left as it was (or holds zeros) and must be read
 // as vacuum (launch_sep_tc_prefix_prep does)
 inline size_t orient_tilemap_bytes(const Plan &p, int batch) {
     return (size_t)batch * ((p.nz + 3) / 4) * ((p.ny + 3) / 4) * ((p.nx + 15) / 16);

@@ -141,7 +141,8 @@ __global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
 // are compacted (ballot); then the block resamples the live tiles -- a voxel's body-frame index is its tile's origin plus a
 // per-thread constant: no index division, no integer -> FP64 conversion (the XU pipe's 4 lanes per scheduler were the limit) --
 // and, for dense output, zero-fills the others with 16-byte stores.
-// tilemap != null: SPARSE output -- the other tiles are not written at all and tilemap[b][bz][tile] says which are (see internal.h).
+// tilemap != null: SPARSE output -- the other tiles are not written at all; tilemap[b][bz][tile] = 1 for the written tiles that received
+// material (see internal.h).
 // (One launch-sized block per tile, each loading the rotation and the box and deciding on its own, was bound by that start-up
 // latency, not by arithmetic or bytes: profiles/r02_orient_render.md.)
 __device__ __forceinline__ void floor_split(double f, int &i, double &t) {   // f = i + t, i = floor(f), |f| < 2^31: FP64 adds only
@@ -165,6 +166,7 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
     __shared__ int tile_off[256];          // offset of that voxel in its slice
     __shared__ unsigned char tile_ext[256];   // (extent - 1) of the tile along x | along y << 4 (ragged edges)
     __shared__ unsigned char hit[256];
+    __shared__ unsigned char occ[256];     // sparse output: the tile received a non-vacuum voxel
     __shared__ unsigned short live[256];   // the chunk's tiles that can hold material, in order
     __shared__ int wcount[8];
     if (threadIdx.x < 9) sR[threadIdx.x] = rotmat[9 * b + threadIdx.x];
@@ -224,9 +226,9 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                 }
                 tile_off[threadIdx.x] = by * 4 * nx + bx * 16;
                 tile_ext[threadIdx.x] = (unsigned char)(wx | (wy << 4));
-                if (tilemap) tilemap[((size_t)b * nbz + bz) * ((size_t)nbx * nby) + t] = h ? 1 : 0;
             }
             hit[threadIdx.x] = h ? 1 : 0;
+            occ[threadIdx.x] = 0;
             // compact the live tiles (ballot + warp counts): the resampling loop below visits only those
             const unsigned bal = __ballot_sync(0xffffffffu, h);
             if ((threadIdx.x & 31) == 0) wcount[threadIdx.x >> 5] = __popc(bal);
@@ -319,9 +321,14 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                     }
                 }
                 dstt[tile_off[tt]] = o;
+                if (tilemap && (o.x != 0.f || o.y != 0.f)) occ[tt] = 1;
             }
         }
         __syncthreads();
+        // the map says which tiles HOLD material, not merely which were written: the box test of phase 1 keeps about twice the tiles an
+        // ellipsoid touches, and the prefix pass then skips the rest (and the layers they leave empty) as well
+        if (tilemap && t0 + (int)threadIdx.x < ntile)
+            tilemap[((size_t)b * nbz + bz) * ((size_t)nbx * nby) + t0 + threadIdx.x] = occ[threadIdx.x];
     }
 }
 
