@@ -258,6 +258,15 @@ __device__ __forceinline__ void cp_async_16(void *smem_dst, const void *gmem_src
     const int n = valid ? 16 : 0;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(n) : "memory");
 }
+// the same with the destination as a shared-memory address
+__device__ __forceinline__ void cp_async_8s(uint32_t smem_dst, const void *gmem_src, bool valid) {
+    const int n = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_dst), "l"(gmem_src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_16s(uint32_t smem_dst, const void *gmem_src, bool valid) {
+    const int n = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gmem_src), "r"(n) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 

@@ -206,62 +206,73 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
     const int nkb = NY / kKB;
     unsigned char *fl = flags + (size_t)b * nz1 * nkb + y / kKB;
     const int nbatch = (nz1 + kBatch - 1) / kBatch;
-    // Sparse input (launch_orient with a tile map): tiles of 16 x 4 x 4 voxels that were not written are vacuum and are not read --
-    // the copy is issued with source size 0, which zero-fills.  The thread's C columns lie in one tile column; the map byte of the
+    // Sparse input (launch_orient / the renderer with a tile map): tiles of 16 x 4 x 4 voxels that hold no material are not read -- the
+    // copy is issued with source size 0, which zero-fills.  The thread's C columns lie in one tile column; the map byte of the
     // layer after the one being fetched is already in flight.
-    const unsigned char *tm = nullptr;
-    size_t tm_stride = 0;
-    int tm_layer = -1, tm_layers = 0;
-    unsigned char tm_cur = 1, tm_next = 1;
-    // ... and a layer of four slices none of whose tiles was written holds no material anywhere: its planes are not written either
-    // (no flag is raised for it, so no stage reads them)
+    // ... and a layer of four slices none of whose tiles holds material is not packed at all (no flag is raised for it, so no stage
+    // reads its planes).
     const unsigned char *ll = layer_live ? layer_live + (size_t)b * ((nz1 + 3) / 4) : nullptr;
-    if (tilemap && y < ny && x < nx) {
-        const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4;
-        tm_layers = (nz1 + 3) / 4;
+    const unsigned char *tmp = nullptr;      // map byte of the layer after the one being fetched
+    size_t tm_stride = 0;
+    unsigned char tm_cur = 1, tm_next = 1;
+    int tm_left = 0;                         // layers after the current one
+    bool okc[kCopies];                       // the copy's columns exist (C = 4: nx is even, a pair of columns is in or out as a whole)
+#pragma unroll
+    for (int c = 0; c < kCopies; ++c) okc[c] = y < ny && x + c * (C / kCopies) < nx;
+    if (tilemap && okc[0]) {
+        const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, layers = (nz1 + 3) / 4;
         tm_stride = (size_t)nbx * nby;
-        tm = tilemap + (size_t)b * tm_layers * tm_stride + (size_t)(y >> 2) * nbx + (x >> 4);
-        tm_next = __ldg(tm);
+        tmp = tilemap + (size_t)b * layers * tm_stride + (size_t)(y >> 2) * nbx + (x >> 4);
+        tm_next = __ldg(tmp);
+        tm_left = layers;
     }
-    auto fetch = [&](int k) {   // batch k -> stage k % kPrefStages; padding columns and slices past the end are zero-filled
-        if (k < nbatch) {
+    // running state of the copies: next slice, its address for this thread's first column, the ring stage it goes to
+    int fj = 0, fstage = 0;
+    const float2 *fsrc = src + x;
+    const uint32_t ring0 = (uint32_t)__cvta_generic_to_shared(&ring[0][0][0][threadIdx.x][0]);
+    constexpr uint32_t kCopyBytes = kPrefThreads * (C / kCopies) * 8, kSliceBytes = kCopies * kCopyBytes, kStageBytes = kBatch * kSliceBytes;
+    auto fetch = [&]() {   // the next batch -> the next stage; padding columns and slices past the end are zero-filled
 #pragma unroll
-            for (int i = 0; i < kBatch; ++i) {
-                const int j = k * kBatch + i;
-                if (tm && (j >> 2) != tm_layer && j < nz1) {
-                    tm_layer = j >> 2;
-                    tm_cur = tm_next;
-                    if (tm_layer + 1 < tm_layers) tm_next = __ldg(tm + (size_t)(tm_layer + 1) * tm_stride);
-                }
+        for (int i = 0; i < kBatch; ++i, ++fj, fsrc += sstride) {
+            if (fj >= nz1) break;
+            if (tmp && (fj & 3) == 0) {      // a new layer of tiles
+                tm_cur = tm_next;
+                --tm_left;
+                tmp += tm_stride;
+                if (tm_left > 0) tm_next = __ldg(tmp);
+            }
 #pragma unroll
-                for (int c = 0; c < kCopies; ++c) {
-                    const int xc = x + c * (C / kCopies);
-                    const bool ok = y < ny && xc < nx && j < nz1 && tm_cur;      // (C = 4: nx is even, a pair of columns is in or out as a whole)
-                    const float2 *g = src + (ok ? (size_t)j * sstride + xc : 0);
-                    if (C == 1) ptx::cp_async_8(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
-                    else ptx::cp_async_16(&ring[k % kPrefStages][i][c][threadIdx.x][0], g, ok);
-                }
+            for (int c = 0; c < kCopies; ++c) {
+                const bool ok = okc[c] && tm_cur;
+                const float2 *g = ok ? fsrc + c * (C / kCopies) : src;
+                const uint32_t d = ring0 + fstage * kStageBytes + i * kSliceBytes + c * kCopyBytes;
+                if (C == 1) ptx::cp_async_8s(d, g, ok);
+                else ptx::cp_async_16s(d, g, ok);
             }
         }
+        fstage = fstage + 1 == kPrefStages ? 0 : fstage + 1;
         ptx::cp_async_commit();   // (an empty group past the end keeps the wait counts uniform)
     };
-    fetch(0);
-    fetch(1);
+    fetch();
+    fetch();
     double Tre[C], Tim[C], gre[C], gim[C];
     float ld[C], lb[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) { Tre[c] = 1.0; Tim[c] = 0.0; gre[c] = 1.0; gim[c] = 0.0; ld[c] = lb[c] = 0.f; }
+    int pstage = 0;
+    __half *dst = out;
     for (int k = 0; k < nbatch; ++k) {
-        fetch(k + 2);
+        fetch();
         ptx::cp_async_wait<2>();   // batch k has landed
         const int jn = min(kBatch, nz1 - k * kBatch);
-        __half *dst = out + (size_t)(k * kBatch) * ostride;
+        const float2 *rs = &ring[pstage][0][0][threadIdx.x][0];
+        pstage = pstage + 1 == kPrefStages ? 0 : pstage + 1;
         float2 v[C];
 #pragma unroll 1
-        for (int i = 0; i < jn; ++i, dst += ostride) {
+        for (int i = 0; i < jn; ++i, dst += ostride, rs += kSliceBytes / 8) {
             if (ll && !__ldg(ll + ((k * kBatch + i) >> 2))) continue;
 #pragma unroll
-            for (int c = 0; c < C; ++c) v[c] = ring[k % kPrefStages][i][c / (C / kCopies)][threadIdx.x][c % (C / kCopies)];
+            for (int c = 0; c < C; ++c) v[c] = rs[(c / (C / kCopies)) * (kCopyBytes / 8) + c % (C / kCopies)];
             bool any = false;
 #pragma unroll
             for (int c = 0; c < C; ++c) any |= (v[c].x != 0.f) | (v[c].y != 0.f);
