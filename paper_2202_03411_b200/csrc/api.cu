@@ -113,7 +113,7 @@ static Plan make_plan(const scatman_grid &g, double lambda, int64_t npix, int ba
         p.off_zturn = take(sizeof(unsigned long long) * (size_t)p.ntiles * kTileP);
     }
     p.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
-    p.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
+    p.off_bbox = take(orient_scratch_bytes(p, batch));
     p.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     p.off_rho = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     p.off_max = take(sizeof(unsigned) * (size_t)batch);
@@ -436,7 +436,9 @@ static int run_path(scatman_ctx *ctx, const float *d_dn, const scatman_grid *gri
     if (h_quat && !all_identity(h_quat, batch)) {
         double *rm = (double *)(ws + p.off_rotmat);
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
-        if (e == cudaSuccess) e = launch_orient(d_dn, p, rm, batch, (float *)(ws + p.off_rot), (int *)(ws + p.off_bbox), st);
+        if (e == cudaSuccess)
+            e = launch_orient(d_dn, p, rm, batch, (float *)(ws + p.off_rot), (int *)(ws + p.off_bbox), st, nullptr, nullptr,
+                              orient_occ_ptr(ws + p.off_bbox, p, batch));
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + p.off_rot);
@@ -578,7 +580,7 @@ static SepPlan make_sep_plan(const scatman_grid &g, double lambda, int npx, int 
         sp.off_ey = take(sizeof(float2) * (size_t)g.ny * npy);
     }
     sp.off_rotmat = take(sizeof(double) * 9 * (size_t)batch);
-    sp.off_bbox = take(sizeof(int) * 6 * (size_t)batch);
+    sp.off_bbox = take(orient_scratch_bytes(p, batch));
     sp.off_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch);
     // FP32 rho~: always for the CUDA-core stages; for the tensor stages only where chunks are too small for the fused pass (when they
     // are not, strength + pack runs only on un-oriented input and borrows the orientation's buffer)
@@ -682,7 +684,7 @@ static int qgrid_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
         if (e == cudaSuccess)
             e = launch_orient(d_dn, p, rm, batch, (float *)(ws + sp.off_rot), (int *)(ws + sp.off_bbox), st,
-                              sp.fused_ok ? stats : nullptr, sp.fused_ok ? ws + sp.off_tilemap : nullptr);
+                              sp.fused_ok ? stats : nullptr, sp.fused_ok ? ws + sp.off_tilemap : nullptr, orient_occ_ptr(ws + sp.off_bbox, p, batch));
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + sp.off_rot);
@@ -879,7 +881,7 @@ static NufftLayout make_nufft_layout(const scatman_grid &g, double lambda, const
                          c = take(sizeof(__half) * 4 * (size_t)t.NQZP * t.NZP);
             if (mine) { L.off_txp = a; L.off_typ = b; L.off_tzp = c; }
         }
-        const size_t o_rm = take(sizeof(double) * 9 * (size_t)batch), o_bb = take(sizeof(int) * 6 * (size_t)batch),
+        const size_t o_rm = take(sizeof(double) * 9 * (size_t)batch), o_bb = take(orient_scratch_bytes(p, batch)),
                      o_rot = take(sizeof(float) * 2 * (size_t)p.nvox * batch),
                      o_rho = tensor && fused_prefix_pays(p, batch < L.tc.nb ? batch : L.tc.nb)   // see make_sep_plan
                                  ? o_rot : take(sizeof(float) * 2 * (size_t)p.nvox * batch),
@@ -983,7 +985,7 @@ static int nufft_impl(scatman_ctx *ctx, const float *d_dn, const scatman_grid *g
         e = upload_rotmats(h_quat, batch, rm, st, &nl);
         if (e == cudaSuccess)
             e = launch_orient(d_dn, p, rm, batch, (float *)(ws + L.off_rot), (int *)(ws + L.off_bbox), st,
-                              L.fused_ok ? stats : nullptr, L.fused_ok ? ws + L.off_tilemap : nullptr);
+                              L.fused_ok ? stats : nullptr, L.fused_ok ? ws + L.off_tilemap : nullptr, orient_occ_ptr(ws + L.off_bbox, p, batch));
         nl += 3;
         if (e != cudaSuccess) return cuda_fail(ctx, e, "orient");
         src = (const float *)(ws + L.off_rot);

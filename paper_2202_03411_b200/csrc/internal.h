@@ -50,7 +50,7 @@ void tensor_schedule(const Plan &p, int num_workers, int *nchunks, int *nzs);
 cudaError_t launch_qmap(const scatman_detector &det, double lambda, double *d_q, cudaStream_t st);
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
                           cudaStream_t st, unsigned *d_stats = nullptr,   // d_stats[batch][3]: also the extremes of the input, FP32 bits
-                          unsigned char *d_tilemap = nullptr);
+                          unsigned char *d_tilemap = nullptr, unsigned char *d_occ = nullptr);   // d_occ: orient_occ_bytes() of scratch (coarse occupancy map)
 // d_tilemap = null: d_out is written everywhere.  Else SPARSE output: only the 16 x 4 x 4-voxel tiles that can hold material are
 // written, and d_tilemap[b][ceil(nz/4)][ceil(ny/4)][ceil(nx/16)] = 1 for those of them that received material -- the rest of d_out is left as it was (or holds zeros) and must be read
 // as vacuum (launch_sep_tc_prefix_prep does)
@@ -58,6 +58,18 @@ inline size_t orient_tilemap_bytes(const Plan &p, int batch) {
     return (size_t)batch * ((p.nz + 3) / 4) * ((p.ny + 3) / 4) * ((p.nx + 15) / 16);
 }
 inline size_t tile_layers_bytes(const Plan &p, int batch) { return (size_t)batch * ((p.nz + 3) / 4); }
+// bbox_kernel's coarse occupancy map for orient_kernel (4^3-voxel blocks); 0 = not used (a slice's map must fit 4 KB of shared memory)
+inline size_t orient_occ_bytes(const Plan &p, int batch) {
+    const size_t sl = (size_t)(p.nx / 4 + 1) * (p.ny / 4 + 1);
+    return sl <= 4096 ? (size_t)batch * (p.nz / 4 + 1) * sl : 0;
+}
+// a0's scratch: the boxes [batch][6] followed by the occupancy map
+inline size_t orient_scratch_bytes(const Plan &p, int batch) {
+    return (sizeof(int) * 6 * (size_t)batch + 255) / 256 * 256 + orient_occ_bytes(p, batch);
+}
+inline unsigned char *orient_occ_ptr(void *d_bbox, const Plan &p, int batch) {
+    return orient_occ_bytes(p, batch) ? (unsigned char *)d_bbox + (sizeof(int) * 6 * (size_t)batch + 255) / 256 * 256 : nullptr;
+}
 // the bound of max |rho~| per item that its extremes {max |delta|, max |beta|, max(0, -beta)} give (p.lambda, dz, nz, rho_mode)
 cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batch, unsigned *d_maxbits, cudaStream_t st);
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,

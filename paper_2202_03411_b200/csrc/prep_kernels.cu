@@ -60,9 +60,20 @@ struct Extremes {
     }
 };
 
+// occ != null: also a coarse occupancy map for orient_kernel, occ[b][nz/4 + 1][ny/4 + 1][nx/4 + 1] bytes: byte (p >> 2) of every axis is
+// set for p = m and p = m + 1 of every non-vacuum voxel m, so that the 2x2x2 interpolation cell with first corner c holds material
+// only if the byte of (c + 1) >> 2 is set -- one cached byte instead of eight gathered corners for the vacuum inside the box.
+constexpr int kOccSliceCap = 4096;   // bytes of a slice's map in shared memory (grids up to ~250 x 250)
 __global__ void __launch_bounds__(256)
-bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox, unsigned *__restrict__ stats) {
+bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restrict__ bbox, unsigned *__restrict__ stats,
+            unsigned char *__restrict__ occ) {
     const int iz = blockIdx.x % nz, b = blockIdx.x / nz;
+    __shared__ unsigned char socc[kOccSliceCap];
+    const int nbx8 = nx / 4 + 1, nby8 = ny / 4 + 1;
+    if (occ) {
+        for (int i = threadIdx.x; i < nbx8 * nby8; i += 256) socc[i] = 0;
+        __syncthreads();
+    }
     const float2 *src = in + ((size_t)b * nz + iz) * (size_t)nx * ny;
     int x0 = 0x7fffffff, y0 = 0x7fffffff, x1 = -1, y1 = -1;
     Extremes ex;
@@ -73,6 +84,12 @@ bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restri
         const int x = e % nx, y = e / nx;
         x0 = min(x0, x); x1 = max(x1, x);
         y0 = min(y0, y); y1 = max(y1, y);
+        if (occ) {
+            const int xa = x >> 2, xb = (x + 1) >> 2, ya = (y >> 2) * nbx8, yb = ((y + 1) >> 2) * nbx8;
+            socc[ya + xa] = 1;
+            if (xb != xa) socc[ya + xb] = 1;
+            if (yb != ya) { socc[yb + xa] = 1; if (xb != xa) socc[yb + xb] = 1; }
+        }
     };
     if ((n & 1) == 0) {
         const float4 *src4 = (const float4 *)src;
@@ -125,6 +142,15 @@ bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restri
             if (stats) ex.store(stats + 3 * b);
         }
     }
+    if (occ) {   // (the block barrier above orders the slice map)
+        const int za = iz >> 2, zb = (iz + 1) >> 2;
+        unsigned char *o = occ + (size_t)b * (nz / 4 + 1) * nby8 * nbx8;
+        for (int i = threadIdx.x; i < nbx8 * nby8; i += 256)
+            if (socc[i]) {
+                o[(size_t)za * nby8 * nbx8 + i] = 1;
+                if (zb != za) o[(size_t)zb * nby8 * nbx8 + i] = 1;
+            }
+    }
 }
 
 __global__ void bbox_init_kernel(int *__restrict__ bbox, int n) {
@@ -156,7 +182,8 @@ __device__ __forceinline__ void floor_split(double f, int &i, double &t) {   // 
 
 __global__ void __launch_bounds__(256, 4)   // 64 registers: four CTAs per SM (at 100 registers two CTAs left the issue slots half empty)
 orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, double dy, double dz, double3 inv,
-              const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out, unsigned char *__restrict__ tilemap) {
+              const double *__restrict__ rotmat, const int *__restrict__ bbox, float2 *__restrict__ out, unsigned char *__restrict__ tilemap,
+              const unsigned char *__restrict__ occ8) {
     const int nbx = (nx + 15) / 16, nby = (ny + 3) / 4, nbz = (nz + 3) / 4;
     const int bz = blockIdx.x % nbz, b = blockIdx.x / nbz;
     __shared__ double sR[9];
@@ -196,6 +223,8 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
     const int wz = min(3, nz - 1 - bz * 4);                         // tile extent - 1 along z
     const bool empty = sbb[3] < 0;                                  // an all-vacuum item
     const float2 *src = in + (size_t)b * nx * ny * nz;
+    const int nbx8 = nx / 4 + 1, nby8 = ny / 4 + 1;
+    const unsigned char *occb = occ8 ? occ8 + (size_t)b * (nz / 4 + 1) * nby8 * nbx8 : nullptr;   // bbox_kernel's coarse occupancy map
     float2 *dstb = out + (size_t)b * nx * ny * nz;
     float2 *dstt = dstb + ((size_t)iz * ny + ly) * nx + lx;         // + tile_off
     // this thread's voxel relative to its tile's first one, in body-frame index units
@@ -213,6 +242,7 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                 const int bx = t % nbx, by = t / nbx;
                 const int wx = min(15, nx - 1 - bx * 16), wy = min(3, ny - 1 - by * 4);
                 h = !empty;
+                int qlo[3], qhi[3];
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
                     const double f0 = sE[9 + d] + (double)(bx * 16) * ex[d] + (double)(by * 4) * ey[d] + (double)(bz * 4) * ez[d];
@@ -223,6 +253,19 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                     // the per-voxel test below is f > bb_lo - 1 && f < bb_hi + 1; a slack of 1e-9 voxels covers the rounding of this
                     // bound against the per-voxel evaluation (a wrongly kept tile only costs time)
                     if (hi <= sbd[d] - 1e-9 || lo >= sbd[3 + d] + 1e-9) h = false;
+                    // blocks of the coarse occupancy map that the first corners of the tile's cells fall into (slack as above)
+                    const int nd = d == 0 ? nx : d == 1 ? ny : nz;
+                    qlo[d] = max(0, (int)floor(lo - 1e-9) + 1) >> 2;
+                    qhi[d] = min(nd, (int)floor(hi + 1e-9) + 1) >> 2;
+                }
+                if (h && occb) {   // no occupied block among them: no cell of the tile holds material
+                    bool any = false;
+                    for (int qz = qlo[2]; qz <= qhi[2] && !any; ++qz)
+                        for (int qy = qlo[1]; qy <= qhi[1] && !any; ++qy) {
+                            const unsigned char *row = occb + ((size_t)qz * nby8 + qy) * nbx8;
+                            for (int qx = qlo[0]; qx <= qhi[0]; ++qx) any |= row[qx] != 0;
+                        }
+                    h = any;
                 }
                 tile_off[threadIdx.x] = by * 4 * nx + bx * 16;
                 tile_ext[threadIdx.x] = (unsigned char)(wx | (wy << 4));
@@ -275,6 +318,11 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                     floor_split(fx, x0, tx);
                     floor_split(fy, y0, ty);
                     floor_split(fz, z0, tz);
+                    // the coarse map says whether the cell can hold material at all (z0 + 1 etc. lie in [0, n]: the box test above)
+                    if (occb && !occb[(((z0 + 1) >> 2) * nby8 + ((y0 + 1) >> 2)) * nbx8 + ((x0 + 1) >> 2)]) {
+                        dstt[tile_off[tt]] = o;
+                        continue;
+                    }
                     // Interior of the cell grid (the usual case): the eight corners without bounds tests.  If they all hold the same value
                     // -- deep inside a homogeneous particle, or in the vacuum around it -- the interpolated value IS that value (the
                     // weights sum to 1 within 1e-16, far below half an FP32 ulp), bit for bit what the weighted sum rounds to: skip it.
@@ -354,7 +402,7 @@ cudaError_t launch_prefix_bound(const unsigned *d_stats, const Plan &p, int batc
 }
 
 cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotmat, int batch, float *d_out, int *d_bbox,
-                          cudaStream_t st, unsigned *d_stats, unsigned char *d_tilemap) {
+                          cudaStream_t st, unsigned *d_stats, unsigned char *d_tilemap, unsigned char *d_occ) {
     if (d_stats) {   // extremes of the body-frame grids: the trilinear samples of the beam-frame grid lie within them
         cudaError_t e = cudaMemsetAsync(d_stats, 0, sizeof(unsigned) * 3 * (size_t)batch, st);
         if (e != cudaSuccess) return e;
@@ -362,7 +410,12 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
     const size_t blocks = (size_t)((p.nz + 3) / 4) * batch;     // one block per layer of 16 x 4 x 4 tiles
     if (blocks > 0x7fffffffull || (size_t)p.nz * batch > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     bbox_init_kernel<<<(6 * batch + 255) / 256, 256, 0, st>>>(d_bbox, 6 * batch);
-    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats);
+    if (d_occ && orient_occ_bytes(p, batch) == 0) d_occ = nullptr;   // a slice's map does not fit shared memory
+    if (d_occ) {
+        cudaError_t e = cudaMemsetAsync(d_occ, 0, orient_occ_bytes(p, batch), st);
+        if (e != cudaSuccess) return e;
+    }
+    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats, d_occ);
     // four resident blocks per SM; at least 16 tiles per block
     const int ntile = ((p.nx + 15) / 16) * ((p.ny + 3) / 4);
     int nsplit = (int)((4 * 148 + blocks - 1) / blocks);
@@ -370,7 +423,7 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
     if (nsplit < 1) nsplit = 1;
     orient_kernel<<<dim3((unsigned)blocks, (unsigned)nsplit), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
                                                    make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
-                                                   (float2 *)d_out, d_tilemap);
+                                                   (float2 *)d_out, d_tilemap, d_occ);
     return cudaGetLastError();
 }
 
