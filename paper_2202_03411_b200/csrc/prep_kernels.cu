@@ -259,13 +259,13 @@ orient_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, double dx, 
                     qhi[d] = min(nd, (int)floor(hi + 1e-9) + 1) >> 2;
                 }
                 if (h && occb) {   // no occupied block among them: no cell of the tile holds material
-                    bool any = false;
-                    for (int qz = qlo[2]; qz <= qhi[2] && !any; ++qz)
-                        for (int qy = qlo[1]; qy <= qhi[1] && !any; ++qy) {
+                    unsigned any = 0;      // (no early exit: the loads are independent and stay in flight together)
+                    for (int qz = qlo[2]; qz <= qhi[2]; ++qz)
+                        for (int qy = qlo[1]; qy <= qhi[1]; ++qy) {
                             const unsigned char *row = occb + ((size_t)qz * nby8 + qy) * nbx8;
-                            for (int qx = qlo[0]; qx <= qhi[0]; ++qx) any |= row[qx] != 0;
+                            for (int qx = qlo[0]; qx <= qhi[0]; ++qx) any |= __ldg(row + qx);
                         }
-                    h = any;
+                    h = any != 0;
                 }
                 tile_off[threadIdx.x] = by * 4 * nx + bx * 16;
                 tile_ext[threadIdx.x] = (unsigned char)(wx | (wy << 4));
@@ -410,17 +410,18 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
     const size_t blocks = (size_t)((p.nz + 3) / 4) * batch;     // one block per layer of 16 x 4 x 4 tiles
     if (blocks > 0x7fffffffull || (size_t)p.nz * batch > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     bbox_init_kernel<<<(6 * batch + 255) / 256, 256, 0, st>>>(d_bbox, 6 * batch);
-    if (d_occ && orient_occ_bytes(p, batch) == 0) d_occ = nullptr;   // a slice's map does not fit shared memory
-    if (d_occ) {
-        cudaError_t e = cudaMemsetAsync(d_occ, 0, orient_occ_bytes(p, batch), st);
-        if (e != cudaSuccess) return e;
-    }
-    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats, d_occ);
     // four resident blocks per SM; at least 16 tiles per block
     const int ntile = ((p.nx + 15) / 16) * ((p.ny + 3) / 4);
     int nsplit = (int)((4 * 148 + blocks - 1) / blocks);
     if (nsplit > ntile / 16) nsplit = ntile / 16;
     if (nsplit < 1) nsplit = 1;
+    if (d_occ && orient_occ_bytes(p, batch) == 0) d_occ = nullptr;   // a slice's map does not fit shared memory
+    if (nsplit > 1) d_occ = nullptr;   // single grids: the map's extra memset and look-ups cost the ~8 us they save on batches per item
+    if (d_occ) {
+        cudaError_t e = cudaMemsetAsync(d_occ, 0, orient_occ_bytes(p, batch), st);
+        if (e != cudaSuccess) return e;
+    }
+    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats, d_occ);
     orient_kernel<<<dim3((unsigned)blocks, (unsigned)nsplit), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
                                                    make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
                                                    (float2 *)d_out, d_tilemap, d_occ);
