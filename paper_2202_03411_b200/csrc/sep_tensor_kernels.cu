@@ -331,11 +331,11 @@ sep_tc_prefix_planes_kernel(const float2 *__restrict__ dn, int nx, int ny, int n
 // its live 64-y blocks of that group.  bounds[seq][0..ns] cut [0, nz) into ns ranges of (almost) equal total weight, so that
 // every work item of a stage carries the same number of live tiles whatever the particle's extent along the beam:
 // bounds[s] = min { j in [0, nz] : E(j) >= target(s) }, E(j) = weight of the slices before j, target(s) = floor(total s / ns).
-// One block of 256 threads per sequence: every thread sums a contiguous run of slices (all flag loads of the block are in
+// One block of 1024 threads per sequence: every thread sums a contiguous run of slices (all flag loads of the block are in
 // flight together), a block scan gives E at the run starts, and each thread then places the bounds that fall into its run.
 // sequence 0: stage X over all nzt slices of the chunk; sequence 1 + b ngs + g: stage YZ of item b, group g (its nz1 slices).
 // Bounds are GLOBAL slice indices (jbase + j).  nyz_seq = 0 skips the stage YZ sequences (the NUFFT route needs only stage X's).
-constexpr int kBoundsThreads = 256;
+constexpr int kBoundsThreads = 1024;
 __global__ void __launch_bounds__(kBoundsThreads)
 sep_tc_bounds_kernel(const unsigned char *__restrict__ flags, int nz1, int nzt, int nkb, int ng, int ngs, int gw,
                      int nsx, int nzs, int *__restrict__ bx, int *__restrict__ by) {   // ngs YZ groups of gw flags
