@@ -1117,7 +1117,7 @@ int scatman_discrepancy(scatman_ctx *ctx, const float *d_I, const float *d_M, in
     cudaSetDevice(ctx->device);
     cudaError_t e = launch_discrepancy(d_I, d_M, m_stride, d_mask, npix, batch, metric, (double *)d_ws, d_out,
                                        (cudaStream_t)cuda_stream);
-    ctx->last_launches = 4;
+    ctx->last_launches = fit_discrepancy_launches(npix, batch);
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "discrepancy");
 }
 
@@ -1140,7 +1140,7 @@ int scatman_discrepancy_static(scatman_ctx *ctx, const float *d_I, const float *
     cudaSetDevice(ctx->device);
     // every word of the scratch that is read (partials, sums) is written first by this call's own kernels: nothing to clear
     cudaError_t e = launch_discrepancy(d_I, d_M, m_stride, d_mask, npix, batch, metric, ctx->fit_static, d_out, (cudaStream_t)cuda_stream);
-    ctx->last_launches = 4;
+    ctx->last_launches = fit_discrepancy_launches(npix, batch);
     return e == cudaSuccess ? SCATMAN_OK : cuda_fail(ctx, e, "discrepancy (static scratch)");
 }
 

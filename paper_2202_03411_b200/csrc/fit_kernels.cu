@@ -16,7 +16,7 @@ namespace scatman {
 namespace {
 
 constexpr int kFitThreads = 256;
-constexpr int kFitChunk = 32768;  // pixels per block
+constexpr int kFitChunk = 32768;  // pixels per block, fewer for problems that would not fill the GPU (fit_chunk)
 
 __device__ __forceinline__ double block_sum(double v, double *s_red) {
     for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
@@ -29,38 +29,64 @@ __device__ __forceinline__ double block_sum(double v, double *s_red) {
     return t;   // valid in thread 0
 }
 
+// One load slot of a thread: G consecutive pixels (4 as one 16-byte load of each pattern and one 4-byte load of the mask when
+// the pixel count, the stride of M and the three addresses allow it, else 1).  The loads of a slot do not wait for one another.
+template <bool kVec>
+struct FitSlot {
+    static constexpr int G = kVec ? 4 : 1;
+    float i[G], m[G];
+    bool on[G];
+    __device__ __forceinline__ void load(const float *Ib, const float *Mb, const unsigned char *mask, int64_t p, bool in) {
+        if constexpr (kVec) {
+            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 vi = in ? __ldg((const float4 *)(Ib + p)) : z;
+            const float4 vm = in && Mb ? __ldg((const float4 *)(Mb + p)) : z;
+            const unsigned w = in ? (mask ? __ldg((const unsigned *)(mask + p)) : 0x01010101u) : 0u;
+            i[0] = vi.x, i[1] = vi.y, i[2] = vi.z, i[3] = vi.w;
+            m[0] = vm.x, m[1] = vm.y, m[2] = vm.z, m[3] = vm.w;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) on[j] = ((w >> (8 * j)) & 0xffu) != 0u;
+        } else {
+            const unsigned char w = in ? (mask ? mask[p] : (unsigned char)1) : (unsigned char)0;
+            i[0] = in ? Ib[p] : 0.f;
+            m[0] = in && Mb ? Mb[p] : 0.f;
+            on[0] = w != 0;
+        }
+    }
+};
+
 }  // namespace
 
 // pass 1: partial[b][chunk][5] = sums over the chunk of w I, w M, w I^2, w M^2, w I M
-__global__ void __launch_bounds__(kFitThreads) fit_sums_kernel(const float *__restrict__ I, const float *__restrict__ M,
+template <bool kVec>
+__global__ void __launch_bounds__(kFitThreads, 4) fit_sums_kernel(const float *__restrict__ I, const float *__restrict__ M,
                                                                int64_t m_stride, const unsigned char *__restrict__ mask,
-                                                               int64_t npix, int nchunk, double *__restrict__ partial) {
+                                                               int64_t npix, int nchunk, int chunk_px, double *__restrict__ partial) {
     __shared__ double s_red[5 * kFitThreads / 32];
     const int b = blockIdx.y, chunk = blockIdx.x;
     const float *Ib = I + (size_t)b * npix;
     const float *Mb = M ? M + (size_t)b * m_stride : nullptr;
     double a[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    const int64_t p1 = min((int64_t)(chunk + 1) * kFitChunk, npix);
-    for (int64_t p0 = (int64_t)chunk * kFitChunk + threadIdx.x; p0 < p1; p0 += 4 * kFitThreads) {
-        float fi[4], fm[4];
+    const int64_t p1 = min((int64_t)(chunk + 1) * chunk_px, npix);
+    constexpr int G = FitSlot<kVec>::G;
+    for (int64_t p0 = (int64_t)chunk * chunk_px + threadIdx.x * G; p0 < p1; p0 += 4 * kFitThreads * G) {
+        FitSlot<kVec> s[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {   // four independent loads in flight per thread
-            const int64_t p = p0 + k * kFitThreads;
-            const bool in = p < p1;   // the three loads do not wait for one another; the mask is applied afterwards
-            const unsigned char w = in ? (mask ? mask[p] : (unsigned char)1) : (unsigned char)0;
-            const float vi = in ? Ib[p] : 0.f, vm = in && Mb ? Mb[p] : 0.f;
-            fi[k] = w ? vi : 0.f;
-            fm[k] = w ? vm : 0.f;
+        for (int k = 0; k < 4; ++k) {   // four independent slots in flight per thread; the mask is applied afterwards
+            const int64_t p = p0 + k * kFitThreads * G;
+            s[k].load(Ib, Mb, mask, p, p < p1);
         }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const double i = (double)fi[k], m = (double)fm[k];
-            a[0] += i;
-            a[1] += m;
-            a[2] += i * i;
-            a[3] += m * m;
-            a[4] += i * m;
-        }
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int j = 0; j < G; ++j) {
+                const double i = s[k].on[j] ? (double)s[k].i[j] : 0.0, m = s[k].on[j] ? (double)s[k].m[j] : 0.0;
+                a[0] += i;
+                a[1] += m;
+                a[2] += i * i;
+                a[3] += m * m;
+                a[4] += i * m;
+            }
     }
     // the five sums through one shared-memory stage
 #pragma unroll
@@ -90,41 +116,56 @@ __global__ void fit_reduce_kernel(const double *__restrict__ partial, int nchunk
 // L2: D = sum w (I / S_I - M / S_M)^2 = S_II / S_I^2 - 2 S_IM / (S_I S_M) + S_MM / S_M^2 would cancel catastrophically
 // for close patterns, so the squared differences are summed directly in a second pass (same cost: HBM-bound).
 // metric 0: w (I / S_I - M / S_M)^2; metric 1: 2 w [M log(M / (c I)) - (M - c I)], c = S_M / S_I
-__global__ void __launch_bounds__(kFitThreads) fit_metric_kernel(const float *__restrict__ I, const float *__restrict__ M,
+template <bool kVec>
+__global__ void __launch_bounds__(kFitThreads, 3) fit_metric_kernel(const float *__restrict__ I, const float *__restrict__ M,
                                                                  int64_t m_stride, const unsigned char *__restrict__ mask,
-                                                                 int64_t npix, int nchunk, int metric,
-                                                                 const double *__restrict__ sums, double *__restrict__ partial) {
+                                                                 int64_t npix, int nchunk, int chunk_px, int metric,
+                                                                 const double *__restrict__ sums,
+                                                                 const double *__restrict__ partial1, double *__restrict__ partial) {
     __shared__ double s_red[kFitThreads / 32];
     const int b = blockIdx.y, chunk = blockIdx.x;
     const float *Ib = I + (size_t)b * npix;
     const float *Mb = M + (size_t)b * m_stride;
-    const double SI = sums[b * 5 + 0], SM = sums[b * 5 + 1];
+    double SI, SM;
+    if (partial1) {   // few chunks per item: every block adds pass 1's partial sums itself, in fit_reduce_kernel's order
+        SI = 0.0, SM = 0.0;
+        for (int c1 = 0; c1 < nchunk; ++c1) {
+            SI += partial1[((size_t)b * nchunk + c1) * 5 + 0];
+            SM += partial1[((size_t)b * nchunk + c1) * 5 + 1];
+        }
+    } else {
+        SI = sums[b * 5 + 0], SM = sums[b * 5 + 1];
+    }
     const double c = SM / SI, rSI = 1.0 / SI, rSM = 1.0 / SM;
     double acc = 0.0;
-    const int64_t p1 = min((int64_t)(chunk + 1) * kFitChunk, npix);
-    for (int64_t p0 = (int64_t)chunk * kFitChunk + threadIdx.x; p0 < p1; p0 += 4 * kFitThreads) {
-        float fi[4], fm[4];
-        bool on[4];
+    const int64_t p1 = min((int64_t)(chunk + 1) * chunk_px, npix);
+    constexpr int G = FitSlot<kVec>::G;
+    for (int64_t p0 = (int64_t)chunk * chunk_px + threadIdx.x * G; p0 < p1; p0 += 4 * kFitThreads * G) {
+        FitSlot<kVec> s[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            const int64_t p = p0 + k * kFitThreads;
-            const bool in = p < p1;
-            const unsigned char w = in ? (mask ? mask[p] : (unsigned char)1) : (unsigned char)0;
-            fi[k] = in ? Ib[p] : 0.f;
-            fm[k] = in ? Mb[p] : 0.f;
-            on[k] = w != 0;
+            const int64_t p = p0 + k * kFitThreads * G;
+            s[k].load(Ib, Mb, mask, p, p < p1);
         }
+        if (metric == SCATMAN_LOSS_L2_NORMALISED) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (!on[k]) continue;
-            const double i = (double)fi[k], m = (double)fm[k];
-            if (metric == SCATMAN_LOSS_L2_NORMALISED) {
-                const double d = __dmul_rn(i, rSI) - __dmul_rn(m, rSM);   // no FMA contraction: identical patterns give exactly 0
-                acc += d * d;
-            } else {
-                const double mu = c * i;
-                acc += 2.0 * ((m > 0.0 ? m * log(m / mu) : 0.0) - (m - mu));
-            }
+            for (int k = 0; k < 4; ++k)
+#pragma unroll
+                for (int j = 0; j < G; ++j) {
+                    // no FMA contraction: identical patterns give exactly 0; a masked pixel adds an exact 0
+                    const double d = __dmul_rn((double)s[k].i[j], rSI) - __dmul_rn((double)s[k].m[j], rSM);
+                    acc += s[k].on[j] ? d * d : 0.0;
+                }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+#pragma unroll
+                for (int j = 0; j < G; ++j) {
+                    if (!s[k].on[j]) continue;
+                    const double i = (double)s[k].i[j], m = (double)s[k].m[j];
+                    const double mu = c * i;
+                    acc += 2.0 * ((m > 0.0 ? m * log(m / mu) : 0.0) - (m - mu));
+                }
         }
     }
     const double t = block_sum(acc, s_red);
@@ -206,11 +247,25 @@ __global__ void store_photons_kernel(PhotonChunk c, int n, double *__restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------------ host
-int fit_nchunk(int64_t npix) { return (int)((npix + kFitChunk - 1) / kFitChunk); }
+// Pixels per block: 32768, but a block walks its chunk in steps of one load round trip each, so a problem with few such
+// chunks (256 patterns of 256^2 pixels: 512) would run as one and a bit waves of long blocks.  Below four waves of blocks
+// (148 SMs x 3 blocks) the chunk shrinks to 8192, then to 2048 (one step of a block).  The scratch stays below 512 KB there,
+// so nothing that fitted the static array (scatman_discrepancy_static) with 32768-pixel chunks stops fitting.
+int fit_chunk(int64_t npix, int batch) {
+    const int64_t enough = 4 * 148 * 3;
+    int chunk = kFitChunk;
+    while (chunk > 2048 && (int64_t)batch * ((npix + chunk - 1) / chunk) < enough) chunk /= 4;
+    return chunk;
+}
+
+int fit_nchunk(int64_t npix, int batch) {
+    const int chunk = fit_chunk(npix, batch);
+    return (int)((npix + chunk - 1) / chunk);
+}
 
 size_t fit_workspace_bytes(int64_t npix, int batch) {
     // partial[b][nchunk][5] + sums[b][5] + partial2[b][nchunk] + photons[b]
-    return sizeof(double) * ((size_t)batch * fit_nchunk(npix) * 6 + (size_t)batch * 6);
+    return sizeof(double) * ((size_t)batch * fit_nchunk(npix, batch) * 6 + (size_t)batch * 6);
 }
 
 // ---- static scratch (scatman_discrepancy_static) ----------------------------------------------------------------------
@@ -237,22 +292,41 @@ cudaError_t fit_static_scratch(int device, double **d_ptr) {
     return cudaSuccess;
 }
 
+// 16-byte loads of the patterns and 4-byte loads of the mask: every item's row starts on such a boundary
+static bool fit_vec_ok(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix) {
+    return (npix & 3) == 0 && (m_stride & 3) == 0 && (((uintptr_t)d_I | (uintptr_t)d_M) & 15) == 0 && ((uintptr_t)d_mask & 3) == 0;
+}
+
 cudaError_t launch_fit_sums(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
-                            int batch, double *d_ws, cudaStream_t st) {
-    const int nchunk = fit_nchunk(npix);
+                            int batch, double *d_ws, cudaStream_t st, bool reduce = true) {
+    const int nchunk = fit_nchunk(npix, batch), chunk_px = fit_chunk(npix, batch);
     double *partial = d_ws, *sums = d_ws + (size_t)batch * nchunk * 5;
-    fit_sums_kernel<<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, partial);
-    fit_reduce_kernel<<<(batch * 5 + 127) / 128, 128, 0, st>>>(partial, nchunk, 5, batch, sums);
+    if (fit_vec_ok(d_I, d_M, m_stride, d_mask, npix))
+        fit_sums_kernel<true><<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, chunk_px, partial);
+    else
+        fit_sums_kernel<false><<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, chunk_px, partial);
+    if (reduce) fit_reduce_kernel<<<(batch * 5 + 127) / 128, 128, 0, st>>>(partial, nchunk, 5, batch, sums);
     return cudaGetLastError();
 }
 
+// With at most this many chunks per item the metric kernel's blocks add pass 1's partial sums themselves (2 x nchunk FP64
+// loads per block from L2) and the launch between the two passes goes.
+constexpr int kFitFoldChunks = 32;
+
+int fit_discrepancy_launches(int64_t npix, int batch) { return fit_nchunk(npix, batch) <= kFitFoldChunks ? 3 : 4; }
+
 cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
                                int batch, int metric, double *d_ws, double *d_out, cudaStream_t st) {
-    cudaError_t e = launch_fit_sums(d_I, d_M, m_stride, d_mask, npix, batch, d_ws, st);
+    const int nchunk = fit_nchunk(npix, batch), chunk_px = fit_chunk(npix, batch);
+    const bool fold = nchunk <= kFitFoldChunks;
+    cudaError_t e = launch_fit_sums(d_I, d_M, m_stride, d_mask, npix, batch, d_ws, st, !fold);
     if (e != cudaSuccess) return e;
-    const int nchunk = fit_nchunk(npix);
     double *sums = d_ws + (size_t)batch * nchunk * 5, *partial2 = sums + (size_t)batch * 5;
-    fit_metric_kernel<<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, metric, sums, partial2);
+    const double *partial1 = fold ? d_ws : nullptr;
+    if (fit_vec_ok(d_I, d_M, m_stride, d_mask, npix))
+        fit_metric_kernel<true><<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, chunk_px, metric, sums, partial1, partial2);
+    else
+        fit_metric_kernel<false><<<dim3(nchunk, batch), kFitThreads, 0, st>>>(d_I, d_M, m_stride, d_mask, npix, nchunk, chunk_px, metric, sums, partial1, partial2);
     fit_reduce_kernel<<<(batch + 127) / 128, 128, 0, st>>>(partial2, nchunk, 1, batch, d_out);
     return cudaGetLastError();
 }
@@ -261,7 +335,7 @@ cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, con
                                   float *d_counts, cudaStream_t st) {
     cudaError_t e = launch_fit_sums(d_I, nullptr, 0, nullptr, npix, batch, d_ws, st);
     if (e != cudaSuccess) return e;
-    const int nchunk = fit_nchunk(npix);
+    const int nchunk = fit_nchunk(npix, batch);
     double *sums = d_ws + (size_t)batch * nchunk * 5;
     double *photons = sums + (size_t)batch * 5 + (size_t)batch * nchunk;
     // the photon numbers travel as kernel arguments (read from h_photons before return whatever memory it is; capturable)

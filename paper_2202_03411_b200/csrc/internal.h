@@ -169,6 +169,7 @@ cudaError_t launch_nufft_interp(const Plan &p, const NufftPlan &n, int nb, int n
 
 // forward-fitting pieces (fit_kernels.cu)
 size_t fit_workspace_bytes(int64_t npix, int batch);
+int fit_discrepancy_launches(int64_t npix, int batch);   // 3 or 4: the sums of few chunks per item are added inside pass 2
 cudaError_t launch_discrepancy(const float *d_I, const float *d_M, int64_t m_stride, const unsigned char *d_mask, int64_t npix,
                                int batch, int metric, double *d_ws, double *d_out, cudaStream_t st);
 cudaError_t launch_ideal_detector(const float *d_I, int64_t npix, int batch, const double *h_photons, uint64_t seed, double *d_ws,

@@ -43,6 +43,35 @@ def test_discrepancy_matches_oracle_over_several_chunks_and_a_ragged_tail(sm, me
         assert np.allclose(got, ref, rtol=1e-11, atol=0), (metric, per_item, got, ref)
 
 
+@pytest.mark.parametrize("metric", [0, 1])
+def test_discrepancy_with_16_byte_loads_and_without(sm, metric):
+    """Pixel counts that are multiples of four take 16-byte loads of the patterns and 4-byte loads of the mask (a last chunk
+    that is not full, a count below one load per thread, mask bytes other than 1, NaN under the mask); the same data
+    through views that start one element later (no longer 16-byte aligned) takes the scalar kernels: both against the oracle."""
+    import torch
+    rng = np.random.default_rng(131 + metric)
+    fn = F.discrepancy_l2 if metric == 0 else F.discrepancy_poisson
+    # (pixels per block: 2048 or 8192 for the small problems, 32768 for the last one -- 1800 chunks; the first has more than 32
+    # chunks per item, so its sums go through the reduction launch, the others add them inside pass 2)
+    for B_, npix, per_item in ((4, 2 * 32768 + 4 * 333, True), (3, 32768, False), (2, 8, False), (3, 4 * 1024 + 4, True),
+                               (600, 3 * 32768 - 20, False)):
+        I = (rng.uniform(0.0, 1.0, (B_, npix)) ** 4 * 1e3 + 1e-3).astype(np.float32)
+        M = rng.poisson(3.0 * I if per_item else 3.0 * I[0]).astype(np.float32)
+        mask = ((rng.uniform(size=npix) < 0.8) * rng.integers(1, 256, npix)).astype(np.uint8)
+        Ibad = I.copy()
+        Ibad[:, mask == 0] = np.nan                                   # what the mask hides is never used
+        ref = fn(I, M, mask)
+        got = sm.discrepancy(dev(Ibad), dev(M), dev(mask), metric=metric).cpu().numpy()
+        assert np.allclose(got, ref, rtol=1e-11, atol=0), (npix, got, ref)
+        assert np.allclose(sm.discrepancy(dev(I), dev(M), metric=metric).cpu().numpy(), fn(I, M, None), rtol=1e-11, atol=0)
+        # one element off the 16-byte grid
+        pad = lambda a: torch.cat([torch.zeros(1, dtype=a.dtype, device="cuda"), a.reshape(-1)])[1:].reshape(a.shape)
+        Iu, Mu, mu = pad(dev(Ibad)), pad(dev(M)), pad(dev(mask))
+        assert Iu.data_ptr() % 16 == 4 and mu.data_ptr() % 4 == 1
+        got = sm.discrepancy(Iu, Mu, mu, metric=metric).cpu().numpy()
+        assert np.allclose(got, ref, rtol=1e-11, atol=0), (npix, got, ref)
+
+
 def test_discrepancy_degenerate_cases(sm):
     rng = np.random.default_rng(7)
     I = rng.uniform(0.5, 2.0, (2, 1000)).astype(np.float32)
