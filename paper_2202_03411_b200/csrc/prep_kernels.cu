@@ -499,15 +499,119 @@ __global__ void strength_kernel(const float2 *__restrict__ dn, int nx, int ny, i
     }
 }
 
+// The same for grids with so few columns that one thread per column leaves the GPU to a handful of warps, each walking its
+// serial chain (128^3: 128 blocks of 128 threads; 32^3: 32 of 64): the column is cut into segments of ZPT slices, one warp of
+// 32 columns per segment.  A thread holds its segment's voxels in registers, forms the product of their factors, the block
+// exchanges the segment products through shared memory, every thread multiplies those of the segments below it (in order,
+// <= 15 products) into its starting T and then writes its slices as strength_kernel does.  The running product is
+// associated differently from the one-thread walk: ~nz 2^-53 relative either way.
+constexpr int kSplitCols = 32;
+constexpr int kSplitMaxSeg = 16;
+
+template <int ZPT>
+__global__ void __launch_bounds__(kSplitCols *kSplitMaxSeg)
+strength_split_kernel(const float2 *__restrict__ dn, int nx, int ny, int nz, double kdz, int rho_mode, float2 *__restrict__ rho,
+                      unsigned *__restrict__ maxbits) {
+    __shared__ double2 segP[kSplitMaxSeg][kSplitCols];
+    __shared__ float wmax[kSplitMaxSeg];
+    const int cx = threadIdx.x & (kSplitCols - 1), seg = threadIdx.x / kSplitCols;
+    const int ix = blockIdx.x * kSplitCols + cx, iy = blockIdx.y, b = blockIdx.z;
+    const int z0 = seg * ZPT;
+    const size_t plane = (size_t)nx * ny;
+    const size_t base = (size_t)b * plane * nz + (size_t)iy * nx + ix;
+    const bool col = ix < nx;
+    float2 cin[ZPT];
+#pragma unroll
+    for (int i = 0; i < ZPT; ++i)
+        cin[i] = col && z0 + i < nz ? __ldg(dn + base + (size_t)(z0 + i) * plane) : make_float2(0.f, 0.f);
+    // the factor of the last (delta, beta) seen is kept across both walks: a homogeneous segment costs one sincos / exp
+    double gre = 1.0, gim = 0.0;
+    float ld = 0.f, lb = 0.f;
+    auto factor = [&](const float2 c) {
+        if (c.x != ld || c.y != lb) {
+            double sn, co;
+            sincos(kdz * (double)c.x, &sn, &co);
+            const double mag = exp(-kdz * (double)c.y);
+            gre = mag * co;
+            gim = mag * sn;
+            ld = c.x;
+            lb = c.y;
+        }
+    };
+    double Pre = 1.0, Pim = 0.0;
+#pragma unroll
+    for (int i = 0; i < ZPT; ++i) {
+        const float2 c = cin[i];
+        if (c.x != 0.f || c.y != 0.f) {
+            factor(c);
+            const double t = Pre * gre - Pim * gim;
+            Pim = Pre * gim + Pim * gre;
+            Pre = t;
+        }
+    }
+    segP[seg][cx] = make_double2(Pre, Pim);
+    __syncthreads();
+    double Tre = 1.0, Tim = 0.0;
+    for (int q = 0; q < seg; ++q) {
+        const double2 pq = segP[q][cx];
+        const double t = Tre * pq.x - Tim * pq.y;
+        Tim = Tre * pq.y + Tim * pq.x;
+        Tre = t;
+    }
+    float vmax = 0.f;
+#pragma unroll
+    for (int i = 0; i < ZPT; ++i) {
+        if (!col || z0 + i >= nz) break;
+        const float2 c = cin[i];
+        float2 o = make_float2(0.f, 0.f);
+        if (c.x != 0.f || c.y != 0.f) {
+            const double d = (double)c.x, be = (double)c.y;
+            double fre = d, fim = be;
+            if (rho_mode == SCATMAN_RHO_N2M1) {  // c (2 - c)
+                fre = d * (2.0 - d) + be * be;
+                fim = 2.0 * be * (1.0 - d);
+            }
+            o.x = (float)(fre * Tre - fim * Tim);
+            o.y = (float)(fre * Tim + fim * Tre);
+            vmax = fmaxf(vmax, fmaxf(fabsf(o.x), fabsf(o.y)));
+            factor(c);
+            const double t = Tre * gre - Tim * gim;
+            Tim = Tre * gim + Tim * gre;
+            Tre = t;
+        }
+        rho[base + (size_t)(z0 + i) * plane] = o;
+    }
+    for (int off = 16; off > 0; off >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, off));
+    if (cx == 0) wmax[seg] = vmax;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float m = 0.f;
+        for (int w = 0; w < (int)(blockDim.x / kSplitCols); ++w) m = fmaxf(m, wmax[w]);
+        if (m > 0.f && maxbits) atomicMax(maxbits + b, __float_as_uint(m));
+    }
+}
+
 cudaError_t launch_strength(const float *d_dn, const Plan &p, int batch, float *d_rho, unsigned *d_maxbits,
                             cudaStream_t st) {
     if (d_maxbits) {   // nullptr: the caller does not want the per-item maximum (scatman_effective_strength)
         cudaError_t e = cudaMemsetAsync(d_maxbits, 0, sizeof(unsigned) * batch, st);
         if (e != cudaSuccess) return e;
     }
+    const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
+    // few columns (below half a thread per lane slot of the GPU): cut the columns along z as well
+    if ((size_t)p.nx * p.ny * batch <= 32768 && p.nz > 8 && p.nz <= 16 * kSplitMaxSeg) {
+        const int zpt = p.nz <= 8 * kSplitMaxSeg ? 8 : 16, nseg = (p.nz + zpt - 1) / zpt;
+        dim3 grid((p.nx + kSplitCols - 1) / kSplitCols, p.ny, batch);
+        if (zpt == 8)
+            strength_split_kernel<8><<<grid, kSplitCols * nseg, 0, st>>>((const float2 *)d_dn, p.nx, p.ny, p.nz, kdz, p.rho_mode,
+                                                                         (float2 *)d_rho, d_maxbits);
+        else
+            strength_split_kernel<16><<<grid, kSplitCols * nseg, 0, st>>>((const float2 *)d_dn, p.nx, p.ny, p.nz, kdz, p.rho_mode,
+                                                                          (float2 *)d_rho, d_maxbits);
+        return cudaGetLastError();
+    }
     const int threads = p.nx >= 128 ? 128 : 64;
     dim3 grid((p.nx + threads - 1) / threads, p.ny, batch);
-    const double kdz = 2.0 * 3.14159265358979323846 / p.lambda * p.dz;
     strength_kernel<<<grid, threads, 0, st>>>((const float2 *)d_dn, p.nx, p.ny, p.nz, kdz, p.rho_mode,
                                               (float2 *)d_rho, d_maxbits);
     return cudaGetLastError();

@@ -59,6 +59,29 @@ def test_effective_strength_matches_oracle(sm):
         assert np.all(got[ref == 0] == 0)
 
 
+@pytest.mark.parametrize("dims", [(40, 5, 130), (33, 3, 256), (33, 3, 257), (21, 4, 8), (64, 2, 9), (200, 170, 12)])
+def test_effective_strength_on_both_column_walks(sm, dims):
+    """Grids with few columns cut every column into segments of 8 or 16 slices (one warp of 32 columns per segment, up to 16
+    segments, the segment products exchanged through shared memory); more than 32768 columns, nz <= 8 or nz > 256 take one
+    thread per column.  Ragged in x, in the last segment and in the segment count; one grid is random (every voxel its own
+    factor), one is two homogeneous bodies with vacuum between and inside them (the cached factor carried across the two
+    walks of a segment, segments that are all vacuum)."""
+    nx, ny, nz = dims
+    voxel, lam = (2.0, 2.0, 3.0), 9.0
+    g1 = W.random_grid(43 + nz, nx, ny, nz, delta=(-0.02, 0.08), beta=(0.0, 0.05))
+    g2 = np.zeros((nz, ny, nx, 2), dtype=np.float32)
+    g2[nz // 7: nz // 2, :, 1: nx - 2] = (0.013, 0.004)
+    g2[nz // 2 + 1: nz - 1, ny // 2:, nx // 3:] = (-0.007, 0.011)
+    g2[nz // 3, :, nx // 2] = 0.0                                     # a hole inside the first body
+    for g in (g1, g2):
+        for mode in (0, 1):
+            rho = sm.effective_strength(dev(g), voxel, lam, rho_mode=mode).cpu().numpy()
+            ref = O.effective_strength(g, voxel, lam, mode) / np.prod(voxel)
+            got = rho[..., 0] + 1j * rho[..., 1]
+            assert np.max(np.abs(got - ref)) <= 2e-7 * np.max(np.abs(ref)), (dims, mode)
+            assert np.all(got[ref == 0] == 0)
+
+
 # ------------------------------------------------------------------------------------------ whole path
 @pytest.mark.parametrize("method", list(METHODS))
 def test_cfg1_sphere_full_pattern(sm, method):
