@@ -93,8 +93,9 @@ bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restri
     };
     if ((n & 1) == 0) {
         const float4 *src4 = (const float4 *)src;
-        const int n2 = n >> 1;
-        for (int e0 = threadIdx.x; e0 < n2; e0 += 4 * 256) {
+        // gridDim.y blocks share a slice (single grids: nz blocks alone would leave SMs idle; never with the occupancy map)
+        const int n2 = (int)((long long)(n >> 1) * (blockIdx.y + 1) / gridDim.y);
+        for (int e0 = (int)((long long)(n >> 1) * blockIdx.y / gridDim.y) + threadIdx.x; e0 < n2; e0 += 4 * 256) {
             float4 v[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) v[u] = e0 + u * 256 < n2 ? __ldg(src4 + e0 + u * 256) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -107,7 +108,8 @@ bbox_kernel(const float2 *__restrict__ in, int nx, int ny, int nz, int *__restri
             }
         }
     } else {
-        for (int e = threadIdx.x; e < n; e += 256) {
+        const int n1 = (int)((long long)n * (blockIdx.y + 1) / gridDim.y);
+        for (int e = (int)((long long)n * blockIdx.y / gridDim.y) + threadIdx.x; e < n1; e += 256) {
             const float2 v = __ldg(src + e);
             if (v.x != 0.f || v.y != 0.f) seen(e);
             ex.see(v.x, v.y);
@@ -421,7 +423,15 @@ cudaError_t launch_orient(const float *d_in, const Plan &p, const double *d_rotm
         cudaError_t e = cudaMemsetAsync(d_occ, 0, orient_occ_bytes(p, batch), st);
         if (e != cudaSuccess) return e;
     }
-    bbox_kernel<<<(unsigned)(p.nz * batch), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats, d_occ);
+    // slices shared by several blocks while there are fewer than two blocks per SM, each part at least 4096 voxels
+    int parts = 1;
+    if (!d_occ) {
+        parts = (int)((2 * 148 + (size_t)p.nz * batch - 1) / ((size_t)p.nz * batch));
+        const int most = (int)(((size_t)p.nx * p.ny) / 4096);
+        if (parts > most) parts = most;
+        if (parts < 1) parts = 1;
+    }
+    bbox_kernel<<<dim3((unsigned)(p.nz * batch), (unsigned)parts), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, d_bbox, d_stats, d_occ);
     orient_kernel<<<dim3((unsigned)blocks, (unsigned)nsplit), 256, 0, st>>>((const float2 *)d_in, p.nx, p.ny, p.nz, p.dx, p.dy, p.dz,
                                                    make_double3(1.0 / p.dx, 1.0 / p.dy, 1.0 / p.dz), d_rotmat, d_bbox,
                                                    (float2 *)d_out, d_tilemap, d_occ);

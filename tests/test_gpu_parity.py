@@ -48,6 +48,27 @@ def test_orient_matches_oracle(sm):
         assert np.allclose(out[b], ref, rtol=2e-7, atol=1e-12)
 
 
+@pytest.mark.parametrize("dims", [(91, 93, 5), (92, 90, 6)])
+def test_orient_single_grid_whose_slices_are_shared_by_several_blocks(sm, dims):
+    """A single grid with few slices of more than 8192 voxels: the bounding-box pass gives every slice to two blocks (odd voxel
+    count: scalar loads; even: 16-byte loads).  Material only near two opposite corners of the slice and at the seam between the
+    parts, so a part that went unseen would shrink the box and the resampling would drop it."""
+    nx, ny, nz = dims
+    g = np.zeros((nz, ny, nx, 2), dtype=np.float32)
+    rng = np.random.default_rng(17)
+    for (ys, xs) in ((slice(10, 13), slice(10, 14)), (slice(ny - 13, ny - 10), slice(nx - 14, nx - 10)), (slice(ny // 2, ny // 2 + 2), slice(10, 12))):
+        blk = g[:, ys, xs]
+        blk[..., 0] = rng.uniform(0.01, 0.05, blk.shape[:-1])
+        blk[..., 1] = rng.uniform(0.001, 0.02, blk.shape[:-1])
+    voxel = (1.0, 1.0, 1.0)
+    quat = W.random_quaternions(rng, 1)
+    quat[0] = (np.cos(0.05), 0.0, 0.0, np.sin(0.05))        # a small turn about z: the material stays inside the grid
+    out = sm.orient(dev(g[None]), voxel, quat).cpu().numpy()
+    ref = O.orient(g, voxel, quat[0])
+    assert np.count_nonzero(ref) > 100
+    assert np.allclose(out[0], ref, rtol=2e-7, atol=1e-12)
+
+
 def test_effective_strength_matches_oracle(sm):
     g = W.random_grid(41, 19, 7, 23, delta=(-0.02, 0.08), beta=(0.0, 0.05))
     voxel, lam = (2.0, 2.0, 3.0), 9.0
